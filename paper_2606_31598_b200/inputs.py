@@ -1,0 +1,54 @@
+"""Seeded synthetic inputs shared by the tests, the oracle legs and bench.py.
+
+This module holds NONE of the method's arithmetic (no Philox4x32, no Box-Muller, no entry rule,
+no matvec): it only draws the *inputs* of phi = H psi with numpy's own generator and lists the
+five BASELINE.json workloads.  Both the CUDA path and the CPU oracle receive the same arrays.
+
+Recipe: psi has i.i.d. complex standard-normal entries from
+``numpy.random.default_rng(seed)``, normalised to unit 2-norm in float64; for complex64 the
+normalised vector is rounded to float32 and BOTH sides use the rounded values.  For k vectors
+column v is drawn from ``default_rng([seed, v])`` and normalised separately; the layout is
+row-major [D][k] (a row of k complex numbers is contiguous).
+"""
+from __future__ import annotations
+
+import numpy as np
+
+# BASELINE.json configs[0..4] (C1..C5).  "matrix_seed" of C4 and "psi_seed" of C2/C5 are not
+# given there; readings R9/R10 fix them to 1234 / 99.
+CONFIGS = {
+    "C1": dict(D=4096, dtype="c128", B=512, mode="procedural", seed=1234, psi_seed=99, k=1),
+    "C2": dict(D=65536, dtype="c128", B=2048, mode="full", seed=1234, psi_seed=99, k=1),
+    "C3": dict(D=32768, dtype="c64", B=1024, mode="procedural", seed=8, seed_h0=7, psi_seed=9, k=16),
+    "C4": dict(D=262144, dtype="c128", B=4096, mode="procedural", seed=1234, psi_seed=11, k=1),
+    "C5": dict(D=131072, dtype="c128", B=4096, mode="partial", seed=21, psi_seed=99, k=1,
+               t=50.0, tol=1e-14, e_min=-2.1, e_max=2.1, hbm_budget=150e9),
+}
+
+
+def make_psi(D: int, seed: int, k: int = 1, dtype: str = "c128") -> np.ndarray:
+    """Normalised random complex vector(s): shape [D] for k == 1, else [D, k] row-major."""
+    cols = []
+    for v in range(k):
+        rng = np.random.default_rng(seed if k == 1 else [seed, v])
+        x = rng.standard_normal(D) + 1j * rng.standard_normal(D)
+        cols.append(x / np.linalg.norm(x))
+    psi = cols[0] if k == 1 else np.ascontiguousarray(np.stack(cols, axis=1))
+    if dtype == "c64":
+        psi = psi.astype(np.complex64)
+    return psi
+
+
+def lambda_grid(k: int, lo: float = 0.0, hi: float = 2.0) -> np.ndarray:
+    """k coupling strengths evenly spaced in [lo, hi], both endpoints included (configs[2])."""
+    if k == 1:
+        return np.array([hi], dtype=np.float64)
+    return lo + (hi - lo) * np.arange(k, dtype=np.float64) / (k - 1)
+
+
+def sample_rows(D: int, n: int, seed: int = 0) -> np.ndarray:
+    """Row sample for full-size parity: both ends, block edges and n random rows, sorted."""
+    rng = np.random.default_rng([D, seed])
+    fixed = np.array([0, 1, D // 2 - 1, D // 2, D - 2, D - 1], dtype=np.int64)
+    rand = rng.integers(0, D, size=n, dtype=np.int64)
+    return np.unique(np.concatenate([fixed, rand]))
