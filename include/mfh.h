@@ -1,0 +1,146 @@
+/*
+ * mfh.h -- C ABI of the B200-native block-procedural matrix-free Hamiltonian-vector product.
+ *
+ * phi = H psi for a dense D x D Hermitian H that is never materialised: for every block pair
+ * (n,m) the block H^[n,m] is generated on the fly from a counter-based seed or streamed from an
+ * HBM-resident cache, applied to psi^[m] and accumulated into phi^[n].
+ *   PAPER.md = /root/reference/PAPER.md (arxiv/paper_2606_31598), cited "P:<line>".
+ *   Block product                     P:107-116 Eq. 4-5;  P:143-147 Eq. 7
+ *   apply_H_block(n,m,psi^[m])        P:135-141 Eq. 6
+ *   Sources: seeded / fused action    P:153-157 Eq. 8;  P:171-175 Eq. 11
+ *   Modes: full / partial cache       P:177-183;  P:431-446 Eq. 27
+ *   Multi-vector Y = A X (R vectors)  P:212-230 Eq. 12-13
+ *   Planner (analytic, measured)      P:258-296 Eq. 14-20;  P:298-360 Eq. 21-23
+ *   Chebyshev propagator              P:705-721 Eq. 41-44
+ * The entry rule, Philox4x32-10 + Box-Muller, the workloads and the tolerances come from
+ * /root/repo/BASELINE.json; readings of silent points are listed in DESIGN.md.
+ *
+ * Conventions
+ *   - Plain C, no torch types.  "dev" pointers are CUDA device pointers on the current device,
+ *     "host" pointers are ordinary host memory.  `stream` is a cudaStream_t passed as void*
+ *     (NULL = the legacy default stream).
+ *   - Complex numbers are interleaved (re, im); MFH_C128 = 2 x double, MFH_C64 = 2 x float.
+ *   - One vector: length D.  k vectors: row-major [D][k] (the k values of a row are contiguous).
+ *   - All vectors are caller-owned and 16-byte aligned; phi must not alias psi.  The cache,
+ *     partial-sum workspace and Chebyshev scratch are library-owned (allocated in mfh_plan /
+ *     on first mfh_chebyshev call, freed in mfh_destroy).
+ *   - Every function returns an int status (MFH_OK = 0); mfh_last_error() gives the message.
+ *   - There is no CPU fallback: every compute entry point needs a CUDA device and fails with
+ *     MFH_ERR_CUDA otherwise.
+ */
+#ifndef MFH_H
+#define MFH_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define MFH_API __attribute__((visibility("default")))
+#else
+#define MFH_API
+#endif
+
+typedef struct mfh_handle_s* mfh_handle; /* opaque; library-owned until mfh_destroy */
+
+enum { MFH_OK = 0, MFH_ERR_INVALID_ARG = 1, MFH_ERR_BAD_STATE = 2, MFH_ERR_OUT_OF_MEMORY = 3,
+       MFH_ERR_CUDA = 4, MFH_ERR_NOT_CONVERGED = 5, MFH_ERR_UNSUPPORTED = 6 };
+enum { MFH_C128 = 0, MFH_C64 = 1 };
+enum { MFH_SRC_GUE = 0,           /* H = lambda * V(seed)                          configs 1,2,4,5 */
+       MFH_SRC_DIAG_PLUS_GUE = 1  /* H_v = diag(h0(seed_h0)) + lambda_v * V(seed)  config 3        */ };
+enum { MFH_MODE_AUTO = 0, MFH_MODE_PROCEDURAL = 1, MFH_MODE_PARTIAL = 2, MFH_MODE_FULL = 3 };
+
+#define MFH_MAX_K 16       /* largest number of simultaneous vectors */
+#define MFH_MIN_B 32       /* block size must be a multiple of this and divide D */
+#define MFH_MAX_B 4096     /* largest block size (shared-memory column accumulators) */
+
+/* Create a Hamiltonian description (host only; no device work, no allocation on the device).
+ *   D        Hilbert-space dimension, 32 <= D <= 2^31, multiple of 32.
+ *   B        block size b; multiple of 32 dividing D, <= MFH_MAX_B; 0 = planner picks.
+ *   seed     64-bit seed of the GUE matrix V: entry (i,j), i<j, is (g1 + i g2)/sqrt(2D) with
+ *            g1,g2 Box-Muller normals from Philox4x32-10(key=seed, ctr=(min(i,j),max(i,j),0,0));
+ *            i>j is the conjugate; i==j is g1/sqrt(D), real (BASELINE.json configs[0]).
+ *   lambda   coupling used when mfh_apply gets lambdas_host == NULL (1.0 for a plain GUE).
+ *   seed_h0  seed of the diagonal H0 (uniform in (-1,1)); ignored for MFH_SRC_GUE.
+ * Errors: MFH_ERR_INVALID_ARG for any violated constraint or unknown enum. */
+MFH_API int mfh_create(mfh_handle* out, int64_t D, int32_t B, uint64_t seed, int32_t source_kind,
+                       double lambda, int32_t dtype, uint64_t seed_h0);
+
+/* Analytic planner only (Algorithm 1; adaptive block size P:409-429; cache budget
+ * Eq. 27).  Pure host arithmetic: needs no GPU, touches no handle.  Enumerates
+ * mode x B candidates, rejects those with M_tot > alpha * hbm_free_bytes (Eq. 18, alpha = 0.9)
+ * and ranks the rest by modelled seconds per job.  Writes a JSON record (chosen plan +
+ * all candidates) to json_out (NUL-terminated, truncated to json_cap).
+ *   mode  MFH_MODE_AUTO or a forced mode;  B  0 = enumerate, else forced.
+ * Errors: MFH_ERR_INVALID_ARG; MFH_ERR_OUT_OF_MEMORY when no candidate fits. */
+MFH_API int mfh_plan_analytic(int64_t D, int32_t dtype, int32_t k, int32_t mode, int32_t B,
+                              int64_t n_applies_hint, int64_t hbm_free_bytes, char* json_out,
+                              size_t json_cap);
+
+/* Plan and commit: choose mode and B (analytic; measure != 0 additionally times the best
+ * candidates on the device, Algorithm 2, R_warm = 1, R_bench = 3, K_bench <= 8), allocate the
+ * cache and the workspace and fill the cache with the generator (one-time cost).
+ *   k                 number of simultaneous vectors later passed to mfh_apply (1..MFH_MAX_K).
+ *   n_applies_hint    expected number of applies R_H (amortises the cache fill); <= 0 means 1.
+ *   hbm_budget_bytes  memory the plan may use; 0 = alpha * currently free device memory.
+ *   json_out          optional (may be NULL) plan record, as for mfh_plan_analytic.
+ * Synchronises `stream` before returning.  May be called again to re-plan.
+ * Errors: INVALID_ARG, OUT_OF_MEMORY (nothing fits / allocation failed), CUDA. */
+MFH_API int mfh_plan(mfh_handle h, int32_t mode, int32_t k, int64_t n_applies_hint,
+                     int64_t hbm_budget_bytes, int32_t measure, void* stream, char* json_out,
+                     size_t json_cap);
+
+/* phi = H psi for k vectors (Eq. 7; Eq. 12 for k > 1), asynchronous on `stream`, no host
+ * synchronisation, no allocation.  k must equal the k given to mfh_plan.
+ *   psi_dev, phi_dev  device, [D][k] complex of the handle's dtype.
+ *   lambdas_host      k doubles (host) or NULL = the handle's lambda for every vector.
+ *   Result: phi[:,v] = h0 (.) psi[:,v] (only MFH_SRC_DIAG_PLUS_GUE) + lambda_v * V psi[:,v].
+ * Errors: BAD_STATE before mfh_plan; INVALID_ARG (NULL pointers, k mismatch); CUDA. */
+MFH_API int mfh_apply(mfh_handle h, const void* psi_dev, void* phi_dev, int32_t k,
+                      const double* lambdas_host, void* stream);
+
+/* Same as mfh_apply but with HOST buffers: copies psi to the device, applies, copies phi back and
+ * synchronises `stream` (the end-to-end call bench.py times).  Host buffers should be pinned. */
+MFH_API int mfh_apply_host(mfh_handle h, const void* psi_host, void* phi_host, int32_t k,
+                           const double* lambdas_host, void* stream);
+
+/* out = exp(-i H t) psi by the Chebyshev expansion (Eq. 41-44), one vector (the handle must be
+ * planned with k = 1; H uses the handle's lambda).  c = (e_max+e_min)/2, R = (e_max-e_min)/2,
+ * a = R t; terms l = 0..K-1 with K = 1 + max{l : |J_l(a)| >= tol}; K-1 calls of the apply path.
+ * Asynchronous on `stream` after the host-side Bessel table; *n_terms_out = K (may be NULL).
+ * [e_min, e_max] must enclose the spectrum (for the GUE of this library: about +-2*lambda).
+ * Errors: INVALID_ARG (e_max <= e_min, non-finite t, tol <= 0, k != 1); BAD_STATE; CUDA. */
+MFH_API int mfh_chebyshev(mfh_handle h, const void* psi_dev, void* out_dev, double t, double e_min,
+                          double e_max, double tol, int32_t* n_terms_out, void* stream);
+
+/* Free the handle and everything it owns.  NULL is accepted. */
+MFH_API int mfh_destroy(mfh_handle h);
+
+/* Thread-local message of the last failing call ("" if none). */
+MFH_API const char* mfh_last_error(void);
+
+/* JSON description of the committed plan (mode, B, cached blocks, bytes, launches per apply). */
+MFH_API int mfh_get_plan(mfh_handle h, char* json_out, size_t json_cap);
+
+/* ---- test-only exports --------------------------------------------------------------------- */
+
+/* Raw Philox4x32-10 words for n index pairs: key = seed, ctr = (min(i,j), max(i,j), stream_id, 0).
+ * i_dev, j_dev: n uint32 (device); words_dev: 4n uint32 (device). */
+MFH_API int mfh_debug_philox(uint64_t seed, uint32_t stream_id, const uint32_t* i_dev,
+                             const uint32_t* j_dev, int64_t n, uint32_t* words_dev, void* stream);
+
+/* Dense block H^[n,m] of V (lambda and H0 not applied) written row-major B x B complex of the
+ * handle's dtype to block_dev -- the same generator the fused kernel and the cache fill use.
+ * Needs B fixed (mfh_create with B != 0, or after mfh_plan). */
+MFH_API int mfh_materialize_block(mfh_handle h, int32_t n, int32_t m, void* block_dev, void* stream);
+
+/* The H0 diagonal (D reals of the handle's real type) written to h0_dev. */
+MFH_API int mfh_debug_h0(mfh_handle h, void* h0_dev, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MFH_H */

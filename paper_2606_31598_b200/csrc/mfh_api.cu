@@ -1,0 +1,401 @@
+// mfh_api.cu -- the C ABI of include/mfh.h: argument checking, plan commit, apply dispatch,
+// the Chebyshev driver and the test exports.  Every step of the path runs in the kernels of
+// mfh_proc.cu / mfh_cached.cu / mfh_vec.cu; this file only marshals.
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstring>
+#include "mfh_internal.cuh"
+#include "mfh_plan.h"
+
+namespace mfh {
+
+static thread_local char g_err[1024] = "";
+
+void set_error(const char* fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+}
+
+size_t complex_bytes(int dtype) { return dtype == MFH_C128 ? 16 : 8; }
+
+static void copy_json(const std::string& s, char* out, size_t cap)
+{
+    if (!out || cap == 0) return;
+    const size_t n = std::min(s.size(), cap - 1);
+    memcpy(out, s.data(), n);
+    out[n] = 0;
+}
+
+static bool valid_B(int64_t D, int32_t B)
+{
+    return B >= MFH_MIN_B && B <= MFH_MAX_B && B % MFH_MIN_B == 0 && D % B == 0;
+}
+
+static int free_plan_resources(mfh_handle h)
+{
+    void** ptrs[] = {&h->d_cache, &h->d_work, &h->d_h0, (void**)&h->d_cache_slot, (void**)&h->d_items,
+                     (void**)&h->d_slot_valid, (void**)&h->d_counter, &h->d_cheb, &h->d_io};
+    for (void** p : ptrs) {
+        if (*p) cudaFree(*p);
+        *p = nullptr;
+    }
+    h->planned = false;
+    return MFH_OK;
+}
+
+// Allocate and upload everything plan `p` needs, then fill the cache.
+static int commit_plan(mfh_handle h, const Plan& p, cudaStream_t st)
+{
+    free_plan_resources(h);
+    h->plan = p;
+    const Plan& q = h->plan;
+    const size_t cb = complex_bytes(h->dtype);
+    cudaError_t e;
+    if (q.cache_bytes) {
+        e = cudaMalloc(&h->d_cache, q.cache_bytes);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            set_error("cache allocation of %zu bytes failed: %s", q.cache_bytes, cudaGetErrorString(e));
+            free_plan_resources(h);
+            return MFH_ERR_OUT_OF_MEMORY;
+        }
+    }
+    e = cudaMalloc(&h->d_work, q.work_bytes);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        set_error("workspace allocation of %zu bytes failed: %s", q.work_bytes, cudaGetErrorString(e));
+        free_plan_resources(h);
+        return MFH_ERR_OUT_OF_MEMORY;
+    }
+    MFH_CUDA_CHECK(cudaMalloc(&h->d_cache_slot, q.cache_slot.size() * sizeof(int32_t)));
+    MFH_CUDA_CHECK(cudaMemcpyAsync(h->d_cache_slot, q.cache_slot.data(), q.cache_slot.size() * sizeof(int32_t),
+                                   cudaMemcpyHostToDevice, st));
+    if (!q.items.empty()) {
+        MFH_CUDA_CHECK(cudaMalloc(&h->d_items, q.items.size() * sizeof(ProcItem)));
+        MFH_CUDA_CHECK(cudaMemcpyAsync(h->d_items, q.items.data(), q.items.size() * sizeof(ProcItem),
+                                       cudaMemcpyHostToDevice, st));
+    }
+    MFH_CUDA_CHECK(cudaMalloc(&h->d_slot_valid, q.slot_valid.size()));
+    MFH_CUDA_CHECK(cudaMemcpyAsync(h->d_slot_valid, q.slot_valid.data(), q.slot_valid.size(),
+                                   cudaMemcpyHostToDevice, st));
+    MFH_CUDA_CHECK(cudaMalloc(&h->d_counter, sizeof(int32_t)));
+    MFH_CUDA_CHECK(cudaMalloc(&h->d_io, (size_t)2 * h->D * q.k * cb));
+    if (h->kind == MFH_SRC_DIAG_PLUS_GUE) {
+        MFH_CUDA_CHECK(cudaMalloc(&h->d_h0, (size_t)h->D * (h->dtype == MFH_C128 ? 8 : 4)));
+        int rc = launch_h0(h, h->d_h0, st);
+        if (rc) return rc;
+    }
+    int rc = launch_fill_cache(h, st);
+    if (rc) return rc;
+    MFH_CUDA_CHECK(cudaStreamSynchronize(st));
+    h->planned = true;
+    return MFH_OK;
+}
+
+static int apply_impl(mfh_handle h, const void* psi, void* phi, const double* lambdas, cudaStream_t st)
+{
+    const Plan& p = h->plan;
+    int rc;
+    if ((rc = launch_cached(h, psi, st))) return rc;
+    if (p.k == 1) {
+        if ((rc = launch_proc_single(h, psi, st))) return rc;
+    } else if (p.slot_multi >= 0) {
+        if ((rc = launch_proc_multi(h, psi, st))) return rc;
+    }
+    return launch_reduce(h, psi, phi, lambdas, st);
+}
+
+// Algorithm 2: time R_bench applies of a committed plan after R_warm warm-ups.
+static int time_plan(mfh_handle h, cudaStream_t st, double& seconds)
+{
+    const int R_warm = 1, R_bench = 3;
+    const size_t bytes = (size_t)h->D * h->plan.k * complex_bytes(h->dtype);
+    char* psi = (char*)h->d_io;
+    char* phi = psi + bytes;
+    MFH_CUDA_CHECK(cudaMemsetAsync(psi, 0, bytes, st));   // timing does not depend on the values
+    cudaEvent_t a, b;
+    MFH_CUDA_CHECK(cudaEventCreate(&a));
+    MFH_CUDA_CHECK(cudaEventCreate(&b));
+    int rc = MFH_OK;
+    for (int r = 0; r < R_warm && !rc; ++r) rc = apply_impl(h, psi, phi, nullptr, st);
+    cudaStreamSynchronize(st);
+    cudaEventRecord(a, st);
+    for (int r = 0; r < R_bench && !rc; ++r) rc = apply_impl(h, psi, phi, nullptr, st);
+    cudaEventRecord(b, st);
+    cudaError_t e = cudaStreamSynchronize(st);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, a, b);
+    cudaEventDestroy(a);
+    cudaEventDestroy(b);
+    if (rc) return rc;
+    MFH_CUDA_CHECK(e);
+    seconds = (double)ms * 1e-3 / R_bench;   // Eq. 21
+    return MFH_OK;
+}
+
+}  // namespace mfh
+
+using namespace mfh;
+
+extern "C" {
+
+MFH_API const char* mfh_last_error(void) { return g_err; }
+
+MFH_API int mfh_create(mfh_handle* out, int64_t D, int32_t B, uint64_t seed, int32_t source_kind,
+                       double lambda, int32_t dtype, uint64_t seed_h0)
+{
+    if (!out) { set_error("mfh_create: out is NULL"); return MFH_ERR_INVALID_ARG; }
+    *out = nullptr;
+    if (D < 32 || D > (int64_t)1 << 31 || D % 32 != 0) {
+        set_error("mfh_create: D=%lld must be a multiple of 32 in [32, 2^31]", (long long)D);
+        return MFH_ERR_INVALID_ARG;
+    }
+    if (B != 0 && !valid_B(D, B)) {
+        set_error("mfh_create: B=%d must be a multiple of %d, <= %d, dividing D=%lld", B, MFH_MIN_B,
+                  MFH_MAX_B, (long long)D);
+        return MFH_ERR_INVALID_ARG;
+    }
+    if (source_kind != MFH_SRC_GUE && source_kind != MFH_SRC_DIAG_PLUS_GUE) {
+        set_error("mfh_create: unknown source kind %d", source_kind);
+        return MFH_ERR_INVALID_ARG;
+    }
+    if (dtype != MFH_C128 && dtype != MFH_C64) {
+        set_error("mfh_create: unknown dtype %d", dtype);
+        return MFH_ERR_INVALID_ARG;
+    }
+    if (!std::isfinite(lambda)) { set_error("mfh_create: lambda is not finite"); return MFH_ERR_INVALID_ARG; }
+    mfh_handle h = new mfh_handle_s();
+    h->D = D;
+    h->B_req = B;
+    h->seed = seed;
+    h->seed_h0 = seed_h0;
+    h->kind = source_kind;
+    h->dtype = dtype;
+    h->lambda = lambda;
+    *out = h;
+    return MFH_OK;
+}
+
+MFH_API int mfh_destroy(mfh_handle h)
+{
+    if (!h) return MFH_OK;
+    free_plan_resources(h);
+    delete h;
+    return MFH_OK;
+}
+
+MFH_API int mfh_plan_analytic(int64_t D, int32_t dtype, int32_t k, int32_t mode, int32_t B,
+                              int64_t n_applies_hint, int64_t hbm_free_bytes, char* json_out,
+                              size_t json_cap)
+{
+    if (D < 32 || D % 32 != 0 || (dtype != MFH_C128 && dtype != MFH_C64) || k < 1 || k > MFH_MAX_K ||
+        mode < MFH_MODE_AUTO || mode > MFH_MODE_FULL || (B != 0 && !valid_B(D, B)) || hbm_free_bytes <= 0) {
+        set_error("mfh_plan_analytic: invalid argument");
+        return MFH_ERR_INVALID_ARG;
+    }
+    std::vector<Candidate> cands;
+    const double budget = planner_alpha() * (double)hbm_free_bytes;   // Eq. 18
+    const int rc = enumerate_candidates(D, dtype, k, mode, B, n_applies_hint, budget, 148, cands);
+    copy_json(plan_json(D, dtype, k, n_applies_hint, budget, 0, cands), json_out, json_cap);
+    if (rc) set_error("mfh_plan_analytic: no candidate fits in %.0f bytes", budget);
+    return rc;
+}
+
+MFH_API int mfh_plan(mfh_handle h, int32_t mode, int32_t k, int64_t n_applies_hint,
+                     int64_t hbm_budget_bytes, int32_t measure, void* stream, char* json_out,
+                     size_t json_cap)
+{
+    if (!h) { set_error("mfh_plan: NULL handle"); return MFH_ERR_INVALID_ARG; }
+    if (k < 1 || k > MFH_MAX_K || mode < MFH_MODE_AUTO || mode > MFH_MODE_FULL || hbm_budget_bytes < 0) {
+        set_error("mfh_plan: invalid argument (k=%d, mode=%d)", k, mode);
+        return MFH_ERR_INVALID_ARG;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0;
+    MFH_CUDA_CHECK(cudaGetDevice(&dev));
+    MFH_CUDA_CHECK(cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev));
+    free_plan_resources(h);   // a re-plan may reuse the memory of the previous plan
+    size_t free_b = 0, total_b = 0;
+    MFH_CUDA_CHECK(cudaMemGetInfo(&free_b, &total_b));
+    double budget = hbm_budget_bytes > 0 ? (double)hbm_budget_bytes : planner_alpha() * (double)free_b;
+    budget = std::min(budget, 0.98 * (double)free_b);
+
+    std::vector<Candidate> cands;
+    int rc = enumerate_candidates(h->D, h->dtype, k, mode, h->B_req, n_applies_hint, budget, h->sm_count, cands);
+    if (rc) {
+        copy_json(plan_json(h->D, h->dtype, k, n_applies_hint, budget, 0, cands), json_out, json_cap);
+        set_error("mfh_plan: no candidate plan fits in %.0f bytes", budget);
+        return rc;
+    }
+    auto make_plan = [&](const Candidate& c) {
+        Plan p;
+        p.B = c.B;
+        p.k = k;
+        p.cached_per_row = c.cached_per_row;
+        build_tables(p, h->D, h->dtype, h->sm_count);
+        return p;
+    };
+    if (measure) {   // Algorithm 2: K_bench best feasible candidates, argmin of the measured time
+        const int K_bench = 8;
+        int tried = 0;
+        for (auto& c : cands) {
+            if (!c.feasible || tried >= K_bench) continue;
+            ++tried;
+            rc = commit_plan(h, make_plan(c), st);
+            if (rc == MFH_ERR_OUT_OF_MEMORY) { c.feasible = false; continue; }
+            if (rc) return rc;
+            double s = 0.0;
+            if ((rc = time_plan(h, st, s))) return rc;
+            c.t_measured = s;
+        }
+        std::stable_sort(cands.begin(), cands.end(), [&](const Candidate& a, const Candidate& b) {
+            const bool ma = a.t_measured >= 0, mb = b.t_measured >= 0;
+            if (ma != mb) return ma;
+            if (!ma) return false;
+            const double n = (double)std::max<int64_t>(n_applies_hint, 1);
+            return n * a.t_measured + a.t_fill < n * b.t_measured + b.t_fill;   // Eq. 22-23 with W = 1
+        });
+        if (cands.empty() || cands[0].t_measured < 0) {
+            set_error("mfh_plan: no candidate could be committed");
+            return MFH_ERR_OUT_OF_MEMORY;
+        }
+    }
+    rc = commit_plan(h, make_plan(cands[0]), st);
+    if (rc) return rc;
+    h->plan.json = plan_json(h->D, h->dtype, k, n_applies_hint, budget, measure, cands);
+    copy_json(h->plan.json, json_out, json_cap);
+    return MFH_OK;
+}
+
+MFH_API int mfh_get_plan(mfh_handle h, char* json_out, size_t json_cap)
+{
+    if (!h || !h->planned) { set_error("mfh_get_plan: handle not planned"); return MFH_ERR_BAD_STATE; }
+    const Plan& p = h->plan;
+    char buf[768];
+    snprintf(buf, sizeof buf,
+             "{\"mode\":\"%s\",\"B\":%d,\"n_blk\":%d,\"k\":%d,\"cached_blocks\":%lld,\"cached_per_row\":%d,"
+             "\"cache_bytes\":%zu,\"work_bytes\":%zu,\"partial_slots\":%d,\"proc_items\":%zu,"
+             "\"proc_warps\":%d,\"proc_row_strips\":%d,\"launches_per_apply\":%d}",
+             p.mode == MFH_MODE_FULL ? "full" : (p.mode == MFH_MODE_PARTIAL ? "partial" : "procedural"), p.B,
+             p.n_blk, p.k, (long long)p.n_cached, p.cached_per_row, p.cache_bytes, p.work_bytes, p.n_slots,
+             p.items.size(), p.warps, p.Q,
+             1 + (p.n_cached > 0) + ((p.k == 1 && !p.items.empty()) || p.slot_multi >= 0));
+    copy_json(buf, json_out, json_cap);
+    return MFH_OK;
+}
+
+MFH_API int mfh_apply(mfh_handle h, const void* psi_dev, void* phi_dev, int32_t k,
+                      const double* lambdas_host, void* stream)
+{
+    if (!h || !psi_dev || !phi_dev || psi_dev == phi_dev) {
+        set_error("mfh_apply: NULL or aliased pointer");
+        return MFH_ERR_INVALID_ARG;
+    }
+    if (!h->planned) { set_error("mfh_apply: call mfh_plan first"); return MFH_ERR_BAD_STATE; }
+    if (k != h->plan.k) {
+        set_error("mfh_apply: k=%d differs from the planned k=%d", k, h->plan.k);
+        return MFH_ERR_INVALID_ARG;
+    }
+    return apply_impl(h, psi_dev, phi_dev, lambdas_host, (cudaStream_t)stream);
+}
+
+MFH_API int mfh_apply_host(mfh_handle h, const void* psi_host, void* phi_host, int32_t k,
+                           const double* lambdas_host, void* stream)
+{
+    if (!h || !psi_host || !phi_host) { set_error("mfh_apply_host: NULL pointer"); return MFH_ERR_INVALID_ARG; }
+    if (!h->planned) { set_error("mfh_apply_host: call mfh_plan first"); return MFH_ERR_BAD_STATE; }
+    if (k != h->plan.k) { set_error("mfh_apply_host: k mismatch"); return MFH_ERR_INVALID_ARG; }
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t bytes = (size_t)h->D * k * complex_bytes(h->dtype);
+    char* psi = (char*)h->d_io;
+    char* phi = psi + bytes;
+    MFH_CUDA_CHECK(cudaMemcpyAsync(psi, psi_host, bytes, cudaMemcpyHostToDevice, st));
+    int rc = apply_impl(h, psi, phi, lambdas_host, st);
+    if (rc) return rc;
+    MFH_CUDA_CHECK(cudaMemcpyAsync(phi_host, phi, bytes, cudaMemcpyDeviceToHost, st));
+    MFH_CUDA_CHECK(cudaStreamSynchronize(st));
+    return MFH_OK;
+}
+
+MFH_API int mfh_chebyshev(mfh_handle h, const void* psi_dev, void* out_dev, double t, double e_min,
+                          double e_max, double tol, int32_t* n_terms_out, void* stream)
+{
+    if (!h || !psi_dev || !out_dev) { set_error("mfh_chebyshev: NULL pointer"); return MFH_ERR_INVALID_ARG; }
+    if (!h->planned) { set_error("mfh_chebyshev: call mfh_plan first"); return MFH_ERR_BAD_STATE; }
+    if (h->plan.k != 1) { set_error("mfh_chebyshev: plan with k = 1"); return MFH_ERR_INVALID_ARG; }
+    if (!(e_max > e_min) || !std::isfinite(t) || !std::isfinite(e_min) || !std::isfinite(e_max) || !(tol > 0.0)) {
+        set_error("mfh_chebyshev: need e_max > e_min, finite t, tol > 0");
+        return MFH_ERR_INVALID_ARG;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    const double c = 0.5 * (e_max + e_min), R = 0.5 * (e_max - e_min), a = R * t;
+    // Bessel table J_l(a) via the C++17 special function (a route different from the oracle's
+    // Miller recurrence), K = 1 + last l with |J_l| >= tol.
+    const double x = std::fabs(a);
+    const int l_max = (int)(x + 80.0 + 12.0 * std::cbrt(x));
+    std::vector<double> J(l_max + 1);
+    int K = 1;
+    for (int l = 0; l <= l_max; ++l) {
+        double v = (x == 0.0) ? (l == 0 ? 1.0 : 0.0) : std::cyl_bessel_j((double)l, x);
+        if (a < 0 && (l & 1)) v = -v;
+        J[l] = v;
+        if (std::fabs(v) >= tol) K = l + 1;
+    }
+    if (K >= l_max) { set_error("mfh_chebyshev: Bessel table too short"); return MFH_ERR_NOT_CONVERGED; }
+    if (n_terms_out) *n_terms_out = K;
+
+    const size_t vb = (size_t)h->D * complex_bytes(h->dtype);
+    if (!h->d_cheb) MFH_CUDA_CHECK(cudaMalloc(&h->d_cheb, 4 * vb));
+    char* base = (char*)h->d_cheb;
+    void *cur = base, *prev = base + vb, *acc = base + 2 * vb, *hq = base + 3 * vb;
+    int rc;
+    if ((rc = launch_cheb_first(h, psi_dev, cur, acc, J[0], st))) return rc;      // Eq. 41
+    for (int l = 1; l < K; ++l) {
+        if ((rc = apply_impl(h, cur, hq, nullptr, st))) return rc;
+        double cr = 0.0, ci = 0.0;                                                  // 2 (-i)^l J_l
+        switch (l & 3) {
+        case 0: cr = 2.0 * J[l]; break;
+        case 1: ci = -2.0 * J[l]; break;
+        case 2: cr = -2.0 * J[l]; break;
+        case 3: ci = 2.0 * J[l]; break;
+        }
+        if ((rc = launch_cheb_step(h, hq, cur, prev, acc, c, 1.0 / R, l == 1, cr, ci, st))) return rc;   // Eq. 42-43
+        std::swap(cur, prev);
+    }
+    return launch_cheb_final(h, acc, out_dev, std::cos(c * t), -std::sin(c * t), st);
+}
+
+MFH_API int mfh_debug_philox(uint64_t seed, uint32_t stream_id, const uint32_t* i_dev,
+                             const uint32_t* j_dev, int64_t n, uint32_t* words_dev, void* stream)
+{
+    if (n < 0 || (n > 0 && (!i_dev || !j_dev || !words_dev))) {
+        set_error("mfh_debug_philox: invalid argument");
+        return MFH_ERR_INVALID_ARG;
+    }
+    return launch_philox_debug(seed, stream_id, i_dev, j_dev, n, words_dev, (cudaStream_t)stream);
+}
+
+MFH_API int mfh_materialize_block(mfh_handle h, int32_t n, int32_t m, void* block_dev, void* stream)
+{
+    if (!h || !block_dev) { set_error("mfh_materialize_block: NULL pointer"); return MFH_ERR_INVALID_ARG; }
+    const int32_t B = h->planned ? h->plan.B : h->B_req;
+    if (B <= 0) { set_error("mfh_materialize_block: block size not fixed yet"); return MFH_ERR_BAD_STATE; }
+    const int32_t n_blk = (int32_t)(h->D / B);
+    if (n < 0 || m < 0 || n >= n_blk || m >= n_blk) {
+        set_error("mfh_materialize_block: block (%d,%d) outside %d x %d", n, m, n_blk, n_blk);
+        return MFH_ERR_INVALID_ARG;
+    }
+    return launch_fill_block(h, B, n, m, block_dev, (cudaStream_t)stream);
+}
+
+MFH_API int mfh_debug_h0(mfh_handle h, void* h0_dev, void* stream)
+{
+    if (!h || !h0_dev) { set_error("mfh_debug_h0: NULL pointer"); return MFH_ERR_INVALID_ARG; }
+    return launch_h0(h, h0_dev, (cudaStream_t)stream);
+}
+
+}  // extern "C"

@@ -1,0 +1,109 @@
+// mfh_internal.cuh -- handle, plan tables and launcher prototypes shared by the .cu files.
+#pragma once
+#include <cstdint>
+#include <cstdio>
+#include <string>
+#include <vector>
+#include <cuda_runtime.h>
+
+#include "mfh.h"
+#include "mfh_gen.cuh"
+
+namespace mfh {
+
+template <typename T> struct Cplx;
+template <> struct Cplx<double> { using type = double2; };
+template <> struct Cplx<float> { using type = float2; };
+
+// Block-pair roles in the procedural kernel (host table N_blk x N_blk, row n, column m).
+enum : uint8_t {
+    PAIR_NONE = 0,      // not generated from (n,m): cached, or covered by the mirrored pair (m,n)
+    PAIR_TWO_SIDED = 1, // n < m, both (n,m) and (m,n) uncached: generate once, use for both
+    PAIR_ONE_SIDED = 2, // generate (n,m) for phi^[n] only
+    PAIR_DIAG = 3       // n == m: upper sub-tiles two-sided, diagonal sub-tiles one-sided
+};
+
+// One work item of the single-vector procedural kernel: a strip of rows of block n times all
+// columns of block m.
+struct ProcItem {
+    int32_t n, m;       // block pair
+    int32_t row0;       // first row of the strip inside block n
+    int32_t nrows;      // strip height (multiple of the macro tile)
+    int32_t kind;       // PAIR_*
+    int32_t col_slot;   // partial slot receiving the column-side sums (-1: none)
+};
+
+struct Plan {
+    int32_t mode = 0;          // MFH_MODE_* actually committed
+    int32_t B = 0, n_blk = 0, k = 0;
+    int32_t Q = 1;             // row strips per block in the procedural kernel
+    int32_t warps = 8;         // warps per CTA of the procedural kernel (macro tile = 32*warps)
+    int64_t n_cached = 0;      // cached blocks
+    int32_t cached_per_row = 0;
+    int32_t n_slots = 0;       // partial vectors in the workspace
+    int32_t slot_cache = -1, slot_row0 = -1, slot_col0 = -1, slot_multi = -1;
+    size_t cache_bytes = 0, work_bytes = 0;
+    std::vector<int32_t> cache_slot;   // [n_blk*n_blk] index of the cached block or -1
+    std::vector<uint8_t> pair_kind;    // [n_blk*n_blk]
+    std::vector<ProcItem> items;
+    std::vector<uint8_t> slot_valid;   // [n_blk][n_slots]
+    std::string json;
+};
+
+}  // namespace mfh
+
+struct mfh_handle_s {
+    int64_t D = 0;
+    int32_t B_req = 0;
+    uint64_t seed = 0, seed_h0 = 0;
+    int32_t kind = 0, dtype = 0;
+    double lambda = 1.0;
+    bool planned = false;
+    mfh::Plan plan;
+    // device resources (library-owned)
+    void* d_cache = nullptr;
+    void* d_work = nullptr;         // partial slots: [n_slots][D][k] complex
+    void* d_h0 = nullptr;           // D reals (DIAG_PLUS_GUE)
+    int32_t* d_cache_slot = nullptr;
+    mfh::ProcItem* d_items = nullptr;
+    uint8_t* d_slot_valid = nullptr;
+    double* d_lambdas = nullptr;    // MFH_MAX_K doubles, refreshed by every apply
+    int32_t* d_counter = nullptr;   // dynamic work counter of the procedural kernel
+    void* d_cheb = nullptr;         // 3 vectors of Chebyshev scratch
+    void* d_io = nullptr;           // psi/phi staging of mfh_apply_host
+    int sm_count = 148;
+};
+
+namespace mfh {
+
+void set_error(const char* fmt, ...);
+size_t complex_bytes(int dtype);
+
+#define MFH_CUDA_CHECK(expr)                                                                   \
+    do {                                                                                       \
+        cudaError_t _e = (expr);                                                               \
+        if (_e != cudaSuccess) {                                                               \
+            mfh::set_error("%s failed: %s (%s:%d)", #expr, cudaGetErrorString(_e), __FILE__,   \
+                           __LINE__);                                                          \
+            return MFH_ERR_CUDA;                                                               \
+        }                                                                                      \
+    } while (0)
+
+// ---- launchers (mfh_proc.cu, mfh_cached.cu, mfh_vec.cu) ----
+int launch_philox_debug(uint64_t seed, uint32_t stream_id, const uint32_t* i, const uint32_t* j,
+                        int64_t n, uint32_t* words, cudaStream_t st);
+int launch_fill_block(mfh_handle h, int32_t B, int32_t n, int32_t m, void* out, cudaStream_t st);
+int launch_fill_cache(mfh_handle h, cudaStream_t st);
+int launch_h0(mfh_handle h, void* out, cudaStream_t st);
+int launch_proc_single(mfh_handle h, const void* psi, cudaStream_t st);
+int launch_proc_multi(mfh_handle h, const void* psi, cudaStream_t st);
+int launch_cached(mfh_handle h, const void* psi, cudaStream_t st);
+int launch_reduce(mfh_handle h, const void* psi, void* phi, const double* lambdas_host, cudaStream_t st);
+int launch_cheb_first(mfh_handle h, const void* psi, void* q_prev, void* acc, double j0,
+                      cudaStream_t st);
+int launch_cheb_step(mfh_handle h, const void* hq, const void* q, void* prev_dst, void* acc, double c,
+                     double inv_r, int first, double coef_re, double coef_im, cudaStream_t st);
+int launch_cheb_final(mfh_handle h, const void* acc, void* out, double ph_re, double ph_im,
+                      cudaStream_t st);
+
+}  // namespace mfh

@@ -1,0 +1,291 @@
+// mfh_plan.cu -- single-GPU execution planner (host code).
+//   Algorithm 1, analytic memory-constrained planning      P:258-296, Eq. 14-20
+//   adaptive block size / cache budget                      P:409-446, Eq. 27
+//   runtime model T = N_blk^2 [t_src + t_mv] (or the max)    P:533-547, Eq. 32-33; Eq. 36
+// and the tables a committed plan needs: which blocks are cached, how the uncached block pairs
+// are split into work items of the fused kernel, and which partial-sum slots feed each block row.
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include "mfh_internal.cuh"
+#include "mfh_plan.h"
+
+namespace mfh {
+
+// Model constants (seconds, bytes/s, generations/s).  Starting values; the measured planner
+// (mfh_plan with measure != 0) overrides the ranking with device timings (Algorithm 2).
+static const double kAlpha = 0.9;            // safety fraction of Eq. 18 (the paper gives none)
+static const double kBwRead = 6.0e12;        // cached streaming, B/s
+static const double kBwWrite = 3.0e12;       // cache fill stores, B/s
+static const double kLaunch = 6e-6;          // per kernel launch
+
+static double gen_pairs_per_s(int dtype) { return dtype == MFH_C128 ? 2.4e11 : 6.0e11; }
+static double gen_entries_per_s(int dtype, int k)
+{
+    // one-sided generation plus 4k FMAs per entry on the same issue slots
+    const double gen = dtype == MFH_C128 ? 1.6e11 : 5.0e11;
+    const double mac = dtype == MFH_C128 ? 2.3e12 : 9.0e12;   // complex MACs/s (FP64 / FP32 FMA rate / 4)
+    return 1.0 / (1.0 / gen + (double)k / mac);
+}
+
+static void appendf(std::string& s, const char* fmt, ...)
+{
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    s += buf;
+}
+
+static const char* mode_name(int mode)
+{
+    switch (mode) {
+    case MFH_MODE_PROCEDURAL: return "procedural";
+    case MFH_MODE_PARTIAL: return "partial";
+    case MFH_MODE_FULL: return "full";
+    }
+    return "auto";
+}
+
+// Offsets d = (m - n) mod N in the order 0, +1, -1, +2, -2, ...: a symmetric band around the
+// diagonal, so that uncached blocks come in mirrored pairs the fused kernel generates once.
+static std::vector<int> band_offsets(int N)
+{
+    std::vector<int> out;
+    std::vector<char> seen(N, 0);
+    for (int d = 0; (int)out.size() < N; ++d) {
+        const int cand[2] = {((d % N) + N) % N, ((-d % N) + N) % N};
+        for (int c : cand)
+            if (!seen[c]) {
+                seen[c] = 1;
+                out.push_back(c);
+            }
+    }
+    return out;
+}
+
+void choose_tiling(int B, int n_pairs, int sm_count, int& warps, int& Q)
+{
+    const int cands[4] = {8, 4, 2, 1};
+    warps = 1;
+    Q = 1;
+    for (int W : cands) {
+        if (B % (32 * W) != 0) continue;
+        const int qmax = B / (32 * W);
+        int q = 1;
+        while (q < qmax && (int64_t)n_pairs * q < 4LL * sm_count) q *= 2;
+        warps = W;
+        Q = q;
+        if ((int64_t)n_pairs * q >= 2LL * sm_count) return;   // enough items for every SM
+    }
+    // nothing reached 2 items per SM: keep the smallest valid W (most items)
+}
+
+void build_tables(Plan& p, int64_t D, int dtype, int sm_count)
+{
+    const int N = p.n_blk = (int)(D / p.B);
+    const int c = p.cached_per_row;
+    p.n_cached = (int64_t)c * N;
+    p.cache_slot.assign((size_t)N * N, -1);
+    const std::vector<int> offs = band_offsets(N);
+    for (int n = 0; n < N; ++n)
+        for (int t = 0; t < c; ++t) p.cache_slot[(size_t)n * N + (n + offs[t]) % N] = n * c + t;
+    auto uncached = [&](int n, int m) { return p.cache_slot[(size_t)n * N + m] < 0; };
+
+    p.pair_kind.assign((size_t)N * N, PAIR_NONE);
+    p.items.clear();
+    int n_pairs = 0;
+    bool any_col = false;
+    if (p.k == 1) {
+        for (int n = 0; n < N; ++n) {
+            if (uncached(n, n)) p.pair_kind[(size_t)n * N + n] = PAIR_DIAG;
+            for (int m = n + 1; m < N; ++m) {
+                const bool a = uncached(n, m), b = uncached(m, n);
+                if (a && b) p.pair_kind[(size_t)n * N + m] = PAIR_TWO_SIDED;
+                else if (a) p.pair_kind[(size_t)n * N + m] = PAIR_ONE_SIDED;
+                else if (b) p.pair_kind[(size_t)m * N + n] = PAIR_ONE_SIDED;
+            }
+        }
+        for (uint8_t kd : p.pair_kind) {
+            n_pairs += (kd != PAIR_NONE);
+            any_col |= (kd == PAIR_TWO_SIDED || kd == PAIR_DIAG);
+        }
+    }
+    choose_tiling(p.B, std::max(n_pairs, 1), sm_count, p.warps, p.Q);
+
+    // partial-sum slots
+    int s = 0;
+    p.slot_cache = p.slot_row0 = p.slot_col0 = p.slot_multi = -1;
+    if (c > 0) p.slot_cache = s++;
+    if (p.k == 1 && n_pairs > 0) {
+        p.slot_row0 = s;
+        s += N;
+        if (any_col) {
+            p.slot_col0 = s;
+            s += N * p.Q;
+        }
+    }
+    if (p.k > 1 && c < N) p.slot_multi = s++;
+    p.n_slots = s;
+    p.slot_valid.assign((size_t)N * std::max(s, 1), 0);
+    auto valid = [&](int b, int slot) -> uint8_t& { return p.slot_valid[(size_t)b * p.n_slots + slot]; };
+    for (int b = 0; b < N; ++b) {
+        if (p.slot_cache >= 0) valid(b, p.slot_cache) = 1;
+        if (p.slot_multi >= 0) valid(b, p.slot_multi) = 1;
+    }
+    if (p.k == 1 && n_pairs > 0) {
+        const int strip = p.B / p.Q;
+        // full-size two-sided items first, the half-size diagonal items last (better tail)
+        for (int pass = 0; pass < 2; ++pass)
+            for (int n = 0; n < N; ++n)
+                for (int m = 0; m < N; ++m) {
+                    const uint8_t kd = p.pair_kind[(size_t)n * N + m];
+                    if (kd == PAIR_NONE || (pass == 0) != (kd != PAIR_DIAG)) continue;
+                    valid(n, p.slot_row0 + m) = 1;
+                    const bool col = (kd == PAIR_TWO_SIDED || kd == PAIR_DIAG);
+                    for (int q = 0; q < p.Q; ++q) {
+                        ProcItem it;
+                        it.n = n;
+                        it.m = m;
+                        it.row0 = q * strip;
+                        it.nrows = strip;
+                        it.kind = kd;
+                        it.col_slot = col ? p.slot_col0 + n * p.Q + q : -1;
+                        if (col) valid(m, it.col_slot) = 1;
+                        p.items.push_back(it);
+                    }
+                }
+    }
+    const size_t cb = complex_bytes(dtype);
+    p.cache_bytes = (size_t)p.n_cached * p.B * p.B * cb;
+    p.work_bytes = (size_t)std::max(p.n_slots, 1) * D * p.k * cb;
+    p.mode = (c == 0) ? MFH_MODE_PROCEDURAL : (c == N ? MFH_MODE_FULL : MFH_MODE_PARTIAL);
+}
+
+// Scratch outside the partial slots: Chebyshev (3 vectors), host-apply staging (2 k vectors), H0.
+static size_t fixed_work_bytes(int64_t D, int dtype, int k)
+{
+    return (size_t)D * complex_bytes(dtype) * (3 + 2 * k) + (size_t)D * 8;
+}
+
+Candidate evaluate_candidate(int64_t D, int dtype, int k, int B, int cached_per_row, int64_t n_applies,
+                             int sm_count)
+{
+    Candidate c;
+    Plan p;
+    p.B = B;
+    p.k = k;
+    p.cached_per_row = cached_per_row;
+    build_tables(p, D, dtype, sm_count);
+    c.B = B;
+    c.mode = p.mode;
+    c.cached_per_row = cached_per_row;
+    c.n_cached = p.n_cached;
+    c.n_blk = p.n_blk;
+    c.cache_bytes = (double)p.cache_bytes;                                   // M_op, Eq. 15-17
+    c.work_bytes = (double)p.work_bytes + (double)fixed_work_bytes(D, dtype, k);   // M_work, Eq. 14
+    const double cb = (double)complex_bytes(dtype);
+    const double f = (double)p.n_cached / ((double)p.n_blk * p.n_blk);
+    const double entries = (double)D * (double)D;
+    c.t_cached = f * entries * cb / kBwRead;
+    if (k == 1) {
+        // generations: one per mirrored pair, one per one-sided entry, ~half of a diagonal block
+        double gens = 0.0;
+        for (uint8_t kd : p.pair_kind) {
+            if (kd == PAIR_TWO_SIDED || kd == PAIR_ONE_SIDED) gens += (double)B * B;
+            else if (kd == PAIR_DIAG) gens += 0.5 * (double)B * (B + 32.0 * p.warps);
+        }
+        double t = gens / gen_pairs_per_s(dtype);
+        if (!p.items.empty()) {   // tail effect of whole-item scheduling
+            const double slots = 2.0 * sm_count;
+            const double waves = (double)p.items.size() / slots;
+            t *= std::ceil(waves) / waves > 1.5 ? 1.5 : std::ceil(waves) / waves;
+        }
+        c.t_proc = t;
+    } else {
+        c.t_proc = (1.0 - f) * entries / gen_entries_per_s(dtype, k);
+    }
+    int launches = 1 + (p.n_cached > 0) + (p.n_cached < (int64_t)p.n_blk * p.n_blk);
+    c.t_reduce = (double)p.n_slots * 0.6 * D * k * cb / kBwRead;
+    c.t_apply = c.t_cached + c.t_proc + c.t_reduce + launches * kLaunch;   // Eq. 32 (not overlapped)
+    c.t_fill = f * entries / gen_entries_per_s(dtype, 0) + f * entries * cb / kBwWrite;
+    c.t_job = (double)std::max<int64_t>(n_applies, 1) * c.t_apply + c.t_fill;
+    c.flops = 8.0 * entries * k;                                            // F_mv, Eq. 13
+    return c;
+}
+
+static void candidate_json(std::string& s, const Candidate& c)
+{
+    appendf(s, "{\"mode\":\"%s\",\"B\":%d,\"n_blk\":%d,\"cached_blocks\":%lld,\"cached_per_row\":%d,",
+            mode_name(c.mode), c.B, c.n_blk, (long long)c.n_cached, c.cached_per_row);
+    appendf(s, "\"cache_bytes\":%.0f,\"work_bytes\":%.0f,\"total_bytes\":%.0f,\"feasible\":%s,",
+            c.cache_bytes, c.work_bytes, c.cache_bytes + c.work_bytes, c.feasible ? "true" : "false");
+    appendf(s, "\"model_apply_s\":%.6g,\"model_cached_s\":%.6g,\"model_proc_s\":%.6g,\"model_fill_s\":%.6g,"
+               "\"model_job_s\":%.6g,\"flops_per_apply\":%.6g,\"measured_apply_s\":%.6g}",
+            c.t_apply, c.t_cached, c.t_proc, c.t_fill, c.t_job, c.flops, c.t_measured);
+}
+
+int enumerate_candidates(int64_t D, int dtype, int k, int mode, int B_req, int64_t n_applies,
+                         double budget_bytes, int sm_count, std::vector<Candidate>& out)
+{
+    out.clear();
+    std::vector<int> Bs;
+    if (B_req > 0) Bs.push_back(B_req);
+    else
+        for (int B = MFH_MAX_B; B >= MFH_MIN_B; B /= 2)
+            if (D % B == 0) Bs.push_back(B);
+    const double cb = (double)complex_bytes(dtype);
+    for (int B : Bs) {
+        const int N = (int)(D / B);
+        // cache budget -> cached blocks per row (Eq. 27 with full blocks; rows kept balanced)
+        auto fits = [&](int c) {
+            Candidate t = evaluate_candidate(D, dtype, k, B, c, n_applies, sm_count);
+            return t.cache_bytes + t.work_bytes <= budget_bytes;
+        };
+        std::vector<int> cs;
+        if (mode == MFH_MODE_AUTO || mode == MFH_MODE_PROCEDURAL) cs.push_back(0);
+        if (mode == MFH_MODE_AUTO || mode == MFH_MODE_FULL) cs.push_back(N);
+        if (mode == MFH_MODE_AUTO || mode == MFH_MODE_PARTIAL) {
+            double room = budget_bytes - (double)fixed_work_bytes(D, dtype, k) - 3.0 * D * k * cb;
+            int c = (int)std::floor(room / ((double)B * B * cb * N));
+            c = std::min(c, N - 1);
+            while (c > 0 && !fits(c)) --c;
+            if (c > 0) cs.push_back(c);
+        }
+        for (int c : cs) {
+            Candidate cand = evaluate_candidate(D, dtype, k, B, c, n_applies, sm_count);
+            cand.feasible = (cand.cache_bytes + cand.work_bytes <= budget_bytes);   // Eq. 18
+            if (k > 1 && c > 0) cand.feasible = false;   // cached multi-vector kernel: not built yet
+            out.push_back(cand);
+        }
+    }
+    std::stable_sort(out.begin(), out.end(), [](const Candidate& a, const Candidate& b) {
+        if (a.feasible != b.feasible) return a.feasible;
+        return a.t_job < b.t_job;
+    });
+    return (!out.empty() && out[0].feasible) ? MFH_OK : MFH_ERR_OUT_OF_MEMORY;
+}
+
+std::string plan_json(int64_t D, int dtype, int k, int64_t n_applies, double budget, int measured,
+                      const std::vector<Candidate>& cands)
+{
+    std::string s;
+    appendf(s, "{\"D\":%lld,\"dtype\":\"%s\",\"k\":%d,\"n_applies_hint\":%lld,\"budget_bytes\":%.0f,"
+               "\"alpha\":%.2f,\"planner\":\"%s\",\"dense_bytes\":%.0f,\"chosen\":",
+            (long long)D, dtype == MFH_C128 ? "c128" : "c64", k, (long long)n_applies, budget, kAlpha,
+            measured ? "measured" : "analytic", (double)D * D * complex_bytes(dtype));
+    if (!cands.empty()) candidate_json(s, cands[0]);
+    else s += "null";
+    s += ",\"candidates\":[";
+    for (size_t i = 0; i < cands.size(); ++i) {
+        if (i) s += ",";
+        candidate_json(s, cands[i]);
+    }
+    s += "]}";
+    return s;
+}
+
+double planner_alpha() { return kAlpha; }
+
+}  // namespace mfh

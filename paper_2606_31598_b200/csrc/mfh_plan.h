@@ -1,0 +1,32 @@
+// mfh_plan.h -- planner types shared by mfh_plan.cu and mfh_api.cu (host only).
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+namespace mfh {
+
+struct Plan;
+
+// One candidate execution plan p and its model.
+struct Candidate {
+    int B = 0, n_blk = 0, mode = 0, cached_per_row = 0;
+    int64_t n_cached = 0;
+    double cache_bytes = 0, work_bytes = 0;              // M_op, M_work (Eq. 14-17)
+    double t_cached = 0, t_proc = 0, t_reduce = 0;       // seconds per apply, by part
+    double t_apply = 0, t_fill = 0, t_job = 0, flops = 0;
+    double t_measured = -1.0;                            // Algorithm 2 (Eq. 21), -1 = not measured
+    bool feasible = false;                               // Eq. 18
+};
+
+void choose_tiling(int B, int n_pairs, int sm_count, int& warps, int& Q);
+void build_tables(Plan& p, int64_t D, int dtype, int sm_count);
+Candidate evaluate_candidate(int64_t D, int dtype, int k, int B, int cached_per_row, int64_t n_applies,
+                             int sm_count);
+int enumerate_candidates(int64_t D, int dtype, int k, int mode, int B_req, int64_t n_applies,
+                         double budget_bytes, int sm_count, std::vector<Candidate>& out);
+std::string plan_json(int64_t D, int dtype, int k, int64_t n_applies, double budget, int measured,
+                      const std::vector<Candidate>& cands);
+double planner_alpha();
+
+}  // namespace mfh

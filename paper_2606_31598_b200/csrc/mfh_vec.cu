@@ -1,0 +1,171 @@
+// mfh_vec.cu -- O(D) vector kernels: the fixed-order reduction of partial sums with the
+// H0 + lambda V epilogue (BASELINE.json configs[2]) and the Chebyshev recurrence updates
+// (Eq. 41-44).  All are HBM-trivial next to the O(D^2) apply.
+#include <algorithm>
+#include "mfh_internal.cuh"
+
+namespace mfh {
+
+struct LamArr {
+    double v[MFH_MAX_K];
+};
+
+// phi[i][v] = h0_i psi[i][v] + lambda_v * sum_{valid slots s} work[s][i][v]; slots are added in
+// index order, so the result does not depend on CTA scheduling (no atomics).
+template <typename T>
+__global__ void __launch_bounds__(256) reduce_kernel(int64_t D, int32_t B, int32_t k, int32_t n_slots,
+                                                     const uint8_t* __restrict__ slot_valid,
+                                                     const typename Cplx<T>::type* __restrict__ work,
+                                                     const T* __restrict__ h0,
+                                                     const typename Cplx<T>::type* __restrict__ psi,
+                                                     typename Cplx<T>::type* __restrict__ phi, LamArr lam)
+{
+    using CT = typename Cplx<T>::type;
+    const int64_t total = D * k;
+    for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < total;
+         e += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t i = e / k;
+        const int v = (int)(e - i * k);
+        const uint8_t* valid = slot_valid + (size_t)(i / B) * n_slots;
+        double sr = 0.0, si = 0.0;
+        for (int s = 0; s < n_slots; ++s) {
+            if (valid[s]) {
+                const CT x = work[(size_t)s * total + e];
+                sr += (double)x.x;
+                si += (double)x.y;
+            }
+        }
+        double outr = lam.v[v] * sr, outi = lam.v[v] * si;
+        if (h0) {
+            const CT p = psi[e];
+            const double d = (double)h0[i];
+            outr = fma(d, (double)p.x, outr);
+            outi = fma(d, (double)p.y, outi);
+        }
+        CT o;
+        o.x = (T)outr;
+        o.y = (T)outi;
+        phi[e] = o;
+    }
+}
+
+int launch_reduce(mfh_handle h, const void* psi, void* phi, const double* lambdas, cudaStream_t st)
+{
+    const Plan& p = h->plan;
+    LamArr lam;
+    for (int v = 0; v < MFH_MAX_K; ++v) lam.v[v] = (v < p.k) ? (lambdas ? lambdas[v] : h->lambda) : 0.0;
+    const int64_t total = h->D * p.k;
+    const int blocks = (int)std::min<int64_t>((total + 255) / 256, (int64_t)h->sm_count * 8);
+    if (h->dtype == MFH_C128)
+        reduce_kernel<double><<<blocks, 256, 0, st>>>(h->D, p.B, p.k, p.n_slots, h->d_slot_valid,
+                                                       (const double2*)h->d_work, (const double*)h->d_h0,
+                                                       (const double2*)psi, (double2*)phi, lam);
+    else
+        reduce_kernel<float><<<blocks, 256, 0, st>>>(h->D, p.B, p.k, p.n_slots, h->d_slot_valid,
+                                                      (const float2*)h->d_work, (const float*)h->d_h0,
+                                                      (const float2*)psi, (float2*)phi, lam);
+    MFH_CUDA_CHECK(cudaGetLastError());
+    return MFH_OK;
+}
+
+// ---- Chebyshev -------------------------------------------------------------------------------
+// first:  q0 = psi, acc = J_0 q0                                            (Eq. 41)
+// step:   next = first ? (Hq - c q)/R : 2 (Hq - c q)/R - prev               (Eq. 42, 43)
+//         dst = next;  acc += coef * next      (coef = 2 (-i)^l J_l(a), complex)
+// final:  out = e^{-ict} acc
+template <typename T>
+__global__ void cheb_first_kernel(int64_t D, const typename Cplx<T>::type* __restrict__ psi,
+                                  typename Cplx<T>::type* __restrict__ q0,
+                                  typename Cplx<T>::type* __restrict__ acc, double j0)
+{
+    using CT = typename Cplx<T>::type;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < D;
+         i += (int64_t)gridDim.x * blockDim.x) {
+        const CT p = psi[i];
+        q0[i] = p;
+        CT a;
+        a.x = (T)(j0 * (double)p.x);
+        a.y = (T)(j0 * (double)p.y);
+        acc[i] = a;
+    }
+}
+
+template <typename T>
+__global__ void cheb_step_kernel(int64_t D, const typename Cplx<T>::type* __restrict__ hq,
+                                 const typename Cplx<T>::type* __restrict__ q,
+                                 typename Cplx<T>::type* prev_dst, typename Cplx<T>::type* __restrict__ acc,
+                                 double c, double inv_r, int first, double cr, double ci)
+{
+    using CT = typename Cplx<T>::type;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < D;
+         i += (int64_t)gridDim.x * blockDim.x) {
+        const CT hv = hq[i], qv = q[i];
+        double nr = ((double)hv.x - c * (double)qv.x) * inv_r;
+        double ni = ((double)hv.y - c * (double)qv.y) * inv_r;
+        if (!first) {
+            const CT pv = prev_dst[i];
+            nr = 2.0 * nr - (double)pv.x;
+            ni = 2.0 * ni - (double)pv.y;
+        }
+        CT nx;
+        nx.x = (T)nr;
+        nx.y = (T)ni;
+        prev_dst[i] = nx;
+        CT a = acc[i];
+        a.x = (T)((double)a.x + cr * nr - ci * ni);
+        a.y = (T)((double)a.y + cr * ni + ci * nr);
+        acc[i] = a;
+    }
+}
+
+template <typename T>
+__global__ void cheb_final_kernel(int64_t D, const typename Cplx<T>::type* __restrict__ acc,
+                                  typename Cplx<T>::type* __restrict__ out, double pr, double pi)
+{
+    using CT = typename Cplx<T>::type;
+    for (int64_t i = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; i < D;
+         i += (int64_t)gridDim.x * blockDim.x) {
+        const CT a = acc[i];
+        CT o;
+        o.x = (T)(pr * (double)a.x - pi * (double)a.y);
+        o.y = (T)(pr * (double)a.y + pi * (double)a.x);
+        out[i] = o;
+    }
+}
+
+static int vec_blocks(mfh_handle h) { return (int)std::min<int64_t>((h->D + 255) / 256, (int64_t)h->sm_count * 8); }
+
+int launch_cheb_first(mfh_handle h, const void* psi, void* q0, void* acc, double j0, cudaStream_t st)
+{
+    if (h->dtype == MFH_C128)
+        cheb_first_kernel<double><<<vec_blocks(h), 256, 0, st>>>(h->D, (const double2*)psi, (double2*)q0, (double2*)acc, j0);
+    else
+        cheb_first_kernel<float><<<vec_blocks(h), 256, 0, st>>>(h->D, (const float2*)psi, (float2*)q0, (float2*)acc, j0);
+    MFH_CUDA_CHECK(cudaGetLastError());
+    return MFH_OK;
+}
+
+int launch_cheb_step(mfh_handle h, const void* hq, const void* q, void* prev_dst, void* acc, double c,
+                     double inv_r, int first, double coef_re, double coef_im, cudaStream_t st)
+{
+    if (h->dtype == MFH_C128)
+        cheb_step_kernel<double><<<vec_blocks(h), 256, 0, st>>>(h->D, (const double2*)hq, (const double2*)q, (double2*)prev_dst,
+                                                                 (double2*)acc, c, inv_r, first, coef_re, coef_im);
+    else
+        cheb_step_kernel<float><<<vec_blocks(h), 256, 0, st>>>(h->D, (const float2*)hq, (const float2*)q, (float2*)prev_dst,
+                                                                (float2*)acc, c, inv_r, first, coef_re, coef_im);
+    MFH_CUDA_CHECK(cudaGetLastError());
+    return MFH_OK;
+}
+
+int launch_cheb_final(mfh_handle h, const void* acc, void* out, double ph_re, double ph_im, cudaStream_t st)
+{
+    if (h->dtype == MFH_C128)
+        cheb_final_kernel<double><<<vec_blocks(h), 256, 0, st>>>(h->D, (const double2*)acc, (double2*)out, ph_re, ph_im);
+    else
+        cheb_final_kernel<float><<<vec_blocks(h), 256, 0, st>>>(h->D, (const float2*)acc, (float2*)out, ph_re, ph_im);
+    MFH_CUDA_CHECK(cudaGetLastError());
+    return MFH_OK;
+}
+
+}  // namespace mfh
