@@ -1,0 +1,368 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the hot path phi = H psi on B200 (BASELINE.json metric).
+
+    python bench.py --gpus N --steps K --warmup W            # the CUDA path (default N=1)
+    python bench.py --impl reference --steps K --warmup W    # the CPU oracle, as it stands
+
+A "step" is one pass of the whole hot path over one batch of synthetic input: one mfh_apply of the
+planned Hamiltonian on one normalised random psi.  At N=1 the workload is BASELINE.json
+configs[1] ("C2": D=65536, complex128, B=2048, full cache, 68.7 GB resident in HBM), the
+configuration the HBM-bound metric is quoted on.  The path does not shard (north_star: one GPU,
+no collectives): --gpus N runs N independent replicas ("replicas only") and the value
+is the sum over ranks divided by the max-over-ranks time.
+
+Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement" for every field.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+from paper_2606_31598_b200.inputs import CONFIGS, lambda_grid, make_psi, sample_rows  # noqa: E402
+
+METRIC = "matrix_entries_per_s"
+UNIT = "entries/s"
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, burst copy)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+# ---- clocks during the timed region (B200_PROFILING.md recipe) --------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self) -> dict:
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        self.thread.join(timeout=2)
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": max(mx), "power_w_max": max(pw),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---- CPU oracle legs (the only places bench.py may execute oracle/) ---------------------------
+def oracle_rows_apply(cfg: dict, psi, rows):
+    import oracle
+    if cfg["k"] > 1:
+        return oracle.apply_scan(cfg["D"], cfg["B"], cfg["seed"], cfg["seed_h0"], lambda_grid(cfg["k"]),
+                                 psi, rows=rows)
+    return oracle.apply(cfg["D"], cfg["B"], cfg["seed"], psi, rows=rows)
+
+
+def cpu_baseline(cfg: dict, psi, target_s: float = 15.0) -> dict:
+    """The oracle as it stands, timed on the host cores on a bounded row sample of the workload."""
+    import oracle
+    D = cfg["D"]
+    probe = sample_rows(D, 250, seed=1)[:256]
+    t0 = time.perf_counter()
+    oracle_rows_apply(cfg, psi, probe)
+    dt = time.perf_counter() - t0
+    n = int(min(max(len(probe) * target_s / max(dt, 1e-6), 256), D))
+    rows = np.arange(n, dtype=np.int64) * (D // n)
+    t0 = time.perf_counter()
+    oracle_rows_apply(cfg, psi, rows)
+    dt = time.perf_counter() - t0
+    return {"value": n * D / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"{n} evenly spaced output rows of {D} ({n * D:.3g} matrix entries, {dt:.1f} s); "
+                      f"implied full apply {D * D / (n * D / dt):.0f} s (extrapolated)"}
+
+
+def run_reference(args, cfg_name: str):
+    """--impl reference: the oracle on the same config/metric; each step a bounded row sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    cfg = CONFIGS[cfg_name]
+    D = cfg["D"]
+    psi = make_psi(D, cfg["psi_seed"], k=cfg["k"], dtype=cfg["dtype"])
+    n = max(64, min(D, int(2.0e8 / D)))          # ~2e8 entries per step: a few seconds on 8 cores
+    rows = np.arange(n, dtype=np.int64) * (D // n)
+    for _ in range(args.warmup):
+        oracle_rows_apply(cfg, psi, rows[: max(8, n // 8)])
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle_rows_apply(cfg, psi, rows)
+    dt = time.perf_counter() - t0
+    value = args.steps * n * D / dt
+    sample = f"{n} evenly spaced output rows of {D} per step ({n * D:.3g} entries)"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": workload_config(cfg_name, cfg),
+            "applies_per_s": value / (D * D),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(name: str, cfg: dict) -> dict:
+    return {"workload": f"{name}: seeded GUE D={cfg['D']} {cfg['dtype']} B={cfg['B']} {cfg['mode']} k={cfg['k']}",
+            "D": cfg["D"], "B": cfg["B"], "mode": cfg["mode"], "k": cfg["k"],
+            "l2_policy": "inputs larger than L2 (cached blocks)" if cfg["mode"] != "procedural"
+            else "no L2-resident input: entries are generated in registers; vectors only (flushed between steps)"}
+
+
+# ---- the CUDA path ---------------------------------------------------------------------------
+def make_handle(mfh, cfg: dict, n_applies: int):
+    kind = "diag_plus_gue" if "seed_h0" in cfg else "gue"
+    h = mfh.Hamiltonian(cfg["D"], cfg["B"], cfg["seed"], cfg["dtype"], kind=kind, seed_h0=cfg.get("seed_h0", 0))
+    plan = h.plan(cfg["mode"], k=cfg["k"], n_applies_hint=n_applies,
+                  hbm_budget_bytes=int(cfg.get("hbm_budget", 0)))
+    return h, plan
+
+
+def time_steps(torch, fn, steps: int, flush=None):
+    """CUDA-event time of `steps` calls on the current stream (ms total).  With `flush`, every step
+    has its own event pair and the L2 flush runs between pairs, outside the timed spans."""
+    if flush is None:
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(steps):
+            fn()
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b)
+    pairs = []
+    for _ in range(steps):
+        flush()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        fn()
+        b.record()
+        pairs.append((a, b))
+    torch.cuda.synchronize()
+    return sum(a.elapsed_time(b) for a, b in pairs)
+
+
+def measure_config(torch, mfh, name: str, steps: int, warmup: int, with_e2e: bool, barrier=None):
+    cfg = CONFIGS[name]
+    D, k = cfg["D"], cfg["k"]
+    psi_np = make_psi(D, cfg["psi_seed"], k=k, dtype=cfg["dtype"])
+    lam = lambda_grid(k) if k > 1 else None
+    t0 = time.perf_counter()
+    h, plan = make_handle(mfh, cfg, max(steps, 1))
+    torch.cuda.synchronize()
+    plan_s = time.perf_counter() - t0
+    info = h.get_plan()
+    psi = torch.from_numpy(psi_np).cuda()
+    phi = torch.empty_like(psi)
+    flush_buf = None
+    flush = None
+    if cfg["mode"] == "procedural":
+        flush_buf = torch.empty(256 * 2**20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+        flush = lambda: flush_buf.fill_(1)  # noqa: E731
+    fn = lambda: h.apply(psi, phi, lambdas=lam)  # noqa: E731
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    if barrier:
+        barrier()
+    ms = time_steps(torch, fn, steps, flush)
+    if barrier:
+        barrier()
+    # per-kernel durations: the same K steps again through mfh_apply_timed (events around each launch)
+    kern = {"cached": 0.0, "procedural": 0.0, "reduce": 0.0, "total": 0.0}
+    for _ in range(steps):
+        if flush:
+            flush()
+            torch.cuda.synchronize()
+        t = h.apply_timed(psi, phi, lambdas=lam)
+        for key in kern:
+            kern[key] += t[key] / steps
+    out = {"name": name, "cfg": cfg, "plan": info, "plan_s": plan_s, "ms_total": ms, "steps": steps,
+           "ms_per_step": ms / steps, "kernel_ms": kern, "psi_np": psi_np,
+           "launches_per_apply": info["launches_per_apply"]}
+    if with_e2e:
+        ph = torch.from_numpy(psi_np).pin_memory()
+        oh = torch.empty_like(ph).pin_memory()
+        for _ in range(max(1, warmup)):
+            h.apply_host(ph, oh, lambdas=lam)
+        e_ms = time_steps(torch, lambda: h.apply_host(ph, oh, lambdas=lam), steps)
+        out["e2e_ms_per_step"] = e_ms / steps
+        out["io_bytes"] = ph.numel() * ph.element_size()
+    h.destroy()
+    del psi, phi, flush_buf
+    torch.cuda.empty_cache()
+    return out
+
+
+def roofline_for(res: dict, hbm_gbs: float, peak_src: str) -> dict:
+    cfg = res["cfg"]
+    D, k = cfg["D"], cfg["k"]
+    cb = 16 if cfg["dtype"] == "c128" else 8
+    kern = res["kernel_ms"]
+    if kern["cached"] >= kern["procedural"]:
+        # HBM-bound cached streaming: algorithmic bytes = cached entries * bytes per entry
+        cached_entries = res["plan"]["cached_blocks"] * cfg["B"] ** 2
+        gbs = cached_entries * cb / (kern["cached"] * 1e-3) / 1e9
+        return {"kernel": "cached_kernel", "bound": "hbm", "achieved": gbs, "peak": hbm_gbs, "unit": "GB/s",
+                "frac": gbs / hbm_gbs, "traffic": None, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": cached_entries * cb, "kernel_ms": kern["cached"],
+                "share_of_step": kern["cached"] / max(kern["total"], 1e-9)}
+    # ALU-bound fused generate-and-apply: unit = matrix entries applied per second by that kernel
+    entries = (D * D - res["plan"]["cached_blocks"] * cfg["B"] ** 2)
+    rate = entries / (kern["procedural"] * 1e-3)
+    peak = PROC_PEAK[cfg["dtype"]]["k1" if k == 1 else "kN"]
+    return {"kernel": "proc_single_kernel" if k == 1 else "proc_multi_kernel", "bound": "alu",
+            "achieved": rate / 1e9, "peak": peak / 1e9, "unit": "Gentries/s", "frac": rate / peak,
+            "traffic": None, "peak_source": "DESIGN.md 'ALU roofline' (FP64/FP32 pipe instruction count at max clock)",
+            "kernel_ms": kern["procedural"], "share_of_step": kern["procedural"] / max(kern["total"], 1e-9)}
+
+
+# ALU ceilings in matrix entries/s derived in DESIGN.md ("ALU roofline") from the SASS instruction
+# count per generated entry and the pipe widths at 1965 MHz.
+PROC_PEAK = {"c128": {"k1": 3.7e11, "kN": 1.0e11}, "c64": {"k1": 1.5e12, "kN": 3.0e11}}
+
+
+def aggregate(dist, local_ms: float, local_units: float, device=None):
+    """max-over-ranks time and sum-over-ranks units (works with nccl and gloo)."""
+    if dist is None:
+        return local_ms, local_units
+    import torch
+    t = torch.tensor([local_ms], dtype=torch.float64, device=device)
+    u = torch.tensor([local_units], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--workload", default="C2", choices=sorted(CONFIGS))
+    ap.add_argument("--no-extra", action="store_true", help="skip the other configs' side measurements")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
+
+    if args.impl == "reference":
+        run_reference(args, args.workload)
+        return
+
+    import torch
+    from paper_2606_31598_b200 import binding as mfh
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
+    mfh.lib()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    barrier = (lambda: (dist.barrier(), torch.cuda.synchronize())) if dist else None
+
+    hbm_gbs, peak_src = load_peaks()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    res = measure_config(torch, mfh, args.workload, args.steps, args.warmup, with_e2e=True, barrier=barrier)
+    clocks = sampler.stop() if rank == 0 else None
+
+    cfg = res["cfg"]
+    D = cfg["D"]
+    dev = torch.device("cuda", local)
+    ms, units = aggregate(dist, res["ms_total"], float(args.steps) * D * D, dev)
+    e_ms, _ = aggregate(dist, res["e2e_ms_per_step"] * args.steps, 0.0, dev)
+    value = units / (ms * 1e-3)
+    e2e_value = units / (e_ms * 1e-3)
+
+    extras = {}
+    if rank == 0 and world == 1 and not args.no_extra:
+        for name, st in (("C1", 20), ("C3", 5), ("C4", 3)):
+            if name == args.workload:
+                continue
+            try:
+                r = measure_config(torch, mfh, name, st, 3, with_e2e=False)
+                rf = roofline_for(r, hbm_gbs, peak_src)
+                c = r["cfg"]
+                extras[name] = {"workload": workload_config(name, c)["workload"], "steps": st,
+                                "ms_per_apply": r["ms_per_step"], "applies_per_s": 1e3 / r["ms_per_step"],
+                                "matrix_entries_per_s": c["D"] ** 2 / (r["ms_per_step"] * 1e-3),
+                                "kernel_ms": r["kernel_ms"], "roofline": rf, "plan_s": r["plan_s"]}
+            except Exception as e:  # a side measurement must not lose the headline line
+                extras[name] = {"error": str(e)}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f64" if cfg["dtype"] == "c128" else "f32",
+                "data": "synthetic", "config": workload_config(args.workload, cfg),
+                "applies_per_s": value / (D * D), "plan": res["plan"], "plan_and_fill_s": res["plan_s"],
+                "kernel_ms": res["kernel_ms"], "roofline": roofline_for(res, hbm_gbs, peak_src),
+                "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": res["io_bytes"],
+                        "d2h_bytes_per_step": res["io_bytes"], "ms_per_step": e_ms / args.steps},
+                "gpu_launches": res["launches_per_apply"] * args.steps, "clocks": clocks,
+                "other_configs": extras}
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(cfg, res["psi_np"])
+        else:
+            line["cpu_baseline"] = None
+        print(json.dumps(line), flush=True)
+    if dist:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

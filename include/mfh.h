@@ -102,6 +102,13 @@ MFH_API int mfh_plan(mfh_handle h, int32_t mode, int32_t k, int64_t n_applies_hi
 MFH_API int mfh_apply(mfh_handle h, const void* psi_dev, void* phi_dev, int32_t k,
                       const double* lambdas_host, void* stream);
 
+/* Measurement export: mfh_apply with CUDA events recorded on `stream` around each of its launches;
+ * synchronises `stream`.  ms_out (host, 4 floats) = milliseconds of { cached streaming kernel,
+ * fused generate-and-apply kernel, reduce/epilogue kernel, whole apply } (0 for a kernel the plan
+ * does not launch).  bench.py uses it for the per-kernel roofline. */
+MFH_API int mfh_apply_timed(mfh_handle h, const void* psi_dev, void* phi_dev, int32_t k,
+                            const double* lambdas_host, void* stream, float* ms_out);
+
 /* Same as mfh_apply but with HOST buffers: copies psi to the device, applies, copies phi back and
  * synchronises `stream` (the end-to-end call bench.py times).  Host buffers should be pinned. */
 MFH_API int mfh_apply_host(mfh_handle h, const void* psi_host, void* phi_host, int32_t k,

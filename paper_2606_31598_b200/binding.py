@@ -1,0 +1,208 @@
+"""Thin ctypes binding of include/mfh.h -- argument marshalling only.
+
+Every step of phi = H psi runs in the CUDA kernels of ``lib/libmfh.so``; this module converts
+torch tensors to device pointers and the current torch stream to a ``cudaStream_t``.  There is no
+CPU fallback: loading fails loudly when the library is missing, and every compute call needs a
+CUDA device.  PyTorch is used for device memory and streams only.
+"""
+from __future__ import annotations
+
+import ctypes
+import json
+import os
+
+from . import build as _build
+
+MFH_OK = 0
+MFH_ERR_INVALID_ARG, MFH_ERR_BAD_STATE, MFH_ERR_OUT_OF_MEMORY = 1, 2, 3
+MFH_ERR_CUDA, MFH_ERR_NOT_CONVERGED, MFH_ERR_UNSUPPORTED = 4, 5, 6
+MFH_C128, MFH_C64 = 0, 1
+MFH_SRC_GUE, MFH_SRC_DIAG_PLUS_GUE = 0, 1
+MFH_MODE_AUTO, MFH_MODE_PROCEDURAL, MFH_MODE_PARTIAL, MFH_MODE_FULL = 0, 1, 2, 3
+MFH_MAX_K = 16
+
+DTYPES = {"c128": MFH_C128, "c64": MFH_C64}
+MODES = {"auto": MFH_MODE_AUTO, "procedural": MFH_MODE_PROCEDURAL, "partial": MFH_MODE_PARTIAL,
+         "full": MFH_MODE_FULL}
+
+# every symbol include/mfh.h declares (tests check that the library exports all of them)
+SYMBOLS = ["mfh_create", "mfh_plan_analytic", "mfh_plan", "mfh_apply", "mfh_apply_host", "mfh_apply_timed",
+           "mfh_chebyshev", "mfh_destroy", "mfh_last_error", "mfh_get_plan", "mfh_debug_philox",
+           "mfh_materialize_block", "mfh_debug_h0"]
+
+_lib = None
+
+
+class MfhError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"mfh error {code}: {msg}")
+        self.code = code
+
+
+def lib():
+    """Load lib/libmfh.so (must have been built: ``python -m paper_2606_31598_b200.build``)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if not os.path.exists(path):
+        raise RuntimeError(f"{path} is missing: build the CUDA library first "
+                           "(python paper_2606_31598_b200/build.py); there is no CPU fallback")
+    L = ctypes.CDLL(path)
+    vp, i32, i64, u32, u64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_uint32, ctypes.c_uint64
+    dbl, cp, sz = ctypes.c_double, ctypes.c_char_p, ctypes.c_size_t
+    L.mfh_create.argtypes = [ctypes.POINTER(vp), i64, i32, u64, i32, dbl, i32, u64]
+    L.mfh_plan_analytic.argtypes = [i64, i32, i32, i32, i32, i64, i64, cp, sz]
+    L.mfh_plan.argtypes = [vp, i32, i32, i64, i64, i32, vp, cp, sz]
+    L.mfh_apply.argtypes = [vp, vp, vp, i32, ctypes.POINTER(dbl), vp]
+    L.mfh_apply_host.argtypes = [vp, vp, vp, i32, ctypes.POINTER(dbl), vp]
+    L.mfh_apply_timed.argtypes = [vp, vp, vp, i32, ctypes.POINTER(dbl), vp, ctypes.POINTER(ctypes.c_float)]
+    L.mfh_chebyshev.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, ctypes.POINTER(i32), vp]
+    L.mfh_destroy.argtypes = [vp]
+    L.mfh_last_error.argtypes = []
+    L.mfh_last_error.restype = cp
+    L.mfh_get_plan.argtypes = [vp, cp, sz]
+    L.mfh_debug_philox.argtypes = [u64, u32, vp, vp, i64, vp, vp]
+    L.mfh_materialize_block.argtypes = [vp, i32, i32, vp, vp]
+    L.mfh_debug_h0.argtypes = [vp, vp, vp]
+    for name in SYMBOLS:
+        if name != "mfh_last_error":
+            getattr(L, name).restype = ctypes.c_int
+    _lib = L
+    return L
+
+
+def _check(rc: int):
+    if rc != MFH_OK:
+        raise MfhError(rc, lib().mfh_last_error().decode())
+
+
+def _stream():
+    import torch
+    return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _lam(lambdas, k):
+    if lambdas is None:
+        return None
+    arr = (ctypes.c_double * k)(*[float(x) for x in lambdas])
+    return arr
+
+
+def plan_analytic(D: int, dtype: str, k: int = 1, mode: str = "auto", B: int = 0,
+                  n_applies_hint: int = 1, hbm_free_bytes: int = 180 * 10**9) -> dict:
+    """Host-only analytic planner (Algorithm 1); needs no GPU."""
+    buf = ctypes.create_string_buffer(1 << 16)
+    rc = lib().mfh_plan_analytic(D, DTYPES[dtype], k, MODES[mode], B, n_applies_hint, hbm_free_bytes,
+                                 buf, len(buf))
+    rec = json.loads(buf.value.decode()) if buf.value else {}
+    if rc != MFH_OK:
+        raise MfhError(rc, lib().mfh_last_error().decode())
+    return rec
+
+
+class Hamiltonian:
+    """Handle of one seeded Hamiltonian (mfh_create ... mfh_destroy)."""
+
+    def __init__(self, D: int, B: int = 0, seed: int = 0, dtype: str = "c128", kind: str = "gue",
+                 lam: float = 1.0, seed_h0: int = 0):
+        self.D, self.dtype, self.k = D, dtype, None
+        self._h = ctypes.c_void_p()
+        src = MFH_SRC_GUE if kind == "gue" else MFH_SRC_DIAG_PLUS_GUE
+        _check(lib().mfh_create(ctypes.byref(self._h), D, B, seed, src, lam, DTYPES[dtype], seed_h0))
+
+    # -- torch plumbing ---------------------------------------------------------------------
+    def _torch_dtype(self):
+        import torch
+        return torch.complex128 if self.dtype == "c128" else torch.complex64
+
+    def _check_vec(self, x, k):
+        assert x.is_cuda and x.is_contiguous() and x.dtype == self._torch_dtype()
+        assert x.numel() == self.D * k, (x.shape, self.D, k)
+
+    # -- C ABI ------------------------------------------------------------------------------
+    def plan(self, mode: str = "auto", k: int = 1, n_applies_hint: int = 1, hbm_budget_bytes: int = 0,
+             measure: bool = False) -> dict:
+        buf = ctypes.create_string_buffer(1 << 16)
+        _check(lib().mfh_plan(self._h, MODES[mode], k, n_applies_hint, int(hbm_budget_bytes),
+                              1 if measure else 0, _stream(), buf, len(buf)))
+        self.k = k
+        return json.loads(buf.value.decode())
+
+    def get_plan(self) -> dict:
+        buf = ctypes.create_string_buffer(4096)
+        _check(lib().mfh_get_plan(self._h, buf, len(buf)))
+        return json.loads(buf.value.decode())
+
+    def apply(self, psi, phi=None, lambdas=None):
+        """phi = H psi on device tensors ([D] or [D,k] complex), asynchronous on the current stream."""
+        import torch
+        k = self.k or 1
+        self._check_vec(psi, k)
+        if phi is None:
+            phi = torch.empty_like(psi)
+        self._check_vec(phi, k)
+        _check(lib().mfh_apply(self._h, psi.data_ptr(), phi.data_ptr(), k, _lam(lambdas, k), _stream()))
+        return phi
+
+    def apply_timed(self, psi, phi, lambdas=None) -> dict:
+        """One apply with CUDA events around each launch; returns milliseconds per kernel."""
+        k = self.k or 1
+        self._check_vec(psi, k)
+        self._check_vec(phi, k)
+        ms = (ctypes.c_float * 4)()
+        _check(lib().mfh_apply_timed(self._h, psi.data_ptr(), phi.data_ptr(), k, _lam(lambdas, k),
+                                     _stream(), ms))
+        return {"cached": ms[0], "procedural": ms[1], "reduce": ms[2], "total": ms[3]}
+
+    def apply_host(self, psi_host, phi_host, lambdas=None):
+        """End-to-end call with HOST (pinned) torch tensors; synchronises."""
+        k = self.k or 1
+        assert not psi_host.is_cuda and not phi_host.is_cuda
+        _check(lib().mfh_apply_host(self._h, psi_host.data_ptr(), phi_host.data_ptr(), k,
+                                    _lam(lambdas, k), _stream()))
+        return phi_host
+
+    def chebyshev(self, psi, t: float, e_min: float, e_max: float, tol: float, out=None):
+        import torch
+        self._check_vec(psi, 1)
+        if out is None:
+            out = torch.empty_like(psi)
+        n = ctypes.c_int32(0)
+        _check(lib().mfh_chebyshev(self._h, psi.data_ptr(), out.data_ptr(), t, e_min, e_max, tol,
+                                   ctypes.byref(n), _stream()))
+        return out, int(n.value)
+
+    def materialize_block(self, n: int, m: int, B: int):
+        import torch
+        out = torch.empty((B, B), dtype=self._torch_dtype(), device="cuda")
+        _check(lib().mfh_materialize_block(self._h, n, m, out.data_ptr(), _stream()))
+        return out
+
+    def h0(self):
+        import torch
+        out = torch.empty(self.D, dtype=torch.float64 if self.dtype == "c128" else torch.float32,
+                          device="cuda")
+        _check(lib().mfh_debug_h0(self._h, out.data_ptr(), _stream()))
+        return out
+
+    def destroy(self):
+        if self._h:
+            lib().mfh_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def debug_philox(seed: int, stream_id: int, i, j):
+    """Raw Philox4x32-10 words [n,4] (uint32 as int64-safe torch.int32 bit patterns) for index pairs."""
+    import torch
+    assert i.is_cuda and j.is_cuda and i.dtype == torch.int32 and j.dtype == torch.int32
+    n = i.numel()
+    words = torch.empty((n, 4), dtype=torch.int32, device="cuda")
+    _check(lib().mfh_debug_philox(seed, stream_id, i.data_ptr(), j.data_ptr(), n, words.data_ptr(), _stream()))
+    return words

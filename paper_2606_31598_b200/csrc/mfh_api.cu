@@ -96,17 +96,24 @@ static int commit_plan(mfh_handle h, const Plan& p, cudaStream_t st)
     return MFH_OK;
 }
 
-static int apply_impl(mfh_handle h, const void* psi, void* phi, const double* lambdas, cudaStream_t st)
+// ev: optional 4 events recorded before/between/after the three launches (mfh_apply_timed).
+static int apply_impl(mfh_handle h, const void* psi, void* phi, const double* lambdas, cudaStream_t st,
+                      cudaEvent_t* ev = nullptr)
 {
     const Plan& p = h->plan;
     int rc;
+    if (ev) cudaEventRecord(ev[0], st);
     if ((rc = launch_cached(h, psi, st))) return rc;
+    if (ev) cudaEventRecord(ev[1], st);
     if (p.k == 1) {
         if ((rc = launch_proc_single(h, psi, st))) return rc;
     } else if (p.slot_multi >= 0) {
         if ((rc = launch_proc_multi(h, psi, st))) return rc;
     }
-    return launch_reduce(h, psi, phi, lambdas, st);
+    if (ev) cudaEventRecord(ev[2], st);
+    rc = launch_reduce(h, psi, phi, lambdas, st);
+    if (ev) cudaEventRecord(ev[3], st);
+    return rc;
 }
 
 // Algorithm 2: time R_bench applies of a committed plan after R_warm warm-ups.
@@ -301,6 +308,30 @@ MFH_API int mfh_apply(mfh_handle h, const void* psi_dev, void* phi_dev, int32_t 
         return MFH_ERR_INVALID_ARG;
     }
     return apply_impl(h, psi_dev, phi_dev, lambdas_host, (cudaStream_t)stream);
+}
+
+MFH_API int mfh_apply_timed(mfh_handle h, const void* psi_dev, void* phi_dev, int32_t k,
+                            const double* lambdas_host, void* stream, float* ms_out)
+{
+    if (!h || !psi_dev || !phi_dev || psi_dev == phi_dev || !ms_out) {
+        set_error("mfh_apply_timed: NULL or aliased pointer");
+        return MFH_ERR_INVALID_ARG;
+    }
+    if (!h->planned) { set_error("mfh_apply_timed: call mfh_plan first"); return MFH_ERR_BAD_STATE; }
+    if (k != h->plan.k) { set_error("mfh_apply_timed: k mismatch"); return MFH_ERR_INVALID_ARG; }
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaEvent_t ev[4];
+    for (auto& e : ev) MFH_CUDA_CHECK(cudaEventCreate(&e));
+    int rc = apply_impl(h, psi_dev, phi_dev, lambdas_host, st, ev);
+    cudaError_t e = cudaStreamSynchronize(st);
+    if (!rc && e == cudaSuccess) {
+        for (int i = 0; i < 3; ++i) cudaEventElapsedTime(&ms_out[i], ev[i], ev[i + 1]);
+        cudaEventElapsedTime(&ms_out[3], ev[0], ev[3]);
+    }
+    for (auto& x : ev) cudaEventDestroy(x);
+    if (rc) return rc;
+    MFH_CUDA_CHECK(e);
+    return MFH_OK;
 }
 
 MFH_API int mfh_apply_host(mfh_handle h, const void* psi_host, void* phi_host, int32_t k,

@@ -1,0 +1,113 @@
+"""CPU-only checks of the boundary: the C-ABI library loads and exports every symbol that
+include/mfh.h declares, host-side argument checking, and the analytic planner's arithmetic
+against the sizes the paper prints."""
+import os
+import re
+
+import pytest
+
+from paper_2606_31598_b200 import binding as mfh
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "mfh.h")).read()
+    declared = sorted(set(re.findall(r"MFH_API\s+(?:const\s+)?\w+\*?\s+(mfh_\w+)\s*\(", hdr)))
+    assert declared == sorted(mfh.SYMBOLS)
+    L = mfh.lib()
+    for name in declared:
+        assert hasattr(L, name), name
+
+
+def test_product_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_2606_31598_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in src and "from oracle" not in src, f
+                assert "mfh_oracle" not in src, f
+
+
+@pytest.mark.parametrize("D,B", [(100, 32), (4096, 48), (4096, 8192), (16, 16), (4096, 96)])
+def test_create_rejects_bad_sizes(D, B):
+    with pytest.raises(mfh.MfhError) as e:
+        mfh.Hamiltonian(D, B)
+    assert e.value.code == mfh.MFH_ERR_INVALID_ARG
+
+
+def test_create_rejects_bad_enums_and_lambda():
+    import ctypes
+    L = mfh.lib()
+    h = ctypes.c_void_p()
+    assert L.mfh_create(ctypes.byref(h), 4096, 512, 1, 7, 1.0, 0, 0) == mfh.MFH_ERR_INVALID_ARG
+    assert L.mfh_create(ctypes.byref(h), 4096, 512, 1, 0, 1.0, 5, 0) == mfh.MFH_ERR_INVALID_ARG
+    assert L.mfh_create(ctypes.byref(h), 4096, 512, 1, 0, float("nan"), 0, 0) == mfh.MFH_ERR_INVALID_ARG
+    assert L.mfh_create(None, 4096, 512, 1, 0, 1.0, 0, 0) == mfh.MFH_ERR_INVALID_ARG
+    assert L.mfh_destroy(None) == mfh.MFH_OK
+
+
+def test_bad_state_before_plan():
+    h = mfh.Hamiltonian(4096, 512, 1234)
+    with pytest.raises(mfh.MfhError) as e:
+        h.get_plan()
+    assert e.value.code == mfh.MFH_ERR_BAD_STATE
+    import ctypes
+    L = mfh.lib()
+    rc = L.mfh_apply(h._h, ctypes.c_void_p(16), ctypes.c_void_p(32), 1, None, None)
+    assert rc == mfh.MFH_ERR_BAD_STATE
+    assert L.mfh_apply(h._h, None, ctypes.c_void_p(32), 1, None, None) == mfh.MFH_ERR_INVALID_ARG
+    h.destroy()
+
+
+# ---- planner arithmetic (Algorithm 1; Eq. 13-18) --------------------------------------------
+
+def test_planner_memory_model_matches_paper_sizes():
+    # a complex64 dense operator of dimension 2^18 needs 8*(2^18)^2 = 2^39 B (512 GiB);
+    # 65536^2 * 8 = 32 GiB; a 4096^2 complex64 block = 128 MiB.
+    r = mfh.plan_analytic(262144, "c64", 1, "procedural", 4096, 1, 180 * 10**9)
+    assert r["dense_bytes"] == 2**39
+    r = mfh.plan_analytic(65536, "c64", 1, "full", 4096, 1000, 180 * 10**9)
+    ch = r["chosen"]
+    assert ch["mode"] == "full" and ch["cache_bytes"] == 32 * 2**30
+    assert ch["cached_blocks"] == 16 * 16 and ch["cache_bytes"] / ch["cached_blocks"] == 128 * 2**20
+
+
+def test_planner_flops_formula():
+    # Eq. 13: F_mv = 8 n_op D_out D_in R; the paper's 2.749e11 = 2 * 4 * 65536^2 * 8.
+    r = mfh.plan_analytic(65536, "c64", 4, "procedural", 4096, 1, 180 * 10**9)
+    assert r["chosen"]["flops_per_apply"] == pytest.approx(8 * 65536**2 * 4, rel=1e-5)
+    assert 2 * r["chosen"]["flops_per_apply"] == pytest.approx(2.749e11, rel=1e-3)
+
+
+def test_planner_rejects_what_does_not_fit():
+    # C4: the dense matrix is 1.1 TB, full cache can never fit (Eq. 18) -> OUT_OF_MEMORY when forced
+    with pytest.raises(mfh.MfhError) as e:
+        mfh.plan_analytic(262144, "c128", 1, "full", 4096, 10, 180 * 10**9)
+    assert e.value.code == mfh.MFH_ERR_OUT_OF_MEMORY
+    r = mfh.plan_analytic(262144, "c128", 1, "auto", 4096, 10, 180 * 10**9)
+    assert r["chosen"]["feasible"] and r["chosen"]["mode"] in ("procedural", "partial")
+    assert r["chosen"]["total_bytes"] <= 0.9 * 180e9
+
+
+def test_planner_c2_full_cache_size_and_c5_partial_budget():
+    r = mfh.plan_analytic(65536, "c128", 1, "full", 2048, 100, 180 * 10**9)
+    ch = r["chosen"]
+    assert ch["cache_bytes"] == 65536**2 * 16 and ch["cached_blocks"] == 1024   # 68.7 GB, 32x32 blocks
+    # C5: 275 GB total, about 150 GB cached (Eq. 27: P_cache = floor(M_cache / (B_c b^2)), row balanced)
+    r = mfh.plan_analytic(131072, "c128", 1, "partial", 4096, 151, int(150e9 / 0.9))
+    ch = r["chosen"]
+    assert ch["mode"] == "partial" and ch["total_bytes"] <= 150e9
+    assert ch["cached_blocks"] == ch["cached_per_row"] * 32
+    assert ch["cache_bytes"] + 32 * 4096**2 * 16 + ch["work_bytes"] > 150e9 * 0.97   # one more per row would not fit
+
+
+def test_planner_enumerates_block_sizes_and_ranks_feasible_first():
+    r = mfh.plan_analytic(65536, "c128", 1, "auto", 0, 100, 180 * 10**9)
+    Bs = {c["B"] for c in r["candidates"]}
+    assert {4096, 2048, 1024, 512} <= Bs
+    flags = [c["feasible"] for c in r["candidates"]]
+    assert flags == sorted(flags, reverse=True)
+    feas = [c["model_job_s"] for c in r["candidates"] if c["feasible"]]
+    assert feas == sorted(feas)

@@ -1,0 +1,223 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element on the
+same seeded inputs.  Tolerances (BASELINE.json north_star): Philox words bit-exact; relative L2
+||phi_gpu - phi_cpu|| / ||phi_cpu|| <= 1e-11 for complex128, <= 1e-4 for complex64 (per column).
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2606_31598_b200 import binding as mfh
+from paper_2606_31598_b200.inputs import CONFIGS, lambda_grid, make_psi
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"c128": 1e-11, "c64": 1e-4}
+
+
+def rel_l2(a, b):
+    a = np.asarray(a, dtype=np.complex128)
+    b = np.asarray(b, dtype=np.complex128)
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+def to_dev(x):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def gpu_apply(D, B, seed, psi, dtype="c128", mode="procedural", k=1, budget=0, **kw):
+    h = mfh.Hamiltonian(D, B, seed, dtype, **kw)
+    plan = h.plan(mode, k=k, hbm_budget_bytes=budget)
+    phi = h.apply(to_dev(psi)).cpu().numpy()
+    return phi, plan, h
+
+
+# ---- generator ------------------------------------------------------------------------------
+
+def _philox_gpu(seed, stream, i, j):
+    import torch
+    w = mfh.debug_philox(seed, stream, to_dev(i.astype(np.uint32).view(np.int32)),
+                         to_dev(j.astype(np.uint32).view(np.int32)))
+    torch.cuda.synchronize()
+    return w.cpu().numpy().view(np.uint32)
+
+
+def test_philox_words_bit_exact_block00_of_c1():
+    a = np.arange(512, dtype=np.uint32)
+    i, j = [x.ravel() for x in np.meshgrid(a, a, indexing="ij")]
+    assert np.array_equal(_philox_gpu(1234, 0, i, j), oracle.philox_pairs(1234, 0, i, j))
+
+
+def test_philox_words_bit_exact_random_pairs_and_corners():
+    rng = np.random.default_rng(5)
+    i = rng.integers(0, 262144, size=1_000_000).astype(np.uint32)
+    j = rng.integers(0, 262144, size=1_000_000).astype(np.uint32)
+    D = 262144
+    i[:4] = [0, 0, D - 1, D - 1]
+    j[:4] = [0, D - 1, 0, D - 1]
+    for seed, stream in [(1234, 0), (7, 1), (2**40 + 3, 0)]:
+        assert np.array_equal(_philox_gpu(seed, stream, i, j), oracle.philox_pairs(seed, stream, i, j))
+
+
+def test_philox_empty_input():
+    import torch
+    e = torch.empty(0, dtype=torch.int32, device="cuda")
+    assert mfh.debug_philox(1, 0, e, e).shape == (0, 4)
+
+
+@pytest.mark.parametrize("dtype,tol", [("c128", 2e-14), ("c64", 3e-6)])
+@pytest.mark.parametrize("n,m", [(0, 0), (0, 3), (3, 0), (7, 7)])
+def test_materialized_block_matches_oracle_entries(dtype, tol, n, m):
+    D, B = 4096, 512
+    h = mfh.Hamiltonian(D, B, 1234, dtype)
+    blk = h.materialize_block(n, m, B).cpu().numpy().astype(np.complex128)
+    ref = oracle.materialize(D, 1234, n * B, B, m * B, B)
+    # entries are O(1/sqrt(D)); absolute error relative to that scale
+    assert np.abs(blk - ref).max() * np.sqrt(D) < tol * 50
+    assert rel_l2(blk, ref) < tol
+    if n == m:
+        assert np.all(blk.imag.diagonal() == 0.0)
+        assert np.array_equal(blk, blk.conj().T)          # bit-exact Hermiticity
+
+
+def test_h0_diagonal_matches_oracle():
+    h = mfh.Hamiltonian(32768, 1024, 8, "c128", kind="diag_plus_gue", seed_h0=7)
+    assert np.array_equal(h.h0().cpu().numpy(), oracle.h0_diagonal(32768, 7))
+
+
+# ---- C1: procedural apply vs oracle and vs explicit dense matmul ----------------------------
+
+def test_c1_procedural_vs_oracle_and_dense():
+    c = CONFIGS["C1"]
+    psi = make_psi(c["D"], c["psi_seed"])
+    phi, plan, h = gpu_apply(c["D"], c["B"], c["seed"], psi)
+    assert plan["chosen"]["mode"] == "procedural"
+    ref = oracle.apply(c["D"], c["B"], c["seed"], psi)
+    assert rel_l2(phi, ref) <= TOL["c128"]
+    H = oracle.materialize(c["D"], c["seed"])
+    assert rel_l2(phi, H @ psi) <= TOL["c128"]
+
+
+@pytest.mark.parametrize("mode,budget", [("procedural", 0), ("full", 0), ("partial", 12e6),
+                                         ("partial", 30e6), ("partial", 60e6)])
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+def test_modes_agree_with_oracle(mode, budget, dtype):
+    D, B = 2048, 256          # 8x8 blocks of 1 MiB (c128): budgets cache ~1..6 blocks per row
+    psi = make_psi(D, 3, dtype=dtype)
+    if dtype == "c64":
+        budget = budget / 2
+    phi, plan, h = gpu_apply(D, B, 42, psi, dtype=dtype, mode=mode, budget=int(budget))
+    assert plan["chosen"]["mode"] == mode
+    ref = oracle.apply(D, B, 42, psi)
+    assert rel_l2(phi, ref) <= TOL[dtype]
+
+
+@pytest.mark.parametrize("D,B", [(32, 32), (96, 32), (160, 32), (1024, 1024), (4096, 4096), (3072, 1024),
+                                 (2048, 64), (4096, 128), (1536, 512), (8192, 2048)])
+def test_partition_invariance_and_ragged_shapes(D, B):
+    # the operator must not depend on the partition
+    psi = make_psi(D, 17)
+    phi, _, _ = gpu_apply(D, B, 1234, psi)
+    ref = oracle.apply(D, B, 1234, psi)
+    assert rel_l2(phi, ref) <= TOL["c128"]
+
+
+def test_apply_is_deterministic_and_repeatable():
+    import torch
+    D, B = 4096, 512
+    psi = to_dev(make_psi(D, 1))
+    for mode, budget in [("procedural", 0), ("partial", int(150e6))]:
+        h = mfh.Hamiltonian(D, B, 9, "c128")
+        h.plan(mode, hbm_budget_bytes=budget)
+        a = h.apply(psi).clone()
+        for _ in range(3):
+            b = h.apply(psi)
+            assert torch.equal(a, b)                      # no atomics in the complex128 path
+
+
+def test_hermiticity_on_gpu():
+    D, B = 4096, 512
+    a, b = make_psi(D, 1), make_psi(D, 2)
+    h = mfh.Hamiltonian(D, B, 77, "c128")
+    h.plan("procedural")
+    Ha = h.apply(to_dev(a)).cpu().numpy()
+    Hb = h.apply(to_dev(b)).cpu().numpy()
+    assert abs(np.vdot(a, Hb) - np.conj(np.vdot(b, Ha))) < 1e-13
+
+
+def test_lambda_scales_single_vector():
+    D, B = 1024, 256
+    psi = make_psi(D, 4)
+    phi, _, _ = gpu_apply(D, B, 5, psi, lam=0.37)
+    assert rel_l2(phi, 0.37 * oracle.apply(D, B, 5, psi)) <= TOL["c128"]
+
+
+# ---- multi-vector / coupling scan (C3 shape) -------------------------------------------------
+
+@pytest.mark.parametrize("dtype,k", [("c64", 16), ("c64", 5), ("c128", 4), ("c128", 16), ("c64", 2)])
+def test_scan_multi_vector_vs_oracle(dtype, k):
+    D, B = 2048, 256
+    Psi = make_psi(D, 9, k=k, dtype=dtype)
+    lam = lambda_grid(k)
+    h = mfh.Hamiltonian(D, B, 8, dtype, kind="diag_plus_gue", seed_h0=7)
+    h.plan("procedural", k=k)
+    Phi = h.apply(to_dev(Psi), lambdas=lam).cpu().numpy()
+    ref = oracle.apply_scan(D, B, 8, 7, lam, Psi)
+    for v in range(k):
+        assert rel_l2(Phi[:, v], ref[:, v]) <= TOL[dtype], v
+    # lambda_0 = 0: column 0 is the textbook special case h0 (.) psi_0
+    h0 = oracle.h0_diagonal(D, 7)
+    assert rel_l2(Phi[:, 0], h0 * Psi[:, 0].astype(np.complex128)) <= (1e-15 if dtype == "c128" else 2e-7)
+
+
+def test_multi_vector_equals_single_vector_applies():
+    D, B, k = 1024, 256, 4
+    Psi = make_psi(D, 21, k=k)
+    h = mfh.Hamiltonian(D, B, 8, "c128")
+    h.plan("procedural", k=k)
+    Phi = h.apply(to_dev(Psi)).cpu().numpy()
+    h1 = mfh.Hamiltonian(D, B, 8, "c128")
+    h1.plan("procedural", k=1)
+    for v in range(k):
+        one = h1.apply(to_dev(Psi[:, v].copy())).cpu().numpy()
+        assert rel_l2(Phi[:, v], one) <= 1e-13
+
+
+# ---- planner on the device -------------------------------------------------------------------
+
+def test_measured_planner_commits_a_working_plan():
+    D = 4096
+    psi = make_psi(D, 2)
+    h = mfh.Hamiltonian(D, 0, 1234, "c128")
+    rec = h.plan("auto", n_applies_hint=50, measure=True)
+    assert rec["planner"] == "measured" and rec["chosen"]["measured_apply_s"] > 0
+    timed = [c for c in rec["candidates"] if c["measured_apply_s"] > 0]
+    assert 1 <= len(timed) <= 8                            # K_bench <= 8
+    B = h.get_plan()["B"]
+    assert rel_l2(h.apply(to_dev(psi)).cpu().numpy(), oracle.apply(D, B, 1234, psi)) <= TOL["c128"]
+
+
+def test_plan_k_mismatch_and_replan():
+    import torch
+    D = 1024
+    h = mfh.Hamiltonian(D, 256, 1, "c128")
+    h.plan("procedural", k=2)
+    h.k = 1
+    with pytest.raises(mfh.MfhError) as e:
+        h.apply(torch.zeros(D, dtype=torch.complex128, device="cuda"))
+    assert e.value.code == mfh.MFH_ERR_INVALID_ARG
+    h.plan("full", k=1)                                   # re-plan is allowed
+    psi = make_psi(D, 2)
+    assert rel_l2(h.apply(to_dev(psi)).cpu().numpy(), oracle.apply(D, 256, 1, psi)) <= TOL["c128"]
+
+
+def test_apply_host_roundtrip():
+    import torch
+    D, B = 2048, 256
+    psi = make_psi(D, 6)
+    h = mfh.Hamiltonian(D, B, 3, "c128")
+    h.plan("procedural")
+    ph = torch.from_numpy(psi).pin_memory()
+    out = torch.empty_like(ph).pin_memory()
+    h.apply_host(ph, out)
+    assert rel_l2(out.numpy(), oracle.apply(D, B, 3, psi)) <= TOL["c128"]
