@@ -47,6 +47,19 @@ static int free_plan_resources(mfh_handle h)
     return MFH_OK;
 }
 
+int ensure_gen_table(mfh_handle h, cudaStream_t st)
+{
+    if (h->gen_ready) return MFH_OK;
+    make_gen_table(h->D, h->gen_host);
+    if (h->dtype == MFH_C128) {
+        if (!h->d_gen_tab) MFH_CUDA_CHECK(cudaMalloc(&h->d_gen_tab, sizeof(GenTabD)));
+        MFH_CUDA_CHECK(cudaMemcpyAsync(h->d_gen_tab, &h->gen_host.tab, sizeof(GenTabD), cudaMemcpyHostToDevice, st));
+        MFH_CUDA_CHECK(cudaStreamSynchronize(st));   // gen_host is pageable: make the copy complete
+    }
+    h->gen_ready = true;
+    return MFH_OK;
+}
+
 // Allocate and upload everything plan `p` needs, then fill the cache.
 static int commit_plan(mfh_handle h, const Plan& p, cudaStream_t st)
 {
@@ -89,7 +102,9 @@ static int commit_plan(mfh_handle h, const Plan& p, cudaStream_t st)
         int rc = launch_h0(h, h->d_h0, st);
         if (rc) return rc;
     }
-    int rc = launch_fill_cache(h, st);
+    int rc = ensure_gen_table(h, st);
+    if (rc) return rc;
+    rc = launch_fill_cache(h, st);
     if (rc) return rc;
     MFH_CUDA_CHECK(cudaStreamSynchronize(st));
     h->planned = true;
@@ -191,6 +206,7 @@ MFH_API int mfh_destroy(mfh_handle h)
 {
     if (!h) return MFH_OK;
     free_plan_resources(h);
+    if (h->d_gen_tab) cudaFree(h->d_gen_tab);
     delete h;
     return MFH_OK;
 }
@@ -286,10 +302,10 @@ MFH_API int mfh_get_plan(mfh_handle h, char* json_out, size_t json_cap)
     snprintf(buf, sizeof buf,
              "{\"mode\":\"%s\",\"B\":%d,\"n_blk\":%d,\"k\":%d,\"cached_blocks\":%lld,\"cached_per_row\":%d,"
              "\"cache_bytes\":%zu,\"work_bytes\":%zu,\"partial_slots\":%d,\"proc_items\":%zu,"
-             "\"proc_warps\":%d,\"proc_row_strips\":%d,\"launches_per_apply\":%d}",
+             "\"proc_rows_per_lane\":%d,\"proc_row_strips\":%d,\"launches_per_apply\":%d}",
              p.mode == MFH_MODE_FULL ? "full" : (p.mode == MFH_MODE_PARTIAL ? "partial" : "procedural"), p.B,
              p.n_blk, p.k, (long long)p.n_cached, p.cached_per_row, p.cache_bytes, p.work_bytes, p.n_slots,
-             p.items.size(), p.warps, p.Q,
+             p.items.size(), p.R, p.Q,
              1 + (p.n_cached > 0) + ((p.k == 1 && !p.items.empty()) || p.slot_multi >= 0));
     copy_json(buf, json_out, json_cap);
     return MFH_OK;

@@ -4,6 +4,11 @@
 // (BASELINE.json configs[0]; partition invariance P:68-70: global indices only).
 // Used by the fused generate-and-apply kernels, the cache fill and the debug exports, so the
 // cached and the procedural path apply bit-identical matrices.
+//
+// The Box-Muller transcendentals are this file's own: the
+// fused c128 kernel is bound by issue slots and the FP64 pipe, and libdevice's 1-ulp log / sqrt /
+// sincospi cost ~210 instructions per entry; the table-driven forms below cost ~50 and keep the
+// absolute error of an entry below 1e-13 of its scale (tolerance of phi: 1e-11 relative L2).
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -31,7 +36,7 @@ inline PhiloxKeys make_philox_keys(uint64_t seed)
 }
 
 // Full 4-word output.  In the fused kernels only x0,x1 are consumed and the compiler removes the
-// dead half of the last two rounds.
+// dead half of the last two rounds (and folds the zero counter words of the first round).
 __device__ __forceinline__ void philox4x32_10(const PhiloxKeys& K, uint32_t c0, uint32_t c1,
                                               uint32_t c2, uint32_t c3, uint32_t& x0, uint32_t& x1,
                                               uint32_t& x2, uint32_t& x3)
@@ -57,71 +62,145 @@ __device__ __forceinline__ void pair_words(const PhiloxKeys& K, uint32_t lo, uin
     philox4x32_10(K, lo, hi, 0u, 0u, x0, x1, x2, x3);
 }
 
-// ---- Box-Muller normals scaled by s:  (s*g1, s*g2),  g1 + i g2 = sqrt(-2 ln u1) e^{2 pi i u2},
-//      u = (x + 1/2) 2^-32  (readings R2, R3). --------------------------------------
+// ---- Box-Muller normals scaled by s = 1/sqrt(2D):  (s g1, s g2),
+//      g1 + i g2 = sqrt(-2 ln u1) e^{2 pi i u2},  u = (x + 1/2) 2^-32   (R2, R3). ------
+//
+// complex128.  With d = x0 + 1/2 = 2^e m (m in [1,2)), c the centre of m's bin among 256 and
+// r = m/c - 1 (|r| <= 2^-9):
+//     L = s^2 (-2 ln u1) = K2 [(32 - e) ln 2 - ln c] - K2 log1p(r),      K2 = 2 s^2 = 1/D,
+// a 256-entry table of (1/c, -K2 ln c), a 33-entry table of K2 (32-e) ln 2 and a degree-4
+// polynomial for log1p (remainder r^5/5 <= 6e-15).  sqrt(L) = L y (1 + e'), y = rsqrt.approx(L)
+// (2^-22), one Newton step (1.5 * 2^-44 = 9e-14 relative).  The angle 2 pi u2 is split into a
+// 1024-entry table of (cos A, sin A) at the bin centres and a residual |b| <= pi/1024:
+// sin b = b - b^3/6 (2e-15), cos b = 1 - b^2/2 + b^4/24 (1e-18), combined by angle addition.
+constexpr int GEN_LOG_BITS = 8;
+constexpr int GEN_SC_BITS = 10;
+
+struct GenTabD {                         // built on the host by make_gen_table(), copied to shared memory
+    double2 tlog[1 << GEN_LOG_BITS];     // (1/c, -K2 ln c)
+    double2 tsc[1 << GEN_SC_BITS];       // (cos A, sin A),  A = 2 pi (idx 2^22 + 2^21 + 1/2) 2^-32
+    double elog[34];                     // K2 (32 - e) ln 2 for e = -1..31  (index e + 1)
+};
+
+struct GenConstD {                       // kernel-parameter constants (constant bank operands)
+    double c1, c2, c3, c4;               // -K2 log1p(r) = r (c1 + r (c2 + r (c3 + r c4)))
+    double ang;                          // 2 pi 2^-32
+};
+
+struct GenHostD {
+    GenTabD tab;
+    GenConstD gc;
+};
+
+void make_gen_table(int64_t D, GenHostD& out);   // mfh_plan.cu (host)
 
 template <typename T> struct Gen;
 
 template <> struct Gen<double> {
-    __device__ __forceinline__ static void normals(uint32_t x0, uint32_t x1, double s, double& a,
-                                                   double& b)
+    using Tab = GenTabD;
+    using Const = GenConstD;
+    static constexpr int TAB_BYTES = (int)sizeof(GenTabD);
+
+    __device__ __forceinline__ static void normals(const GenTabD* __restrict__ tab, const GenConstD& gc,
+                                                   uint32_t x0, uint32_t x1, double& a, double& b)
     {
-        // 2^52 + x as a double by bit pattern, then one exact FMA: (x + 1/2) 2^-32.
-        const double d0 = __hiloint2double(0x43300000, (int)x0);
-        const double d1 = __hiloint2double(0x43300000, (int)x1);
-        const double u1 = fma(d0, 0x1p-32, -(0x1p52 - 0.5) * 0x1p-32);
-        const double two_u2 = fma(d1, 0x1p-31, -(0x1p52 - 0.5) * 0x1p-31);
-        const double r = s * sqrt(-2.0 * log(u1));
-        double sn, cs;
-        sincospi(two_u2, &sn, &cs);
-        a = r * cs;
-        b = r * sn;
+        // radius: d = x0 + 1/2 exactly (2^52 + x0 by bit pattern, minus 2^52 - 1/2)
+        const double d = __hiloint2double(0x43300000, (int)x0) - 0x1.fffffffffffffp51;
+        const int hi = __double2hiint(d);
+        const double m = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, __double2loint(d));
+        const double2 tl = tab->tlog[(hi >> (20 - GEN_LOG_BITS)) & ((1 << GEN_LOG_BITS) - 1)];
+        const double el = tab->elog[(hi >> 20) - 1022];
+        const double r = fma(m, tl.x, -1.0);
+        double p = fma(r, gc.c4, gc.c3);
+        p = fma(r, p, gc.c2);
+        p = fma(r, p, gc.c1);
+        const double L = fma(r, p, tl.y + el);
+        double y;
+        asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(L));
+        const double sq = L * y, hy = 0.5 * y;
+        const double e = fma(-sq, hy, 0.5);
+        const double rad = fma(sq, e, sq);
+        // angle
+        const double2 cs = tab->tsc[x1 >> (32 - GEN_SC_BITS)];
+        const int resid = (int)(x1 & ((1u << (32 - GEN_SC_BITS)) - 1u)) - (1 << (31 - GEN_SC_BITS));
+        const double bb = (double)resid * gc.ang;
+        const double b2 = bb * bb;
+        const double sb = fma(b2 * (-1.0 / 6.0), bb, bb);
+        const double q = fma(b2, 1.0 / 24.0, -0.5) * b2;
+        const double rc = rad * cs.x, rs = rad * cs.y;
+        a = fma(-rs, sb, fma(rc, q, rc));
+        b = fma(rc, sb, fma(rs, q, rs));
     }
+};
+
+// complex64: SFU forms (lg2 / sqrt / sin / cos .approx, absolute error <= 5e-7 per normal;
+// tolerance of phi: 1e-4).  u1 is rounded to float (may round to 1 -> radius 0; R6);
+// the angle is taken as a signed turn fraction in [-1/2, 1/2) so the SFU argument stays in [-pi, pi).
+struct GenTabF {
+    float unused;
+};
+struct GenConstF {
+    float neg_k2_ln2;   // -K2 ln 2:  L = K2 (-ln u1) = neg_k2_ln2 * log2(u1)
 };
 
 template <> struct Gen<float> {
-    __device__ __forceinline__ static void normals(uint32_t x0, uint32_t x1, float s, float& a,
-                                                   float& b)
+    using Tab = GenTabF;
+    using Const = GenConstF;
+    static constexpr int TAB_BYTES = 0;
+
+    __device__ __forceinline__ static void normals(const GenTabF*, const GenConstF& gc, uint32_t x0,
+                                                   uint32_t x1, float& a, float& b)
     {
-        // u1 rounded to float (may round to 1 -> r = 0; error <= 6e-8, R6).
         const float u1 = fmaf((float)x0, 0x1p-32f, 0x1p-33f);
-        // angle as a signed turn fraction in [-1/2, 1/2): same angle mod 1, full float precision
-        const float two_u2 = fmaf((float)(int32_t)x1, 0x1p-31f, 0x1p-32f);
-        const float r = s * sqrtf(-2.0f * logf(u1));
-        float sn, cs;
-        sincospif(two_u2, &sn, &cs);
-        a = r * cs;
-        b = r * sn;
+        const float L = gc.neg_k2_ln2 * __log2f(u1);
+        float rad;
+        asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(rad) : "f"(L));
+        const float ang = fmaf((float)(int32_t)x1, 0x1.921fb6p-30f, 0x1.921fb6p-31f);   // 2 pi (x1 + 1/2) 2^-32
+        a = rad * __cosf(ang);
+        b = rad * __sinf(ang);
     }
 };
 
-// Scales of the entry rule: off-diagonal 1/sqrt(2D), diagonal 1/sqrt(D).
-template <typename T> struct Scales {
-    T off;
-    T diag;
+template <typename T> struct GenArgs {   // what a kernel needs to call the generator
+    PhiloxKeys K;
+    typename Gen<T>::Const gc;
+    const typename Gen<T>::Tab* tab_global;   // device copy of the table (nullptr for float)
 };
 
-// General entry H_ij for any (i,j): conjugate below the diagonal, real on it.
+// Copy the generator table to shared memory (all threads of the CTA; caller synchronises).
 template <typename T>
-__device__ __forceinline__ void entry_any(const PhiloxKeys& K, const Scales<T>& S, uint32_t i,
+__device__ __forceinline__ const typename Gen<T>::Tab* stage_gen_table(const GenArgs<T>& G, void* smem)
+{
+    if constexpr (Gen<T>::TAB_BYTES > 0) {
+        const uint4* src = reinterpret_cast<const uint4*>(G.tab_global);
+        uint4* dst = reinterpret_cast<uint4*>(smem);
+        for (int t = threadIdx.x; t < Gen<T>::TAB_BYTES / 16; t += blockDim.x) dst[t] = src[t];
+    }
+    return reinterpret_cast<const typename Gen<T>::Tab*>(smem);
+}
+
+// General entry H_ij for any (i,j): conjugate below the diagonal, real and scaled by 1/sqrt(D)
+// (= sqrt(2) s) on it.
+template <typename T>
+__device__ __forceinline__ void entry_any(const GenArgs<T>& G, const typename Gen<T>::Tab* tab, uint32_t i,
                                           uint32_t j, T& hr, T& hi)
 {
     uint32_t x0, x1;
-    pair_words(K, min(i, j), max(i, j), x0, x1);
+    pair_words(G.K, min(i, j), max(i, j), x0, x1);
     T a, b;
-    Gen<T>::normals(x0, x1, (i == j) ? S.diag : S.off, a, b);
-    hr = a;
+    Gen<T>::normals(tab, G.gc, x0, x1, a, b);
+    hr = (i == j) ? a * T(1.4142135623730951) : a;
     hi = (i < j) ? b : ((i > j) ? -b : T(0));
 }
 
 // Entry for a pair known to satisfy i < j (strictly upper triangle).
 template <typename T>
-__device__ __forceinline__ void entry_upper(const PhiloxKeys& K, const Scales<T>& S, uint32_t i,
+__device__ __forceinline__ void entry_upper(const GenArgs<T>& G, const typename Gen<T>::Tab* tab, uint32_t i,
                                             uint32_t j, T& hr, T& hi)
 {
     uint32_t x0, x1;
-    pair_words(K, i, j, x0, x1);
-    Gen<T>::normals(x0, x1, S.off, hr, hi);
+    pair_words(G.K, i, j, x0, x1);
+    Gen<T>::normals(tab, G.gc, x0, x1, hr, hi);
 }
 
 }  // namespace mfh

@@ -37,7 +37,7 @@ struct Plan {
     int32_t mode = 0;          // MFH_MODE_* actually committed
     int32_t B = 0, n_blk = 0, k = 0;
     int32_t Q = 1;             // row strips per block in the procedural kernel
-    int32_t warps = 8;         // warps per CTA of the procedural kernel (macro tile = 32*warps)
+    int32_t R = 4;             // rows per lane in the procedural kernel (row tile = 32*R rows)
     int64_t n_cached = 0;      // cached blocks
     int32_t cached_per_row = 0;
     int32_t n_slots = 0;       // partial vectors in the workspace
@@ -71,6 +71,9 @@ struct mfh_handle_s {
     int32_t* d_counter = nullptr;   // dynamic work counter of the procedural kernel
     void* d_cheb = nullptr;         // 3 vectors of Chebyshev scratch
     void* d_io = nullptr;           // psi/phi staging of mfh_apply_host
+    mfh::GenHostD gen_host;         // generator table + constants for this D (host copy)
+    mfh::GenTabD* d_gen_tab = nullptr;   // device copy (c128 only), kept until mfh_destroy
+    bool gen_ready = false;
     int sm_count = 148;
 };
 
@@ -88,6 +91,8 @@ size_t complex_bytes(int dtype);
             return MFH_ERR_CUDA;                                                               \
         }                                                                                      \
     } while (0)
+
+int ensure_gen_table(mfh_handle h, cudaStream_t st);   // mfh_api.cu: build + upload once per handle
 
 // ---- launchers (mfh_proc.cu, mfh_cached.cu, mfh_vec.cu) ----
 int launch_philox_debug(uint64_t seed, uint32_t stream_id, const uint32_t* i, const uint32_t* j,

@@ -65,21 +65,47 @@ static std::vector<int> band_offsets(int N)
     return out;
 }
 
-void choose_tiling(int B, int n_pairs, int sm_count, int& warps, int& Q)
+// Rows per lane R (row tile = 32 R rows) and row strips per block Q of the fused kernel.
+// Prefer R = 4 (one psi_j load and one shuffle pair per 4 generated entries); go lower only when
+// the block is too small or there would not be one item per resident CTA.  Q grows until there
+// are ~24 items per SM (tail of the dynamic schedule below ~2 %) while the column-side partial
+// slots (N_blk * Q vectors) stay small.
+void choose_tiling(int B, int n_blk, int n_pairs, int sm_count, int& R, int& Q)
 {
-    const int cands[4] = {8, 4, 2, 1};
-    warps = 1;
-    Q = 1;
-    for (int W : cands) {
-        if (B % (32 * W) != 0) continue;
-        const int qmax = B / (32 * W);
-        int q = 1;
-        while (q < qmax && (int64_t)n_pairs * q < 4LL * sm_count) q *= 2;
-        warps = W;
-        Q = q;
-        if ((int64_t)n_pairs * q >= 2LL * sm_count) return;   // enough items for every SM
+    R = 1;
+    for (int r : {4, 2, 1}) {
+        if (B % (32 * r) != 0) continue;
+        R = r;
+        if ((int64_t)n_pairs * (B / (32 * r)) >= 2LL * sm_count) break;
     }
-    // nothing reached 2 items per SM: keep the smallest valid W (most items)
+    const int qmax = B / (32 * R);
+    Q = 1;
+    while (Q * 2 <= qmax && (int64_t)n_pairs * Q < 48LL * sm_count && (int64_t)n_blk * Q * 2 <= 512) Q *= 2;
+}
+
+// Generator table of mfh_gen.cuh for dimension D (host arithmetic in long double).
+void make_gen_table(int64_t D, GenHostD& out)
+{
+    const long double K2 = 1.0L / (long double)D;             // 2 s^2, s = 1/sqrt(2D)
+    const long double LN2 = 0.693147180559945309417232121458L;
+    const long double PI = 3.141592653589793238462643383280L;
+    const int NL = 1 << GEN_LOG_BITS, NS = 1 << GEN_SC_BITS;
+    for (int i = 0; i < NL; ++i) {
+        const double inv = (double)(1.0L / (1.0L + ((long double)i + 0.5L) / NL));   // 1/c, then c := 1/inv exactly
+        out.tab.tlog[i].x = inv;
+        out.tab.tlog[i].y = (double)(K2 * logl((long double)inv));                   // -K2 ln c
+    }
+    for (int i = 0; i < NS; ++i) {
+        const long double A = 2.0L * PI * (((long double)i + 0.5L) * 4194304.0L * (1024.0L / NS) + 0.5L) / 4294967296.0L;
+        out.tab.tsc[i].x = (double)cosl(A);
+        out.tab.tsc[i].y = (double)sinl(A);
+    }
+    for (int idx = 0; idx < 34; ++idx) out.tab.elog[idx] = (double)(K2 * (long double)(33 - idx) * LN2);
+    out.gc.c1 = (double)(-K2);
+    out.gc.c2 = (double)(K2 / 2.0L);
+    out.gc.c3 = (double)(-K2 / 3.0L);
+    out.gc.c4 = (double)(K2 / 4.0L);
+    out.gc.ang = (double)(2.0L * PI / 4294967296.0L);
 }
 
 void build_tables(Plan& p, int64_t D, int dtype, int sm_count)
@@ -112,7 +138,7 @@ void build_tables(Plan& p, int64_t D, int dtype, int sm_count)
             any_col |= (kd == PAIR_TWO_SIDED || kd == PAIR_DIAG);
         }
     }
-    choose_tiling(p.B, std::max(n_pairs, 1), sm_count, p.warps, p.Q);
+    choose_tiling(p.B, N, std::max(n_pairs, 1), sm_count, p.R, p.Q);
 
     // partial-sum slots
     int s = 0;
@@ -194,7 +220,7 @@ Candidate evaluate_candidate(int64_t D, int dtype, int k, int B, int cached_per_
         double gens = 0.0;
         for (uint8_t kd : p.pair_kind) {
             if (kd == PAIR_TWO_SIDED || kd == PAIR_ONE_SIDED) gens += (double)B * B;
-            else if (kd == PAIR_DIAG) gens += 0.5 * (double)B * (B + 32.0 * p.warps);
+            else if (kd == PAIR_DIAG) gens += 0.5 * (double)B * (B + 32.0 * p.R) + 0.5 * 32.0 * p.R * B;
         }
         double t = gens / gen_pairs_per_s(dtype);
         if (!p.items.empty()) {   // tail effect of whole-item scheduling

@@ -19,7 +19,7 @@ struct Candidate {
     bool feasible = false;                               // Eq. 18
 };
 
-void choose_tiling(int B, int n_pairs, int sm_count, int& warps, int& Q);
+void choose_tiling(int B, int n_blk, int n_pairs, int sm_count, int& R, int& Q);
 void build_tables(Plan& p, int64_t D, int dtype, int sm_count);
 Candidate evaluate_candidate(int64_t D, int dtype, int k, int B, int cached_per_row, int64_t n_applies,
                              int sm_count);

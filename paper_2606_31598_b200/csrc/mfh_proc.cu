@@ -6,12 +6,22 @@
 
 namespace mfh {
 
-template <typename T> static Scales<T> make_scales(int64_t D)
+template <typename T> static GenArgs<T> make_gen_args(mfh_handle h);
+template <> GenArgs<double> make_gen_args<double>(mfh_handle h)
 {
-    Scales<T> s;
-    s.off = (T)(1.0 / sqrt(2.0 * (double)D));
-    s.diag = (T)(1.0 / sqrt((double)D));
-    return s;
+    GenArgs<double> G;
+    G.K = make_philox_keys(h->seed);
+    G.gc = h->gen_host.gc;
+    G.tab_global = h->d_gen_tab;
+    return G;
+}
+template <> GenArgs<float> make_gen_args<float>(mfh_handle h)
+{
+    GenArgs<float> G;
+    G.K = make_philox_keys(h->seed);
+    G.gc.neg_k2_ln2 = (float)(-0.6931471805599453 / (double)h->D);
+    G.tab_global = nullptr;
+    return G;
 }
 
 // --------------------------------------------------------------------------------------------
@@ -46,12 +56,13 @@ int launch_philox_debug(uint64_t seed, uint32_t stream_id, const uint32_t* i, co
 // rows strided over blockIdx.y, columns over the threads (coalesced 16-byte stores).
 // --------------------------------------------------------------------------------------------
 template <typename T>
-__global__ void __launch_bounds__(256) fill_kernel(PhiloxKeys K, Scales<T> S, int32_t B, int32_t n_blk,
+__global__ void __launch_bounds__(256) fill_kernel(const GenArgs<T> G, int32_t B, int32_t n_blk,
                                                    const int32_t* __restrict__ cache_slot,
                                                    int32_t single_n, int32_t single_m,
                                                    typename Cplx<T>::type* __restrict__ out)
 {
     using CT = typename Cplx<T>::type;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
     int32_t n, m;
     size_t base;
     if (cache_slot) {
@@ -65,12 +76,14 @@ __global__ void __launch_bounds__(256) fill_kernel(PhiloxKeys K, Scales<T> S, in
         m = single_m;
         base = 0;
     }
+    const typename Gen<T>::Tab* tab = stage_gen_table<T>(G, smem_raw);
+    __syncthreads();
     for (int32_t a = blockIdx.y; a < B; a += gridDim.y) {
         const uint32_t i = (uint32_t)n * B + a;
         CT* row = out + base + (size_t)a * B;
         for (int32_t b = threadIdx.x; b < B; b += blockDim.x) {
             T hr, hi;
-            entry_any<T>(K, S, i, (uint32_t)m * B + b, hr, hi);
+            entry_any<T>(G, tab, i, (uint32_t)m * B + b, hr, hi);
             CT v;
             v.x = hr;
             v.y = hi;
@@ -79,34 +92,36 @@ __global__ void __launch_bounds__(256) fill_kernel(PhiloxKeys K, Scales<T> S, in
     }
 }
 
-int launch_fill_block(mfh_handle h, int32_t B, int32_t n, int32_t m, void* out, cudaStream_t st)
+template <typename T>
+static int launch_fill_t(mfh_handle h, dim3 grid, int32_t B, int32_t n_blk, const int32_t* cache_slot,
+                         int32_t n, int32_t m, void* out, cudaStream_t st)
 {
-    const PhiloxKeys K = make_philox_keys(h->seed);
-    dim3 grid(1, std::min(B, 1024));
-    if (h->dtype == MFH_C128)
-        fill_kernel<double><<<grid, 256, 0, st>>>(K, make_scales<double>(h->D), B, 0, nullptr, n, m,
-                                                   (double2*)out);
-    else
-        fill_kernel<float><<<grid, 256, 0, st>>>(K, make_scales<float>(h->D), B, 0, nullptr, n, m,
-                                                  (float2*)out);
+    using CT = typename Cplx<T>::type;
+    fill_kernel<T><<<grid, 256, Gen<T>::TAB_BYTES, st>>>(make_gen_args<T>(h), B, n_blk, cache_slot, n, m,
+                                                          (CT*)out);
     MFH_CUDA_CHECK(cudaGetLastError());
     return MFH_OK;
+}
+
+int launch_fill_block(mfh_handle h, int32_t B, int32_t n, int32_t m, void* out, cudaStream_t st)
+{
+    int rc = ensure_gen_table(h, st);
+    if (rc) return rc;
+    dim3 grid(1, std::min(B, 1024));
+    return h->dtype == MFH_C128 ? launch_fill_t<double>(h, grid, B, 0, nullptr, n, m, out, st)
+                                : launch_fill_t<float>(h, grid, B, 0, nullptr, n, m, out, st);
 }
 
 int launch_fill_cache(mfh_handle h, cudaStream_t st)
 {
     const Plan& p = h->plan;
     if (p.n_cached == 0) return MFH_OK;
-    const PhiloxKeys K = make_philox_keys(h->seed);
+    int rc = ensure_gen_table(h, st);
+    if (rc) return rc;
     dim3 grid(p.n_blk * p.n_blk, std::min(p.B, 64));
-    if (h->dtype == MFH_C128)
-        fill_kernel<double><<<grid, 256, 0, st>>>(K, make_scales<double>(h->D), p.B, p.n_blk,
-                                                   h->d_cache_slot, 0, 0, (double2*)h->d_cache);
-    else
-        fill_kernel<float><<<grid, 256, 0, st>>>(K, make_scales<float>(h->D), p.B, p.n_blk,
-                                                  h->d_cache_slot, 0, 0, (float2*)h->d_cache);
-    MFH_CUDA_CHECK(cudaGetLastError());
-    return MFH_OK;
+    return h->dtype == MFH_C128
+               ? launch_fill_t<double>(h, grid, p.B, p.n_blk, h->d_cache_slot, 0, 0, h->d_cache, st)
+               : launch_fill_t<float>(h, grid, p.B, p.n_blk, h->d_cache_slot, 0, 0, h->d_cache, st);
 }
 
 // --------------------------------------------------------------------------------------------
@@ -137,25 +152,29 @@ int launch_h0(mfh_handle h, void* out, cudaStream_t st)
     return MFH_OK;
 }
 
+
 // --------------------------------------------------------------------------------------------
 // Fused generate-and-apply, ONE vector, Hermitian reuse (Eq. 11).
 //
 // Work item = rows [row0, row0+nrows) of block n  x  all columns of block m  (n <= m, or any
-// (n,m) for a one-sided item).  A CTA of W warps walks macro tiles of 32W x 32W entries; inside
-// a macro tile warp w owns the 32 rows w*32.. and at step t works on column sub-tile (w+t)%W, so
-// in every step each warp has its own rows AND its own columns.  Inside a 32x32 sub-tile lane l
-// owns row l and at step s handles column (l+s)%32: the entry H_ij (i<j) is generated once in
+// (n,m) for a one-sided item).  The CTA walks the strip in row tiles of TR = 32 R rows: lane l
+// owns the R rows l, l+32, ... of the tile (psi_i and the row accumulators stay in registers for
+// the whole tile), warp w owns the 32-column sub-tiles w, w+W, ... of the block, so every column
+// belongs to exactly one warp: no atomics, and no barrier inside a tile.  In a sub-tile, at step s
+// lane l handles column (l+s) mod 32 of its R rows: each entry H_ij (i<j) is generated once in
 // registers and used twice,
 //     row side     phi_i += H_ij psi_j              (accumulator stays in lane l)
 //     column side  phi_j += conj(H_ij) psi_i        (accumulator rotates lane l+1 -> l each step)
-// so after 32 steps lane l holds the complete column-l sum of the sub-tile: no atomics anywhere.
-// Column sums are added to a shared-memory array (exclusive per step, barrier between steps),
-// row sums live in registers across the whole item.  Results go to partial slots that the
-// reduce kernel adds in a fixed order (deterministic).
+// so after 32 steps lane l holds the complete column-l sum of the sub-tile, which the owning warp
+// adds to the CTA's shared column array.  Row sums are combined across the W warps through shared
+// memory in a fixed order at the end of each tile.  Results go to partial-sum slots that the
+// reduce kernel adds in index order (deterministic, repeatable bit for bit).
 // --------------------------------------------------------------------------------------------
+constexpr int PROC_WARPS = 8;
+constexpr int PROC_THREADS = 32 * PROC_WARPS;
+
 template <typename T> struct ProcParams {
-    PhiloxKeys K;
-    Scales<T> S;
+    GenArgs<T> G;
     int32_t B, n_blk, n_items, slot_row0;
     int64_t D;
     const ProcItem* items;
@@ -164,100 +183,120 @@ template <typename T> struct ProcParams {
     int32_t* counter;
 };
 
-template <typename T, int W>
-__global__ void __launch_bounds__(32 * W) proc_single_kernel(const ProcParams<T> P)
+template <typename T, int R>
+__global__ void __launch_bounds__(PROC_THREADS, 2) proc_single_kernel(const ProcParams<T> P)
 {
     using CT = typename Cplx<T>::type;
-    constexpr int MT = 32 * W;
+    constexpr int W = PROC_WARPS, TR = 32 * R;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    CT* colsum = reinterpret_cast<CT*>(smem_raw);   // [B]  column-side sums of the item
-    CT* psic = colsum + P.B;                        // [MT] psi of the current column macro tile
-    __shared__ int s_item;
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const int B = P.B;
+    const typename Gen<T>::Tab* tab = stage_gen_table<T>(P.G, smem_raw);
+    CT* colsum = reinterpret_cast<CT*>(smem_raw + Gen<T>::TAB_BYTES);   // [B]     column-side sums of the item
+    CT* rowred = colsum + B;                                           // [W][TR] row sums of the tile per warp
+    CT* psiw = rowred + W * TR + w * 32;                               // [32]    psi of the warp's sub-tile
+    __shared__ int s_item;
+    const int n_ct = B / 32;
 
     for (;;) {
+        __syncthreads();
         if (tid == 0) s_item = atomicAdd(P.counter, 1);
         __syncthreads();
         const int it = s_item;
-        __syncthreads();
         if (it >= P.n_items) break;
         const ProcItem I = P.items[it];
         const bool one_sided_item = (I.kind == PAIR_ONE_SIDED);
         const bool diag_item = (I.kind == PAIR_DIAG);
-        for (int c = tid; c < B; c += MT) colsum[c] = CT{T(0), T(0)};
-        const int ncm = B / MT;
+        for (int c = tid; c < B; c += PROC_THREADS) colsum[c] = CT{T(0), T(0)};
+        __syncthreads();
 
-        for (int rloc = I.row0; rloc < I.row0 + I.nrows; rloc += MT) {
-            const uint32_t i = (uint32_t)I.n * B + rloc + w * 32 + lane;
-            const CT psi_i = P.psi[i];
-            T accr = T(0), acci = T(0);
-            const int rmac = rloc / MT;
-            for (int cm = diag_item ? rmac : 0; cm < ncm; ++cm) {
-                __syncthreads();
-                psic[tid] = P.psi[(size_t)I.m * B + cm * MT + tid];
-                __syncthreads();
-                const bool mdiag = diag_item && (cm == rmac);
+        for (int rt = I.row0 / TR; rt < (I.row0 + I.nrows) / TR; ++rt) {
+            const uint32_t i0 = (uint32_t)I.n * B + rt * TR + lane;
+            CT psi_i[R];
+            T accr[R], acci[R];
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                psi_i[r] = P.psi[i0 + 32 * r];
+                accr[r] = acci[r] = T(0);
+            }
+            // diagonal block: sub-tiles left of the tile's diagonal square are covered by transposes
+            const int cs_first = diag_item ? rt * R : 0;
+            for (int cs = cs_first + w; cs < n_ct; cs += W) {
+                const uint32_t j0 = (uint32_t)I.m * B + cs * 32;
+                __syncwarp();
+                psiw[lane] = P.psi[j0 + lane];
+                __syncwarp();
+                if (one_sided_item || (diag_item && cs < (rt + 1) * R)) {
 #pragma unroll 1
-                for (int t = 0; t < W; ++t) {
-                    const int cs = (w + t) & (W - 1);
-                    const uint32_t j0 = (uint32_t)I.m * B + cm * MT + cs * 32;
-                    const CT* pc = psic + cs * 32;
-                    if (one_sided_item || (mdiag && cs == w)) {
-#pragma unroll 2
-                        for (int s = 0; s < 32; ++s) {
+                    for (int s = 0; s < 32; ++s) {
+                        const int c = (lane + s) & 31;
+                        const CT p = psiw[c];
+#pragma unroll
+                        for (int r = 0; r < R; ++r) {
                             T hr, hi;
-                            entry_any<T>(P.K, P.S, i, j0 + s, hr, hi);
-                            const CT p = pc[s];
-                            accr = fma(hr, p.x, accr);
-                            accr = fma(-hi, p.y, accr);
-                            acci = fma(hr, p.y, acci);
-                            acci = fma(hi, p.x, acci);
+                            entry_any<T>(P.G, tab, i0 + 32 * r, j0 + c, hr, hi);
+                            accr[r] = fma(hr, p.x, accr[r]);
+                            accr[r] = fma(-hi, p.y, accr[r]);
+                            acci[r] = fma(hr, p.y, acci[r]);
+                            acci[r] = fma(hi, p.x, acci[r]);
                         }
-                    } else if (!(mdiag && cs < w)) {
-                        T cr = T(0), ci = T(0);
-#pragma unroll 2
-                        for (int s = 0; s < 32; ++s) {
-                            const int c = (lane + s) & 31;
-                            T hr, hi;
-                            entry_upper<T>(P.K, P.S, i, j0 + c, hr, hi);
-                            const CT p = pc[c];
-                            accr = fma(hr, p.x, accr);
-                            accr = fma(-hi, p.y, accr);
-                            acci = fma(hr, p.y, acci);
-                            acci = fma(hi, p.x, acci);
-                            cr = fma(hr, psi_i.x, cr);     // conj(H_ij) psi_i
-                            cr = fma(hi, psi_i.y, cr);
-                            ci = fma(hr, psi_i.y, ci);
-                            ci = fma(-hi, psi_i.x, ci);
-                            cr = __shfl_sync(0xffffffffu, cr, (lane + 1) & 31);
-                            ci = __shfl_sync(0xffffffffu, ci, (lane + 1) & 31);
-                        }
-                        CT& dst = colsum[cm * MT + cs * 32 + lane];
-                        dst.x += cr;
-                        dst.y += ci;
                     }
-                    __syncthreads();
+                } else {
+                    T cr = T(0), ci = T(0);
+#pragma unroll 1
+                    for (int s = 0; s < 32; ++s) {
+                        const int c = (lane + s) & 31;
+                        const CT p = psiw[c];
+#pragma unroll
+                        for (int r = 0; r < R; ++r) {
+                            T hr, hi;
+                            entry_upper<T>(P.G, tab, i0 + 32 * r, j0 + c, hr, hi);
+                            accr[r] = fma(hr, p.x, accr[r]);
+                            accr[r] = fma(-hi, p.y, accr[r]);
+                            acci[r] = fma(hr, p.y, acci[r]);
+                            acci[r] = fma(hi, p.x, acci[r]);
+                            cr = fma(hr, psi_i[r].x, cr);     // conj(H_ij) psi_i
+                            cr = fma(hi, psi_i[r].y, cr);
+                            ci = fma(hr, psi_i[r].y, ci);
+                            ci = fma(-hi, psi_i[r].x, ci);
+                        }
+                        cr = __shfl_sync(0xffffffffu, cr, (lane + 1) & 31);
+                        ci = __shfl_sync(0xffffffffu, ci, (lane + 1) & 31);
+                    }
+                    CT& dst = colsum[cs * 32 + lane];   // this warp is the only writer of these columns
+                    dst.x += cr;
+                    dst.y += ci;
                 }
             }
-            P.work[(size_t)(P.slot_row0 + I.m) * P.D + i] = CT{accr, acci};
+#pragma unroll
+            for (int r = 0; r < R; ++r) rowred[w * TR + lane + 32 * r] = CT{accr[r], acci[r]};
+            __syncthreads();
+            if (tid < TR) {
+                T sr = T(0), si = T(0);
+#pragma unroll
+                for (int ww = 0; ww < W; ++ww) {
+                    const CT v = rowred[ww * TR + tid];
+                    sr += v.x;
+                    si += v.y;
+                }
+                P.work[(size_t)(P.slot_row0 + I.m) * P.D + (size_t)I.n * B + rt * TR + tid] = CT{sr, si};
+            }
+            __syncthreads();
         }
-        __syncthreads();
         if (I.col_slot >= 0) {
             CT* dst = P.work + (size_t)I.col_slot * P.D + (size_t)I.m * B;
-            for (int c = tid; c < B; c += MT) dst[c] = colsum[c];
+            for (int c = tid; c < B; c += PROC_THREADS) dst[c] = colsum[c];
         }
     }
 }
 
-template <typename T, int W>
+template <typename T, int R>
 static int launch_proc_single_t(mfh_handle h, const void* psi, cudaStream_t st)
 {
     using CT = typename Cplx<T>::type;
     const Plan& p = h->plan;
     ProcParams<T> P;
-    P.K = make_philox_keys(h->seed);
-    P.S = make_scales<T>(h->D);
+    P.G = make_gen_args<T>(h);
     P.B = p.B;
     P.n_blk = p.n_blk;
     P.n_items = (int32_t)p.items.size();
@@ -267,20 +306,23 @@ static int launch_proc_single_t(mfh_handle h, const void* psi, cudaStream_t st)
     P.psi = (const CT*)psi;
     P.work = (CT*)h->d_work;
     P.counter = h->d_counter;
-    const size_t smem = (size_t)(p.B + 32 * W) * sizeof(CT);
-    auto kern = proc_single_kernel<T, W>;
+    auto smem_for = [](int B) {
+        return (size_t)Gen<T>::TAB_BYTES + (size_t)(B + PROC_WARPS * 32 * R + PROC_WARPS * 32) * sizeof(CT);
+    };
+    const size_t smem = smem_for(p.B);
+    auto kern = proc_single_kernel<T, R>;
     static bool attr_done = false;
     if (!attr_done) {
         MFH_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                            (int)((MFH_MAX_B + 32 * W) * sizeof(CT))));
+                                            (int)smem_for(MFH_MAX_B)));
         attr_done = true;
     }
     int per_sm = 1;
-    MFH_CUDA_CHECK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, 32 * W, smem));
+    MFH_CUDA_CHECK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, PROC_THREADS, smem));
     if (per_sm < 1) per_sm = 1;
     const int grid = std::min<int>(P.n_items, h->sm_count * per_sm);
     MFH_CUDA_CHECK(cudaMemsetAsync(h->d_counter, 0, sizeof(int32_t), st));
-    kern<<<grid, 32 * W, smem, st>>>(P);
+    kern<<<grid, PROC_THREADS, smem, st>>>(P);
     MFH_CUDA_CHECK(cudaGetLastError());
     return MFH_OK;
 }
@@ -289,13 +331,12 @@ int launch_proc_single(mfh_handle h, const void* psi, cudaStream_t st)
 {
     if (h->plan.items.empty()) return MFH_OK;
     const bool f64 = (h->dtype == MFH_C128);
-    switch (h->plan.warps) {
-    case 8: return f64 ? launch_proc_single_t<double, 8>(h, psi, st) : launch_proc_single_t<float, 8>(h, psi, st);
+    switch (h->plan.R) {
     case 4: return f64 ? launch_proc_single_t<double, 4>(h, psi, st) : launch_proc_single_t<float, 4>(h, psi, st);
     case 2: return f64 ? launch_proc_single_t<double, 2>(h, psi, st) : launch_proc_single_t<float, 2>(h, psi, st);
     case 1: return f64 ? launch_proc_single_t<double, 1>(h, psi, st) : launch_proc_single_t<float, 1>(h, psi, st);
     }
-    set_error("unsupported warps per CTA %d", h->plan.warps);
+    set_error("unsupported rows per lane %d", h->plan.R);
     return MFH_ERR_INVALID_ARG;
 }
 
@@ -307,8 +348,7 @@ int launch_proc_single(mfh_handle h, const void* psi, cudaStream_t st)
 // result is written once with no partial sums over m.
 // --------------------------------------------------------------------------------------------
 template <typename T> struct MultiParams {
-    PhiloxKeys K;
-    Scales<T> S;
+    GenArgs<T> G;
     int32_t B, n_blk, k, slot_multi;
     int64_t D;
     const int32_t* cache_slot;
@@ -321,7 +361,9 @@ __global__ void __launch_bounds__(32 * W) proc_multi_kernel(const MultiParams<T>
 {
     using CT = typename Cplx<T>::type;
     constexpr int CH = 32;                         // columns per staged chunk
-    __shared__ __align__(16) CT psis[CH][KT];
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const typename Gen<T>::Tab* tab = stage_gen_table<T>(P.G, smem_raw);
+    CT(*psis)[KT] = reinterpret_cast<CT(*)[KT]>(smem_raw + Gen<T>::TAB_BYTES);   // [CH][KT]
     const int tid = threadIdx.x;
     const uint32_t i = blockIdx.x * (32 * W) + tid;
     const int n = (int)(i / (uint32_t)P.B);
@@ -343,7 +385,7 @@ __global__ void __launch_bounds__(32 * W) proc_multi_kernel(const MultiParams<T>
 #pragma unroll 2
             for (int c = 0; c < CH; ++c) {
                 T hr, hi;
-                entry_any<T>(P.K, P.S, i, j0 + c, hr, hi);
+                entry_any<T>(P.G, tab, i, j0 + c, hr, hi);
 #pragma unroll
                 for (int v = 0; v < KT; ++v) {
                     const CT p = psis[c][v];
@@ -367,8 +409,7 @@ static int launch_proc_multi_t(mfh_handle h, const void* psi, cudaStream_t st)
     using CT = typename Cplx<T>::type;
     const Plan& p = h->plan;
     MultiParams<T> P;
-    P.K = make_philox_keys(h->seed);
-    P.S = make_scales<T>(h->D);
+    P.G = make_gen_args<T>(h);
     P.B = p.B;
     P.n_blk = p.n_blk;
     P.k = p.k;
@@ -377,11 +418,12 @@ static int launch_proc_multi_t(mfh_handle h, const void* psi, cudaStream_t st)
     P.cache_slot = h->d_cache_slot;
     P.psi = (const CT*)psi;
     P.work = (CT*)h->d_work;
+    const size_t smem = (size_t)Gen<T>::TAB_BYTES + 32 * KT * sizeof(CT);
     // 32W rows per CTA must divide B; prefer 128-row CTAs, fall back to one warp.
     if (p.B % 128 == 0)
-        proc_multi_kernel<T, KT, 4><<<(unsigned)(h->D / 128), 128, 0, st>>>(P);
+        proc_multi_kernel<T, KT, 4><<<(unsigned)(h->D / 128), 128, smem, st>>>(P);
     else
-        proc_multi_kernel<T, KT, 1><<<(unsigned)(h->D / 32), 32, 0, st>>>(P);
+        proc_multi_kernel<T, KT, 1><<<(unsigned)(h->D / 32), 32, smem, st>>>(P);
     MFH_CUDA_CHECK(cudaGetLastError());
     return MFH_OK;
 }
