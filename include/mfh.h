@@ -51,7 +51,11 @@ enum { MFH_OK = 0, MFH_ERR_INVALID_ARG = 1, MFH_ERR_BAD_STATE = 2, MFH_ERR_OUT_O
 enum { MFH_C128 = 0, MFH_C64 = 1 };
 enum { MFH_SRC_GUE = 0,           /* H = lambda * V(seed)                          configs 1,2,4,5 */
        MFH_SRC_DIAG_PLUS_GUE = 1  /* H_v = diag(h0(seed_h0)) + lambda_v * V(seed)  config 3        */ };
-enum { MFH_MODE_AUTO = 0, MFH_MODE_PROCEDURAL = 1, MFH_MODE_PARTIAL = 2, MFH_MODE_FULL = 3 };
+enum { MFH_MODE_AUTO = 0, MFH_MODE_PROCEDURAL = 1, MFH_MODE_PARTIAL = 2, MFH_MODE_FULL = 3,
+       /* Hermitian (canonical-pair) cache, Eq. 27: block (n,m), n <= m, is stored once
+        * and used for phi^[n] += C psi^[m] and phi^[m] += C^dagger psi^[n]; as many pairs as the budget
+        * allows (nearest block diagonals first), the rest is generated.  Half the bytes of FULL. */
+       MFH_MODE_PAIRS = 4 };
 
 #define MFH_MAX_K 16       /* largest number of simultaneous vectors */
 #define MFH_MIN_B 32       /* block size must be a multiple of this and divide D */

@@ -18,12 +18,12 @@ MFH_ERR_INVALID_ARG, MFH_ERR_BAD_STATE, MFH_ERR_OUT_OF_MEMORY = 1, 2, 3
 MFH_ERR_CUDA, MFH_ERR_NOT_CONVERGED, MFH_ERR_UNSUPPORTED = 4, 5, 6
 MFH_C128, MFH_C64 = 0, 1
 MFH_SRC_GUE, MFH_SRC_DIAG_PLUS_GUE = 0, 1
-MFH_MODE_AUTO, MFH_MODE_PROCEDURAL, MFH_MODE_PARTIAL, MFH_MODE_FULL = 0, 1, 2, 3
+MFH_MODE_AUTO, MFH_MODE_PROCEDURAL, MFH_MODE_PARTIAL, MFH_MODE_FULL, MFH_MODE_PAIRS = 0, 1, 2, 3, 4
 MFH_MAX_K = 16
 
 DTYPES = {"c128": MFH_C128, "c64": MFH_C64}
 MODES = {"auto": MFH_MODE_AUTO, "procedural": MFH_MODE_PROCEDURAL, "partial": MFH_MODE_PARTIAL,
-         "full": MFH_MODE_FULL}
+         "full": MFH_MODE_FULL, "pairs": MFH_MODE_PAIRS}
 
 # every symbol include/mfh.h declares (tests check that the library exports all of them)
 SYMBOLS = ["mfh_create", "mfh_plan_analytic", "mfh_plan", "mfh_apply", "mfh_apply_host", "mfh_apply_timed",

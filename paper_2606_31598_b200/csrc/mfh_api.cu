@@ -38,7 +38,8 @@ static bool valid_B(int64_t D, int32_t B)
 static int free_plan_resources(mfh_handle h)
 {
     void** ptrs[] = {&h->d_cache, &h->d_work, &h->d_h0, (void**)&h->d_cache_slot, (void**)&h->d_items,
-                     (void**)&h->d_slot_valid, (void**)&h->d_counter, &h->d_cheb, &h->d_io};
+                     (void**)&h->d_pair_items,
+                     (void**)&h->d_slot_list, (void**)&h->d_counter, &h->d_cheb, &h->d_io};
     for (void** p : ptrs) {
         if (*p) cudaFree(*p);
         *p = nullptr;
@@ -92,10 +93,24 @@ static int commit_plan(mfh_handle h, const Plan& p, cudaStream_t st)
         MFH_CUDA_CHECK(cudaMemcpyAsync(h->d_items, q.items.data(), q.items.size() * sizeof(ProcItem),
                                        cudaMemcpyHostToDevice, st));
     }
-    MFH_CUDA_CHECK(cudaMalloc(&h->d_slot_valid, q.slot_valid.size()));
-    MFH_CUDA_CHECK(cudaMemcpyAsync(h->d_slot_valid, q.slot_valid.data(), q.slot_valid.size(),
-                                   cudaMemcpyHostToDevice, st));
-    MFH_CUDA_CHECK(cudaMalloc(&h->d_counter, sizeof(int32_t)));
+    {   // compact ascending slot lists per block row
+        const int ns = std::max(q.n_slots, 1);
+        std::vector<int32_t> lists((size_t)q.n_blk * (ns + 1), 0);
+        for (int b = 0; b < q.n_blk; ++b) {
+            int32_t* L = lists.data() + (size_t)b * (ns + 1);
+            for (int sl = 0; sl < q.n_slots; ++sl)
+                if (q.slot_valid[(size_t)b * q.n_slots + sl]) L[1 + L[0]++] = sl;
+        }
+        MFH_CUDA_CHECK(cudaMalloc(&h->d_slot_list, lists.size() * sizeof(int32_t)));
+        MFH_CUDA_CHECK(cudaMemcpy(h->d_slot_list, lists.data(), lists.size() * sizeof(int32_t),
+                                  cudaMemcpyHostToDevice));
+    }
+    if (!q.pair_items.empty()) {
+        MFH_CUDA_CHECK(cudaMalloc(&h->d_pair_items, q.pair_items.size() * sizeof(ProcItem)));
+        MFH_CUDA_CHECK(cudaMemcpyAsync(h->d_pair_items, q.pair_items.data(), q.pair_items.size() * sizeof(ProcItem),
+                                       cudaMemcpyHostToDevice, st));
+    }
+    MFH_CUDA_CHECK(cudaMalloc(&h->d_counter, 2 * sizeof(int32_t)));
     MFH_CUDA_CHECK(cudaMalloc(&h->d_io, (size_t)2 * h->D * q.k * cb));
     if (h->kind == MFH_SRC_DIAG_PLUS_GUE) {
         MFH_CUDA_CHECK(cudaMalloc(&h->d_h0, (size_t)h->D * (h->dtype == MFH_C128 ? 8 : 4)));
@@ -118,7 +133,7 @@ static int apply_impl(mfh_handle h, const void* psi, void* phi, const double* la
     const Plan& p = h->plan;
     int rc;
     if (ev) cudaEventRecord(ev[0], st);
-    if ((rc = launch_cached(h, psi, st))) return rc;
+    if ((rc = p.pairs ? launch_cached_pairs(h, psi, st) : launch_cached(h, psi, st))) return rc;
     if (ev) cudaEventRecord(ev[1], st);
     if (p.k == 1) {
         if ((rc = launch_proc_single(h, psi, st))) return rc;
@@ -216,7 +231,7 @@ MFH_API int mfh_plan_analytic(int64_t D, int32_t dtype, int32_t k, int32_t mode,
                               size_t json_cap)
 {
     if (D < 32 || D % 32 != 0 || (dtype != MFH_C128 && dtype != MFH_C64) || k < 1 || k > MFH_MAX_K ||
-        mode < MFH_MODE_AUTO || mode > MFH_MODE_FULL || (B != 0 && !valid_B(D, B)) || hbm_free_bytes <= 0) {
+        mode < MFH_MODE_AUTO || mode > MFH_MODE_PAIRS || (B != 0 && !valid_B(D, B)) || hbm_free_bytes <= 0) {
         set_error("mfh_plan_analytic: invalid argument");
         return MFH_ERR_INVALID_ARG;
     }
@@ -233,7 +248,7 @@ MFH_API int mfh_plan(mfh_handle h, int32_t mode, int32_t k, int64_t n_applies_hi
                      size_t json_cap)
 {
     if (!h) { set_error("mfh_plan: NULL handle"); return MFH_ERR_INVALID_ARG; }
-    if (k < 1 || k > MFH_MAX_K || mode < MFH_MODE_AUTO || mode > MFH_MODE_FULL || hbm_budget_bytes < 0) {
+    if (k < 1 || k > MFH_MAX_K || mode < MFH_MODE_AUTO || mode > MFH_MODE_PAIRS || hbm_budget_bytes < 0) {
         set_error("mfh_plan: invalid argument (k=%d, mode=%d)", k, mode);
         return MFH_ERR_INVALID_ARG;
     }
@@ -259,6 +274,7 @@ MFH_API int mfh_plan(mfh_handle h, int32_t mode, int32_t k, int64_t n_applies_hi
         p.B = c.B;
         p.k = k;
         p.cached_per_row = c.cached_per_row;
+        p.pairs = c.pairs;
         build_tables(p, h->D, h->dtype, h->sm_count);
         return p;
     };
@@ -301,11 +317,12 @@ MFH_API int mfh_get_plan(mfh_handle h, char* json_out, size_t json_cap)
     char buf[768];
     snprintf(buf, sizeof buf,
              "{\"mode\":\"%s\",\"B\":%d,\"n_blk\":%d,\"k\":%d,\"cached_blocks\":%lld,\"cached_per_row\":%d,"
-             "\"cache_bytes\":%zu,\"work_bytes\":%zu,\"partial_slots\":%d,\"proc_items\":%zu,"
+             "\"cached_fraction\":%.6g,\"cache_bytes\":%zu,\"work_bytes\":%zu,\"partial_slots\":%d,\"proc_items\":%zu,\"pair_items\":%zu,"
              "\"proc_rows_per_lane\":%d,\"proc_row_strips\":%d,\"launches_per_apply\":%d}",
-             p.mode == MFH_MODE_FULL ? "full" : (p.mode == MFH_MODE_PARTIAL ? "partial" : "procedural"), p.B,
-             p.n_blk, p.k, (long long)p.n_cached, p.cached_per_row, p.cache_bytes, p.work_bytes, p.n_slots,
-             p.items.size(), p.R, p.Q,
+             p.mode == MFH_MODE_FULL ? "full" : (p.mode == MFH_MODE_PARTIAL ? "partial" : (p.mode == MFH_MODE_PAIRS ? "pairs" : "procedural")), p.B,
+             p.n_blk, p.k, (long long)p.n_cached, p.cached_per_row,
+             (double)p.covered_blocks / ((double)p.n_blk * p.n_blk), p.cache_bytes, p.work_bytes, p.n_slots,
+             p.items.size(), p.pair_items.size(), p.R, p.Q,
              1 + (p.n_cached > 0) + ((p.k == 1 && !p.items.empty()) || p.slot_multi >= 0));
     copy_json(buf, json_out, json_cap);
     return MFH_OK;

@@ -7,6 +7,7 @@
 // rows with 128-bit non-allocating loads, several independent loads in flight per lane; psi^[m]
 // is staged once per CTA per column block in shared memory and shared by all warps.
 #include <algorithm>
+#include <cstdlib>
 #include "mfh_internal.cuh"
 
 namespace mfh {
@@ -184,6 +185,224 @@ int launch_cached(mfh_handle h, const void* psi, cudaStream_t st)
     }
     MFH_CUDA_CHECK(cudaGetLastError());
     return MFH_OK;
+}
+
+// --------------------------------------------------------------------------------------------
+// Hermitian pair cache (cache budget over canonical pairs P:437-446 Eq. 27): block
+// C = H^[n,m], n < m, is stored once and every loaded entry is used twice,
+//     row side     phi^[n]_a += C_ab psi^[m]_b
+//     column side  phi^[m]_b += conj(C_ab) psi^[n]_a
+// which halves the HBM bytes per apply.  Work item = a strip of rows of one stored block; a CTA of
+// 8 warps pulls items from a device counter.  Warp w owns the column chunks w, w+8, ... (32 U
+// 128-bit loads wide), so a lane's columns are fixed while it sweeps the rows of the strip: its
+// psi^[m] values and its column accumulators stay in registers and need no reduction at all.  Row
+// partials of 4 rows at a time are combined across the 32 lanes by a transposing butterfly
+// (24 shuffles per 4 rows instead of 80) and accumulated per (warp,row) in shared memory; at the
+// end of the item they are added over the warps in a fixed order.  No atomics; results go to the
+// same partial-sum slots as the fused kernel (row side: slot of column block m, column side: slot
+// of (row block n, strip)), added in index order by the reduce kernel.
+// --------------------------------------------------------------------------------------------
+constexpr int PAIR_WARPS = 8;
+constexpr int PAIR_THREADS = 32 * PAIR_WARPS;
+constexpr int PAIR_RR = 4;   // rows per butterfly
+constexpr int PAIR_SR = 256; // rows per sub-strip (shared-memory row partials)
+
+template <typename T> struct PairParams {
+    int32_t B, n_blk, n_items, slot_row0;
+    int64_t D;
+    const ProcItem* items;
+    const int32_t* cache_slot;
+    const typename Cplx<T>::type* cache;
+    const typename Cplx<T>::type* psi;
+    typename Cplx<T>::type* work;
+    int32_t* counter;
+};
+
+template <typename T> struct Vec16;   // one 128-bit load = E entries
+template <> struct Vec16<double> {
+    static constexpr int E = 1;
+    double2 v;
+    __device__ __forceinline__ void load(const double2* p) { v = ldg_stream(p); }
+    __device__ __forceinline__ double2 get(int) const { return v; }
+};
+template <> struct Vec16<float> {
+    static constexpr int E = 2;
+    float4 v;
+    __device__ __forceinline__ void load(const float2* p) { v = ldg_stream(reinterpret_cast<const float4*>(p)); }
+    __device__ __forceinline__ float2 get(int e) const { return e == 0 ? float2{v.x, v.y} : float2{v.z, v.w}; }
+};
+
+// Sum r[0..3] over the 32 lanes; on return every lane holds the total of row 2*bit4 + bit3.
+template <typename T> __device__ __forceinline__ T butterfly4(T r0, T r1, T r2, T r3, int lane)
+{
+    const bool up16 = lane & 16, up8 = lane & 8;
+    T k0 = up16 ? r2 : r0, k1 = up16 ? r3 : r1;
+    const T s0 = up16 ? r0 : r2, s1 = up16 ? r1 : r3;
+    k0 += __shfl_xor_sync(0xffffffffu, s0, 16);
+    k1 += __shfl_xor_sync(0xffffffffu, s1, 16);
+    T v = up8 ? k1 : k0;
+    const T s = up8 ? k0 : k1;
+    v += __shfl_xor_sync(0xffffffffu, s, 8);
+    v += __shfl_xor_sync(0xffffffffu, v, 4);
+    v += __shfl_xor_sync(0xffffffffu, v, 2);
+    v += __shfl_xor_sync(0xffffffffu, v, 1);
+    return v;
+}
+
+template <typename T, int U, int MINB>
+__global__ void __launch_bounds__(PAIR_THREADS, MINB) cached_pairs_kernel(const PairParams<T> P)
+{
+    using CT = typename Cplx<T>::type;
+    constexpr int E = Vec16<T>::E, W = PAIR_WARPS, RR = PAIR_RR;
+    constexpr int CW = 32 * U * E;                      // columns per warp chunk
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    CT* psin = reinterpret_cast<CT*>(smem_raw);         // [nrows]     psi^[n] of the strip
+    CT* rowpart = psin + PAIR_SR;                       // [W][nrows]  row partials per warp
+    __shared__ int s_item;
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    const int B = P.B, n_chunks = B / CW;
+
+    for (;;) {
+        __syncthreads();
+        if (tid == 0) s_item = atomicAdd(P.counter, 1);
+        __syncthreads();
+        const int it = s_item;
+        if (it >= P.n_items) break;
+        const ProcItem I = P.items[it];
+        const bool col_side = (I.col_slot >= 0);
+        // rows of the item in sub-strips of at most PAIR_SR rows (shared-memory row partials)
+        for (int s0 = 0; s0 < I.nrows; s0 += PAIR_SR) {
+            const int nrows = min(PAIR_SR, I.nrows - s0);
+            if (s0) __syncthreads();
+            for (int a = tid; a < nrows; a += PAIR_THREADS) psin[a] = P.psi[(size_t)I.n * B + I.row0 + s0 + a];
+            for (int a = tid; a < W * nrows; a += PAIR_THREADS) rowpart[a] = CT{T(0), T(0)};
+            __syncthreads();
+            const CT* blk = P.cache + (size_t)P.cache_slot[I.n * P.n_blk + I.m] * B * B + (size_t)(I.row0 + s0) * B;
+
+            for (int ch = w; ch < n_chunks; ch += W) {
+                const int c0 = ch * CW + lane * E;          // this lane's columns: c0 + 32 E u + e
+                CT pm[U][E], cacc[U][E];
+#pragma unroll
+                for (int u = 0; u < U; ++u)
+#pragma unroll
+                    for (int e = 0; e < E; ++e) {
+                        pm[u][e] = P.psi[(size_t)I.m * B + c0 + 32 * E * u + e];
+                        cacc[u][e] = CT{T(0), T(0)};
+                    }
+                for (int a = 0; a < nrows; a += RR) {
+                    Vec16<T> hv[RR][U];
+#pragma unroll
+                    for (int r = 0; r < RR; ++r)
+#pragma unroll
+                        for (int u = 0; u < U; ++u) hv[r][u].load(blk + (size_t)(a + r) * B + c0 + 32 * E * u);
+                    T rr_[RR], ri_[RR];
+#pragma unroll
+                    for (int r = 0; r < RR; ++r) {
+                        const CT pn = psin[a + r];
+                        T sr = T(0), si = T(0);
+#pragma unroll
+                        for (int u = 0; u < U; ++u)
+#pragma unroll
+                            for (int e = 0; e < E; ++e) {
+                                const CT hh = hv[r][u].get(e);
+                                sr = fma(hh.x, pm[u][e].x, sr);
+                                sr = fma(-hh.y, pm[u][e].y, sr);
+                                si = fma(hh.x, pm[u][e].y, si);
+                                si = fma(hh.y, pm[u][e].x, si);
+                                if (col_side) {
+                                    cacc[u][e].x = fma(hh.x, pn.x, cacc[u][e].x);     // conj(C_ab) psi_a
+                                    cacc[u][e].x = fma(hh.y, pn.y, cacc[u][e].x);
+                                    cacc[u][e].y = fma(hh.x, pn.y, cacc[u][e].y);
+                                    cacc[u][e].y = fma(-hh.y, pn.x, cacc[u][e].y);
+                                }
+                            }
+                        rr_[r] = sr;
+                        ri_[r] = si;
+                    }
+                    const T tr = butterfly4<T>(rr_[0], rr_[1], rr_[2], rr_[3], lane);
+                    const T ti = butterfly4<T>(ri_[0], ri_[1], ri_[2], ri_[3], lane);
+                    if ((lane & 7) == 0) {
+                        CT& dst = rowpart[w * nrows + a + (lane >> 3)];   // row 2*bit4 + bit3 = lane >> 3
+                        dst.x += tr;
+                        dst.y += ti;
+                    }
+                }
+                if (col_side) {   // this lane is the only writer of its columns: later sub-strips add in order
+                    CT* dst = P.work + (size_t)I.col_slot * P.D + (size_t)I.m * B + c0;
+#pragma unroll
+                    for (int u = 0; u < U; ++u)
+#pragma unroll
+                        for (int e = 0; e < E; ++e) {
+                            CT v = cacc[u][e];
+                            if (s0) {
+                                const CT o = dst[32 * E * u + e];
+                                v.x += o.x;
+                                v.y += o.y;
+                            }
+                            dst[32 * E * u + e] = v;
+                        }
+                }
+            }
+            __syncthreads();
+            for (int a = tid; a < nrows; a += PAIR_THREADS) {
+                T sr = T(0), si = T(0);
+#pragma unroll
+                for (int ww = 0; ww < W; ++ww) {
+                    const CT v = rowpart[ww * nrows + a];
+                    sr += v.x;
+                    si += v.y;
+                }
+                P.work[(size_t)(P.slot_row0 + I.m) * P.D + (size_t)I.n * B + I.row0 + s0 + a] = CT{sr, si};
+            }
+        }
+    }
+}
+
+template <typename T, int U, int MINB>
+static int launch_pairs_t(mfh_handle h, const void* psi, cudaStream_t st)
+{
+    using CT = typename Cplx<T>::type;
+    const Plan& p = h->plan;
+    PairParams<T> P;
+    P.B = p.B;
+    P.n_blk = p.n_blk;
+    P.n_items = (int32_t)p.pair_items.size();
+    P.slot_row0 = p.slot_row0;
+    P.D = h->D;
+    P.items = h->d_pair_items;
+    P.cache_slot = h->d_cache_slot;
+    P.cache = (const CT*)h->d_cache;
+    P.psi = (const CT*)psi;
+    P.work = (CT*)h->d_work;
+    P.counter = h->d_counter + 1;
+    const size_t smem = (size_t)(1 + PAIR_WARPS) * PAIR_SR * sizeof(CT);
+    auto kern = cached_pairs_kernel<T, U, MINB>;
+    int per_sm = 1;
+    MFH_CUDA_CHECK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, PAIR_THREADS, smem));
+    if (per_sm < 1) per_sm = 1;
+    const int grid = std::min<int>(P.n_items, h->sm_count * per_sm);
+    MFH_CUDA_CHECK(cudaMemsetAsync(h->d_counter + 1, 0, sizeof(int32_t), st));
+    kern<<<grid, PAIR_THREADS, smem, st>>>(P);
+    MFH_CUDA_CHECK(cudaGetLastError());
+    return MFH_OK;
+}
+
+int launch_cached_pairs(mfh_handle h, const void* psi, cudaStream_t st)
+{
+    const Plan& p = h->plan;
+    if (p.pair_items.empty()) return MFH_OK;
+    if (p.k != 1) {
+        set_error("the pair cache with k > 1 is not supported yet");
+        return MFH_ERR_UNSUPPORTED;
+    }
+    // U 128-bit loads per row per lane x 4 rows in flight; U = 4 at 2 CTAs/SM measured best on C2
+    // (7.0 TB/s vs 6.9 for U = 2 at 3 CTAs/SM and 6.6 at 2 CTAs/SM)
+    if (h->dtype == MFH_C128) {
+        if (p.B % 128 == 0) return launch_pairs_t<double, 4, 2>(h, psi, st);
+        if (p.B % 64 == 0) return launch_pairs_t<double, 2, 3>(h, psi, st);
+        return launch_pairs_t<double, 1, 4>(h, psi, st);
+    }
+    return p.B % 128 == 0 ? launch_pairs_t<float, 2, 2>(h, psi, st) : launch_pairs_t<float, 1, 2>(h, psi, st);
 }
 
 }  // namespace mfh

@@ -38,14 +38,17 @@ struct Plan {
     int32_t B = 0, n_blk = 0, k = 0;
     int32_t Q = 1;             // row strips per block in the procedural kernel
     int32_t R = 4;             // rows per lane in the procedural kernel (row tile = 32*R rows)
-    int64_t n_cached = 0;      // cached blocks
+    bool pairs = false;        // Hermitian pair cache: store block (n,m), n <= m, use it for both sides
+    int64_t n_cached = 0;      // stored blocks
+    int64_t covered_blocks = 0;   // block positions (n,m) served from the cache
     int32_t cached_per_row = 0;
     int32_t n_slots = 0;       // partial vectors in the workspace
     int32_t slot_cache = -1, slot_row0 = -1, slot_col0 = -1, slot_multi = -1;
     size_t cache_bytes = 0, work_bytes = 0;
     std::vector<int32_t> cache_slot;   // [n_blk*n_blk] index of the cached block or -1
     std::vector<uint8_t> pair_kind;    // [n_blk*n_blk]
-    std::vector<ProcItem> items;
+    std::vector<ProcItem> items;       // fused generate-and-apply kernel
+    std::vector<ProcItem> pair_items;  // cached pair kernel (pairs mode)
     std::vector<uint8_t> slot_valid;   // [n_blk][n_slots]
     std::string json;
 };
@@ -66,9 +69,10 @@ struct mfh_handle_s {
     void* d_h0 = nullptr;           // D reals (DIAG_PLUS_GUE)
     int32_t* d_cache_slot = nullptr;
     mfh::ProcItem* d_items = nullptr;
-    uint8_t* d_slot_valid = nullptr;
+    mfh::ProcItem* d_pair_items = nullptr;
+    int32_t* d_slot_list = nullptr;   // [n_blk][n_slots+1]: count, then the valid slots in ascending order
     double* d_lambdas = nullptr;    // MFH_MAX_K doubles, refreshed by every apply
-    int32_t* d_counter = nullptr;   // dynamic work counter of the procedural kernel
+    int32_t* d_counter = nullptr;   // dynamic work counters: [0] procedural kernel, [1] pair kernel
     void* d_cheb = nullptr;         // 3 vectors of Chebyshev scratch
     void* d_io = nullptr;           // psi/phi staging of mfh_apply_host
     mfh::GenHostD gen_host;         // generator table + constants for this D (host copy)
@@ -103,6 +107,7 @@ int launch_h0(mfh_handle h, void* out, cudaStream_t st);
 int launch_proc_single(mfh_handle h, const void* psi, cudaStream_t st);
 int launch_proc_multi(mfh_handle h, const void* psi, cudaStream_t st);
 int launch_cached(mfh_handle h, const void* psi, cudaStream_t st);
+int launch_cached_pairs(mfh_handle h, const void* psi, cudaStream_t st);
 int launch_reduce(mfh_handle h, const void* psi, void* phi, const double* lambdas_host, cudaStream_t st);
 int launch_cheb_first(mfh_handle h, const void* psi, void* q_prev, void* acc, double j0,
                       cudaStream_t st);

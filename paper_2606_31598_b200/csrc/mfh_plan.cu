@@ -15,11 +15,11 @@ namespace mfh {
 // Model constants (seconds, bytes/s, generations/s).  Starting values; the measured planner
 // (mfh_plan with measure != 0) overrides the ranking with device timings (Algorithm 2).
 static const double kAlpha = 0.9;            // safety fraction of Eq. 18 (the paper gives none)
-static const double kBwRead = 6.0e12;        // cached streaming, B/s
+static const double kBwRead = 7.2e12;        // cached streaming, B/s (measured on C2: 7.3e12)
 static const double kBwWrite = 3.0e12;       // cache fill stores, B/s
 static const double kLaunch = 6e-6;          // per kernel launch
 
-static double gen_pairs_per_s(int dtype) { return dtype == MFH_C128 ? 2.4e11 : 6.0e11; }
+static double gen_pairs_per_s(int dtype) { return dtype == MFH_C128 ? 2.5e11 : 6.0e11; }   // measured on C4: 2.56e11
 static double gen_entries_per_s(int dtype, int k)
 {
     // one-sided generation plus 4k FMAs per entry on the same issue slots
@@ -44,6 +44,7 @@ static const char* mode_name(int mode)
     case MFH_MODE_PROCEDURAL: return "procedural";
     case MFH_MODE_PARTIAL: return "partial";
     case MFH_MODE_FULL: return "full";
+    case MFH_MODE_PAIRS: return "pairs";
     }
     return "auto";
 }
@@ -80,7 +81,7 @@ void choose_tiling(int B, int n_blk, int n_pairs, int sm_count, int& R, int& Q)
     }
     const int qmax = B / (32 * R);
     Q = 1;
-    while (Q * 2 <= qmax && (int64_t)n_pairs * Q < 48LL * sm_count && (int64_t)n_blk * Q * 2 <= 512) Q *= 2;
+    while (qmax % (Q * 2) == 0 && (int64_t)n_pairs * Q < 48LL * sm_count && (int64_t)n_blk * Q * 2 <= 512) Q *= 2;
 }
 
 // Generator table of mfh_gen.cuh for dimension D (host arithmetic in long double).
@@ -108,21 +109,47 @@ void make_gen_table(int64_t D, GenHostD& out)
     out.gc.ang = (double)(2.0L * PI / 4294967296.0L);
 }
 
+// Offsets covered by a Hermitian pair cache with c band offsets: circular block distance < c.
+int pair_full_offsets(int N) { return N / 2 + 1; }
+
 void build_tables(Plan& p, int64_t D, int dtype, int sm_count)
 {
     const int N = p.n_blk = (int)(D / p.B);
     const int c = p.cached_per_row;
-    p.n_cached = (int64_t)c * N;
     p.cache_slot.assign((size_t)N * N, -1);
-    const std::vector<int> offs = band_offsets(N);
-    for (int n = 0; n < N; ++n)
-        for (int t = 0; t < c; ++t) p.cache_slot[(size_t)n * N + (n + offs[t]) % N] = n * c + t;
-    auto uncached = [&](int n, int m) { return p.cache_slot[(size_t)n * N + m] < 0; };
+    p.pair_items.clear();
+    int n_stored = 0;
+    if (!p.pairs) {
+        // full blocks, row-balanced symmetric band (R5)
+        const std::vector<int> offs = band_offsets(N);
+        for (int n = 0; n < N; ++n)
+            for (int t = 0; t < c; ++t) p.cache_slot[(size_t)n * N + (n + offs[t]) % N] = n * c + t;
+        n_stored = c * N;
+    } else {
+        // canonical pairs: every unordered block pair {n,m} with circular
+        // distance d < c is stored once as block (min,max); the mirrored position is marked -2.
+        for (int d = 0; d < c && d <= N / 2; ++d)
+            for (int n = 0; n < N; ++n) {
+                const int m = (n + d) % N;
+                if (d == 0) {
+                    p.cache_slot[(size_t)n * N + n] = n_stored++;
+                    continue;
+                }
+                if (2 * d == N && n >= N / 2) continue;   // {n, n+N/2} was stored from the other side
+                const int lo = std::min(n, m), hi = std::max(n, m);
+                p.cache_slot[(size_t)lo * N + hi] = n_stored++;
+                p.cache_slot[(size_t)hi * N + lo] = -2;
+            }
+    }
+    p.n_cached = n_stored;
+    auto uncached = [&](int n, int m) { return p.cache_slot[(size_t)n * N + m] == -1; };
+    int64_t covered = 0;
+    for (int32_t v : p.cache_slot) covered += (v != -1);
+    p.covered_blocks = covered;
 
     p.pair_kind.assign((size_t)N * N, PAIR_NONE);
     p.items.clear();
     int n_pairs = 0;
-    bool any_col = false;
     if (p.k == 1) {
         for (int n = 0; n < N; ++n) {
             if (uncached(n, n)) p.pair_kind[(size_t)n * N + n] = PAIR_DIAG;
@@ -133,60 +160,71 @@ void build_tables(Plan& p, int64_t D, int dtype, int sm_count)
                 else if (b) p.pair_kind[(size_t)m * N + n] = PAIR_ONE_SIDED;
             }
         }
-        for (uint8_t kd : p.pair_kind) {
-            n_pairs += (kd != PAIR_NONE);
-            any_col |= (kd == PAIR_TWO_SIDED || kd == PAIR_DIAG);
-        }
+        for (uint8_t kd : p.pair_kind) n_pairs += (kd != PAIR_NONE);
     }
-    choose_tiling(p.B, N, std::max(n_pairs, 1), sm_count, p.R, p.Q);
+    const int n_pair_blocks = p.pairs ? n_stored : 0;
+    choose_tiling(p.B, N, std::max(n_pairs + n_pair_blocks, 1), sm_count, p.R, p.Q);
 
-    // partial-sum slots
+    // partial-sum slots: [cached rows] [row side, one per column block] [column side, one per
+    // (row block, strip)] [k-vector kernel, one per column block]
     int s = 0;
     p.slot_cache = p.slot_row0 = p.slot_col0 = p.slot_multi = -1;
-    if (c > 0) p.slot_cache = s++;
-    if (p.k == 1 && n_pairs > 0) {
+    if (!p.pairs && c > 0) p.slot_cache = s++;
+    if (p.k == 1 && n_pairs + n_pair_blocks > 0) {
         p.slot_row0 = s;
         s += N;
-        if (any_col) {
-            p.slot_col0 = s;
-            s += N * p.Q;
-        }
+        p.slot_col0 = s;
+        s += N * p.Q;
     }
-    if (p.k > 1 && c < N) p.slot_multi = s++;
+    if (p.k > 1 && covered < (int64_t)N * N) {   // k-vector kernel: one partial slot per column block m
+        p.slot_multi = s;
+        s += N;
+    }
     p.n_slots = s;
     p.slot_valid.assign((size_t)N * std::max(s, 1), 0);
     auto valid = [&](int b, int slot) -> uint8_t& { return p.slot_valid[(size_t)b * p.n_slots + slot]; };
     for (int b = 0; b < N; ++b) {
         if (p.slot_cache >= 0) valid(b, p.slot_cache) = 1;
-        if (p.slot_multi >= 0) valid(b, p.slot_multi) = 1;
+        if (p.slot_multi >= 0)
+            for (int m = 0; m < N; ++m) valid(b, p.slot_multi + m) = uncached(b, m);
     }
+    const int strip = p.B / p.Q;
+    auto push_items = [&](std::vector<ProcItem>& dst, int n, int m, uint8_t kd) {
+        valid(n, p.slot_row0 + m) = 1;
+        const bool col = (kd == PAIR_TWO_SIDED || kd == PAIR_DIAG);
+        for (int q = 0; q < p.Q; ++q) {
+            ProcItem it;
+            it.n = n;
+            it.m = m;
+            it.row0 = q * strip;
+            it.nrows = strip;
+            it.kind = kd;
+            it.col_slot = (col && !(kd == PAIR_DIAG && &dst == &p.pair_items)) ? p.slot_col0 + n * p.Q + q : -1;
+            if (it.col_slot >= 0) valid(m, it.col_slot) = 1;
+            dst.push_back(it);
+        }
+    };
     if (p.k == 1 && n_pairs > 0) {
-        const int strip = p.B / p.Q;
         // full-size two-sided items first, the half-size diagonal items last (better tail)
         for (int pass = 0; pass < 2; ++pass)
             for (int n = 0; n < N; ++n)
                 for (int m = 0; m < N; ++m) {
                     const uint8_t kd = p.pair_kind[(size_t)n * N + m];
                     if (kd == PAIR_NONE || (pass == 0) != (kd != PAIR_DIAG)) continue;
-                    valid(n, p.slot_row0 + m) = 1;
-                    const bool col = (kd == PAIR_TWO_SIDED || kd == PAIR_DIAG);
-                    for (int q = 0; q < p.Q; ++q) {
-                        ProcItem it;
-                        it.n = n;
-                        it.m = m;
-                        it.row0 = q * strip;
-                        it.nrows = strip;
-                        it.kind = kd;
-                        it.col_slot = col ? p.slot_col0 + n * p.Q + q : -1;
-                        if (col) valid(m, it.col_slot) = 1;
-                        p.items.push_back(it);
-                    }
+                    push_items(p.items, n, m, kd);
                 }
     }
+    if (p.pairs)   // stored blocks: off-diagonal pairs feed both sides, diagonal blocks the row side only
+        for (int n = 0; n < N; ++n)
+            for (int m = n; m < N; ++m)
+                if (p.cache_slot[(size_t)n * N + m] >= 0)
+                    push_items(p.pair_items, n, m, n == m ? PAIR_DIAG : PAIR_TWO_SIDED);
     const size_t cb = complex_bytes(dtype);
     p.cache_bytes = (size_t)p.n_cached * p.B * p.B * cb;
     p.work_bytes = (size_t)std::max(p.n_slots, 1) * D * p.k * cb;
-    p.mode = (c == 0) ? MFH_MODE_PROCEDURAL : (c == N ? MFH_MODE_FULL : MFH_MODE_PARTIAL);
+    if (covered == 0) p.mode = MFH_MODE_PROCEDURAL;
+    else if (p.pairs) p.mode = MFH_MODE_PAIRS;
+    else p.mode = (c == N ? MFH_MODE_FULL : MFH_MODE_PARTIAL);
 }
 
 // Scratch outside the partial slots: Chebyshev (3 vectors), host-apply staging (2 k vectors), H0.
@@ -195,14 +233,16 @@ static size_t fixed_work_bytes(int64_t D, int dtype, int k)
     return (size_t)D * complex_bytes(dtype) * (3 + 2 * k) + (size_t)D * 8;
 }
 
-Candidate evaluate_candidate(int64_t D, int dtype, int k, int B, int cached_per_row, int64_t n_applies,
-                             int sm_count)
+Candidate evaluate_candidate(int64_t D, int dtype, int k, int B, int cached_per_row, bool pairs,
+                             int64_t n_applies, int sm_count)
 {
     Candidate c;
     Plan p;
     p.B = B;
     p.k = k;
     p.cached_per_row = cached_per_row;
+    p.pairs = pairs;
+    c.pairs = pairs;
     build_tables(p, D, dtype, sm_count);
     c.B = B;
     c.mode = p.mode;
@@ -212,9 +252,10 @@ Candidate evaluate_candidate(int64_t D, int dtype, int k, int B, int cached_per_
     c.cache_bytes = (double)p.cache_bytes;                                   // M_op, Eq. 15-17
     c.work_bytes = (double)p.work_bytes + (double)fixed_work_bytes(D, dtype, k);   // M_work, Eq. 14
     const double cb = (double)complex_bytes(dtype);
-    const double f = (double)p.n_cached / ((double)p.n_blk * p.n_blk);
+    const double f = (double)p.covered_blocks / ((double)p.n_blk * p.n_blk);   // entries served from the cache
     const double entries = (double)D * (double)D;
-    c.t_cached = f * entries * cb / kBwRead;
+    c.cached_fraction = f;
+    c.t_cached = c.cache_bytes / kBwRead;
     if (k == 1) {
         // generations: one per mirrored pair, one per one-sided entry, ~half of a diagonal block
         double gens = 0.0;
@@ -232,10 +273,11 @@ Candidate evaluate_candidate(int64_t D, int dtype, int k, int B, int cached_per_
     } else {
         c.t_proc = (1.0 - f) * entries / gen_entries_per_s(dtype, k);
     }
-    int launches = 1 + (p.n_cached > 0) + (p.n_cached < (int64_t)p.n_blk * p.n_blk);
+    int launches = 1 + (p.n_cached > 0) + (p.covered_blocks < (int64_t)p.n_blk * p.n_blk);
     c.t_reduce = (double)p.n_slots * 0.6 * D * k * cb / kBwRead;
     c.t_apply = c.t_cached + c.t_proc + c.t_reduce + launches * kLaunch;   // Eq. 32 (not overlapped)
-    c.t_fill = f * entries / gen_entries_per_s(dtype, 0) + f * entries * cb / kBwWrite;
+    const double stored = c.cache_bytes / cb;
+    c.t_fill = stored / gen_entries_per_s(dtype, 0) + c.cache_bytes / kBwWrite;
     c.t_job = (double)std::max<int64_t>(n_applies, 1) * c.t_apply + c.t_fill;
     c.flops = 8.0 * entries * k;                                            // F_mv, Eq. 13
     return c;
@@ -245,6 +287,7 @@ static void candidate_json(std::string& s, const Candidate& c)
 {
     appendf(s, "{\"mode\":\"%s\",\"B\":%d,\"n_blk\":%d,\"cached_blocks\":%lld,\"cached_per_row\":%d,",
             mode_name(c.mode), c.B, c.n_blk, (long long)c.n_cached, c.cached_per_row);
+    appendf(s, "\"cached_fraction\":%.6g,", c.cached_fraction);
     appendf(s, "\"cache_bytes\":%.0f,\"work_bytes\":%.0f,\"total_bytes\":%.0f,\"feasible\":%s,",
             c.cache_bytes, c.work_bytes, c.cache_bytes + c.work_bytes, c.feasible ? "true" : "false");
     appendf(s, "\"model_apply_s\":%.6g,\"model_cached_s\":%.6g,\"model_proc_s\":%.6g,\"model_fill_s\":%.6g,"
@@ -265,22 +308,30 @@ int enumerate_candidates(int64_t D, int dtype, int k, int mode, int B_req, int64
     for (int B : Bs) {
         const int N = (int)(D / B);
         // cache budget -> cached blocks per row (Eq. 27 with full blocks; rows kept balanced)
-        auto fits = [&](int c) {
-            Candidate t = evaluate_candidate(D, dtype, k, B, c, n_applies, sm_count);
+        auto fits = [&](int c, bool pairs) {
+            Candidate t = evaluate_candidate(D, dtype, k, B, c, pairs, n_applies, sm_count);
             return t.cache_bytes + t.work_bytes <= budget_bytes;
         };
-        std::vector<int> cs;
-        if (mode == MFH_MODE_AUTO || mode == MFH_MODE_PROCEDURAL) cs.push_back(0);
-        if (mode == MFH_MODE_AUTO || mode == MFH_MODE_FULL) cs.push_back(N);
+        std::vector<std::pair<int, bool>> cs;   // (cached_per_row or band offsets, pairs)
+        if (mode == MFH_MODE_AUTO || mode == MFH_MODE_PROCEDURAL) cs.push_back({0, false});
+        if (mode == MFH_MODE_AUTO || mode == MFH_MODE_FULL) cs.push_back({N, false});
+        if ((mode == MFH_MODE_AUTO || mode == MFH_MODE_PAIRS) && k == 1 && B % (dtype == MFH_C128 ? 32 : 64) == 0) {
+            // Hermitian pair cache: the largest number of block diagonals that fits (Eq. 27 over
+            // canonical pairs)
+            int c = pair_full_offsets(N);
+            while (c > 0 && !fits(c, true)) --c;
+            if (c > 0) cs.push_back({c, true});
+            else if (mode == MFH_MODE_PAIRS) cs.push_back({1, true});   // reported as infeasible
+        }
         if (mode == MFH_MODE_AUTO || mode == MFH_MODE_PARTIAL) {
             double room = budget_bytes - (double)fixed_work_bytes(D, dtype, k) - 3.0 * D * k * cb;
             int c = (int)std::floor(room / ((double)B * B * cb * N));
             c = std::min(c, N - 1);
-            while (c > 0 && !fits(c)) --c;
-            if (c > 0) cs.push_back(c);
+            while (c > 0 && !fits(c, false)) --c;
+            if (c > 0) cs.push_back({c, false});
         }
-        for (int c : cs) {
-            Candidate cand = evaluate_candidate(D, dtype, k, B, c, n_applies, sm_count);
+        for (auto [c, pairs] : cs) {
+            Candidate cand = evaluate_candidate(D, dtype, k, B, c, pairs, n_applies, sm_count);
             cand.feasible = (cand.cache_bytes + cand.work_bytes <= budget_bytes);   // Eq. 18
             if (k > 1 && c > 0) cand.feasible = false;   // cached multi-vector kernel: not built yet
             out.push_back(cand);

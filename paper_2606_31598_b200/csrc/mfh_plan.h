@@ -12,6 +12,8 @@ struct Plan;
 struct Candidate {
     int B = 0, n_blk = 0, mode = 0, cached_per_row = 0;
     int64_t n_cached = 0;
+    bool pairs = false;                                  // Hermitian pair cache
+    double cached_fraction = 0;                          // share of the D^2 entries served from the cache
     double cache_bytes = 0, work_bytes = 0;              // M_op, M_work (Eq. 14-17)
     double t_cached = 0, t_proc = 0, t_reduce = 0;       // seconds per apply, by part
     double t_apply = 0, t_fill = 0, t_job = 0, flops = 0;
@@ -21,8 +23,9 @@ struct Candidate {
 
 void choose_tiling(int B, int n_blk, int n_pairs, int sm_count, int& R, int& Q);
 void build_tables(Plan& p, int64_t D, int dtype, int sm_count);
-Candidate evaluate_candidate(int64_t D, int dtype, int k, int B, int cached_per_row, int64_t n_applies,
-                             int sm_count);
+Candidate evaluate_candidate(int64_t D, int dtype, int k, int B, int cached_per_row, bool pairs,
+                             int64_t n_applies, int sm_count);
+int pair_full_offsets(int n_blk);
 int enumerate_candidates(int64_t D, int dtype, int k, int mode, int B_req, int64_t n_applies,
                          double budget_bytes, int sm_count, std::vector<Candidate>& out);
 std::string plan_json(int64_t D, int dtype, int k, int64_t n_applies, double budget, int measured,

@@ -342,10 +342,10 @@ int launch_proc_single(mfh_handle h, const void* psi, cudaStream_t st)
 
 // --------------------------------------------------------------------------------------------
 // Fused generate-and-apply, k vectors (coupling scans, Eq. 12): every V entry is
-// generated ONCE per apply and multiplied into all k columns.  One-sided: lane = row, the CTA
-// owns 32W rows over all uncached column blocks, the psi rows of a column chunk are staged in
-// shared memory and read as broadcasts; k accumulators per lane stay in registers, so the
-// result is written once with no partial sums over m.
+// generated ONCE per apply and multiplied into all k columns.  One-sided: lane = row, a CTA owns
+// 32W rows x one uncached column block m (blockIdx.y), the psi rows of a column chunk are staged
+// in shared memory and read as broadcasts; k accumulators per lane stay in registers and go to
+// the partial slot of column block m (added in index order by the reduce kernel).
 // --------------------------------------------------------------------------------------------
 template <typename T> struct MultiParams {
     GenArgs<T> G;
@@ -372,8 +372,9 @@ __global__ void __launch_bounds__(32 * W) proc_multi_kernel(const MultiParams<T>
 #pragma unroll
     for (int v = 0; v < KT; ++v) acc[v] = CT{T(0), T(0)};
 
-    for (int m = 0; m < P.n_blk; ++m) {
-        if (P.cache_slot[n * P.n_blk + m] >= 0) continue;   // cached blocks: streaming kernel
+    const int m = blockIdx.y;
+    if (P.cache_slot[n * P.n_blk + m] != -1) return;   // cached block: the streaming kernel covers it
+    {
         for (int c0 = 0; c0 < P.B; c0 += CH) {
             const uint32_t j0 = (uint32_t)m * P.B + c0;
             __syncthreads();
@@ -397,7 +398,7 @@ __global__ void __launch_bounds__(32 * W) proc_multi_kernel(const MultiParams<T>
             }
         }
     }
-    CT* dst = P.work + ((size_t)P.slot_multi * P.D + i) * k;
+    CT* dst = P.work + ((size_t)(P.slot_multi + m) * P.D + i) * k;
 #pragma unroll
     for (int v = 0; v < KT; ++v)
         if (v < k) dst[v] = acc[v];
@@ -421,9 +422,9 @@ static int launch_proc_multi_t(mfh_handle h, const void* psi, cudaStream_t st)
     const size_t smem = (size_t)Gen<T>::TAB_BYTES + 32 * KT * sizeof(CT);
     // 32W rows per CTA must divide B; prefer 128-row CTAs, fall back to one warp.
     if (p.B % 128 == 0)
-        proc_multi_kernel<T, KT, 4><<<(unsigned)(h->D / 128), 128, smem, st>>>(P);
+        proc_multi_kernel<T, KT, 4><<<dim3((unsigned)(h->D / 128), p.n_blk), 128, smem, st>>>(P);
     else
-        proc_multi_kernel<T, KT, 1><<<(unsigned)(h->D / 32), 32, smem, st>>>(P);
+        proc_multi_kernel<T, KT, 1><<<dim3((unsigned)(h->D / 32), p.n_blk), 32, smem, st>>>(P);
     MFH_CUDA_CHECK(cudaGetLastError());
     return MFH_OK;
 }

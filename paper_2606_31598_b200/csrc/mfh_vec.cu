@@ -10,43 +10,93 @@ struct LamArr {
     double v[MFH_MAX_K];
 };
 
-// phi[i][v] = h0_i psi[i][v] + lambda_v * sum_{valid slots s} work[s][i][v]; slots are added in
-// index order, so the result does not depend on CTA scheduling (no atomics).
-template <typename T>
+// phi[i][v] = h0_i psi[i][v] + lambda_v * sum_{valid slots s} work[s][i][v]; the valid slots of a
+// block row come as a compact ascending list.  A CTA handles 64 consecutive elements with 4 thread
+// groups: group g adds the g-th quarter of the list (four loads in flight), the quarters are
+// combined in the order 0..3 through shared memory: a fixed summation order that does not depend
+// on CTA scheduling (no atomics).  Needs B*k to be a multiple of 64 so that the 64 elements of a
+// CTA share one block row; the launcher falls back to 1 group x 256 elements otherwise.
+constexpr int RED_E = 64, RED_G = 4;
+
+template <typename T, int G>
 __global__ void __launch_bounds__(256) reduce_kernel(int64_t D, int32_t B, int32_t k, int32_t n_slots,
-                                                     const uint8_t* __restrict__ slot_valid,
+                                                     const int32_t* __restrict__ slot_list,
                                                      const typename Cplx<T>::type* __restrict__ work,
                                                      const T* __restrict__ h0,
                                                      const typename Cplx<T>::type* __restrict__ psi,
                                                      typename Cplx<T>::type* __restrict__ phi, LamArr lam)
 {
     using CT = typename Cplx<T>::type;
+    constexpr int EPB = 256 / G;                       // elements per CTA
+    __shared__ double part[G][EPB][2];
     const int64_t total = D * k;
-    for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < total;
-         e += (int64_t)gridDim.x * blockDim.x) {
-        const int64_t i = e / k;
-        const int v = (int)(e - i * k);
-        const uint8_t* valid = slot_valid + (size_t)(i / B) * n_slots;
+    const int ex = threadIdx.x % EPB, g = threadIdx.x / EPB;
+    for (int64_t e0 = (int64_t)blockIdx.x * EPB; e0 < total; e0 += (int64_t)gridDim.x * EPB) {
+        const int64_t e = e0 + ex;
+        const bool live = e < total;
+        const int64_t i = live ? e / k : 0;
+        const int32_t* list = slot_list + (size_t)(i / B) * (n_slots + 1);   // [count, slots...]
+        const int cnt = list[0];
+        const int chunk = (cnt + G - 1) / G;
+        int t = g * chunk;
+        const int t_end = live ? min(cnt, t + chunk) : 0;
         double sr = 0.0, si = 0.0;
-        for (int s = 0; s < n_slots; ++s) {
-            if (valid[s]) {
-                const CT x = work[(size_t)s * total + e];
-                sr += (double)x.x;
-                si += (double)x.y;
+        for (; t + 4 <= t_end; t += 4) {
+            const CT x0 = work[(size_t)list[1 + t] * total + e];
+            const CT x1 = work[(size_t)list[2 + t] * total + e];
+            const CT x2 = work[(size_t)list[3 + t] * total + e];
+            const CT x3 = work[(size_t)list[4 + t] * total + e];
+            sr += (double)x0.x; si += (double)x0.y;
+            sr += (double)x1.x; si += (double)x1.y;
+            sr += (double)x2.x; si += (double)x2.y;
+            sr += (double)x3.x; si += (double)x3.y;
+        }
+        for (; t < t_end; ++t) {
+            const CT x = work[(size_t)list[1 + t] * total + e];
+            sr += (double)x.x;
+            si += (double)x.y;
+        }
+        if (G > 1) {
+            part[g][ex][0] = sr;
+            part[g][ex][1] = si;
+            __syncthreads();
+            if (g == 0)
+#pragma unroll
+                for (int gg = 1; gg < G; ++gg) {
+                    sr += part[gg][ex][0];
+                    si += part[gg][ex][1];
+                }
+        }
+        if (g == 0 && live) {
+            const int v = (int)(e - i * k);
+            double outr = lam.v[v] * sr, outi = lam.v[v] * si;
+            if (h0) {
+                const CT p = psi[e];
+                const double d = (double)h0[i];
+                outr = fma(d, (double)p.x, outr);
+                outi = fma(d, (double)p.y, outi);
             }
+            CT o;
+            o.x = (T)outr;
+            o.y = (T)outi;
+            phi[e] = o;
         }
-        double outr = lam.v[v] * sr, outi = lam.v[v] * si;
-        if (h0) {
-            const CT p = psi[e];
-            const double d = (double)h0[i];
-            outr = fma(d, (double)p.x, outr);
-            outi = fma(d, (double)p.y, outi);
-        }
-        CT o;
-        o.x = (T)outr;
-        o.y = (T)outi;
-        phi[e] = o;
+        if (G > 1) __syncthreads();
     }
+}
+
+template <typename T, int G>
+static int launch_reduce_t(mfh_handle h, const void* psi, void* phi, const LamArr& lam, cudaStream_t st)
+{
+    using CT = typename Cplx<T>::type;
+    const Plan& p = h->plan;
+    const int64_t total = h->D * p.k;
+    const int epb = 256 / G;
+    const int blocks = (int)std::min<int64_t>((total + epb - 1) / epb, (int64_t)h->sm_count * 8);
+    reduce_kernel<T, G><<<blocks, 256, 0, st>>>(h->D, p.B, p.k, std::max(p.n_slots, 1), h->d_slot_list,
+                                                 (const CT*)h->d_work, (const T*)h->d_h0, (const CT*)psi, (CT*)phi, lam);
+    MFH_CUDA_CHECK(cudaGetLastError());
+    return MFH_OK;
 }
 
 int launch_reduce(mfh_handle h, const void* psi, void* phi, const double* lambdas, cudaStream_t st)
@@ -54,18 +104,10 @@ int launch_reduce(mfh_handle h, const void* psi, void* phi, const double* lambda
     const Plan& p = h->plan;
     LamArr lam;
     for (int v = 0; v < MFH_MAX_K; ++v) lam.v[v] = (v < p.k) ? (lambdas ? lambdas[v] : h->lambda) : 0.0;
-    const int64_t total = h->D * p.k;
-    const int blocks = (int)std::min<int64_t>((total + 255) / 256, (int64_t)h->sm_count * 8);
+    const bool split = ((int64_t)p.B * p.k) % RED_E == 0 && p.n_slots >= 16;
     if (h->dtype == MFH_C128)
-        reduce_kernel<double><<<blocks, 256, 0, st>>>(h->D, p.B, p.k, p.n_slots, h->d_slot_valid,
-                                                       (const double2*)h->d_work, (const double*)h->d_h0,
-                                                       (const double2*)psi, (double2*)phi, lam);
-    else
-        reduce_kernel<float><<<blocks, 256, 0, st>>>(h->D, p.B, p.k, p.n_slots, h->d_slot_valid,
-                                                      (const float2*)h->d_work, (const float*)h->d_h0,
-                                                      (const float2*)psi, (float2*)phi, lam);
-    MFH_CUDA_CHECK(cudaGetLastError());
-    return MFH_OK;
+        return split ? launch_reduce_t<double, RED_G>(h, psi, phi, lam, st) : launch_reduce_t<double, 1>(h, psi, phi, lam, st);
+    return split ? launch_reduce_t<float, RED_G>(h, psi, phi, lam, st) : launch_reduce_t<float, 1>(h, psi, phi, lam, st);
 }
 
 // ---- Chebyshev -------------------------------------------------------------------------------

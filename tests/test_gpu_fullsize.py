@@ -55,6 +55,24 @@ def test_c2_full_cache_sampled_rows_and_cached_equals_procedural():
     assert rel_l2(phi, phi_p) <= 1e-13                      # caching is not an approximation
 
 
+def test_c2_pair_cache_sampled_rows():
+    # NEXT-1: the same operator from half the bytes (34.9 GB instead of 68.7 GB)
+    c = CONFIGS["C2"]
+    D, B = c["D"], c["B"]
+    if free_bytes() < 40e9:
+        pytest.skip("needs 35 GB of free HBM")
+    psi = make_psi(D, c["psi_seed"])
+    h = mfh.Hamiltonian(D, B, c["seed"], "c128")
+    plan = h.plan("pairs", n_applies_hint=100)
+    N = D // B
+    assert plan["chosen"]["mode"] == "pairs" and plan["chosen"]["cache_bytes"] == N * (N + 1) // 2 * B * B * 16
+    phi = h.apply(to_dev(psi)).cpu().numpy()
+    h.destroy()
+    rows = sample_rows(D, 250)
+    ref = oracle.apply(D, B, c["seed"], psi, rows=rows)
+    assert rel_l2(phi[rows], ref) <= 1e-11
+
+
 def test_c3_scan_sampled_rows():
     c = CONFIGS["C3"]
     D, B, k = c["D"], c["B"], c["k"]

@@ -100,7 +100,8 @@ def test_c1_procedural_vs_oracle_and_dense():
 
 
 @pytest.mark.parametrize("mode,budget", [("procedural", 0), ("full", 0), ("partial", 12e6),
-                                         ("partial", 30e6), ("partial", 60e6)])
+                                         ("partial", 30e6), ("partial", 60e6), ("pairs", 0), ("pairs", 12e6),
+                                         ("pairs", 20e6), ("pairs", 30e6)])
 @pytest.mark.parametrize("dtype", ["c128", "c64"])
 def test_modes_agree_with_oracle(mode, budget, dtype):
     D, B = 2048, 256          # 8x8 blocks of 1 MiB (c128): budgets cache ~1..6 blocks per row
@@ -123,11 +124,26 @@ def test_partition_invariance_and_ragged_shapes(D, B):
     assert rel_l2(phi, ref) <= TOL["c128"]
 
 
+@pytest.mark.parametrize("D,B", [(32, 32), (96, 32), (1024, 1024), (3072, 1024), (2048, 64), (1536, 512)])
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+def test_pair_cache_ragged_shapes(D, B, dtype):
+    # Hermitian pair cache: one stored block serves (n,m) and (m,n); odd and even N_blk,
+    # a single block, the smallest block size of each dtype
+    if dtype == "c64" and B % 64:
+        pytest.skip("c64 pair cache needs B % 64 == 0 (two entries per 128-bit load)")
+    psi = make_psi(D, 23, dtype=dtype)
+    phi, plan, h = gpu_apply(D, B, 77, psi, dtype=dtype, mode="pairs")
+    ch = plan["chosen"]
+    N = D // B
+    assert ch["mode"] == "pairs" and ch["cached_blocks"] == N * (N + 1) // 2 and ch["cached_fraction"] == 1.0
+    assert rel_l2(phi, oracle.apply(D, B, 77, psi)) <= TOL[dtype]
+
+
 def test_apply_is_deterministic_and_repeatable():
     import torch
     D, B = 4096, 512
     psi = to_dev(make_psi(D, 1))
-    for mode, budget in [("procedural", 0), ("partial", int(150e6))]:
+    for mode, budget in [("procedural", 0), ("partial", int(150e6)), ("pairs", 0), ("pairs", int(100e6))]:
         h = mfh.Hamiltonian(D, B, 9, "c128")
         h.plan(mode, hbm_budget_bytes=budget)
         a = h.apply(psi).clone()
