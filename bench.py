@@ -29,7 +29,9 @@ if ROOT not in sys.path:
 
 import numpy as np  # noqa: E402
 
-from paper_2606_31598_b200.inputs import CONFIGS, lambda_grid, make_psi, sample_rows  # noqa: E402
+from paper_2606_31598_b200.inputs import CONFIGS, VARIANTS, lambda_grid, make_psi, sample_rows  # noqa: E402
+
+ALL = dict(CONFIGS, **VARIANTS)
 
 METRIC = "matrix_entries_per_s"
 UNIT = "entries/s"
@@ -125,7 +127,7 @@ def run_reference(args, cfg_name: str):
     if rank != 0:
         return
     import oracle
-    cfg = CONFIGS[cfg_name]
+    cfg = ALL[cfg_name]
     D = cfg["D"]
     psi = make_psi(D, cfg["psi_seed"], k=cfg["k"], dtype=cfg["dtype"])
     n = max(64, min(D, int(2.0e8 / D)))          # ~2e8 entries per step: a few seconds on 8 cores
@@ -190,7 +192,7 @@ def time_steps(torch, fn, steps: int, flush=None):
 
 
 def measure_config(torch, mfh, name: str, steps: int, warmup: int, with_e2e: bool, barrier=None):
-    cfg = CONFIGS[name]
+    cfg = ALL[name]
     D, k = cfg["D"], cfg["k"]
     psi_np = make_psi(D, cfg["psi_seed"], k=k, dtype=cfg["dtype"])
     lam = lambda_grid(k) if k > 1 else None
@@ -242,31 +244,40 @@ def measure_config(torch, mfh, name: str, steps: int, warmup: int, with_e2e: boo
 
 
 def roofline_for(res: dict, hbm_gbs: float, peak_src: str) -> dict:
+    """Roofline of the dominant kernel of one apply."""
     cfg = res["cfg"]
     D, k = cfg["D"], cfg["k"]
-    cb = 16 if cfg["dtype"] == "c128" else 8
     kern = res["kernel_ms"]
     if kern["cached"] >= kern["procedural"]:
-        # HBM-bound cached streaming: algorithmic bytes = cached entries * bytes per entry
-        cached_entries = res["plan"]["cached_blocks"] * cfg["B"] ** 2
-        gbs = cached_entries * cb / (kern["cached"] * 1e-3) / 1e9
-        return {"kernel": "cached_kernel", "bound": "hbm", "achieved": gbs, "peak": hbm_gbs, "unit": "GB/s",
-                "frac": gbs / hbm_gbs, "traffic": None, "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": cached_entries * cb, "kernel_ms": kern["cached"],
+        # HBM-bound cached streaming: algorithmic bytes = stored entries * bytes per entry
+        nbytes = res["plan"]["cache_bytes"]
+        gbs = nbytes / (kern["cached"] * 1e-3) / 1e9
+        name = "cached_pairs_kernel" if res["plan"]["mode"] == "pairs" else "cached_kernel"
+        return {"kernel": name, "bound": "hbm", "achieved": gbs, "peak": hbm_gbs, "unit": "GB/s",
+                "frac": gbs / hbm_gbs, "traffic": NCU_TRAFFIC.get((name, cfg["D"])), "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": nbytes, "kernel_ms": kern["cached"],
                 "share_of_step": kern["cached"] / max(kern["total"], 1e-9)}
     # ALU-bound fused generate-and-apply: unit = matrix entries applied per second by that kernel
-    entries = (D * D - res["plan"]["cached_blocks"] * cfg["B"] ** 2)
+    entries = D * D * (1.0 - res["plan"]["cached_fraction"])
     rate = entries / (kern["procedural"] * 1e-3)
-    peak = PROC_PEAK[cfg["dtype"]]["k1" if k == 1 else "kN"]
+    key = (cfg["dtype"], "k1" if k == 1 else "kN")
+    peak = ISSUE_LANES_PER_S / INSTR_PER_ENTRY[key]
     return {"kernel": "proc_single_kernel" if k == 1 else "proc_multi_kernel", "bound": "alu",
             "achieved": rate / 1e9, "peak": peak / 1e9, "unit": "Gentries/s", "frac": rate / peak,
-            "traffic": None, "peak_source": "DESIGN.md 'ALU roofline' (FP64/FP32 pipe instruction count at max clock)",
+            "traffic": None, "instr_per_entry": INSTR_PER_ENTRY[key],
+            "peak_source": "issue-slot bound: 148 SMs x 4 schedulers x 32 lanes x 1.965 GHz / SASS instructions "
+                           "per matrix entry (DESIGN.md 6.2/6.3)",
             "kernel_ms": kern["procedural"], "share_of_step": kern["procedural"] / max(kern["total"], 1e-9)}
 
 
-# ALU ceilings in matrix entries/s derived in DESIGN.md ("ALU roofline") from the SASS instruction
-# count per generated entry and the pipe widths at 1965 MHz.
-PROC_PEAK = {"c128": {"k1": 3.7e11, "kN": 1.0e11}, "c64": {"k1": 1.5e12, "kN": 3.0e11}}
+# ALU ceiling (DESIGN.md 6.2): every SM issues at most 4 warp instructions per clock.  Instructions
+# per matrix entry are counted in the SASS of the inner loops (cuobjdump; the two-sided c128 loop
+# spends 92 per generated pair = 46 per entry; the c64 k=16 loop 134 per entry).
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full captures
+# (profiles/r01_*_ncu_full*.md), keyed by (kernel, D).
+NCU_TRAFFIC = {("cached_kernel", 65536): 68.730302e9 + 4.515584e6}
+ISSUE_LANES_PER_S = 148 * 4 * 32 * 1.965e9
+INSTR_PER_ENTRY = {("c128", "k1"): 46.0, ("c128", "kN"): 150.0, ("c64", "k1"): 40.0, ("c64", "kN"): 134.0}
 
 
 def aggregate(dist, local_ms: float, local_units: float, device=None):
@@ -287,7 +298,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--workload", default="C2", choices=sorted(CONFIGS))
+    ap.add_argument("--workload", default="C2", choices=sorted(ALL))
     ap.add_argument("--no-extra", action="store_true", help="skip the other configs' side measurements")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -329,7 +340,7 @@ def main():
 
     extras = {}
     if rank == 0 and world == 1 and not args.no_extra:
-        for name, st in (("C1", 20), ("C3", 5), ("C4", 3)):
+        for name, st in (("C1", 20), ("C3", 5), ("C4", 3), ("C2-pairs", 10), ("C5", 3), ("C5-pairs", 5)):
             if name == args.workload:
                 continue
             try:
@@ -337,6 +348,7 @@ def main():
                 rf = roofline_for(r, hbm_gbs, peak_src)
                 c = r["cfg"]
                 extras[name] = {"workload": workload_config(name, c)["workload"], "steps": st,
+                                "plan": {kk: r["plan"][kk] for kk in ("mode", "B", "cached_fraction", "cache_bytes")},
                                 "ms_per_apply": r["ms_per_step"], "applies_per_s": 1e3 / r["ms_per_step"],
                                 "matrix_entries_per_s": c["D"] ** 2 / (r["ms_per_step"] * 1e-3),
                                 "kernel_ms": r["kernel_ms"], "roofline": rf, "plan_s": r["plan_s"]}

@@ -26,6 +26,13 @@ CONFIGS = {
 }
 
 
+# The same operators from the Hermitian pair cache: side measurements only.
+VARIANTS = {
+    "C2-pairs": dict(CONFIGS["C2"], mode="pairs"),
+    "C5-pairs": dict(CONFIGS["C5"], mode="pairs"),
+}
+
+
 def make_psi(D: int, seed: int, k: int = 1, dtype: str = "c128") -> np.ndarray:
     """Normalised random complex vector(s): shape [D] for k == 1, else [D, k] row-major."""
     cols = []
