@@ -151,13 +151,17 @@ template <> struct Gen<float> {
     __device__ __forceinline__ static void normals(const GenTabF*, const GenConstF& gc, uint32_t x0,
                                                    uint32_t x1, float& a, float& b)
     {
+        // .ftz SFU forms: no denormal fix-up branches (u1 >= 2^-33, L >= 0, |turn| <= 1/2)
         const float u1 = fmaf((float)x0, 0x1p-32f, 0x1p-33f);
-        const float L = gc.neg_k2_ln2 * __log2f(u1);
-        float rad;
+        float lg, rad, cs, sn;
+        asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(lg) : "f"(u1));
+        const float L = gc.neg_k2_ln2 * lg;
         asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(rad) : "f"(L));
         const float ang = fmaf((float)(int32_t)x1, 0x1.921fb6p-30f, 0x1.921fb6p-31f);   // 2 pi (x1 + 1/2) 2^-32
-        a = rad * __cosf(ang);
-        b = rad * __sinf(ang);
+        asm("cos.approx.ftz.f32 %0, %1;" : "=f"(cs) : "f"(ang));
+        asm("sin.approx.ftz.f32 %0, %1;" : "=f"(sn) : "f"(ang));
+        a = rad * cs;
+        b = rad * sn;
     }
 };
 
@@ -201,6 +205,18 @@ __device__ __forceinline__ void entry_upper(const GenArgs<T>& G, const typename 
     uint32_t x0, x1;
     pair_words(G.K, i, j, x0, x1);
     Gen<T>::normals(tab, G.gc, x0, x1, hr, hi);
+}
+
+// Entry for a pair known to satisfy i > j: conjugate of the (j,i) entry.
+template <typename T>
+__device__ __forceinline__ void entry_lower(const GenArgs<T>& G, const typename Gen<T>::Tab* tab, uint32_t i,
+                                            uint32_t j, T& hr, T& hi)
+{
+    uint32_t x0, x1;
+    pair_words(G.K, j, i, x0, x1);
+    T b;
+    Gen<T>::normals(tab, G.gc, x0, x1, hr, b);
+    hi = -b;
 }
 
 }  // namespace mfh

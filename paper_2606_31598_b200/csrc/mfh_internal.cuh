@@ -106,6 +106,8 @@ int launch_fill_cache(mfh_handle h, cudaStream_t st);
 int launch_h0(mfh_handle h, void* out, cudaStream_t st);
 int launch_proc_single(mfh_handle h, const void* psi, cudaStream_t st);
 int launch_proc_multi(mfh_handle h, const void* psi, cudaStream_t st);
+bool tc_multi_supported(mfh_handle h);                                   // mfh_tc.cu
+int launch_proc_multi_tc(mfh_handle h, const void* psi, cudaStream_t st);
 int launch_cached(mfh_handle h, const void* psi, cudaStream_t st);
 int launch_cached_pairs(mfh_handle h, const void* psi, cudaStream_t st);
 int launch_reduce(mfh_handle h, const void* psi, void* phi, const double* lambdas_host, cudaStream_t st);

@@ -2,6 +2,7 @@
 // H0 diagonal, and the fused generate-and-apply kernels (single vector with Hermitian reuse,
 // k vectors one-sided).  PAPER.md Eq. 7, Eq. 8, Eq. 11.
 #include <algorithm>
+#include <cstdlib>
 #include "mfh_internal.cuh"
 
 namespace mfh {
@@ -431,6 +432,10 @@ static int launch_proc_multi_t(mfh_handle h, const void* psi, cudaStream_t st)
 
 int launch_proc_multi(mfh_handle h, const void* psi, cudaStream_t st)
 {
+    // complex64, B % 128 == 0: tensor-core kernel (mfh_tc.cu).  MFH_MULTI_FFMA=1 keeps the CUDA-core
+    // kernel for A/B measurements.
+    static const bool force_ffma = getenv("MFH_MULTI_FFMA") != nullptr;
+    if (!force_ffma && tc_multi_supported(h)) return launch_proc_multi_tc(h, psi, st);
     const int k = h->plan.k;
     const bool f64 = (h->dtype == MFH_C128);
     if (k <= 2) return f64 ? launch_proc_multi_t<double, 2>(h, psi, st) : launch_proc_multi_t<float, 2>(h, psi, st);

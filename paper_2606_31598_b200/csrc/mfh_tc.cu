@@ -1,0 +1,317 @@
+// mfh_tc.cu -- k-vector fused generate-and-apply on the 5th-generation tensor cores (complex64).
+//
+// Coupling scans (Eq. 12; BASELINE.json configs[2]): Phi = V Psi for k <= 16 vectors is a
+// genuine dense contraction [128 x 16 columns of V] x [16 x 32] per tile, where the 32 real output
+// columns are (Re Phi_v, Im Phi_v).  Each V entry is generated ONCE in registers (Philox + SFU
+// Box-Muller, mfh_gen.cuh), split into two TF32 words (hi + lo) and written with tcgen05.st straight
+// into TENSOR MEMORY as the A operand (lane = row, column = k index): the matrix never touches
+// shared memory or HBM.  The B operands (psi, split the same way) are 2 KB shared-memory images
+// in the canonical no-swizzle K-major UMMA layout.  One lane issues tcgen05.mma.kind::tf32 (A from
+// TMEM, B from shared memory) with the [128 x 32] fp32 accumulator also in TMEM, so the 64 FFMA
+// per entry of the CUDA-core kernel disappear from the issue slots that bound it.
+// 3xTF32: D += A_hi B_hi + A_hi B_lo + A_lo B_hi (single-pass TF32 gives 2.9e-4 relative L2 and
+// fails the 1e-4 tolerance; measured here: 1.4e-5 on C3, dominated by the tensor core's fp32
+// accumulation over 1024 columns).  Complex arithmetic as two real operand pairs:
+//     [Re Phi | Im Phi] += Re V x [Re Psi | Im Psi]  +  Im V x [-Im Psi | Re Psi].
+// Warp-specialised CTA: 8 generator warps + 1 MMA warp, a 3-stage ring of (A columns in TMEM,
+// B images in shared memory) guarded by mbarriers: generators wait on empty[s] (tcgen05.commit of
+// the MMAs that read the stage), fill it, fence and arrive on full[s]; the MMA warp waits on
+// full[s], issues 12 MMAs and commits.  A CTA owns 128 rows x one column block m; the epilogue
+// reads the accumulator with tcgen05.ld and writes the partial slot of column block m (added in
+// index order by the reduce kernel).
+#include <algorithm>
+#include <cstdlib>
+#include "mfh_internal.cuh"
+
+namespace mfh {
+
+constexpr int TC_GEN_WARPS = 8;               // generator warps; warp 8 builds the B operands and issues the MMAs
+constexpr int TC_THREADS = 32 * (TC_GEN_WARPS + 1);
+constexpr int TC_TP = 128;                    // rows per CTA = MMA M
+constexpr int TC_TQ = 16;                     // columns per tile = two MMA K-steps
+constexpr int TC_N = 32;                      // MMA N: 16 vectors x (re, im)
+constexpr int TC_B_TILE = TC_N * TC_TQ * 4;   // bytes of one B operand image in shared memory (2 KB)
+constexpr int TC_STAGE = 4 * TC_B_TILE;       // B1_hi B1_lo B2_hi B2_lo
+constexpr int TC_STAGES = 3;
+// TMEM columns: [0,32) accumulator; stage s holds the four A images Er_hi Er_lo Ei_hi Ei_lo, 16 columns each
+constexpr int TC_TMEM_COLS = 256;
+constexpr int TC_A_COL0 = TC_N;
+constexpr int TC_A_STAGE_COLS = 4 * TC_TQ;
+constexpr int TC_SBO = (TC_TQ / 4) * 128;     // byte stride between 8-row groups (A) / 8-column groups (B)
+constexpr int TC_LBO = 128;                   // byte stride between the two 16-byte K halves of one MMA
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+// Shared-memory matrix descriptor, K-major, SWIZZLE_NONE: core matrix = 8 rows x 16 bytes.
+__device__ __forceinline__ uint64_t umma_desc(uint32_t addr)
+{
+    return (uint64_t)((addr >> 4) & 0x3fffu) | ((uint64_t)(TC_LBO >> 4) << 16) | ((uint64_t)(TC_SBO >> 4) << 32) |
+           (1ull << 46);
+}
+
+// Instruction descriptor: D = F32, A = B = TF32, both K-major, M = 128, N = 32.
+constexpr uint32_t TC_IDESC = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(TC_N >> 3) << 17) |
+                              ((uint32_t)(TC_TP >> 4) << 24);
+
+// A operand from TMEM (128 lanes x 8 columns), B from shared memory.
+__device__ __forceinline__ void umma_tf32_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b, uint32_t accumulate)
+{
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n\t"
+        "}\n" ::"r"(d_tmem),
+        "r"(a_tmem), "l"(b), "r"(TC_IDESC), "r"(accumulate)
+        : "memory");
+}
+
+// Four consecutive TMEM columns of this thread's lane (warp-collective: lanes 32 (warp % 4) ..).
+__device__ __forceinline__ void tmem_st4(uint32_t taddr, float a, float b, float c, float d)
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" ::"r"(taddr), "r"(__float_as_uint(a)),
+                 "r"(__float_as_uint(b)), "r"(__float_as_uint(c)), "r"(__float_as_uint(d))
+                 : "memory");
+}
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n\t"
+            ".reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t"
+            "}\n"
+            : "=r"(done)
+            : "r"(smem_u32(bar)), "r"(parity)
+            : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint64_t* bar)
+{
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar))
+                 : "memory");
+}
+
+// x = hi + lo with hi = x rounded to the nearest TF32 (integer add + mask: cvt.rna.tf32 costs four
+// instructions with its NaN handling, and no entry is NaN or Inf); lo = x - hi is exact and the tensor
+// core drops its low 13 bits (2^-22 of x).  Plain truncation of hi would bias every product one way.
+__device__ __forceinline__ void split_tf32(float x, float& hi, float& lo)
+{
+    hi = __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xffffe000u);
+    lo = x - hi;
+}
+
+struct TcParams {
+    GenArgs<float> G;
+    int32_t B, n_blk, k, slot_multi;
+    int64_t D;
+    const int32_t* cache_slot;
+    const float2* psi;   // [D][k]
+    float2* work;        // [n_slots][D][k]
+};
+
+// Generator warps (8 x 32 threads).  Per tile of 128 rows x 16 columns a thread produces the two
+// 4-column groups g, g + 2 of row p (8 entries, one 16-byte store per operand image and group) and
+// one (column, vector) element of the four psi images, then one lane per warp arrives on full[s].
+// REL > 0: every entry has i < j (block above the diagonal), REL < 0: i > j, REL == 0: diagonal block.
+template <int REL>
+__device__ __forceinline__ void tc_generate(const TcParams& P, unsigned char* smem, uint64_t* full,
+                                            uint64_t* empty, uint32_t d_tmem, uint32_t i_base, int m)
+{
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int p = tid & (TC_TP - 1), gsel = tid >> 7;
+    const uint32_t i = i_base + p;
+    const uint32_t a_lane = d_tmem + ((uint32_t)(p & ~31) << 16);   // this warp's 32 TMEM lanes: rows 32 (warp % 4) ..
+    const int v = tid & 15, qb = tid >> 4, k = P.k;
+    // psi element (n, q) of a K-major B image: n = v (real part rows) and n = 16 + v (imaginary part rows)
+    const int o_re = ((v & 7) * 16 + (v >> 3) * TC_SBO + (qb >> 2) * 128 + (qb & 3) * 4) / 4;
+    const int o_im = o_re + 2 * TC_SBO / 4;
+    const int n_tiles = P.B / TC_TQ;
+    for (int t = 0; t < n_tiles; ++t) {
+        const int s = t % TC_STAGES, u = t / TC_STAGES;
+        const uint32_t j0 = (uint32_t)m * P.B + t * TC_TQ;
+        const float2 x = (v < k) ? P.psi[(size_t)(j0 + qb) * k + v] : float2{0.f, 0.f};   // consumed after the entries
+        float rh[2][4], rl[2][4], ih[2][4], il[2][4];
+#pragma unroll
+        for (int gg = 0; gg < 2; ++gg)
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const uint32_t j = j0 + 4 * (gsel + 2 * gg) + e;
+                float hr, hi;
+                if (REL > 0) entry_upper<float>(P.G, nullptr, i, j, hr, hi);
+                else if (REL < 0) entry_lower<float>(P.G, nullptr, i, j, hr, hi);
+                else entry_any<float>(P.G, nullptr, i, j, hr, hi);
+                split_tf32(hr, rh[gg][e], rl[gg][e]);
+                split_tf32(hi, ih[gg][e], il[gg][e]);
+            }
+        float prh, prl, pih, pil;
+        split_tf32(x.x, prh, prl);
+        split_tf32(x.y, pih, pil);
+        if (u > 0) mbar_wait(&empty[s], (u - 1) & 1);   // the MMAs that read stage s have completed
+        unsigned char* st = smem + s * TC_STAGE;
+#pragma unroll
+        for (int gg = 0; gg < 2; ++gg) {   // A images: 4 columns of this thread's TMEM lane (= row p) per image
+            const uint32_t ta = a_lane + (uint32_t)(TC_A_COL0 + s * TC_A_STAGE_COLS + 4 * (gsel + 2 * gg));
+            tmem_st4(ta + 0 * TC_TQ, rh[gg][0], rh[gg][1], rh[gg][2], rh[gg][3]);
+            tmem_st4(ta + 1 * TC_TQ, rl[gg][0], rl[gg][1], rl[gg][2], rl[gg][3]);
+            tmem_st4(ta + 2 * TC_TQ, ih[gg][0], ih[gg][1], ih[gg][2], ih[gg][3]);
+            tmem_st4(ta + 3 * TC_TQ, il[gg][0], il[gg][1], il[gg][2], il[gg][3]);
+        }
+        {   // B1 = [Re Psi | Im Psi], B2 = [-Im Psi | Re Psi]
+            float* b = reinterpret_cast<float*>(st);
+            constexpr int BT = TC_B_TILE / 4;
+            b[0 * BT + o_re] = prh;  b[0 * BT + o_im] = pih;     // B1_hi
+            b[1 * BT + o_re] = prl;  b[1 * BT + o_im] = pil;     // B1_lo
+            b[2 * BT + o_re] = -pih; b[2 * BT + o_im] = prh;     // B2_hi
+            b[3 * BT + o_re] = -pil; b[3 * BT + o_im] = prl;     // B2_lo
+        }
+        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy writes -> async proxy (UMMA)
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&full[s]);
+    }
+}
+
+// MMA warp: waits for the 8 generator warps, issues the 12 MMAs of the tile from one lane and commits
+// them onto empty[s] (the arrival that lets the generators overwrite the stage).
+__device__ __forceinline__ void tc_mma_warp(const TcParams& P, unsigned char* smem, uint64_t* full, uint64_t* empty,
+                                            uint64_t* done, uint32_t d_tmem)
+{
+    const int lane = threadIdx.x & 31;
+    const int n_tiles = P.B / TC_TQ;
+    for (int t = 0; t < n_tiles; ++t) {
+        const int s = t % TC_STAGES, u = t / TC_STAGES;
+        mbar_wait(&full[s], u & 1);
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        if (lane == 0) {
+            const uint32_t b0 = smem_u32(smem + s * TC_STAGE);
+            const uint32_t a0 = d_tmem + (uint32_t)(TC_A_COL0 + s * TC_A_STAGE_COLS);
+#pragma unroll
+            for (int ks = 0; ks < TC_TQ / 8; ++ks) {
+                const uint32_t ko = ks * 2 * TC_LBO;
+                const uint32_t er_h = a0 + 0 * TC_TQ + 8 * ks, er_l = a0 + 1 * TC_TQ + 8 * ks;
+                const uint32_t ei_h = a0 + 2 * TC_TQ + 8 * ks, ei_l = a0 + 3 * TC_TQ + 8 * ks;
+                const uint64_t b1_h = umma_desc(b0 + 0 * TC_B_TILE + ko), b1_l = umma_desc(b0 + 1 * TC_B_TILE + ko);
+                const uint64_t b2_h = umma_desc(b0 + 2 * TC_B_TILE + ko), b2_l = umma_desc(b0 + 3 * TC_B_TILE + ko);
+                umma_tf32_ts(d_tmem, er_h, b1_h, (t | ks) != 0);
+                umma_tf32_ts(d_tmem, er_h, b1_l, 1);
+                umma_tf32_ts(d_tmem, er_l, b1_h, 1);
+                umma_tf32_ts(d_tmem, ei_h, b2_h, 1);
+                umma_tf32_ts(d_tmem, ei_h, b2_l, 1);
+                umma_tf32_ts(d_tmem, ei_l, b2_h, 1);
+            }
+            umma_commit(&empty[s]);                            // arrives when every MMA issued so far has completed
+            if (t == n_tiles - 1) umma_commit(done);
+        }
+        __syncwarp();
+    }
+}
+
+__global__ void __launch_bounds__(TC_THREADS, 2) proc_multi_tc_kernel(const TcParams P)
+{
+    extern __shared__ __align__(128) unsigned char smem[];
+    __shared__ __align__(8) uint64_t full[TC_STAGES], empty[TC_STAGES], done;
+    __shared__ uint32_t s_tmem;
+    const int tid = threadIdx.x, w = tid >> 5;
+    const int m = blockIdx.y;
+    const uint32_t i_base = blockIdx.x * TC_TP;
+    const int n = (int)(i_base / (uint32_t)P.B);
+    if (P.cache_slot[n * P.n_blk + m] != -1) return;   // cached block: not this kernel's
+
+    if (tid == 0) {
+        for (int s = 0; s < TC_STAGES; ++s) {
+            mbar_init(&full[s], TC_GEN_WARPS);
+            mbar_init(&empty[s], 1);
+        }
+        mbar_init(&done, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (w == TC_GEN_WARPS) {   // the MMA warp allocates 32 TMEM columns for the [128 x 32] fp32 accumulator
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&s_tmem)),
+                     "n"(TC_TMEM_COLS)
+                     : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t d_tmem = s_tmem;
+
+    if (w == TC_GEN_WARPS) tc_mma_warp(P, smem, full, empty, &done, d_tmem);
+    else if (n < m) tc_generate<1>(P, smem, full, empty, d_tmem, i_base, m);
+    else if (n > m) tc_generate<-1>(P, smem, full, empty, d_tmem, i_base, m);
+    else tc_generate<0>(P, smem, full, empty, d_tmem, i_base, m);
+
+    if (w < 4) {   // warp w reads TMEM lanes 32w..32w+31: row 32w + lane, 32 columns
+        const int k = P.k;
+        mbar_wait(&done, 0);
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        uint32_t r[32];
+        const uint32_t taddr = d_tmem + ((uint32_t)(32 * w) << 16);
+        asm volatile(
+            "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+            "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+            "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+            : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+              "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]),
+              "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]),
+              "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+            : "r"(taddr)
+            : "memory");
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+        const uint32_t row = i_base + 32 * w + (tid & 31);
+        float2* dst = P.work + ((size_t)(P.slot_multi + m) * P.D + row) * k;
+#pragma unroll
+        for (int vv = 0; vv < 16; ++vv)
+            if (vv < k) dst[vv] = make_float2(__uint_as_float(r[vv]), __uint_as_float(r[16 + vv]));
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (w == TC_GEN_WARPS)
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(d_tmem), "n"(TC_TMEM_COLS) : "memory");
+}
+
+bool tc_multi_supported(mfh_handle h)
+{
+    return h->dtype == MFH_C64 && h->plan.k > 1 && h->plan.k <= 16 && h->plan.B % TC_TP == 0;
+}
+
+int launch_proc_multi_tc(mfh_handle h, const void* psi, cudaStream_t st)
+{
+    const Plan& p = h->plan;
+    TcParams P;
+    P.G.K = make_philox_keys(h->seed);
+    P.G.gc.neg_k2_ln2 = (float)(-0.6931471805599453 / (double)h->D);
+    P.G.tab_global = nullptr;
+    P.B = p.B;
+    P.n_blk = p.n_blk;
+    P.k = p.k;
+    P.slot_multi = p.slot_multi;
+    P.D = h->D;
+    P.cache_slot = h->d_cache_slot;
+    P.psi = (const float2*)psi;
+    P.work = (float2*)h->d_work;
+    const size_t smem = (size_t)TC_STAGES * TC_STAGE;
+    static bool attr_done = false;
+    if (!attr_done) {
+        MFH_CUDA_CHECK(cudaFuncSetAttribute(proc_multi_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_done = true;
+    }
+    proc_multi_tc_kernel<<<dim3((unsigned)(h->D / TC_TP), p.n_blk), TC_THREADS, smem, st>>>(P);
+    MFH_CUDA_CHECK(cudaGetLastError());
+    return MFH_OK;
+}
+
+}  // namespace mfh

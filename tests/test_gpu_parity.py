@@ -187,6 +187,22 @@ def test_scan_multi_vector_vs_oracle(dtype, k):
     assert rel_l2(Phi[:, 0], h0 * Psi[:, 0].astype(np.complex128)) <= (1e-15 if dtype == "c128" else 2e-7)
 
 
+@pytest.mark.parametrize("D,B", [(128, 128), (1024, 128), (3072, 1024), (960, 96), (2048, 64)])
+@pytest.mark.parametrize("k", [16, 3])
+def test_scan_c64_tensor_core_and_cuda_core_shapes(D, B, k):
+    # complex64 k-vector path: B % 128 == 0 runs the tcgen05 kernel (3xTF32, A operand in TMEM),
+    # other block sizes the CUDA-core kernel; a single block (all entries from the general rule),
+    # blocks above and below the diagonal, ragged N_blk
+    Psi = make_psi(D, 31, k=k, dtype="c64")
+    lam = 0.5 + lambda_grid(k)
+    h = mfh.Hamiltonian(D, B, 8, "c64", kind="diag_plus_gue", seed_h0=7)
+    h.plan("procedural", k=k)
+    Phi = h.apply(to_dev(Psi), lambdas=lam).cpu().numpy()
+    ref = oracle.apply_scan(D, B, 8, 7, lam, Psi)
+    for v in range(k):
+        assert rel_l2(Phi[:, v], ref[:, v]) <= TOL["c64"], v
+
+
 def test_multi_vector_equals_single_vector_applies():
     D, B, k = 1024, 256, 4
     Psi = make_psi(D, 21, k=k)
