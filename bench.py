@@ -226,7 +226,7 @@ def measure_config(torch, mfh, name: str, steps: int, warmup: int, with_e2e: boo
         t = h.apply_timed(psi, phi, lambdas=lam)
         for key in kern:
             kern[key] += t[key] / steps
-    out = {"name": name, "cfg": cfg, "plan": info, "plan_s": plan_s, "ms_total": ms, "steps": steps,
+    out = {"name": name, "cfg": cfg, "pipe_rate": mfh.pipe_rate, "plan": info, "plan_s": plan_s, "ms_total": ms, "steps": steps,
            "ms_per_step": ms / steps, "kernel_ms": kern, "psi_np": psi_np,
            "launches_per_apply": info["launches_per_apply"]}
     if with_e2e:
@@ -261,23 +261,35 @@ def roofline_for(res: dict, hbm_gbs: float, peak_src: str) -> dict:
     entries = D * D * (1.0 - res["plan"]["cached_fraction"])
     rate = entries / (kern["procedural"] * 1e-3)
     key = (cfg["dtype"], "k1" if k == 1 else "kN")
-    peak = ISSUE_LANES_PER_S / INSTR_PER_ENTRY[key]
-    return {"kernel": "proc_single_kernel" if k == 1 else "proc_multi_kernel", "bound": "alu",
-            "achieved": rate / 1e9, "peak": peak / 1e9, "unit": "Gentries/s", "frac": rate / peak,
-            "traffic": None, "instr_per_entry": INSTR_PER_ENTRY[key],
-            "peak_source": "issue-slot bound: 148 SMs x 4 schedulers x 32 lanes x 1.965 GHz / SASS instructions "
-                           "per matrix entry (DESIGN.md 6.2/6.3)",
+    issue_peak = ISSUE_LANES_PER_S / INSTR_PER_ENTRY[key]
+    mix = MIX_OF.get(key)
+    if mix is not None:
+        # ceiling measured live on this GPU: synthetic kernel with the inner loop's instruction counts
+        name, entries_per_unit = mix
+        peak = res["pipe_rate"](name) * entries_per_unit
+        src = (f"measured now: mfh_debug_pipe_rates({name}) x {entries_per_unit} entries per unit -- synthetic kernel "
+               "with the per-entry IMAD.WIDE/LOP3/DFMA/MUFU/FFMA counts of the inner loop, no memory traffic "
+               "(DESIGN.md 6.2)")
+    else:
+        peak, src = issue_peak, "issue-slot bound (DESIGN.md 6.2)"
+    kname = "proc_single_kernel" if k == 1 else ("proc_multi_tc_kernel" if cfg["dtype"] == "c64" else "proc_multi_kernel")
+    return {"kernel": kname, "bound": "alu", "achieved": rate / 1e9, "peak": peak / 1e9, "unit": "Gentries/s",
+            "frac": rate / peak, "traffic": None, "peak_source": src,
+            "issue_slot_peak": issue_peak / 1e9, "frac_of_issue_slots": rate / issue_peak,
+            "instr_per_entry": INSTR_PER_ENTRY[key],
             "kernel_ms": kern["procedural"], "share_of_step": kern["procedural"] / max(kern["total"], 1e-9)}
 
 
-# ALU ceiling: every SM issues at most 4 warp instructions per clock.  Instructions
-# per matrix entry are counted in the SASS of the inner loops (cuobjdump; the two-sided c128 loop
-# spends 92 per generated pair = 46 per entry; the c64 k=16 loop 134 per entry).
+# ALU ceilings.  (1) Measured: the library's synthetic instruction-mix kernel.
+# (2) Nominal: every SM issues at most 4 warp instructions per clock; instructions per matrix entry
+# counted in the SASS of the inner loops (cuobjdump): the two-sided c128 loop spends 88 per generated
+# pair = 44 per entry, the c64 tensor-core loop 62 per entry.
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full captures
 # (profiles/r01_*_ncu_full*.md), keyed by (kernel, D).
 NCU_TRAFFIC = {("cached_kernel", 65536): 68.730302e9 + 4.515584e6}
 ISSUE_LANES_PER_S = 148 * 4 * 32 * 1.965e9
-INSTR_PER_ENTRY = {("c128", "k1"): 46.0, ("c128", "kN"): 150.0, ("c64", "k1"): 40.0, ("c64", "kN"): 134.0}
+INSTR_PER_ENTRY = {("c128", "k1"): 44.0, ("c128", "kN"): 150.0, ("c64", "k1"): 40.0, ("c64", "kN"): 62.0}
+MIX_OF = {("c128", "k1"): ("c128_pair", 2), ("c64", "kN"): ("c64_entry", 1)}
 
 
 def aggregate(dist, local_ms: float, local_units: float, device=None):

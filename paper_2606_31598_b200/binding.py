@@ -28,7 +28,7 @@ MODES = {"auto": MFH_MODE_AUTO, "procedural": MFH_MODE_PROCEDURAL, "partial": MF
 # every symbol include/mfh.h declares (tests check that the library exports all of them)
 SYMBOLS = ["mfh_create", "mfh_plan_analytic", "mfh_plan", "mfh_apply", "mfh_apply_host", "mfh_apply_timed",
            "mfh_chebyshev", "mfh_destroy", "mfh_last_error", "mfh_get_plan", "mfh_debug_philox",
-           "mfh_materialize_block", "mfh_debug_h0"]
+           "mfh_materialize_block", "mfh_debug_h0", "mfh_debug_pipe_rates"]
 
 _lib = None
 
@@ -65,6 +65,7 @@ def lib():
     L.mfh_debug_philox.argtypes = [u64, u32, vp, vp, i64, vp, vp]
     L.mfh_materialize_block.argtypes = [vp, i32, i32, vp, vp]
     L.mfh_debug_h0.argtypes = [vp, vp, vp]
+    L.mfh_debug_pipe_rates.argtypes = [i32, ctypes.POINTER(dbl), vp]
     for name in SYMBOLS:
         if name != "mfh_last_error":
             getattr(L, name).restype = ctypes.c_int
@@ -206,3 +207,13 @@ def debug_philox(seed: int, stream_id: int, i, j):
     words = torch.empty((n, 4), dtype=torch.int32, device="cuda")
     _check(lib().mfh_debug_philox(seed, stream_id, i.data_ptr(), j.data_ptr(), n, words.data_ptr(), _stream()))
     return words
+
+
+MIXES = {"c128_pair": 0, "c64_entry": 1, "philox": 2, "dfma31": 3}
+
+
+def pipe_rate(mix: str) -> float:
+    """Units per second of the synthetic instruction-mix kernel (mfh_debug_pipe_rates)."""
+    out = ctypes.c_double(0.0)
+    _check(lib().mfh_debug_pipe_rates(MIXES[mix], ctypes.byref(out), _stream()))
+    return float(out.value)

@@ -35,31 +35,61 @@ inline PhiloxKeys make_philox_keys(uint64_t seed)
     return K;
 }
 
-// Full 4-word output.  In the fused kernels only x0,x1 are consumed and the compiler removes the
-// dead half of the last two rounds (and folds the zero counter words of the first round).
+// 32x32 -> 64 multiply by a Philox constant.  Written as PTX: from the C expression
+// (uint64_t)M * x nvcc emits the IMAD.WIDE plus an extra integer add per product; the wide multiply
+// issues at a quarter of the FP32 rate on sm_100 and is the scarcest pipe of the generator.
+__device__ __forceinline__ void mul_m0(uint32_t x, uint32_t& lo, uint32_t& hi)
+{
+    uint64_t p;
+    asm("mul.wide.u32 %0, %1, 0xD2511F53;" : "=l"(p) : "r"(x));
+    lo = (uint32_t)p;
+    hi = (uint32_t)(p >> 32);
+}
+__device__ __forceinline__ void mul_m1(uint32_t x, uint32_t& lo, uint32_t& hi)
+{
+    uint64_t p;
+    asm("mul.wide.u32 %0, %1, 0xCD9E8D57;" : "=l"(p) : "r"(x));
+    lo = (uint32_t)p;
+    hi = (uint32_t)(p >> 32);
+}
+
+// Full 4-word output (debug export, H0 diagonal).
 __device__ __forceinline__ void philox4x32_10(const PhiloxKeys& K, uint32_t c0, uint32_t c1,
                                               uint32_t c2, uint32_t c3, uint32_t& x0, uint32_t& x1,
                                               uint32_t& x2, uint32_t& x3)
 {
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
-        const uint64_t p0 = (uint64_t)0xD2511F53u * (uint64_t)c0;   // IMAD.WIDE.U32
-        const uint64_t p1 = (uint64_t)0xCD9E8D57u * (uint64_t)c2;
-        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ K.k0[r];    // LOP3
-        const uint32_t n1 = (uint32_t)p1;
-        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ K.k1[r];
-        const uint32_t n3 = (uint32_t)p0;
-        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        uint32_t lo0, hi0, lo1, hi1;
+        mul_m0(c0, lo0, hi0);
+        mul_m1(c2, lo1, hi1);
+        const uint32_t n0 = hi1 ^ c1 ^ K.k0[r];    // LOP3
+        const uint32_t n2 = hi0 ^ c3 ^ K.k1[r];
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
     }
     x0 = c0; x1 = c1; x2 = c2; x3 = c3;
 }
 
-// Words (x0,x1) of the matrix stream for an ordered pair lo <= hi.
+// Words (x0,x1) of the matrix stream for an ordered pair lo <= hi: counter (lo, hi, 0, 0).  The zero
+// counter words remove one multiply from the first round, the unused words x2,x3 one from the last:
+// 18 wide multiplies and 18 three-input xors per call.
 __device__ __forceinline__ void pair_words(const PhiloxKeys& K, uint32_t lo, uint32_t hi,
                                            uint32_t& x0, uint32_t& x1)
 {
-    uint32_t x2, x3;
-    philox4x32_10(K, lo, hi, 0u, 0u, x0, x1, x2, x3);
+    uint32_t lo0, hi0, lo1, hi1;
+    mul_m0(lo, lo0, hi0);                           // round 0: c2 = c3 = 0
+    uint32_t c0 = hi ^ K.k0[0], c1 = 0u, c2 = hi0 ^ K.k1[0], c3 = lo0;
+#pragma unroll
+    for (int r = 1; r < 9; ++r) {
+        mul_m0(c0, lo0, hi0);
+        mul_m1(c2, lo1, hi1);
+        const uint32_t n0 = hi1 ^ c1 ^ K.k0[r];
+        const uint32_t n2 = hi0 ^ c3 ^ K.k1[r];
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+    }
+    mul_m1(c2, lo1, hi1);                           // round 9: only x0, x1 are consumed
+    x0 = hi1 ^ c1 ^ K.k0[9];
+    x1 = lo1;
 }
 
 // ---- Box-Muller normals scaled by s = 1/sqrt(2D):  (s g1, s g2),

@@ -28,13 +28,20 @@ namespace mfh {
 constexpr int TC_GEN_WARPS = 8;               // generator warps; warp 8 builds the B operands and issues the MMAs
 constexpr int TC_THREADS = 32 * (TC_GEN_WARPS + 1);
 constexpr int TC_TP = 128;                    // rows per CTA = MMA M
-constexpr int TC_TQ = 16;                     // columns per tile = two MMA K-steps
+#ifndef MFH_TC_TQ
+#define MFH_TC_TQ 16
+#endif
+#ifndef MFH_TC_MINB
+#define MFH_TC_MINB 2
+#endif
+constexpr int TC_TQ = MFH_TC_TQ;              // columns per tile = TQ/8 MMA K-steps
+constexpr int TC_NG = TC_TQ / 8;              // 4-column groups per generator thread and tile
 constexpr int TC_N = 32;                      // MMA N: 16 vectors x (re, im)
 constexpr int TC_B_TILE = TC_N * TC_TQ * 4;   // bytes of one B operand image in shared memory (2 KB)
 constexpr int TC_STAGE = 4 * TC_B_TILE;       // B1_hi B1_lo B2_hi B2_lo
 constexpr int TC_STAGES = 3;
 // TMEM columns: [0,32) accumulator; stage s holds the four A images Er_hi Er_lo Ei_hi Ei_lo, 16 columns each
-constexpr int TC_TMEM_COLS = 256;
+constexpr int TC_TMEM_COLS = (TC_N + TC_STAGES * 4 * TC_TQ) <= 128 ? 128 : 256;
 constexpr int TC_A_COL0 = TC_N;
 constexpr int TC_A_STAGE_COLS = 4 * TC_TQ;
 constexpr int TC_SBO = (TC_TQ / 4) * 128;     // byte stride between 8-row groups (A) / 8-column groups (B)
@@ -141,10 +148,10 @@ __device__ __forceinline__ void tc_generate(const TcParams& P, unsigned char* sm
     for (int t = 0; t < n_tiles; ++t) {
         const int s = t % TC_STAGES, u = t / TC_STAGES;
         const uint32_t j0 = (uint32_t)m * P.B + t * TC_TQ;
-        const float2 x = (v < k) ? P.psi[(size_t)(j0 + qb) * k + v] : float2{0.f, 0.f};   // consumed after the entries
-        float rh[2][4], rl[2][4], ih[2][4], il[2][4];
+        const float2 x = (v < k && qb < TC_TQ) ? P.psi[(size_t)(j0 + qb) * k + v] : float2{0.f, 0.f};   // consumed after the entries
+        float rh[TC_NG][4], rl[TC_NG][4], ih[TC_NG][4], il[TC_NG][4];
 #pragma unroll
-        for (int gg = 0; gg < 2; ++gg)
+        for (int gg = 0; gg < TC_NG; ++gg)
 #pragma unroll
             for (int e = 0; e < 4; ++e) {
                 const uint32_t j = j0 + 4 * (gsel + 2 * gg) + e;
@@ -161,14 +168,14 @@ __device__ __forceinline__ void tc_generate(const TcParams& P, unsigned char* sm
         if (u > 0) mbar_wait(&empty[s], (u - 1) & 1);   // the MMAs that read stage s have completed
         unsigned char* st = smem + s * TC_STAGE;
 #pragma unroll
-        for (int gg = 0; gg < 2; ++gg) {   // A images: 4 columns of this thread's TMEM lane (= row p) per image
+        for (int gg = 0; gg < TC_NG; ++gg) {   // A images: 4 columns of this thread's TMEM lane (= row p) per image
             const uint32_t ta = a_lane + (uint32_t)(TC_A_COL0 + s * TC_A_STAGE_COLS + 4 * (gsel + 2 * gg));
             tmem_st4(ta + 0 * TC_TQ, rh[gg][0], rh[gg][1], rh[gg][2], rh[gg][3]);
             tmem_st4(ta + 1 * TC_TQ, rl[gg][0], rl[gg][1], rl[gg][2], rl[gg][3]);
             tmem_st4(ta + 2 * TC_TQ, ih[gg][0], ih[gg][1], ih[gg][2], ih[gg][3]);
             tmem_st4(ta + 3 * TC_TQ, il[gg][0], il[gg][1], il[gg][2], il[gg][3]);
         }
-        {   // B1 = [Re Psi | Im Psi], B2 = [-Im Psi | Re Psi]
+        if (qb < TC_TQ) {   // B1 = [Re Psi | Im Psi], B2 = [-Im Psi | Re Psi]
             float* b = reinterpret_cast<float*>(st);
             constexpr int BT = TC_B_TILE / 4;
             b[0 * BT + o_re] = prh;  b[0 * BT + o_im] = pih;     // B1_hi
@@ -219,7 +226,7 @@ __device__ __forceinline__ void tc_mma_warp(const TcParams& P, unsigned char* sm
     }
 }
 
-__global__ void __launch_bounds__(TC_THREADS, 2) proc_multi_tc_kernel(const TcParams P)
+__global__ void __launch_bounds__(TC_THREADS, MFH_TC_MINB) proc_multi_tc_kernel(const TcParams P)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     __shared__ __align__(8) uint64_t full[TC_STAGES], empty[TC_STAGES], done;
