@@ -156,12 +156,12 @@ MFH_API int mfh_debug_h0(mfh_handle h, void* h0_dev, void* stream);
 /* Instruction-mix ceiling of the fused generate-and-apply kernels: times a synthetic
  * kernel that issues, per unit, the same instruction counts as one generated entry -- no memory traffic,
  * four independent units in flight per thread -- and returns units per second (host double).
- *   MFH_MIX_C128_PAIR   14 32x32->64 multiplies + 25 ALU ops + 31 DFMA: one generated complex128 pair
+ *   MFH_MIX_C128_PAIR   14 32x32->64 multiplies + 26 ALU ops + 32 DFMA: one generated complex128 pair
  *                       {i,j} used for both phi_i and phi_j (2 matrix entries); of the 18 multiplies of a
  *                       Philox4x32-10 call the fused kernel shares 4 between the rows of a lane
  *   MFH_MIX_C64_ENTRY   14 multiplies + 22 ALU ops + 4 SFU ops + 11 FP32 ops: one generated complex64
  *                       entry whose multiply-accumulate runs on the tensor cores
- *   MFH_MIX_PHILOX      one full Philox call (18 multiplies, 18 xors);   MFH_MIX_DFMA31  31 DFMA alone
+ *   MFH_MIX_PHILOX      one full Philox call (18 multiplies, 18 xors);   MFH_MIX_DFMA31  the 32 FP64 operations alone
  * Synchronises `stream`.  Errors: INVALID_ARG, CUDA. */
 enum { MFH_MIX_C128_PAIR = 0, MFH_MIX_C64_ENTRY = 1, MFH_MIX_PHILOX = 2, MFH_MIX_DFMA31 = 3 };
 MFH_API int mfh_debug_pipe_rates(int32_t mix, double* units_per_s, void* stream);

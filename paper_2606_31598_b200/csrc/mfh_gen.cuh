@@ -99,8 +99,8 @@ __device__ __forceinline__ void pair_words(const PhiloxKeys& K, uint32_t lo, uin
 // r = m/c - 1 (|r| <= 2^-9):
 //     L = s^2 (-2 ln u1) = K2 [(32 - e) ln 2 - ln c] - K2 log1p(r),      K2 = 2 s^2 = 1/D,
 // a 256-entry table of (1/c, -K2 ln c), a 33-entry table of K2 (32-e) ln 2 and a degree-4
-// polynomial for log1p (remainder r^5/5 <= 6e-15).  sqrt(L) = L y (1 + e'), y = rsqrt.approx(L)
-// (2^-22), one Newton step (1.5 * 2^-44 = 9e-14 relative).  The angle 2 pi u2 is split into a
+// polynomial for log1p (remainder r^5/5 <= 6e-15).  sqrt(L) = L y (1 + e + 3/2 e^2), y = rsqrt.approx(L)
+// (2^-21), e = 1/2 - 1/2 L y^2: third-order correct (1e-19 relative).  The angle 2 pi u2 is split into a
 // 1024-entry table of (cos A, sin A) at the bin centres and a residual |b| <= pi/1024:
 // sin b = b - b^3/6 (2e-15), cos b = 1 - b^2/2 + b^4/24 (1e-18), combined by angle addition.
 constexpr int GEN_LOG_BITS = 8;
@@ -147,9 +147,13 @@ template <> struct Gen<double> {
         const double L = fma(r, p, tl.y + el);
         double y;
         asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(L));
-        const double sq = L * y, hy = 0.5 * y;
+        // sqrt(L) = sq (1 + e + 3/2 e^2 + O(e^3)) with sq = L y, e = 1/2 - 1/2 L y^2 (|e| <= 2^-21):
+        // the second-order term removes the -3/2 delta^2 bias a single Newton step would leave in
+        // every entry (1.9e-13, which a Chebyshev propagation over 151 applies would add up)
+        const double sq = L * y;
+        const double hy = __hiloint2double(__double2hiint(y) - 0x00100000, __double2loint(y));   // y / 2
         const double e = fma(-sq, hy, 0.5);
-        const double rad = fma(sq, e, sq);
+        const double rad = fma(sq, e * fma(e, 1.5, 1.0), sq);
         // angle
         const double2 cs = tab->tsc[x1 >> (32 - GEN_SC_BITS)];
         const int resid = (int)(x1 & ((1u << (32 - GEN_SC_BITS)) - 1u)) - (1 << (31 - GEN_SC_BITS));
