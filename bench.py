@@ -252,7 +252,8 @@ def roofline_for(res: dict, hbm_gbs: float, peak_src: str) -> dict:
         # HBM-bound cached streaming: algorithmic bytes = stored entries * bytes per entry
         nbytes = res["plan"]["cache_bytes"]
         gbs = nbytes / (kern["cached"] * 1e-3) / 1e9
-        name = "cached_pairs_kernel" if res["plan"]["mode"] == "pairs" else "cached_kernel"
+        name = "cached_pairs_kernel" if res["plan"]["mode"] == "pairs" else (
+            "cached_kernel" if k == 1 else "cached_multi_tc_kernel")
         return {"kernel": name, "bound": "hbm", "achieved": gbs, "peak": hbm_gbs, "unit": "GB/s",
                 "frac": gbs / hbm_gbs, "traffic": NCU_TRAFFIC.get((name, cfg["D"])), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": nbytes, "kernel_ms": kern["cached"],
@@ -353,7 +354,8 @@ def main():
 
     extras = {}
     if rank == 0 and world == 1 and not args.no_extra:
-        for name, st in (("C1", 20), ("C3", 5), ("C4", 3), ("C2-pairs", 10), ("C5", 3), ("C5-pairs", 5)):
+        for name, st in (("C1", 20), ("C3", 5), ("C3-cached", 10), ("C4", 3), ("C2-pairs", 10), ("C5", 3),
+                         ("C5-pairs", 5)):
             if name == args.workload:
                 continue
             try:

@@ -119,6 +119,7 @@ static int commit_plan(mfh_handle h, const Plan& p, cudaStream_t st)
     }
     int rc = ensure_gen_table(h, st);
     if (rc) return rc;
+    if (q.k > 1 && q.n_cached > 0 && (rc = make_cache_tensor_map(h))) return rc;
     rc = launch_fill_cache(h, st);
     if (rc) return rc;
     MFH_CUDA_CHECK(cudaStreamSynchronize(st));
@@ -137,7 +138,7 @@ static int apply_impl(mfh_handle h, const void* psi, void* phi, const double* la
     if (ev) cudaEventRecord(ev[1], st);
     if (p.k == 1) {
         if ((rc = launch_proc_single(h, psi, st))) return rc;
-    } else if (p.slot_multi >= 0) {
+    } else if (p.slot_multi >= 0 && p.covered_blocks < (int64_t)p.n_blk * p.n_blk) {
         if ((rc = launch_proc_multi(h, psi, st))) return rc;
     }
     if (ev) cudaEventRecord(ev[2], st);
@@ -323,7 +324,8 @@ MFH_API int mfh_get_plan(mfh_handle h, char* json_out, size_t json_cap)
              p.n_blk, p.k, (long long)p.n_cached, p.cached_per_row,
              (double)p.covered_blocks / ((double)p.n_blk * p.n_blk), p.cache_bytes, p.work_bytes, p.n_slots,
              p.items.size(), p.pair_items.size(), p.R, p.Q,
-             1 + (p.n_cached > 0) + ((p.k == 1 && !p.items.empty()) || p.slot_multi >= 0));
+             1 + (p.n_cached > 0) + ((p.k == 1 && !p.items.empty()) ||
+                                      (p.k > 1 && p.covered_blocks < (int64_t)p.n_blk * p.n_blk)));
     copy_json(buf, json_out, json_cap);
     return MFH_OK;
 }

@@ -162,7 +162,8 @@ int launch_cached(mfh_handle h, const void* psi, cudaStream_t st)
     const Plan& p = h->plan;
     if (p.n_cached == 0) return MFH_OK;
     if (p.k != 1) {
-        set_error("cached blocks with k > 1 are not supported yet");
+        if (tc_cached_multi_supported(h->dtype, p.k, p.B)) return launch_cached_multi_tc(h, psi, st);
+        set_error("cached blocks with k > 1 need complex64 and B %% 128 == 0");
         return MFH_ERR_UNSUPPORTED;
     }
     const unsigned grid = (unsigned)(h->D / CACHED_ROWS);

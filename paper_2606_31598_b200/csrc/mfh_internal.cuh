@@ -4,6 +4,7 @@
 #include <cstdio>
 #include <string>
 #include <vector>
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include "mfh.h"
@@ -78,6 +79,7 @@ struct mfh_handle_s {
     mfh::GenHostD gen_host;         // generator table + constants for this D (host copy)
     mfh::GenTabD* d_gen_tab = nullptr;   // device copy (c128 only), kept until mfh_destroy
     bool gen_ready = false;
+    alignas(64) CUtensorMap cache_tmap;   // TMA view of the cache (cached k-vector kernel)
     int sm_count = 148;
 };
 
@@ -108,6 +110,9 @@ int launch_proc_single(mfh_handle h, const void* psi, cudaStream_t st);
 int launch_proc_multi(mfh_handle h, const void* psi, cudaStream_t st);
 bool tc_multi_supported(mfh_handle h);                                   // mfh_tc.cu
 int launch_proc_multi_tc(mfh_handle h, const void* psi, cudaStream_t st);
+bool tc_cached_multi_supported(int dtype, int k, int B);
+int make_cache_tensor_map(mfh_handle h);
+int launch_cached_multi_tc(mfh_handle h, const void* psi, cudaStream_t st);
 int launch_cached(mfh_handle h, const void* psi, cudaStream_t st);
 int launch_cached_pairs(mfh_handle h, const void* psi, cudaStream_t st);
 int launch_reduce(mfh_handle h, const void* psi, void* phi, const double* lambdas_host, cudaStream_t st);

@@ -169,14 +169,14 @@ void build_tables(Plan& p, int64_t D, int dtype, int sm_count)
     // (row block, strip)] [k-vector kernel, one per column block]
     int s = 0;
     p.slot_cache = p.slot_row0 = p.slot_col0 = p.slot_multi = -1;
-    if (!p.pairs && c > 0) p.slot_cache = s++;
+    if (!p.pairs && c > 0 && p.k == 1) p.slot_cache = s++;
     if (p.k == 1 && n_pairs + n_pair_blocks > 0) {
         p.slot_row0 = s;
         s += N;
         p.slot_col0 = s;
         s += N * p.Q;
     }
-    if (p.k > 1 && covered < (int64_t)N * N) {   // k-vector kernel: one partial slot per column block m
+    if (p.k > 1) {   // k-vector kernels (generated and cached blocks): one partial slot per column block m
         p.slot_multi = s;
         s += N;
     }
@@ -186,7 +186,7 @@ void build_tables(Plan& p, int64_t D, int dtype, int sm_count)
     for (int b = 0; b < N; ++b) {
         if (p.slot_cache >= 0) valid(b, p.slot_cache) = 1;
         if (p.slot_multi >= 0)
-            for (int m = 0; m < N; ++m) valid(b, p.slot_multi + m) = uncached(b, m);
+            for (int m = 0; m < N; ++m) valid(b, p.slot_multi + m) = 1;
     }
     const int strip = p.B / p.Q;
     auto push_items = [&](std::vector<ProcItem>& dst, int n, int m, uint8_t kd) {
@@ -333,7 +333,8 @@ int enumerate_candidates(int64_t D, int dtype, int k, int mode, int B_req, int64
         for (auto [c, pairs] : cs) {
             Candidate cand = evaluate_candidate(D, dtype, k, B, c, pairs, n_applies, sm_count);
             cand.feasible = (cand.cache_bytes + cand.work_bytes <= budget_bytes);   // Eq. 18
-            if (k > 1 && c > 0) cand.feasible = false;   // cached multi-vector kernel: not built yet
+            // cached k-vector blocks: tensor-core kernel, complex64 with B % 128 == 0 only
+            if (k > 1 && c > 0 && (pairs || !tc_cached_multi_supported(dtype, k, B))) cand.feasible = false;
             out.push_back(cand);
         }
     }

@@ -21,6 +21,7 @@
 // index order by the reduce kernel).
 #include <algorithm>
 #include <cstdlib>
+#include <cuda.h>
 #include "mfh_internal.cuh"
 
 namespace mfh {
@@ -117,6 +118,29 @@ __device__ __forceinline__ void split_tf32(float x, float& hi, float& lo)
 {
     hi = __uint_as_float((__float_as_uint(x) + 0x1000u) & 0xffffe000u);
     lo = x - hi;
+}
+
+// Epilogue of warp w < 4: TMEM lanes 32w..32w+31 hold rows 32w + lane of the [128 x 32] accumulator
+// (columns 0..15 real parts, 16..31 imaginary parts of the k vectors); dst = this row's k outputs.
+__device__ __forceinline__ void tc_epilogue(uint32_t d_tmem, int w, float2* dst, int k)
+{
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    uint32_t r[32];
+    const uint32_t taddr = d_tmem + ((uint32_t)(32 * w) << 16);
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]),
+          "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]),
+          "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+        : "r"(taddr)
+        : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+    for (int vv = 0; vv < 16; ++vv)
+        if (vv < k) dst[vv] = make_float2(__uint_as_float(r[vv]), __uint_as_float(r[16 + vv]));
 }
 
 struct TcParams {
@@ -261,28 +285,9 @@ __global__ void __launch_bounds__(TC_THREADS, MFH_TC_MINB) proc_multi_tc_kernel(
     else if (n > m) tc_generate<-1>(P, smem, full, empty, d_tmem, i_base, m);
     else tc_generate<0>(P, smem, full, empty, d_tmem, i_base, m);
 
-    if (w < 4) {   // warp w reads TMEM lanes 32w..32w+31: row 32w + lane, 32 columns
-        const int k = P.k;
+    if (w < 4) {
         mbar_wait(&done, 0);
-        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        uint32_t r[32];
-        const uint32_t taddr = d_tmem + ((uint32_t)(32 * w) << 16);
-        asm volatile(
-            "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
-            "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
-            "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
-            : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
-              "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]),
-              "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]),
-              "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
-            : "r"(taddr)
-            : "memory");
-        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-        const uint32_t row = i_base + 32 * w + (tid & 31);
-        float2* dst = P.work + ((size_t)(P.slot_multi + m) * P.D + row) * k;
-#pragma unroll
-        for (int vv = 0; vv < 16; ++vv)
-            if (vv < k) dst[vv] = make_float2(__uint_as_float(r[vv]), __uint_as_float(r[16 + vv]));
+        tc_epilogue(d_tmem, w, P.work + ((size_t)(P.slot_multi + m) * P.D + i_base + 32 * w + (tid & 31)) * P.k, P.k);
     }
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
@@ -317,6 +322,256 @@ int launch_proc_multi_tc(mfh_handle h, const void* psi, cudaStream_t st)
         attr_done = true;
     }
     proc_multi_tc_kernel<<<dim3((unsigned)(h->D / TC_TP), p.n_blk), TC_THREADS, smem, st>>>(P);
+    MFH_CUDA_CHECK(cudaGetLastError());
+    return MFH_OK;
+}
+
+// --------------------------------------------------------------------------------------------
+// Cached k-vector kernel (complex64): "reads each V block once for k vectors" (north_star (c);
+// Y = A X with R simultaneous vectors, Eq. 12, on cached blocks P:177-183).
+//
+// A cached block is row-major B x B interleaved complex64, i.e. a real K-major matrix
+// [B rows][2B floats] with K index k' = 2 q + c (c = 0 real, 1 imaginary part of column q), and
+//     [Re Phi | Im Phi][p] = sum_k' A[p][k'] Bmat[k'][:],   Bmat[2q] = [Re Psi_q | Im Psi_q],
+//                                                            Bmat[2q+1] = [-Im Psi_q | Re Psi_q].
+// HBM-bound: 8 bytes per entry against 128 flop, which only the tensor cores sustain.  A CTA owns
+// 128 rows x one cached block and walks it in tiles of 16 complex columns (32 floats = 128 B per
+// row): a producer lane issues one TMA tensor copy (cp.async.bulk.tensor.2d, 128B swizzle, 16 KB)
+// per tile into a 4-stage shared-memory ring; 8 converter warps read their row's words (conflict-
+// free through the swizzle), split them into TF32 hi + lo and write them with tcgen05.st into TMEM
+// as the A operand, and build the psi images; the MMA warp issues 12 tcgen05.mma per tile (3xTF32:
+// A_hi B_hi + A_hi B_lo + A_lo B_hi) and commits onto the mbarrier that frees the TMEM stage.
+// --------------------------------------------------------------------------------------------
+constexpr int CT_STAGES = 4;                  // shared-memory stages of raw tiles (TMA)
+constexpr int CT_TSTAGES = 3;                 // TMEM stages of split A operands
+constexpr int CT_KF = 32;                     // floats per tile row = 16 complex columns = 4 MMA K-steps
+constexpr int CT_RAW = TC_TP * CT_KF * 4;     // 16 KB raw tile
+constexpr int CT_B_TILE = TC_N * CT_KF * 4;   // 4 KB psi image
+constexpr int CT_BSTAGE = 2 * CT_B_TILE;      // hi, lo
+constexpr int CT_SBO = (CT_KF / 4) * 128;     // 1 KB between 8-column groups of a psi image
+constexpr int CT_A_STAGE_COLS = 2 * CT_KF;    // A_hi, A_lo: 32 TMEM columns each
+constexpr int CT_THREADS = 32 * (TC_GEN_WARPS + 2);   // 8 converter warps, MMA warp, TMA warp
+constexpr int CT_PSI = (CT_KF / 2) * 16 * 8;  // psi rows of one tile: 16 columns x <= 16 vectors x 8 B
+constexpr int CT_SMEM = CT_STAGES * (CT_RAW + CT_PSI) + CT_TSTAGES * CT_BSTAGE + 1024;   // + alignment slack
+
+__device__ __forceinline__ uint64_t umma_desc_sbo(uint32_t addr, int sbo)
+{
+    return (uint64_t)((addr >> 4) & 0x3fffu) | ((uint64_t)(TC_LBO >> 4) << 16) | ((uint64_t)(sbo >> 4) << 32) |
+           (1ull << 46);
+}
+
+struct CtParams {
+    int32_t B, n_blk, k, slot_multi;
+    int64_t D;
+    const int32_t* cache_slot;
+    const float2* psi;
+    float2* work;
+};
+
+__global__ void __launch_bounds__(CT_THREADS, 2)
+cached_multi_tc_kernel(const CtParams P, const __grid_constant__ CUtensorMap tmap)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw_[];
+    __shared__ __align__(8) uint64_t raw_full[CT_STAGES], raw_empty[CT_STAGES], a_full[CT_TSTAGES], a_empty[CT_TSTAGES], done;
+    __shared__ uint32_t s_tmem;
+    const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
+    const int m = blockIdx.y;
+    const uint32_t i_base = blockIdx.x * TC_TP;
+    const int n = (int)(i_base / (uint32_t)P.B);
+    const int32_t slot = P.cache_slot[n * P.n_blk + m];
+    if (slot < 0) return;   // generated block: the fused kernel's
+    // 1024-byte aligned stage base (128B swizzle pattern repeats every 8 rows x 128 B)
+    unsigned char* smem = smem_raw_ + ((1024u - (smem_u32(smem_raw_) & 1023u)) & 1023u);
+    unsigned char* psis = smem + CT_STAGES * CT_RAW;    // [CT_STAGES][16 columns][k] complex, filled by the producer
+    unsigned char* bimg = psis + CT_STAGES * CT_PSI;
+
+    if (tid == 0) {
+        for (int s = 0; s < CT_STAGES; ++s) {
+            mbar_init(&raw_full[s], 1);
+            mbar_init(&raw_empty[s], TC_GEN_WARPS);
+        }
+        for (int s = 0; s < CT_TSTAGES; ++s) {
+            mbar_init(&a_full[s], TC_GEN_WARPS);
+            mbar_init(&a_empty[s], 1);
+        }
+        mbar_init(&done, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (w == TC_GEN_WARPS) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&s_tmem)),
+                     "n"(256)
+                     : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t d_tmem = s_tmem;
+    const int n_tiles = P.B / (CT_KF / 2);
+    const int row0 = slot * P.B + (int)(i_base - (uint32_t)n * P.B);   // first row of the strip in the cache "image"
+
+    if (w == TC_GEN_WARPS + 1) {
+        // ---- TMA producer: one lane ----
+        if (lane == 0) {
+            for (int t = 0; t < n_tiles; ++t) {
+                const int s = t % CT_STAGES, u = t / CT_STAGES;
+                if (u > 0) mbar_wait(&raw_empty[s], (u - 1) & 1);
+                const uint32_t psi_bytes = (uint32_t)((CT_KF / 2) * P.k * sizeof(float2));
+                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&raw_full[s])),
+                             "r"(CT_RAW + psi_bytes)
+                             : "memory");
+                // the 16 psi rows of the tile are contiguous in [D][k]: one 1-D bulk copy
+                asm volatile(
+                    "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                        smem_u32(psis + s * CT_PSI)),
+                    "l"(P.psi + ((size_t)m * P.B + (size_t)t * (CT_KF / 2)) * P.k), "r"(psi_bytes), "r"(smem_u32(&raw_full[s]))
+                    : "memory");
+                asm volatile(
+                    "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::
+                        "r"(smem_u32(smem + s * CT_RAW)),
+                    "l"(&tmap), "r"(t * CT_KF), "r"(row0), "r"(smem_u32(&raw_full[s]))
+                    : "memory");
+            }
+        }
+    } else if (w == TC_GEN_WARPS) {
+        // ---- MMA warp ----
+        for (int t = 0; t < n_tiles; ++t) {
+            const int s = t % CT_TSTAGES, u = t / CT_TSTAGES;
+            mbar_wait(&a_full[s], u & 1);
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            if (lane == 0) {
+                const uint32_t b0 = smem_u32(bimg + s * CT_BSTAGE);
+                const uint32_t a0 = d_tmem + (uint32_t)(TC_N + s * CT_A_STAGE_COLS);
+#pragma unroll
+                for (int ks = 0; ks < CT_KF / 8; ++ks) {
+                    const uint64_t b_h = umma_desc_sbo(b0 + ks * 2 * TC_LBO, CT_SBO);
+                    const uint64_t b_l = umma_desc_sbo(b0 + CT_B_TILE + ks * 2 * TC_LBO, CT_SBO);
+                    umma_tf32_ts(d_tmem, a0 + 8 * ks, b_h, (t | ks) != 0);
+                    umma_tf32_ts(d_tmem, a0 + 8 * ks, b_l, 1);
+                    umma_tf32_ts(d_tmem, a0 + CT_KF + 8 * ks, b_h, 1);
+                }
+                umma_commit(&a_empty[s]);
+                if (t == n_tiles - 1) umma_commit(&done);
+            }
+            __syncwarp();
+        }
+    } else {
+        // ---- converter warps: thread = (row p, 4 of the 8 four-float groups of the row) ----
+        const int p = tid & (TC_TP - 1), gsel = tid >> 7, k = P.k;
+        const uint32_t a_lane = d_tmem + ((uint32_t)(p & ~31) << 16);
+        const int v = tid & 15, qb = tid >> 4;   // psi element (column qb of the tile, vector v)
+        // psi image element (n, k'): rows n = v and 16 + v, K positions k' = 2 qb and 2 qb + 1 (adjacent floats)
+        const int o_re = ((v & 7) * 16 + (v >> 3) * CT_SBO + (qb >> 1) * 128 + (qb & 1) * 8) / 4;
+        const int o_im = o_re + 2 * CT_SBO / 4;
+        for (int t = 0; t < n_tiles; ++t) {
+            const int s = t % CT_STAGES, u = t / CT_STAGES;
+            const int ts = t % CT_TSTAGES, tu = t / CT_TSTAGES;
+            mbar_wait(&raw_full[s], u & 1);
+            const float2 x = (v < k) ? reinterpret_cast<const float2*>(psis + s * CT_PSI)[qb * k + v] : float2{0.f, 0.f};
+            float4 raw[4];
+            const unsigned char* rp = smem + s * CT_RAW + p * 128;
+#pragma unroll
+            for (int gg = 0; gg < 4; ++gg) {
+                const int g = gsel + 2 * gg;   // logical 16-byte chunk of the row; 128B swizzle: chunk ^ (row % 8)
+                raw[gg] = *reinterpret_cast<const float4*>(rp + ((g ^ (p & 7)) << 4));
+            }
+            float prh, prl, pih, pil;
+            split_tf32(x.x, prh, prl);
+            split_tf32(x.y, pih, pil);
+            if (tu > 0) mbar_wait(&a_empty[ts], (tu - 1) & 1);
+#pragma unroll
+            for (int gg = 0; gg < 4; ++gg) {
+                const int g = gsel + 2 * gg;
+                float h0, l0, h1, l1, h2, l2, h3, l3;
+                split_tf32(raw[gg].x, h0, l0);
+                split_tf32(raw[gg].y, h1, l1);
+                split_tf32(raw[gg].z, h2, l2);
+                split_tf32(raw[gg].w, h3, l3);
+                const uint32_t ta = a_lane + (uint32_t)(TC_N + ts * CT_A_STAGE_COLS + 4 * g);
+                tmem_st4(ta, h0, h1, h2, h3);
+                tmem_st4(ta + CT_KF, l0, l1, l2, l3);
+            }
+            // every lane has consumed its shared-memory words (the splits depend on them): only now may
+            // the TMA producer overwrite the raw stage
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&raw_empty[s]);
+            {
+                float* b = reinterpret_cast<float*>(bimg + ts * CT_BSTAGE);
+                constexpr int BT = CT_B_TILE / 4;
+                *reinterpret_cast<float2*>(b + o_re) = make_float2(prh, -pih);        // n = v:      Re Psi, -Im Psi
+                *reinterpret_cast<float2*>(b + o_im) = make_float2(pih, prh);         // n = 16 + v: Im Psi,  Re Psi
+                *reinterpret_cast<float2*>(b + BT + o_re) = make_float2(prl, -pil);
+                *reinterpret_cast<float2*>(b + BT + o_im) = make_float2(pil, prl);
+            }
+            asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&a_full[ts]);
+        }
+        if (w < 4) {
+            mbar_wait(&done, 0);
+            tc_epilogue(d_tmem, w, P.work + ((size_t)(P.slot_multi + m) * P.D + i_base + 32 * w + lane) * k, k);
+        }
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (w == TC_GEN_WARPS)
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(d_tmem), "n"(256) : "memory");
+}
+
+bool tc_cached_multi_supported(int dtype, int k, int B) { return dtype == MFH_C64 && k > 1 && k <= 16 && B % TC_TP == 0; }
+
+// Tensor map over the whole cache seen as [stored_blocks * B rows][2 B floats]; box = 128 rows x 32 floats.
+int make_cache_tensor_map(mfh_handle h)
+{
+    typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static EncodeFn encode = nullptr;
+    if (!encode) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        MFH_CUDA_CHECK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+        if (!fn || qres != cudaDriverEntryPointSuccess) {
+            set_error("cuTensorMapEncodeTiled is not available in this driver");
+            return MFH_ERR_CUDA;
+        }
+        encode = (EncodeFn)fn;
+    }
+    const Plan& p = h->plan;
+    const cuuint64_t dims[2] = {(cuuint64_t)2 * p.B, (cuuint64_t)p.n_cached * p.B};
+    const cuuint64_t strides[1] = {(cuuint64_t)2 * p.B * sizeof(float)};
+    const cuuint32_t box[2] = {CT_KF, TC_TP};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = encode(&h->cache_tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, h->d_cache, dims, strides, box, estr,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        set_error("cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+        return MFH_ERR_CUDA;
+    }
+    return MFH_OK;
+}
+
+int launch_cached_multi_tc(mfh_handle h, const void* psi, cudaStream_t st)
+{
+    const Plan& p = h->plan;
+    CtParams P;
+    P.B = p.B;
+    P.n_blk = p.n_blk;
+    P.k = p.k;
+    P.slot_multi = p.slot_multi;
+    P.D = h->D;
+    P.cache_slot = h->d_cache_slot;
+    P.psi = (const float2*)psi;
+    P.work = (float2*)h->d_work;
+    static bool attr_done = false;
+    if (!attr_done) {
+        MFH_CUDA_CHECK(cudaFuncSetAttribute(cached_multi_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, CT_SMEM));
+        attr_done = true;
+    }
+    cached_multi_tc_kernel<<<dim3((unsigned)(h->D / TC_TP), p.n_blk), CT_THREADS, CT_SMEM, st>>>(P, h->cache_tmap);
     MFH_CUDA_CHECK(cudaGetLastError());
     return MFH_OK;
 }

@@ -30,6 +30,8 @@ CONFIGS = {
 VARIANTS = {
     "C2-pairs": dict(CONFIGS["C2"], mode="pairs"),
     "C5-pairs": dict(CONFIGS["C5"], mode="pairs"),
+    # C3's coupling scan with V cached (8.6 GB): each stored block is read once for the 16 vectors
+    "C3-cached": dict(CONFIGS["C3"], mode="full"),
 }
 
 

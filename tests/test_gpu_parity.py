@@ -203,6 +203,23 @@ def test_scan_c64_tensor_core_and_cuda_core_shapes(D, B, k):
         assert rel_l2(Phi[:, v], ref[:, v]) <= TOL["c64"], v
 
 
+@pytest.mark.parametrize("mode,budget", [("full", 0), ("partial", 6e6), ("partial", 14e6)])
+@pytest.mark.parametrize("k", [16, 5])
+def test_scan_c64_cached_blocks_tensor_core(mode, budget, k):
+    # cached k-vector path: each stored V block is read once for all k vectors (TMA -> TMEM -> tcgen05),
+    # alone and mixed with generated blocks
+    D, B = 2048, 256          # 8x8 blocks of 512 KiB
+    Psi = make_psi(D, 13, k=k, dtype="c64")
+    lam = 0.25 + lambda_grid(k)
+    h = mfh.Hamiltonian(D, B, 8, "c64", kind="diag_plus_gue", seed_h0=7)
+    plan = h.plan(mode, k=k, hbm_budget_bytes=int(budget))
+    assert plan["chosen"]["mode"] == mode
+    Phi = h.apply(to_dev(Psi), lambdas=lam).cpu().numpy()
+    ref = oracle.apply_scan(D, B, 8, 7, lam, Psi)
+    for v in range(k):
+        assert rel_l2(Phi[:, v], ref[:, v]) <= TOL["c64"], v
+
+
 def test_multi_vector_equals_single_vector_applies():
     D, B, k = 1024, 256, 4
     Psi = make_psi(D, 21, k=k)
