@@ -119,7 +119,6 @@ static int commit_plan(mfh_handle h, const Plan& p, cudaStream_t st)
     }
     int rc = ensure_gen_table(h, st);
     if (rc) return rc;
-    if (q.k > 1 && q.n_cached > 0 && (rc = make_cache_tensor_map(h))) return rc;
     rc = launch_fill_cache(h, st);
     if (rc) return rc;
     MFH_CUDA_CHECK(cudaStreamSynchronize(st));

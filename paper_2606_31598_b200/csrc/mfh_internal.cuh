@@ -4,7 +4,6 @@
 #include <cstdio>
 #include <string>
 #include <vector>
-#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include "mfh.h"
@@ -33,6 +32,16 @@ struct ProcItem {
     int32_t kind;       // PAIR_*
     int32_t col_slot;   // partial slot receiving the column-side sums (-1: none)
 };
+
+// Tiled cache layout of k-vector plans (complex64): element (a, b) of a B x B block, in floats from the
+// block start.  Tiles of 128 rows x 32 floats (16 complex columns) are contiguous 16 KB runs, ordered
+// column tile fastest inside a row tile; inside a tile row r holds 8 chunks of 16 bytes, chunk c stored
+// at position c ^ (r & 7) (the 128-byte swizzle the tensor-core kernel reads conflict-free).
+__host__ __device__ inline size_t tiled_cache_offset(int B, int a, int b)
+{
+    const int rt = a >> 7, r = a & 127, kt = b >> 4, c = (b & 15) >> 1;
+    return ((size_t)rt * (B >> 4) + kt) * 4096 + (size_t)r * 32 + (size_t)((c ^ (r & 7)) << 2) + (size_t)((b & 1) << 1);
+}
 
 struct Plan {
     int32_t mode = 0;          // MFH_MODE_* actually committed
@@ -79,7 +88,6 @@ struct mfh_handle_s {
     mfh::GenHostD gen_host;         // generator table + constants for this D (host copy)
     mfh::GenTabD* d_gen_tab = nullptr;   // device copy (c128 only), kept until mfh_destroy
     bool gen_ready = false;
-    alignas(64) CUtensorMap cache_tmap;   // TMA view of the cache (cached k-vector kernel)
     int sm_count = 148;
 };
 
@@ -111,7 +119,6 @@ int launch_proc_multi(mfh_handle h, const void* psi, cudaStream_t st);
 bool tc_multi_supported(mfh_handle h);                                   // mfh_tc.cu
 int launch_proc_multi_tc(mfh_handle h, const void* psi, cudaStream_t st);
 bool tc_cached_multi_supported(int dtype, int k, int B);
-int make_cache_tensor_map(mfh_handle h);
 int launch_cached_multi_tc(mfh_handle h, const void* psi, cudaStream_t st);
 int launch_cached(mfh_handle h, const void* psi, cudaStream_t st);
 int launch_cached_pairs(mfh_handle h, const void* psi, cudaStream_t st);

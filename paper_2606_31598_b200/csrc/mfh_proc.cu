@@ -59,7 +59,7 @@ int launch_philox_debug(uint64_t seed, uint32_t stream_id, const uint32_t* i, co
 template <typename T>
 __global__ void __launch_bounds__(256) fill_kernel(const GenArgs<T> G, int32_t B, int32_t n_blk,
                                                    const int32_t* __restrict__ cache_slot,
-                                                   int32_t single_n, int32_t single_m,
+                                                   int32_t single_n, int32_t single_m, int32_t tiled,
                                                    typename Cplx<T>::type* __restrict__ out)
 {
     using CT = typename Cplx<T>::type;
@@ -88,17 +88,18 @@ __global__ void __launch_bounds__(256) fill_kernel(const GenArgs<T> G, int32_t B
             CT v;
             v.x = hr;
             v.y = hi;
-            row[b] = v;
+            if (tiled) reinterpret_cast<CT*>(reinterpret_cast<T*>(out + base) + tiled_cache_offset(B, a, b))[0] = v;
+            else row[b] = v;
         }
     }
 }
 
 template <typename T>
 static int launch_fill_t(mfh_handle h, dim3 grid, int32_t B, int32_t n_blk, const int32_t* cache_slot,
-                         int32_t n, int32_t m, void* out, cudaStream_t st)
+                         int32_t n, int32_t m, int32_t tiled, void* out, cudaStream_t st)
 {
     using CT = typename Cplx<T>::type;
-    fill_kernel<T><<<grid, 256, Gen<T>::TAB_BYTES, st>>>(make_gen_args<T>(h), B, n_blk, cache_slot, n, m,
+    fill_kernel<T><<<grid, 256, Gen<T>::TAB_BYTES, st>>>(make_gen_args<T>(h), B, n_blk, cache_slot, n, m, tiled,
                                                           (CT*)out);
     MFH_CUDA_CHECK(cudaGetLastError());
     return MFH_OK;
@@ -109,8 +110,8 @@ int launch_fill_block(mfh_handle h, int32_t B, int32_t n, int32_t m, void* out, 
     int rc = ensure_gen_table(h, st);
     if (rc) return rc;
     dim3 grid(1, std::min(B, 1024));
-    return h->dtype == MFH_C128 ? launch_fill_t<double>(h, grid, B, 0, nullptr, n, m, out, st)
-                                : launch_fill_t<float>(h, grid, B, 0, nullptr, n, m, out, st);
+    return h->dtype == MFH_C128 ? launch_fill_t<double>(h, grid, B, 0, nullptr, n, m, 0, out, st)
+                                : launch_fill_t<float>(h, grid, B, 0, nullptr, n, m, 0, out, st);
 }
 
 int launch_fill_cache(mfh_handle h, cudaStream_t st)
@@ -121,8 +122,8 @@ int launch_fill_cache(mfh_handle h, cudaStream_t st)
     if (rc) return rc;
     dim3 grid(p.n_blk * p.n_blk, std::min(p.B, 64));
     return h->dtype == MFH_C128
-               ? launch_fill_t<double>(h, grid, p.B, p.n_blk, h->d_cache_slot, 0, 0, h->d_cache, st)
-               : launch_fill_t<float>(h, grid, p.B, p.n_blk, h->d_cache_slot, 0, 0, h->d_cache, st);
+               ? launch_fill_t<double>(h, grid, p.B, p.n_blk, h->d_cache_slot, 0, 0, 0, h->d_cache, st)
+               : launch_fill_t<float>(h, grid, p.B, p.n_blk, h->d_cache_slot, 0, 0, p.k > 1 ? 1 : 0, h->d_cache, st);
 }
 
 // --------------------------------------------------------------------------------------------

@@ -10,18 +10,17 @@
 // TMEM, B from shared memory) with the [128 x 32] fp32 accumulator also in TMEM, so the 64 FFMA
 // per entry of the CUDA-core kernel disappear from the issue slots that bound it.
 // 3xTF32: D += A_hi B_hi + A_hi B_lo + A_lo B_hi (single-pass TF32 gives 2.9e-4 relative L2 and
-// fails the 1e-4 tolerance; measured here: 1.4e-5 on C3, dominated by the tensor core's fp32
+// fails the 1e-4 tolerance; measured here: 9.5e-6 on C3, dominated by the tensor core's fp32
 // accumulation over 1024 columns).  Complex arithmetic as two real operand pairs:
 //     [Re Phi | Im Phi] += Re V x [Re Psi | Im Psi]  +  Im V x [-Im Psi | Re Psi].
 // Warp-specialised CTA: 8 generator warps + 1 MMA warp, a 3-stage ring of (A columns in TMEM,
 // B images in shared memory) guarded by mbarriers: generators wait on empty[s] (tcgen05.commit of
 // the MMAs that read the stage), fill it, fence and arrive on full[s]; the MMA warp waits on
-// full[s], issues 12 MMAs and commits.  A CTA owns 128 rows x one column block m; the epilogue
+// full[s], issues 8 MMAs (see TC_ACC_COLS) and commits.  A CTA owns 128 rows x one column block m; the epilogue
 // reads the accumulator with tcgen05.ld and writes the partial slot of column block m (added in
 // index order by the reduce kernel).
 #include <algorithm>
 #include <cstdlib>
-#include <cuda.h>
 #include "mfh_internal.cuh"
 
 namespace mfh {
@@ -41,9 +40,9 @@ constexpr int TC_N = 32;                      // MMA N: 16 vectors x (re, im)
 constexpr int TC_B_TILE = TC_N * TC_TQ * 4;   // bytes of one B operand image in shared memory (2 KB)
 constexpr int TC_STAGE = 4 * TC_B_TILE;       // B1_hi B1_lo B2_hi B2_lo
 constexpr int TC_STAGES = 3;
-// TMEM columns: [0,32) accumulator; stage s holds the four A images Er_hi Er_lo Ei_hi Ei_lo, 16 columns each
-constexpr int TC_TMEM_COLS = (TC_N + TC_STAGES * 4 * TC_TQ) <= 128 ? 128 : 256;
-constexpr int TC_A_COL0 = TC_N;
+// TMEM columns: [0,64) accumulator (two halves, see TC_ACC_COLS); stage s holds the four A images Er_hi Er_lo Ei_hi Ei_lo, 16 columns each
+constexpr int TC_TMEM_COLS = (2 * TC_N + TC_STAGES * 4 * TC_TQ) <= 128 ? 128 : 256;
+constexpr int TC_A_COL0 = 2 * TC_N;
 constexpr int TC_A_STAGE_COLS = 4 * TC_TQ;
 constexpr int TC_SBO = (TC_TQ / 4) * 128;     // byte stride between 8-row groups (A) / 8-column groups (B)
 constexpr int TC_LBO = 128;                   // byte stride between the two 16-byte K halves of one MMA
@@ -57,11 +56,19 @@ __device__ __forceinline__ uint64_t umma_desc(uint32_t addr)
            (1ull << 46);
 }
 
-// Instruction descriptor: D = F32, A = B = TF32, both K-major, M = 128, N = 32.
-constexpr uint32_t TC_IDESC = (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(TC_N >> 3) << 17) |
-                              ((uint32_t)(TC_TP >> 4) << 24);
+// Instruction descriptor: D = F32, A = B = TF32, both K-major, M = 128, N = 32 or 64.
+constexpr uint32_t tc_idesc(int n)
+{
+    return (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(TC_TP >> 4) << 24);
+}
+// 3xTF32 with two instructions per operand pair: the hi and lo images of B are adjacent in shared memory
+// (8 row groups of one stride), so  A_hi x [B_hi | B_lo]  is ONE N = 64 MMA into accumulator columns
+// [0,32) and [32,64), and  A_lo x B_hi  one N = 32 MMA into [0,32); the epilogue adds the two halves.
+// The small MMAs of this kernel cost a fixed ~100 clocks each, so their number is what matters.
+constexpr int TC_ACC_COLS = 2 * TC_N;
 
 // A operand from TMEM (128 lanes x 8 columns), B from shared memory.
+template <int N>
 __device__ __forceinline__ void umma_tf32_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b, uint32_t accumulate)
 {
     asm volatile(
@@ -70,7 +77,7 @@ __device__ __forceinline__ void umma_tf32_ts(uint32_t d_tmem, uint32_t a_tmem, u
         "setp.ne.b32 p, %4, 0;\n\t"
         "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n\t"
         "}\n" ::"r"(d_tmem),
-        "r"(a_tmem), "l"(b), "r"(TC_IDESC), "r"(accumulate)
+        "r"(a_tmem), "l"(b), "r"(tc_idesc(N)), "r"(accumulate)
         : "memory");
 }
 
@@ -125,22 +132,28 @@ __device__ __forceinline__ void split_tf32(float x, float& hi, float& lo)
 __device__ __forceinline__ void tc_epilogue(uint32_t d_tmem, int w, float2* dst, int k)
 {
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-    uint32_t r[32];
-    const uint32_t taddr = d_tmem + ((uint32_t)(32 * w) << 16);
-    asm volatile(
-        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
-        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
-        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
-        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
-          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]),
-          "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]),
-          "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
-        : "r"(taddr)
-        : "memory");
-    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+    float acc[32];
+#pragma unroll
+    for (int half = 0; half < 2; ++half) {   // columns [0,32): A_hi B_hi + A_lo B_hi;  [32,64): A_hi B_lo
+        uint32_t r[32];
+        const uint32_t taddr = d_tmem + ((uint32_t)(32 * w) << 16) + 32 * half;
+        asm volatile(
+            "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+            "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+            "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+            : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+              "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]),
+              "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]),
+              "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+            : "r"(taddr)
+            : "memory");
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+        for (int c = 0; c < 32; ++c) acc[c] = half ? acc[c] + __uint_as_float(r[c]) : __uint_as_float(r[c]);
+    }
 #pragma unroll
     for (int vv = 0; vv < 16; ++vv)
-        if (vv < k) dst[vv] = make_float2(__uint_as_float(r[vv]), __uint_as_float(r[16 + vv]));
+        if (vv < k) dst[vv] = make_float2(acc[vv], acc[16 + vv]);
 }
 
 struct TcParams {
@@ -215,7 +228,7 @@ __device__ __forceinline__ void tc_generate(const TcParams& P, unsigned char* sm
     }
 }
 
-// MMA warp: waits for the 8 generator warps, issues the 12 MMAs of the tile from one lane and commits
+// MMA warp: waits for the 8 generator warps, issues the 8 MMAs of the tile from one lane and commits
 // them onto empty[s] (the arrival that lets the generators overwrite the stage).
 __device__ __forceinline__ void tc_mma_warp(const TcParams& P, unsigned char* smem, uint64_t* full, uint64_t* empty,
                                             uint64_t* done, uint32_t d_tmem)
@@ -234,14 +247,12 @@ __device__ __forceinline__ void tc_mma_warp(const TcParams& P, unsigned char* sm
                 const uint32_t ko = ks * 2 * TC_LBO;
                 const uint32_t er_h = a0 + 0 * TC_TQ + 8 * ks, er_l = a0 + 1 * TC_TQ + 8 * ks;
                 const uint32_t ei_h = a0 + 2 * TC_TQ + 8 * ks, ei_l = a0 + 3 * TC_TQ + 8 * ks;
-                const uint64_t b1_h = umma_desc(b0 + 0 * TC_B_TILE + ko), b1_l = umma_desc(b0 + 1 * TC_B_TILE + ko);
-                const uint64_t b2_h = umma_desc(b0 + 2 * TC_B_TILE + ko), b2_l = umma_desc(b0 + 3 * TC_B_TILE + ko);
-                umma_tf32_ts(d_tmem, er_h, b1_h, (t | ks) != 0);
-                umma_tf32_ts(d_tmem, er_h, b1_l, 1);
-                umma_tf32_ts(d_tmem, er_l, b1_h, 1);
-                umma_tf32_ts(d_tmem, ei_h, b2_h, 1);
-                umma_tf32_ts(d_tmem, ei_h, b2_l, 1);
-                umma_tf32_ts(d_tmem, ei_l, b2_h, 1);
+                const uint64_t b1 = umma_desc(b0 + 0 * TC_B_TILE + ko);   // [B1_hi | B1_lo] for N = 64, B1_hi for N = 32
+                const uint64_t b2 = umma_desc(b0 + 2 * TC_B_TILE + ko);
+                umma_tf32_ts<64>(d_tmem, er_h, b1, (t | ks) != 0);
+                umma_tf32_ts<32>(d_tmem, er_l, b1, 1);
+                umma_tf32_ts<64>(d_tmem, ei_h, b2, 1);
+                umma_tf32_ts<32>(d_tmem, ei_l, b2, 1);
             }
             umma_commit(&empty[s]);                            // arrives when every MMA issued so far has completed
             if (t == n_tiles - 1) umma_commit(done);
@@ -336,10 +347,12 @@ int launch_proc_multi_tc(mfh_handle h, const void* psi, cudaStream_t st)
 //                                                            Bmat[2q+1] = [-Im Psi_q | Re Psi_q].
 // HBM-bound: 8 bytes per entry against 128 flop, which only the tensor cores sustain.  A CTA owns
 // 128 rows x one cached block and walks it in tiles of 16 complex columns (32 floats = 128 B per
-// row): a producer lane issues one TMA tensor copy (cp.async.bulk.tensor.2d, 128B swizzle, 16 KB)
-// per tile into a 4-stage shared-memory ring; 8 converter warps read their row's words (conflict-
-// free through the swizzle), split them into TF32 hi + lo and write them with tcgen05.st into TMEM
-// as the A operand, and build the psi images; the MMA warp issues 12 tcgen05.mma per tile (3xTF32:
+// row).  For k-vector plans the cache is stored TILED: each [128 rows x 32 floats] tile is one
+// contiguous 16 KB run in HBM (full DRAM page locality; a row-major block would give 128-byte
+// pieces 8 KB apart), rows XOR-swizzled in 16-byte chunks so that the shared-memory image is read
+// without bank conflicts.  A producer lane issues one TMA bulk copy (cp.async.bulk, 16 KB) per tile
+// into a 4-stage shared-memory ring; 8 converter warps read their row's words, split them into TF32 hi + lo and write them with tcgen05.st into TMEM
+// as the A operand, and build the psi images; the MMA warp issues 8 tcgen05.mma per tile (3xTF32:
 // A_hi B_hi + A_hi B_lo + A_lo B_hi) and commits onto the mbarrier that frees the TMEM stage.
 // --------------------------------------------------------------------------------------------
 constexpr int CT_STAGES = 4;                  // shared-memory stages of raw tiles (TMA)
@@ -364,12 +377,12 @@ struct CtParams {
     int32_t B, n_blk, k, slot_multi;
     int64_t D;
     const int32_t* cache_slot;
+    const float2* cache;   // tiled layout
     const float2* psi;
     float2* work;
 };
 
-__global__ void __launch_bounds__(CT_THREADS, 2)
-cached_multi_tc_kernel(const CtParams P, const __grid_constant__ CUtensorMap tmap)
+__global__ void __launch_bounds__(CT_THREADS, 2) cached_multi_tc_kernel(const CtParams P)
 {
     extern __shared__ __align__(128) unsigned char smem_raw_[];
     __shared__ __align__(8) uint64_t raw_full[CT_STAGES], raw_empty[CT_STAGES], a_full[CT_TSTAGES], a_empty[CT_TSTAGES], done;
@@ -408,7 +421,9 @@ cached_multi_tc_kernel(const CtParams P, const __grid_constant__ CUtensorMap tma
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const uint32_t d_tmem = s_tmem;
     const int n_tiles = P.B / (CT_KF / 2);
-    const int row0 = slot * P.B + (int)(i_base - (uint32_t)n * P.B);   // first row of the strip in the cache "image"
+    // the strip's tiles: block slot, row tile (i_base - n B) / 128, then B/16 tiles of 16 KB
+    const unsigned char* strip = reinterpret_cast<const unsigned char*>(P.cache) + (size_t)slot * P.B * P.B * 8 +
+                                 (size_t)((i_base - (uint32_t)n * P.B) / TC_TP) * (P.B / (CT_KF / 2)) * CT_RAW;
 
     if (w == TC_GEN_WARPS + 1) {
         // ---- TMA producer: one lane ----
@@ -426,10 +441,11 @@ cached_multi_tc_kernel(const CtParams P, const __grid_constant__ CUtensorMap tma
                         smem_u32(psis + s * CT_PSI)),
                     "l"(P.psi + ((size_t)m * P.B + (size_t)t * (CT_KF / 2)) * P.k), "r"(psi_bytes), "r"(smem_u32(&raw_full[s]))
                     : "memory");
+                // tile t of the strip: 16 KB contiguous in the tiled cache layout (mfh_internal.cuh tiled_cache_offset)
                 asm volatile(
-                    "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::
-                        "r"(smem_u32(smem + s * CT_RAW)),
-                    "l"(&tmap), "r"(t * CT_KF), "r"(row0), "r"(smem_u32(&raw_full[s]))
+                    "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                        smem_u32(smem + s * CT_RAW)),
+                    "l"(strip + (size_t)t * CT_RAW), "r"(CT_RAW), "r"(smem_u32(&raw_full[s]))
                     : "memory");
             }
         }
@@ -441,14 +457,12 @@ cached_multi_tc_kernel(const CtParams P, const __grid_constant__ CUtensorMap tma
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             if (lane == 0) {
                 const uint32_t b0 = smem_u32(bimg + s * CT_BSTAGE);
-                const uint32_t a0 = d_tmem + (uint32_t)(TC_N + s * CT_A_STAGE_COLS);
+                const uint32_t a0 = d_tmem + (uint32_t)(TC_ACC_COLS + s * CT_A_STAGE_COLS);
 #pragma unroll
                 for (int ks = 0; ks < CT_KF / 8; ++ks) {
-                    const uint64_t b_h = umma_desc_sbo(b0 + ks * 2 * TC_LBO, CT_SBO);
-                    const uint64_t b_l = umma_desc_sbo(b0 + CT_B_TILE + ks * 2 * TC_LBO, CT_SBO);
-                    umma_tf32_ts(d_tmem, a0 + 8 * ks, b_h, (t | ks) != 0);
-                    umma_tf32_ts(d_tmem, a0 + 8 * ks, b_l, 1);
-                    umma_tf32_ts(d_tmem, a0 + CT_KF + 8 * ks, b_h, 1);
+                    const uint64_t b = umma_desc_sbo(b0 + ks * 2 * TC_LBO, CT_SBO);   // [B_hi | B_lo] / B_hi
+                    umma_tf32_ts<64>(d_tmem, a0 + 8 * ks, b, (t | ks) != 0);
+                    umma_tf32_ts<32>(d_tmem, a0 + CT_KF + 8 * ks, b, 1);
                 }
                 umma_commit(&a_empty[s]);
                 if (t == n_tiles - 1) umma_commit(&done);
@@ -487,7 +501,7 @@ cached_multi_tc_kernel(const CtParams P, const __grid_constant__ CUtensorMap tma
                 split_tf32(raw[gg].y, h1, l1);
                 split_tf32(raw[gg].z, h2, l2);
                 split_tf32(raw[gg].w, h3, l3);
-                const uint32_t ta = a_lane + (uint32_t)(TC_N + ts * CT_A_STAGE_COLS + 4 * g);
+                const uint32_t ta = a_lane + (uint32_t)(TC_ACC_COLS + ts * CT_A_STAGE_COLS + 4 * g);
                 tmem_st4(ta, h0, h1, h2, h3);
                 tmem_st4(ta + CT_KF, l0, l1, l2, l3);
             }
@@ -522,38 +536,6 @@ cached_multi_tc_kernel(const CtParams P, const __grid_constant__ CUtensorMap tma
 
 bool tc_cached_multi_supported(int dtype, int k, int B) { return dtype == MFH_C64 && k > 1 && k <= 16 && B % TC_TP == 0; }
 
-// Tensor map over the whole cache seen as [stored_blocks * B rows][2 B floats]; box = 128 rows x 32 floats.
-int make_cache_tensor_map(mfh_handle h)
-{
-    typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-    static EncodeFn encode = nullptr;
-    if (!encode) {
-        void* fn = nullptr;
-        cudaDriverEntryPointQueryResult qres;
-        MFH_CUDA_CHECK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
-        if (!fn || qres != cudaDriverEntryPointSuccess) {
-            set_error("cuTensorMapEncodeTiled is not available in this driver");
-            return MFH_ERR_CUDA;
-        }
-        encode = (EncodeFn)fn;
-    }
-    const Plan& p = h->plan;
-    const cuuint64_t dims[2] = {(cuuint64_t)2 * p.B, (cuuint64_t)p.n_cached * p.B};
-    const cuuint64_t strides[1] = {(cuuint64_t)2 * p.B * sizeof(float)};
-    const cuuint32_t box[2] = {CT_KF, TC_TP};
-    const cuuint32_t estr[2] = {1, 1};
-    const CUresult r = encode(&h->cache_tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, h->d_cache, dims, strides, box, estr,
-                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) {
-        set_error("cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
-        return MFH_ERR_CUDA;
-    }
-    return MFH_OK;
-}
-
 int launch_cached_multi_tc(mfh_handle h, const void* psi, cudaStream_t st)
 {
     const Plan& p = h->plan;
@@ -564,6 +546,7 @@ int launch_cached_multi_tc(mfh_handle h, const void* psi, cudaStream_t st)
     P.slot_multi = p.slot_multi;
     P.D = h->D;
     P.cache_slot = h->d_cache_slot;
+    P.cache = (const float2*)h->d_cache;
     P.psi = (const float2*)psi;
     P.work = (float2*)h->d_work;
     static bool attr_done = false;
@@ -571,7 +554,7 @@ int launch_cached_multi_tc(mfh_handle h, const void* psi, cudaStream_t st)
         MFH_CUDA_CHECK(cudaFuncSetAttribute(cached_multi_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, CT_SMEM));
         attr_done = true;
     }
-    cached_multi_tc_kernel<<<dim3((unsigned)(h->D / TC_TP), p.n_blk), CT_THREADS, CT_SMEM, st>>>(P, h->cache_tmap);
+    cached_multi_tc_kernel<<<dim3((unsigned)(h->D / TC_TP), p.n_blk), CT_THREADS, CT_SMEM, st>>>(P);
     MFH_CUDA_CHECK(cudaGetLastError());
     return MFH_OK;
 }
