@@ -104,6 +104,10 @@ using namespace mfh;
 extern "C" MFH_API int mfh_debug_pipe_rates(int32_t mix, double* units_per_s, void* stream)
 {
     if (!units_per_s) { set_error("mfh_debug_pipe_rates: NULL pointer"); return MFH_ERR_INVALID_ARG; }
+    if (mix < MFH_MIX_C128_PAIR || mix > MFH_MIX_DFMA31) {
+        set_error("mfh_debug_pipe_rates: unknown mix %d", mix);
+        return MFH_ERR_INVALID_ARG;
+    }
     int dev = 0, sms = 0;
     MFH_CUDA_CHECK(cudaGetDevice(&dev));
     MFH_CUDA_CHECK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));

@@ -1,6 +1,7 @@
 """CPU-only checks of the boundary: the C-ABI library loads and exports every symbol that
 include/mfh.h declares, host-side argument checking, and the analytic planner's arithmetic
 against the sizes the paper prints."""
+import ctypes
 import os
 import re
 
@@ -111,3 +112,25 @@ def test_planner_enumerates_block_sizes_and_ranks_feasible_first():
     assert flags == sorted(flags, reverse=True)
     feas = [c["model_job_s"] for c in r["candidates"] if c["feasible"]]
     assert feas == sorted(feas)
+
+
+def test_pairs_mode_and_pipe_rate_arguments():
+    # Hermitian pair cache in the analytic planner: half the bytes of the full cache, all entries covered
+    r = mfh.plan_analytic(65536, "c128", 1, "pairs", 2048, 100, 180 * 10**9)
+    ch = r["chosen"]
+    assert ch["mode"] == "pairs" and ch["cached_fraction"] == 1.0
+    assert ch["cached_blocks"] == 32 * 33 // 2 and ch["cache_bytes"] == 528 * 2048**2 * 16
+    # C5: the whole operator fits the 150 GB budget as pairs (141.7 GB), not as full blocks (275 GB)
+    r = mfh.plan_analytic(131072, "c128", 1, "pairs", 4096, 151, int(150e9 / 0.9))
+    assert r["chosen"]["cached_fraction"] == 1.0 and r["chosen"]["total_bytes"] <= 150e9
+    # k-vector plans: cached blocks need the tensor-core kernel (complex64, B % 128 == 0); never pairs
+    r = mfh.plan_analytic(32768, "c64", 16, "full", 1024, 100, 180 * 10**9)
+    assert r["chosen"]["feasible"] and r["chosen"]["cache_bytes"] == 32768**2 * 8
+    with pytest.raises(mfh.MfhError) as e:
+        mfh.plan_analytic(32768, "c128", 16, "full", 1024, 100, 180 * 10**9)
+    assert e.value.code == mfh.MFH_ERR_OUT_OF_MEMORY
+    # measurement export: argument errors come before any device work
+    L = mfh.lib()
+    out = ctypes.c_double(0.0)
+    assert L.mfh_debug_pipe_rates(99, ctypes.byref(out), None) == mfh.MFH_ERR_INVALID_ARG
+    assert L.mfh_debug_pipe_rates(0, None, None) == mfh.MFH_ERR_INVALID_ARG
