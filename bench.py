@@ -288,7 +288,8 @@ def roofline_for(res: dict, hbm_gbs: float, peak_src: str) -> dict:
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full captures
 # (profiles/r01_*_ncu_full*.md), keyed by (kernel, D).
 NCU_TRAFFIC = {("cached_kernel", 65536): 68.730302e9 + 4.515584e6,
-               ("cached_pairs_kernel", 65536): 35.438780e9 + 249.902592e6}
+               ("cached_pairs_kernel", 65536): 35.438780e9 + 249.902592e6,
+               ("cached_multi_tc_kernel", 32768): 8.596603e9 + 134.462720e6}
 ISSUE_LANES_PER_S = 148 * 4 * 32 * 1.965e9
 INSTR_PER_ENTRY = {("c128", "k1"): 44.0, ("c128", "kN"): 150.0, ("c64", "k1"): 40.0, ("c64", "kN"): 62.0}
 MIX_OF = {("c128", "k1"): ("c128_pair", 2), ("c64", "kN"): ("c64_entry", 1)}
