@@ -229,6 +229,17 @@ def measure_config(torch, mfh, name: str, steps: int, warmup: int, with_e2e: boo
     out = {"name": name, "cfg": cfg, "pipe_rate": mfh.pipe_rate, "plan": info, "plan_s": plan_s, "ms_total": ms, "steps": steps,
            "ms_per_step": ms / steps, "kernel_ms": kern, "psi_np": psi_np,
            "launches_per_apply": info["launches_per_apply"]}
+    if "t" in cfg and k == 1:
+        # BASELINE.json configs[4]: one Chebyshev propagation e^{-iHt} psi (K-1 applies), timed with events
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        outv, K = h.chebyshev(psi, cfg["t"], cfg["e_min"], cfg["e_max"], cfg["tol"])
+        b.record()
+        torch.cuda.synchronize()
+        out["chebyshev"] = {"t": cfg["t"], "tol": cfg["tol"], "bounds": [cfg["e_min"], cfg["e_max"]], "terms": K,
+                            "applies": K - 1, "seconds": a.elapsed_time(b) * 1e-3,
+                            "norm_error": abs(float(torch.linalg.vector_norm(outv).item()) - 1.0)}
+        del outv
     if with_e2e:
         ph = torch.from_numpy(psi_np).pin_memory()
         oh = torch.empty_like(ph).pin_memory()
@@ -368,6 +379,8 @@ def main():
                                 "ms_per_apply": r["ms_per_step"], "applies_per_s": 1e3 / r["ms_per_step"],
                                 "matrix_entries_per_s": c["D"] ** 2 / (r["ms_per_step"] * 1e-3),
                                 "kernel_ms": r["kernel_ms"], "roofline": rf, "plan_s": r["plan_s"]}
+                if "chebyshev" in r:
+                    extras[name]["chebyshev"] = r["chebyshev"]
             except Exception as e:  # a side measurement must not lose the headline line
                 extras[name] = {"error": str(e)}
 
