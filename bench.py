@@ -259,6 +259,17 @@ def roofline_for(res: dict, hbm_gbs: float, peak_src: str) -> dict:
     cfg = res["cfg"]
     D, k = cfg["D"], cfg["k"]
     kern = res["kernel_ms"]
+    if res["plan"]["mode"] == "partial" and kern["cached"] < 0.01 * kern["procedural"]:
+        # overlapped partial mode: ONE kernel streams the cached blocks and generates the rest (Eq. 33);
+        # its HBM roofline is the cached bytes over the whole kernel time
+        nbytes = res["plan"]["cache_bytes"]
+        gbs = nbytes / (kern["procedural"] * 1e-3) / 1e9
+        gen = D * D * (1.0 - res["plan"]["cached_fraction"]) / (kern["procedural"] * 1e-3)
+        return {"kernel": "partial_overlap_kernel", "bound": "hbm", "achieved": gbs, "peak": hbm_gbs, "unit": "GB/s",
+                "frac": gbs / hbm_gbs, "traffic": None, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": nbytes, "kernel_ms": kern["procedural"],
+                "generated_entries_per_s_in_the_same_kernel": gen,
+                "share_of_step": kern["procedural"] / max(kern["total"], 1e-9)}
     if kern["cached"] >= kern["procedural"]:
         # HBM-bound cached streaming: algorithmic bytes = stored entries * bytes per entry
         nbytes = res["plan"]["cache_bytes"]

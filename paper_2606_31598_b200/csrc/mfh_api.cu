@@ -133,9 +133,12 @@ static int apply_impl(mfh_handle h, const void* psi, void* phi, const double* la
     const Plan& p = h->plan;
     int rc;
     if (ev) cudaEventRecord(ev[0], st);
-    if ((rc = p.pairs ? launch_cached_pairs(h, psi, st) : launch_cached(h, psi, st))) return rc;
+    const bool overlap = partial_overlap_supported(h);   // cached and generated parts in one kernel (Eq. 33)
+    if (!overlap && (rc = p.pairs ? launch_cached_pairs(h, psi, st) : launch_cached(h, psi, st))) return rc;
     if (ev) cudaEventRecord(ev[1], st);
-    if (p.k == 1) {
+    if (overlap) {
+        if ((rc = launch_partial_overlap(h, psi, st))) return rc;
+    } else if (p.k == 1) {
         if ((rc = launch_proc_single(h, psi, st))) return rc;
     } else if (p.slot_multi >= 0 && p.covered_blocks < (int64_t)p.n_blk * p.n_blk) {
         if ((rc = launch_proc_multi(h, psi, st))) return rc;

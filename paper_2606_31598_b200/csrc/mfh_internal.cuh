@@ -115,6 +115,8 @@ int launch_fill_block(mfh_handle h, int32_t B, int32_t n, int32_t m, void* out, 
 int launch_fill_cache(mfh_handle h, cudaStream_t st);
 int launch_h0(mfh_handle h, void* out, cudaStream_t st);
 int launch_proc_single(mfh_handle h, const void* psi, cudaStream_t st);
+bool partial_overlap_supported(mfh_handle h);
+int launch_partial_overlap(mfh_handle h, const void* psi, cudaStream_t st);   // cached + generated in one kernel
 int launch_proc_multi(mfh_handle h, const void* psi, cudaStream_t st);
 bool tc_multi_supported(mfh_handle h);                                   // mfh_tc.cu
 int launch_proc_multi_tc(mfh_handle h, const void* psi, cudaStream_t st);

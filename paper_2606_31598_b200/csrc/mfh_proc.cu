@@ -185,12 +185,12 @@ template <typename T> struct ProcParams {
     int32_t* counter;
 };
 
+// The item loop of one CTA: runs until the device counter is exhausted.
 template <typename T, int R>
-__global__ void __launch_bounds__(PROC_THREADS, 2) proc_single_kernel(const ProcParams<T> P)
+__device__ __forceinline__ void proc_items(const ProcParams<T>& P, unsigned char* smem_raw)
 {
     using CT = typename Cplx<T>::type;
     constexpr int W = PROC_WARPS, TR = 32 * R;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const int B = P.B;
     const typename Gen<T>::Tab* tab = stage_gen_table<T>(P.G, smem_raw);
@@ -293,6 +293,117 @@ __global__ void __launch_bounds__(PROC_THREADS, 2) proc_single_kernel(const Proc
 }
 
 template <typename T, int R>
+__global__ void __launch_bounds__(PROC_THREADS, 2) proc_single_kernel(const ProcParams<T> P)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    proc_items<T, R>(P, smem_raw);
+}
+
+// --------------------------------------------------------------------------------------------
+// Partial-cache mode, overlapped (Eq. 33: T = max of the cached and the generated part
+// instead of their sum).  The cached part loads the memory pipe, the generated part the ALU
+// pipes, but two kernels that each fill the SMs run back to back.  So both parts run in ONE
+// persistent kernel with two CTAs per SM: CTAs of the first wave prefer fused generate-and-apply
+// items, CTAs of the second wave prefer cached row strips, and whoever exhausts its own queue
+// takes work from the other (two device counters).  A cached strip is 32 whole operator rows
+// (4 per warp, 4 x 4 independent 128-bit streaming loads per lane = 64 KB in flight per CTA)
+// over all cached blocks of the block row, psi^[m] staged in shared memory: the loop of
+// cached_kernel_c128 made persistent.  Same partial-sum slots and the same fixed-order reduce.
+// --------------------------------------------------------------------------------------------
+template <typename T> struct StripParams {
+    int32_t B, n_blk, slot_cache, n_strips;
+    int64_t D;
+    const int32_t* cache_slot;
+    const typename Cplx<T>::type* cache;
+    const typename Cplx<T>::type* psi;
+    typename Cplx<T>::type* work;
+    int32_t* counter;
+};
+
+constexpr int STRIP_RPW = 4, STRIP_ROWS = PROC_WARPS * STRIP_RPW, STRIP_U = 4;
+
+__device__ __forceinline__ double2 ldg_stream_d2(const double2* p)
+{
+    double2 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
+    return v;
+}
+
+__device__ __forceinline__ void cached_strips(const StripParams<double>& S, unsigned char* smem_raw)
+{
+    double2* psis = reinterpret_cast<double2*>(smem_raw);   // [B]
+    __shared__ int s_strip;
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    const int B = S.B;
+    for (;;) {
+        __syncthreads();
+        if (tid == 0) s_strip = atomicAdd(S.counter, 1);
+        __syncthreads();
+        const int it = s_strip;
+        if (it >= S.n_strips) break;
+        const int64_t row0 = (int64_t)it * STRIP_ROWS;
+        const int n = (int)(row0 / B);
+        const int a0 = (int)(row0 % B) + w * STRIP_RPW;
+        double accr[STRIP_RPW], acci[STRIP_RPW];
+#pragma unroll
+        for (int r = 0; r < STRIP_RPW; ++r) accr[r] = acci[r] = 0.0;
+        for (int m = 0; m < S.n_blk; ++m) {
+            const int32_t slot = S.cache_slot[n * S.n_blk + m];
+            if (slot < 0) continue;
+            __syncthreads();
+            for (int c = tid; c < B; c += PROC_THREADS) psis[c] = S.psi[(size_t)m * B + c];
+            __syncthreads();
+            const double2* rowp = S.cache + (size_t)slot * B * B + (size_t)a0 * B;
+            for (int c = lane; c < B; c += 32 * STRIP_U) {
+                double2 hv[STRIP_RPW][STRIP_U];
+#pragma unroll
+                for (int r = 0; r < STRIP_RPW; ++r)
+#pragma unroll
+                    for (int u = 0; u < STRIP_U; ++u)
+                        if (c + 32 * u < B) hv[r][u] = ldg_stream_d2(rowp + (size_t)r * B + c + 32 * u);
+#pragma unroll
+                for (int u = 0; u < STRIP_U; ++u) {
+                    if (c + 32 * u < B) {
+                        const double2 p = psis[c + 32 * u];
+#pragma unroll
+                        for (int r = 0; r < STRIP_RPW; ++r) {
+                            accr[r] = fma(hv[r][u].x, p.x, accr[r]);
+                            accr[r] = fma(-hv[r][u].y, p.y, accr[r]);
+                            acci[r] = fma(hv[r][u].x, p.y, acci[r]);
+                            acci[r] = fma(hv[r][u].y, p.x, acci[r]);
+                        }
+                    }
+                }
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < STRIP_RPW; ++r) {
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                accr[r] += __shfl_xor_sync(0xffffffffu, accr[r], o);
+                acci[r] += __shfl_xor_sync(0xffffffffu, acci[r], o);
+            }
+            if (lane == 0)
+                S.work[(size_t)S.slot_cache * S.D + row0 + w * STRIP_RPW + r] = double2{accr[r], acci[r]};
+        }
+    }
+}
+
+template <int R>
+__global__ void __launch_bounds__(PROC_THREADS, 2)
+partial_overlap_kernel(const ProcParams<double> P, const StripParams<double> S, int first_wave)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    if ((int)blockIdx.x < first_wave) {
+        proc_items<double, R>(P, smem_raw);
+        cached_strips(S, smem_raw);
+    } else {
+        cached_strips(S, smem_raw);
+        proc_items<double, R>(P, smem_raw);
+    }
+}
+
+template <typename T, int R>
 static int launch_proc_single_t(mfh_handle h, const void* psi, cudaStream_t st)
 {
     using CT = typename Cplx<T>::type;
@@ -337,6 +448,71 @@ int launch_proc_single(mfh_handle h, const void* psi, cudaStream_t st)
     case 4: return f64 ? launch_proc_single_t<double, 4>(h, psi, st) : launch_proc_single_t<float, 4>(h, psi, st);
     case 2: return f64 ? launch_proc_single_t<double, 2>(h, psi, st) : launch_proc_single_t<float, 2>(h, psi, st);
     case 1: return f64 ? launch_proc_single_t<double, 1>(h, psi, st) : launch_proc_single_t<float, 1>(h, psi, st);
+    }
+    set_error("unsupported rows per lane %d", h->plan.R);
+    return MFH_ERR_INVALID_ARG;
+}
+
+bool partial_overlap_supported(mfh_handle h)
+{
+    const Plan& p = h->plan;
+    static const bool off = getenv("MFH_PARTIAL_SEQUENTIAL") != nullptr;   // A/B measurements
+    return !off && h->dtype == MFH_C128 && p.k == 1 && !p.pairs && p.n_cached > 0 && !p.items.empty() &&
+           h->D % STRIP_ROWS == 0 && p.B % STRIP_ROWS == 0;
+}
+
+template <int R> static int launch_partial_overlap_t(mfh_handle h, const void* psi, cudaStream_t st)
+{
+    const Plan& p = h->plan;
+    ProcParams<double> P;
+    P.G = make_gen_args<double>(h);
+    P.B = p.B;
+    P.n_blk = p.n_blk;
+    P.n_items = (int32_t)p.items.size();
+    P.slot_row0 = p.slot_row0;
+    P.D = h->D;
+    P.items = h->d_items;
+    P.psi = (const double2*)psi;
+    P.work = (double2*)h->d_work;
+    P.counter = h->d_counter;
+    StripParams<double> S;
+    S.B = p.B;
+    S.n_blk = p.n_blk;
+    S.slot_cache = p.slot_cache;
+    S.n_strips = (int32_t)(h->D / STRIP_ROWS);
+    S.D = h->D;
+    S.cache_slot = h->d_cache_slot;
+    S.cache = (const double2*)h->d_cache;
+    S.psi = (const double2*)psi;
+    S.work = (double2*)h->d_work;
+    S.counter = h->d_counter + 1;
+    auto smem_for = [](int B) {
+        return (size_t)Gen<double>::TAB_BYTES + (size_t)(B + PROC_WARPS * 32 * R + PROC_WARPS * 32) * sizeof(double2);
+    };
+    const size_t smem = smem_for(p.B);
+    auto kern = partial_overlap_kernel<R>;
+    static bool attr_done = false;
+    if (!attr_done) {
+        MFH_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_for(MFH_MAX_B)));
+        attr_done = true;
+    }
+    int per_sm = 1;
+    MFH_CUDA_CHECK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, PROC_THREADS, smem));
+    if (per_sm < 1) per_sm = 1;
+    const int grid = h->sm_count * per_sm;
+    const int first_wave = per_sm > 1 ? h->sm_count * (per_sm / 2) : grid / 2;   // CTAs that prefer generated items
+    MFH_CUDA_CHECK(cudaMemsetAsync(h->d_counter, 0, 2 * sizeof(int32_t), st));
+    kern<<<grid, PROC_THREADS, smem, st>>>(P, S, first_wave);
+    MFH_CUDA_CHECK(cudaGetLastError());
+    return MFH_OK;
+}
+
+int launch_partial_overlap(mfh_handle h, const void* psi, cudaStream_t st)
+{
+    switch (h->plan.R) {
+    case 4: return launch_partial_overlap_t<4>(h, psi, st);
+    case 2: return launch_partial_overlap_t<2>(h, psi, st);
+    case 1: return launch_partial_overlap_t<1>(h, psi, st);
     }
     set_error("unsupported rows per lane %d", h->plan.R);
     return MFH_ERR_INVALID_ARG;
