@@ -162,6 +162,22 @@ def test_hermiticity_on_gpu():
     assert abs(np.vdot(a, Hb) - np.conj(np.vdot(b, Ha))) < 1e-13
 
 
+@pytest.mark.parametrize("mode,budget", [("procedural", 0), ("full", 0), ("partial", 30e6), ("pairs", 0), ("pairs", 20e6)])
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+def test_h0_plus_lambda_v_single_vector_all_modes(mode, budget, dtype):
+    # H = diag(h0) + lambda V with one vector: the epilogue of the reduce kernel on top of every cache mode
+    # (complex128 partial = the overlapped kernel, complex64 partial = cached + fused kernels back to back)
+    D, B, lam = 2048, 256, 0.7
+    psi = make_psi(D, 6, dtype=dtype)
+    if dtype == "c64":
+        budget = budget / 2
+    phi, plan, h = gpu_apply(D, B, 8, psi, dtype=dtype, mode=mode, budget=int(budget), kind="diag_plus_gue",
+                             lam=lam, seed_h0=7)
+    assert plan["chosen"]["mode"] == mode
+    ref = oracle.apply_scan(D, B, 8, 7, [lam], psi.reshape(D, 1))[:, 0]
+    assert rel_l2(phi, ref) <= TOL[dtype]
+
+
 def test_lambda_scales_single_vector():
     D, B = 1024, 256
     psi = make_psi(D, 4)
