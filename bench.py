@@ -240,6 +240,11 @@ def measure_config(torch, mfh, name: str, steps: int, warmup: int, with_e2e: boo
                             "applies": K - 1, "seconds": a.elapsed_time(b) * 1e-3,
                             "norm_error": abs(float(torch.linalg.vector_norm(outv).item()) - 1.0)}
         del outv
+        # NEXT-2: the bounds the paper's way, from 40 matrix-free Lanczos steps with a 5 % margin
+        t0 = time.perf_counter()
+        e0, e1, _, _ = h.lanczos_bounds(psi, m=40, margin=0.05)
+        out["chebyshev"]["lanczos_bounds"] = {"m": 40, "margin": 0.05, "e_min": e0, "e_max": e1,
+                                              "seconds": time.perf_counter() - t0}
     if with_e2e:
         ph = torch.from_numpy(psi_np).pin_memory()
         oh = torch.empty_like(ph).pin_memory()

@@ -127,6 +127,24 @@ MFH_API int mfh_apply_host(mfh_handle h, const void* psi_host, void* phi_host, i
 MFH_API int mfh_chebyshev(mfh_handle h, const void* psi_dev, void* out_dev, double t, double e_min,
                           double e_max, double tol, int32_t* n_terms_out, void* stream);
 
+/* Spectral bounds by matrix-free Lanczos ("matrix-free Lanczos iterations estimate spectral bounds
+ * E_min and E_max"; --lanczos-m 40; reading R18).  m steps (capped at D) of the plain
+ * three-term recurrence from v_1 = psi/||psi||, each step one apply of the planned path (k = 1) plus O(D)
+ * vector kernels with the scalars kept on the device; theta_min, theta_max = extreme eigenvalues of the
+ * tridiagonal T_m (host, Sturm bisection); with c, R the centre and half-width of [theta_min, theta_max]:
+ *     *e_min = c - (1 + margin) R,   *e_max = c + (1 + margin) R        (Ritz values lie inside the spectrum).
+ *   psi_dev              start vector (device, [D] complex), any non-zero norm; not modified
+ *   alpha_host, beta_host  optional host arrays of m doubles receiving the recurrence coefficients
+ * Synchronises `stream`.  Errors: INVALID_ARG, BAD_STATE (no plan), NOT_CONVERGED (breakdown), CUDA. */
+MFH_API int mfh_lanczos_bounds(mfh_handle h, const void* psi_dev, int32_t m, double margin, double* e_min,
+                               double* e_max, double* alpha_host, double* beta_host, void* stream);
+
+/* n_steps successive propagations out = [exp(-i H tau)]^n_steps psi, each one Chebyshev expansion as in
+ * mfh_chebyshev (the paper propagates N = 200 steps of tau).  out_dev must not alias psi_dev.
+ * *n_terms_out = terms per step. */
+MFH_API int mfh_chebyshev_steps(mfh_handle h, const void* psi_dev, void* out_dev, double tau, int32_t n_steps,
+                                double e_min, double e_max, double tol, int32_t* n_terms_out, void* stream);
+
 /* Free the handle and everything it owns.  NULL is accepted. */
 MFH_API int mfh_destroy(mfh_handle h);
 

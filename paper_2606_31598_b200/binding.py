@@ -27,7 +27,7 @@ MODES = {"auto": MFH_MODE_AUTO, "procedural": MFH_MODE_PROCEDURAL, "partial": MF
 
 # every symbol include/mfh.h declares (tests check that the library exports all of them)
 SYMBOLS = ["mfh_create", "mfh_plan_analytic", "mfh_plan", "mfh_apply", "mfh_apply_host", "mfh_apply_timed",
-           "mfh_chebyshev", "mfh_destroy", "mfh_last_error", "mfh_get_plan", "mfh_debug_philox",
+           "mfh_chebyshev", "mfh_chebyshev_steps", "mfh_lanczos_bounds", "mfh_destroy", "mfh_last_error", "mfh_get_plan", "mfh_debug_philox",
            "mfh_materialize_block", "mfh_debug_h0", "mfh_debug_pipe_rates"]
 
 _lib = None
@@ -58,6 +58,9 @@ def lib():
     L.mfh_apply_host.argtypes = [vp, vp, vp, i32, ctypes.POINTER(dbl), vp]
     L.mfh_apply_timed.argtypes = [vp, vp, vp, i32, ctypes.POINTER(dbl), vp, ctypes.POINTER(ctypes.c_float)]
     L.mfh_chebyshev.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, ctypes.POINTER(i32), vp]
+    L.mfh_chebyshev_steps.argtypes = [vp, vp, vp, dbl, i32, dbl, dbl, dbl, ctypes.POINTER(i32), vp]
+    L.mfh_lanczos_bounds.argtypes = [vp, vp, i32, dbl, ctypes.POINTER(dbl), ctypes.POINTER(dbl), ctypes.POINTER(dbl),
+                                     ctypes.POINTER(dbl), vp]
     L.mfh_destroy.argtypes = [vp]
     L.mfh_last_error.argtypes = []
     L.mfh_last_error.restype = cp
@@ -173,6 +176,28 @@ class Hamiltonian:
         _check(lib().mfh_chebyshev(self._h, psi.data_ptr(), out.data_ptr(), t, e_min, e_max, tol,
                                    ctypes.byref(n), _stream()))
         return out, int(n.value)
+
+    def chebyshev_steps(self, psi, tau: float, n_steps: int, e_min: float, e_max: float, tol: float, out=None):
+        import torch
+        self._check_vec(psi, 1)
+        if out is None:
+            out = torch.empty_like(psi)
+        n = ctypes.c_int32(0)
+        _check(lib().mfh_chebyshev_steps(self._h, psi.data_ptr(), out.data_ptr(), tau, n_steps, e_min, e_max, tol,
+                                         ctypes.byref(n), _stream()))
+        return out, int(n.value)
+
+    def lanczos_bounds(self, psi, m: int = 40, margin: float = 0.05):
+        """(e_min, e_max, alpha[m], beta[m]) from m matrix-free Lanczos steps started at psi."""
+        import numpy as np
+        self._check_vec(psi, 1)
+        mm = min(m, self.D)
+        e0, e1 = ctypes.c_double(0.0), ctypes.c_double(0.0)
+        alpha = (ctypes.c_double * mm)()
+        beta = (ctypes.c_double * mm)()
+        _check(lib().mfh_lanczos_bounds(self._h, psi.data_ptr(), m, margin, ctypes.byref(e0), ctypes.byref(e1),
+                                        alpha, beta, _stream()))
+        return float(e0.value), float(e1.value), np.array(alpha[:]), np.array(beta[:])
 
     def materialize_block(self, n: int, m: int, B: int):
         import torch

@@ -39,7 +39,7 @@ static int free_plan_resources(mfh_handle h)
 {
     void** ptrs[] = {&h->d_cache, &h->d_work, &h->d_h0, (void**)&h->d_cache_slot, (void**)&h->d_items,
                      (void**)&h->d_pair_items,
-                     (void**)&h->d_slot_list, (void**)&h->d_counter, &h->d_cheb, &h->d_io};
+                     (void**)&h->d_slot_list, (void**)&h->d_counter, &h->d_cheb, &h->d_io, &h->d_lanczos};
     for (void** p : ptrs) {
         if (*p) cudaFree(*p);
         *p = nullptr;
@@ -417,7 +417,7 @@ MFH_API int mfh_chebyshev(mfh_handle h, const void* psi_dev, void* out_dev, doub
     if (n_terms_out) *n_terms_out = K;
 
     const size_t vb = (size_t)h->D * complex_bytes(h->dtype);
-    if (!h->d_cheb) MFH_CUDA_CHECK(cudaMalloc(&h->d_cheb, 4 * vb));
+    if (!h->d_cheb) MFH_CUDA_CHECK(cudaMalloc(&h->d_cheb, 5 * vb));   // cur, prev, acc, Hq + ping-pong of mfh_chebyshev_steps
     char* base = (char*)h->d_cheb;
     void *cur = base, *prev = base + vb, *acc = base + 2 * vb, *hq = base + 3 * vb;
     int rc;
@@ -435,6 +435,111 @@ MFH_API int mfh_chebyshev(mfh_handle h, const void* psi_dev, void* out_dev, doub
         std::swap(cur, prev);
     }
     return launch_cheb_final(h, acc, out_dev, std::cos(c * t), -std::sin(c * t), st);
+}
+
+// Extreme eigenvalues of the symmetric tridiagonal T (diagonal a[0..m-1], off-diagonal b[0..m-2]) by
+// Sturm-sequence bisection inside the Gershgorin interval (host; m <= a few hundred).
+static void tridiag_extremes(const std::vector<double>& a, const std::vector<double>& b, int m, double& tmin, double& tmax)
+{
+    double lo = a[0], hi = a[0];
+    for (int j = 0; j < m; ++j) {
+        const double r = (j > 0 ? std::fabs(b[j - 1]) : 0.0) + (j < m - 1 ? std::fabs(b[j]) : 0.0);
+        lo = std::min(lo, a[j] - r);
+        hi = std::max(hi, a[j] + r);
+    }
+    auto count_below = [&](double x) {   // number of eigenvalues < x
+        int cnt = 0;
+        double q = a[0] - x;
+        if (q < 0) ++cnt;
+        for (int j = 1; j < m; ++j) {
+            const double d = (q == 0.0) ? 1e-300 : q;
+            q = a[j] - x - b[j - 1] * b[j - 1] / d;
+            if (q < 0) ++cnt;
+        }
+        return cnt;
+    };
+    auto kth = [&](int kk) {   // kk-th smallest eigenvalue (0-based)
+        double l = lo, h = hi;
+        for (int it = 0; it < 200 && h - l > 4e-16 * std::max(std::fabs(l), std::fabs(h)); ++it) {
+            const double mid = 0.5 * (l + h);
+            if (count_below(mid) > kk) h = mid; else l = mid;
+        }
+        return 0.5 * (l + h);
+    };
+    tmin = kth(0);
+    tmax = kth(m - 1);
+}
+
+MFH_API int mfh_lanczos_bounds(mfh_handle h, const void* psi_dev, int32_t m, double margin, double* e_min,
+                               double* e_max, double* alpha_host, double* beta_host, void* stream)
+{
+    if (!h || !psi_dev || !e_min || !e_max) { set_error("mfh_lanczos_bounds: NULL pointer"); return MFH_ERR_INVALID_ARG; }
+    if (m < 1 || m > 4096 || !(margin >= 0.0) || !std::isfinite(margin)) {
+        set_error("mfh_lanczos_bounds: need 1 <= m <= 4096 and margin >= 0");
+        return MFH_ERR_INVALID_ARG;
+    }
+    if (!h->planned) { set_error("mfh_lanczos_bounds: call mfh_plan first"); return MFH_ERR_BAD_STATE; }
+    if (h->plan.k != 1) { set_error("mfh_lanczos_bounds: plan with k = 1"); return MFH_ERR_INVALID_ARG; }
+    cudaStream_t st = (cudaStream_t)stream;
+    m = (int32_t)std::min<int64_t>(m, h->D);
+    const size_t vb = (size_t)h->D * complex_bytes(h->dtype);
+    const size_t scal_doubles = 2 * 4096 + 8 + (size_t)lz_partial_doubles();
+    if (!h->d_lanczos) MFH_CUDA_CHECK(cudaMalloc(&h->d_lanczos, 3 * vb + scal_doubles * sizeof(double)));
+    char* base = (char*)h->d_lanczos;
+    void *v = base, *v_prev = base + vb, *w = base + 2 * vb;
+    double* d_alpha = (double*)(base + 3 * vb);
+    double* d_beta = d_alpha + 4096;
+    double* d_norm0 = d_beta + 4096;
+    double* d_partial = d_norm0 + 8;
+    int rc;
+    // v_1 = psi / ||psi||
+    if ((rc = launch_lz_dot(h, psi_dev, psi_dev, d_partial, d_norm0, 1, st))) return rc;
+    if ((rc = launch_lz_scale(h, psi_dev, v, d_norm0, st))) return rc;
+    for (int j = 0; j < m; ++j) {
+        if ((rc = apply_impl(h, v, w, nullptr, st))) return rc;                                   // w = H v_j
+        if ((rc = launch_lz_dot(h, v, w, d_partial, d_alpha + j, 0, st))) return rc;              // alpha_j = Re <v_j, w>
+        if ((rc = launch_lz_update(h, w, v, v_prev, d_alpha + j, j ? d_beta + j - 1 : nullptr,    // w -= alpha v + beta v_prev
+                                   d_partial, d_beta + j, st))) return rc;                        // beta_j = ||w||
+        if ((rc = launch_lz_scale(h, w, v_prev, d_beta + j, st))) return rc;                      // v_{j+1} = w / beta_j
+        std::swap(v, v_prev);
+    }
+    std::vector<double> a(m), b(m);
+    MFH_CUDA_CHECK(cudaMemcpyAsync(a.data(), d_alpha, m * sizeof(double), cudaMemcpyDeviceToHost, st));
+    MFH_CUDA_CHECK(cudaMemcpyAsync(b.data(), d_beta, m * sizeof(double), cudaMemcpyDeviceToHost, st));
+    MFH_CUDA_CHECK(cudaStreamSynchronize(st));
+    for (int j = 0; j < m; ++j)
+        if (!std::isfinite(a[j]) || !std::isfinite(b[j])) {
+            set_error("mfh_lanczos_bounds: breakdown at step %d (invariant subspace or zero start vector)", j);
+            return MFH_ERR_NOT_CONVERGED;
+        }
+    double tmin, tmax;
+    tridiag_extremes(a, b, m, tmin, tmax);
+    const double c = 0.5 * (tmax + tmin), R = 0.5 * (tmax - tmin);
+    *e_min = c - (1.0 + margin) * R;
+    *e_max = c + (1.0 + margin) * R;
+    if (alpha_host) memcpy(alpha_host, a.data(), m * sizeof(double));
+    if (beta_host) memcpy(beta_host, b.data(), m * sizeof(double));
+    return MFH_OK;
+}
+
+MFH_API int mfh_chebyshev_steps(mfh_handle h, const void* psi_dev, void* out_dev, double tau, int32_t n_steps,
+                                double e_min, double e_max, double tol, int32_t* n_terms_out, void* stream)
+{
+    if (n_steps < 1) { set_error("mfh_chebyshev_steps: n_steps must be >= 1"); return MFH_ERR_INVALID_ARG; }
+    if (!h || !psi_dev || !out_dev || psi_dev == out_dev) {
+        set_error("mfh_chebyshev_steps: NULL or aliased pointer");
+        return MFH_ERR_INVALID_ARG;
+    }
+    // out <- U(tau) psi, then out <- U(tau) out through the library's own ping-pong buffer
+    int rc = mfh_chebyshev(h, psi_dev, out_dev, tau, e_min, e_max, tol, n_terms_out, stream);
+    if (rc || n_steps == 1) return rc;
+    const size_t vb = (size_t)h->D * complex_bytes(h->dtype);
+    char* scratch = (char*)h->d_cheb + 4 * vb;   // fifth vector of the Chebyshev scratch (allocated below)
+    for (int s = 1; s < n_steps; ++s) {
+        MFH_CUDA_CHECK(cudaMemcpyAsync(scratch, out_dev, vb, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+        if ((rc = mfh_chebyshev(h, scratch, out_dev, tau, e_min, e_max, tol, nullptr, stream))) return rc;
+    }
+    return MFH_OK;
 }
 
 MFH_API int mfh_debug_philox(uint64_t seed, uint32_t stream_id, const uint32_t* i_dev,

@@ -85,6 +85,7 @@ struct mfh_handle_s {
     int32_t* d_counter = nullptr;   // dynamic work counters: [0] procedural kernel, [1] pair kernel
     void* d_cheb = nullptr;         // 3 vectors of Chebyshev scratch
     void* d_io = nullptr;           // psi/phi staging of mfh_apply_host
+    void* d_lanczos = nullptr;      // 3 Lanczos vectors + alpha/beta/norm scalars + reduction partials
     mfh::GenHostD gen_host;         // generator table + constants for this D (host copy)
     mfh::GenTabD* d_gen_tab = nullptr;   // device copy (c128 only), kept until mfh_destroy
     bool gen_ready = false;
@@ -131,5 +132,10 @@ int launch_cheb_step(mfh_handle h, const void* hq, const void* q, void* prev_dst
                      double inv_r, int first, double coef_re, double coef_im, cudaStream_t st);
 int launch_cheb_final(mfh_handle h, const void* acc, void* out, double ph_re, double ph_im,
                       cudaStream_t st);
+int launch_lz_dot(mfh_handle h, const void* x, const void* y, double* partial, double* dst, int take_sqrt, cudaStream_t st);
+int launch_lz_update(mfh_handle h, void* w, const void* v, const void* v_prev, const double* alpha, const double* beta_prev,
+                     double* partial, double* beta_dst, cudaStream_t st);
+int launch_lz_scale(mfh_handle h, const void* src, void* dst, const double* scale, cudaStream_t st);
+int lz_partial_doubles();
 
 }  // namespace mfh

@@ -210,4 +210,144 @@ int launch_cheb_final(mfh_handle h, const void* acc, void* out, double ph_re, do
     return MFH_OK;
 }
 
+// ---- Lanczos ("matrix-free Lanczos iterations estimate spectral bounds") ----------------
+// All scalars stay on the device (alpha[], beta[] arrays), so the m steps run without a host
+// synchronisation; reductions are two-stage (per-CTA partial, then one CTA adds the partials in
+// index order): deterministic.
+constexpr int LZ_BLOCKS = 296, LZ_THREADS = 256;
+
+template <typename T>
+__device__ __forceinline__ void block_sum2(double& a, double& b)
+{
+    __shared__ double sa[LZ_THREADS / 32], sb[LZ_THREADS / 32];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        a += __shfl_xor_sync(0xffffffffu, a, o);
+        b += __shfl_xor_sync(0xffffffffu, b, o);
+    }
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (lane == 0) { sa[w] = a; sb[w] = b; }
+    __syncthreads();
+    if (w == 0) {
+        a = lane < LZ_THREADS / 32 ? sa[lane] : 0.0;
+        b = lane < LZ_THREADS / 32 ? sb[lane] : 0.0;
+#pragma unroll
+        for (int o = 4; o > 0; o >>= 1) {
+            a += __shfl_xor_sync(0xffffffffu, a, o);
+            b += __shfl_xor_sync(0xffffffffu, b, o);
+        }
+    }
+}
+
+// partial[2b], partial[2b+1] = sum over CTA b's elements of conj(x) y  (x == y gives the squared norm)
+template <typename T>
+__global__ void __launch_bounds__(LZ_THREADS) lz_dot_kernel(int64_t D, const typename Cplx<T>::type* __restrict__ x,
+                                                            const typename Cplx<T>::type* __restrict__ y,
+                                                            double* __restrict__ partial)
+{
+    double re = 0.0, im = 0.0;
+    for (int64_t i = blockIdx.x * (int64_t)LZ_THREADS + threadIdx.x; i < D; i += (int64_t)gridDim.x * LZ_THREADS) {
+        const auto a = x[i], b = y[i];
+        re += (double)a.x * (double)b.x + (double)a.y * (double)b.y;
+        im += (double)a.x * (double)b.y - (double)a.y * (double)b.x;
+    }
+    block_sum2<T>(re, im);
+    if (threadIdx.x == 0) { partial[2 * blockIdx.x] = re; partial[2 * blockIdx.x + 1] = im; }
+}
+
+// One CTA: dst[0] = Re(sum of partials) (take_sqrt == 0) or sqrt of it (take_sqrt == 1).
+__global__ void __launch_bounds__(32) lz_finalize_kernel(const double* __restrict__ partial, int n, double* dst, int take_sqrt)
+{
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int b = 0; b < n; ++b) s += partial[2 * b];
+        dst[0] = take_sqrt ? sqrt(s) : s;
+    }
+}
+
+// w = w - alpha v - beta_prev v_prev, and the partial squared norm of the new w.
+template <typename T>
+__global__ void __launch_bounds__(LZ_THREADS) lz_update_kernel(int64_t D, typename Cplx<T>::type* __restrict__ w,
+                                                               const typename Cplx<T>::type* __restrict__ v,
+                                                               const typename Cplx<T>::type* __restrict__ v_prev,
+                                                               const double* __restrict__ alpha, const double* __restrict__ beta_prev,
+                                                               double* __restrict__ partial)
+{
+    using CT = typename Cplx<T>::type;
+    const double a = alpha[0], bp = beta_prev ? beta_prev[0] : 0.0;
+    double re = 0.0, im = 0.0;
+    for (int64_t i = blockIdx.x * (int64_t)LZ_THREADS + threadIdx.x; i < D; i += (int64_t)gridDim.x * LZ_THREADS) {
+        const CT wv = w[i], vv = v[i];
+        double xr = (double)wv.x - a * (double)vv.x, xi = (double)wv.y - a * (double)vv.y;
+        if (beta_prev) {
+            const CT pv = v_prev[i];
+            xr -= bp * (double)pv.x;
+            xi -= bp * (double)pv.y;
+        }
+        CT o;
+        o.x = (T)xr;
+        o.y = (T)xi;
+        w[i] = o;
+        re += (double)o.x * (double)o.x + (double)o.y * (double)o.y;
+    }
+    block_sum2<T>(re, im);
+    if (threadIdx.x == 0) { partial[2 * blockIdx.x] = re; partial[2 * blockIdx.x + 1] = 0.0; }
+}
+
+// dst = src / scale[0]
+template <typename T>
+__global__ void __launch_bounds__(LZ_THREADS) lz_scale_kernel(int64_t D, const typename Cplx<T>::type* __restrict__ src,
+                                                              typename Cplx<T>::type* __restrict__ dst, const double* __restrict__ scale)
+{
+    using CT = typename Cplx<T>::type;
+    const double inv = 1.0 / scale[0];
+    for (int64_t i = blockIdx.x * (int64_t)LZ_THREADS + threadIdx.x; i < D; i += (int64_t)gridDim.x * LZ_THREADS) {
+        const CT s = src[i];
+        CT o;
+        o.x = (T)((double)s.x * inv);
+        o.y = (T)((double)s.y * inv);
+        dst[i] = o;
+    }
+}
+
+template <typename T> static int lz_dot_t(mfh_handle h, const void* x, const void* y, double* partial, cudaStream_t st)
+{
+    using CT = typename Cplx<T>::type;
+    lz_dot_kernel<T><<<LZ_BLOCKS, LZ_THREADS, 0, st>>>(h->D, (const CT*)x, (const CT*)y, partial);
+    MFH_CUDA_CHECK(cudaGetLastError());
+    return MFH_OK;
+}
+int launch_lz_dot(mfh_handle h, const void* x, const void* y, double* partial, double* dst, int take_sqrt, cudaStream_t st)
+{
+    int rc = h->dtype == MFH_C128 ? lz_dot_t<double>(h, x, y, partial, st) : lz_dot_t<float>(h, x, y, partial, st);
+    if (rc) return rc;
+    lz_finalize_kernel<<<1, 32, 0, st>>>(partial, LZ_BLOCKS, dst, take_sqrt);
+    MFH_CUDA_CHECK(cudaGetLastError());
+    return MFH_OK;
+}
+int launch_lz_update(mfh_handle h, void* w, const void* v, const void* v_prev, const double* alpha, const double* beta_prev,
+                     double* partial, double* beta_dst, cudaStream_t st)
+{
+    if (h->dtype == MFH_C128)
+        lz_update_kernel<double><<<LZ_BLOCKS, LZ_THREADS, 0, st>>>(h->D, (double2*)w, (const double2*)v, (const double2*)v_prev,
+                                                                   alpha, beta_prev, partial);
+    else
+        lz_update_kernel<float><<<LZ_BLOCKS, LZ_THREADS, 0, st>>>(h->D, (float2*)w, (const float2*)v, (const float2*)v_prev,
+                                                                  alpha, beta_prev, partial);
+    MFH_CUDA_CHECK(cudaGetLastError());
+    lz_finalize_kernel<<<1, 32, 0, st>>>(partial, LZ_BLOCKS, beta_dst, 1);
+    MFH_CUDA_CHECK(cudaGetLastError());
+    return MFH_OK;
+}
+int launch_lz_scale(mfh_handle h, const void* src, void* dst, const double* scale, cudaStream_t st)
+{
+    if (h->dtype == MFH_C128)
+        lz_scale_kernel<double><<<LZ_BLOCKS, LZ_THREADS, 0, st>>>(h->D, (const double2*)src, (double2*)dst, scale);
+    else
+        lz_scale_kernel<float><<<LZ_BLOCKS, LZ_THREADS, 0, st>>>(h->D, (const float2*)src, (float2*)dst, scale);
+    MFH_CUDA_CHECK(cudaGetLastError());
+    return MFH_OK;
+}
+int lz_partial_doubles() { return 2 * LZ_BLOCKS; }
+
 }  // namespace mfh
