@@ -61,3 +61,18 @@ def sample_rows(D: int, n: int, seed: int = 0) -> np.ndarray:
     fixed = np.array([0, 1, D // 2 - 1, D // 2, D - 2, D - 1], dtype=np.int64)
     rand = rng.integers(0, D, size=n, dtype=np.int64)
     return np.unique(np.concatenate([fixed, rand]))
+
+
+def small_hermitian(d: int, seed: int) -> np.ndarray:
+    """Seeded d x d Hermitian matrix with O(1) entries (system-side operators H_S, A of the system-bath
+    workload; an input of the method, not part of its arithmetic)."""
+    rng = np.random.default_rng([seed, d])
+    M = rng.standard_normal((d, d)) + 1j * rng.standard_normal((d, d))
+    return (M + M.conj().T) / 2.0
+
+
+# The paper's own run (P:691-703, P:771-775): 18 qubits, d_S = 4, d_B = 65536, complex64, two cached dense
+# bath-side operators (H_B, B_1) applied to R = 4 columns, N_blk = 16 (b = 4096).  Operators synthetic (R19).
+SYSTEM_BATH = dict(d_B=65536, d_S=4, B=4096, dtype="c64", seed_HB=31, seed_B1=32, seed_HS=33, seed_A=34,
+                   g=0.5, psi_seed=35, mode="full", paper_seconds_per_apply=0.104089,
+                   paper_hardware="2 x NVIDIA L40S (one row group), CuPy, complex64 (P:771-775)")
