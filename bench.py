@@ -29,7 +29,8 @@ if ROOT not in sys.path:
 
 import numpy as np  # noqa: E402
 
-from paper_2606_31598_b200.inputs import CONFIGS, VARIANTS, lambda_grid, make_psi, sample_rows  # noqa: E402
+from paper_2606_31598_b200.inputs import (CONFIGS, SYSTEM_BATH, VARIANTS, lambda_grid, make_psi, sample_rows,  # noqa: E402
+                                          small_hermitian)
 
 ALL = dict(CONFIGS, **VARIANTS)
 
@@ -259,6 +260,36 @@ def measure_config(torch, mfh, name: str, steps: int, warmup: int, with_e2e: boo
     return out
 
 
+def measure_system_bath(torch, mfh, steps: int, hbm_gbs: float) -> dict:
+    """NEXT-3: the paper's own workload shape: 18 qubits, two cached dense complex64
+    bath-side operators (32 GiB each) applied to R = d_S = 4 columns; operators synthetic (R19)."""
+    c = SYSTEM_BATH
+    d_B, d_S = c["d_B"], c["d_S"]
+    sb = mfh.SystemBath(d_B, d_S, c["B"], c["seed_HB"], c["seed_B1"], small_hermitian(d_S, c["seed_HS"]),
+                        small_hermitian(d_S, c["seed_A"]), c["g"], dtype=c["dtype"])
+    t0 = time.perf_counter()
+    plan = sb.plan(c["mode"], n_applies_hint=steps)
+    torch.cuda.synchronize()
+    plan_s = time.perf_counter() - t0
+    X = torch.from_numpy(make_psi(d_B, c["psi_seed"], k=d_S, dtype=c["dtype"])).cuda()
+    Y = torch.empty_like(X)
+    for _ in range(3):
+        sb.apply(X, Y)
+    torch.cuda.synchronize()
+    ms = time_steps(torch, lambda: sb.apply(X, Y), steps) / steps
+    nbytes = plan["H_B"]["cache_bytes"] + plan["B_1"]["cache_bytes"]
+    sb.destroy()
+    del X, Y
+    torch.cuda.empty_cache()
+    return {"workload": f"system-bath 18 qubits: d_S={d_S}, d_B={d_B}, {c['dtype']}, B={c['B']}, 2 cached bath operators x {d_S} columns",
+            "ms_per_apply": ms, "applies_per_s": 1e3 / ms, "flops_per_apply": plan["flops_per_apply"],
+            "cached_bytes": nbytes, "achieved_gbs": nbytes / (ms * 1e-3) / 1e9, "frac_of_measured_hbm": nbytes / (ms * 1e-3) / 1e9 / hbm_gbs,
+            "plan_and_fill_s": plan_s,
+            "paper": {"seconds_per_apply": c["paper_seconds_per_apply"], "hardware": c["paper_hardware"],
+                      "note": "context only: other machine, the paper's own (unpublished) operators",
+                      "ratio_paper_over_this": c["paper_seconds_per_apply"] / (ms * 1e-3)}}
+
+
 def roofline_for(res: dict, hbm_gbs: float, peak_src: str) -> dict:
     """Roofline of the dominant kernel of one apply."""
     cfg = res["cfg"]
@@ -399,6 +430,10 @@ def main():
                     extras[name]["chebyshev"] = r["chebyshev"]
             except Exception as e:  # a side measurement must not lose the headline line
                 extras[name] = {"error": str(e)}
+        try:
+            extras["SB18"] = measure_system_bath(torch, mfh, 10, hbm_gbs)
+        except Exception as e:
+            extras["SB18"] = {"error": str(e)}
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,

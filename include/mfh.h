@@ -154,6 +154,24 @@ MFH_API const char* mfh_last_error(void);
 /* JSON description of the committed plan (mode, B, cached blocks, bytes, launches per apply). */
 MFH_API int mfh_get_plan(mfh_handle h, char* json_out, size_t json_cap);
 
+/* ---- system-bath Hamiltonian (the paper's own workload shape, R19) -------
+ *     H = H_S (x) I_B + I_S (x) H_B + g A (x) B_1   on   w in C^{d_S} (x) C^{d_B}
+ * with H_B, B_1 two dense d_B x d_B bath-side operators (seeded GUE, entry rule of mfh_create) applied
+ * to R = d_S simultaneous state components (Eq. 12-13, n_op = 2).  The state is X[b][s], row-major
+ * [d_B][d_S] complex of `dtype` (the k-vector layout with D = d_B, k = d_S); the result
+ *     Y = H_B X + g (B_1 X) A^T + X H_S^T.
+ *   HS_host, A_host   d_S x d_S Hermitian matrices, row-major interleaved complex doubles (host)
+ *   d_S <= MFH_MAX_K; d_B, B as in mfh_create.  mfh_sb_plan plans both bath operators with k = d_S
+ *   (cached blocks need complex64 and B % 128 == 0) inside the budget (0 = 0.9 x free memory).
+ * Errors as for mfh_create / mfh_plan / mfh_apply. */
+typedef struct mfh_sb_s* mfh_sb_handle;
+MFH_API int mfh_sb_create(mfh_sb_handle* out, int64_t d_B, int32_t d_S, int32_t B, uint64_t seed_HB, uint64_t seed_B1,
+                          int32_t dtype, const double* HS_host, const double* A_host, double g);
+MFH_API int mfh_sb_plan(mfh_sb_handle h, int32_t mode, int64_t n_applies_hint, int64_t hbm_budget_bytes, void* stream,
+                        char* json_out, size_t json_cap);
+MFH_API int mfh_sb_apply(mfh_sb_handle h, const void* x_dev, void* y_dev, void* stream);
+MFH_API int mfh_sb_destroy(mfh_sb_handle h);
+
 /* ---- test-only exports --------------------------------------------------------------------- */
 
 /* Raw Philox4x32-10 words for n index pairs: key = seed, ctr = (min(i,j), max(i,j), stream_id, 0).

@@ -28,7 +28,8 @@ MODES = {"auto": MFH_MODE_AUTO, "procedural": MFH_MODE_PROCEDURAL, "partial": MF
 # every symbol include/mfh.h declares (tests check that the library exports all of them)
 SYMBOLS = ["mfh_create", "mfh_plan_analytic", "mfh_plan", "mfh_apply", "mfh_apply_host", "mfh_apply_timed",
            "mfh_chebyshev", "mfh_chebyshev_steps", "mfh_lanczos_bounds", "mfh_destroy", "mfh_last_error", "mfh_get_plan", "mfh_debug_philox",
-           "mfh_materialize_block", "mfh_debug_h0", "mfh_debug_pipe_rates"]
+           "mfh_materialize_block", "mfh_debug_h0", "mfh_debug_pipe_rates", "mfh_sb_create", "mfh_sb_plan", "mfh_sb_apply",
+           "mfh_sb_destroy"]
 
 _lib = None
 
@@ -69,6 +70,10 @@ def lib():
     L.mfh_materialize_block.argtypes = [vp, i32, i32, vp, vp]
     L.mfh_debug_h0.argtypes = [vp, vp, vp]
     L.mfh_debug_pipe_rates.argtypes = [i32, ctypes.POINTER(dbl), vp]
+    L.mfh_sb_create.argtypes = [ctypes.POINTER(vp), i64, i32, i32, u64, u64, i32, vp, vp, dbl]
+    L.mfh_sb_plan.argtypes = [vp, i32, i64, i64, vp, cp, sz]
+    L.mfh_sb_apply.argtypes = [vp, vp, vp, vp]
+    L.mfh_sb_destroy.argtypes = [vp]
     for name in SYMBOLS:
         if name != "mfh_last_error":
             getattr(L, name).restype = ctypes.c_int
@@ -215,6 +220,45 @@ class Hamiltonian:
     def destroy(self):
         if self._h:
             lib().mfh_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+class SystemBath:
+    """H = H_S (x) I + I (x) H_B + g A (x) B_1 on X[d_B][d_S] (mfh_sb_create ... mfh_sb_destroy)."""
+
+    def __init__(self, d_B: int, d_S: int, B: int, seed_HB: int, seed_B1: int, H_S, A, g: float, dtype: str = "c64"):
+        import numpy as np
+        self.d_B, self.d_S, self.dtype = d_B, d_S, dtype
+        hs = np.ascontiguousarray(H_S, dtype=np.complex128)
+        a = np.ascontiguousarray(A, dtype=np.complex128)
+        assert hs.shape == (d_S, d_S) and a.shape == (d_S, d_S)
+        self._h = ctypes.c_void_p()
+        _check(lib().mfh_sb_create(ctypes.byref(self._h), d_B, d_S, B, seed_HB, seed_B1, DTYPES[dtype],
+                                   hs.ctypes.data, a.ctypes.data, float(g)))
+
+    def plan(self, mode: str = "auto", n_applies_hint: int = 1, hbm_budget_bytes: int = 0) -> dict:
+        buf = ctypes.create_string_buffer(1 << 14)
+        _check(lib().mfh_sb_plan(self._h, MODES[mode], n_applies_hint, int(hbm_budget_bytes), _stream(), buf, len(buf)))
+        return json.loads(buf.value.decode())
+
+    def apply(self, X, Y=None):
+        import torch
+        want = torch.complex128 if self.dtype == "c128" else torch.complex64
+        assert X.is_cuda and X.is_contiguous() and X.dtype == want and X.numel() == self.d_B * self.d_S
+        if Y is None:
+            Y = torch.empty_like(X)
+        _check(lib().mfh_sb_apply(self._h, X.data_ptr(), Y.data_ptr(), _stream()))
+        return Y
+
+    def destroy(self):
+        if self._h:
+            lib().mfh_sb_destroy(self._h)
             self._h = ctypes.c_void_p()
 
     def __del__(self):
