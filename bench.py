@@ -302,7 +302,7 @@ def roofline_for(res: dict, hbm_gbs: float, peak_src: str) -> dict:
         gbs = nbytes / (kern["procedural"] * 1e-3) / 1e9
         gen = D * D * (1.0 - res["plan"]["cached_fraction"]) / (kern["procedural"] * 1e-3)
         return {"kernel": "partial_overlap_kernel", "bound": "hbm", "achieved": gbs, "peak": hbm_gbs, "unit": "GB/s",
-                "frac": gbs / hbm_gbs, "traffic": None, "peak_source": peak_src,
+                "frac": gbs / hbm_gbs, "traffic": NCU_TRAFFIC.get(("partial_overlap_kernel", D)), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": nbytes, "kernel_ms": kern["procedural"],
                 "generated_entries_per_s_in_the_same_kernel": gen,
                 "share_of_step": kern["procedural"] / max(kern["total"], 1e-9)}
@@ -345,7 +345,8 @@ def roofline_for(res: dict, hbm_gbs: float, peak_src: str) -> dict:
 # pair = 44 per entry, the c64 tensor-core loop 62 per entry.
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full captures
 # (profiles/r01_*_ncu_full*.md), keyed by (kernel, D).
-NCU_TRAFFIC = {("cached_kernel", 65536): 68.730302e9 + 4.515584e6,
+NCU_TRAFFIC = {("cached_kernel", 65536): 68.724718e9 + 4.461824e6,
+               ("partial_overlap_kernel", 131072): 146.039268e9 + 247.162624e6,
                ("cached_pairs_kernel", 65536): 35.438780e9 + 249.902592e6,
                ("cached_multi_tc_kernel", 32768): 8.596603e9 + 134.462720e6}
 ISSUE_LANES_PER_S = 148 * 4 * 32 * 1.965e9
