@@ -145,6 +145,38 @@ MFH_API int mfh_lanczos_bounds(mfh_handle h, const void* psi_dev, int32_t m, dou
 MFH_API int mfh_chebyshev_steps(mfh_handle h, const void* psi_dev, void* out_dev, double tau, int32_t n_steps,
                                 double e_min, double e_max, double tol, int32_t* n_terms_out, void* stream);
 
+/* Distributed execution over `world` GPUs, one process and one handle per GPU (P:185-191 block-row
+ * accumulation; P:461-469 row-parallel strategy; P:597-618 row distribution; R20, 6.10).  Call
+ * before mfh_plan (drops a committed plan).  Every rank receives the FULL psi; after mfh_apply the ranks run
+ * one exchange step of D * B_c bytes (linear in D), done by the caller (NCCL through torch.distributed
+ * in paper_2606_31598_b200/distributed.py):
+ *   MFH_PART_ROWS   the paper's scheme: rank r owns the block rows n_blk*r/world <= n < n_blk*(r+1)/world,
+ *                   caches / generates only those and writes ONLY the rows of phi it owns (the other rows of
+ *                   phi_dev are left untouched); exchange = all-gather of the segments.  No Hermitian reuse
+ *                   across ranks: blocks whose mirror lies on another rank are generated one-sided.
+ *   MFH_PART_PAIRS  the unordered block pairs {n,m} are dealt round-robin to the ranks (order: circular
+ *                   distance d = 0..n_blk/2, then n); a rank owns both positions of its pairs, so every
+ *                   Hermitian pair is generated or stored once in the whole job; mfh_apply writes a
+ *                   full-length partial phi (the H0 term on the rank that owns block (n,n));
+ *                   exchange = all-reduce (sum).
+ *   MFH_PART_NONE   single GPU (world must be 1).
+ * mfh_chebyshev / mfh_chebyshev_steps / mfh_lanczos_bounds chain applies, so on a partitioned handle they
+ * call the exchange hook registered with mfh_set_exchange after every apply (MFH_ERR_BAD_STATE if none).
+ * Errors: INVALID_ARG (rank outside [0, world), world < 1, unknown scheme, world > 1 with MFH_PART_NONE). */
+enum { MFH_PART_NONE = 0, MFH_PART_ROWS = 1, MFH_PART_PAIRS = 2 };
+MFH_API int mfh_set_partition(mfh_handle h, int32_t rank, int32_t world, int32_t scheme);
+
+/* Exchange hook of a partitioned handle: called on the host by the chained drivers right after an apply
+ * has been enqueued, with the device vector the apply wrote (bytes = D * k * B_c) and the stream; it must
+ * enqueue the all-gather (MFH_PART_ROWS) or all-reduce (MFH_PART_PAIRS) of that vector in stream order and
+ * return 0.  The library itself contains no communication code.  fn = NULL removes the hook. */
+typedef int (*mfh_exchange_fn)(void* user, void* phi_dev, size_t bytes, void* stream);
+MFH_API int mfh_set_exchange(mfh_handle h, mfh_exchange_fn fn, void* user);
+
+/* First block row and number of block rows that mfh_apply writes on this handle (after mfh_plan):
+ * the owned slab for MFH_PART_ROWS, [0, n_blk) otherwise.  B_out receives the planned block size. */
+MFH_API int mfh_get_partition_rows(mfh_handle h, int32_t* first_block_row, int32_t* n_block_rows, int32_t* B_out);
+
 /* Free the handle and everything it owns.  NULL is accepted. */
 MFH_API int mfh_destroy(mfh_handle h);
 

@@ -20,6 +20,8 @@ MFH_C128, MFH_C64 = 0, 1
 MFH_SRC_GUE, MFH_SRC_DIAG_PLUS_GUE = 0, 1
 MFH_MODE_AUTO, MFH_MODE_PROCEDURAL, MFH_MODE_PARTIAL, MFH_MODE_FULL, MFH_MODE_PAIRS = 0, 1, 2, 3, 4
 MFH_MAX_K = 16
+MFH_PART_NONE, MFH_PART_ROWS, MFH_PART_PAIRS = 0, 1, 2
+PARTITIONS = {"none": MFH_PART_NONE, "rows": MFH_PART_ROWS, "pairs": MFH_PART_PAIRS}
 
 DTYPES = {"c128": MFH_C128, "c64": MFH_C64}
 MODES = {"auto": MFH_MODE_AUTO, "procedural": MFH_MODE_PROCEDURAL, "partial": MFH_MODE_PARTIAL,
@@ -29,7 +31,7 @@ MODES = {"auto": MFH_MODE_AUTO, "procedural": MFH_MODE_PROCEDURAL, "partial": MF
 SYMBOLS = ["mfh_create", "mfh_plan_analytic", "mfh_plan", "mfh_apply", "mfh_apply_host", "mfh_apply_timed",
            "mfh_chebyshev", "mfh_chebyshev_steps", "mfh_lanczos_bounds", "mfh_destroy", "mfh_last_error", "mfh_get_plan", "mfh_debug_philox",
            "mfh_materialize_block", "mfh_debug_h0", "mfh_debug_pipe_rates", "mfh_sb_create", "mfh_sb_plan", "mfh_sb_apply",
-           "mfh_sb_destroy"]
+           "mfh_sb_destroy", "mfh_set_partition", "mfh_get_partition_rows", "mfh_set_exchange"]
 
 _lib = None
 
@@ -62,6 +64,9 @@ def lib():
     L.mfh_chebyshev_steps.argtypes = [vp, vp, vp, dbl, i32, dbl, dbl, dbl, ctypes.POINTER(i32), vp]
     L.mfh_lanczos_bounds.argtypes = [vp, vp, i32, dbl, ctypes.POINTER(dbl), ctypes.POINTER(dbl), ctypes.POINTER(dbl),
                                      ctypes.POINTER(dbl), vp]
+    L.mfh_set_partition.argtypes = [vp, i32, i32, i32]
+    L.mfh_set_exchange.argtypes = [vp, vp, vp]
+    L.mfh_get_partition_rows.argtypes = [vp, ctypes.POINTER(i32), ctypes.POINTER(i32), ctypes.POINTER(i32)]
     L.mfh_destroy.argtypes = [vp]
     L.mfh_last_error.argtypes = []
     L.mfh_last_error.restype = cp
@@ -137,6 +142,16 @@ class Hamiltonian:
                               1 if measure else 0, _stream(), buf, len(buf)))
         self.k = k
         return json.loads(buf.value.decode())
+
+    def set_partition(self, rank: int, world: int, scheme: str = "pairs"):
+        """Distributed execution: this handle computes rank `rank`'s share of phi (call before plan)."""
+        _check(lib().mfh_set_partition(self._h, rank, world, PARTITIONS[scheme]))
+
+    def partition_rows(self):
+        """(first row, number of rows) of phi that apply() writes on this handle."""
+        a, b, c = ctypes.c_int32(0), ctypes.c_int32(0), ctypes.c_int32(0)
+        _check(lib().mfh_get_partition_rows(self._h, ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)))
+        return a.value * c.value, b.value * c.value
 
     def get_plan(self) -> dict:
         buf = ctypes.create_string_buffer(4096)

@@ -100,6 +100,8 @@ static int commit_plan(mfh_handle h, const Plan& p, cudaStream_t st)
             int32_t* L = lists.data() + (size_t)b * (ns + 1);
             for (int sl = 0; sl < q.n_slots; ++sl)
                 if (q.slot_valid[(size_t)b * q.n_slots + sl]) L[1 + L[0]++] = sl;
+            if (b < q.row_first || b >= q.row_first + q.row_count) L[0] |= SLOT_SKIP_ROW;
+            if (!q.own[(size_t)b * q.n_blk + b]) L[0] |= SLOT_NO_H0;
         }
         MFH_CUDA_CHECK(cudaMalloc(&h->d_slot_list, lists.size() * sizeof(int32_t)));
         MFH_CUDA_CHECK(cudaMemcpy(h->d_slot_list, lists.data(), lists.size() * sizeof(int32_t),
@@ -112,6 +114,7 @@ static int commit_plan(mfh_handle h, const Plan& p, cudaStream_t st)
     }
     MFH_CUDA_CHECK(cudaMalloc(&h->d_counter, 2 * sizeof(int32_t)));
     MFH_CUDA_CHECK(cudaMalloc(&h->d_io, (size_t)2 * h->D * q.k * cb));
+    MFH_CUDA_CHECK(cudaMemsetAsync(h->d_io, 0, (size_t)2 * h->D * q.k * cb, st));   // MFH_PART_ROWS leaves foreign rows untouched
     if (h->kind == MFH_SRC_DIAG_PLUS_GUE) {
         MFH_CUDA_CHECK(cudaMalloc(&h->d_h0, (size_t)h->D * (h->dtype == MFH_C128 ? 8 : 4)));
         int rc = launch_h0(h, h->d_h0, st);
@@ -140,13 +143,30 @@ static int apply_impl(mfh_handle h, const void* psi, void* phi, const double* la
         if ((rc = launch_partial_overlap(h, psi, st))) return rc;
     } else if (p.k == 1) {
         if ((rc = launch_proc_single(h, psi, st))) return rc;
-    } else if (p.slot_multi >= 0 && p.covered_blocks < (int64_t)p.n_blk * p.n_blk) {
+    } else if (p.slot_multi >= 0 && p.covered_blocks < p.owned_blocks) {
         if ((rc = launch_proc_multi(h, psi, st))) return rc;
     }
     if (ev) cudaEventRecord(ev[2], st);
     rc = launch_reduce(h, psi, phi, lambdas, st);
     if (ev) cudaEventRecord(ev[3], st);
     return rc;
+}
+
+// An apply inside a chain (Chebyshev, Lanczos): on a partitioned handle the result must be complete on
+// every rank before the next O(D) update, so the registered exchange hook runs right after the apply.
+static int apply_chained(mfh_handle h, const void* psi, void* phi, cudaStream_t st)
+{
+    int rc = apply_impl(h, psi, phi, nullptr, st);
+    if (rc || (h->part_world <= 1 && !h->exchange)) return rc;   // a registered hook also runs at world 1 (tests)
+    if (!h->exchange) {
+        set_error("partitioned handle (world %d): register an exchange hook with mfh_set_exchange", h->part_world);
+        return MFH_ERR_BAD_STATE;
+    }
+    if (h->exchange(h->exchange_user, phi, (size_t)h->D * h->plan.k * complex_bytes(h->dtype), (void*)st)) {
+        set_error("exchange hook failed");
+        return MFH_ERR_CUDA;
+    }
+    return MFH_OK;
 }
 
 // Algorithm 2: time R_bench applies of a committed plan after R_warm warm-ups.
@@ -229,6 +249,39 @@ MFH_API int mfh_destroy(mfh_handle h)
     return MFH_OK;
 }
 
+MFH_API int mfh_set_partition(mfh_handle h, int32_t rank, int32_t world, int32_t scheme)
+{
+    if (!h) { set_error("mfh_set_partition: NULL handle"); return MFH_ERR_INVALID_ARG; }
+    if (world < 1 || rank < 0 || rank >= world || scheme < MFH_PART_NONE || scheme > MFH_PART_PAIRS ||
+        (scheme == MFH_PART_NONE && world != 1)) {
+        set_error("mfh_set_partition: invalid rank %d / world %d / scheme %d", rank, world, scheme);
+        return MFH_ERR_INVALID_ARG;
+    }
+    free_plan_resources(h);   // a committed plan belongs to the previous partition
+    h->part_rank = rank;
+    h->part_world = world;
+    h->part_scheme = world == 1 ? (int32_t)MFH_PART_NONE : scheme;
+    return MFH_OK;
+}
+
+MFH_API int mfh_set_exchange(mfh_handle h, mfh_exchange_fn fn, void* user)
+{
+    if (!h) { set_error("mfh_set_exchange: NULL handle"); return MFH_ERR_INVALID_ARG; }
+    h->exchange = fn;
+    h->exchange_user = user;
+    return MFH_OK;
+}
+
+MFH_API int mfh_get_partition_rows(mfh_handle h, int32_t* first_block_row, int32_t* n_block_rows, int32_t* B_out)
+{
+    if (!h || !first_block_row || !n_block_rows) { set_error("mfh_get_partition_rows: NULL pointer"); return MFH_ERR_INVALID_ARG; }
+    if (!h->planned) { set_error("mfh_get_partition_rows: call mfh_plan first"); return MFH_ERR_BAD_STATE; }
+    *first_block_row = h->plan.row_first;
+    *n_block_rows = h->plan.row_count;
+    if (B_out) *B_out = h->plan.B;
+    return MFH_OK;
+}
+
 MFH_API int mfh_plan_analytic(int64_t D, int32_t dtype, int32_t k, int32_t mode, int32_t B,
                               int64_t n_applies_hint, int64_t hbm_free_bytes, char* json_out,
                               size_t json_cap)
@@ -266,7 +319,11 @@ MFH_API int mfh_plan(mfh_handle h, int32_t mode, int32_t k, int64_t n_applies_hi
     budget = std::min(budget, 0.98 * (double)free_b);
 
     std::vector<Candidate> cands;
-    int rc = enumerate_candidates(h->D, h->dtype, k, mode, h->B_req, n_applies_hint, budget, h->sm_count, cands);
+    Partition part;
+    part.rank = h->part_rank;
+    part.world = h->part_world;
+    part.scheme = h->part_scheme;
+    int rc = enumerate_candidates(h->D, h->dtype, k, mode, h->B_req, n_applies_hint, budget, h->sm_count, cands, part);
     if (rc) {
         copy_json(plan_json(h->D, h->dtype, k, n_applies_hint, budget, 0, cands), json_out, json_cap);
         set_error("mfh_plan: no candidate plan fits in %.0f bytes", budget);
@@ -278,6 +335,9 @@ MFH_API int mfh_plan(mfh_handle h, int32_t mode, int32_t k, int64_t n_applies_hi
         p.k = k;
         p.cached_per_row = c.cached_per_row;
         p.pairs = c.pairs;
+        p.part_rank = part.rank;
+        p.part_world = part.world;
+        p.part_scheme = part.scheme;
         build_tables(p, h->D, h->dtype, h->sm_count);
         return p;
     };
@@ -317,17 +377,20 @@ MFH_API int mfh_get_plan(mfh_handle h, char* json_out, size_t json_cap)
 {
     if (!h || !h->planned) { set_error("mfh_get_plan: handle not planned"); return MFH_ERR_BAD_STATE; }
     const Plan& p = h->plan;
-    char buf[768];
+    char buf[1024];
     snprintf(buf, sizeof buf,
-             "{\"mode\":\"%s\",\"B\":%d,\"n_blk\":%d,\"k\":%d,\"cached_blocks\":%lld,\"cached_per_row\":%d,"
+             "{\"partition\":{\"scheme\":\"%s\",\"rank\":%d,\"world\":%d,\"owned_blocks\":%lld,\"first_block_row\":%d,\"block_rows\":%d},"
+             "\"mode\":\"%s\",\"B\":%d,\"n_blk\":%d,\"k\":%d,\"cached_blocks\":%lld,\"cached_per_row\":%d,"
              "\"cached_fraction\":%.6g,\"cache_bytes\":%zu,\"work_bytes\":%zu,\"partial_slots\":%d,\"proc_items\":%zu,\"pair_items\":%zu,"
              "\"proc_rows_per_lane\":%d,\"proc_row_strips\":%d,\"launches_per_apply\":%d}",
+             p.part_scheme == MFH_PART_ROWS ? "rows" : (p.part_scheme == MFH_PART_PAIRS ? "pairs" : "none"), p.part_rank, p.part_world,
+             (long long)p.owned_blocks, p.row_first, p.row_count,
              p.mode == MFH_MODE_FULL ? "full" : (p.mode == MFH_MODE_PARTIAL ? "partial" : (p.mode == MFH_MODE_PAIRS ? "pairs" : "procedural")), p.B,
              p.n_blk, p.k, (long long)p.n_cached, p.cached_per_row,
-             (double)p.covered_blocks / ((double)p.n_blk * p.n_blk), p.cache_bytes, p.work_bytes, p.n_slots,
+             (double)p.covered_blocks / (double)std::max<int64_t>(p.owned_blocks, 1), p.cache_bytes, p.work_bytes, p.n_slots,
              p.items.size(), p.pair_items.size(), p.R, p.Q,
              1 + (p.n_cached > 0) + ((p.k == 1 && !p.items.empty()) ||
-                                      (p.k > 1 && p.covered_blocks < (int64_t)p.n_blk * p.n_blk)));
+                                      (p.k > 1 && p.covered_blocks < p.owned_blocks)));
     copy_json(buf, json_out, json_cap);
     return MFH_OK;
 }
@@ -423,7 +486,7 @@ MFH_API int mfh_chebyshev(mfh_handle h, const void* psi_dev, void* out_dev, doub
     int rc;
     if ((rc = launch_cheb_first(h, psi_dev, cur, acc, J[0], st))) return rc;      // Eq. 41
     for (int l = 1; l < K; ++l) {
-        if ((rc = apply_impl(h, cur, hq, nullptr, st))) return rc;
+        if ((rc = apply_chained(h, cur, hq, st))) return rc;
         double cr = 0.0, ci = 0.0;                                                  // 2 (-i)^l J_l
         switch (l & 3) {
         case 0: cr = 2.0 * J[l]; break;
@@ -496,7 +559,7 @@ MFH_API int mfh_lanczos_bounds(mfh_handle h, const void* psi_dev, int32_t m, dou
     if ((rc = launch_lz_dot(h, psi_dev, psi_dev, d_partial, d_norm0, 1, st))) return rc;
     if ((rc = launch_lz_scale(h, psi_dev, v, d_norm0, st))) return rc;
     for (int j = 0; j < m; ++j) {
-        if ((rc = apply_impl(h, v, w, nullptr, st))) return rc;                                   // w = H v_j
+        if ((rc = apply_chained(h, v, w, st))) return rc;                                         // w = H v_j
         if ((rc = launch_lz_dot(h, v, w, d_partial, d_alpha + j, 0, st))) return rc;              // alpha_j = Re <v_j, w>
         if ((rc = launch_lz_update(h, w, v, v_prev, d_alpha + j, j ? d_beta + j - 1 : nullptr,    // w -= alpha v + beta v_prev
                                    d_partial, d_beta + j, st))) return rc;                        // beta_j = ||w||

@@ -55,7 +55,11 @@ struct Plan {
     int32_t n_slots = 0;       // partial vectors in the workspace
     int32_t slot_cache = -1, slot_row0 = -1, slot_col0 = -1, slot_multi = -1;
     size_t cache_bytes = 0, work_bytes = 0;
-    std::vector<int32_t> cache_slot;   // [n_blk*n_blk] index of the cached block or -1
+    int32_t part_rank = 0, part_world = 1, part_scheme = 0;   // mfh_set_partition
+    int64_t owned_blocks = 0;     // block positions this rank is responsible for (n_blk^2 on one GPU)
+    int32_t row_first = 0, row_count = 0;   // block rows of phi this rank writes
+    std::vector<uint8_t> own;          // [n_blk*n_blk] 1 = position owned by this rank
+    std::vector<int32_t> cache_slot;   // [n_blk*n_blk] cached block index, -1 generated, -2 served by the mirrored pair, -3 not owned
     std::vector<uint8_t> pair_kind;    // [n_blk*n_blk]
     std::vector<ProcItem> items;       // fused generate-and-apply kernel
     std::vector<ProcItem> pair_items;  // cached pair kernel (pairs mode)
@@ -71,6 +75,9 @@ struct mfh_handle_s {
     uint64_t seed = 0, seed_h0 = 0;
     int32_t kind = 0, dtype = 0;
     double lambda = 1.0;
+    int32_t part_rank = 0, part_world = 1, part_scheme = 0;   // mfh_set_partition
+    mfh_exchange_fn exchange = nullptr;                       // mfh_set_exchange
+    void* exchange_user = nullptr;
     bool planned = false;
     mfh::Plan plan;
     // device resources (library-owned)
@@ -80,7 +87,7 @@ struct mfh_handle_s {
     int32_t* d_cache_slot = nullptr;
     mfh::ProcItem* d_items = nullptr;
     mfh::ProcItem* d_pair_items = nullptr;
-    int32_t* d_slot_list = nullptr;   // [n_blk][n_slots+1]: count, then the valid slots in ascending order
+    int32_t* d_slot_list = nullptr;   // [n_blk][n_slots+1]: count | flags, then the valid slots in ascending order
     double* d_lambdas = nullptr;    // MFH_MAX_K doubles, refreshed by every apply
     int32_t* d_counter = nullptr;   // dynamic work counters: [0] procedural kernel, [1] pair kernel
     void* d_cheb = nullptr;         // 3 vectors of Chebyshev scratch
@@ -93,6 +100,11 @@ struct mfh_handle_s {
 };
 
 namespace mfh {
+
+// flags in the count word of a block row's slot list (reduce kernel)
+constexpr int32_t SLOT_SKIP_ROW = 1 << 30;   // MFH_PART_ROWS: block row not owned, phi left untouched
+constexpr int32_t SLOT_NO_H0 = 1 << 29;      // MFH_PART_PAIRS: diagonal block on another rank, no h0 (.) psi term
+constexpr int32_t SLOT_COUNT_MASK = (1 << 29) - 1;
 
 void set_error(const char* fmt, ...);
 size_t complex_bytes(int dtype);

@@ -112,31 +112,75 @@ void make_gen_table(int64_t D, GenHostD& out)
 // Offsets covered by a Hermitian pair cache with c band offsets: circular block distance < c.
 int pair_full_offsets(int N) { return N / 2 + 1; }
 
+// Ownership of the block positions under mfh_set_partition (R20).
+void partition_mask(int N, const Partition& part, std::vector<uint8_t>& own)
+{
+    own.assign((size_t)N * N, part.world <= 1 ? 1 : 0);
+    if (part.world <= 1) return;
+    if (part.scheme == MFH_PART_ROWS) {
+        // contiguous slabs of block rows (the paper's row sets R_j)
+        const int lo = (int)((int64_t)N * part.rank / part.world), hi = (int)((int64_t)N * (part.rank + 1) / part.world);
+        for (int n = lo; n < hi; ++n)
+            for (int m = 0; m < N; ++m) own[(size_t)n * N + m] = 1;
+        return;
+    }
+    // unordered pairs {n, n+d} dealt round-robin, nearest block diagonals first: each rank gets the same
+    // mix of distances (so of cached and generated pairs) and a pair's two positions stay together
+    int64_t idx = 0;
+    for (int d = 0; d <= N / 2; ++d)
+        for (int n = 0; n < N; ++n) {
+            if (2 * d == N && n >= N / 2) continue;
+            const int m = (n + d) % N;
+            if (idx++ % part.world == part.rank) own[(size_t)n * N + m] = own[(size_t)m * N + n] = 1;
+        }
+}
+
 void build_tables(Plan& p, int64_t D, int dtype, int sm_count)
 {
     const int N = p.n_blk = (int)(D / p.B);
     const int c = p.cached_per_row;
+    Partition part;
+    part.rank = p.part_rank;
+    part.world = p.part_world;
+    part.scheme = p.part_scheme;
+    partition_mask(N, part, p.own);
+    auto own = [&](int n, int m) { return p.own[(size_t)n * N + m] != 0; };
+    p.owned_blocks = 0;
+    for (uint8_t o : p.own) p.owned_blocks += o;
+    p.row_first = 0;
+    p.row_count = N;
+    if (part.world > 1 && part.scheme == MFH_PART_ROWS) {
+        p.row_first = (int)((int64_t)N * part.rank / part.world);
+        p.row_count = (int)((int64_t)N * (part.rank + 1) / part.world) - p.row_first;
+    }
     p.cache_slot.assign((size_t)N * N, -1);
+    for (int n = 0; n < N; ++n)
+        for (int m = 0; m < N; ++m)
+            if (!own(n, m)) p.cache_slot[(size_t)n * N + m] = -3;
     p.pair_items.clear();
     int n_stored = 0;
     if (!p.pairs) {
-        // full blocks, row-balanced symmetric band (R5)
+        // full blocks, row-balanced symmetric band (R5), owned positions only
         const std::vector<int> offs = band_offsets(N);
         for (int n = 0; n < N; ++n)
-            for (int t = 0; t < c; ++t) p.cache_slot[(size_t)n * N + (n + offs[t]) % N] = n * c + t;
-        n_stored = c * N;
+            for (int t = 0; t < c; ++t) {
+                const int m = (n + offs[t]) % N;
+                if (own(n, m)) p.cache_slot[(size_t)n * N + m] = n_stored++;
+            }
     } else {
         // canonical pairs: every unordered block pair {n,m} with circular
         // distance d < c is stored once as block (min,max); the mirrored position is marked -2.
+        // A pair split between two ranks (MFH_PART_ROWS) is not stored: both halves are generated.
         for (int d = 0; d < c && d <= N / 2; ++d)
             for (int n = 0; n < N; ++n) {
                 const int m = (n + d) % N;
                 if (d == 0) {
-                    p.cache_slot[(size_t)n * N + n] = n_stored++;
+                    if (own(n, n)) p.cache_slot[(size_t)n * N + n] = n_stored++;
                     continue;
                 }
                 if (2 * d == N && n >= N / 2) continue;   // {n, n+N/2} was stored from the other side
                 const int lo = std::min(n, m), hi = std::max(n, m);
+                if (!own(lo, hi) || !own(hi, lo)) continue;
                 p.cache_slot[(size_t)lo * N + hi] = n_stored++;
                 p.cache_slot[(size_t)hi * N + lo] = -2;
             }
@@ -144,7 +188,7 @@ void build_tables(Plan& p, int64_t D, int dtype, int sm_count)
     p.n_cached = n_stored;
     auto uncached = [&](int n, int m) { return p.cache_slot[(size_t)n * N + m] == -1; };
     int64_t covered = 0;
-    for (int32_t v : p.cache_slot) covered += (v != -1);
+    for (int32_t v : p.cache_slot) covered += (v >= 0 || v == -2);
     p.covered_blocks = covered;
 
     p.pair_kind.assign((size_t)N * N, PAIR_NONE);
@@ -169,7 +213,7 @@ void build_tables(Plan& p, int64_t D, int dtype, int sm_count)
     // (row block, strip)] [k-vector kernel, one per column block]
     int s = 0;
     p.slot_cache = p.slot_row0 = p.slot_col0 = p.slot_multi = -1;
-    if (!p.pairs && c > 0 && p.k == 1) p.slot_cache = s++;
+    if (!p.pairs && n_stored > 0 && p.k == 1) p.slot_cache = s++;
     if (p.k == 1 && n_pairs + n_pair_blocks > 0) {
         p.slot_row0 = s;
         s += N;
@@ -186,7 +230,7 @@ void build_tables(Plan& p, int64_t D, int dtype, int sm_count)
     for (int b = 0; b < N; ++b) {
         if (p.slot_cache >= 0) valid(b, p.slot_cache) = 1;
         if (p.slot_multi >= 0)
-            for (int m = 0; m < N; ++m) valid(b, p.slot_multi + m) = 1;
+            for (int m = 0; m < N; ++m) valid(b, p.slot_multi + m) = own(b, m);   // nobody writes a block that is not ours
     }
     const int strip = p.B / p.Q;
     auto push_items = [&](std::vector<ProcItem>& dst, int n, int m, uint8_t kd) {
@@ -224,7 +268,7 @@ void build_tables(Plan& p, int64_t D, int dtype, int sm_count)
     p.work_bytes = (size_t)std::max(p.n_slots, 1) * D * p.k * cb;
     if (covered == 0) p.mode = MFH_MODE_PROCEDURAL;
     else if (p.pairs) p.mode = MFH_MODE_PAIRS;
-    else p.mode = (c == N ? MFH_MODE_FULL : MFH_MODE_PARTIAL);
+    else p.mode = (covered == p.owned_blocks ? MFH_MODE_FULL : MFH_MODE_PARTIAL);
 }
 
 // Scratch outside the partial slots: Chebyshev (3 vectors), host-apply staging (2 k vectors), H0.
@@ -234,7 +278,7 @@ static size_t fixed_work_bytes(int64_t D, int dtype, int k)
 }
 
 Candidate evaluate_candidate(int64_t D, int dtype, int k, int B, int cached_per_row, bool pairs,
-                             int64_t n_applies, int sm_count)
+                             int64_t n_applies, int sm_count, const Partition& part)
 {
     Candidate c;
     Plan p;
@@ -242,6 +286,9 @@ Candidate evaluate_candidate(int64_t D, int dtype, int k, int B, int cached_per_
     p.k = k;
     p.cached_per_row = cached_per_row;
     p.pairs = pairs;
+    p.part_rank = part.rank;
+    p.part_world = part.world;
+    p.part_scheme = part.scheme;
     c.pairs = pairs;
     build_tables(p, D, dtype, sm_count);
     c.B = B;
@@ -252,8 +299,8 @@ Candidate evaluate_candidate(int64_t D, int dtype, int k, int B, int cached_per_
     c.cache_bytes = (double)p.cache_bytes;                                   // M_op, Eq. 15-17
     c.work_bytes = (double)p.work_bytes + (double)fixed_work_bytes(D, dtype, k);   // M_work, Eq. 14
     const double cb = (double)complex_bytes(dtype);
-    const double f = (double)p.covered_blocks / ((double)p.n_blk * p.n_blk);   // entries served from the cache
-    const double entries = (double)D * (double)D;
+    const double f = (double)p.covered_blocks / (double)std::max<int64_t>(p.owned_blocks, 1);   // entries served from the cache
+    const double entries = (double)p.owned_blocks * B * B;                     // entries this rank applies
     c.cached_fraction = f;
     c.t_cached = c.cache_bytes / kBwRead;
     if (k == 1) {
@@ -273,13 +320,13 @@ Candidate evaluate_candidate(int64_t D, int dtype, int k, int B, int cached_per_
     } else {
         c.t_proc = (1.0 - f) * entries / gen_entries_per_s(dtype, k);
     }
-    int launches = 1 + (p.n_cached > 0) + (p.covered_blocks < (int64_t)p.n_blk * p.n_blk);
+    int launches = 1 + (p.n_cached > 0) + (p.covered_blocks < p.owned_blocks);
     c.t_reduce = (double)p.n_slots * 0.6 * D * k * cb / kBwRead;
     c.t_apply = c.t_cached + c.t_proc + c.t_reduce + launches * kLaunch;   // Eq. 32 (not overlapped)
     const double stored = c.cache_bytes / cb;
     c.t_fill = stored / gen_entries_per_s(dtype, 0) + c.cache_bytes / kBwWrite;
     c.t_job = (double)std::max<int64_t>(n_applies, 1) * c.t_apply + c.t_fill;
-    c.flops = 8.0 * entries * k;                                            // F_mv, Eq. 13
+    c.flops = 8.0 * entries * k;                                            // F_mv, Eq. 13 (this rank's share)
     return c;
 }
 
@@ -296,7 +343,7 @@ static void candidate_json(std::string& s, const Candidate& c)
 }
 
 int enumerate_candidates(int64_t D, int dtype, int k, int mode, int B_req, int64_t n_applies,
-                         double budget_bytes, int sm_count, std::vector<Candidate>& out)
+                         double budget_bytes, int sm_count, std::vector<Candidate>& out, const Partition& part)
 {
     out.clear();
     std::vector<int> Bs;
@@ -309,7 +356,7 @@ int enumerate_candidates(int64_t D, int dtype, int k, int mode, int B_req, int64
         const int N = (int)(D / B);
         // cache budget -> cached blocks per row (Eq. 27 with full blocks; rows kept balanced)
         auto fits = [&](int c, bool pairs) {
-            Candidate t = evaluate_candidate(D, dtype, k, B, c, pairs, n_applies, sm_count);
+            Candidate t = evaluate_candidate(D, dtype, k, B, c, pairs, n_applies, sm_count, part);
             return t.cache_bytes + t.work_bytes <= budget_bytes;
         };
         std::vector<std::pair<int, bool>> cs;   // (cached_per_row or band offsets, pairs)
@@ -325,13 +372,13 @@ int enumerate_candidates(int64_t D, int dtype, int k, int mode, int B_req, int64
         }
         if (mode == MFH_MODE_AUTO || mode == MFH_MODE_PARTIAL) {
             double room = budget_bytes - (double)fixed_work_bytes(D, dtype, k) - 3.0 * D * k * cb;
-            int c = (int)std::floor(room / ((double)B * B * cb * N));
+            int c = (int)std::floor(room * std::max(part.world, 1) / ((double)B * B * cb * N));   // a rank stores ~c N / world blocks
             c = std::min(c, N - 1);
             while (c > 0 && !fits(c, false)) --c;
             if (c > 0) cs.push_back({c, false});
         }
         for (auto [c, pairs] : cs) {
-            Candidate cand = evaluate_candidate(D, dtype, k, B, c, pairs, n_applies, sm_count);
+            Candidate cand = evaluate_candidate(D, dtype, k, B, c, pairs, n_applies, sm_count, part);
             cand.feasible = (cand.cache_bytes + cand.work_bytes <= budget_bytes);   // Eq. 18
             // cached k-vector blocks: tensor-core kernel, complex64 with B % 128 == 0 only
             if (k > 1 && c > 0 && (pairs || !tc_cached_multi_supported(dtype, k, B))) cand.feasible = false;

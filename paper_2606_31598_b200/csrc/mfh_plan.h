@@ -8,6 +8,13 @@ namespace mfh {
 
 struct Plan;
 
+// Distributed execution (mfh_set_partition): which block positions this rank owns.
+struct Partition {
+    int rank = 0, world = 1, scheme = 0;   // MFH_PART_*
+};
+// own[n * n_blk + m] = 1 where block position (n,m) belongs to the rank (R20).
+void partition_mask(int n_blk, const Partition& part, std::vector<uint8_t>& own);
+
 // One candidate execution plan p and its model.
 struct Candidate {
     int B = 0, n_blk = 0, mode = 0, cached_per_row = 0;
@@ -24,10 +31,11 @@ struct Candidate {
 void choose_tiling(int B, int n_blk, int n_pairs, int sm_count, int& R, int& Q);
 void build_tables(Plan& p, int64_t D, int dtype, int sm_count);
 Candidate evaluate_candidate(int64_t D, int dtype, int k, int B, int cached_per_row, bool pairs,
-                             int64_t n_applies, int sm_count);
+                             int64_t n_applies, int sm_count, const Partition& part = Partition());
 int pair_full_offsets(int n_blk);
 int enumerate_candidates(int64_t D, int dtype, int k, int mode, int B_req, int64_t n_applies,
-                         double budget_bytes, int sm_count, std::vector<Candidate>& out);
+                         double budget_bytes, int sm_count, std::vector<Candidate>& out,
+                         const Partition& part = Partition());
 std::string plan_json(int64_t D, int dtype, int k, int64_t n_applies, double budget, int measured,
                       const std::vector<Candidate>& cands);
 double planner_alpha();

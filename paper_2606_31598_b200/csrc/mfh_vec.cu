@@ -36,7 +36,8 @@ __global__ void __launch_bounds__(256) reduce_kernel(int64_t D, int32_t B, int32
         const bool live = e < total;
         const int64_t i = live ? e / k : 0;
         const int32_t* list = slot_list + (size_t)(i / B) * (n_slots + 1);   // [count, slots...]
-        const int cnt = list[0];
+        const int head = list[0];                                             // count | SLOT_* flags
+        const int cnt = head & SLOT_COUNT_MASK;
         const int chunk = (cnt + G - 1) / G;
         int t = g * chunk;
         const int t_end = live ? min(cnt, t + chunk) : 0;
@@ -67,10 +68,10 @@ __global__ void __launch_bounds__(256) reduce_kernel(int64_t D, int32_t B, int32
                     si += part[gg][ex][1];
                 }
         }
-        if (g == 0 && live) {
+        if (g == 0 && live && !(head & SLOT_SKIP_ROW)) {
             const int v = (int)(e - i * k);
             double outr = lam.v[v] * sr, outi = lam.v[v] * si;
-            if (h0) {
+            if (h0 && !(head & SLOT_NO_H0)) {
                 const CT p = psi[e];
                 const double d = (double)h0[i];
                 outr = fma(d, (double)p.x, outr);

@@ -1,0 +1,164 @@
+"""GPU parity of distributed execution (NEXT-4; mfh_set_partition).
+
+One GPU is enough: the ranks of a job never wait on one another inside an apply (every rank reads the full
+psi, the exchange follows), so rank r of W is run as its own handle, one after the other, and each
+contribution is compared element by element with the oracle's contribution of the same rank
+(oracle/partition.py states the ownership rule independently)."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2606_31598_b200 import binding as mfh
+from paper_2606_31598_b200.inputs import lambda_grid, make_psi
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"c128": 1e-11, "c64": 1e-4}
+SENTINEL = 7.25 - 3.5j
+
+
+def to_dev(x):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def rank_apply(D, B, seed, psi, dtype, mode, rank, world, scheme, k=1, budget=0, lambdas=None, **kw):
+    """Contribution of one rank: phi prefilled with a sentinel so that untouched rows show."""
+    import torch
+    h = mfh.Hamiltonian(D, B, seed, dtype, **kw)
+    h.set_partition(rank, world, scheme)
+    h.plan(mode, k=k, hbm_budget_bytes=budget)
+    plan = h.get_plan()
+    x = to_dev(psi)
+    phi = torch.full_like(x, SENTINEL)
+    h.apply(x, phi, lambdas)
+    out = phi.cpu().numpy().astype(np.complex128)
+    lo, cnt = h.partition_rows()
+    h.destroy()
+    return out, plan, (lo, cnt)
+
+
+def scaled_err(a, b, scale):
+    return float(np.linalg.norm(a - b) / scale)
+
+
+@pytest.mark.parametrize("scheme", ["rows", "pairs"])
+@pytest.mark.parametrize("mode", ["procedural", "partial", "full", "pairs"])
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+@pytest.mark.parametrize("world", [2, 3])
+def test_each_rank_matches_the_oracle_contribution(scheme, mode, dtype, world):
+    D, B, seed = 2048, 256, 1234                                   # 8 x 8 blocks, ragged at world 3
+    psi = make_psi(D, 99, dtype=dtype)
+    full = oracle.apply(D, B, seed, psi)
+    scale = np.linalg.norm(full)
+    budget = int(0.45 * D * D * (16 if dtype == "c128" else 8) / world) if mode == "partial" else 0
+    total = np.zeros(D, dtype=np.complex128)
+    for r in range(world):
+        got, plan, (lo, cnt) = rank_apply(D, B, seed, psi, dtype, mode, r, world, scheme, budget=budget)
+        ref = oracle.apply_partition(D, B, seed, psi, r, world, scheme)
+        assert plan["partition"]["rank"] == r and plan["partition"]["world"] == world
+        assert plan["partition"]["owned_blocks"] == int(oracle.owned_blocks(D // B, r, world, scheme).sum())
+        if scheme == "rows":
+            assert (lo, cnt) == (B * (8 * r // world), B * (8 * (r + 1) // world) - B * (8 * r // world))
+            outside = np.ones(D, dtype=bool)
+            outside[lo:lo + cnt] = False
+            assert np.all(got[outside] == SENTINEL)                # foreign rows untouched
+            got = np.where(outside, 0.0, got)
+        else:
+            assert (lo, cnt) == (0, D)
+        assert scaled_err(got, ref, scale) <= TOL[dtype], (r, plan)
+        total += got
+    assert scaled_err(total, full, scale) <= TOL[dtype]
+
+
+@pytest.mark.parametrize("scheme", ["rows", "pairs"])
+def test_coupling_scan_k_vectors_partitioned(scheme):
+    """H0 + lambda_v V with k = 16 (complex64, tensor-core kernels): the H0 term appears exactly once."""
+    D, B, k, world = 2048, 256, 16, 2
+    Psi = make_psi(D, 9, k=k, dtype="c64")
+    lam = lambda_grid(k)
+    full = oracle.apply_scan(D, B, 8, 7, lam, Psi)
+    for mode in ("procedural", "full"):
+        total = np.zeros((D, k), dtype=np.complex128)
+        for r in range(world):
+            got, plan, (lo, cnt) = rank_apply(D, B, 8, Psi, "c64", mode, r, world, scheme, k=k, lambdas=lam,
+                                              kind="diag_plus_gue", seed_h0=7)
+            if scheme == "rows":
+                outside = np.ones(D, dtype=bool)
+                outside[lo:lo + cnt] = False
+                got[outside] = 0.0
+            total += got
+        for v in range(k):
+            err = np.linalg.norm(total[:, v] - full[:, v]) / np.linalg.norm(full[:, v])
+            assert err <= 1e-4, (mode, v, err)
+
+
+def test_world_8_pairs_procedural_c128_sum_and_balance():
+    """C1's operator over 8 ranks: contributions add up to the full apply; the generation work is even."""
+    D, B, seed, world = 4096, 256, 1234, 8                          # 16 x 16 blocks: 136 pairs, 17 per rank
+    psi = make_psi(D, 99)
+    full = oracle.apply(D, B, seed, psi)
+    total = np.zeros(D, dtype=np.complex128)
+    items = []
+    for r in range(world):
+        got, plan, _ = rank_apply(D, B, seed, psi, "c128", "procedural", r, world, "pairs")
+        total += got
+        items.append(plan["proc_items"])
+    assert np.linalg.norm(total - full) <= 1e-11 * np.linalg.norm(full)
+    assert max(items) - min(items) <= max(items) // 8 + 1
+
+
+def test_invalid_partition_arguments_and_replan():
+    h = mfh.Hamiltonian(1024, 128, 1, "c128")
+    for args in [(2, 2, "rows"), (-1, 2, "pairs"), (0, 0, "rows"), (0, 2, "none")]:
+        with pytest.raises(mfh.MfhError) as e:
+            h.set_partition(*args)
+        assert e.value.code == mfh.MFH_ERR_INVALID_ARG
+    h.plan("procedural")
+    h.set_partition(1, 2, "rows")                                   # drops the plan
+    with pytest.raises(mfh.MfhError) as e:
+        h.apply(to_dev(make_psi(1024, 1)))
+    assert e.value.code == mfh.MFH_ERR_BAD_STATE
+    h.plan("procedural")
+    assert h.partition_rows() == (512, 512)
+    h.destroy()
+
+
+def test_chained_drivers_call_the_exchange_hook():
+    """mfh_chebyshev / mfh_lanczos_bounds on a handle with a registered hook: one call per apply, on the
+    library-owned vector, and the result is unchanged by an identity exchange.  A partitioned handle
+    without a hook refuses to chain."""
+    import torch
+    from paper_2606_31598_b200.distributed import install_exchange_hook
+    D, B = 1024, 128
+    psi = to_dev(make_psi(D, 3))
+    h = mfh.Hamiltonian(D, B, 21, "c128")
+    h.plan("procedural")
+    ref, K = h.chebyshev(psi, 3.0, -2.1, 2.1, 1e-12)
+    seen = []
+
+    def probe(flat, scheme, rows, group):                            # identity exchange that records its input
+        seen.append((tuple(flat.shape), float(torch.linalg.vector_norm(flat))))
+        return flat
+
+    import paper_2606_31598_b200.distributed as dmod
+    orig = dmod.exchange
+    dmod.exchange = probe
+    try:
+        install_exchange_hook(h, "pairs", (0, D))
+        out, K2 = h.chebyshev(psi, 3.0, -2.1, 2.1, 1e-12)
+        torch.cuda.synchronize()
+    finally:
+        dmod.exchange = orig
+    assert K2 == K and h._exchange_state["calls"] == K - 1 and "error" not in h._exchange_state
+    assert all(s[0] == (D, 2) and s[1] > 0 for s in seen)
+    assert torch.equal(out, ref)
+    h.destroy()
+
+    h2 = mfh.Hamiltonian(D, B, 21, "c128")
+    h2.set_partition(0, 2, "pairs")
+    h2.plan("procedural")
+    with pytest.raises(mfh.MfhError) as e:
+        h2.chebyshev(psi, 1.0, -2.1, 2.1, 1e-10)
+    assert e.value.code == mfh.MFH_ERR_BAD_STATE
+    h2.destroy()
