@@ -290,6 +290,32 @@ def measure_system_bath(torch, mfh, steps: int, hbm_gbs: float) -> dict:
                       "ratio_paper_over_this": c["paper_seconds_per_apply"] / (ms * 1e-3)}}
 
 
+def measure_partition_projection(torch, mfh, name: str = "C4", worlds=(2, 8), steps: int = 3) -> dict:
+    """NEXT-4 on one GPU: the local apply time of rank 0 of a W-GPU job (mfh_set_partition), which is what
+    every rank of the job would spend between two exchanges of D * B_c bytes.  The exchange itself (NCCL over
+    NVSwitch) cannot be timed on this one-GPU box and is NOT included."""
+    cfg = ALL[name]
+    D = cfg["D"]
+    psi = torch.from_numpy(make_psi(D, cfg["psi_seed"], dtype=cfg["dtype"])).cuda()
+    phi = torch.zeros_like(psi)
+    flush_buf = torch.empty(256 * 2**20, dtype=torch.uint8, device="cuda")
+    out = {"workload": workload_config(name, cfg)["workload"], "exchange_bytes_per_apply": psi.numel() * psi.element_size(),
+           "note": "per-rank kernel time of rank 0, exchange not included (one-GPU box)", "ranks": {}}
+    for scheme in ("rows", "pairs"):
+        for W in worlds:
+            h = mfh.Hamiltonian(D, cfg["B"], cfg["seed"], cfg["dtype"])
+            h.set_partition(0, W, scheme)
+            h.plan(cfg["mode"], k=1, hbm_budget_bytes=int(cfg.get("hbm_budget", 0)))
+            for _ in range(2):
+                h.apply(psi, phi)
+            torch.cuda.synchronize()
+            ms = time_steps(torch, lambda: h.apply(psi, phi), steps, lambda: flush_buf.fill_(1)) / steps
+            out["ranks"][f"{scheme}/W={W}"] = {"ms_per_apply_rank0": ms, "owned_blocks": h.get_plan()["partition"]["owned_blocks"],
+                                               "projected_entries_per_s_job": D * D / (ms * 1e-3)}
+            h.destroy()
+    return out
+
+
 def roofline_for(res: dict, hbm_gbs: float, peak_src: str) -> dict:
     """Roofline of the dominant kernel of one apply."""
     cfg = res["cfg"]
@@ -366,6 +392,48 @@ def aggregate(dist, local_ms: float, local_units: float, device=None):
     return float(t.item()), float(u.item())
 
 
+def run_partitioned(torch, dist, args, rank: int, world: int, local: int):
+    """--partition rows|pairs with N > 1 (NEXT-4): one operator over the N GPUs, every step = local apply +
+    one NCCL exchange of D * B_c bytes; value = D^2 entries per step over the max-over-ranks time."""
+    from paper_2606_31598_b200.distributed import DistributedHamiltonian
+    cfg = ALL[args.workload]
+    D, k = cfg["D"], cfg["k"]
+    kind = "diag_plus_gue" if "seed_h0" in cfg else "gue"
+    dh = DistributedHamiltonian(D, cfg["B"], cfg["seed"], cfg["dtype"], kind=kind, seed_h0=cfg.get("seed_h0", 0),
+                                scheme=args.partition)
+    dh.plan(mode=cfg["mode"], k=k, n_applies_hint=args.steps, hbm_budget_bytes=int(cfg.get("hbm_budget", 0)))
+    info = dh.h.get_plan()
+    psi = torch.from_numpy(make_psi(D, cfg["psi_seed"], k=k, dtype=cfg["dtype"])).cuda()
+    phi = torch.zeros_like(psi)
+    lam = lambda_grid(k) if k > 1 else None
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    for _ in range(args.warmup):
+        dh.apply(psi, phi, lam)
+    torch.cuda.synchronize()
+    dist.barrier()
+    torch.cuda.synchronize()
+    ms_local = time_steps(torch, lambda: dh.apply(psi, phi, lam), args.steps)
+    dist.barrier()
+    torch.cuda.synchronize()
+    clocks = sampler.stop() if rank == 0 else None
+    ms, _ = aggregate(dist, ms_local, 0.0, torch.device("cuda", local))
+    value = args.steps * float(D) * D / (ms * 1e-3)
+    if rank == 0:
+        wc = workload_config(args.workload, cfg)
+        wc["partition"] = {"scheme": args.partition, "world": world, "exchange_bytes_per_apply": psi.numel() * psi.element_size()}
+        print(json.dumps({"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                          "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+                          "scaling": "strong", "vs_baseline": None, "dtype": "f64" if cfg["dtype"] == "c128" else "f32",
+                          "data": "synthetic", "config": wc, "applies_per_s": value / (float(D) * D), "plan": info,
+                          "gpu_launches": info["launches_per_apply"] * args.steps, "clocks": clocks,
+                          "e2e": None, "roofline": None, "cpu_baseline": None}), flush=True)
+    dh.destroy()
+    dist.barrier()
+    dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -373,6 +441,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--workload", default="C2", choices=sorted(ALL))
+    ap.add_argument("--partition", default="none", choices=["none", "rows", "pairs"],
+                    help="N > 1 only: ONE operator over the N GPUs (mfh_set_partition + one NCCL exchange per apply, "
+                         "strong scaling) instead of N replicas")
     ap.add_argument("--no-extra", action="store_true", help="skip the other configs' side measurements")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -396,6 +467,10 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     barrier = (lambda: (dist.barrier(), torch.cuda.synchronize())) if dist else None
+
+    if world > 1 and args.partition != "none":
+        run_partitioned(torch, dist, args, rank, world, local)
+        return
 
     hbm_gbs, peak_src = load_peaks()
     sampler = ClockSampler(local)
@@ -435,6 +510,10 @@ def main():
             extras["SB18"] = measure_system_bath(torch, mfh, 10, hbm_gbs)
         except Exception as e:
             extras["SB18"] = {"error": str(e)}
+        try:
+            extras["C4-partitioned"] = measure_partition_projection(torch, mfh)
+        except Exception as e:
+            extras["C4-partitioned"] = {"error": str(e)}
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
