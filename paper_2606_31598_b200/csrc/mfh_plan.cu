@@ -342,15 +342,33 @@ static void candidate_json(std::string& s, const Candidate& c)
             c.t_apply, c.t_cached, c.t_proc, c.t_fill, c.t_job, c.flops, c.t_measured);
 }
 
+// Largest c in [0, c_max] with ok(c) (ok is monotone: more cached blocks need more memory); bisection,
+// because every probe builds the plan tables.
+template <typename F> static int largest_fitting(int c_max, F ok)
+{
+    if (c_max <= 0) return 0;
+    if (ok(c_max)) return c_max;
+    int lo = 0, hi = c_max;   // ok(lo) assumed (c = 0 caches nothing), !ok(hi)
+    while (hi - lo > 1) {
+        const int mid = lo + (hi - lo) / 2;
+        if (ok(mid)) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
 int enumerate_candidates(int64_t D, int dtype, int k, int mode, int B_req, int64_t n_applies,
                          double budget_bytes, int sm_count, std::vector<Candidate>& out, const Partition& part)
 {
     out.clear();
     std::vector<int> Bs;
     if (B_req > 0) Bs.push_back(B_req);
-    else
+    else {
+        // adaptive block size: powers of two dividing D, at most kMaxEnumBlocks block rows --
+        // smaller blocks only add per-block overhead (Eq. 32), and the tables grow as N_blk^2
+        const int kMaxEnumBlocks = 256;
         for (int B = MFH_MAX_B; B >= MFH_MIN_B; B /= 2)
-            if (D % B == 0) Bs.push_back(B);
+            if (D % B == 0 && (D / B <= kMaxEnumBlocks || Bs.empty())) Bs.push_back(B);
+    }
     const double cb = (double)complex_bytes(dtype);
     for (int B : Bs) {
         const int N = (int)(D / B);
@@ -365,16 +383,14 @@ int enumerate_candidates(int64_t D, int dtype, int k, int mode, int B_req, int64
         if ((mode == MFH_MODE_AUTO || mode == MFH_MODE_PAIRS) && k == 1 && B % (dtype == MFH_C128 ? 32 : 64) == 0) {
             // Hermitian pair cache: the largest number of block diagonals that fits (Eq. 27 over
             // canonical pairs)
-            int c = pair_full_offsets(N);
-            while (c > 0 && !fits(c, true)) --c;
+            int c = largest_fitting(pair_full_offsets(N), [&](int cc) { return fits(cc, true); });
             if (c > 0) cs.push_back({c, true});
             else if (mode == MFH_MODE_PAIRS) cs.push_back({1, true});   // reported as infeasible
         }
         if (mode == MFH_MODE_AUTO || mode == MFH_MODE_PARTIAL) {
             double room = budget_bytes - (double)fixed_work_bytes(D, dtype, k) - 3.0 * D * k * cb;
             int c = (int)std::floor(room * std::max(part.world, 1) / ((double)B * B * cb * N));   // a rank stores ~c N / world blocks
-            c = std::min(c, N - 1);
-            while (c > 0 && !fits(c, false)) --c;
+            c = largest_fitting(std::min(c, N - 1), [&](int cc) { return fits(cc, false); });
             if (c > 0) cs.push_back({c, false});
         }
         for (auto [c, pairs] : cs) {

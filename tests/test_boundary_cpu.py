@@ -134,3 +134,18 @@ def test_pairs_mode_and_pipe_rate_arguments():
     out = ctypes.c_double(0.0)
     assert L.mfh_debug_pipe_rates(99, ctypes.byref(out), None) == mfh.MFH_ERR_INVALID_ARG
     assert L.mfh_debug_pipe_rates(0, None, None) == mfh.MFH_ERR_INVALID_ARG
+
+
+def test_auto_enumeration_is_fast_at_the_largest_sizes():
+    """B = 0 enumerates block sizes; the candidate search must stay interactive at D = 2^18 (it once built
+    N_blk^2 tables for N_blk = 8192 thousands of times)."""
+    import time
+    t0 = time.time()
+    for D, dtype, k, free, n in [(262144, "c128", 1, 180e9, 10), (131072, "c128", 1, 150e9 / 0.9, 151),
+                                 (32768, "c64", 16, 180e9, 100)]:
+        rec = mfh.plan_analytic(D, dtype, k=k, n_applies_hint=n, hbm_free_bytes=int(free))
+        assert rec["chosen"]["feasible"] and all(c["n_blk"] <= 256 for c in rec["candidates"])
+    assert time.time() - t0 < 20.0
+    # C5 inside its 150 GB budget: the Hermitian pair cache holds the whole operator, AUTO prefers it to partial
+    rec = mfh.plan_analytic(131072, "c128", k=1, n_applies_hint=151, hbm_free_bytes=int(150e9 / 0.9))
+    assert rec["chosen"]["mode"] == "pairs" and rec["chosen"]["cached_fraction"] == 1.0
