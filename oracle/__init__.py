@@ -165,7 +165,8 @@ def apply_scan(D: int, B: int, seed_v: int, seed_h0: int, lambdas, Psi, rows=Non
     return out
 
 
-from .chebyshev import bessel_j_table, chebyshev_n_terms, chebyshev_propagate  # noqa: E402,F401
+from .chebyshev import (bessel_i_scaled_table, bessel_j_table, chebyshev_imag_n_terms, chebyshev_imag_propagate,  # noqa: E402,F401
+                        chebyshev_n_terms, chebyshev_propagate)
 from .lanczos import lanczos_bounds, lanczos_tridiagonal, ritz_extremes  # noqa: E402,F401
 from .system_bath import sb_apply  # noqa: E402,F401
 from .partition import apply_partition, combine as combine_partition, owned_blocks  # noqa: E402,F401
