@@ -127,6 +127,16 @@ MFH_API int mfh_apply_host(mfh_handle h, const void* psi_host, void* phi_host, i
 MFH_API int mfh_chebyshev(mfh_handle h, const void* psi_dev, void* out_dev, double t, double e_min,
                           double e_max, double tol, int32_t* n_terms_out, void* stream);
 
+/* out = exp(-beta (H - e_min)) psi, the imaginary-time (thermal / TPQ) Chebyshev filter the paper runs before its
+ * real-time propagation ("the imaginary-time TPQ Chebyshev filter used order 80"; the series is not
+ * printed there, R21).  Same recurrence as mfh_chebyshev (Eq. 41-43) with the modified-Bessel
+ * coefficients of e^{-a x} = I_0(a) + 2 sum_l (-1)^l I_l(a) T_l(x), a = R beta, scaled by e^{-a}:
+ *     out = sum_{l<K} (2 - delta_l0) (-1)^l [e^{-a} I_l(a)] T_l(H~) psi,   K = 1 + max{l : 2 e^{-a} I_l(a) >= tol},
+ * so exp(-beta H) psi = exp(-beta e_min) * out and no factor exceeds 1.  beta >= 0, R beta <= 600.
+ * *n_terms_out = K (may be NULL); K-1 applies of the planned path (k = 1).  Errors as mfh_chebyshev. */
+MFH_API int mfh_chebyshev_imag(mfh_handle h, const void* psi_dev, void* out_dev, double beta, double e_min,
+                               double e_max, double tol, int32_t* n_terms_out, void* stream);
+
 /* Spectral bounds by matrix-free Lanczos ("matrix-free Lanczos iterations estimate spectral bounds
  * E_min and E_max"; --lanczos-m 40; reading R18).  m steps (capped at D) of the plain
  * three-term recurrence from v_1 = psi/||psi||, each step one apply of the planned path (k = 1) plus O(D)

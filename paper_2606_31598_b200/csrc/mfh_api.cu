@@ -452,52 +452,92 @@ MFH_API int mfh_apply_host(mfh_handle h, const void* psi_host, void* phi_host, i
     return MFH_OK;
 }
 
-MFH_API int mfh_chebyshev(mfh_handle h, const void* psi_dev, void* out_dev, double t, double e_min,
-                          double e_max, double tol, int32_t* n_terms_out, void* stream)
+// The Chebyshev series driver shared by the real- and imaginary-time entry points: terms l = 0..K-1 of
+// out = phase * sum_l coef_l T_l(H~) psi with complex coefficients coef[l] = (re, im); K-1 chained applies.
+static int chebyshev_series(mfh_handle h, const void* psi_dev, void* out_dev, double c, double R, int K,
+                            const std::vector<double>& coef_re, const std::vector<double>& coef_im, double ph_re,
+                            double ph_im, cudaStream_t st)
 {
-    if (!h || !psi_dev || !out_dev) { set_error("mfh_chebyshev: NULL pointer"); return MFH_ERR_INVALID_ARG; }
-    if (!h->planned) { set_error("mfh_chebyshev: call mfh_plan first"); return MFH_ERR_BAD_STATE; }
-    if (h->plan.k != 1) { set_error("mfh_chebyshev: plan with k = 1"); return MFH_ERR_INVALID_ARG; }
-    if (!(e_max > e_min) || !std::isfinite(t) || !std::isfinite(e_min) || !std::isfinite(e_max) || !(tol > 0.0)) {
-        set_error("mfh_chebyshev: need e_max > e_min, finite t, tol > 0");
-        return MFH_ERR_INVALID_ARG;
-    }
-    cudaStream_t st = (cudaStream_t)stream;
-    const double c = 0.5 * (e_max + e_min), R = 0.5 * (e_max - e_min), a = R * t;   // P:707
-    // Bessel table J_l(a) via the C++17 special function (a route different from the oracle's
-    // Miller recurrence), K = 1 + last l with |J_l| >= tol.
-    const double x = std::fabs(a);
-    const int l_max = (int)(x + 80.0 + 12.0 * std::cbrt(x));
-    std::vector<double> J(l_max + 1);
-    int K = 1;
-    for (int l = 0; l <= l_max; ++l) {
-        double v = (x == 0.0) ? (l == 0 ? 1.0 : 0.0) : std::cyl_bessel_j((double)l, x);
-        if (a < 0 && (l & 1)) v = -v;
-        J[l] = v;
-        if (std::fabs(v) >= tol) K = l + 1;
-    }
-    if (K >= l_max) { set_error("mfh_chebyshev: Bessel table too short"); return MFH_ERR_NOT_CONVERGED; }
-    if (n_terms_out) *n_terms_out = K;
-
     const size_t vb = (size_t)h->D * complex_bytes(h->dtype);
     if (!h->d_cheb) MFH_CUDA_CHECK(cudaMalloc(&h->d_cheb, 5 * vb));   // cur, prev, acc, Hq + ping-pong of mfh_chebyshev_steps
     char* base = (char*)h->d_cheb;
     void *cur = base, *prev = base + vb, *acc = base + 2 * vb, *hq = base + 3 * vb;
     int rc;
-    if ((rc = launch_cheb_first(h, psi_dev, cur, acc, J[0], st))) return rc;      // Eq. 41
+    if ((rc = launch_cheb_first(h, psi_dev, cur, acc, coef_re[0], st))) return rc;      // Eq. 41 (coef_0 is real)
     for (int l = 1; l < K; ++l) {
         if ((rc = apply_chained(h, cur, hq, st))) return rc;
-        double cr = 0.0, ci = 0.0;                                                  // 2 (-i)^l J_l
-        switch (l & 3) {
-        case 0: cr = 2.0 * J[l]; break;
-        case 1: ci = -2.0 * J[l]; break;
-        case 2: cr = -2.0 * J[l]; break;
-        case 3: ci = 2.0 * J[l]; break;
-        }
-        if ((rc = launch_cheb_step(h, hq, cur, prev, acc, c, 1.0 / R, l == 1, cr, ci, st))) return rc;   // Eq. 42-43
+        if ((rc = launch_cheb_step(h, hq, cur, prev, acc, c, 1.0 / R, l == 1, coef_re[l], coef_im[l], st))) return rc;   // Eq. 42-43
         std::swap(cur, prev);
     }
-    return launch_cheb_final(h, acc, out_dev, std::cos(c * t), -std::sin(c * t), st);
+    return launch_cheb_final(h, acc, out_dev, ph_re, ph_im, st);
+}
+
+static int chebyshev_check(const char* fn, mfh_handle h, const void* psi_dev, const void* out_dev, double t, double e_min,
+                           double e_max, double tol)
+{
+    if (!h || !psi_dev || !out_dev) { set_error("%s: NULL pointer", fn); return MFH_ERR_INVALID_ARG; }
+    if (!h->planned) { set_error("%s: call mfh_plan first", fn); return MFH_ERR_BAD_STATE; }
+    if (h->plan.k != 1) { set_error("%s: plan with k = 1", fn); return MFH_ERR_INVALID_ARG; }
+    if (!(e_max > e_min) || !std::isfinite(t) || !std::isfinite(e_min) || !std::isfinite(e_max) || !(tol > 0.0)) {
+        set_error("%s: need e_max > e_min, finite t, tol > 0", fn);
+        return MFH_ERR_INVALID_ARG;
+    }
+    return MFH_OK;
+}
+
+MFH_API int mfh_chebyshev(mfh_handle h, const void* psi_dev, void* out_dev, double t, double e_min,
+                          double e_max, double tol, int32_t* n_terms_out, void* stream)
+{
+    int rc = chebyshev_check("mfh_chebyshev", h, psi_dev, out_dev, t, e_min, e_max, tol);
+    if (rc) return rc;
+    const double c = 0.5 * (e_max + e_min), R = 0.5 * (e_max - e_min), a = R * t;   // P:707
+    // Bessel table J_l(a) via the C++17 special function (a route different from the oracle's
+    // Miller recurrence), K = 1 + last l with |J_l| >= tol.
+    const double x = std::fabs(a);
+    const int l_max = (int)(x + 80.0 + 12.0 * std::cbrt(x));
+    std::vector<double> cr(l_max + 1, 0.0), ci(l_max + 1, 0.0);
+    int K = 1;
+    for (int l = 0; l <= l_max; ++l) {
+        double v = (x == 0.0) ? (l == 0 ? 1.0 : 0.0) : std::cyl_bessel_j((double)l, x);
+        if (a < 0 && (l & 1)) v = -v;
+        if (std::fabs(v) >= tol) K = l + 1;
+        if (l == 0) { cr[0] = v; continue; }
+        switch (l & 3) {                                                            // 2 (-i)^l J_l
+        case 0: cr[l] = 2.0 * v; break;
+        case 1: ci[l] = -2.0 * v; break;
+        case 2: cr[l] = -2.0 * v; break;
+        case 3: ci[l] = 2.0 * v; break;
+        }
+    }
+    if (K >= l_max) { set_error("mfh_chebyshev: Bessel table too short"); return MFH_ERR_NOT_CONVERGED; }
+    if (n_terms_out) *n_terms_out = K;
+    return chebyshev_series(h, psi_dev, out_dev, c, R, K, cr, ci, std::cos(c * t), -std::sin(c * t), (cudaStream_t)stream);
+}
+
+MFH_API int mfh_chebyshev_imag(mfh_handle h, const void* psi_dev, void* out_dev, double beta, double e_min,
+                               double e_max, double tol, int32_t* n_terms_out, void* stream)
+{
+    int rc = chebyshev_check("mfh_chebyshev_imag", h, psi_dev, out_dev, beta, e_min, e_max, tol);
+    if (rc) return rc;
+    const double c = 0.5 * (e_max + e_min), R = 0.5 * (e_max - e_min), a = R * beta;
+    if (beta < 0.0 || a > 600.0) {
+        set_error("mfh_chebyshev_imag: need beta >= 0 and R beta <= 600 (got %g)", a);
+        return MFH_ERR_INVALID_ARG;
+    }
+    // e^{-a} I_l(a) from the C++17 special function (the oracle uses Miller's recurrence); the scaled
+    // values decrease monotonically in l.
+    const int l_max = (int)(a + 60.0 + 12.0 * std::sqrt(a * 40.0 + 1.0));
+    std::vector<double> cr(l_max + 1, 0.0), ci(l_max + 1, 0.0);
+    const double ea = std::exp(-a);
+    int K = 1;
+    for (int l = 0; l <= l_max; ++l) {
+        const double v = (a == 0.0) ? (l == 0 ? 1.0 : 0.0) : std::cyl_bessel_i((double)l, a) * ea;
+        if (2.0 * v >= tol) K = l + 1;
+        cr[l] = (l == 0 ? 1.0 : 2.0) * ((l & 1) ? -v : v);
+    }
+    if (K >= l_max) { set_error("mfh_chebyshev_imag: Bessel table too short"); return MFH_ERR_NOT_CONVERGED; }
+    if (n_terms_out) *n_terms_out = K;
+    return chebyshev_series(h, psi_dev, out_dev, c, R, K, cr, ci, 1.0, 0.0, (cudaStream_t)stream);
 }
 
 // Extreme eigenvalues of the symmetric tridiagonal T (diagonal a[0..m-1], off-diagonal b[0..m-2]) by
