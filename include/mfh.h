@@ -204,7 +204,7 @@ MFH_API int mfh_get_plan(mfh_handle h, char* json_out, size_t json_cap);
  *     Y = H_B X + g (B_1 X) A^T + X H_S^T.
  *   HS_host, A_host   d_S x d_S Hermitian matrices, row-major interleaved complex doubles (host)
  *   d_S <= MFH_MAX_K; d_B, B as in mfh_create.  mfh_sb_plan plans both bath operators with k = d_S
- *   (cached blocks need complex64 and B % 128 == 0) inside the budget (0 = 0.9 x free memory).
+ *   (cached blocks need B % 128 == 0) inside the budget (0 = 0.9 x free memory).
  * Errors as for mfh_create / mfh_plan / mfh_apply. */
 typedef struct mfh_sb_s* mfh_sb_handle;
 MFH_API int mfh_sb_create(mfh_sb_handle* out, int64_t d_B, int32_t d_S, int32_t B, uint64_t seed_HB, uint64_t seed_B1,

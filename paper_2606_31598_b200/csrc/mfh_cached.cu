@@ -164,13 +164,139 @@ __global__ void __launch_bounds__(32 * CACHED_WARPS) cached_kernel_c64(const Cac
     }
 }
 
+// --------------------------------------------------------------------------------------------
+// k vectors from cached complex128 blocks (coupling scans and the system-bath action in double precision;
+// Eq. 12, north_star (c): "reads each V block once for k vectors").  4 k DFMA per 16-byte entry:
+// FP64-pipe bound from k = 8 up (k = 16: 64 DFMA per entry = 1 entry/clk/SM = 4.5 TB/s of matrix), HBM bound
+// below; there is no FP64 tensor path that would beat the 64 lanes/clk/SM of the CUDA cores, so this is a
+// CUDA-core kernel.  A CTA of 128 threads owns 128 rows x one cached block (lane = row, k complex
+// accumulators in registers, no reduction); column chunks of 16 entries are staged in shared memory by
+// cp.async (16-byte LDGSTS, coalesced 256-byte row runs, double-buffered) in rows padded to 17 entries so
+// that the lane = row reads are bank-conflict free; the psi rows of the chunk sit beside them and are read as
+// broadcasts.  Output: the partial slot of column block m, as the other k-vector kernels.
+// --------------------------------------------------------------------------------------------
+constexpr int CM_ROWS = 128, CM_COLS = 16, CM_PAD = CM_COLS + 1;
+
+struct CachedMultiParams {
+    int32_t B, n_blk, k, slot_multi;
+    int64_t D;
+    const int32_t* cache_slot;
+    const double2* cache;
+    const double2* psi;   // [D][k]
+    double2* work;        // [n_slots][D][k]
+};
+
+__device__ __forceinline__ void cp_async16(void* dst_smem, const void* src)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(dst_smem)), "l"(src)
+                 : "memory");
+}
+
+template <int KT>
+__global__ void __launch_bounds__(CM_ROWS) cached_multi_kernel_c128(const CachedMultiParams P)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int TILE = CM_ROWS * CM_PAD;               // entries per stage (padded)
+    double2* tiles = reinterpret_cast<double2*>(smem_raw);             // [2][128][17]
+    double2* psis = tiles + 2 * TILE;                                  // [2][16][KT]
+    const int t = threadIdx.x, m = blockIdx.y, k = P.k;
+    const int64_t i_base = (int64_t)blockIdx.x * CM_ROWS;
+    const int n = (int)(i_base / P.B);
+    const int32_t slot = P.cache_slot[n * P.n_blk + m];
+    if (slot < 0) return;                                               // generated (or foreign) block
+    const double2* blk = P.cache + (size_t)slot * P.B * P.B + (size_t)(i_base - (int64_t)n * P.B) * P.B;
+    const double2* psim = P.psi + (size_t)m * P.B * k;
+    const int n_chunks = P.B / CM_COLS;
+
+    auto issue = [&](int ch, int st) {
+        // 128 rows x 16 entries: thread t copies entry (t & 15) of rows (t >> 4) + 8 j
+        double2* dst = tiles + st * TILE;
+        const double2* src = blk + (size_t)ch * CM_COLS + (t & 15);
+#pragma unroll
+        for (int j = 0; j < CM_ROWS / 8; ++j) {
+            const int r = (t >> 4) + 8 * j;
+            cp_async16(dst + r * CM_PAD + (t & 15), src + (size_t)r * P.B);
+        }
+        // psi rows of the chunk: 16 x k entries, contiguous in [D][k]
+        const double2* ps = psim + (size_t)ch * CM_COLS * k;
+        for (int e = t; e < CM_COLS * k; e += CM_ROWS) cp_async16(psis + st * CM_COLS * KT + (e / k) * KT + (e % k), ps + e);
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+
+    double2 acc[KT];
+#pragma unroll
+    for (int v = 0; v < KT; ++v) acc[v] = double2{0.0, 0.0};
+    if (k < KT)   // unused vector slots of the staged psi rows stay zero
+        for (int e = t; e < 2 * CM_COLS * KT; e += CM_ROWS) psis[e] = double2{0.0, 0.0};
+    __syncthreads();
+    issue(0, 0);
+    for (int ch = 0; ch < n_chunks; ++ch) {
+        const int st = ch & 1;
+        if (ch + 1 < n_chunks) {
+            issue(ch + 1, st ^ 1);
+            asm volatile("cp.async.wait_group 1;" ::: "memory");
+        } else {
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+        }
+        __syncthreads();
+        const double2* row = tiles + st * TILE + t * CM_PAD;
+        const double2* pc = psis + st * CM_COLS * KT;
+#pragma unroll 4
+        for (int c = 0; c < CM_COLS; ++c) {
+            const double2 hv = row[c];
+#pragma unroll
+            for (int v = 0; v < KT; ++v) {
+                const double2 p = pc[c * KT + v];
+                acc[v].x = fma(hv.x, p.x, acc[v].x);
+                acc[v].x = fma(-hv.y, p.y, acc[v].x);
+                acc[v].y = fma(hv.x, p.y, acc[v].y);
+                acc[v].y = fma(hv.y, p.x, acc[v].y);
+            }
+        }
+        __syncthreads();   // the stage is free for the copy issued in the next iteration
+    }
+    double2* dst = P.work + ((size_t)(P.slot_multi + m) * P.D + i_base + t) * k;
+#pragma unroll
+    for (int v = 0; v < KT; ++v)
+        if (v < k) dst[v] = acc[v];
+}
+
+bool cached_multi_c128_supported(int dtype, int k, int B) { return dtype == MFH_C128 && k > 1 && k <= MFH_MAX_K && B % CM_ROWS == 0; }
+
+template <int KT> static int launch_cached_multi_c128_t(mfh_handle h, const void* psi, cudaStream_t st)
+{
+    const Plan& p = h->plan;
+    CachedMultiParams P{p.B, p.n_blk, p.k, p.slot_multi, h->D, h->d_cache_slot, (const double2*)h->d_cache,
+                        (const double2*)psi, (double2*)h->d_work};
+    const size_t smem = (size_t)(2 * CM_ROWS * CM_PAD + 2 * CM_COLS * KT) * sizeof(double2);
+    auto kern = cached_multi_kernel_c128<KT>;
+    static bool attr_done = false;
+    if (!attr_done) {
+        MFH_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_done = true;
+    }
+    kern<<<dim3((unsigned)(h->D / CM_ROWS), p.n_blk), CM_ROWS, smem, st>>>(P);
+    MFH_CUDA_CHECK(cudaGetLastError());
+    return MFH_OK;
+}
+
+static int launch_cached_multi_c128(mfh_handle h, const void* psi, cudaStream_t st)
+{
+    const int k = h->plan.k;
+    if (k <= 2) return launch_cached_multi_c128_t<2>(h, psi, st);
+    if (k <= 4) return launch_cached_multi_c128_t<4>(h, psi, st);
+    if (k <= 8) return launch_cached_multi_c128_t<8>(h, psi, st);
+    return launch_cached_multi_c128_t<16>(h, psi, st);
+}
+
 int launch_cached(mfh_handle h, const void* psi, cudaStream_t st)
 {
     const Plan& p = h->plan;
     if (p.n_cached == 0) return MFH_OK;
     if (p.k != 1) {
         if (tc_cached_multi_supported(h->dtype, p.k, p.B)) return launch_cached_multi_tc(h, psi, st);
-        set_error("cached blocks with k > 1 need complex64 and B %% 128 == 0");
+        if (cached_multi_c128_supported(h->dtype, p.k, p.B)) return launch_cached_multi_c128(h, psi, st);
+        set_error("cached blocks with k > 1 need B %% 128 == 0");
         return MFH_ERR_UNSUPPORTED;
     }
     const unsigned grid = (unsigned)(h->D / CACHED_ROWS);

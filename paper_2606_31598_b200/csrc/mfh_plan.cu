@@ -396,8 +396,9 @@ int enumerate_candidates(int64_t D, int dtype, int k, int mode, int B_req, int64
         for (auto [c, pairs] : cs) {
             Candidate cand = evaluate_candidate(D, dtype, k, B, c, pairs, n_applies, sm_count, part);
             cand.feasible = (cand.cache_bytes + cand.work_bytes <= budget_bytes);   // Eq. 18
-            // cached k-vector blocks: tensor-core kernel, complex64 with B % 128 == 0 only
-            if (k > 1 && c > 0 && (pairs || !tc_cached_multi_supported(dtype, k, B))) cand.feasible = false;
+            // cached k-vector blocks: B % 128 == 0 (tensor-core kernel for complex64, FP64 CUDA-core kernel for complex128)
+            if (k > 1 && c > 0 && (pairs || !(tc_cached_multi_supported(dtype, k, B) || cached_multi_c128_supported(dtype, k, B))))
+                cand.feasible = false;
             out.push_back(cand);
         }
     }

@@ -123,12 +123,16 @@ def test_pairs_mode_and_pipe_rate_arguments():
     # C5: the whole operator fits the 150 GB budget as pairs (141.7 GB), not as full blocks (275 GB)
     r = mfh.plan_analytic(131072, "c128", 1, "pairs", 4096, 151, int(150e9 / 0.9))
     assert r["chosen"]["cached_fraction"] == 1.0 and r["chosen"]["total_bytes"] <= 150e9
-    # k-vector plans: cached blocks need the tensor-core kernel (complex64, B % 128 == 0); never pairs
+    # k-vector plans: cached blocks need B % 128 == 0 (tensor-core kernel for complex64, FP64 kernel for
+    # complex128); never pairs
     r = mfh.plan_analytic(32768, "c64", 16, "full", 1024, 100, 180 * 10**9)
     assert r["chosen"]["feasible"] and r["chosen"]["cache_bytes"] == 32768**2 * 8
-    with pytest.raises(mfh.MfhError) as e:
-        mfh.plan_analytic(32768, "c128", 16, "full", 1024, 100, 180 * 10**9)
-    assert e.value.code == mfh.MFH_ERR_OUT_OF_MEMORY
+    r = mfh.plan_analytic(32768, "c128", 16, "full", 1024, 100, 180 * 10**9)
+    assert r["chosen"]["feasible"] and r["chosen"]["cache_bytes"] == 32768**2 * 16
+    for dtype, B, mode in [("c128", 96, "full"), ("c64", 96, "full"), ("c128", 1024, "pairs")]:
+        with pytest.raises(mfh.MfhError) as e:
+            mfh.plan_analytic(3072 * 8, dtype, 16, mode, B, 100, 180 * 10**9)
+        assert e.value.code == mfh.MFH_ERR_OUT_OF_MEMORY
     # measurement export: argument errors come before any device work
     L = mfh.lib()
     out = ctypes.c_double(0.0)

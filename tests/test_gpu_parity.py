@@ -220,20 +220,33 @@ def test_scan_c64_tensor_core_and_cuda_core_shapes(D, B, k):
 
 
 @pytest.mark.parametrize("mode,budget", [("full", 0), ("partial", 12e6), ("partial", 24e6)])
-@pytest.mark.parametrize("k", [16, 5])
-def test_scan_c64_cached_blocks_tensor_core(mode, budget, k):
-    # cached k-vector path: each stored V block is read once for all k vectors (TMA -> TMEM -> tcgen05),
-    # alone and mixed with generated blocks
-    D, B = 2048, 256          # 8x8 blocks of 512 KiB
-    Psi = make_psi(D, 13, k=k, dtype="c64")
+@pytest.mark.parametrize("dtype,k", [("c64", 16), ("c64", 5), ("c128", 16), ("c128", 8), ("c128", 3), ("c128", 2)])
+def test_scan_cached_blocks_k_vectors(mode, budget, dtype, k):
+    # cached k-vector path: each stored V block is read once for all k vectors (complex64: TMA -> TMEM ->
+    # tcgen05; complex128: cp.async staging -> FP64 CUDA cores), alone and mixed with generated blocks
+    D, B = 2048, 256          # 8x8 blocks of 512 KiB (c64) / 1 MiB (c128)
+    Psi = make_psi(D, 13, k=k, dtype=dtype)
     lam = 0.25 + lambda_grid(k)
-    h = mfh.Hamiltonian(D, B, 8, "c64", kind="diag_plus_gue", seed_h0=7)
-    plan = h.plan(mode, k=k, hbm_budget_bytes=int(budget))
+    h = mfh.Hamiltonian(D, B, 8, dtype, kind="diag_plus_gue", seed_h0=7)
+    plan = h.plan(mode, k=k, hbm_budget_bytes=int(budget * (2 if dtype == "c128" else 1)))
     assert plan["chosen"]["mode"] == mode
     Phi = h.apply(to_dev(Psi), lambdas=lam).cpu().numpy()
     ref = oracle.apply_scan(D, B, 8, 7, lam, Psi)
     for v in range(k):
-        assert rel_l2(Phi[:, v], ref[:, v]) <= TOL["c64"], v
+        assert rel_l2(Phi[:, v], ref[:, v]) <= TOL[dtype], v
+
+
+def test_scan_c128_cached_single_block_and_min_block():
+    # one 128 x 128 block (every entry from the general rule) and the smallest supported block size
+    for D, B, k in [(128, 128, 16), (1024, 128, 7)]:
+        Psi = make_psi(D, 17, k=k)
+        lam = lambda_grid(k)
+        h = mfh.Hamiltonian(D, B, 8, "c128", kind="diag_plus_gue", seed_h0=7)
+        h.plan("full", k=k)
+        Phi = h.apply(to_dev(Psi), lambdas=lam).cpu().numpy()
+        ref = oracle.apply_scan(D, B, 8, 7, lam, Psi)
+        for v in range(k):
+            assert rel_l2(Phi[:, v], ref[:, v]) <= TOL["c128"], (D, v)
 
 
 def test_multi_vector_equals_single_vector_applies():
