@@ -468,7 +468,12 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     barrier = (lambda: (dist.barrier(), torch.cuda.synchronize())) if dist else None
 
-    if world > 1 and args.partition != "none":
+    if args.partition != "none":
+        if dist is None:   # one GPU: a single-rank group, so that the same code path runs (and is tested) here
+            import torch.distributed as dist
+            os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+            os.environ.setdefault("MASTER_PORT", "29617")
+            dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", local))
         run_partitioned(torch, dist, args, rank, world, local)
         return
 

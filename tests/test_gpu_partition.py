@@ -162,3 +162,19 @@ def test_chained_drivers_call_the_exchange_hook():
         h2.chebyshev(psi, 1.0, -2.1, 2.1, 1e-10)
     assert e.value.code == mfh.MFH_ERR_BAD_STATE
     h2.destroy()
+
+
+def test_bench_partition_mode_runs_on_one_gpu():
+    """bench.py --partition: the sharded-job arm (DistributedHamiltonian + NCCL exchange) with a single-rank
+    group; the line must carry the contract keys and the C1 throughput of the plain arm's order."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--workload", "C1", "--partition", "pairs",
+                        "--steps", "5", "--warmup", "3"], capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stderr[-2000:]
+    line = json.loads(r.stdout.strip().splitlines()[-1])
+    assert line["scaling"] == "strong" and line["n_gpus"] == 1 and line["config"]["partition"]["scheme"] == "pairs"
+    assert line["value"] > 1e10 and line["gpu_launches"] > 0
