@@ -84,6 +84,21 @@ MFH_API int mfh_plan_analytic(int64_t D, int32_t dtype, int32_t k, int32_t mode,
                               int64_t n_applies_hint, int64_t hbm_free_bytes, char* json_out,
                               size_t json_cap);
 
+/* Node-level analytic planner (Algorithm 1 with the task waves of Eq. 19; "parameter-parallel",
+ * "row-parallel", "hybrid"; worked example P:765-779).  Pure host arithmetic.  n_tasks independent outer-loop jobs
+ * (coupling values, ...) of n_applies_per_task applications of n_op dense operators on k vectors are spread over
+ * n_gpus GPUs in groups of p_row GPUs (p_row = 1: parameter-parallel, p_row = n_gpus: row-parallel, between:
+ * hybrid); inside a group the operator is partitioned with `scheme` (MFH_PART_ROWS / MFH_PART_PAIRS, see
+ * mfh_set_partition).  For every p_row dividing n_gpus: C = n_gpus / p_row groups, W = ceil(n_tasks / C) waves
+ * (Eq. 19), the best memory-feasible single-GPU plan of one rank of the group (Eq. 14-18 with alpha = 0.9 on
+ * hbm_free_bytes_per_gpu, each operator getting 1/n_op of it), seconds per application = n_op x (local apply
+ * + exchange of D k B_c bytes), score = W x n_applies_per_task x seconds per application (Eq. 22 with the model
+ * time).  The JSON lists every p_row (feasible or not) and the chosen one (smallest score; ties -> smaller p_row).
+ * Errors: INVALID_ARG; OUT_OF_MEMORY when no p_row has a feasible plan. */
+MFH_API int mfh_plan_node_analytic(int64_t D, int32_t dtype, int32_t k, int32_t n_op, int64_t n_tasks, int32_t n_gpus,
+                                   int64_t hbm_free_bytes_per_gpu, int32_t mode, int32_t B, int32_t scheme,
+                                   int64_t n_applies_per_task, char* json_out, size_t json_cap);
+
 /* Plan and commit: choose mode and B (analytic; measure != 0 additionally times the best
  * candidates on the device, Algorithm 2, R_warm = 1, R_bench = 3, K_bench <= 8), allocate the
  * cache and the workspace and fill the cache with the generator (one-time cost).

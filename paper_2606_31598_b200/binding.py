@@ -28,7 +28,7 @@ MODES = {"auto": MFH_MODE_AUTO, "procedural": MFH_MODE_PROCEDURAL, "partial": MF
          "full": MFH_MODE_FULL, "pairs": MFH_MODE_PAIRS}
 
 # every symbol include/mfh.h declares (tests check that the library exports all of them)
-SYMBOLS = ["mfh_create", "mfh_plan_analytic", "mfh_plan", "mfh_apply", "mfh_apply_host", "mfh_apply_timed",
+SYMBOLS = ["mfh_create", "mfh_plan_analytic", "mfh_plan_node_analytic", "mfh_plan", "mfh_apply", "mfh_apply_host", "mfh_apply_timed",
            "mfh_chebyshev", "mfh_chebyshev_imag", "mfh_chebyshev_steps", "mfh_lanczos_bounds", "mfh_destroy", "mfh_last_error", "mfh_get_plan", "mfh_debug_philox",
            "mfh_materialize_block", "mfh_debug_h0", "mfh_debug_pipe_rates", "mfh_sb_create", "mfh_sb_plan", "mfh_sb_apply",
            "mfh_sb_destroy", "mfh_set_partition", "mfh_get_partition_rows", "mfh_set_exchange"]
@@ -56,6 +56,7 @@ def lib():
     dbl, cp, sz = ctypes.c_double, ctypes.c_char_p, ctypes.c_size_t
     L.mfh_create.argtypes = [ctypes.POINTER(vp), i64, i32, u64, i32, dbl, i32, u64]
     L.mfh_plan_analytic.argtypes = [i64, i32, i32, i32, i32, i64, i64, cp, sz]
+    L.mfh_plan_node_analytic.argtypes = [i64, i32, i32, i32, i64, i32, i64, i32, i32, i32, i64, cp, sz]
     L.mfh_plan.argtypes = [vp, i32, i32, i64, i64, i32, vp, cp, sz]
     L.mfh_apply.argtypes = [vp, vp, vp, i32, ctypes.POINTER(dbl), vp]
     L.mfh_apply_host.argtypes = [vp, vp, vp, i32, ctypes.POINTER(dbl), vp]
@@ -110,6 +111,18 @@ def plan_analytic(D: int, dtype: str, k: int = 1, mode: str = "auto", B: int = 0
     buf = ctypes.create_string_buffer(1 << 16)
     rc = lib().mfh_plan_analytic(D, DTYPES[dtype], k, MODES[mode], B, n_applies_hint, hbm_free_bytes,
                                  buf, len(buf))
+    rec = json.loads(buf.value.decode()) if buf.value else {}
+    if rc != MFH_OK:
+        raise MfhError(rc, lib().mfh_last_error().decode())
+    return rec
+
+
+def plan_node_analytic(D: int, dtype: str, k: int, n_op: int, n_tasks: int, n_gpus: int, hbm_free_bytes_per_gpu: int,
+                       mode: str = "auto", B: int = 0, scheme: str = "pairs", n_applies_per_task: int = 1) -> dict:
+    """Host-only node-level planner: row-group size, GPU groups and task waves (Eq. 19); needs no GPU."""
+    buf = ctypes.create_string_buffer(1 << 16)
+    rc = lib().mfh_plan_node_analytic(D, DTYPES[dtype], k, n_op, n_tasks, n_gpus, int(hbm_free_bytes_per_gpu), MODES[mode], B,
+                                      PARTITIONS[scheme], n_applies_per_task, buf, len(buf))
     rec = json.loads(buf.value.decode()) if buf.value else {}
     if rc != MFH_OK:
         raise MfhError(rc, lib().mfh_last_error().decode())

@@ -299,6 +299,24 @@ MFH_API int mfh_plan_analytic(int64_t D, int32_t dtype, int32_t k, int32_t mode,
     return rc;
 }
 
+MFH_API int mfh_plan_node_analytic(int64_t D, int32_t dtype, int32_t k, int32_t n_op, int64_t n_tasks, int32_t n_gpus,
+                                   int64_t hbm_free_bytes_per_gpu, int32_t mode, int32_t B, int32_t scheme,
+                                   int64_t n_applies_per_task, char* json_out, size_t json_cap)
+{
+    if (D < 32 || D % 32 != 0 || (dtype != MFH_C128 && dtype != MFH_C64) || k < 1 || k > MFH_MAX_K || n_op < 1 || n_op > 16 ||
+        n_tasks < 1 || n_gpus < 1 || n_gpus > 1024 || hbm_free_bytes_per_gpu <= 0 || mode < MFH_MODE_AUTO || mode > MFH_MODE_PAIRS ||
+        (B != 0 && !valid_B(D, B)) || (scheme != MFH_PART_ROWS && scheme != MFH_PART_PAIRS) || n_applies_per_task < 1) {
+        set_error("mfh_plan_node_analytic: invalid argument");
+        return MFH_ERR_INVALID_ARG;
+    }
+    std::string json;
+    const int rc = plan_node(D, dtype, k, n_op, n_tasks, n_gpus, (double)hbm_free_bytes_per_gpu, mode, B, scheme,
+                             n_applies_per_task, json);
+    copy_json(json, json_out, json_cap);
+    if (rc) set_error("mfh_plan_node_analytic: no row-group size has a plan that fits");
+    return rc;
+}
+
 MFH_API int mfh_plan(mfh_handle h, int32_t mode, int32_t k, int64_t n_applies_hint,
                      int64_t hbm_budget_bytes, int32_t measure, void* stream, char* json_out,
                      size_t json_cap)

@@ -430,4 +430,69 @@ std::string plan_json(int64_t D, int dtype, int k, int64_t n_applies, double bud
 
 double planner_alpha() { return kAlpha; }
 
+// Exchange step of a row group (all-gather or all-reduce of D k B_c bytes over NVLink 5 / NVSwitch): a
+// latency term plus the bytes a rank receives at a conservative 400 GB/s.
+static double exchange_seconds(int64_t D, int dtype, int k, int p_row)
+{
+    if (p_row <= 1) return 0.0;
+    const double bytes = (double)D * k * complex_bytes(dtype);
+    return 20e-6 + bytes * (double)(p_row - 1) / p_row / 400e9;
+}
+
+int plan_node(int64_t D, int dtype, int k, int n_op, int64_t n_tasks, int n_gpus, double free_per_gpu, int mode, int B_req,
+              int scheme, int64_t n_applies_per_task, std::string& json)
+{
+    const double budget = kAlpha * free_per_gpu / n_op;   // Eq. 18, the operators share the memory evenly
+    struct Row {
+        int p_row, groups;
+        int64_t waves;
+        bool feasible;
+        Candidate c;
+        double t_apply, score;
+    };
+    std::vector<Row> rows;
+    int best = -1;
+    for (int p_row = 1; p_row <= n_gpus; ++p_row) {
+        if (n_gpus % p_row) continue;
+        Row r;
+        r.p_row = p_row;
+        r.groups = n_gpus / p_row;                                        // C(p)
+        r.waves = (n_tasks + r.groups - 1) / r.groups;                     // Eq. 19
+        Partition part;
+        part.rank = 0;
+        part.world = p_row;
+        part.scheme = p_row > 1 ? scheme : (int)MFH_PART_NONE;
+        std::vector<Candidate> cands;
+        const int rc = enumerate_candidates(D, dtype, k, mode, B_req, r.waves * n_applies_per_task, budget, 148, cands, part);
+        r.feasible = (rc == MFH_OK);
+        if (!cands.empty()) r.c = cands[0];
+        r.t_apply = r.feasible ? n_op * (r.c.t_apply + exchange_seconds(D, dtype, k, p_row)) : 0.0;
+        r.score = r.feasible ? (double)r.waves * ((double)n_applies_per_task * r.t_apply + n_op * r.c.t_fill / std::max<int64_t>(r.waves, 1)) : 0.0;
+        if (r.feasible && (best < 0 || r.score < rows[best].score)) best = (int)rows.size();
+        rows.push_back(r);
+    }
+    auto row_json = [&](const Row& r) {
+        appendf(json, "{\"p_row\":%d,\"groups\":%d,\"waves\":%lld,\"strategy\":\"%s\",\"feasible\":%s,", r.p_row, r.groups,
+                (long long)r.waves, r.p_row == 1 ? "parameter-parallel" : (r.p_row == n_gpus ? "row-parallel" : "hybrid"),
+                r.feasible ? "true" : "false");
+        appendf(json, "\"mode\":\"%s\",\"B\":%d,\"operator_bytes_per_gpu\":%.0f,\"work_bytes_per_gpu\":%.0f,"
+                      "\"total_bytes_per_gpu\":%.0f,\"model_apply_s\":%.6g,\"score_s\":%.6g}",
+                mode_name(r.c.mode), r.c.B, n_op * r.c.cache_bytes, n_op * r.c.work_bytes,
+                n_op * (r.c.cache_bytes + r.c.work_bytes), r.t_apply, r.score);
+    };
+    appendf(json, "{\"D\":%lld,\"dtype\":\"%s\",\"k\":%d,\"n_op\":%d,\"n_tasks\":%lld,\"n_gpus\":%d,\"alpha\":%.2f,"
+                  "\"budget_bytes_per_gpu\":%.0f,\"scheme\":\"%s\",\"flops_per_apply\":%.6g,\"chosen\":",
+            (long long)D, dtype == MFH_C128 ? "c128" : "c64", k, n_op, (long long)n_tasks, n_gpus, kAlpha, kAlpha * free_per_gpu,
+            scheme == MFH_PART_ROWS ? "rows" : "pairs", 8.0 * n_op * (double)D * (double)D * k);
+    if (best >= 0) row_json(rows[best]);
+    else json += "null";
+    json += ",\"row_groups\":[";
+    for (size_t i = 0; i < rows.size(); ++i) {
+        if (i) json += ",";
+        row_json(rows[i]);
+    }
+    json += "]}";
+    return best >= 0 ? MFH_OK : MFH_ERR_OUT_OF_MEMORY;
+}
+
 }  // namespace mfh

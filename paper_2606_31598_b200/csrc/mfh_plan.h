@@ -39,5 +39,8 @@ int enumerate_candidates(int64_t D, int dtype, int k, int mode, int B_req, int64
 std::string plan_json(int64_t D, int dtype, int k, int64_t n_applies, double budget, int measured,
                       const std::vector<Candidate>& cands);
 double planner_alpha();
+// Node-level plan space (Eq. 19): JSON over the row-group sizes; returns MFH_OK or MFH_ERR_OUT_OF_MEMORY.
+int plan_node(int64_t D, int dtype, int k, int n_op, int64_t n_tasks, int n_gpus, double free_per_gpu, int mode, int B_req,
+              int scheme, int64_t n_applies_per_task, std::string& json);
 
 }  // namespace mfh

@@ -59,6 +59,41 @@ def exchange(phi, scheme: str, rows, group=None):
     return phi
 
 
+def row_groups(world: int, p_row: int):
+    """GPU groups of a hybrid plan: consecutive ranks form a row group of size p_row,
+    e.g. world 8, p_row 2 -> [[0, 1], [2, 3], [4, 5], [6, 7]] (the grouping the paper's run prints)."""
+    if p_row < 1 or world % p_row:
+        raise ValueError(f"row-group size {p_row} does not divide {world} GPUs")
+    return [list(range(g * p_row, (g + 1) * p_row)) for g in range(world // p_row)]
+
+
+def task_waves(n_tasks: int, n_groups: int):
+    """Independent tasks (coupling values, ...) dealt to the groups wave by wave: wave w holds the tasks
+    w C .. w C + C - 1, task t runs on group t mod C; len(result) = W(p) = ceil(N_task / C) (Eq. 19)."""
+    return [[(t % n_groups, t) for t in range(w * n_groups, min((w + 1) * n_groups, n_tasks))]
+            for w in range((n_tasks + n_groups - 1) // n_groups)]
+
+
+def make_group(p_row: int):
+    """Create the process groups of a hybrid plan (collective: every rank calls it) and return
+    (this rank's group, its group index, number of groups).  p_row = 1: parameter-parallel, no exchange;
+    p_row = world: row-parallel."""
+    import torch.distributed as dist
+    world, rank = dist.get_world_size(), dist.get_rank()
+    mine = None
+    groups = row_groups(world, p_row)
+    for g, ranks in enumerate(groups):
+        pg = dist.new_group(ranks)            # every rank must take part in every new_group call
+        if rank in ranks:
+            mine = (pg, g)
+    return mine[0], mine[1], len(groups)
+
+
+def my_tasks(n_tasks: int, group_index: int, n_groups: int):
+    """The tasks of one group, in wave order."""
+    return [t for wave in task_waves(n_tasks, n_groups) for (g, t) in wave if g == group_index]
+
+
 class _DevicePtr:
     """A library-owned device vector seen through the CUDA array interface (no copy, no ownership)."""
 

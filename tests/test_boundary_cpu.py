@@ -153,3 +153,54 @@ def test_auto_enumeration_is_fast_at_the_largest_sizes():
     # C5 inside its 150 GB budget: the Hermitian pair cache holds the whole operator, AUTO prefers it to partial
     rec = mfh.plan_analytic(131072, "c128", k=1, n_applies_hint=151, hbm_free_bytes=int(150e9 / 0.9))
     assert rec["chosen"]["mode"] == "pairs" and rec["chosen"]["cached_fraction"] == 1.0
+
+
+def test_node_planner_reproduces_the_papers_hybrid_plan():
+    """P:765-779 and Fig. 1: eight 43.97 GiB GPUs, two dense complex64 bath operators of d_B = 65536 on R = 4
+    columns, 20 coupling values -> full-cache hybrid plan with row-group size 2: gpu groups [[0,1],...,[6,7]], 32 GiB
+    of operator storage per GPU, five waves; row-group size 4 needs ten waves; one GPU cannot hold 64 GiB."""
+    from paper_2606_31598_b200.distributed import row_groups, task_waves
+    GiB = 2**30
+    rec = mfh.plan_node_analytic(65536, "c64", 4, 2, 20, 8, int(43.97 * GiB), mode="full", B=4096, scheme="rows",
+                                 n_applies_per_task=1000)
+    by = {r["p_row"]: r for r in rec["row_groups"]}
+    assert sorted(by) == [1, 2, 4, 8]
+    assert not by[1]["feasible"] and by[1]["operator_bytes_per_gpu"] == 64 * GiB          # Eq. 15, Eq. 18
+    ch = rec["chosen"]
+    assert ch["p_row"] == 2 and ch["groups"] == 4 and ch["waves"] == 5 and ch["strategy"] == "hybrid"
+    assert ch["operator_bytes_per_gpu"] == 32 * GiB                                       # "32 GiB ... per GPU"
+    assert ch["total_bytes_per_gpu"] <= 32.2 * GiB                                        # "32.1 GiB total"
+    assert rec["flops_per_apply"] == pytest.approx(2.749e11, rel=1e-3)                    # "2 d_S d_R^2 8"
+    assert by[4]["waves"] == 10 and by[8]["waves"] == 20 and by[8]["strategy"] == "row-parallel"
+    assert by[4]["model_apply_s"] < ch["model_apply_s"] and by[4]["score_s"] > ch["score_s"]   # Fig. 1 A2
+    # the printed score: five waves of the measured 0.104089 s
+    assert len(task_waves(20, ch["groups"])) == 5 and 5 * 0.104089 == pytest.approx(0.520447, abs=3e-6)
+    assert row_groups(8, 2) == [[0, 1], [2, 3], [4, 5], [6, 7]]                            # "gpu groups = ..."
+    # with the mode left open the planner still prefers the fully cached row groups of two
+    auto = mfh.plan_node_analytic(65536, "c64", 4, 2, 20, 8, int(43.97 * GiB), n_applies_per_task=1000, scheme="rows")
+    assert auto["chosen"]["p_row"] == 2 and auto["chosen"]["mode"] == "full"
+    # one B200 holds both operators: with 16 tasks on eight GPUs parameter-parallel execution wins (two full waves);
+    # with the paper's 20 tasks its third wave is half empty and row groups of two (five full waves) stay ahead
+    b200 = mfh.plan_node_analytic(65536, "c64", 4, 2, 16, 8, 180 * 10**9, n_applies_per_task=1000)
+    assert b200["chosen"]["p_row"] == 1 and b200["chosen"]["waves"] == 2 and b200["chosen"]["strategy"] == "parameter-parallel"
+    b200 = mfh.plan_node_analytic(65536, "c64", 4, 2, 20, 8, 180 * 10**9, n_applies_per_task=1000)
+    assert b200["row_groups"][0]["feasible"] and b200["row_groups"][0]["waves"] == 3 and b200["chosen"]["p_row"] == 2
+    with pytest.raises(mfh.MfhError) as e:
+        mfh.plan_node_analytic(65536, "c64", 4, 2, 20, 8, 2 * GiB, mode="full", B=4096)
+    assert e.value.code == mfh.MFH_ERR_OUT_OF_MEMORY
+    with pytest.raises(mfh.MfhError) as e:
+        mfh.plan_node_analytic(65536, "c64", 4, 0, 20, 8, 40 * GiB)
+    assert e.value.code == mfh.MFH_ERR_INVALID_ARG
+
+
+def test_task_waves_cover_every_task_once():
+    from paper_2606_31598_b200.distributed import my_tasks, row_groups, task_waves
+    for n_tasks, C in [(20, 4), (20, 8), (7, 3), (1, 4), (16, 16)]:
+        waves = task_waves(n_tasks, C)
+        assert len(waves) == -(-n_tasks // C)
+        flat = [t for w in waves for (_, t) in w]
+        assert flat == list(range(n_tasks))
+        assert all(len({g for (g, _) in w}) == len(w) for w in waves)          # a group runs one task per wave
+        assert sorted(t for g in range(C) for t in my_tasks(n_tasks, g, C)) == list(range(n_tasks))
+    with pytest.raises(ValueError):
+        row_groups(8, 3)

@@ -66,3 +66,55 @@ def test_exchange_completes_phi_on_every_rank(world):
     for rank, p in enumerate(procs):
         out, _ = p.communicate(timeout=600)
         assert p.returncode == 0 and f"ok {rank}" in out, out
+
+
+HYBRID_WORKER = r"""
+import os, sys
+sys.path.insert(0, os.environ["MFH_ROOT"])
+import numpy as np, torch
+import torch.distributed as dist
+import oracle
+from paper_2606_31598_b200.distributed import exchange, make_group, my_tasks, slab
+from paper_2606_31598_b200.inputs import make_psi
+dist.init_process_group("gloo")
+rank, world = dist.get_rank(), dist.get_world_size()
+p_row, n_tasks = 2, 5                                   # 2 groups of 2 ranks, 5 coupling values -> 3 waves
+group, g, C = make_group(p_row)
+assert C == world // p_row and g == rank // p_row
+gr = dist.get_rank(group)
+D, B, seed = 256, 32, 8
+n_blk = D // B
+lams = np.linspace(0.0, 2.0, n_tasks)
+done = {}
+for t in my_tasks(n_tasks, g, C):                        # the group's tasks, wave by wave
+    psi = make_psi(D, 100 + t)
+    for scheme in ("rows", "pairs"):
+        part = lams[t] * oracle.apply_partition(D, B, seed, psi, gr, p_row, scheme)
+        lo, hi = slab(n_blk, gr, p_row) if scheme == "rows" else (0, n_blk)
+        phi = exchange(torch.from_numpy(part.copy()), scheme, (lo * B, (hi - lo) * B), group).numpy()
+        ref = lams[t] * oracle.apply(D, B, seed, psi)
+        assert np.linalg.norm(phi - ref) <= 1e-13 * max(np.linalg.norm(ref), 1e-300) + 1e-300, (t, scheme)
+    done[t] = True
+allt = [None] * world
+dist.all_gather_object(allt, sorted(done))
+assert sorted({t for lst in allt for t in lst}) == list(range(n_tasks))      # every task ran somewhere
+assert all(allt[r] == allt[r - r % p_row] for r in range(world))             # the ranks of a group ran the same tasks
+dist.barrier()
+dist.destroy_process_group()
+print("ok", rank)
+"""
+
+
+def test_hybrid_groups_and_task_waves_world_4():
+    """Parameter-parallel groups x row-parallel ranks: 4 ranks, row groups of 2, 5 tasks."""
+    port = _free_port()
+    world = 4
+    procs = []
+    for rank in range(world):
+        env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank),
+                   WORLD_SIZE=str(world), LOCAL_RANK=str(rank), MFH_ROOT=ROOT, OMP_NUM_THREADS="2")
+        procs.append(subprocess.Popen([sys.executable, "-c", HYBRID_WORKER], env=env, stdout=subprocess.PIPE,
+                                      stderr=subprocess.STDOUT, text=True))
+    for rank, p in enumerate(procs):
+        out, _ = p.communicate(timeout=600)
+        assert p.returncode == 0 and f"ok {rank}" in out, out
