@@ -259,6 +259,13 @@ MFH_API int mfh_debug_h0(mfh_handle h, void* h0_dev, void* stream);
 enum { MFH_MIX_C128_PAIR = 0, MFH_MIX_C64_ENTRY = 1, MFH_MIX_PHILOX = 2, MFH_MIX_DFMA31 = 3 };
 MFH_API int mfh_debug_pipe_rates(int32_t mix, double* units_per_s, void* stream);
 
+/* Read-only HBM stream probe: times a kernel that reads `bytes` of buf_dev once (8 independent 128-bit
+ * non-allocating loads per thread, grid = 8 CTAs per SM) and returns bytes per second (best of 3 after a
+ * warm-up).  The roofline denominator for kernels that read a cached matrix once; a device-to-device copy
+ * (MEASURED_PEAKS.json) also pays the write turn-around.  buf_dev: device, 16-byte aligned, >= 1 MiB and
+ * larger than L2 for an HBM figure.  Synchronises `stream`.  Errors: INVALID_ARG, CUDA. */
+MFH_API int mfh_debug_read_bandwidth(const void* buf_dev, size_t bytes, double* bytes_per_s, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

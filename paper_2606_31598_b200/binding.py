@@ -31,7 +31,7 @@ MODES = {"auto": MFH_MODE_AUTO, "procedural": MFH_MODE_PROCEDURAL, "partial": MF
 SYMBOLS = ["mfh_create", "mfh_plan_analytic", "mfh_plan_node_analytic", "mfh_plan", "mfh_apply", "mfh_apply_host", "mfh_apply_timed",
            "mfh_chebyshev", "mfh_chebyshev_imag", "mfh_chebyshev_steps", "mfh_lanczos_bounds", "mfh_destroy", "mfh_last_error", "mfh_get_plan", "mfh_debug_philox",
            "mfh_materialize_block", "mfh_debug_h0", "mfh_debug_pipe_rates", "mfh_sb_create", "mfh_sb_plan", "mfh_sb_apply",
-           "mfh_sb_destroy", "mfh_set_partition", "mfh_get_partition_rows", "mfh_set_exchange"]
+           "mfh_sb_destroy", "mfh_set_partition", "mfh_get_partition_rows", "mfh_set_exchange", "mfh_debug_read_bandwidth"]
 
 _lib = None
 
@@ -77,6 +77,7 @@ def lib():
     L.mfh_materialize_block.argtypes = [vp, i32, i32, vp, vp]
     L.mfh_debug_h0.argtypes = [vp, vp, vp]
     L.mfh_debug_pipe_rates.argtypes = [i32, ctypes.POINTER(dbl), vp]
+    L.mfh_debug_read_bandwidth.argtypes = [vp, sz, ctypes.POINTER(dbl), vp]
     L.mfh_sb_create.argtypes = [ctypes.POINTER(vp), i64, i32, i32, u64, u64, i32, vp, vp, dbl]
     L.mfh_sb_plan.argtypes = [vp, i32, i64, i64, vp, cp, sz]
     L.mfh_sb_apply.argtypes = [vp, vp, vp, vp]
@@ -325,4 +326,11 @@ def pipe_rate(mix: str) -> float:
     """Units per second of the synthetic instruction-mix kernel (mfh_debug_pipe_rates)."""
     out = ctypes.c_double(0.0)
     _check(lib().mfh_debug_pipe_rates(MIXES[mix], ctypes.byref(out), _stream()))
+    return float(out.value)
+
+
+def read_bandwidth(buf) -> float:
+    """Bytes per second of a read-only stream over a device tensor (mfh_debug_read_bandwidth)."""
+    out = ctypes.c_double(0.0)
+    _check(lib().mfh_debug_read_bandwidth(buf.data_ptr(), buf.numel() * buf.element_size(), ctypes.byref(out), _stream()))
     return float(out.value)

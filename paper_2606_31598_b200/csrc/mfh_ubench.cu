@@ -97,9 +97,71 @@ static int run_mix(int sm_count, cudaStream_t st, double* units_per_s)
     return MFH_OK;
 }
 
+// Read-only HBM stream: every thread keeps 8 independent 128-bit non-allocating loads in flight over a
+// grid-strided sweep of the buffer and xor-folds the words; one word per thread is written at the end.
+// The denominator for kernels that READ a matrix once (a device-to-device copy, the MEASURED_PEAKS.json
+// figure, also pays the write turn-around).
+__global__ void __launch_bounds__(256) read_stream_kernel(const uint4* __restrict__ buf, size_t n16, uint32_t* out)
+{
+    uint32_t acc = 0;
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    for (; i + 7 * stride < n16; i += 8 * stride) {
+        uint4 v[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+            asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
+                         : "=r"(v[u].x), "=r"(v[u].y), "=r"(v[u].z), "=r"(v[u].w)
+                         : "l"(buf + i + u * stride));
+#pragma unroll
+        for (int u = 0; u < 8; ++u) acc ^= v[u].x ^ v[u].y ^ v[u].z ^ v[u].w;
+    }
+    for (; i < n16; i += stride) {
+        const uint4 v = buf[i];
+        acc ^= v.x ^ v.y ^ v.z ^ v.w;
+    }
+    out[blockIdx.x * blockDim.x + threadIdx.x] = acc;
+}
+
 }  // namespace mfh
 
 using namespace mfh;
+
+extern "C" MFH_API int mfh_debug_read_bandwidth(const void* buf_dev, size_t bytes, double* bytes_per_s, void* stream)
+{
+    if (!buf_dev || !bytes_per_s || bytes < (1u << 20) || ((uintptr_t)buf_dev & 15)) {
+        set_error("mfh_debug_read_bandwidth: need a 16-byte aligned device buffer of at least 1 MiB");
+        return MFH_ERR_INVALID_ARG;
+    }
+    int dev = 0, sms = 0;
+    MFH_CUDA_CHECK(cudaGetDevice(&dev));
+    MFH_CUDA_CHECK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    cudaStream_t st = (cudaStream_t)stream;
+    const int grid = sms * 8;
+    uint32_t* out = nullptr;
+    MFH_CUDA_CHECK(cudaMalloc(&out, (size_t)grid * 256 * sizeof(uint32_t)));
+    cudaEvent_t e0, e1;
+    MFH_CUDA_CHECK(cudaEventCreate(&e0));
+    MFH_CUDA_CHECK(cudaEventCreate(&e1));
+    float best = 1e30f;
+    cudaError_t e = cudaSuccess;
+    for (int rep = 0; rep < 4 && e == cudaSuccess; ++rep) {   // first repetition warms up
+        cudaEventRecord(e0, st);
+        read_stream_kernel<<<grid, 256, 0, st>>>((const uint4*)buf_dev, bytes / 16, out);
+        cudaEventRecord(e1, st);
+        e = cudaEventSynchronize(e1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (rep > 0) best = std::min(best, ms);
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(out);
+    MFH_CUDA_CHECK(e);
+    MFH_CUDA_CHECK(cudaGetLastError());
+    *bytes_per_s = (double)(bytes / 16 * 16) / ((double)best * 1e-3);
+    return MFH_OK;
+}
 
 extern "C" MFH_API int mfh_debug_pipe_rates(int32_t mix, double* units_per_s, void* stream)
 {

@@ -300,3 +300,13 @@ def test_apply_host_roundtrip():
     out = torch.empty_like(ph).pin_memory()
     h.apply_host(ph, out)
     assert rel_l2(out.numpy(), oracle.apply(D, B, 3, psi)) <= TOL["c128"]
+
+
+def test_read_only_stream_probe_reports_a_plausible_hbm_rate():
+    import torch
+    buf = torch.ones(2 * 2**30, dtype=torch.uint8, device="cuda")       # 2 GiB, far above the 126 MB L2
+    gbs = mfh.read_bandwidth(buf) / 1e9
+    assert 3000.0 < gbs < 8200.0                                       # B200 HBM3e: ~8 TB/s nominal
+    with pytest.raises(mfh.MfhError) as e:
+        mfh.read_bandwidth(buf[:1024])
+    assert e.value.code == mfh.MFH_ERR_INVALID_ARG
