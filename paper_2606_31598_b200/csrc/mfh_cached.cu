@@ -176,6 +176,12 @@ __global__ void __launch_bounds__(32 * CACHED_WARPS) cached_kernel_c64(const Cac
 // broadcasts.  Output: the partial slot of column block m, as the other k-vector kernels.
 // --------------------------------------------------------------------------------------------
 constexpr int CM_ROWS = 128, CM_COLS = 16, CM_PAD = CM_COLS + 1;
+#ifndef MFH_CM_VS16
+#define MFH_CM_VS16 2
+#endif
+#ifndef MFH_CM_VS8
+#define MFH_CM_VS8 1
+#endif
 
 struct CachedMultiParams {
     int32_t B, n_blk, k, slot_multi;
@@ -192,14 +198,17 @@ __device__ __forceinline__ void cp_async16(void* dst_smem, const void* src)
                  : "memory");
 }
 
-template <int KT>
-__global__ void __launch_bounds__(CM_ROWS) cached_multi_kernel_c128(const CachedMultiParams P)
+// VS = threads per row: each handles KT / VS of the vectors (k = 16 runs two threads per row, which halves the
+// accumulator registers per thread and doubles the warps that hide the DFMA and shared-memory latencies).
+template <int KT, int VS>
+__global__ void __launch_bounds__(CM_ROWS * VS) cached_multi_kernel_c128(const CachedMultiParams P)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int TILE = CM_ROWS * CM_PAD;               // entries per stage (padded)
+    constexpr int NT = CM_ROWS * VS, KV = KT / VS;
     double2* tiles = reinterpret_cast<double2*>(smem_raw);             // [2][128][17]
     double2* psis = tiles + 2 * TILE;                                  // [2][16][KT]
-    const int t = threadIdx.x, m = blockIdx.y, k = P.k;
+    const int t = threadIdx.x, row = t & (CM_ROWS - 1), v0 = (t / CM_ROWS) * KV, m = blockIdx.y, k = P.k;
     const int64_t i_base = (int64_t)blockIdx.x * CM_ROWS;
     const int n = (int)(i_base / P.B);
     const int32_t slot = P.cache_slot[n * P.n_blk + m];
@@ -209,25 +218,25 @@ __global__ void __launch_bounds__(CM_ROWS) cached_multi_kernel_c128(const Cached
     const int n_chunks = P.B / CM_COLS;
 
     auto issue = [&](int ch, int st) {
-        // 128 rows x 16 entries: thread t copies entry (t & 15) of rows (t >> 4) + 8 j
+        // 128 rows x 16 entries: thread t copies entry (t & 15) of rows (t >> 4) + (NT / 16) j
         double2* dst = tiles + st * TILE;
         const double2* src = blk + (size_t)ch * CM_COLS + (t & 15);
 #pragma unroll
-        for (int j = 0; j < CM_ROWS / 8; ++j) {
-            const int r = (t >> 4) + 8 * j;
+        for (int j = 0; j < CM_ROWS * 16 / NT; ++j) {
+            const int r = (t >> 4) + (NT / 16) * j;
             cp_async16(dst + r * CM_PAD + (t & 15), src + (size_t)r * P.B);
         }
         // psi rows of the chunk: 16 x k entries, contiguous in [D][k]
         const double2* ps = psim + (size_t)ch * CM_COLS * k;
-        for (int e = t; e < CM_COLS * k; e += CM_ROWS) cp_async16(psis + st * CM_COLS * KT + (e / k) * KT + (e % k), ps + e);
+        for (int e = t; e < CM_COLS * k; e += NT) cp_async16(psis + st * CM_COLS * KT + (e / k) * KT + (e % k), ps + e);
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
 
-    double2 acc[KT];
+    double2 acc[KV];
 #pragma unroll
-    for (int v = 0; v < KT; ++v) acc[v] = double2{0.0, 0.0};
+    for (int v = 0; v < KV; ++v) acc[v] = double2{0.0, 0.0};
     if (k < KT)   // unused vector slots of the staged psi rows stay zero
-        for (int e = t; e < 2 * CM_COLS * KT; e += CM_ROWS) psis[e] = double2{0.0, 0.0};
+        for (int e = t; e < 2 * CM_COLS * KT; e += NT) psis[e] = double2{0.0, 0.0};
     __syncthreads();
     issue(0, 0);
     for (int ch = 0; ch < n_chunks; ++ch) {
@@ -239,13 +248,13 @@ __global__ void __launch_bounds__(CM_ROWS) cached_multi_kernel_c128(const Cached
             asm volatile("cp.async.wait_group 0;" ::: "memory");
         }
         __syncthreads();
-        const double2* row = tiles + st * TILE + t * CM_PAD;
-        const double2* pc = psis + st * CM_COLS * KT;
+        const double2* rowp = tiles + st * TILE + row * CM_PAD;
+        const double2* pc = psis + st * CM_COLS * KT + v0;
 #pragma unroll 4
         for (int c = 0; c < CM_COLS; ++c) {
-            const double2 hv = row[c];
+            const double2 hv = rowp[c];
 #pragma unroll
-            for (int v = 0; v < KT; ++v) {
+            for (int v = 0; v < KV; ++v) {
                 const double2 p = pc[c * KT + v];
                 acc[v].x = fma(hv.x, p.x, acc[v].x);
                 acc[v].x = fma(-hv.y, p.y, acc[v].x);
@@ -255,27 +264,27 @@ __global__ void __launch_bounds__(CM_ROWS) cached_multi_kernel_c128(const Cached
         }
         __syncthreads();   // the stage is free for the copy issued in the next iteration
     }
-    double2* dst = P.work + ((size_t)(P.slot_multi + m) * P.D + i_base + t) * k;
+    double2* dst = P.work + ((size_t)(P.slot_multi + m) * P.D + i_base + row) * k + v0;
 #pragma unroll
-    for (int v = 0; v < KT; ++v)
-        if (v < k) dst[v] = acc[v];
+    for (int v = 0; v < KV; ++v)
+        if (v0 + v < k) dst[v] = acc[v];
 }
 
 bool cached_multi_c128_supported(int dtype, int k, int B) { return dtype == MFH_C128 && k > 1 && k <= MFH_MAX_K && B % CM_ROWS == 0; }
 
-template <int KT> static int launch_cached_multi_c128_t(mfh_handle h, const void* psi, cudaStream_t st)
+template <int KT, int VS> static int launch_cached_multi_c128_t(mfh_handle h, const void* psi, cudaStream_t st)
 {
     const Plan& p = h->plan;
     CachedMultiParams P{p.B, p.n_blk, p.k, p.slot_multi, h->D, h->d_cache_slot, (const double2*)h->d_cache,
                         (const double2*)psi, (double2*)h->d_work};
     const size_t smem = (size_t)(2 * CM_ROWS * CM_PAD + 2 * CM_COLS * KT) * sizeof(double2);
-    auto kern = cached_multi_kernel_c128<KT>;
+    auto kern = cached_multi_kernel_c128<KT, VS>;
     static bool attr_done = false;
     if (!attr_done) {
         MFH_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_done = true;
     }
-    kern<<<dim3((unsigned)(h->D / CM_ROWS), p.n_blk), CM_ROWS, smem, st>>>(P);
+    kern<<<dim3((unsigned)(h->D / CM_ROWS), p.n_blk), CM_ROWS * VS, smem, st>>>(P);
     MFH_CUDA_CHECK(cudaGetLastError());
     return MFH_OK;
 }
@@ -283,10 +292,10 @@ template <int KT> static int launch_cached_multi_c128_t(mfh_handle h, const void
 static int launch_cached_multi_c128(mfh_handle h, const void* psi, cudaStream_t st)
 {
     const int k = h->plan.k;
-    if (k <= 2) return launch_cached_multi_c128_t<2>(h, psi, st);
-    if (k <= 4) return launch_cached_multi_c128_t<4>(h, psi, st);
-    if (k <= 8) return launch_cached_multi_c128_t<8>(h, psi, st);
-    return launch_cached_multi_c128_t<16>(h, psi, st);
+    if (k <= 2) return launch_cached_multi_c128_t<2, 1>(h, psi, st);
+    if (k <= 4) return launch_cached_multi_c128_t<4, 1>(h, psi, st);
+    if (k <= 8) return launch_cached_multi_c128_t<8, MFH_CM_VS8>(h, psi, st);
+    return launch_cached_multi_c128_t<16, MFH_CM_VS16>(h, psi, st);
 }
 
 int launch_cached(mfh_handle h, const void* psi, cudaStream_t st)
