@@ -356,6 +356,30 @@ def measure_graph_replay(torch, mfh, name: str = "C1", n: int = 50) -> dict:
             "chebyshev": {"t": 50.0, "terms": K, "ms_eager": cheb_eager_ms, "ms_graph": cheb_graph_ms}}
 
 
+def measure_auto_planner(torch, mfh) -> dict:
+    """a-6 end to end: mfh_plan(AUTO, B = 0, measure = 1) (Algorithm 2: the K_bench <= 8 best analytic candidates timed
+    on the device, argmin of n_applies x measured time + fill) on the operators of C2 (100 applies), C5 (151 applies
+    inside 150 GB) and C3 (100 scans): which plan it commits, its measured apply time and how long planning took."""
+    out = {}
+    for name, n_applies in (("C2", 100), ("C5", 151), ("C3", 100)):
+        cfg = ALL[name]
+        kind = "diag_plus_gue" if "seed_h0" in cfg else "gue"
+        h = mfh.Hamiltonian(cfg["D"], 0, cfg["seed"], cfg["dtype"], kind=kind, seed_h0=cfg.get("seed_h0", 0))
+        t0 = time.perf_counter()
+        rec = h.plan("auto", k=cfg["k"], n_applies_hint=n_applies, hbm_budget_bytes=int(cfg.get("hbm_budget", 0)), measure=True)
+        torch.cuda.synchronize()
+        c = rec["chosen"]
+        out[name] = {"operator": f"D={cfg['D']} {cfg['dtype']} k={cfg['k']}", "n_applies_hint": n_applies,
+                     "chosen": {kk: c[kk] for kk in ("mode", "B", "cache_bytes", "cached_fraction")},
+                     "measured_ms_per_apply": c["measured_apply_s"] * 1e3, "model_ms_per_apply": c["model_apply_s"] * 1e3,
+                     "matrix_entries_per_s": cfg["D"] ** 2 / c["measured_apply_s"],
+                     "candidates_timed": sum(1 for x in rec["candidates"] if x["measured_apply_s"] > 0),
+                     "plan_seconds": time.perf_counter() - t0}
+        h.destroy()
+        torch.cuda.empty_cache()
+    return out
+
+
 def roofline_for(res: dict, hbm_gbs: float, peak_src: str) -> dict:
     """Roofline of the dominant kernel of one apply."""
     cfg = res["cfg"]
@@ -583,6 +607,10 @@ def main():
             extras["SB18"] = measure_system_bath(torch, mfh, 10, hbm_gbs)
         except Exception as e:
             extras["SB18"] = {"error": str(e)}
+        try:
+            extras["planner-auto-measured"] = measure_auto_planner(torch, mfh)
+        except Exception as e:
+            extras["planner-auto-measured"] = {"error": str(e)}
         try:
             extras["C1-graph"] = measure_graph_replay(torch, mfh)
         except Exception as e:
