@@ -496,13 +496,16 @@ __global__ void __launch_bounds__(CT_THREADS, 2) cached_multi_tc_kernel(const Ct
 #pragma unroll
             for (int gg = 0; gg < 4; ++gg) {
                 const int g = gsel + 2 * gg;
-                float h0, l0, h1, l1, h2, l2, h3, l3;
-                split_tf32(raw[gg].x, h0, l0);
-                split_tf32(raw[gg].y, h1, l1);
-                split_tf32(raw[gg].z, h2, l2);
-                split_tf32(raw[gg].w, h3, l3);
+                // A_hi = the raw words (the tensor core reads only the TF32 part, i.e. truncates), A_lo = x - trunc(x),
+                // exact: one instruction per value less than rounding hi to nearest.  The truncation of hi is undone
+                // by lo; what remains one-sided is the tensor core's truncation of lo itself (2^-21 of x) and the
+                // dropped lo x lo term, far below the fp32 accumulation error that dominates (1e-5).
+                const float l0 = raw[gg].x - __uint_as_float(__float_as_uint(raw[gg].x) & 0xffffe000u);
+                const float l1 = raw[gg].y - __uint_as_float(__float_as_uint(raw[gg].y) & 0xffffe000u);
+                const float l2 = raw[gg].z - __uint_as_float(__float_as_uint(raw[gg].z) & 0xffffe000u);
+                const float l3 = raw[gg].w - __uint_as_float(__float_as_uint(raw[gg].w) & 0xffffe000u);
                 const uint32_t ta = a_lane + (uint32_t)(TC_ACC_COLS + ts * CT_A_STAGE_COLS + 4 * g);
-                tmem_st4(ta, h0, h1, h2, h3);
+                tmem_st4(ta, raw[gg].x, raw[gg].y, raw[gg].z, raw[gg].w);
                 tmem_st4(ta + CT_KF, l0, l1, l2, l3);
             }
             // every lane has consumed its shared-memory words (the splits depend on them): only now may
