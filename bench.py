@@ -442,7 +442,7 @@ def roofline_for(res: dict, hbm_gbs: float, peak_src: str) -> dict:
 # ALU ceilings.  (1) Measured: the library's synthetic instruction-mix kernel.
 # (2) Nominal: every SM issues at most 4 warp instructions per clock; instructions per matrix entry
 # counted in the SASS of the inner loops (cuobjdump): the two-sided c128 loop spends 88 per generated
-# pair = 44 per entry, the c64 tensor-core loop 62 per entry.
+# pair = 44 per entry, the c64 tensor-core loop 60 per entry.
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full captures
 # (profiles/r01_*_ncu_full*.md), keyed by (kernel, D).
 NCU_TRAFFIC = {("cached_kernel", 65536): 68.724718e9 + 4.461824e6,
@@ -450,7 +450,7 @@ NCU_TRAFFIC = {("cached_kernel", 65536): 68.724718e9 + 4.461824e6,
                ("cached_pairs_kernel", 65536): 35.438780e9 + 249.902592e6,
                ("cached_multi_tc_kernel", 32768): 8.596603e9 + 134.462720e6}
 ISSUE_LANES_PER_S = 148 * 4 * 32 * 1.965e9
-INSTR_PER_ENTRY = {("c128", "k1"): 44.0, ("c128", "kN"): 150.0, ("c64", "k1"): 40.0, ("c64", "kN"): 62.0}
+INSTR_PER_ENTRY = {("c128", "k1"): 44.0, ("c128", "kN"): 150.0, ("c64", "k1"): 40.0, ("c64", "kN"): 60.0}
 MIX_OF = {("c128", "k1"): ("c128_pair", 2), ("c64", "kN"): ("c64_entry", 1)}
 
 

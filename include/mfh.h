@@ -252,7 +252,7 @@ MFH_API int mfh_debug_h0(mfh_handle h, void* h0_dev, void* stream);
  *   MFH_MIX_C128_PAIR   14 32x32->64 multiplies + 26 ALU ops + 32 DFMA: one generated complex128 pair
  *                       {i,j} used for both phi_i and phi_j (2 matrix entries); of the 18 multiplies of a
  *                       Philox4x32-10 call the fused kernel shares 4 between the rows of a lane
- *   MFH_MIX_C64_ENTRY   14 multiplies + 22 ALU ops + 4 SFU ops + 11 FP32 ops: one generated complex64
+ *   MFH_MIX_C64_ENTRY   14 multiplies + 20 ALU ops + 4 SFU ops + 11 FP32 ops: one generated complex64
  *                       entry whose multiply-accumulate runs on the tensor cores
  *   MFH_MIX_PHILOX      one full Philox call (18 multiplies, 18 xors);   MFH_MIX_DFMA31  the 32 FP64 operations alone
  * Synchronises `stream`.  Errors: INVALID_ARG, CUDA. */

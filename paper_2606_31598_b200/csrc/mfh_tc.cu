@@ -196,8 +196,11 @@ __device__ __forceinline__ void tc_generate(const TcParams& P, unsigned char* sm
                 if (REL > 0) entry_upper<float>(P.G, nullptr, i, j, hr, hi);
                 else if (REL < 0) entry_lower<float>(P.G, nullptr, i, j, hr, hi);
                 else entry_any<float>(P.G, nullptr, i, j, hr, hi);
-                split_tf32(hr, rh[gg][e], rl[gg][e]);
-                split_tf32(hi, ih[gg][e], il[gg][e]);
+                // A_hi = the value itself (the tensor core reads its TF32 part), A_lo = x - trunc(x), exact
+                rh[gg][e] = hr;
+                rl[gg][e] = hr - __uint_as_float(__float_as_uint(hr) & 0xffffe000u);
+                ih[gg][e] = hi;
+                il[gg][e] = hi - __uint_as_float(__float_as_uint(hi) & 0xffffe000u);
             }
         float prh, prl, pih, pil;
         split_tf32(x.x, prh, prl);

@@ -177,7 +177,7 @@ extern "C" MFH_API int mfh_debug_pipe_rates(int32_t mix, double* units_per_s, vo
     switch (mix) {
     // counts per unit from the SASS of the inner loops
     case MFH_MIX_C128_PAIR: return run_mix<14, 12, 32, 0, 0>(sms, st, units_per_s);
-    case MFH_MIX_C64_ENTRY: return run_mix<14, 8, 0, 4, 11>(sms, st, units_per_s);
+    case MFH_MIX_C64_ENTRY: return run_mix<14, 6, 0, 4, 11>(sms, st, units_per_s);
     case MFH_MIX_PHILOX: return run_mix<18, 0, 0, 0, 0>(sms, st, units_per_s);
     case MFH_MIX_DFMA31: return run_mix<0, 0, 32, 0, 0>(sms, st, units_per_s);
     }
