@@ -169,3 +169,58 @@ def test_chebyshev_shifted_asymmetric_bounds():
     ref, K_ref = oracle.chebyshev_propagate(lambda v: H @ v, psi, 7.5, -2.2, 2.6, 1e-13)
     assert K == K_ref
     assert rel_l2(out.cpu().numpy(), ref) <= 1e-11
+
+
+def test_c3_scan_from_cached_blocks_sampled_rows():
+    """C3's operator cached (8.6 GB complex64 -> tensor-core kernel; 17.2 GB complex128 -> FP64 kernel)."""
+    c = CONFIGS["C3"]
+    D, B, k = c["D"], c["B"], c["k"]
+    lam = lambda_grid(k)
+    rows = sample_rows(D, 200)
+    for dtype, tol in (("c64", 1e-4), ("c128", 1e-11)):
+        Psi = make_psi(D, c["psi_seed"], k=k, dtype=dtype)
+        h = mfh.Hamiltonian(D, B, c["seed"], dtype, kind="diag_plus_gue", seed_h0=c["seed_h0"])
+        plan = h.plan("full", k=k)
+        assert plan["chosen"]["cache_bytes"] == D * D * (8 if dtype == "c64" else 16)
+        Phi = h.apply(to_dev(Psi), lambdas=lam).cpu().numpy()
+        ref = oracle.apply_scan(D, B, c["seed"], c["seed_h0"], lam, Psi, rows=rows)
+        for v in range(k):
+            assert rel_l2(Phi[rows, v], ref[:, v]) <= tol, (dtype, v)
+        h.destroy()
+
+
+def test_c4_partitioned_over_8_ranks():
+    """NEXT-4 at C4's size, one rank after the other on this GPU: the eight pair-set contributions add up to the
+    single-GPU apply (partition invariance, "does not change the Hamiltonian or omit any block
+    products"), and a row-slab rank reproduces its rows of the oracle and leaves the others untouched."""
+    import torch
+    c = CONFIGS["C4"]
+    D, B = c["D"], c["B"]
+    psi_np = make_psi(D, c["psi_seed"])
+    psi = to_dev(psi_np)
+    h = mfh.Hamiltonian(D, B, c["seed"], "c128")
+    h.plan("procedural")
+    full = h.apply(psi).clone()
+    h.destroy()
+    total = torch.zeros_like(full)
+    for r in range(8):
+        hr = mfh.Hamiltonian(D, B, c["seed"], "c128")
+        hr.set_partition(r, 8, "pairs")
+        hr.plan("procedural")
+        total += hr.apply(psi)
+        hr.destroy()
+    assert float(torch.linalg.vector_norm(total - full) / torch.linalg.vector_norm(full)) <= 1e-13
+    hr = mfh.Hamiltonian(D, B, c["seed"], "c128")
+    hr.set_partition(5, 8, "rows")
+    hr.plan("procedural")
+    lo, cnt = hr.partition_rows()
+    assert (lo, cnt) == (5 * D // 8, D // 8)
+    phi = torch.full_like(full, 3.0 - 4.0j)
+    hr.apply(psi, phi)
+    got = phi.cpu().numpy()
+    rows = lo + sample_rows(cnt, 60)
+    ref = oracle.apply(D, B, c["seed"], psi_np, rows=rows)
+    assert rel_l2(got[rows], ref) <= 1e-11
+    assert np.all(got[:lo] == 3.0 - 4.0j) and np.all(got[lo + cnt:] == 3.0 - 4.0j)
+    assert rel_l2(got[lo:lo + cnt], full.cpu().numpy()[lo:lo + cnt]) <= 1e-13
+    hr.destroy()
