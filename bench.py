@@ -554,8 +554,12 @@ def main():
     if args.partition != "none":
         if dist is None:   # one GPU: a single-rank group, so that the same code path runs (and is tested) here
             import torch.distributed as dist
+            import socket
+            with socket.socket() as sk:   # any free port: nothing else joins this group
+                sk.bind(("127.0.0.1", 0))
+                port = sk.getsockname()[1]
             os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-            os.environ.setdefault("MASTER_PORT", "29617")
+            os.environ.setdefault("MASTER_PORT", str(port))
             dist.init_process_group("nccl", rank=0, world_size=1, device_id=torch.device("cuda", local))
         run_partitioned(torch, dist, args, rank, world, local)
         return
