@@ -395,6 +395,13 @@ int enumerate_candidates(int64_t D, int dtype, int k, int mode, int B_req, int64
             int c = (int)std::floor(room * std::max(part.world, 1) / ((double)B * B * cb * N));   // a rank stores ~c N / world blocks
             c = largest_fitting(std::min(c, N - 1), [&](int cc) { return fits(cc, false); });
             if (c > 0) cs.push_back({c, false});
+            // The overlapped kernel (complex128, one vector) shares every SM between the cached and the generated
+            // part, and "as much as fits" is not its optimum (C5: 146 GB cached 31.4 ms, 100 GB 29.1 ms): two
+            // smaller caches are offered as well; the analytic model (Eq. 32, a sum) ranks them below the largest,
+            // the measured pass (Algorithm 2) decides.
+            if (dtype == MFH_C128 && k == 1)
+                for (int cc : {(3 * c) / 4, (3 * c) / 5})
+                    if (cc > 0 && cc < c) cs.push_back({cc, false});
         }
         for (auto [c, pairs] : cs) {
             Candidate cand = evaluate_candidate(D, dtype, k, B, c, pairs, n_applies, sm_count, part);
