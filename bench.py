@@ -164,10 +164,8 @@ def workload_config(name: str, cfg: dict) -> dict:
 def make_handle(mfh, cfg: dict, n_applies: int):
     kind = "diag_plus_gue" if "seed_h0" in cfg else "gue"
     h = mfh.Hamiltonian(cfg["D"], cfg["B"], cfg["seed"], cfg["dtype"], kind=kind, seed_h0=cfg.get("seed_h0", 0))
-    # partial mode: the measured planner (Algorithm 2) picks the cached fraction inside the budget -- for the
-    # overlapped kernel "as much as fits" is not the fastest; the other modes leave nothing to choose
     plan = h.plan(cfg["mode"], k=cfg["k"], n_applies_hint=n_applies,
-                  hbm_budget_bytes=int(cfg.get("hbm_budget", 0)), measure=(cfg["mode"] == "partial"))
+                  hbm_budget_bytes=int(cfg.get("hbm_budget", 0)))
     return h, plan
 
 
