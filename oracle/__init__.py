@@ -170,3 +170,4 @@ from .chebyshev import (bessel_i_scaled_table, bessel_j_table, chebyshev_imag_n_
 from .lanczos import lanczos_bounds, lanczos_tridiagonal, ritz_extremes  # noqa: E402,F401
 from .system_bath import sb_apply  # noqa: E402,F401
 from .partition import apply_partition, combine as combine_partition, owned_blocks  # noqa: E402,F401
+from .analytic import analytic_apply, analytic_matrix, theta_array  # noqa: E402,F401
