@@ -50,7 +50,9 @@ enum { MFH_OK = 0, MFH_ERR_INVALID_ARG = 1, MFH_ERR_BAD_STATE = 2, MFH_ERR_OUT_O
        MFH_ERR_CUDA = 4, MFH_ERR_NOT_CONVERGED = 5, MFH_ERR_UNSUPPORTED = 6 };
 enum { MFH_C128 = 0, MFH_C64 = 1 };
 enum { MFH_SRC_GUE = 0,           /* H = lambda * V(seed)                          configs 1,2,4,5 */
-       MFH_SRC_DIAG_PLUS_GUE = 1  /* H_v = diag(h0(seed_h0)) + lambda_v * V(seed)  config 3        */ };
+       MFH_SRC_DIAG_PLUS_GUE = 1, /* H_v = diag(h0(seed_h0)) + lambda_v * V(seed)  config 3        */
+       MFH_SRC_ANALYTIC = 2       /* H = lambda * F(theta), entries from a formula (Eq. 9): see
+                                     mfh_set_source_params; seeds are ignored                       */ };
 enum { MFH_MODE_AUTO = 0, MFH_MODE_PROCEDURAL = 1, MFH_MODE_PARTIAL = 2, MFH_MODE_FULL = 3,
        /* Hermitian (canonical-pair) cache, Eq. 27: block (n,m), n <= m, is stored once
         * and used for phi^[n] += C psi^[m] and phi^[m] += C^dagger psi^[n]; as many pairs as the budget
@@ -72,6 +74,16 @@ enum { MFH_MODE_AUTO = 0, MFH_MODE_PROCEDURAL = 1, MFH_MODE_PARTIAL = 2, MFH_MOD
  * Errors: MFH_ERR_INVALID_ARG for any violated constraint or unknown enum. */
 MFH_API int mfh_create(mfh_handle* out, int64_t D, int32_t B, uint64_t seed, int32_t source_kind,
                        double lambda, int32_t dtype, uint64_t seed_h0);
+
+/* Parameters of the analytic source (MFH_SRC_ANALYTIC; Eq. 9 "H^[n,m]_ab = f(n, m, a, b; theta) ... computed
+ * when needed"; R22).  The paper names no f; this library provides one dense six-parameter family in
+ * GLOBAL indices (partition invariant): a chain with power-law hopping, a Peierls phase and a quasi-periodic potential,
+ *     H_ij = -t e^{+i phi} / (j - i)^alpha  (i < j),   H_ij = conj(H_ji)  (i > j),   H_ii = W cos(2 pi beta i + delta).
+ * theta_host: 6 doubles (t, alpha, phi, W, beta, delta), all finite, alpha >= 0.  Call before mfh_plan (drops a
+ * committed plan).  Every mode works (the cache is filled from the formula; the fused kernels evaluate it in
+ * registers); k-vector plans use the CUDA-core kernels.  Errors: INVALID_ARG (NULL, non-finite, alpha < 0, handle
+ * not created with MFH_SRC_ANALYTIC). */
+MFH_API int mfh_set_source_params(mfh_handle h, const double* theta_host);
 
 /* Analytic planner only (Algorithm 1; adaptive block size P:409-429; cache budget
  * Eq. 27).  Pure host arithmetic: needs no GPU, touches no handle.  Enumerates

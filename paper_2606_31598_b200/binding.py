@@ -17,7 +17,8 @@ MFH_OK = 0
 MFH_ERR_INVALID_ARG, MFH_ERR_BAD_STATE, MFH_ERR_OUT_OF_MEMORY = 1, 2, 3
 MFH_ERR_CUDA, MFH_ERR_NOT_CONVERGED, MFH_ERR_UNSUPPORTED = 4, 5, 6
 MFH_C128, MFH_C64 = 0, 1
-MFH_SRC_GUE, MFH_SRC_DIAG_PLUS_GUE = 0, 1
+MFH_SRC_GUE, MFH_SRC_DIAG_PLUS_GUE, MFH_SRC_ANALYTIC = 0, 1, 2
+SOURCES = {"gue": MFH_SRC_GUE, "diag_plus_gue": MFH_SRC_DIAG_PLUS_GUE, "analytic": MFH_SRC_ANALYTIC}
 MFH_MODE_AUTO, MFH_MODE_PROCEDURAL, MFH_MODE_PARTIAL, MFH_MODE_FULL, MFH_MODE_PAIRS = 0, 1, 2, 3, 4
 MFH_MAX_K = 16
 MFH_PART_NONE, MFH_PART_ROWS, MFH_PART_PAIRS = 0, 1, 2
@@ -31,7 +32,7 @@ MODES = {"auto": MFH_MODE_AUTO, "procedural": MFH_MODE_PROCEDURAL, "partial": MF
 SYMBOLS = ["mfh_create", "mfh_plan_analytic", "mfh_plan_node_analytic", "mfh_plan", "mfh_apply", "mfh_apply_host", "mfh_apply_timed",
            "mfh_chebyshev", "mfh_chebyshev_imag", "mfh_chebyshev_steps", "mfh_lanczos_bounds", "mfh_destroy", "mfh_last_error", "mfh_get_plan", "mfh_debug_philox",
            "mfh_materialize_block", "mfh_debug_h0", "mfh_debug_pipe_rates", "mfh_sb_create", "mfh_sb_plan", "mfh_sb_apply",
-           "mfh_sb_destroy", "mfh_set_partition", "mfh_get_partition_rows", "mfh_set_exchange", "mfh_debug_read_bandwidth"]
+           "mfh_sb_destroy", "mfh_set_partition", "mfh_get_partition_rows", "mfh_set_exchange", "mfh_debug_read_bandwidth", "mfh_set_source_params"]
 
 _lib = None
 
@@ -68,6 +69,7 @@ def lib():
                                      ctypes.POINTER(dbl), vp]
     L.mfh_set_partition.argtypes = [vp, i32, i32, i32]
     L.mfh_set_exchange.argtypes = [vp, vp, vp]
+    L.mfh_set_source_params.argtypes = [vp, ctypes.POINTER(dbl)]
     L.mfh_get_partition_rows.argtypes = [vp, ctypes.POINTER(i32), ctypes.POINTER(i32), ctypes.POINTER(i32)]
     L.mfh_destroy.argtypes = [vp]
     L.mfh_last_error.argtypes = []
@@ -137,8 +139,7 @@ class Hamiltonian:
                  lam: float = 1.0, seed_h0: int = 0):
         self.D, self.dtype, self.k = D, dtype, None
         self._h = ctypes.c_void_p()
-        src = MFH_SRC_GUE if kind == "gue" else MFH_SRC_DIAG_PLUS_GUE
-        _check(lib().mfh_create(ctypes.byref(self._h), D, B, seed, src, lam, DTYPES[dtype], seed_h0))
+        _check(lib().mfh_create(ctypes.byref(self._h), D, B, seed, SOURCES[kind], lam, DTYPES[dtype], seed_h0))
 
     # -- torch plumbing ---------------------------------------------------------------------
     def _torch_dtype(self):
@@ -157,6 +158,11 @@ class Hamiltonian:
                               1 if measure else 0, _stream(), buf, len(buf)))
         self.k = k
         return json.loads(buf.value.decode())
+
+    def set_source_params(self, theta):
+        """Parameters (t, alpha, phi, W, beta, delta) of the analytic source (kind="analytic"); call before plan."""
+        arr = (ctypes.c_double * 6)(*[float(x) for x in theta])
+        _check(lib().mfh_set_source_params(self._h, arr))
 
     def set_partition(self, rank: int, world: int, scheme: str = "pairs"):
         """Distributed execution: this handle computes rank `rank`'s share of phi (call before plan)."""

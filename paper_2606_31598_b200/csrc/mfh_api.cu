@@ -219,7 +219,7 @@ MFH_API int mfh_create(mfh_handle* out, int64_t D, int32_t B, uint64_t seed, int
                   MFH_MAX_B, (long long)D);
         return MFH_ERR_INVALID_ARG;
     }
-    if (source_kind != MFH_SRC_GUE && source_kind != MFH_SRC_DIAG_PLUS_GUE) {
+    if (source_kind != MFH_SRC_GUE && source_kind != MFH_SRC_DIAG_PLUS_GUE && source_kind != MFH_SRC_ANALYTIC) {
         set_error("mfh_create: unknown source kind %d", source_kind);
         return MFH_ERR_INVALID_ARG;
     }
@@ -246,6 +246,25 @@ MFH_API int mfh_destroy(mfh_handle h)
     free_plan_resources(h);
     if (h->d_gen_tab) cudaFree(h->d_gen_tab);
     delete h;
+    return MFH_OK;
+}
+
+MFH_API int mfh_set_source_params(mfh_handle h, const double* theta_host)
+{
+    if (!h || !theta_host) { set_error("mfh_set_source_params: NULL pointer"); return MFH_ERR_INVALID_ARG; }
+    if (h->kind != MFH_SRC_ANALYTIC) { set_error("mfh_set_source_params: handle is not MFH_SRC_ANALYTIC"); return MFH_ERR_INVALID_ARG; }
+    for (int q = 0; q < 6; ++q)
+        if (!std::isfinite(theta_host[q])) { set_error("mfh_set_source_params: theta[%d] is not finite", q); return MFH_ERR_INVALID_ARG; }
+    if (theta_host[1] < 0.0) { set_error("mfh_set_source_params: alpha must be >= 0"); return MFH_ERR_INVALID_ARG; }
+    free_plan_resources(h);
+    h->analytic.t = theta_host[0];
+    h->analytic.alpha = theta_host[1];
+    h->analytic.cphi = std::cos(theta_host[2]);
+    h->analytic.sphi = std::sin(theta_host[2]);
+    h->analytic.W = theta_host[3];
+    h->analytic.beta2pi = 6.283185307179586476925 * theta_host[4];
+    h->analytic.delta = theta_host[5];
+    h->analytic_set = true;
     return MFH_OK;
 }
 
@@ -325,6 +344,10 @@ MFH_API int mfh_plan(mfh_handle h, int32_t mode, int32_t k, int64_t n_applies_hi
     if (k < 1 || k > MFH_MAX_K || mode < MFH_MODE_AUTO || mode > MFH_MODE_PAIRS || hbm_budget_bytes < 0) {
         set_error("mfh_plan: invalid argument (k=%d, mode=%d)", k, mode);
         return MFH_ERR_INVALID_ARG;
+    }
+    if (h->kind == MFH_SRC_ANALYTIC && !h->analytic_set) {
+        set_error("mfh_plan: MFH_SRC_ANALYTIC needs mfh_set_source_params first");
+        return MFH_ERR_BAD_STATE;
     }
     cudaStream_t st = (cudaStream_t)stream;
     int dev = 0;

@@ -199,11 +199,34 @@ template <> struct Gen<float> {
     }
 };
 
+// Analytic source (Eq. 9; R22): H_ij = -t e^{+i phi} / (j - i)^alpha for i < j, its
+// conjugate for i > j, H_ii = W cos(2 pi beta i + delta).  cos/sin of phi and 2 pi beta are prepared on the host.
+struct AnalyticArgs {
+    double t, alpha, cphi, sphi, W, beta2pi, delta;
+};
+enum { SRC_SEEDED = 0, SRC_ANALYTIC = 1 };   // template parameter of the kernels that generate entries
+
 template <typename T> struct GenArgs {   // what a kernel needs to call the generator
     PhiloxKeys K;
     typename Gen<T>::Const gc;
     const typename Gen<T>::Tab* tab_global;   // device copy of the table (nullptr for float)
+    AnalyticArgs an;                          // SRC_ANALYTIC only
 };
+
+// Entry of the analytic source, evaluated in double (pow, cos) and rounded to T.
+template <typename T>
+__device__ __forceinline__ void analytic_entry(const AnalyticArgs& A, uint32_t i, uint32_t j, T& hr, T& hi)
+{
+    if (i == j) {
+        hr = (T)(A.W * cos(fma(A.beta2pi, (double)i, A.delta)));
+        hi = T(0);
+        return;
+    }
+    const double d = (double)(i < j ? j - i : i - j);
+    const double a = -A.t * pow(d, -A.alpha);
+    hr = (T)(a * A.cphi);
+    hi = (T)(i < j ? a * A.sphi : -(a * A.sphi));
+}
 
 // Copy the generator table to shared memory (all threads of the CTA; caller synchronises).
 template <typename T>
@@ -219,10 +242,14 @@ __device__ __forceinline__ const typename Gen<T>::Tab* stage_gen_table(const Gen
 
 // General entry H_ij for any (i,j): conjugate below the diagonal, real and scaled by 1/sqrt(D)
 // (= sqrt(2) s) on it.
-template <typename T>
+template <typename T, int SRC = SRC_SEEDED>
 __device__ __forceinline__ void entry_any(const GenArgs<T>& G, const typename Gen<T>::Tab* tab, uint32_t i,
                                           uint32_t j, T& hr, T& hi)
 {
+    if constexpr (SRC == SRC_ANALYTIC) {
+        analytic_entry<T>(G.an, i, j, hr, hi);
+        return;
+    }
     uint32_t x0, x1;
     pair_words(G.K, min(i, j), max(i, j), x0, x1);
     T a, b;
@@ -232,20 +259,28 @@ __device__ __forceinline__ void entry_any(const GenArgs<T>& G, const typename Ge
 }
 
 // Entry for a pair known to satisfy i < j (strictly upper triangle).
-template <typename T>
+template <typename T, int SRC = SRC_SEEDED>
 __device__ __forceinline__ void entry_upper(const GenArgs<T>& G, const typename Gen<T>::Tab* tab, uint32_t i,
                                             uint32_t j, T& hr, T& hi)
 {
+    if constexpr (SRC == SRC_ANALYTIC) {
+        analytic_entry<T>(G.an, i, j, hr, hi);
+        return;
+    }
     uint32_t x0, x1;
     pair_words(G.K, i, j, x0, x1);
     Gen<T>::normals(tab, G.gc, x0, x1, hr, hi);
 }
 
 // Entry for a pair known to satisfy i > j: conjugate of the (j,i) entry.
-template <typename T>
+template <typename T, int SRC = SRC_SEEDED>
 __device__ __forceinline__ void entry_lower(const GenArgs<T>& G, const typename Gen<T>::Tab* tab, uint32_t i,
                                             uint32_t j, T& hr, T& hi)
 {
+    if constexpr (SRC == SRC_ANALYTIC) {
+        analytic_entry<T>(G.an, i, j, hr, hi);
+        return;
+    }
     uint32_t x0, x1;
     pair_words(G.K, j, i, x0, x1);
     T b;

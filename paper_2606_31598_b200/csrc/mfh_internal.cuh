@@ -75,6 +75,8 @@ struct mfh_handle_s {
     uint64_t seed = 0, seed_h0 = 0;
     int32_t kind = 0, dtype = 0;
     double lambda = 1.0;
+    mfh::AnalyticArgs analytic = {0, 0, 1, 0, 0, 0, 0};          // mfh_set_source_params (MFH_SRC_ANALYTIC)
+    bool analytic_set = false;
     int32_t part_rank = 0, part_world = 1, part_scheme = 0;   // mfh_set_partition
     mfh_exchange_fn exchange = nullptr;                       // mfh_set_exchange
     void* exchange_user = nullptr;

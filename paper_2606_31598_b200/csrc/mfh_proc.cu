@@ -14,6 +14,7 @@ template <> GenArgs<double> make_gen_args<double>(mfh_handle h)
     G.K = make_philox_keys(h->seed);
     G.gc = h->gen_host.gc;
     G.tab_global = h->d_gen_tab;
+    G.an = h->analytic;
     return G;
 }
 template <> GenArgs<float> make_gen_args<float>(mfh_handle h)
@@ -22,6 +23,7 @@ template <> GenArgs<float> make_gen_args<float>(mfh_handle h)
     G.K = make_philox_keys(h->seed);
     G.gc.neg_k2_ln2 = (float)(-0.6931471805599453 / (double)h->D);
     G.tab_global = nullptr;
+    G.an = h->analytic;
     return G;
 }
 
@@ -56,7 +58,7 @@ int launch_philox_debug(uint64_t seed, uint32_t stream_id, const uint32_t* i, co
 // Block materialisation (test export) and cache fill: one dense B x B block per blockIdx.x,
 // rows strided over blockIdx.y, columns over the threads (coalesced 16-byte stores).
 // --------------------------------------------------------------------------------------------
-template <typename T>
+template <typename T, int SRC>
 __global__ void __launch_bounds__(256) fill_kernel(const GenArgs<T> G, int32_t B, int32_t n_blk,
                                                    const int32_t* __restrict__ cache_slot,
                                                    int32_t single_n, int32_t single_m, int32_t tiled,
@@ -84,7 +86,7 @@ __global__ void __launch_bounds__(256) fill_kernel(const GenArgs<T> G, int32_t B
         CT* row = out + base + (size_t)a * B;
         for (int32_t b = threadIdx.x; b < B; b += blockDim.x) {
             T hr, hi;
-            entry_any<T>(G, tab, i, (uint32_t)m * B + b, hr, hi);
+            entry_any<T, SRC>(G, tab, i, (uint32_t)m * B + b, hr, hi);
             CT v;
             v.x = hr;
             v.y = hi;
@@ -99,8 +101,12 @@ static int launch_fill_t(mfh_handle h, dim3 grid, int32_t B, int32_t n_blk, cons
                          int32_t n, int32_t m, int32_t tiled, void* out, cudaStream_t st)
 {
     using CT = typename Cplx<T>::type;
-    fill_kernel<T><<<grid, 256, Gen<T>::TAB_BYTES, st>>>(make_gen_args<T>(h), B, n_blk, cache_slot, n, m, tiled,
-                                                          (CT*)out);
+    if (h->kind == MFH_SRC_ANALYTIC)
+        fill_kernel<T, SRC_ANALYTIC><<<grid, 256, Gen<T>::TAB_BYTES, st>>>(make_gen_args<T>(h), B, n_blk, cache_slot, n, m,
+                                                                            tiled, (CT*)out);
+    else
+        fill_kernel<T, SRC_SEEDED><<<grid, 256, Gen<T>::TAB_BYTES, st>>>(make_gen_args<T>(h), B, n_blk, cache_slot, n, m,
+                                                                          tiled, (CT*)out);
     MFH_CUDA_CHECK(cudaGetLastError());
     return MFH_OK;
 }
@@ -186,7 +192,7 @@ template <typename T> struct ProcParams {
 };
 
 // The item loop of one CTA: runs until the device counter is exhausted.
-template <typename T, int R>
+template <typename T, int R, int SRC = SRC_SEEDED>
 __device__ __forceinline__ void proc_items(const ProcParams<T>& P, unsigned char* smem_raw)
 {
     using CT = typename Cplx<T>::type;
@@ -236,7 +242,7 @@ __device__ __forceinline__ void proc_items(const ProcParams<T>& P, unsigned char
 #pragma unroll
                         for (int r = 0; r < R; ++r) {
                             T hr, hi;
-                            entry_any<T>(P.G, tab, i0 + 32 * r, j0 + c, hr, hi);
+                            entry_any<T, SRC>(P.G, tab, i0 + 32 * r, j0 + c, hr, hi);
                             accr[r] = fma(hr, p.x, accr[r]);
                             accr[r] = fma(-hi, p.y, accr[r]);
                             acci[r] = fma(hr, p.y, acci[r]);
@@ -252,7 +258,7 @@ __device__ __forceinline__ void proc_items(const ProcParams<T>& P, unsigned char
 #pragma unroll
                         for (int r = 0; r < R; ++r) {
                             T hr, hi;
-                            entry_upper<T>(P.G, tab, i0 + 32 * r, j0 + c, hr, hi);
+                            entry_upper<T, SRC>(P.G, tab, i0 + 32 * r, j0 + c, hr, hi);
                             accr[r] = fma(hr, p.x, accr[r]);
                             accr[r] = fma(-hi, p.y, accr[r]);
                             acci[r] = fma(hr, p.y, acci[r]);
@@ -292,11 +298,11 @@ __device__ __forceinline__ void proc_items(const ProcParams<T>& P, unsigned char
     }
 }
 
-template <typename T, int R>
+template <typename T, int R, int SRC = SRC_SEEDED>
 __global__ void __launch_bounds__(PROC_THREADS, 2) proc_single_kernel(const ProcParams<T> P)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    proc_items<T, R>(P, smem_raw);
+    proc_items<T, R, SRC>(P, smem_raw);
 }
 
 // --------------------------------------------------------------------------------------------
@@ -423,12 +429,13 @@ static int launch_proc_single_t(mfh_handle h, const void* psi, cudaStream_t st)
         return (size_t)Gen<T>::TAB_BYTES + (size_t)(B + PROC_WARPS * 32 * R + PROC_WARPS * 32) * sizeof(CT);
     };
     const size_t smem = smem_for(p.B);
-    auto kern = proc_single_kernel<T, R>;
-    static bool attr_done = false;
-    if (!attr_done) {
+    const bool analytic = (h->kind == MFH_SRC_ANALYTIC);
+    auto kern = analytic ? proc_single_kernel<T, R, SRC_ANALYTIC> : proc_single_kernel<T, R, SRC_SEEDED>;
+    static bool attr_done[2] = {false, false};
+    if (!attr_done[analytic]) {
         MFH_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                             (int)smem_for(MFH_MAX_B)));
-        attr_done = true;
+        attr_done[analytic] = true;
     }
     int per_sm = 1;
     MFH_CUDA_CHECK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, PROC_THREADS, smem));
@@ -457,7 +464,7 @@ bool partial_overlap_supported(mfh_handle h)
 {
     const Plan& p = h->plan;
     static const bool off = getenv("MFH_PARTIAL_SEQUENTIAL") != nullptr;   // A/B measurements
-    return !off && h->dtype == MFH_C128 && p.k == 1 && !p.pairs && p.n_cached > 0 && !p.items.empty() &&
+    return !off && h->kind != MFH_SRC_ANALYTIC && h->dtype == MFH_C128 && p.k == 1 && !p.pairs && p.n_cached > 0 && !p.items.empty() &&
            h->D % STRIP_ROWS == 0 && p.B % STRIP_ROWS == 0;
 }
 
@@ -534,7 +541,7 @@ template <typename T> struct MultiParams {
     typename Cplx<T>::type* work;        // [n_slots][D][k]
 };
 
-template <typename T, int KT, int W>
+template <typename T, int KT, int W, int SRC = SRC_SEEDED>
 __global__ void __launch_bounds__(32 * W) proc_multi_kernel(const MultiParams<T> P)
 {
     using CT = typename Cplx<T>::type;
@@ -564,7 +571,7 @@ __global__ void __launch_bounds__(32 * W) proc_multi_kernel(const MultiParams<T>
 #pragma unroll 2
             for (int c = 0; c < CH; ++c) {
                 T hr, hi;
-                entry_any<T>(P.G, tab, i, j0 + c, hr, hi);
+                entry_any<T, SRC>(P.G, tab, i, j0 + c, hr, hi);
 #pragma unroll
                 for (int v = 0; v < KT; ++v) {
                     const CT p = psis[c][v];
@@ -599,10 +606,16 @@ static int launch_proc_multi_t(mfh_handle h, const void* psi, cudaStream_t st)
     P.work = (CT*)h->d_work;
     const size_t smem = (size_t)Gen<T>::TAB_BYTES + 32 * KT * sizeof(CT);
     // 32W rows per CTA must divide B; prefer 128-row CTAs, fall back to one warp.
-    if (p.B % 128 == 0)
-        proc_multi_kernel<T, KT, 4><<<dim3((unsigned)(h->D / 128), p.n_blk), 128, smem, st>>>(P);
-    else
-        proc_multi_kernel<T, KT, 1><<<dim3((unsigned)(h->D / 32), p.n_blk), 32, smem, st>>>(P);
+    const bool analytic = (h->kind == MFH_SRC_ANALYTIC);
+    if (p.B % 128 == 0) {
+        const dim3 grid((unsigned)(h->D / 128), p.n_blk);
+        if (analytic) proc_multi_kernel<T, KT, 4, SRC_ANALYTIC><<<grid, 128, smem, st>>>(P);
+        else proc_multi_kernel<T, KT, 4, SRC_SEEDED><<<grid, 128, smem, st>>>(P);
+    } else {
+        const dim3 grid((unsigned)(h->D / 32), p.n_blk);
+        if (analytic) proc_multi_kernel<T, KT, 1, SRC_ANALYTIC><<<grid, 32, smem, st>>>(P);
+        else proc_multi_kernel<T, KT, 1, SRC_SEEDED><<<grid, 32, smem, st>>>(P);
+    }
     MFH_CUDA_CHECK(cudaGetLastError());
     return MFH_OK;
 }

@@ -311,7 +311,8 @@ __global__ void __launch_bounds__(TC_THREADS, MFH_TC_MINB) proc_multi_tc_kernel(
 
 bool tc_multi_supported(mfh_handle h)
 {
-    return h->dtype == MFH_C64 && h->plan.k > 1 && h->plan.k <= 16 && h->plan.B % TC_TP == 0;
+    // seeded source only: the generator warps of this kernel are the Philox / SFU Box-Muller path
+    return h->kind != MFH_SRC_ANALYTIC && h->dtype == MFH_C64 && h->plan.k > 1 && h->plan.k <= 16 && h->plan.B % TC_TP == 0;
 }
 
 int launch_proc_multi_tc(mfh_handle h, const void* psi, cudaStream_t st)

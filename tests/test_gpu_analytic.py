@@ -1,0 +1,117 @@
+"""GPU parity of the analytic source (MFH_SRC_ANALYTIC; Eq. 9; R22): the same kernels,
+planner and cache modes with entries evaluated from a formula instead of the seeded generator, against
+oracle/analytic.py (the dense definition)."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2606_31598_b200 import binding as mfh
+from paper_2606_31598_b200.inputs import make_psi
+
+pytestmark = pytest.mark.gpu
+
+TH = dict(t=0.7, alpha=1.3, phi=0.4, W=1.1, beta=(np.sqrt(5.0) - 1.0) / 2.0, delta=0.25)
+TOL = {"c128": 1e-11, "c64": 1e-4}
+
+
+def to_dev(x):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def rel_l2(a, b):
+    return float(np.linalg.norm(np.asarray(a, dtype=np.complex128) - b) / np.linalg.norm(b))
+
+
+def handle(D, B, dtype, theta=TH, lam=1.0):
+    h = mfh.Hamiltonian(D, B, 0, dtype, kind="analytic", lam=lam)
+    h.set_source_params(oracle.theta_array(theta))
+    return h
+
+
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+@pytest.mark.parametrize("n,m", [(0, 0), (1, 3), (3, 1)])
+def test_materialized_block_matches_the_formula(dtype, n, m):
+    D, B = 1024, 256
+    h = handle(D, B, dtype)
+    blk = h.materialize_block(n, m, B).cpu().numpy().astype(np.complex128)
+    ref = oracle.analytic_matrix(D, TH, n * B, B, m * B, B)
+    assert np.abs(blk - ref).max() <= (1e-14 if dtype == "c128" else 2e-7) * np.abs(ref).max()
+    h.destroy()
+
+
+@pytest.mark.parametrize("dtype", ["c128", "c64"])
+@pytest.mark.parametrize("mode", ["procedural", "partial", "full", "pairs"])
+@pytest.mark.parametrize("k", [1, 4])
+def test_apply_in_every_mode_vs_oracle(dtype, mode, k):
+    if mode == "pairs" and k > 1:
+        pytest.skip("the pair cache serves one vector")
+    D, B = 2048, 256
+    Psi = make_psi(D, 41, k=k, dtype=dtype)
+    h = handle(D, B, dtype, lam=0.8)
+    cb = 16 if dtype == "c128" else 8
+    plan = h.plan(mode, k=k, hbm_budget_bytes=int(0.45 * D * D * cb) if mode == "partial" else 0)
+    assert plan["chosen"]["mode"] == mode
+    Phi = h.apply(to_dev(Psi)).cpu().numpy().reshape(D, k)
+    ref = 0.8 * oracle.analytic_apply(D, TH, Psi.reshape(D, k))
+    for v in range(k):
+        assert rel_l2(Phi[:, v], ref[:, v]) <= TOL[dtype], (plan["chosen"], v)
+    h.destroy()
+
+
+def test_closed_forms_on_the_gpu():
+    """alpha = 0: H = -t (J - I), H psi = -t (sum(psi) - psi); t = 0: the diagonal potential."""
+    D, B = 4096, 512
+    psi = make_psi(D, 43)
+    h = handle(D, B, "c128", dict(TH, alpha=0.0, phi=0.0, W=0.0))
+    h.plan("procedural")
+    phi = h.apply(to_dev(psi)).cpu().numpy()
+    ref = -0.7 * (psi.sum() - psi)
+    assert np.linalg.norm(phi - ref) <= 1e-12 * np.linalg.norm(ref)
+    h.set_source_params(oracle.theta_array(dict(TH, t=0.0)))       # drops the plan
+    h.plan("procedural")
+    phi = h.apply(to_dev(psi)).cpu().numpy()
+    pot = 1.1 * np.cos(2 * np.pi * TH["beta"] * np.arange(D) + 0.25)
+    assert np.linalg.norm(phi - pot * psi) <= 1e-13 * np.linalg.norm(psi)
+    h.destroy()
+
+
+def test_chebyshev_and_partition_on_the_analytic_source():
+    import torch
+    D, B = 1024, 128
+    th = dict(TH, alpha=2.0)
+    H = oracle.analytic_matrix(D, th)
+    w = np.linalg.eigvalsh(H)
+    psi = make_psi(D, 44)
+    h = handle(D, B, "c128", th)
+    h.plan("pairs")
+    out, K = h.chebyshev(to_dev(psi), 4.0, w[0] - 0.1, w[-1] + 0.1, 1e-13)
+    ev, U = np.linalg.eigh(H)
+    exact = U @ (np.exp(-1j * ev * 4.0) * (U.conj().T @ psi))
+    assert np.linalg.norm(out.cpu().numpy() - exact) <= 1e-11
+    h.destroy()
+    total = np.zeros(D, dtype=np.complex128)
+    for r in range(3):
+        hr = handle(D, B, "c128", th)
+        hr.set_partition(r, 3, "pairs")
+        hr.plan("procedural")
+        total += hr.apply(to_dev(psi), torch.zeros(D, dtype=torch.complex128, device="cuda")).cpu().numpy()
+        hr.destroy()
+    assert np.linalg.norm(total - H @ psi) <= 1e-11 * np.linalg.norm(H @ psi)
+
+
+def test_argument_errors():
+    h = mfh.Hamiltonian(1024, 128, 0, "c128", kind="analytic")
+    with pytest.raises(mfh.MfhError) as e:
+        h.plan("procedural")                                       # parameters not set
+    assert e.value.code == mfh.MFH_ERR_BAD_STATE
+    for bad in [(1, -0.5, 0, 0, 0, 0), (float("nan"), 1, 0, 0, 0, 0)]:
+        with pytest.raises(mfh.MfhError) as e:
+            h.set_source_params(bad)
+        assert e.value.code == mfh.MFH_ERR_INVALID_ARG
+    g = mfh.Hamiltonian(1024, 128, 1, "c128")
+    with pytest.raises(mfh.MfhError) as e:
+        g.set_source_params((1, 1, 0, 0, 0, 0))                    # not an analytic handle
+    assert e.value.code == mfh.MFH_ERR_INVALID_ARG
+    h.destroy()
+    g.destroy()
