@@ -51,8 +51,10 @@ enum { MFH_OK = 0, MFH_ERR_INVALID_ARG = 1, MFH_ERR_BAD_STATE = 2, MFH_ERR_OUT_O
 enum { MFH_C128 = 0, MFH_C64 = 1 };
 enum { MFH_SRC_GUE = 0,           /* H = lambda * V(seed)                          configs 1,2,4,5 */
        MFH_SRC_DIAG_PLUS_GUE = 1, /* H_v = diag(h0(seed_h0)) + lambda_v * V(seed)  config 3        */
-       MFH_SRC_ANALYTIC = 2       /* H = lambda * F(theta), entries from a formula (Eq. 9): see
-                                     mfh_set_source_params; seeds are ignored                       */ };
+       MFH_SRC_ANALYTIC = 2,      /* H = lambda * F(theta), entries from a formula (Eq. 9): see
+                                     mfh_set_source_params; seeds are ignored                       */
+       MFH_SRC_EXTERNAL = 3       /* H = lambda * (blocks supplied by the caller, Eq. 10): see
+                                     mfh_set_block; seeds are ignored                               */ };
 enum { MFH_MODE_AUTO = 0, MFH_MODE_PROCEDURAL = 1, MFH_MODE_PARTIAL = 2, MFH_MODE_FULL = 3,
        /* Hermitian (canonical-pair) cache, Eq. 27: block (n,m), n <= m, is stored once
         * and used for phi^[n] += C psi^[m] and phi^[m] += C^dagger psi^[n]; as many pairs as the budget
@@ -84,6 +86,20 @@ MFH_API int mfh_create(mfh_handle* out, int64_t D, int32_t B, uint64_t seed, int
  * registers); k-vector plans use the CUDA-core kernels.  Errors: INVALID_ARG (NULL, non-finite, alpha < 0, handle
  * not created with MFH_SRC_ANALYTIC). */
 MFH_API int mfh_set_source_params(mfh_handle h, const double* theta_host);
+
+/* Externally stored blocks (MFH_SRC_EXTERNAL; Eq. 10 "H^[n,m] = D[key(n,m)] ... the block is loaded or
+ * reconstructed only for the currently active part of the matrix-vector product").  Host memory reaches this GPU at
+ * ~40 GB/s against 7 TB/s from HBM, so an external block is loaded ONCE into the HBM cache and
+ * streamed from there: plan the handle with MFH_MODE_FULL (any dense operator, Hermitian or not; all N_blk^2 blocks)
+ * or MFH_MODE_PAIRS (Hermitian operators; only the canonical blocks n <= m, used for both positions), then hand every
+ * stored block over once:
+ *   block      B x B complex of the handle's dtype, row-major, interleaved (re, im); host (pageable or pinned) or device
+ *   is_device  0: host pointer, 1: device pointer
+ * The copy is enqueued on `stream`; a host block is consumed before the call returns.  mfh_apply fails with
+ * MFH_ERR_BAD_STATE until every stored block of the plan (of this rank, for a partitioned handle) has been set; a
+ * block may be set again at any time (time-dependent operators).  Errors: INVALID_ARG (not an external handle, block
+ * outside the plan's stored set, e.g. n > m in pairs mode), BAD_STATE (no plan), CUDA. */
+MFH_API int mfh_set_block(mfh_handle h, int32_t n, int32_t m, const void* block, int32_t is_device, void* stream);
 
 /* Analytic planner only (Algorithm 1; adaptive block size P:409-429; cache budget
  * Eq. 27).  Pure host arithmetic: needs no GPU, touches no handle.  Enumerates

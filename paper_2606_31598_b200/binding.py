@@ -17,8 +17,9 @@ MFH_OK = 0
 MFH_ERR_INVALID_ARG, MFH_ERR_BAD_STATE, MFH_ERR_OUT_OF_MEMORY = 1, 2, 3
 MFH_ERR_CUDA, MFH_ERR_NOT_CONVERGED, MFH_ERR_UNSUPPORTED = 4, 5, 6
 MFH_C128, MFH_C64 = 0, 1
-MFH_SRC_GUE, MFH_SRC_DIAG_PLUS_GUE, MFH_SRC_ANALYTIC = 0, 1, 2
-SOURCES = {"gue": MFH_SRC_GUE, "diag_plus_gue": MFH_SRC_DIAG_PLUS_GUE, "analytic": MFH_SRC_ANALYTIC}
+MFH_SRC_GUE, MFH_SRC_DIAG_PLUS_GUE, MFH_SRC_ANALYTIC, MFH_SRC_EXTERNAL = 0, 1, 2, 3
+SOURCES = {"gue": MFH_SRC_GUE, "diag_plus_gue": MFH_SRC_DIAG_PLUS_GUE, "analytic": MFH_SRC_ANALYTIC,
+           "external": MFH_SRC_EXTERNAL}
 MFH_MODE_AUTO, MFH_MODE_PROCEDURAL, MFH_MODE_PARTIAL, MFH_MODE_FULL, MFH_MODE_PAIRS = 0, 1, 2, 3, 4
 MFH_MAX_K = 16
 MFH_PART_NONE, MFH_PART_ROWS, MFH_PART_PAIRS = 0, 1, 2
@@ -32,7 +33,7 @@ MODES = {"auto": MFH_MODE_AUTO, "procedural": MFH_MODE_PROCEDURAL, "partial": MF
 SYMBOLS = ["mfh_create", "mfh_plan_analytic", "mfh_plan_node_analytic", "mfh_plan", "mfh_apply", "mfh_apply_host", "mfh_apply_timed",
            "mfh_chebyshev", "mfh_chebyshev_imag", "mfh_chebyshev_steps", "mfh_lanczos_bounds", "mfh_destroy", "mfh_last_error", "mfh_get_plan", "mfh_debug_philox",
            "mfh_materialize_block", "mfh_debug_h0", "mfh_debug_pipe_rates", "mfh_sb_create", "mfh_sb_plan", "mfh_sb_apply",
-           "mfh_sb_destroy", "mfh_set_partition", "mfh_get_partition_rows", "mfh_set_exchange", "mfh_debug_read_bandwidth", "mfh_set_source_params"]
+           "mfh_sb_destroy", "mfh_set_partition", "mfh_get_partition_rows", "mfh_set_exchange", "mfh_debug_read_bandwidth", "mfh_set_source_params", "mfh_set_block"]
 
 _lib = None
 
@@ -70,6 +71,7 @@ def lib():
     L.mfh_set_partition.argtypes = [vp, i32, i32, i32]
     L.mfh_set_exchange.argtypes = [vp, vp, vp]
     L.mfh_set_source_params.argtypes = [vp, ctypes.POINTER(dbl)]
+    L.mfh_set_block.argtypes = [vp, i32, i32, vp, i32, vp]
     L.mfh_get_partition_rows.argtypes = [vp, ctypes.POINTER(i32), ctypes.POINTER(i32), ctypes.POINTER(i32)]
     L.mfh_destroy.argtypes = [vp]
     L.mfh_last_error.argtypes = []
@@ -163,6 +165,18 @@ class Hamiltonian:
         """Parameters (t, alpha, phi, W, beta, delta) of the analytic source (kind="analytic"); call before plan."""
         arr = (ctypes.c_double * 6)(*[float(x) for x in theta])
         _check(lib().mfh_set_source_params(self._h, arr))
+
+    def set_block(self, n: int, m: int, block):
+        """Supply the stored block (n, m) of an external operator (kind="external"): a B x B complex torch tensor
+        (device or host) or numpy array of the handle's dtype, row-major."""
+        import numpy as np
+        if isinstance(block, np.ndarray):
+            want = np.complex128 if self.dtype == "c128" else np.complex64
+            arr = np.ascontiguousarray(block, dtype=want)
+            _check(lib().mfh_set_block(self._h, n, m, arr.ctypes.data, 0, _stream()))
+        else:
+            assert block.is_contiguous() and block.dtype == self._torch_dtype()
+            _check(lib().mfh_set_block(self._h, n, m, block.data_ptr(), 1 if block.is_cuda else 0, _stream()))
 
     def set_partition(self, rank: int, world: int, scheme: str = "pairs"):
         """Distributed execution: this handle computes rank `rank`'s share of phi (call before plan)."""

@@ -122,8 +122,13 @@ static int commit_plan(mfh_handle h, const Plan& p, cudaStream_t st)
     }
     int rc = ensure_gen_table(h, st);
     if (rc) return rc;
-    rc = launch_fill_cache(h, st);
-    if (rc) return rc;
+    if (h->kind == MFH_SRC_EXTERNAL) {   // the caller supplies the stored blocks (mfh_set_block)
+        h->ext_set.assign((size_t)q.n_cached, 0);
+        h->ext_missing = q.n_cached;
+    } else {
+        rc = launch_fill_cache(h, st);
+        if (rc) return rc;
+    }
     MFH_CUDA_CHECK(cudaStreamSynchronize(st));
     h->planned = true;
     return MFH_OK;
@@ -135,6 +140,11 @@ static int apply_impl(mfh_handle h, const void* psi, void* phi, const double* la
 {
     const Plan& p = h->plan;
     int rc;
+    if (h->kind == MFH_SRC_EXTERNAL && h->ext_missing > 0) {
+        set_error("external operator: %lld of %lld stored blocks have not been set (mfh_set_block)", (long long)h->ext_missing,
+                  (long long)p.n_cached);
+        return MFH_ERR_BAD_STATE;
+    }
     if (ev) cudaEventRecord(ev[0], st);
     const bool overlap = partial_overlap_supported(h);   // cached and generated parts in one kernel (Eq. 33)
     if (!overlap && (rc = p.pairs ? launch_cached_pairs(h, psi, st) : launch_cached(h, psi, st))) return rc;
@@ -219,7 +229,7 @@ MFH_API int mfh_create(mfh_handle* out, int64_t D, int32_t B, uint64_t seed, int
                   MFH_MAX_B, (long long)D);
         return MFH_ERR_INVALID_ARG;
     }
-    if (source_kind != MFH_SRC_GUE && source_kind != MFH_SRC_DIAG_PLUS_GUE && source_kind != MFH_SRC_ANALYTIC) {
+    if (source_kind < MFH_SRC_GUE || source_kind > MFH_SRC_EXTERNAL) {
         set_error("mfh_create: unknown source kind %d", source_kind);
         return MFH_ERR_INVALID_ARG;
     }
@@ -265,6 +275,47 @@ MFH_API int mfh_set_source_params(mfh_handle h, const double* theta_host)
     h->analytic.beta2pi = 6.283185307179586476925 * theta_host[4];
     h->analytic.delta = theta_host[5];
     h->analytic_set = true;
+    return MFH_OK;
+}
+
+MFH_API int mfh_set_block(mfh_handle h, int32_t n, int32_t m, const void* block, int32_t is_device, void* stream)
+{
+    if (!h || !block) { set_error("mfh_set_block: NULL pointer"); return MFH_ERR_INVALID_ARG; }
+    if (h->kind != MFH_SRC_EXTERNAL) { set_error("mfh_set_block: handle is not MFH_SRC_EXTERNAL"); return MFH_ERR_INVALID_ARG; }
+    if (!h->planned) { set_error("mfh_set_block: call mfh_plan first"); return MFH_ERR_BAD_STATE; }
+    const Plan& p = h->plan;
+    if (n < 0 || m < 0 || n >= p.n_blk || m >= p.n_blk) {
+        set_error("mfh_set_block: block (%d,%d) outside %d x %d", n, m, p.n_blk, p.n_blk);
+        return MFH_ERR_INVALID_ARG;
+    }
+    const int32_t slot = p.cache_slot[(size_t)n * p.n_blk + m];
+    if (slot < 0) {
+        set_error("mfh_set_block: block (%d,%d) is not stored by this plan (%s)", n, m,
+                  slot == -2 ? "pair cache: pass the canonical block n <= m" : "owned by another rank");
+        return MFH_ERR_INVALID_ARG;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t bytes = (size_t)p.B * p.B * complex_bytes(h->dtype);
+    int rc;
+    if (is_device) {
+        rc = launch_store_block(h, slot, block, st);
+    } else if (h->dtype == MFH_C64 && p.k > 1) {
+        void* tmp = nullptr;   // tiled cache: stage on the device, then re-lay
+        MFH_CUDA_CHECK(cudaMalloc(&tmp, bytes));
+        MFH_CUDA_CHECK(cudaMemcpyAsync(tmp, block, bytes, cudaMemcpyHostToDevice, st));
+        rc = launch_store_block(h, slot, tmp, st);
+        cudaStreamSynchronize(st);
+        cudaFree(tmp);
+    } else {
+        MFH_CUDA_CHECK(cudaMemcpyAsync((char*)h->d_cache + (size_t)slot * bytes, block, bytes, cudaMemcpyHostToDevice, st));
+        MFH_CUDA_CHECK(cudaStreamSynchronize(st));   // the host block may be reused by the caller
+        rc = MFH_OK;
+    }
+    if (rc) return rc;
+    if (!h->ext_set[slot]) {
+        h->ext_set[slot] = 1;
+        --h->ext_missing;
+    }
     return MFH_OK;
 }
 
@@ -345,6 +396,14 @@ MFH_API int mfh_plan(mfh_handle h, int32_t mode, int32_t k, int64_t n_applies_hi
         set_error("mfh_plan: invalid argument (k=%d, mode=%d)", k, mode);
         return MFH_ERR_INVALID_ARG;
     }
+    if (h->kind == MFH_SRC_EXTERNAL) {
+        if (mode == MFH_MODE_AUTO) mode = MFH_MODE_FULL;
+        if (mode != MFH_MODE_FULL && mode != MFH_MODE_PAIRS) {
+            set_error("mfh_plan: external blocks need MFH_MODE_FULL or MFH_MODE_PAIRS (nothing can be generated)");
+            return MFH_ERR_INVALID_ARG;
+        }
+        measure = 0;   // nothing to time before the blocks are there
+    }
     if (h->kind == MFH_SRC_ANALYTIC && !h->analytic_set) {
         set_error("mfh_plan: MFH_SRC_ANALYTIC needs mfh_set_source_params first");
         return MFH_ERR_BAD_STATE;
@@ -406,6 +465,10 @@ MFH_API int mfh_plan(mfh_handle h, int32_t mode, int32_t k, int64_t n_applies_hi
             set_error("mfh_plan: no candidate could be committed");
             return MFH_ERR_OUT_OF_MEMORY;
         }
+    }
+    if (h->kind == MFH_SRC_EXTERNAL && cands[0].cached_fraction < 1.0) {
+        set_error("mfh_plan: the external operator does not fit the budget as a %s cache", mode == MFH_MODE_PAIRS ? "pair" : "full");
+        return MFH_ERR_OUT_OF_MEMORY;
     }
     rc = commit_plan(h, make_plan(cands[0]), st);
     if (rc) return rc;

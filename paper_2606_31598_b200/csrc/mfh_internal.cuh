@@ -77,6 +77,8 @@ struct mfh_handle_s {
     double lambda = 1.0;
     mfh::AnalyticArgs analytic = {0, 0, 1, 0, 0, 0, 0};          // mfh_set_source_params (MFH_SRC_ANALYTIC)
     bool analytic_set = false;
+    std::vector<uint8_t> ext_set;                                 // MFH_SRC_EXTERNAL: per cache slot, block supplied
+    int64_t ext_missing = 0;                                      // stored blocks not supplied yet
     int32_t part_rank = 0, part_world = 1, part_scheme = 0;   // mfh_set_partition
     mfh_exchange_fn exchange = nullptr;                       // mfh_set_exchange
     void* exchange_user = nullptr;
@@ -128,6 +130,7 @@ int launch_philox_debug(uint64_t seed, uint32_t stream_id, const uint32_t* i, co
                         int64_t n, uint32_t* words, cudaStream_t st);
 int launch_fill_block(mfh_handle h, int32_t B, int32_t n, int32_t m, void* out, cudaStream_t st);
 int launch_fill_cache(mfh_handle h, cudaStream_t st);
+int launch_store_block(mfh_handle h, int32_t slot, const void* src_dev, cudaStream_t st);   // external block -> cache slot
 int launch_h0(mfh_handle h, void* out, cudaStream_t st);
 int launch_proc_single(mfh_handle h, const void* psi, cudaStream_t st);
 bool partial_overlap_supported(mfh_handle h);

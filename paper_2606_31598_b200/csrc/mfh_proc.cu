@@ -132,6 +132,30 @@ int launch_fill_cache(mfh_handle h, cudaStream_t st)
                : launch_fill_t<float>(h, grid, p.B, p.n_blk, h->d_cache_slot, 0, 0, p.k > 1 ? 1 : 0, h->d_cache, st);
 }
 
+// External block (Eq. 10) -> cache slot: a plain copy for row-major caches, a re-layout for the tiled cache
+// of complex64 k-vector plans (mfh_internal.cuh tiled_cache_offset).
+__global__ void __launch_bounds__(256) retile_kernel(int32_t B, const float2* __restrict__ src, float2* __restrict__ dst)
+{
+    for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < (int64_t)B * B; e += (int64_t)gridDim.x * blockDim.x) {
+        const int a = (int)(e / B), b = (int)(e % B);
+        reinterpret_cast<float2*>(reinterpret_cast<float*>(dst) + tiled_cache_offset(B, a, b))[0] = src[e];
+    }
+}
+
+int launch_store_block(mfh_handle h, int32_t slot, const void* src_dev, cudaStream_t st)
+{
+    const Plan& p = h->plan;
+    const size_t cb = complex_bytes(h->dtype), bytes = (size_t)p.B * p.B * cb;
+    char* dst = (char*)h->d_cache + (size_t)slot * bytes;
+    if (h->dtype == MFH_C64 && p.k > 1) {
+        retile_kernel<<<std::min(p.B * p.B / 256, 148 * 8), 256, 0, st>>>(p.B, (const float2*)src_dev, (float2*)dst);
+        MFH_CUDA_CHECK(cudaGetLastError());
+    } else {
+        MFH_CUDA_CHECK(cudaMemcpyAsync(dst, src_dev, bytes, cudaMemcpyDeviceToDevice, st));
+    }
+    return MFH_OK;
+}
+
 // --------------------------------------------------------------------------------------------
 // H0 diagonal of configs[2]: h0_i = 2u - 1, u = (x0 + 1/2) 2^-32, ctr = (i, i, stream 1, 0).
 // --------------------------------------------------------------------------------------------

@@ -65,6 +65,14 @@ def sample_rows(D: int, n: int, seed: int = 0) -> np.ndarray:
     return np.unique(np.concatenate([fixed, rand]))
 
 
+def dense_matrix(D: int, seed: int, hermitian: bool = True) -> np.ndarray:
+    """Seeded dense D x D complex matrix with O(1/sqrt(D)) entries: the externally stored operator of the Eq. 10
+    tests (an input of the method, not part of its arithmetic)."""
+    rng = np.random.default_rng([seed, D, 10])
+    M = (rng.standard_normal((D, D)) + 1j * rng.standard_normal((D, D))) / np.sqrt(2.0 * D)
+    return (M + M.conj().T) / np.sqrt(2.0) if hermitian else M
+
+
 def small_hermitian(d: int, seed: int) -> np.ndarray:
     """Seeded d x d Hermitian matrix with O(1) entries (system-side operators H_S, A of the system-bath
     workload; an input of the method, not part of its arithmetic)."""
