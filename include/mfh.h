@@ -127,6 +127,24 @@ MFH_API int mfh_plan_node_analytic(int64_t D, int32_t dtype, int32_t k, int32_t 
                                    int64_t hbm_free_bytes_per_gpu, int32_t mode, int32_t B, int32_t scheme,
                                    int64_t n_applies_per_task, char* json_out, size_t json_cap);
 
+/* Neural surrogate of the planner (host only; Eq. 24-26, Algorithm 3).  A one-hidden-layer
+ * network on componentwise normalised plan features predicts the logarithm of the measured apply time:
+ *     z = (x - mu) / sigma,   f(x) = tanh(z W1 + b1) W2 + b2   (Eq. 24),   t_NN(p) = exp(f(x(p)))   (Eq. 25),
+ * trained by minimising the log-time mean-squared error (Eq. 26) over the records (x(p), t_mv(p)) the measured
+ * planner produces; it only RANKS candidates, a local measurement of the top K_NN stays the decision rule.
+ *   theta  = [mu (F) | sigma (F) | W1 (F x H, row-major) | b1 (H) | W2 (H) | b2], mfh_surrogate_theta_size doubles
+ *   X      = [n][F] features (paper_2606_31598_b200/surrogate.py builds x(p) from a plan record), t_seconds > 0
+ * mfh_surrogate_fit: mu, sigma from the data (sigma = 1 for constant features), seeded initial weights, `epochs`
+ * full-batch Adam steps of size lr; *final_loss = Eq. 26 at the end.  mfh_surrogate_loss_grad: Eq. 26 and its
+ * gradient with respect to [W1 | b1 | W2 | b2] (test export; grad_out may be NULL).  Errors: INVALID_ARG. */
+MFH_API int64_t mfh_surrogate_theta_size(int32_t n_features, int32_t hidden);
+MFH_API int mfh_surrogate_fit(const double* X, const double* t_seconds, int64_t n, int32_t n_features, int32_t hidden,
+                              int32_t epochs, double lr, uint64_t seed, double* theta_out, double* final_loss);
+MFH_API int mfh_surrogate_predict(const double* theta, int32_t n_features, int32_t hidden, const double* X, int64_t n,
+                                  double* t_pred_seconds);
+MFH_API int mfh_surrogate_loss_grad(const double* theta, int32_t n_features, int32_t hidden, const double* X,
+                                    const double* t_seconds, int64_t n, double* loss_out, double* grad_out);
+
 /* Plan and commit: choose mode and B (analytic; measure != 0 additionally times the best
  * candidates on the device, Algorithm 2, R_warm = 1, R_bench = 3, K_bench <= 8), allocate the
  * cache and the workspace and fill the cache with the generator (one-time cost).

@@ -172,3 +172,4 @@ from .system_bath import sb_apply  # noqa: E402,F401
 from .partition import apply_partition, combine as combine_partition, owned_blocks  # noqa: E402,F401
 from .analytic import analytic_apply, analytic_matrix, theta_array  # noqa: E402,F401
 from .external import block_apply, stored_blocks  # noqa: E402,F401
+from . import surrogate  # noqa: E402,F401

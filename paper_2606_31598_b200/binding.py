@@ -33,7 +33,8 @@ MODES = {"auto": MFH_MODE_AUTO, "procedural": MFH_MODE_PROCEDURAL, "partial": MF
 SYMBOLS = ["mfh_create", "mfh_plan_analytic", "mfh_plan_node_analytic", "mfh_plan", "mfh_apply", "mfh_apply_host", "mfh_apply_timed",
            "mfh_chebyshev", "mfh_chebyshev_imag", "mfh_chebyshev_steps", "mfh_lanczos_bounds", "mfh_destroy", "mfh_last_error", "mfh_get_plan", "mfh_debug_philox",
            "mfh_materialize_block", "mfh_debug_h0", "mfh_debug_pipe_rates", "mfh_sb_create", "mfh_sb_plan", "mfh_sb_apply",
-           "mfh_sb_destroy", "mfh_set_partition", "mfh_get_partition_rows", "mfh_set_exchange", "mfh_debug_read_bandwidth", "mfh_set_source_params", "mfh_set_block"]
+           "mfh_sb_destroy", "mfh_set_partition", "mfh_get_partition_rows", "mfh_set_exchange", "mfh_debug_read_bandwidth", "mfh_set_source_params", "mfh_set_block", "mfh_surrogate_theta_size", "mfh_surrogate_fit",
+           "mfh_surrogate_predict", "mfh_surrogate_loss_grad"]
 
 _lib = None
 
@@ -87,7 +88,7 @@ def lib():
     L.mfh_sb_apply.argtypes = [vp, vp, vp, vp]
     L.mfh_sb_destroy.argtypes = [vp]
     for name in SYMBOLS:
-        if name != "mfh_last_error":
+        if name not in ("mfh_last_error", "mfh_surrogate_theta_size"):
             getattr(L, name).restype = ctypes.c_int
     _lib = L
     return L

@@ -1,0 +1,122 @@
+"""Neural surrogate of the planner (Algorithm 3): marshalling around the library's
+``mfh_surrogate_*`` host functions plus the feature vector x(p) of a plan record.
+
+The arithmetic (normalisation, Eq. 24-26, Adam) runs in ``lib/libmfh.so``; this module only builds feature rows from
+the JSON records that ``mfh_plan`` / ``mfh_plan_analytic`` return and keeps a portable benchmark log."""
+from __future__ import annotations
+
+import ctypes
+import json
+import math
+
+import numpy as np
+
+from .binding import MFH_OK, MfhError, lib
+
+# x(p) of P:370: (log D, log R, log N_blk, log b, log N_task, p_row, W(p), 1_full, 1_partial, 1_procedural,
+# 1_pairs [this build's fourth storage mode], log F_mv, M_op/M_free, M_work/M_free, M_tot/M_free, 1_complex64,
+# log GPU memory, log multiprocessors)
+FEATURES = ("log_D", "log_R", "log_n_blk", "log_b", "log_n_task", "p_row", "waves", "is_full", "is_partial",
+            "is_procedural", "is_pairs", "log_flops", "op_over_free", "work_over_free", "tot_over_free", "is_c64",
+            "log_gpu_bytes", "log_sms")
+F = len(FEATURES)
+
+
+def features(D: int, dtype: str, k: int, cand: dict, free_bytes: float, n_task: int = 1, p_row: int = 1, waves: int = 1,
+             gpu_bytes: float = 180e9, sms: int = 148) -> np.ndarray:
+    """Feature row of one candidate record (the dicts in plan["candidates"])."""
+    mode = cand["mode"]
+    return np.array([math.log(D), math.log(k), math.log(cand["n_blk"]), math.log(cand["B"]), math.log(n_task),
+                     float(p_row), float(waves), float(mode == "full"), float(mode == "partial"),
+                     float(mode == "procedural"), float(mode == "pairs"), math.log(cand["flops_per_apply"]),
+                     cand["cache_bytes"] / free_bytes, cand["work_bytes"] / free_bytes, cand["total_bytes"] / free_bytes,
+                     float(dtype == "c64"), math.log(gpu_bytes), math.log(sms)], dtype=np.float64)
+
+
+def _p(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+def _setup():
+    L = lib()
+    dp, i32, i64 = ctypes.POINTER(ctypes.c_double), ctypes.c_int32, ctypes.c_int64
+    L.mfh_surrogate_theta_size.argtypes = [i32, i32]
+    L.mfh_surrogate_theta_size.restype = i64
+    L.mfh_surrogate_fit.argtypes = [dp, dp, i64, i32, i32, i32, ctypes.c_double, ctypes.c_uint64, dp, dp]
+    L.mfh_surrogate_predict.argtypes = [dp, i32, i32, dp, i64, dp]
+    L.mfh_surrogate_loss_grad.argtypes = [dp, i32, i32, dp, dp, i64, dp, dp]
+    return L
+
+
+def theta_size(n_features: int, hidden: int) -> int:
+    return int(_setup().mfh_surrogate_theta_size(n_features, hidden))
+
+
+def fit(X, t_seconds, hidden: int = 16, epochs: int = 3000, lr: float = 0.01, seed: int = 0):
+    """Train f_theta on records (x_i, t_i); returns (theta, final Eq.-26 loss)."""
+    X = np.ascontiguousarray(X, dtype=np.float64)
+    t = np.ascontiguousarray(t_seconds, dtype=np.float64)
+    n, nf = X.shape
+    theta = np.zeros(theta_size(nf, hidden), dtype=np.float64)
+    loss = ctypes.c_double(0.0)
+    rc = _setup().mfh_surrogate_fit(_p(X), _p(t), n, nf, hidden, epochs, lr, seed, _p(theta), ctypes.byref(loss))
+    if rc != MFH_OK:
+        raise MfhError(rc, lib().mfh_last_error().decode())
+    return theta, float(loss.value)
+
+
+def predict(theta, X, hidden: int = 16) -> np.ndarray:
+    X = np.ascontiguousarray(X, dtype=np.float64).reshape(-1, np.shape(X)[-1])
+    out = np.empty(X.shape[0], dtype=np.float64)
+    th = np.ascontiguousarray(theta, dtype=np.float64)
+    rc = _setup().mfh_surrogate_predict(_p(th), X.shape[1], hidden, _p(X), X.shape[0], _p(out))
+    if rc != MFH_OK:
+        raise MfhError(rc, lib().mfh_last_error().decode())
+    return out
+
+
+def loss_grad(theta, X, t_seconds, hidden: int = 16):
+    X = np.ascontiguousarray(X, dtype=np.float64)
+    t = np.ascontiguousarray(t_seconds, dtype=np.float64)
+    th = np.ascontiguousarray(theta, dtype=np.float64)
+    nf = X.shape[1]
+    grad = np.empty(nf * hidden + 2 * hidden + 1, dtype=np.float64)
+    loss = ctypes.c_double(0.0)
+    rc = _setup().mfh_surrogate_loss_grad(_p(th), nf, hidden, _p(X), _p(t), X.shape[0], ctypes.byref(loss), _p(grad))
+    if rc != MFH_OK:
+        raise MfhError(rc, lib().mfh_last_error().decode())
+    return float(loss.value), grad
+
+
+def records_from_plan(D: int, dtype: str, k: int, plan: dict, free_bytes: float):
+    """(feature row, measured seconds) for every candidate the measured planner timed."""
+    out = []
+    for c in plan["candidates"]:
+        if c.get("measured_apply_s", -1) > 0:
+            out.append((features(D, dtype, k, c, free_bytes), c["measured_apply_s"]))
+    return out
+
+
+def rank(theta, D: int, dtype: str, k: int, plan: dict, free_bytes: float, hidden: int = 16):
+    """Feasible candidates of an analytic plan record ordered by t_NN(p) W(p) (W = 1 on one GPU)."""
+    cands = [c for c in plan["candidates"] if c["feasible"]]
+    X = np.stack([features(D, dtype, k, c, free_bytes) for c in cands])
+    t = predict(theta, X, hidden)
+    order = np.argsort(t)
+    return [(cands[i], float(t[i])) for i in order]
+
+
+def save_log(path: str, rows):
+    """Portable benchmark log: one JSON object per line {"x": [...], "t": seconds, "meta": {...}}."""
+    with open(path, "w") as f:
+        for x, t, meta in rows:
+            f.write(json.dumps({"x": [float(v) for v in x], "t": float(t), "meta": meta}) + "\n")
+
+
+def load_log(path: str):
+    X, t, meta = [], [], []
+    for line in open(path):
+        if line.strip():
+            r = json.loads(line)
+            X.append(r["x"]); t.append(r["t"]); meta.append(r.get("meta", {}))
+    return np.array(X, dtype=np.float64), np.array(t, dtype=np.float64), meta

@@ -1,0 +1,84 @@
+"""The planner's neural surrogate (Algorithm 3, Eq. 24-26; host code of the library, no GPU needed) against the
+numpy oracle: forward pass, loss, gradient by central differences, and training on a planted runtime law."""
+import numpy as np
+import pytest
+
+from oracle import surrogate as orc
+from paper_2606_31598_b200 import binding as mfh
+from paper_2606_31598_b200 import surrogate as sur
+
+F, H = 6, 5
+
+
+def _random_theta(rng):
+    th = rng.standard_normal(sur.theta_size(F, H))
+    th[F:2 * F] = 0.5 + rng.random(F)                         # sigma > 0
+    return th
+
+
+def test_theta_layout_forward_and_loss_match_the_oracle():
+    rng = np.random.default_rng(1)
+    assert sur.theta_size(F, H) == 2 * F + F * H + 2 * H + 1
+    th = _random_theta(rng)
+    X = rng.standard_normal((40, F))
+    t = np.exp(rng.standard_normal(40))
+    assert np.allclose(sur.predict(th, X, H), orc.predict(th, F, H, X), rtol=1e-13, atol=0)
+    loss, _ = sur.loss_grad(th, X, t, H)
+    assert loss == pytest.approx(orc.loss(th, F, H, X, t), rel=1e-13)
+
+
+def test_gradient_against_central_differences_of_the_oracle_loss():
+    rng = np.random.default_rng(2)
+    th = _random_theta(rng)
+    X = rng.standard_normal((25, F))
+    t = np.exp(rng.standard_normal(25))
+    _, grad = sur.loss_grad(th, X, t, H)
+    eps = 1e-6
+    for q in range(grad.size):                                # every trained parameter: W1, b1, W2, b2
+        tp, tm = th.copy(), th.copy()
+        tp[2 * F + q] += eps
+        tm[2 * F + q] -= eps
+        fd = (orc.loss(tp, F, H, X, t) - orc.loss(tm, F, H, X, t)) / (2 * eps)
+        assert grad[q] == pytest.approx(fd, rel=2e-6, abs=1e-9), q
+
+
+def test_training_recovers_a_planted_runtime_law():
+    """t = c * bytes / bandwidth with a mode-dependent factor: log t is a smooth function of the features."""
+    rng = np.random.default_rng(3)
+    n = 400
+    X = np.zeros((n, F))
+    X[:, 0] = rng.uniform(20, 26, n)                          # log bytes
+    X[:, 1] = rng.integers(0, 2, n)                           # a mode flag
+    X[:, 2] = rng.uniform(0, 1, n)                            # memory pressure
+    X[:, 3] = 7.0                                             # a constant feature (sigma = 1 rule)
+    X[:, 4:] = rng.standard_normal((n, F - 4)) * 0.01
+    t = np.exp(X[:, 0] - 29.0 + 0.7 * X[:, 1] + 0.3 * X[:, 2] ** 2)
+    theta, loss = sur.fit(X[:300], t[:300], hidden=H, epochs=4000, lr=0.01, seed=5)
+    assert loss < 2e-3 and loss == pytest.approx(orc.loss(theta, F, H, X[:300], t[:300]), rel=1e-12)
+    mu, sigma = theta[:F], theta[F:2 * F]
+    assert np.allclose(mu, X[:300].mean(axis=0)) and np.allclose(sigma[:3], X[:300, :3].std(axis=0)) and sigma[3] == 1.0
+    pred = sur.predict(theta, X[300:], H)
+    assert np.sqrt(np.mean(np.log(pred / t[300:]) ** 2)) < 0.08          # held-out log-time error
+    theta2, _ = sur.fit(X[:300], t[:300], hidden=H, epochs=4000, lr=0.01, seed=5)
+    assert np.array_equal(theta, theta2)                                 # seeded, deterministic
+
+
+def test_features_ranking_and_argument_errors(tmp_path):
+    rec = mfh.plan_analytic(65536, "c128", k=1, n_applies_hint=100, hbm_free_bytes=180 * 10**9)
+    free = 0.9 * 180e9
+    rows = [sur.features(65536, "c128", 1, c, free) for c in rec["candidates"]]
+    assert all(r.shape == (sur.F,) and np.all(np.isfinite(r)) for r in rows)
+    X = np.stack(rows)
+    t = np.array([max(c["model_apply_s"], 1e-6) for c in rec["candidates"]])
+    theta, _ = sur.fit(X, t, hidden=8, epochs=2000, lr=0.02, seed=1)
+    ranked = sur.rank(theta, 65536, "c128", 1, rec, free, hidden=8)
+    assert len(ranked) == sum(c["feasible"] for c in rec["candidates"])
+    assert [p for _, p in ranked] == sorted(p for _, p in ranked)
+    path = tmp_path / "log.jsonl"
+    sur.save_log(str(path), [(x, tt, {"D": 65536}) for x, tt in zip(X, t)])
+    X2, t2, meta = sur.load_log(str(path))
+    assert np.array_equal(X2, X) and np.allclose(t2, t) and meta[0]["D"] == 65536
+    with pytest.raises(mfh.MfhError):
+        sur.fit(X, -t, hidden=8)
+    with pytest.raises(mfh.MfhError):
+        sur.fit(X[:1], t[:1], hidden=8)
