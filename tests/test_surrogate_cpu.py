@@ -82,3 +82,19 @@ def test_features_ranking_and_argument_errors(tmp_path):
         sur.fit(X, -t, hidden=8)
     with pytest.raises(mfh.MfhError):
         sur.fit(X[:1], t[:1], hidden=8)
+
+
+def test_surrogate_trained_on_the_shipped_b200_log_ranks_a_held_out_size():
+    """paper_2606_31598_b200/data/plan_log_b200.jsonl: 240 candidates timed by the measured planner on one B200
+    (collect_plan_log.py).  Trained without the D = 16384 problems, the surrogate's first choice there is within 25 %
+    of the best measured plan and its log-time error is a fraction of the spread of the times."""
+    import os
+    from paper_2606_31598_b200 import collect_plan_log as cpl
+    path = os.path.join(os.path.dirname(cpl.__file__), "data", "plan_log_b200.jsonl")
+    X, t, meta = sur.load_log(path)
+    assert X.shape == (240, sur.F) and np.all(t > 0)
+    rows = list(zip(X, t, meta))
+    rep = cpl.evaluate(rows, held_out_D={16384}, hidden=16, epochs=3000)
+    assert rep["train_records"] == 192 and rep["test_records"] == 48
+    assert rep["test_rms_log_error"] < 0.35 < float(np.std(np.log(t)))
+    assert max(p["regret"] for p in rep["problems"]) < 1.25
