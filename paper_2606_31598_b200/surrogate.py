@@ -120,3 +120,31 @@ def load_log(path: str):
             r = json.loads(line)
             X.append(r["x"]); t.append(r["t"]); meta.append(r.get("meta", {}))
     return np.array(X, dtype=np.float64), np.array(t, dtype=np.float64), meta
+
+
+def hybrid_plan(theta, D: int, dtype: str, k: int = 1, seed: int = 0, kind: str = "gue", seed_h0: int = 0,
+                n_applies_hint: int = 1, hbm_budget_bytes: int = 0, k_nn: int = 3, hidden: int = 16):
+    """Algorithm 3, hybrid mode: enumerate the memory-feasible candidates with the analytic planner, rank
+    them by t_NN(p), commit and time only the top `k_nn` on the device and keep the best measured one (Eq. 23).
+    Returns (handle with the chosen plan committed, report).  Needs CUDA."""
+    import torch
+    from .binding import Hamiltonian, plan_analytic
+    free = torch.cuda.mem_get_info()[0]
+    budget = hbm_budget_bytes if hbm_budget_bytes > 0 else 0.9 * free
+    rec = plan_analytic(D, dtype, k=k, n_applies_hint=n_applies_hint, hbm_free_bytes=int(budget / 0.9))
+    ranked = rank(theta, D, dtype, k, rec, rec["budget_bytes"], hidden)[:k_nn]
+    n = max(n_applies_hint, 1)
+    tried, best = [], None
+    for cand, t_nn in ranked:
+        h = Hamiltonian(D, cand["B"], seed, dtype, kind=kind, seed_h0=seed_h0)
+        r = h.plan(cand["mode"], k=k, n_applies_hint=n_applies_hint, hbm_budget_bytes=int(budget), measure=True)
+        c = r["chosen"]
+        job = n * c["measured_apply_s"] + c["model_fill_s"]
+        tried.append({"mode": c["mode"], "B": c["B"], "t_nn_s": t_nn, "measured_apply_s": c["measured_apply_s"], "job_s": job})
+        if best is None or job < best[1]:
+            if best is not None:
+                best[0].destroy()
+            best = (h, job, tried[-1])
+        else:
+            h.destroy()
+    return best[0], {"feasible_candidates": sum(c["feasible"] for c in rec["candidates"]), "timed": tried, "chosen": best[2]}

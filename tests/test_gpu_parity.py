@@ -310,3 +310,22 @@ def test_read_only_stream_probe_reports_a_plausible_hbm_rate():
     with pytest.raises(mfh.MfhError) as e:
         mfh.read_bandwidth(buf[:1024])
     assert e.value.code == mfh.MFH_ERR_INVALID_ARG
+
+
+def test_hybrid_surrogate_planner_commits_a_working_plan():
+    """Algorithm 3: rank by the surrogate trained on the shipped B200 log, time the top 3, apply."""
+    import os
+    from paper_2606_31598_b200 import surrogate as sur
+    X, t, _ = sur.load_log(os.path.join(os.path.dirname(sur.__file__), "data", "plan_log_b200.jsonl"))
+    theta, _ = sur.fit(X, t, hidden=16, epochs=2000, lr=0.01, seed=1)
+    D = 8192
+    h, rep = sur.hybrid_plan(theta, D, "c128", seed=1234, n_applies_hint=100, k_nn=3)
+    assert len(rep["timed"]) == 3 and rep["feasible_candidates"] > 3
+    assert rep["chosen"]["job_s"] == min(x["job_s"] for x in rep["timed"])
+    assert all(0.2 < x["t_nn_s"] / x["measured_apply_s"] < 5.0 for x in rep["timed"])     # the ranking is informed
+    psi = make_psi(D, 99)
+    phi = h.apply(to_dev(psi)).cpu().numpy()
+    B = h.get_plan()["B"]
+    rows = np.arange(0, D, 61)
+    assert rel_l2(phi[rows], oracle.apply(D, B, 1234, psi, rows=rows)) <= TOL["c128"]
+    h.destroy()
