@@ -188,6 +188,16 @@ MFH_API int mfh_apply_host(mfh_handle h, const void* psi_host, void* phi_host, i
 MFH_API int mfh_chebyshev(mfh_handle h, const void* psi_dev, void* out_dev, double t, double e_min,
                           double e_max, double tol, int32_t* n_terms_out, void* stream);
 
+/* Coupling scan with propagation (the paper's outer loop over coupling values, "independent outer-loop
+ * parameters, such as coupling strengths", run here as k simultaneous columns of ONE k-vector plan, Eq. 12):
+ *     out[:, v] = exp(-i H_v t) psi[:, v],   H_v = diag(h0) + lambda_v V   (MFH_SRC_DIAG_PLUS_GUE; lambda_v V otherwise),
+ * all k columns with the same Chebyshev series (same bounds: [e_min, e_max] must enclose the spectrum of EVERY H_v, so
+ * K is set by the widest one), each of the K-1 applies generating or reading every block once for all k columns.
+ *   psi_dev, out_dev  [D][k] of the planned k;  lambdas_host  k doubles or NULL (the handle's lambda for all)
+ * Errors as mfh_chebyshev. */
+MFH_API int mfh_chebyshev_scan(mfh_handle h, const void* psi_dev, void* out_dev, double t, double e_min, double e_max,
+                               double tol, const double* lambdas_host, int32_t* n_terms_out, void* stream);
+
 /* out = exp(-beta (H - e_min)) psi, the imaginary-time (thermal / TPQ) Chebyshev filter the paper runs before its
  * real-time propagation ("the imaginary-time TPQ Chebyshev filter used order 80"; the series is not
  * printed there, R21).  Same recurrence as mfh_chebyshev (Eq. 41-43) with the modified-Bessel

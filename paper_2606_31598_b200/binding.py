@@ -31,7 +31,7 @@ MODES = {"auto": MFH_MODE_AUTO, "procedural": MFH_MODE_PROCEDURAL, "partial": MF
 
 # every symbol include/mfh.h declares (tests check that the library exports all of them)
 SYMBOLS = ["mfh_create", "mfh_plan_analytic", "mfh_plan_node_analytic", "mfh_plan", "mfh_apply", "mfh_apply_host", "mfh_apply_timed",
-           "mfh_chebyshev", "mfh_chebyshev_imag", "mfh_chebyshev_steps", "mfh_lanczos_bounds", "mfh_destroy", "mfh_last_error", "mfh_get_plan", "mfh_debug_philox",
+           "mfh_chebyshev", "mfh_chebyshev_imag", "mfh_chebyshev_scan", "mfh_chebyshev_steps", "mfh_lanczos_bounds", "mfh_destroy", "mfh_last_error", "mfh_get_plan", "mfh_debug_philox",
            "mfh_materialize_block", "mfh_debug_h0", "mfh_debug_pipe_rates", "mfh_sb_create", "mfh_sb_plan", "mfh_sb_apply",
            "mfh_sb_destroy", "mfh_set_partition", "mfh_get_partition_rows", "mfh_set_exchange", "mfh_debug_read_bandwidth", "mfh_set_source_params", "mfh_set_block", "mfh_surrogate_theta_size", "mfh_surrogate_fit",
            "mfh_surrogate_predict", "mfh_surrogate_loss_grad"]
@@ -65,6 +65,7 @@ def lib():
     L.mfh_apply_host.argtypes = [vp, vp, vp, i32, ctypes.POINTER(dbl), vp]
     L.mfh_apply_timed.argtypes = [vp, vp, vp, i32, ctypes.POINTER(dbl), vp, ctypes.POINTER(ctypes.c_float)]
     L.mfh_chebyshev.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, ctypes.POINTER(i32), vp]
+    L.mfh_chebyshev_scan.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, ctypes.POINTER(dbl), ctypes.POINTER(i32), vp]
     L.mfh_chebyshev_imag.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, ctypes.POINTER(i32), vp]
     L.mfh_chebyshev_steps.argtypes = [vp, vp, vp, dbl, i32, dbl, dbl, dbl, ctypes.POINTER(i32), vp]
     L.mfh_lanczos_bounds.argtypes = [vp, vp, i32, dbl, ctypes.POINTER(dbl), ctypes.POINTER(dbl), ctypes.POINTER(dbl),
@@ -231,6 +232,18 @@ class Hamiltonian:
         n = ctypes.c_int32(0)
         _check(lib().mfh_chebyshev(self._h, psi.data_ptr(), out.data_ptr(), t, e_min, e_max, tol,
                                    ctypes.byref(n), _stream()))
+        return out, int(n.value)
+
+    def chebyshev_scan(self, psi, t: float, e_min: float, e_max: float, tol: float, lambdas=None, out=None):
+        """out[:, v] = exp(-i H_v t) psi[:, v] for the k columns of a k-vector plan; returns (out, n_terms)."""
+        import torch
+        k = self.k or 1
+        self._check_vec(psi, k)
+        if out is None:
+            out = torch.empty_like(psi)
+        n = ctypes.c_int32(0)
+        _check(lib().mfh_chebyshev_scan(self._h, psi.data_ptr(), out.data_ptr(), t, e_min, e_max, tol, _lam(lambdas, k),
+                                        ctypes.byref(n), _stream()))
         return out, int(n.value)
 
     def chebyshev_imag(self, psi, beta: float, e_min: float, e_max: float, tol: float, out=None):

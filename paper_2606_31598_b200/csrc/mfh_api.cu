@@ -164,9 +164,9 @@ static int apply_impl(mfh_handle h, const void* psi, void* phi, const double* la
 
 // An apply inside a chain (Chebyshev, Lanczos): on a partitioned handle the result must be complete on
 // every rank before the next O(D) update, so the registered exchange hook runs right after the apply.
-static int apply_chained(mfh_handle h, const void* psi, void* phi, cudaStream_t st)
+static int apply_chained(mfh_handle h, const void* psi, void* phi, cudaStream_t st, const double* lambdas = nullptr)
 {
-    int rc = apply_impl(h, psi, phi, nullptr, st);
+    int rc = apply_impl(h, psi, phi, lambdas, st);
     if (rc || (h->part_world <= 1 && !h->exchange)) return rc;   // a registered hook also runs at world 1 (tests)
     if (!h->exchange) {
         set_error("partitioned handle (world %d): register an exchange hook with mfh_set_exchange", h->part_world);
@@ -560,16 +560,16 @@ MFH_API int mfh_apply_host(mfh_handle h, const void* psi_host, void* phi_host, i
 // out = phase * sum_l coef_l T_l(H~) psi with complex coefficients coef[l] = (re, im); K-1 chained applies.
 static int chebyshev_series(mfh_handle h, const void* psi_dev, void* out_dev, double c, double R, int K,
                             const std::vector<double>& coef_re, const std::vector<double>& coef_im, double ph_re,
-                            double ph_im, cudaStream_t st)
+                            double ph_im, cudaStream_t st, const double* lambdas = nullptr)
 {
-    const size_t vb = (size_t)h->D * complex_bytes(h->dtype);
+    const size_t vb = (size_t)h->D * h->plan.k * complex_bytes(h->dtype);   // k columns: the O(D) updates are element-wise
     if (!h->d_cheb) MFH_CUDA_CHECK(cudaMalloc(&h->d_cheb, 5 * vb));   // cur, prev, acc, Hq + ping-pong of mfh_chebyshev_steps
     char* base = (char*)h->d_cheb;
     void *cur = base, *prev = base + vb, *acc = base + 2 * vb, *hq = base + 3 * vb;
     int rc;
     if ((rc = launch_cheb_first(h, psi_dev, cur, acc, coef_re[0], st))) return rc;      // Eq. 41 (coef_0 is real)
     for (int l = 1; l < K; ++l) {
-        if ((rc = apply_chained(h, cur, hq, st))) return rc;
+        if ((rc = apply_chained(h, cur, hq, st, lambdas))) return rc;
         if ((rc = launch_cheb_step(h, hq, cur, prev, acc, c, 1.0 / R, l == 1, coef_re[l], coef_im[l], st))) return rc;   // Eq. 42-43
         std::swap(cur, prev);
     }
@@ -577,11 +577,11 @@ static int chebyshev_series(mfh_handle h, const void* psi_dev, void* out_dev, do
 }
 
 static int chebyshev_check(const char* fn, mfh_handle h, const void* psi_dev, const void* out_dev, double t, double e_min,
-                           double e_max, double tol)
+                           double e_max, double tol, bool any_k = false)
 {
     if (!h || !psi_dev || !out_dev) { set_error("%s: NULL pointer", fn); return MFH_ERR_INVALID_ARG; }
     if (!h->planned) { set_error("%s: call mfh_plan first", fn); return MFH_ERR_BAD_STATE; }
-    if (h->plan.k != 1) { set_error("%s: plan with k = 1", fn); return MFH_ERR_INVALID_ARG; }
+    if (!any_k && h->plan.k != 1) { set_error("%s: plan with k = 1", fn); return MFH_ERR_INVALID_ARG; }
     if (!(e_max > e_min) || !std::isfinite(t) || !std::isfinite(e_min) || !std::isfinite(e_max) || !(tol > 0.0)) {
         set_error("%s: need e_max > e_min, finite t, tol > 0", fn);
         return MFH_ERR_INVALID_ARG;
@@ -589,10 +589,10 @@ static int chebyshev_check(const char* fn, mfh_handle h, const void* psi_dev, co
     return MFH_OK;
 }
 
-MFH_API int mfh_chebyshev(mfh_handle h, const void* psi_dev, void* out_dev, double t, double e_min,
-                          double e_max, double tol, int32_t* n_terms_out, void* stream)
+static int chebyshev_real_time(const char* fn, mfh_handle h, const void* psi_dev, void* out_dev, double t, double e_min,
+                               double e_max, double tol, int32_t* n_terms_out, void* stream, const double* lambdas, bool any_k)
 {
-    int rc = chebyshev_check("mfh_chebyshev", h, psi_dev, out_dev, t, e_min, e_max, tol);
+    int rc = chebyshev_check(fn, h, psi_dev, out_dev, t, e_min, e_max, tol, any_k);
     if (rc) return rc;
     const double c = 0.5 * (e_max + e_min), R = 0.5 * (e_max - e_min), a = R * t;
     // Bessel table J_l(a) via the C++17 special function (a route different from the oracle's
@@ -613,9 +613,21 @@ MFH_API int mfh_chebyshev(mfh_handle h, const void* psi_dev, void* out_dev, doub
         case 3: ci[l] = 2.0 * v; break;
         }
     }
-    if (K >= l_max) { set_error("mfh_chebyshev: Bessel table too short"); return MFH_ERR_NOT_CONVERGED; }
+    if (K >= l_max) { set_error("%s: Bessel table too short", fn); return MFH_ERR_NOT_CONVERGED; }
     if (n_terms_out) *n_terms_out = K;
-    return chebyshev_series(h, psi_dev, out_dev, c, R, K, cr, ci, std::cos(c * t), -std::sin(c * t), (cudaStream_t)stream);
+    return chebyshev_series(h, psi_dev, out_dev, c, R, K, cr, ci, std::cos(c * t), -std::sin(c * t), (cudaStream_t)stream, lambdas);
+}
+
+MFH_API int mfh_chebyshev(mfh_handle h, const void* psi_dev, void* out_dev, double t, double e_min,
+                          double e_max, double tol, int32_t* n_terms_out, void* stream)
+{
+    return chebyshev_real_time("mfh_chebyshev", h, psi_dev, out_dev, t, e_min, e_max, tol, n_terms_out, stream, nullptr, false);
+}
+
+MFH_API int mfh_chebyshev_scan(mfh_handle h, const void* psi_dev, void* out_dev, double t, double e_min, double e_max,
+                               double tol, const double* lambdas_host, int32_t* n_terms_out, void* stream)
+{
+    return chebyshev_real_time("mfh_chebyshev_scan", h, psi_dev, out_dev, t, e_min, e_max, tol, n_terms_out, stream, lambdas_host, true);
 }
 
 MFH_API int mfh_chebyshev_imag(mfh_handle h, const void* psi_dev, void* out_dev, double beta, double e_min,

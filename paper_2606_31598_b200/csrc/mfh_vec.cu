@@ -176,14 +176,14 @@ __global__ void cheb_final_kernel(int64_t D, const typename Cplx<T>::type* __res
     }
 }
 
-static int vec_blocks(mfh_handle h) { return (int)std::min<int64_t>((h->D + 255) / 256, (int64_t)h->sm_count * 8); }
+static int vec_blocks(mfh_handle h) { return (int)std::min<int64_t>((h->D * h->plan.k + 255) / 256, (int64_t)h->sm_count * 8); }
 
 int launch_cheb_first(mfh_handle h, const void* psi, void* q0, void* acc, double j0, cudaStream_t st)
 {
     if (h->dtype == MFH_C128)
-        cheb_first_kernel<double><<<vec_blocks(h), 256, 0, st>>>(h->D, (const double2*)psi, (double2*)q0, (double2*)acc, j0);
+        cheb_first_kernel<double><<<vec_blocks(h), 256, 0, st>>>(h->D * h->plan.k, (const double2*)psi, (double2*)q0, (double2*)acc, j0);
     else
-        cheb_first_kernel<float><<<vec_blocks(h), 256, 0, st>>>(h->D, (const float2*)psi, (float2*)q0, (float2*)acc, j0);
+        cheb_first_kernel<float><<<vec_blocks(h), 256, 0, st>>>(h->D * h->plan.k, (const float2*)psi, (float2*)q0, (float2*)acc, j0);
     MFH_CUDA_CHECK(cudaGetLastError());
     return MFH_OK;
 }
@@ -192,10 +192,10 @@ int launch_cheb_step(mfh_handle h, const void* hq, const void* q, void* prev_dst
                      double inv_r, int first, double coef_re, double coef_im, cudaStream_t st)
 {
     if (h->dtype == MFH_C128)
-        cheb_step_kernel<double><<<vec_blocks(h), 256, 0, st>>>(h->D, (const double2*)hq, (const double2*)q, (double2*)prev_dst,
+        cheb_step_kernel<double><<<vec_blocks(h), 256, 0, st>>>(h->D * h->plan.k, (const double2*)hq, (const double2*)q, (double2*)prev_dst,
                                                                  (double2*)acc, c, inv_r, first, coef_re, coef_im);
     else
-        cheb_step_kernel<float><<<vec_blocks(h), 256, 0, st>>>(h->D, (const float2*)hq, (const float2*)q, (float2*)prev_dst,
+        cheb_step_kernel<float><<<vec_blocks(h), 256, 0, st>>>(h->D * h->plan.k, (const float2*)hq, (const float2*)q, (float2*)prev_dst,
                                                                 (float2*)acc, c, inv_r, first, coef_re, coef_im);
     MFH_CUDA_CHECK(cudaGetLastError());
     return MFH_OK;
@@ -204,9 +204,9 @@ int launch_cheb_step(mfh_handle h, const void* hq, const void* q, void* prev_dst
 int launch_cheb_final(mfh_handle h, const void* acc, void* out, double ph_re, double ph_im, cudaStream_t st)
 {
     if (h->dtype == MFH_C128)
-        cheb_final_kernel<double><<<vec_blocks(h), 256, 0, st>>>(h->D, (const double2*)acc, (double2*)out, ph_re, ph_im);
+        cheb_final_kernel<double><<<vec_blocks(h), 256, 0, st>>>(h->D * h->plan.k, (const double2*)acc, (double2*)out, ph_re, ph_im);
     else
-        cheb_final_kernel<float><<<vec_blocks(h), 256, 0, st>>>(h->D, (const float2*)acc, (float2*)out, ph_re, ph_im);
+        cheb_final_kernel<float><<<vec_blocks(h), 256, 0, st>>>(h->D * h->plan.k, (const float2*)acc, (float2*)out, ph_re, ph_im);
     MFH_CUDA_CHECK(cudaGetLastError());
     return MFH_OK;
 }

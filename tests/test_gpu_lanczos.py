@@ -85,3 +85,34 @@ def test_lanczos_argument_errors_and_c64():
     H = oracle.materialize(D, 21)
     r0, r1, _, _ = oracle.lanczos_bounds(lambda v: H @ v, psi.astype(np.complex128), m=30, margin=0.05)
     assert abs(e0 - r0) < 1e-4 and abs(e1 - r1) < 1e-4
+
+
+@pytest.mark.parametrize("dtype,mode", [("c128", "procedural"), ("c128", "full"), ("c64", "procedural"), ("c64", "full")])
+def test_coupling_scan_propagation_k_columns(dtype, mode):
+    """mfh_chebyshev_scan: k states propagated under k Hamiltonians H_v = diag(h0) + lambda_v V at once (one k-vector
+    plan, every block generated or read once per term), against the exact eigh propagator of each H_v and the
+    oracle's step-by-step series."""
+    from paper_2606_31598_b200.inputs import lambda_grid
+    D, B, k, t = 1024, 128, 4, 2.5
+    lam = lambda_grid(k)                                   # 0, 2/3, 4/3, 2
+    Psi = make_psi(D, 9, k=k, dtype=dtype)
+    h = mfh.Hamiltonian(D, B, 8, dtype, kind="diag_plus_gue", seed_h0=7)
+    h.plan(mode, k=k)
+    tol = 1e-13 if dtype == "c128" else 1e-7
+    out, K = h.chebyshev_scan(to_dev(Psi), t, -5.2, 5.2, tol, lambdas=lam)
+    out = out.cpu().numpy().astype(np.complex128)
+    V = oracle.materialize(D, 8)
+    h0 = oracle.h0_diagonal(D, 7)
+    assert K == oracle.chebyshev_n_terms(5.2 * t, tol)
+    for v in range(k):
+        Hv = np.diag(h0) + lam[v] * V
+        w, U = np.linalg.eigh(Hv)
+        assert w[0] > -5.2 and w[-1] < 5.2
+        psi_v = Psi[:, v].astype(np.complex128)
+        exact = U @ (np.exp(-1j * w * t) * (U.conj().T @ psi_v))
+        bound = 1e-11 if dtype == "c128" else 1e-4
+        assert np.linalg.norm(out[:, v] - exact) <= bound * np.linalg.norm(psi_v), v
+        if dtype == "c128":
+            ref, _ = oracle.chebyshev_propagate(lambda x: Hv @ x, psi_v, t, -5.2, 5.2, tol)
+            assert np.linalg.norm(out[:, v] - ref) <= 1e-11
+    h.destroy()
