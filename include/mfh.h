@@ -22,8 +22,12 @@
  *   - Complex numbers are interleaved (re, im); MFH_C128 = 2 x double, MFH_C64 = 2 x float.
  *   - One vector: length D.  k vectors: row-major [D][k] (the k values of a row are contiguous).
  *   - All vectors are caller-owned and 16-byte aligned; phi must not alias psi.  The cache,
- *     partial-sum workspace and Chebyshev scratch are library-owned (allocated in mfh_plan /
- *     on first mfh_chebyshev call, freed in mfh_destroy).
+ *     partial-sum workspace and the Chebyshev / Lanczos scratch are library-owned (all allocated in
+ *     mfh_plan, freed in mfh_destroy): after mfh_plan no entry point allocates device memory, so
+ *     mfh_apply and the chained drivers can be captured in a CUDA graph without a warm-up call.
+ *   - Devices: a handle lives on the CUDA device that was current in mfh_plan; every later call on it
+ *     must be made with that device current (MFH_ERR_BAD_STATE otherwise).  One process per GPU or
+ *     any number of devices per process both work: per-device kernel attributes are kept per handle.
  *   - Every function returns an int status (MFH_OK = 0); mfh_last_error() gives the message.
  *   - There is no CPU fallback: every compute entry point needs a CUDA device and fails with
  *     MFH_ERR_CUDA otherwise.
@@ -296,6 +300,11 @@ MFH_API int mfh_debug_philox(uint64_t seed, uint32_t stream_id, const uint32_t* 
  * handle's dtype to block_dev -- the same generator the fused kernel and the cache fill use.
  * Needs B fixed (mfh_create with B != 0, or after mfh_plan). */
 MFH_API int mfh_materialize_block(mfh_handle h, int32_t n, int32_t m, void* block_dev, void* stream);
+
+/* The Bessel table behind mfh_chebyshev (Jacobi-Anger coefficients, R7): J_l(x) for l = 0..l_max written to
+ * out_host (l_max + 1 doubles, host), x >= 0, by Miller's downward recurrence normalised with
+ * J_0 + 2 sum_j J_2j = 1 (valid for every x; host only, no GPU).  Errors: INVALID_ARG. */
+MFH_API int mfh_debug_bessel_j(double x, int32_t l_max, double* out_host);
 
 /* The H0 diagonal (D reals of the handle's real type) written to h0_dev. */
 MFH_API int mfh_debug_h0(mfh_handle h, void* h0_dev, void* stream);

@@ -32,7 +32,7 @@ MODES = {"auto": MFH_MODE_AUTO, "procedural": MFH_MODE_PROCEDURAL, "partial": MF
 # every symbol include/mfh.h declares (tests check that the library exports all of them)
 SYMBOLS = ["mfh_create", "mfh_plan_analytic", "mfh_plan_node_analytic", "mfh_plan", "mfh_apply", "mfh_apply_host", "mfh_apply_timed",
            "mfh_chebyshev", "mfh_chebyshev_imag", "mfh_chebyshev_scan", "mfh_chebyshev_steps", "mfh_lanczos_bounds", "mfh_destroy", "mfh_last_error", "mfh_get_plan", "mfh_debug_philox",
-           "mfh_materialize_block", "mfh_debug_h0", "mfh_debug_pipe_rates", "mfh_sb_create", "mfh_sb_plan", "mfh_sb_apply",
+           "mfh_materialize_block", "mfh_debug_h0", "mfh_debug_bessel_j", "mfh_debug_pipe_rates", "mfh_sb_create", "mfh_sb_plan", "mfh_sb_apply",
            "mfh_sb_destroy", "mfh_set_partition", "mfh_get_partition_rows", "mfh_set_exchange", "mfh_debug_read_bandwidth", "mfh_set_source_params", "mfh_set_block", "mfh_surrogate_theta_size", "mfh_surrogate_fit",
            "mfh_surrogate_predict", "mfh_surrogate_loss_grad"]
 
@@ -82,6 +82,7 @@ def lib():
     L.mfh_debug_philox.argtypes = [u64, u32, vp, vp, i64, vp, vp]
     L.mfh_materialize_block.argtypes = [vp, i32, i32, vp, vp]
     L.mfh_debug_h0.argtypes = [vp, vp, vp]
+    L.mfh_debug_bessel_j.argtypes = [dbl, i32, ctypes.POINTER(dbl)]
     L.mfh_debug_pipe_rates.argtypes = [i32, ctypes.POINTER(dbl), vp]
     L.mfh_debug_read_bandwidth.argtypes = [vp, sz, ctypes.POINTER(dbl), vp]
     L.mfh_sb_create.argtypes = [ctypes.POINTER(vp), i64, i32, i32, u64, u64, i32, vp, vp, dbl]
@@ -351,6 +352,14 @@ def debug_philox(seed: int, stream_id: int, i, j):
     words = torch.empty((n, 4), dtype=torch.int32, device="cuda")
     _check(lib().mfh_debug_philox(seed, stream_id, i.data_ptr(), j.data_ptr(), n, words.data_ptr(), _stream()))
     return words
+
+
+def bessel_j_table(x: float, l_max: int):
+    """J_l(x), l = 0..l_max, as the library's Chebyshev driver computes them (host only)."""
+    import numpy as np
+    out = (ctypes.c_double * (l_max + 1))()
+    _check(lib().mfh_debug_bessel_j(float(x), int(l_max), out))
+    return np.array(out[:])
 
 
 MIXES = {"c128_pair": 0, "c64_entry": 1, "philox": 2, "dfma31": 3}

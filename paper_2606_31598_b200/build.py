@@ -53,7 +53,6 @@ def build(force: bool = False, verbose: bool = False) -> str:
     nvcc = _nvcc()
     procs, objs = [], []
     extra = ["-Xptxas", "-v"] if verbose else []
-    extra += os.environ.get("MFH_NVCC_EXTRA", "").split()   # e.g. -DMFH_TC_TQ=8 for tuning experiments
     for s in srcs:
         o = os.path.join(obj_dir, os.path.basename(s)[:-3] + ".o")
         objs.append(o)

@@ -39,7 +39,7 @@ static int free_plan_resources(mfh_handle h)
 {
     void** ptrs[] = {&h->d_cache, &h->d_work, &h->d_h0, (void**)&h->d_cache_slot, (void**)&h->d_items,
                      (void**)&h->d_pair_items,
-                     (void**)&h->d_slot_list, (void**)&h->d_counter, &h->d_cheb, &h->d_io, &h->d_lanczos};
+                     (void**)&h->d_slot_list, (void**)&h->d_counter, &h->d_cheb, &h->d_io, &h->d_lanczos, &h->d_stage};
     for (void** p : ptrs) {
         if (*p) cudaFree(*p);
         *p = nullptr;
@@ -59,6 +59,14 @@ int ensure_gen_table(mfh_handle h, cudaStream_t st)
     }
     h->gen_ready = true;
     return MFH_OK;
+}
+
+// Scratch of the chained drivers (library-owned, allocated by mfh_plan): Chebyshev cur, prev, acc, Hq + the ping-pong
+// vector of mfh_chebyshev_steps; Lanczos v, v_prev, w + alpha[4096], beta[4096], 8 scalars and the reduction partials.
+static size_t cheb_scratch_bytes(int64_t D, int dtype, int k) { return (size_t)5 * D * k * complex_bytes(dtype); }
+static size_t lanczos_scratch_bytes(int64_t D, int dtype)
+{
+    return (size_t)3 * D * complex_bytes(dtype) + (2 * 4096 + 8 + (size_t)lz_partial_doubles()) * sizeof(double);
 }
 
 // Allocate and upload everything plan `p` needs, then fill the cache.
@@ -115,6 +123,10 @@ static int commit_plan(mfh_handle h, const Plan& p, cudaStream_t st)
     MFH_CUDA_CHECK(cudaMalloc(&h->d_counter, 2 * sizeof(int32_t)));
     MFH_CUDA_CHECK(cudaMalloc(&h->d_io, (size_t)2 * h->D * q.k * cb));
     MFH_CUDA_CHECK(cudaMemsetAsync(h->d_io, 0, (size_t)2 * h->D * q.k * cb, st));   // MFH_PART_ROWS leaves foreign rows untouched
+    // scratch of the chained drivers, allocated here so that mfh_chebyshev* / mfh_lanczos_bounds never allocate
+    // (they can be captured in a CUDA graph without a warm-up call)
+    MFH_CUDA_CHECK(cudaMalloc(&h->d_cheb, cheb_scratch_bytes(h->D, h->dtype, q.k)));
+    if (q.k == 1) MFH_CUDA_CHECK(cudaMalloc(&h->d_lanczos, lanczos_scratch_bytes(h->D, h->dtype)));
     if (h->kind == MFH_SRC_DIAG_PLUS_GUE) {
         MFH_CUDA_CHECK(cudaMalloc(&h->d_h0, (size_t)h->D * (h->dtype == MFH_C128 ? 8 : 4)));
         int rc = launch_h0(h, h->d_h0, st);
@@ -139,7 +151,11 @@ static int apply_impl(mfh_handle h, const void* psi, void* phi, const double* la
                       cudaEvent_t* ev = nullptr)
 {
     const Plan& p = h->plan;
-    int rc;
+    int rc, dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != h->device) {
+        set_error("the handle was planned on CUDA device %d, the current device is %d", h->device, dev);
+        return MFH_ERR_BAD_STATE;
+    }
     if (h->kind == MFH_SRC_EXTERNAL && h->ext_missing > 0) {
         set_error("external operator: %lld of %lld stored blocks have not been set (mfh_set_block)", (long long)h->ext_missing,
                   (long long)p.n_cached);
@@ -189,7 +205,11 @@ static int time_plan(mfh_handle h, cudaStream_t st, double& seconds)
     MFH_CUDA_CHECK(cudaMemsetAsync(psi, 0, bytes, st));   // timing does not depend on the values
     cudaEvent_t a, b;
     MFH_CUDA_CHECK(cudaEventCreate(&a));
-    MFH_CUDA_CHECK(cudaEventCreate(&b));
+    if (cudaEventCreate(&b) != cudaSuccess) {
+        cudaEventDestroy(a);
+        set_error("time_plan: cudaEventCreate failed");
+        return MFH_ERR_CUDA;
+    }
     int rc = MFH_OK;
     for (int r = 0; r < R_warm && !rc; ++r) rc = apply_impl(h, psi, phi, nullptr, st);
     cudaStreamSynchronize(st);
@@ -300,12 +320,11 @@ MFH_API int mfh_set_block(mfh_handle h, int32_t n, int32_t m, const void* block,
     if (is_device) {
         rc = launch_store_block(h, slot, block, st);
     } else if (h->dtype == MFH_C64 && p.k > 1) {
-        void* tmp = nullptr;   // tiled cache: stage on the device, then re-lay
-        MFH_CUDA_CHECK(cudaMalloc(&tmp, bytes));
-        MFH_CUDA_CHECK(cudaMemcpyAsync(tmp, block, bytes, cudaMemcpyHostToDevice, st));
-        rc = launch_store_block(h, slot, tmp, st);
-        cudaStreamSynchronize(st);
-        cudaFree(tmp);
+        // tiled cache: stage on the device (one reusable block, freed with the plan), then re-lay
+        if (!h->d_stage) MFH_CUDA_CHECK(cudaMalloc(&h->d_stage, bytes));
+        MFH_CUDA_CHECK(cudaMemcpyAsync(h->d_stage, block, bytes, cudaMemcpyHostToDevice, st));
+        rc = launch_store_block(h, slot, h->d_stage, st);
+        MFH_CUDA_CHECK(cudaStreamSynchronize(st));   // the host block and the staging block may be reused
     } else {
         MFH_CUDA_CHECK(cudaMemcpyAsync((char*)h->d_cache + (size_t)slot * bytes, block, bytes, cudaMemcpyHostToDevice, st));
         MFH_CUDA_CHECK(cudaStreamSynchronize(st));   // the host block may be reused by the caller
@@ -413,6 +432,19 @@ MFH_API int mfh_plan(mfh_handle h, int32_t mode, int32_t k, int64_t n_applies_hi
     MFH_CUDA_CHECK(cudaGetDevice(&dev));
     MFH_CUDA_CHECK(cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev));
     free_plan_resources(h);   // a re-plan may reuse the memory of the previous plan
+    if (dev != h->device) {   // the generator table and the kernel attributes belong to the previous device
+        if (h->d_gen_tab) cudaFree(h->d_gen_tab);
+        h->d_gen_tab = nullptr;
+        h->gen_ready = false;
+        h->smem_attr.clear();
+        h->device = dev;
+    }
+    if (h->part_world > 1 && h->B_req == 0) {
+        // block ownership is defined in block indices: ranks that picked different B would own sets that do not tile H
+        set_error("mfh_plan: a partitioned handle (world %d) needs the block size fixed in mfh_create (B != 0): every "
+                  "rank must plan the same B", h->part_world);
+        return MFH_ERR_INVALID_ARG;
+    }
     size_t free_b = 0, total_b = 0;
     MFH_CUDA_CHECK(cudaMemGetInfo(&free_b, &total_b));
     double budget = hbm_budget_bytes > 0 ? (double)hbm_budget_bytes : planner_alpha() * (double)free_b;
@@ -467,6 +499,11 @@ MFH_API int mfh_plan(mfh_handle h, int32_t mode, int32_t k, int64_t n_applies_hi
         }
     }
     if (h->kind == MFH_SRC_EXTERNAL && cands[0].cached_fraction < 1.0) {
+        if (mode == MFH_MODE_PAIRS && part.world > 1 && part.scheme == MFH_PART_ROWS) {
+            set_error("mfh_plan: an external pair cache cannot be partitioned by rows (a pair split between two ranks is "
+                      "stored by neither and nothing can be generated); use MFH_PART_PAIRS or MFH_MODE_FULL");
+            return MFH_ERR_UNSUPPORTED;
+        }
         set_error("mfh_plan: the external operator does not fit the budget as a %s cache", mode == MFH_MODE_PAIRS ? "pair" : "full");
         return MFH_ERR_OUT_OF_MEMORY;
     }
@@ -525,7 +562,12 @@ MFH_API int mfh_apply_timed(mfh_handle h, const void* psi_dev, void* phi_dev, in
     if (k != h->plan.k) { set_error("mfh_apply_timed: k mismatch"); return MFH_ERR_INVALID_ARG; }
     cudaStream_t st = (cudaStream_t)stream;
     cudaEvent_t ev[4];
-    for (auto& e : ev) MFH_CUDA_CHECK(cudaEventCreate(&e));
+    for (int i = 0; i < 4; ++i)
+        if (cudaEventCreate(&ev[i]) != cudaSuccess) {
+            while (i-- > 0) cudaEventDestroy(ev[i]);
+            set_error("mfh_apply_timed: cudaEventCreate failed");
+            return MFH_ERR_CUDA;
+        }
     int rc = apply_impl(h, psi_dev, phi_dev, lambdas_host, st, ev);
     cudaError_t e = cudaStreamSynchronize(st);
     if (!rc && e == cudaSuccess) {
@@ -563,7 +605,6 @@ static int chebyshev_series(mfh_handle h, const void* psi_dev, void* out_dev, do
                             double ph_im, cudaStream_t st, const double* lambdas = nullptr)
 {
     const size_t vb = (size_t)h->D * h->plan.k * complex_bytes(h->dtype);   // k columns: the O(D) updates are element-wise
-    if (!h->d_cheb) MFH_CUDA_CHECK(cudaMalloc(&h->d_cheb, 5 * vb));   // cur, prev, acc, Hq + ping-pong of mfh_chebyshev_steps
     char* base = (char*)h->d_cheb;
     void *cur = base, *prev = base + vb, *acc = base + 2 * vb, *hq = base + 3 * vb;
     int rc;
@@ -589,20 +630,51 @@ static int chebyshev_check(const char* fn, mfh_handle h, const void* psi_dev, co
     return MFH_OK;
 }
 
+// J_l(x), l = 0..l_max, x >= 0, by downward recurrence J_{l-1} = (2l/x) J_l - J_{l+1} started far above both l_max
+// and x (where J is negligible) and normalised with J_0 + 2 sum_{j>=1} J_{2j} = 1.  Stable for every x: the
+// recurrence is followed in its growing direction.  (std::cyl_bessel_j switches to an asymptotic form that is wrong
+// for x > 1000 at large order: J_500(1001) came out as -4e33.)
+static void bessel_j_table(double x, int l_max, std::vector<double>& J)
+{
+    J.assign((size_t)l_max + 1, 0.0);
+    if (x == 0.0) { J[0] = 1.0; return; }
+    int start = std::max(l_max, (int)x) + 40 + (int)(12.0 * std::cbrt(std::max(x, 1.0)));
+    start += start & 1;                                      // even
+    double jp = 0.0, jc = 1e-300, norm = 0.0;                // J_{start+1}, J_start (arbitrary scale)
+    std::vector<double> raw((size_t)l_max + 1, 0.0);
+    for (int l = start; l >= 0; --l) {
+        // jc = J_l (scaled)
+        if (l <= l_max) raw[l] = jc;
+        if (l == 0) norm += jc;
+        else if ((l & 1) == 0) norm += 2.0 * jc;
+        if (l > 0) {
+            const double jm = (2.0 * l / x) * jc - jp;       // J_{l-1}
+            jp = jc;
+            jc = jm;
+            if (std::fabs(jc) > 1e250) {                     // rescale before overflow
+                jc *= 1e-250; jp *= 1e-250; norm *= 1e-250;
+                for (double& r : raw) r *= 1e-250;
+            }
+        }
+    }
+    for (int l = 0; l <= l_max; ++l) J[l] = raw[l] / norm;
+}
+
 static int chebyshev_real_time(const char* fn, mfh_handle h, const void* psi_dev, void* out_dev, double t, double e_min,
                                double e_max, double tol, int32_t* n_terms_out, void* stream, const double* lambdas, bool any_k)
 {
     int rc = chebyshev_check(fn, h, psi_dev, out_dev, t, e_min, e_max, tol, any_k);
     if (rc) return rc;
     const double c = 0.5 * (e_max + e_min), R = 0.5 * (e_max - e_min), a = R * t;
-    // Bessel table J_l(a) via the C++17 special function (a route different from the oracle's
-    // Miller recurrence), K = 1 + last l with |J_l| >= tol.
+    // Bessel table J_l(|a|), l = 0..l_max (bessel_j_table below), K = 1 + last l with |J_l| >= tol.
     const double x = std::fabs(a);
     const int l_max = (int)(x + 80.0 + 12.0 * std::cbrt(x));
-    std::vector<double> cr(l_max + 1, 0.0), ci(l_max + 1, 0.0);
+    std::vector<double> cr(l_max + 1, 0.0), ci(l_max + 1, 0.0), J;
+    bessel_j_table(x, l_max, J);
     int K = 1;
     for (int l = 0; l <= l_max; ++l) {
-        double v = (x == 0.0) ? (l == 0 ? 1.0 : 0.0) : std::cyl_bessel_j((double)l, x);
+        double v = J[l];
+        if (!std::isfinite(v)) { set_error("%s: Bessel coefficient J_%d(%g) is not finite", fn, l, x); return MFH_ERR_NOT_CONVERGED; }
         if (a < 0 && (l & 1)) v = -v;
         if (std::fabs(v) >= tol) K = l + 1;
         if (l == 0) { cr[0] = v; continue; }
@@ -702,8 +774,6 @@ MFH_API int mfh_lanczos_bounds(mfh_handle h, const void* psi_dev, int32_t m, dou
     cudaStream_t st = (cudaStream_t)stream;
     m = (int32_t)std::min<int64_t>(m, h->D);
     const size_t vb = (size_t)h->D * complex_bytes(h->dtype);
-    const size_t scal_doubles = 2 * 4096 + 8 + (size_t)lz_partial_doubles();
-    if (!h->d_lanczos) MFH_CUDA_CHECK(cudaMalloc(&h->d_lanczos, 3 * vb + scal_doubles * sizeof(double)));
     char* base = (char*)h->d_lanczos;
     void *v = base, *v_prev = base + vb, *w = base + 2 * vb;
     double* d_alpha = (double*)(base + 3 * vb);
@@ -774,6 +844,10 @@ MFH_API int mfh_debug_philox(uint64_t seed, uint32_t stream_id, const uint32_t* 
 MFH_API int mfh_materialize_block(mfh_handle h, int32_t n, int32_t m, void* block_dev, void* stream)
 {
     if (!h || !block_dev) { set_error("mfh_materialize_block: NULL pointer"); return MFH_ERR_INVALID_ARG; }
+    if (h->kind == MFH_SRC_EXTERNAL) {
+        set_error("mfh_materialize_block: an external operator has no generator (its blocks are the caller's, mfh_set_block)");
+        return MFH_ERR_UNSUPPORTED;
+    }
     const int32_t B = h->planned ? h->plan.B : h->B_req;
     if (B <= 0) { set_error("mfh_materialize_block: block size not fixed yet"); return MFH_ERR_BAD_STATE; }
     const int32_t n_blk = (int32_t)(h->D / B);
@@ -782,6 +856,18 @@ MFH_API int mfh_materialize_block(mfh_handle h, int32_t n, int32_t m, void* bloc
         return MFH_ERR_INVALID_ARG;
     }
     return launch_fill_block(h, B, n, m, block_dev, (cudaStream_t)stream);
+}
+
+MFH_API int mfh_debug_bessel_j(double x, int32_t l_max, double* out_host)
+{
+    if (!out_host || l_max < 0 || l_max > (1 << 24) || !(x >= 0.0) || !std::isfinite(x)) {
+        set_error("mfh_debug_bessel_j: need x >= 0 finite, 0 <= l_max <= 2^24, out != NULL");
+        return MFH_ERR_INVALID_ARG;
+    }
+    std::vector<double> J;
+    bessel_j_table(x, l_max, J);
+    memcpy(out_host, J.data(), ((size_t)l_max + 1) * sizeof(double));
+    return MFH_OK;
 }
 
 MFH_API int mfh_debug_h0(mfh_handle h, void* h0_dev, void* stream)

@@ -8,7 +8,6 @@
 // C2: 7.48 TB/s; 2 rows x 4 loads 7.39, 2 x 8 7.33, 1 x 8 7.37, 4 x 4 7.48 at 124 registers); psi^[m]
 // is staged once per CTA per column block in shared memory and shared by all warps.
 #include <algorithm>
-#include <cstdlib>
 #include "mfh_internal.cuh"
 
 namespace mfh {
@@ -37,16 +36,10 @@ template <typename T> struct CachedParams {
     typename Cplx<T>::type* work;
 };
 
-#ifndef MFH_CACHED_RPW
-#define MFH_CACHED_RPW 4
-#endif
-#ifndef MFH_CACHED_U
-#define MFH_CACHED_U 2
-#endif
 constexpr int CACHED_WARPS = 8;
-constexpr int CACHED_RPW = MFH_CACHED_RPW;            // rows per warp
+constexpr int CACHED_RPW = 4;                         // rows per warp
 constexpr int CACHED_ROWS = CACHED_WARPS * CACHED_RPW;
-constexpr int CACHED_U = MFH_CACHED_U;                // independent loads per row per lane
+constexpr int CACHED_U = 2;                           // independent loads per row per lane
 
 // ---- complex128: one 16-byte load = one entry ----
 __global__ void __launch_bounds__(32 * CACHED_WARPS) cached_kernel_c128(const CachedParams<double> P)
@@ -176,12 +169,6 @@ __global__ void __launch_bounds__(32 * CACHED_WARPS) cached_kernel_c64(const Cac
 // broadcasts.  Output: the partial slot of column block m, as the other k-vector kernels.
 // --------------------------------------------------------------------------------------------
 constexpr int CM_ROWS = 128, CM_COLS = 16, CM_PAD = CM_COLS + 1;
-#ifndef MFH_CM_VS16
-#define MFH_CM_VS16 2
-#endif
-#ifndef MFH_CM_VS8
-#define MFH_CM_VS8 1
-#endif
 
 struct CachedMultiParams {
     int32_t B, n_blk, k, slot_multi;
@@ -279,11 +266,7 @@ template <int KT, int VS> static int launch_cached_multi_c128_t(mfh_handle h, co
                         (const double2*)psi, (double2*)h->d_work};
     const size_t smem = (size_t)(2 * CM_ROWS * CM_PAD + 2 * CM_COLS * KT) * sizeof(double2);
     auto kern = cached_multi_kernel_c128<KT, VS>;
-    static bool attr_done = false;
-    if (!attr_done) {
-        MFH_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_done = true;
-    }
+    if (int rc = ensure_dyn_smem(h, kern, (int)smem)) return rc;
     kern<<<dim3((unsigned)(h->D / CM_ROWS), p.n_blk), CM_ROWS * VS, smem, st>>>(P);
     MFH_CUDA_CHECK(cudaGetLastError());
     return MFH_OK;
@@ -294,8 +277,8 @@ static int launch_cached_multi_c128(mfh_handle h, const void* psi, cudaStream_t 
     const int k = h->plan.k;
     if (k <= 2) return launch_cached_multi_c128_t<2, 1>(h, psi, st);
     if (k <= 4) return launch_cached_multi_c128_t<4, 1>(h, psi, st);
-    if (k <= 8) return launch_cached_multi_c128_t<8, MFH_CM_VS8>(h, psi, st);
-    return launch_cached_multi_c128_t<16, MFH_CM_VS16>(h, psi, st);
+    if (k <= 8) return launch_cached_multi_c128_t<8, 1>(h, psi, st);
+    return launch_cached_multi_c128_t<16, 2>(h, psi, st);
 }
 
 int launch_cached(mfh_handle h, const void* psi, cudaStream_t st)
@@ -309,19 +292,13 @@ int launch_cached(mfh_handle h, const void* psi, cudaStream_t st)
         return MFH_ERR_UNSUPPORTED;
     }
     const unsigned grid = (unsigned)(h->D / CACHED_ROWS);
-    static bool attr_done = false;
-    if (!attr_done) {
-        MFH_CUDA_CHECK(cudaFuncSetAttribute(cached_kernel_c128, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                            MFH_MAX_B * 16));
-        MFH_CUDA_CHECK(cudaFuncSetAttribute(cached_kernel_c64, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                            MFH_MAX_B * 8));
-        attr_done = true;
-    }
     if (h->dtype == MFH_C128) {
+        if (int rc = ensure_dyn_smem(h, cached_kernel_c128, MFH_MAX_B * 16)) return rc;
         CachedParams<double> P{p.B, p.n_blk, p.slot_cache, h->D, h->d_cache_slot,
                                (const double2*)h->d_cache, (const double2*)psi, (double2*)h->d_work};
         cached_kernel_c128<<<grid, 32 * CACHED_WARPS, (size_t)p.B * 16, st>>>(P);
     } else {
+        if (int rc = ensure_dyn_smem(h, cached_kernel_c64, MFH_MAX_B * 8)) return rc;
         CachedParams<float> P{p.B, p.n_blk, p.slot_cache, h->D, h->d_cache_slot,
                               (const float2*)h->d_cache, (const float2*)psi, (float2*)h->d_work};
         cached_kernel_c64<<<grid, 32 * CACHED_WARPS, (size_t)p.B * 8, st>>>(P);

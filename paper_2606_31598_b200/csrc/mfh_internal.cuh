@@ -3,6 +3,7 @@
 #include <cstdint>
 #include <cstdio>
 #include <string>
+#include <utility>
 #include <vector>
 #include <cuda_runtime.h>
 
@@ -101,6 +102,11 @@ struct mfh_handle_s {
     mfh::GenTabD* d_gen_tab = nullptr;   // device copy (c128 only), kept until mfh_destroy
     bool gen_ready = false;
     int sm_count = 148;
+    int device = -1;                // the CUDA device the plan lives on (set by mfh_plan)
+    // kernels whose cudaFuncAttributeMaxDynamicSharedMemorySize has been raised on `device` for this handle: the
+    // attribute is per device, so it is remembered per handle, not per process
+    std::vector<std::pair<const void*, int>> smem_attr;
+    void* d_stage = nullptr;        // mfh_set_block: one reusable B x B staging block (tiled caches)
 };
 
 namespace mfh {
@@ -122,6 +128,17 @@ size_t complex_bytes(int dtype);
             return MFH_ERR_CUDA;                                                               \
         }                                                                                      \
     } while (0)
+
+// Raise the dynamic shared-memory limit of `kernel` to `bytes` on the handle's device (once per handle and kernel).
+template <typename K> inline int ensure_dyn_smem(mfh_handle h, K kernel, int bytes)
+{
+    const void* f = reinterpret_cast<const void*>(kernel);
+    for (const auto& e : h->smem_attr)
+        if (e.first == f && e.second >= bytes) return MFH_OK;
+    MFH_CUDA_CHECK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    h->smem_attr.push_back({f, bytes});
+    return MFH_OK;
+}
 
 int ensure_gen_table(mfh_handle h, cudaStream_t st);   // mfh_api.cu: build + upload once per handle
 

@@ -274,10 +274,11 @@ void build_tables(Plan& p, int64_t D, int dtype, int sm_count)
     else p.mode = (covered == p.owned_blocks ? MFH_MODE_FULL : MFH_MODE_PARTIAL);
 }
 
-// Scratch outside the partial slots: Chebyshev (3 vectors), host-apply staging (2 k vectors), H0.
+// Scratch outside the partial slots: Chebyshev (5 k vectors), host-apply staging (2 k vectors), Lanczos (3 vectors
+// + 80 KB of scalars, k = 1 plans), H0.
 static size_t fixed_work_bytes(int64_t D, int dtype, int k)
 {
-    return (size_t)D * complex_bytes(dtype) * (3 + 2 * k) + (size_t)D * 8;
+    return (size_t)D * complex_bytes(dtype) * (7 * k + (k == 1 ? 3 : 0)) + (size_t)D * 8 + (k == 1 ? 81920 : 0);
 }
 
 Candidate evaluate_candidate(int64_t D, int dtype, int k, int B, int cached_per_row, bool pairs,

@@ -2,7 +2,6 @@
 // H0 diagonal, and the fused generate-and-apply kernels (single vector with Hermitian reuse,
 // k vectors one-sided).  PAPER.md Eq. 7, Eq. 8, Eq. 11.
 #include <algorithm>
-#include <cstdlib>
 #include "mfh_internal.cuh"
 
 namespace mfh {
@@ -455,12 +454,7 @@ static int launch_proc_single_t(mfh_handle h, const void* psi, cudaStream_t st)
     const size_t smem = smem_for(p.B);
     const bool analytic = (h->kind == MFH_SRC_ANALYTIC);
     auto kern = analytic ? proc_single_kernel<T, R, SRC_ANALYTIC> : proc_single_kernel<T, R, SRC_SEEDED>;
-    static bool attr_done[2] = {false, false};
-    if (!attr_done[analytic]) {
-        MFH_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                            (int)smem_for(MFH_MAX_B)));
-        attr_done[analytic] = true;
-    }
+    if (int rc = ensure_dyn_smem(h, kern, (int)smem_for(MFH_MAX_B))) return rc;
     int per_sm = 1;
     MFH_CUDA_CHECK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, PROC_THREADS, smem));
     if (per_sm < 1) per_sm = 1;
@@ -487,8 +481,7 @@ int launch_proc_single(mfh_handle h, const void* psi, cudaStream_t st)
 bool partial_overlap_supported(mfh_handle h)
 {
     const Plan& p = h->plan;
-    static const bool off = getenv("MFH_PARTIAL_SEQUENTIAL") != nullptr;   // A/B measurements
-    return !off && h->kind != MFH_SRC_ANALYTIC && h->dtype == MFH_C128 && p.k == 1 && !p.pairs && p.n_cached > 0 && !p.items.empty() &&
+    return h->kind != MFH_SRC_ANALYTIC && h->dtype == MFH_C128 && p.k == 1 && !p.pairs && p.n_cached > 0 && !p.items.empty() &&
            h->D % STRIP_ROWS == 0 && p.B % STRIP_ROWS == 0;
 }
 
@@ -522,11 +515,7 @@ template <int R> static int launch_partial_overlap_t(mfh_handle h, const void* p
     };
     const size_t smem = smem_for(p.B);
     auto kern = partial_overlap_kernel<R>;
-    static bool attr_done = false;
-    if (!attr_done) {
-        MFH_CUDA_CHECK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_for(MFH_MAX_B)));
-        attr_done = true;
-    }
+    if (int rc = ensure_dyn_smem(h, kern, (int)smem_for(MFH_MAX_B))) return rc;
     int per_sm = 1;
     MFH_CUDA_CHECK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, PROC_THREADS, smem));
     if (per_sm < 1) per_sm = 1;
@@ -646,10 +635,8 @@ static int launch_proc_multi_t(mfh_handle h, const void* psi, cudaStream_t st)
 
 int launch_proc_multi(mfh_handle h, const void* psi, cudaStream_t st)
 {
-    // complex64, B % 128 == 0: tensor-core kernel (mfh_tc.cu).  MFH_MULTI_FFMA=1 keeps the CUDA-core
-    // kernel for A/B measurements.
-    static const bool force_ffma = getenv("MFH_MULTI_FFMA") != nullptr;
-    if (!force_ffma && tc_multi_supported(h)) return launch_proc_multi_tc(h, psi, st);
+    // complex64, B % 128 == 0: tensor-core kernel (mfh_tc.cu)
+    if (tc_multi_supported(h)) return launch_proc_multi_tc(h, psi, st);
     const int k = h->plan.k;
     const bool f64 = (h->dtype == MFH_C128);
     if (k <= 2) return f64 ? launch_proc_multi_t<double, 2>(h, psi, st) : launch_proc_multi_t<float, 2>(h, psi, st);

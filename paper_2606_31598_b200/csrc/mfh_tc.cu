@@ -20,7 +20,6 @@
 // reads the accumulator with tcgen05.ld and writes the partial slot of column block m (added in
 // index order by the reduce kernel).
 #include <algorithm>
-#include <cstdlib>
 #include "mfh_internal.cuh"
 
 namespace mfh {
@@ -28,13 +27,7 @@ namespace mfh {
 constexpr int TC_GEN_WARPS = 8;               // generator warps; warp 8 builds the B operands and issues the MMAs
 constexpr int TC_THREADS = 32 * (TC_GEN_WARPS + 1);
 constexpr int TC_TP = 128;                    // rows per CTA = MMA M
-#ifndef MFH_TC_TQ
-#define MFH_TC_TQ 16
-#endif
-#ifndef MFH_TC_MINB
-#define MFH_TC_MINB 2
-#endif
-constexpr int TC_TQ = MFH_TC_TQ;              // columns per tile = TQ/8 MMA K-steps
+constexpr int TC_TQ = 16;                     // columns per tile = TQ/8 MMA K-steps
 constexpr int TC_NG = TC_TQ / 8;              // 4-column groups per generator thread and tile
 constexpr int TC_N = 32;                      // MMA N: 16 vectors x (re, im)
 constexpr int TC_B_TILE = TC_N * TC_TQ * 4;   // bytes of one B operand image in shared memory (2 KB)
@@ -264,7 +257,7 @@ __device__ __forceinline__ void tc_mma_warp(const TcParams& P, unsigned char* sm
     }
 }
 
-__global__ void __launch_bounds__(TC_THREADS, MFH_TC_MINB) proc_multi_tc_kernel(const TcParams P)
+__global__ void __launch_bounds__(TC_THREADS, 2) proc_multi_tc_kernel(const TcParams P)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     __shared__ __align__(8) uint64_t full[TC_STAGES], empty[TC_STAGES], done;
@@ -331,11 +324,7 @@ int launch_proc_multi_tc(mfh_handle h, const void* psi, cudaStream_t st)
     P.psi = (const float2*)psi;
     P.work = (float2*)h->d_work;
     const size_t smem = (size_t)TC_STAGES * TC_STAGE;
-    static bool attr_done = false;
-    if (!attr_done) {
-        MFH_CUDA_CHECK(cudaFuncSetAttribute(proc_multi_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_done = true;
-    }
+    if (int rc = ensure_dyn_smem(h, proc_multi_tc_kernel, (int)smem)) return rc;
     proc_multi_tc_kernel<<<dim3((unsigned)(h->D / TC_TP), p.n_blk), TC_THREADS, smem, st>>>(P);
     MFH_CUDA_CHECK(cudaGetLastError());
     return MFH_OK;
@@ -556,11 +545,7 @@ int launch_cached_multi_tc(mfh_handle h, const void* psi, cudaStream_t st)
     P.cache = (const float2*)h->d_cache;
     P.psi = (const float2*)psi;
     P.work = (float2*)h->d_work;
-    static bool attr_done = false;
-    if (!attr_done) {
-        MFH_CUDA_CHECK(cudaFuncSetAttribute(cached_multi_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, CT_SMEM));
-        attr_done = true;
-    }
+    if (int rc = ensure_dyn_smem(h, cached_multi_tc_kernel, CT_SMEM)) return rc;
     cached_multi_tc_kernel<<<dim3((unsigned)(h->D / TC_TP), p.n_blk), CT_THREADS, CT_SMEM, st>>>(P);
     MFH_CUDA_CHECK(cudaGetLastError());
     return MFH_OK;

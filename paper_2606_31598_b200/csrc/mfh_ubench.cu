@@ -73,8 +73,11 @@ static int run_mix(int sm_count, cudaStream_t st, double* units_per_s)
     uint32_t* out = nullptr;
     MFH_CUDA_CHECK(cudaMalloc(&out, (size_t)grid * UB_THREADS * sizeof(uint32_t)));
     cudaEvent_t e0, e1;
-    MFH_CUDA_CHECK(cudaEventCreate(&e0));
-    MFH_CUDA_CHECK(cudaEventCreate(&e1));
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) {
+        cudaFree(out);
+        set_error("pipe-rate microbenchmark: cudaEventCreate failed");
+        return MFH_ERR_CUDA;
+    }
     float best = 1e30f;
     for (int rep = 0; rep < 4; ++rep) {   // first repetition warms up
         cudaEventRecord(e0, st);
@@ -84,6 +87,8 @@ static int run_mix(int sm_count, cudaStream_t st, double* units_per_s)
         float ms = 0.f;
         cudaEventElapsedTime(&ms, e0, e1);
         if (e != cudaSuccess || cudaGetLastError() != cudaSuccess) {
+            cudaEventDestroy(e0);
+            cudaEventDestroy(e1);
             cudaFree(out);
             set_error("pipe-rate microbenchmark failed: %s", cudaGetErrorString(e));
             return MFH_ERR_CUDA;
@@ -141,8 +146,11 @@ extern "C" MFH_API int mfh_debug_read_bandwidth(const void* buf_dev, size_t byte
     uint32_t* out = nullptr;
     MFH_CUDA_CHECK(cudaMalloc(&out, (size_t)grid * 256 * sizeof(uint32_t)));
     cudaEvent_t e0, e1;
-    MFH_CUDA_CHECK(cudaEventCreate(&e0));
-    MFH_CUDA_CHECK(cudaEventCreate(&e1));
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) {
+        cudaFree(out);
+        set_error("mfh_debug_read_bandwidth: cudaEventCreate failed");
+        return MFH_ERR_CUDA;
+    }
     float best = 1e30f;
     cudaError_t e = cudaSuccess;
     for (int rep = 0; rep < 4 && e == cudaSuccess; ++rep) {   // first repetition warms up

@@ -65,6 +65,21 @@ def sample_rows(D: int, n: int, seed: int = 0) -> np.ndarray:
     return np.unique(np.concatenate([fixed, rand]))
 
 
+def stratified_rows(D: int, B: int, n_min: int = 8192, tile: int = 128) -> np.ndarray:
+    """Row sample for full-size parity that provably covers the kernels' decomposition: every `tile`-row tile of the
+    operator contributes S = ceil(n_min / (D / tile)) rows at residues (37 t + s * (tile // S)) mod tile (t = tile
+    index, s = 0..S-1), so every tile, hence every block row, every residue mod `tile` (every (lane, row-in-lane)
+    position of a 32 x 4 row tile) and every warp's strip is hit; plus the first and last row of every block.  Sorted,
+    unique, deterministic (no random numbers)."""
+    n_tiles = D // tile
+    S = min(tile, max(1, -(-n_min // n_tiles)))
+    t = np.arange(n_tiles, dtype=np.int64)[:, None]
+    s = np.arange(S, dtype=np.int64)[None, :]
+    rows = (t * tile + (37 * t + s * (tile // S)) % tile).ravel()
+    blocks = np.arange(D // B, dtype=np.int64) * B
+    return np.unique(np.concatenate([rows, blocks, blocks + B - 1]))
+
+
 def dense_matrix(D: int, seed: int, hermitian: bool = True) -> np.ndarray:
     """Seeded dense D x D complex matrix with O(1/sqrt(D)) entries: the externally stored operator of the Eq. 10
     tests (an input of the method, not part of its arithmetic)."""

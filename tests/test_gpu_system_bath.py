@@ -1,12 +1,12 @@
 """GPU parity of the NEXT-3 widening: the system-bath Hamiltonian action -- two dense
 bath-side operators on R = d_S state components -- against the oracle, at small size element by
-element and at the paper's size (18 qubits: d_S = 4, d_B = 65536, complex64, cached) on sampled rows."""
+element (the paper's size, 18 qubits, is covered in test_gpu_fullsize.py)."""
 import numpy as np
 import pytest
 
 import oracle
 from paper_2606_31598_b200 import binding as mfh
-from paper_2606_31598_b200.inputs import SYSTEM_BATH, make_psi, sample_rows, small_hermitian
+from paper_2606_31598_b200.inputs import make_psi, small_hermitian
 
 pytestmark = pytest.mark.gpu
 
@@ -45,23 +45,3 @@ def test_system_bath_rejects_non_hermitian_system_operators():
     with pytest.raises(mfh.MfhError) as e:
         mfh.SystemBath(1024, 2, 256, 1, 2, M, M.conj().T @ M, 0.1)
     assert e.value.code == mfh.MFH_ERR_INVALID_ARG
-
-
-def test_system_bath_paper_size_sampled_rows():
-    import torch
-    c = SYSTEM_BATH
-    if torch.cuda.mem_get_info()[0] < 80e9:
-        pytest.skip("needs 69 GB of free HBM")
-    d_B, d_S, B = c["d_B"], c["d_S"], c["B"]
-    H_S, A = small_hermitian(d_S, c["seed_HS"]), small_hermitian(d_S, c["seed_A"])
-    X = make_psi(d_B, c["psi_seed"], k=d_S, dtype="c64")
-    sb = mfh.SystemBath(d_B, d_S, B, c["seed_HB"], c["seed_B1"], H_S, A, c["g"], dtype="c64")
-    plan = sb.plan("full")
-    assert plan["H_B"]["cache_bytes"] == 8 * d_B**2 == 32 * 2**30          # 32 GiB per operator
-    assert plan["flops_per_apply"] == pytest.approx(2.749e11, rel=1e-3)      # 2 * 4 * 65536^2 * 8
-    Y = sb.apply(to_dev(X)).cpu().numpy()
-    rows = sample_rows(d_B, 100)
-    ref = oracle.sb_apply(d_B, B, c["seed_HB"], c["seed_B1"], H_S, A, c["g"], X, rows=rows)
-    for s in range(d_S):
-        assert rel_l2(Y[rows, s], ref[:, s]) <= 1e-4, s
-    sb.destroy()

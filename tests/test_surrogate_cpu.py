@@ -98,3 +98,40 @@ def test_surrogate_trained_on_the_shipped_b200_log_ranks_a_held_out_size():
     assert rep["train_records"] == 192 and rep["test_records"] == 48
     assert rep["test_rms_log_error"] < 0.35 < float(np.std(np.log(t)))
     assert max(p["regret"] for p in rep["problems"]) < 1.25
+
+
+def _hand_case():
+    import os
+    vals = {}
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "surrogate_hand.txt")):
+        if line.strip() and not line.startswith("#"):
+            name, v = line.split()
+            vals[name] = float(v)
+    # theta = [mu | sigma | W1 (F x H) | b1 | W2 | b2] for F = 2, H = 1 (the case worked out in the golden file)
+    theta = np.array([1.0, 2.0, 2.0, 0.5, 0.5, -1.0, 0.25, 2.0, -0.5])
+    X = np.array([[3.0, 2.25], [-1.0, 2.5]])
+    t = np.array([np.e, np.exp(-2.0)])
+    return vals, theta, X, t
+
+
+def test_oracle_surrogate_matches_the_hand_worked_case():
+    """Pin of oracle/surrogate.py (Eq. 24-26) on numbers worked out by hand in tests/golden/surrogate_hand.txt: a
+    transposed W1, a missing normalisation, a dropped bias or a loss without the 1/N would each miss them."""
+    vals, theta, X, t = _hand_case()
+    f = orc.f_theta(theta, 2, 1, X)
+    assert f[0] == pytest.approx(vals["f_1"], rel=1e-14) and f[1] == pytest.approx(vals["f_2"], rel=1e-14)
+    p = orc.predict(theta, 2, 1, X)
+    assert p[0] == pytest.approx(vals["t_nn_1"], rel=1e-14) and p[1] == pytest.approx(vals["t_nn_2"], rel=1e-14)
+    assert orc.loss(theta, 2, 1, X, t) == pytest.approx(vals["loss"], rel=1e-14)
+    # asymmetric F x H: with H = 2 the second hidden unit sees only feature 2 (W1 row-major [F][H])
+    th2 = np.array([0.0, 0.0, 1.0, 1.0, 1.0, 0.0, 0.0, 1.0, 0.0, 0.0, 1.0, 10.0, 0.0])   # W1 = [[1, 0], [0, 1]], W2 = (1, 10)
+    x = np.array([[0.5, -0.25]])
+    assert orc.f_theta(th2, 2, 2, x)[0] == pytest.approx(np.tanh(0.5) + 10.0 * np.tanh(-0.25), rel=1e-15)
+
+
+def test_library_surrogate_matches_the_hand_worked_case():
+    vals, theta, X, t = _hand_case()
+    p = sur.predict(theta, X, hidden=1)
+    assert p[0] == pytest.approx(vals["t_nn_1"], rel=1e-14) and p[1] == pytest.approx(vals["t_nn_2"], rel=1e-14)
+    loss, _ = sur.loss_grad(theta, X, t, hidden=1)
+    assert loss == pytest.approx(vals["loss"], rel=1e-14)
