@@ -245,6 +245,9 @@ MFH_API int mfh_chebyshev_steps(mfh_handle h, const void* psi_dev, void* out_dev
  *                   full-length partial phi (the H0 term on the rank that owns block (n,n));
  *                   exchange = all-reduce (sum).
  *   MFH_PART_NONE   single GPU (world must be 1).
+ * Block ownership is defined in block indices, so every rank must plan the SAME block size: with world > 1
+ * mfh_plan refuses a handle created with B = 0 (MFH_ERR_INVALID_ARG) -- fix B in mfh_create on every rank
+ * (paper_2606_31598_b200/distributed.py also compares the planned (B, n_blk, k) of all ranks).
  * mfh_chebyshev / mfh_chebyshev_steps / mfh_lanczos_bounds chain applies, so on a partitioned handle they
  * call the exchange hook registered with mfh_set_exchange after every apply (MFH_ERR_BAD_STATE if none).
  * Errors: INVALID_ARG (rank outside [0, world), world < 1, unknown scheme, world > 1 with MFH_PART_NONE). */

@@ -415,6 +415,12 @@ MFH_API int mfh_plan(mfh_handle h, int32_t mode, int32_t k, int64_t n_applies_hi
         set_error("mfh_plan: invalid argument (k=%d, mode=%d)", k, mode);
         return MFH_ERR_INVALID_ARG;
     }
+    if (h->part_world > 1 && h->B_req == 0) {
+        // block ownership is defined in block indices: ranks that picked different B would own sets that do not tile H
+        set_error("mfh_plan: a partitioned handle (world %d) needs the block size fixed in mfh_create (B != 0): every "
+                  "rank must plan the same B", h->part_world);
+        return MFH_ERR_INVALID_ARG;
+    }
     if (h->kind == MFH_SRC_EXTERNAL) {
         if (mode == MFH_MODE_AUTO) mode = MFH_MODE_FULL;
         if (mode != MFH_MODE_FULL && mode != MFH_MODE_PAIRS) {
@@ -439,12 +445,7 @@ MFH_API int mfh_plan(mfh_handle h, int32_t mode, int32_t k, int64_t n_applies_hi
         h->smem_attr.clear();
         h->device = dev;
     }
-    if (h->part_world > 1 && h->B_req == 0) {
-        // block ownership is defined in block indices: ranks that picked different B would own sets that do not tile H
-        set_error("mfh_plan: a partitioned handle (world %d) needs the block size fixed in mfh_create (B != 0): every "
-                  "rank must plan the same B", h->part_world);
-        return MFH_ERR_INVALID_ARG;
-    }
+
     size_t free_b = 0, total_b = 0;
     MFH_CUDA_CHECK(cudaMemGetInfo(&free_b, &total_b));
     double budget = hbm_budget_bytes > 0 ? (double)hbm_budget_bytes : planner_alpha() * (double)free_b;

@@ -35,9 +35,7 @@ def exchange(phi, scheme: str, rows, group=None):
     ("rows": valid on rows[0]:rows[0]+rows[1] only).  On return every rank holds the complete phi."""
     import torch
     import torch.distributed as dist
-    world = dist.get_world_size(group)
-    if world == 1:
-        return phi
+    world = dist.get_world_size(group)   # world 1 issues the same collectives (a single-rank NCCL group exercises the path)
     if scheme == "pairs":
         view = torch.view_as_real(phi) if phi.is_complex() else phi
         dist.all_reduce(view, op=dist.ReduceOp.SUM, group=group)
@@ -144,9 +142,19 @@ class DistributedHamiltonian:
         self.D = D
 
     def plan(self, **kw):
+        """mfh_plan on every rank.  Block ownership is defined in block indices, so the ranks must agree on B: the
+        library refuses B = 0 on a partitioned handle, and the planned (B, n_blk, k) of all ranks are compared here
+        (a mismatch would give a silently wrong phi: blocks missing or counted twice)."""
+        import torch.distributed as dist
         rec = self.h.plan(**kw)
         self.rows = self.h.partition_rows()
         k = kw.get("k", 1)
+        info = self.h.get_plan()
+        mine = (int(info["B"]), int(info["n_blk"]), int(info["k"]))
+        every = [None] * self.world
+        dist.all_gather_object(every, mine, group=self.group)
+        if any(tuple(x) != mine for x in every):
+            raise RuntimeError(f"ranks planned different block structures (B, n_blk, k): {every}")
         install_exchange_hook(self.h, self.scheme, self.rows, k, self.group)
         return rec
 

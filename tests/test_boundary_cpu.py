@@ -204,3 +204,32 @@ def test_task_waves_cover_every_task_once():
         assert sorted(t for g in range(C) for t in my_tasks(n_tasks, g, C)) == list(range(n_tasks))
     with pytest.raises(ValueError):
         row_groups(8, 3)
+
+
+def test_partitioned_handle_needs_a_fixed_block_size():
+    """Block ownership is defined in block indices: mfh_plan refuses B = 0 on a partitioned handle before any device
+    work (ranks picking different B would own sets that do not tile H)."""
+    import ctypes
+    L = mfh.lib()
+    h = mfh.Hamiltonian(4096, 0, 1234)
+    h.set_partition(0, 2, "pairs")
+    buf = ctypes.create_string_buffer(64)
+    assert L.mfh_plan(h._h, mfh.MFH_MODE_PROCEDURAL, 1, 1, 0, 0, None, buf, 64) == mfh.MFH_ERR_INVALID_ARG
+    assert b"same B" in L.mfh_last_error()
+    h.destroy()
+
+
+def test_bessel_table_of_the_chebyshev_driver_against_scipy():
+    """mfh_chebyshev's Jacobi-Anger coefficients (Miller recurrence) at small, moderate and LARGE arguments; the large
+    ones are where std::cyl_bessel_j breaks down (x > 1000 at high order)."""
+    import numpy as np
+    from scipy.special import jv
+    for x in (0.0, 0.3, 7.5, 105.0, 713.0, 1001.0, 2000.0):
+        l_max = int(x + 80 + 12 * np.cbrt(x))
+        J = mfh.bessel_j_table(x, l_max)
+        ref = jv(np.arange(l_max + 1), x)
+        assert np.all(np.isfinite(J)) and np.max(np.abs(J - ref)) < 1e-13, x
+        assert abs(J[0] ** 2 + 2.0 * np.sum(J[1:] ** 2) - 1.0) < 1e-12      # sum rule J_0^2 + 2 sum J_l^2 = 1
+    assert mfh.bessel_j_table(1001.0, 500)[500] == pytest.approx(-0.0270214558893, rel=1e-9)   # libstdc++ gave -4.2e33
+    with pytest.raises(mfh.MfhError):
+        mfh.bessel_j_table(-1.0, 10)

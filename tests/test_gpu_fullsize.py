@@ -342,6 +342,26 @@ def test_chebyshev_t0_is_identity_and_bad_args():
         h.chebyshev(to_dev(psi), float("inf"), -2.1, 2.1, 1e-14)
 
 
+def test_chebyshev_large_argument_R_t_above_1000():
+    """a = R t = 1500: about 1600 terms.  The Bessel table must stay accurate there (Miller recurrence; the C++17
+    special function breaks down for x > 1000); exact reference by eigh."""
+    D, B = 512, 128
+    t, e0, e1, tol = 1500.0 / 2.1, -2.1, 2.1, 1e-13
+    psi = make_psi(D, 7)
+    h = mfh.Hamiltonian(D, B, 21, "c128")
+    h.plan("full")
+    out, K = h.chebyshev(to_dev(psi), t, e0, e1, tol)
+    assert K == oracle.chebyshev_n_terms(2.1 * t, tol) and 1500 < K < 1700
+    H = oracle.materialize(D, 21)
+    w, U = np.linalg.eigh(H)
+    exact = U @ (np.exp(-1j * w * t) * (U.conj().T @ psi))
+    got = out.cpu().numpy()
+    assert np.all(np.isfinite(got.view(np.float64)))
+    assert rel_l2(got, exact) <= 5e-11
+    assert abs(np.linalg.norm(got) - 1.0) <= 1e-10
+    h.destroy()
+
+
 def test_chebyshev_shifted_asymmetric_bounds():
     # c != 0 exercises the -c q term of H~ and the e^{-ict} phase (P:707)
     D, B = 1024, 256

@@ -178,3 +178,62 @@ def test_bench_partition_mode_runs_on_one_gpu():
     line = json.loads(r.stdout.strip().splitlines()[-1])
     assert line["scaling"] == "strong" and line["n_gpus"] == 1 and line["config"]["partition"]["scheme"] == "pairs"
     assert line["value"] > 1e10 and line["gpu_launches"] > 0
+
+
+_NCCL_WORLD1 = r"""
+import os, socket, sys
+import numpy as np, torch, torch.distributed as dist
+sys.path.insert(0, sys.argv[1])
+from paper_2606_31598_b200 import binding as mfh
+from paper_2606_31598_b200 import distributed as dmod
+from paper_2606_31598_b200.inputs import make_psi
+with socket.socket() as sk:
+    sk.bind(("127.0.0.1", 0)); port = sk.getsockname()[1]
+torch.cuda.set_device(0)
+dist.init_process_group("nccl", init_method=f"tcp://127.0.0.1:{port}", rank=0, world_size=1, device_id=torch.device("cuda", 0))
+calls = {"all_reduce": 0, "all_gather_into_tensor": 0}
+for name in calls:                                    # count the collectives that reach the backend
+    orig = getattr(dist, name)
+    def wrap(*a, _o=orig, _n=name, **k):
+        calls[_n] += 1
+        return _o(*a, **k)
+    setattr(dist, name, wrap)
+D, B = 2048, 256
+for dtype, k in (("c128", 1), ("c64", 4)):
+    psi = torch.from_numpy(make_psi(D, 99, k=k, dtype=dtype)).cuda()
+    h = mfh.Hamiltonian(D, B, 21, dtype); h.plan("procedural", k=k)
+    ref = h.apply(psi).clone()
+    ref_c = h.chebyshev(psi, 3.0, -2.1, 2.1, 1e-12)[0].clone() if k == 1 else None
+    h.destroy()
+    for scheme in ("pairs", "rows"):
+        before = dict(calls)
+        dh = dmod.DistributedHamiltonian(D, B, 21, dtype, scheme=scheme)
+        dh.plan(mode="procedural", k=k)
+        phi = dh.apply(psi)                            # apply + NCCL exchange (in place on the complex tensor)
+        torch.cuda.synchronize()
+        assert torch.equal(phi, ref), (dtype, scheme)
+        key = "all_reduce" if scheme == "pairs" else "all_gather_into_tensor"
+        assert calls[key] == before[key] + 1, (calls, before)
+        if k == 1:
+            out, K = dh.chebyshev(psi, 3.0, -2.1, 2.1, 1e-12)   # the library's driver calls the hook after every apply
+            torch.cuda.synchronize()
+            st = dh.h._exchange_state
+            assert "error" not in st and st["calls"] == K - 1, st
+            assert calls[key] == before[key] + 1 + (K - 1)
+            assert torch.equal(out, ref_c), (dtype, scheme)
+        dh.destroy()
+dist.destroy_process_group()
+print("NCCL-WORLD1-OK", calls)
+"""
+
+
+def test_exchange_and_chained_hook_on_the_nccl_backend_world_1():
+    """distributed.exchange and the mfh_chebyshev exchange hook on the real backend: a single-rank NCCL group issues
+    the same collectives as a multi-GPU job (all_reduce on the real view of the complex vector, in-place
+    all_gather_into_tensor), in stream order with the library's kernels.  No N > 1 run exists (one GPU per call)."""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, "-c", _NCCL_WORLD1, root], capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0 and "NCCL-WORLD1-OK" in r.stdout, (r.stdout[-1500:], r.stderr[-3000:])
