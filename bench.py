@@ -104,6 +104,18 @@ def oracle_rows_apply(cfg: dict, psi, rows):
     return oracle.apply(cfg["D"], cfg["B"], cfg["seed"], psi, rows=rows)
 
 
+def cpu_info() -> dict:
+    model = "unknown"
+    try:
+        for ln in open("/proc/cpuinfo"):
+            if ln.startswith("model name"):
+                model = ln.split(":", 1)[1].strip()
+                break
+    except OSError:
+        pass
+    return {"cpu_model": model, "nproc": os.cpu_count()}
+
+
 def cpu_baseline(cfg: dict, psi, target_s: float = 15.0) -> dict:
     """The oracle as it stands, timed on the host cores on a bounded row sample of the workload."""
     import oracle
@@ -117,7 +129,8 @@ def cpu_baseline(cfg: dict, psi, target_s: float = 15.0) -> dict:
     t0 = time.perf_counter()
     oracle_rows_apply(cfg, psi, rows)
     dt = time.perf_counter() - t0
-    return {"value": n * D / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+    return {"value": n * D / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", **cpu_info(),
+            "omp_threads": oracle.num_threads(), "entries_per_s_per_core": n * D / dt / max(oracle.num_threads(), 1),
             "sample": f"{n} evenly spaced output rows of {D} ({n * D:.3g} matrix entries, {dt:.1f} s); "
                       f"implied full apply {D * D / (n * D / dt):.0f} s (extrapolated)"}
 
@@ -146,8 +159,8 @@ def run_reference(args, cfg_name: str):
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic", "config": workload_config(cfg_name, cfg),
             "applies_per_s": value / (D * D),
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-                             "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", **cpu_info(),
+                             "omp_threads": oracle.num_threads(), "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -215,18 +228,15 @@ def measure_config(torch, mfh, name: str, steps: int, warmup: int, with_e2e: boo
     torch.cuda.synchronize()
     if barrier:
         barrier()
+    # per-kernel durations from the SAME pass: mfh_timing_begin arms event records around each launch of the next
+    # K applies (no synchronisation inside the pass), so kernel_ms.total <= ms_per_step by construction
+    h.timing_begin(steps)
     ms = time_steps(torch, fn, steps, flush)
+    recs = h.timing_end()
     if barrier:
         barrier()
-    # per-kernel durations: the same K steps again through mfh_apply_timed (events around each launch)
-    kern = {"cached": 0.0, "procedural": 0.0, "reduce": 0.0, "total": 0.0}
-    for _ in range(steps):
-        if flush:
-            flush()
-            torch.cuda.synchronize()
-        t = h.apply_timed(psi, phi, lambdas=lam)
-        for key in kern:
-            kern[key] += t[key] / steps
+    assert len(recs) == steps, (len(recs), steps)
+    kern = {key: sum(r[key] for r in recs) / steps for key in ("cached", "procedural", "reduce", "total")}
     out = {"name": name, "cfg": cfg, "pipe_rate": mfh.pipe_rate, "plan": info, "plan_s": plan_s, "ms_total": ms, "steps": steps,
            "ms_per_step": ms / steps, "kernel_ms": kern, "psi_np": psi_np,
            "launches_per_apply": info["launches_per_apply"]}
@@ -392,7 +402,7 @@ def roofline_for(res: dict, hbm_gbs: float, peak_src: str) -> dict:
         gbs = nbytes / (kern["procedural"] * 1e-3) / 1e9
         gen = D * D * (1.0 - res["plan"]["cached_fraction"]) / (kern["procedural"] * 1e-3)
         return {"kernel": "partial_overlap_kernel", "bound": "hbm", "achieved": gbs, "peak": hbm_gbs, "unit": "GB/s",
-                "frac": gbs / hbm_gbs, "traffic": NCU_TRAFFIC.get(("partial_overlap_kernel", D)), "peak_source": peak_src,
+                "frac": gbs / hbm_gbs, **ncu_traffic("partial_overlap_kernel", D), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": nbytes, "kernel_ms": kern["procedural"],
                 "generated_entries_per_s_in_the_same_kernel": gen,
                 "share_of_step": kern["procedural"] / max(kern["total"], 1e-9)}
@@ -402,7 +412,7 @@ def roofline_for(res: dict, hbm_gbs: float, peak_src: str) -> dict:
         tf = flops / (kern["cached"] * 1e-3) / 1e12
         peak = 148 * 64 * 2 * 1.965e9 / 1e12
         return {"kernel": "cached_multi_kernel_c128", "bound": "alu", "achieved": tf, "peak": peak, "unit": "TFLOP/s",
-                "frac": tf / peak, "traffic": None,
+                "frac": tf / peak, "traffic": None, "traffic_source": None,
                 "peak_source": "nominal FP64: 148 SMs x 64 DFMA lanes/clk x 2 flop x 1.965 GHz (B200_PROFILING.md unit counts; "
                                "the SM clock under FP64 load is power-capped below that)",
                 "kernel_ms": kern["cached"], "share_of_step": kern["cached"] / max(kern["total"], 1e-9)}
@@ -413,45 +423,83 @@ def roofline_for(res: dict, hbm_gbs: float, peak_src: str) -> dict:
         name = "cached_pairs_kernel" if res["plan"]["mode"] == "pairs" else (
             "cached_kernel" if k == 1 else ("cached_multi_tc_kernel" if cfg["dtype"] == "c64" else "cached_multi_kernel_c128"))
         return {"kernel": name, "bound": "hbm", "achieved": gbs, "peak": hbm_gbs, "unit": "GB/s",
-                "frac": gbs / hbm_gbs, "traffic": NCU_TRAFFIC.get((name, cfg["D"])), "peak_source": peak_src,
+                "frac": gbs / hbm_gbs, **ncu_traffic(name, cfg["D"]), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": nbytes, "kernel_ms": kern["cached"],
                 "share_of_step": kern["cached"] / max(kern["total"], 1e-9)}
-    # ALU-bound fused generate-and-apply: unit = matrix entries applied per second by that kernel
+    # ALU-bound fused generate-and-apply: unit = matrix entries applied per second by that kernel.
+    # Headline denominator = an implementation-independent pipe peak from the guide's unit counts and clocks: the FP64
+    # pipe for the complex128 kernel (64 DFMA lanes/clk/SM), the issue slots for the complex64 tensor-core generator;
+    # the measured instruction-mix ceiling and the component ceilings (the library's own generator functions, one
+    # component at a time) are reported beside it.
     entries = D * D * (1.0 - res["plan"]["cached_fraction"])
     rate = entries / (kern["procedural"] * 1e-3)
     key = (cfg["dtype"], "k1" if k == 1 else "kN")
-    issue_peak = ISSUE_LANES_PER_S / INSTR_PER_ENTRY[key]
+    cnt = SASS_COUNTS[key]
+    issue_peak = ISSUE_LANES_PER_S / cnt["instr_per_entry"]
+    kname = "proc_single_kernel" if k == 1 else ("proc_multi_tc_kernel" if cfg["dtype"] == "c64" else "proc_multi_kernel")
+    out = {"kernel": kname, "bound": "alu", "achieved": rate / 1e9, "unit": "Gentries/s", "traffic": None, "traffic_source": None,
+           "issue_slot_peak": issue_peak / 1e9, "frac_of_issue_slots": rate / issue_peak,
+           "instr_per_entry": cnt["instr_per_entry"], "sass_counts_source": cnt["source"],
+           "kernel_ms": kern["procedural"], "share_of_step": kern["procedural"] / max(kern["total"], 1e-9)}
+    if cnt.get("fp64_per_entry"):
+        fp64_peak = FP64_LANES_PER_S / cnt["fp64_per_entry"]
+        out.update({"peak": fp64_peak / 1e9, "frac": rate / fp64_peak, "fp64_per_entry": cnt["fp64_per_entry"],
+                    "peak_source": f"FP64 pipe: 148 SMs x 64 DFMA lanes/clk x 1.965 GHz (B200_PROFILING.md unit counts and clocks) / "
+                                   f"{cnt['fp64_per_entry']} FP64 instructions per entry in the inner loop's SASS ({cnt['source']}); "
+                                   "nominal clock, the run itself is power-capped below it (see clocks)"})
+    else:
+        out.update({"peak": issue_peak / 1e9, "frac": rate / issue_peak,
+                    "peak_source": f"issue slots: 148 SMs x 4 warp instructions/clk x 1.965 GHz / {cnt['instr_per_entry']} instructions "
+                                   f"per entry in the inner loop's SASS ({cnt['source']})"})
     mix = MIX_OF.get(key)
     if mix is not None:
-        # ceiling measured live on this GPU: synthetic kernel with the inner loop's instruction counts
+        # second number: ceiling measured live on this GPU by a synthetic kernel with the inner loop's instruction counts
         name, entries_per_unit = mix
-        peak = res["pipe_rate"](name) * entries_per_unit
-        src = (f"measured now: mfh_debug_pipe_rates({name}) x {entries_per_unit} entries per unit -- synthetic kernel "
-               "with the per-entry IMAD.WIDE/LOP3/DFMA/MUFU/FFMA counts of the inner loop, no memory traffic "
-               "(DESIGN.md 6.2)")
-    else:
-        peak, src = issue_peak, "issue-slot bound (DESIGN.md 6.2)"
-    kname = "proc_single_kernel" if k == 1 else ("proc_multi_tc_kernel" if cfg["dtype"] == "c64" else "proc_multi_kernel")
-    return {"kernel": kname, "bound": "alu", "achieved": rate / 1e9, "peak": peak / 1e9, "unit": "Gentries/s",
-            "frac": rate / peak, "traffic": None, "peak_source": src,
-            "issue_slot_peak": issue_peak / 1e9, "frac_of_issue_slots": rate / issue_peak,
-            "instr_per_entry": INSTR_PER_ENTRY[key],
-            "kernel_ms": kern["procedural"], "share_of_step": kern["procedural"] / max(kern["total"], 1e-9)}
+        mix_peak = res["pipe_rate"](name) * entries_per_unit
+        out.update({"mix_ceiling": mix_peak / 1e9, "frac_of_mix_ceiling": rate / mix_peak,
+                    "mix_ceiling_source": f"measured now: mfh_debug_pipe_rates({name}) x {entries_per_unit} entries per unit "
+                                          "(synthetic kernel with the per-entry IMAD.WIDE/LOP3/DFMA/MUFU/FFMA counts, DESIGN.md 6.2)"})
+    comp = COMPONENTS_OF.get(key)
+    if comp is not None:
+        # Philox-only, Philox+Box-Muller and MAC-only micro-kernels built from the library's own device
+        # functions; generated pairs/s, two entries per pair with Hermitian reuse, one entry per pair without
+        epp = comp["entries_per_pair"]
+        r = {nm: res["pipe_rate"](nm) * epp for nm in comp["kernels"]}
+        gen, mac = r[comp["kernels"][1]], r[comp["kernels"][2]]
+        serial = 1.0 / (1.0 / gen + 1.0 / mac)
+        out["components"] = {"unit": "Gentries/s", "philox_only": r[comp["kernels"][0]] / 1e9, "philox_box_muller": gen / 1e9,
+                             "mac_only": mac / 1e9, "harmonic_gen_plus_mac": serial / 1e9,
+                             "frac_of_harmonic": rate / serial, "frac_of_generation_alone": rate / gen}
+    return out
 
 
-# ALU ceilings.  (1) Measured: the library's synthetic instruction-mix kernel.
-# (2) Nominal: every SM issues at most 4 warp instructions per clock; instructions per matrix entry
-# counted in the SASS of the inner loops (cuobjdump): the two-sided c128 loop spends 88 per generated
-# pair = 44 per entry, the c64 tensor-core loop 60 per entry.
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full captures
-# (profiles/r01_*_ncu_full*.md), keyed by (kernel, D).
-NCU_TRAFFIC = {("cached_kernel", 65536): 68.724718e9 + 4.461824e6,
-               ("partial_overlap_kernel", 131072): 146.039268e9 + 247.162624e6,
-               ("cached_pairs_kernel", 65536): 35.438780e9 + 249.902592e6,
-               ("cached_multi_tc_kernel", 32768): 8.596603e9 + 134.462720e6}
+# ALU ceilings.  Instruction counts per matrix entry come from the SASS of the inner loops (cuobjdump;
+# tables in profiles/).  Nominal pipe peaks: every SM issues at most 4 warp instructions per clock and has 64 FP64
+# lanes (B200_PROFILING.md unit counts, 1.965 GHz).
 ISSUE_LANES_PER_S = 148 * 4 * 32 * 1.965e9
-INSTR_PER_ENTRY = {("c128", "k1"): 44.0, ("c128", "kN"): 150.0, ("c64", "k1"): 40.0, ("c64", "kN"): 60.0}
+FP64_LANES_PER_S = 148 * 64 * 1.965e9
+SASS_COUNTS = {("c128", "k1"): {"instr_per_entry": 45.25, "fp64_per_entry": 16.0, "source": "profiles/r02_proc_single_sass.md"},
+               ("c128", "kN"): {"instr_per_entry": 150.0, "fp64_per_entry": 0, "source": "DESIGN.md 6.3"},
+               ("c64", "k1"): {"instr_per_entry": 40.0, "fp64_per_entry": 0, "source": "DESIGN.md 6.2"},
+               ("c64", "kN"): {"instr_per_entry": 60.0, "fp64_per_entry": 0, "source": "DESIGN.md 6.3"}}
 MIX_OF = {("c128", "k1"): ("c128_pair", 2), ("c64", "kN"): ("c64_entry", 1)}
+COMPONENTS_OF = {("c128", "k1"): {"kernels": ("comp_philox", "comp_philox_bm_c128", "comp_mac_c128"), "entries_per_pair": 2},
+                 ("c64", "k1"): {"kernels": ("comp_philox", "comp_philox_bm_c64", "comp_mac_c64"), "entries_per_pair": 2}}
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full captures, keyed by
+# (kernel, D): (bytes per launch, the capture it was read from).  A kernel without a capture reports "traffic": null.
+NCU_TRAFFIC = {("cached_kernel", 65536): (68.724718e9 + 4.461824e6, "profiles/r01_cached_c2_ncu_full.md"),
+               ("partial_overlap_kernel", 131072): (146.039268e9 + 247.162624e6, "profiles/r01_partial_overlap_c5_ncu_full.md"),
+               ("cached_pairs_kernel", 65536): (35.438780e9 + 249.902592e6, "profiles/r01_pairs_c2_ncu_full.md"),
+               ("cached_multi_tc_kernel", 32768): (8.596603e9 + 134.462720e6, "profiles/r01_cached_multi_tc_c3_ncu_full.md")}
+
+
+def ncu_traffic(kernel: str, D: int) -> dict:
+    """Traffic of a committed ncu capture (not measured in this run: bench.py never runs under a profiler) and the
+    file it came from."""
+    v = NCU_TRAFFIC.get((kernel, D))
+    return {"traffic": v[0] if v else None, "traffic_source": v[1] if v else None}
 
 
 def add_read_probe(rf: dict, read_probe_gbs):
@@ -529,6 +577,7 @@ def main():
                          "strong scaling) instead of N replicas")
     ap.add_argument("--no-extra", action="store_true", help="skip the other configs' side measurements")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--save", default="", help="also write the JSON line (with other_configs) to this file")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
 
@@ -640,6 +689,11 @@ def main():
         else:
             line["cpu_baseline"] = None
         print(json.dumps(line), flush=True)
+        if args.save:
+            os.makedirs(os.path.dirname(os.path.abspath(args.save)), exist_ok=True)
+            with open(args.save, "w") as f:
+                json.dump(line, f, indent=1)
+                f.write("\n")
     if dist:
         dist.barrier()
         dist.destroy_process_group()

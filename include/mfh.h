@@ -178,6 +178,15 @@ MFH_API int mfh_apply(mfh_handle h, const void* psi_dev, void* phi_dev, int32_t 
 MFH_API int mfh_apply_timed(mfh_handle h, const void* psi_dev, void* phi_dev, int32_t k,
                             const double* lambdas_host, void* stream, float* ms_out);
 
+/* Measurement export, in-pass: arm per-launch timing for the next n_applies calls of mfh_apply on this handle.  Each
+ * of them records CUDA events on its stream before, between and after its launches -- no synchronisation, so the
+ * applies run back to back exactly as in an untimed loop and the per-kernel durations come from the SAME pass as the
+ * loop's own time.  mfh_timing_end synchronises `stream`, writes 4 floats per recorded apply to ms_out (layout as
+ * mfh_apply_timed: cached, fused, reduce, whole apply), stores the number of recorded applies and disarms.
+ * ms_out must hold 4 * n_applies floats.  Errors: INVALID_ARG, BAD_STATE (no plan), CUDA. */
+MFH_API int mfh_timing_begin(mfh_handle h, int32_t n_applies);
+MFH_API int mfh_timing_end(mfh_handle h, float* ms_out, int32_t* n_recorded, void* stream);
+
 /* Same as mfh_apply but with HOST buffers: copies psi to the device, applies, copies phi back and
  * synchronises `stream` (the end-to-end call bench.py times).  Host buffers should be pinned. */
 MFH_API int mfh_apply_host(mfh_handle h, const void* psi_host, void* phi_host, int32_t k,
@@ -304,6 +313,20 @@ MFH_API int mfh_debug_philox(uint64_t seed, uint32_t stream_id, const uint32_t* 
  * Needs B fixed (mfh_create with B != 0, or after mfh_plan). */
 MFH_API int mfh_materialize_block(mfh_handle h, int32_t n, int32_t m, void* block_dev, void* stream);
 
+/* Self-check exports (compute-sanitizer is not available on every machine; tests/test_gpu_selfcheck.py):
+ *   mfh_debug_poison     fills the partial-sum workspace and the Chebyshev scratch with 0xFF bytes (NaN in both
+ *                        precisions), asynchronously on `stream`: a kernel that reads a partial sum no kernel of the
+ *                        same apply has written turns phi into NaN (the substitute for initcheck).
+ *   mfh_debug_selfcheck  every library-owned plan buffer sits between two 4 KB guard bands filled with a byte pattern
+ *                        at allocation; counts the guard bytes that no longer hold it (out-of-bounds writes; the
+ *                        write side of memcheck).  Synchronises `stream`.
+ * Errors: BAD_STATE (no plan), INVALID_ARG, CUDA. */
+/* Test of the test: overwrites the guard byte right before (after = 0) or right after (after = 1) the buffer_index-th
+ * library-owned buffer, as an out-of-bounds write would; mfh_debug_selfcheck must then report it. */
+MFH_API int mfh_debug_corrupt_guard(mfh_handle h, int32_t buffer_index, int32_t after);
+MFH_API int mfh_debug_poison(mfh_handle h, void* stream);
+MFH_API int mfh_debug_selfcheck(mfh_handle h, int64_t* bad_guard_bytes, void* stream);
+
 /* The Bessel table behind mfh_chebyshev (Jacobi-Anger coefficients, R7): J_l(x) for l = 0..l_max written to
  * out_host (l_max + 1 doubles, host), x >= 0, by Miller's downward recurrence normalised with
  * J_0 + 2 sum_j J_2j = 1 (valid for every x; host only, no GPU).  Errors: INVALID_ARG. */
@@ -323,8 +346,17 @@ MFH_API int mfh_debug_h0(mfh_handle h, void* h0_dev, void* stream);
  *   MFH_MIX_C64_ENTRY   14 multiplies + 20 ALU ops + 4 SFU ops + 11 FP32 ops: one generated complex64
  *                       entry whose multiply-accumulate runs on the tensor cores
  *   MFH_MIX_PHILOX      one full Philox call (18 multiplies, 18 xors);   MFH_MIX_DFMA31  the 32 FP64 operations alone
+ * Component ceilings ("Philox-only, Philox+Box-Muller, MAC-only micro-kernels"), which call the
+ * library's own generator functions (not typed-in instruction counts) in the fused kernel's shape -- 8 warps, 2 CTAs
+ * per SM, 4 rows per lane -- and return generated PAIRS per second (one pair = two matrix entries with Hermitian reuse):
+ *   MFH_COMP_PHILOX          pair_words() only, words xor-reduced
+ *   MFH_COMP_PHILOX_BM_C128  + the FP64 Box-Muller of the complex128 kernels (tables in shared memory), entries summed
+ *   MFH_COMP_MAC_C128        the two-sided multiply-accumulate alone (8 DFMA per pair, psi_j from shared memory, the
+ *                            column accumulator rotated by shuffles) on entries that cost half an add each
+ *   MFH_COMP_PHILOX_BM_C64 / MFH_COMP_MAC_C64   the same for the complex64 CUDA-core kernel (SFU Box-Muller, FFMA)
  * Synchronises `stream`.  Errors: INVALID_ARG, CUDA. */
-enum { MFH_MIX_C128_PAIR = 0, MFH_MIX_C64_ENTRY = 1, MFH_MIX_PHILOX = 2, MFH_MIX_DFMA31 = 3 };
+enum { MFH_MIX_C128_PAIR = 0, MFH_MIX_C64_ENTRY = 1, MFH_MIX_PHILOX = 2, MFH_MIX_DFMA31 = 3, MFH_COMP_PHILOX = 4,
+       MFH_COMP_PHILOX_BM_C128 = 5, MFH_COMP_MAC_C128 = 6, MFH_COMP_PHILOX_BM_C64 = 7, MFH_COMP_MAC_C64 = 8 };
 MFH_API int mfh_debug_pipe_rates(int32_t mix, double* units_per_s, void* stream);
 
 /* Read-only HBM stream probe: times a kernel that reads `bytes` of buf_dev once (8 independent 128-bit

@@ -30,9 +30,9 @@ MODES = {"auto": MFH_MODE_AUTO, "procedural": MFH_MODE_PROCEDURAL, "partial": MF
          "full": MFH_MODE_FULL, "pairs": MFH_MODE_PAIRS}
 
 # every symbol include/mfh.h declares (tests check that the library exports all of them)
-SYMBOLS = ["mfh_create", "mfh_plan_analytic", "mfh_plan_node_analytic", "mfh_plan", "mfh_apply", "mfh_apply_host", "mfh_apply_timed",
+SYMBOLS = ["mfh_create", "mfh_plan_analytic", "mfh_plan_node_analytic", "mfh_plan", "mfh_apply", "mfh_apply_host", "mfh_apply_timed", "mfh_timing_begin", "mfh_timing_end",
            "mfh_chebyshev", "mfh_chebyshev_imag", "mfh_chebyshev_scan", "mfh_chebyshev_steps", "mfh_lanczos_bounds", "mfh_destroy", "mfh_last_error", "mfh_get_plan", "mfh_debug_philox",
-           "mfh_materialize_block", "mfh_debug_h0", "mfh_debug_bessel_j", "mfh_debug_pipe_rates", "mfh_sb_create", "mfh_sb_plan", "mfh_sb_apply",
+           "mfh_materialize_block", "mfh_debug_h0", "mfh_debug_bessel_j", "mfh_debug_poison", "mfh_debug_selfcheck", "mfh_debug_corrupt_guard", "mfh_debug_pipe_rates", "mfh_sb_create", "mfh_sb_plan", "mfh_sb_apply",
            "mfh_sb_destroy", "mfh_set_partition", "mfh_get_partition_rows", "mfh_set_exchange", "mfh_debug_read_bandwidth", "mfh_set_source_params", "mfh_set_block", "mfh_surrogate_theta_size", "mfh_surrogate_fit",
            "mfh_surrogate_predict", "mfh_surrogate_loss_grad"]
 
@@ -64,6 +64,8 @@ def lib():
     L.mfh_apply.argtypes = [vp, vp, vp, i32, ctypes.POINTER(dbl), vp]
     L.mfh_apply_host.argtypes = [vp, vp, vp, i32, ctypes.POINTER(dbl), vp]
     L.mfh_apply_timed.argtypes = [vp, vp, vp, i32, ctypes.POINTER(dbl), vp, ctypes.POINTER(ctypes.c_float)]
+    L.mfh_timing_begin.argtypes = [vp, i32]
+    L.mfh_timing_end.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(i32), vp]
     L.mfh_chebyshev.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, ctypes.POINTER(i32), vp]
     L.mfh_chebyshev_scan.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, ctypes.POINTER(dbl), ctypes.POINTER(i32), vp]
     L.mfh_chebyshev_imag.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, ctypes.POINTER(i32), vp]
@@ -82,6 +84,9 @@ def lib():
     L.mfh_debug_philox.argtypes = [u64, u32, vp, vp, i64, vp, vp]
     L.mfh_materialize_block.argtypes = [vp, i32, i32, vp, vp]
     L.mfh_debug_h0.argtypes = [vp, vp, vp]
+    L.mfh_debug_poison.argtypes = [vp, vp]
+    L.mfh_debug_corrupt_guard.argtypes = [vp, i32, i32]
+    L.mfh_debug_selfcheck.argtypes = [vp, ctypes.POINTER(i64), vp]
     L.mfh_debug_bessel_j.argtypes = [dbl, i32, ctypes.POINTER(dbl)]
     L.mfh_debug_pipe_rates.argtypes = [i32, ctypes.POINTER(dbl), vp]
     L.mfh_debug_read_bandwidth.argtypes = [vp, sz, ctypes.POINTER(dbl), vp]
@@ -217,6 +222,19 @@ class Hamiltonian:
                                      _stream(), ms))
         return {"cached": ms[0], "procedural": ms[1], "reduce": ms[2], "total": ms[3]}
 
+    def timing_begin(self, n_applies: int):
+        """Arm in-pass per-kernel timing for the next n_applies apply() calls (no synchronisation inside the pass)."""
+        self._timing_n = int(n_applies)
+        _check(lib().mfh_timing_begin(self._h, self._timing_n))
+
+    def timing_end(self):
+        """Synchronise and return one dict of milliseconds per recorded apply (keys as apply_timed)."""
+        ms = (ctypes.c_float * (4 * self._timing_n))()
+        n = ctypes.c_int32(0)
+        _check(lib().mfh_timing_end(self._h, ms, ctypes.byref(n), _stream()))
+        return [{"cached": ms[4 * a], "procedural": ms[4 * a + 1], "reduce": ms[4 * a + 2], "total": ms[4 * a + 3]}
+                for a in range(n.value)]
+
     def apply_host(self, psi_host, phi_host, lambdas=None):
         """End-to-end call with HOST (pinned) torch tensors; synchronises."""
         k = self.k or 1
@@ -293,6 +311,16 @@ class Hamiltonian:
         _check(lib().mfh_debug_h0(self._h, out.data_ptr(), _stream()))
         return out
 
+    def debug_poison(self):
+        """Fill the library's partial-sum workspace and Chebyshev scratch with NaN (self-check: stale reads)."""
+        _check(lib().mfh_debug_poison(self._h, _stream()))
+
+    def debug_selfcheck(self) -> int:
+        """Number of corrupted guard-band bytes around the library-owned buffers (0 = no out-of-bounds write)."""
+        bad = ctypes.c_int64(-1)
+        _check(lib().mfh_debug_selfcheck(self._h, ctypes.byref(bad), _stream()))
+        return int(bad.value)
+
     def destroy(self):
         if self._h:
             lib().mfh_destroy(self._h)
@@ -362,7 +390,8 @@ def bessel_j_table(x: float, l_max: int):
     return np.array(out[:])
 
 
-MIXES = {"c128_pair": 0, "c64_entry": 1, "philox": 2, "dfma31": 3}
+MIXES = {"c128_pair": 0, "c64_entry": 1, "philox": 2, "dfma31": 3, "comp_philox": 4, "comp_philox_bm_c128": 5,
+         "comp_mac_c128": 6, "comp_philox_bm_c64": 7, "comp_mac_c64": 8}
 
 
 def pipe_rate(mix: str) -> float:

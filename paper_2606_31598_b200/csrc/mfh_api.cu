@@ -35,15 +35,33 @@ static bool valid_B(int64_t D, int32_t B)
     return B >= MFH_MIN_B && B <= MFH_MAX_B && B % MFH_MIN_B == 0 && D % B == 0;
 }
 
+// Every library-owned device buffer of a plan is allocated with a guard band of GUARD_BYTES on both sides, filled
+// with GUARD_BYTE.  mfh_debug_selfcheck counts the guard bytes that no longer hold the pattern: an out-of-bounds
+// WRITE of any kernel into or next to these buffers shows up there (compute-sanitizer is closed on this pool).
+static const size_t GUARD_BYTES = 4096;
+static const unsigned char GUARD_BYTE = 0xA5;
+
+static cudaError_t guarded_malloc(mfh_handle h, void** user, size_t bytes)
+{
+    char* base = nullptr;
+    cudaError_t e = cudaMalloc(&base, bytes + 2 * GUARD_BYTES);
+    if (e != cudaSuccess) return e;
+    e = cudaMemset(base, GUARD_BYTE, GUARD_BYTES);
+    if (e == cudaSuccess) e = cudaMemset(base + GUARD_BYTES + bytes, GUARD_BYTE, GUARD_BYTES);
+    if (e != cudaSuccess) { cudaFree(base); return e; }
+    *user = base + GUARD_BYTES;
+    h->guarded.push_back({base, bytes});
+    return cudaSuccess;
+}
+
 static int free_plan_resources(mfh_handle h)
 {
     void** ptrs[] = {&h->d_cache, &h->d_work, &h->d_h0, (void**)&h->d_cache_slot, (void**)&h->d_items,
                      (void**)&h->d_pair_items,
-                     (void**)&h->d_slot_list, (void**)&h->d_counter, &h->d_cheb, &h->d_io, &h->d_lanczos, &h->d_stage};
-    for (void** p : ptrs) {
-        if (*p) cudaFree(*p);
-        *p = nullptr;
-    }
+                     (void**)&h->d_slot_list, (void**)&h->d_counter, (void**)&h->d_expected, &h->d_cheb, &h->d_io, &h->d_lanczos, &h->d_stage};
+    for (void** p : ptrs) *p = nullptr;
+    for (auto& g : h->guarded) cudaFree(g.first);
+    h->guarded.clear();
     h->planned = false;
     return MFH_OK;
 }
@@ -69,6 +87,10 @@ static size_t lanczos_scratch_bytes(int64_t D, int dtype)
     return (size_t)3 * D * complex_bytes(dtype) + (2 * 4096 + 8 + (size_t)lz_partial_doubles()) * sizeof(double);
 }
 
+// Largest D whose procedural k = 1 plans fold the reduce into the fused kernel: below it an apply is launch-bound
+// (C1: 58 us, three launches); above it the separate reduce kernel costs < 1 % and keeps its wider parallelism.
+static const int64_t kFusedTailMaxD = 32768;
+
 // Allocate and upload everything plan `p` needs, then fill the cache.
 static int commit_plan(mfh_handle h, const Plan& p, cudaStream_t st)
 {
@@ -78,7 +100,7 @@ static int commit_plan(mfh_handle h, const Plan& p, cudaStream_t st)
     const size_t cb = complex_bytes(h->dtype);
     cudaError_t e;
     if (q.cache_bytes) {
-        e = cudaMalloc(&h->d_cache, q.cache_bytes);
+        e = guarded_malloc(h, (void**)&h->d_cache, q.cache_bytes);
         if (e != cudaSuccess) {
             cudaGetLastError();
             set_error("cache allocation of %zu bytes failed: %s", q.cache_bytes, cudaGetErrorString(e));
@@ -86,18 +108,18 @@ static int commit_plan(mfh_handle h, const Plan& p, cudaStream_t st)
             return MFH_ERR_OUT_OF_MEMORY;
         }
     }
-    e = cudaMalloc(&h->d_work, q.work_bytes);
+    e = guarded_malloc(h, (void**)&h->d_work, q.work_bytes);
     if (e != cudaSuccess) {
         cudaGetLastError();
         set_error("workspace allocation of %zu bytes failed: %s", q.work_bytes, cudaGetErrorString(e));
         free_plan_resources(h);
         return MFH_ERR_OUT_OF_MEMORY;
     }
-    MFH_CUDA_CHECK(cudaMalloc(&h->d_cache_slot, q.cache_slot.size() * sizeof(int32_t)));
+    MFH_CUDA_CHECK(guarded_malloc(h, (void**)&h->d_cache_slot, q.cache_slot.size() * sizeof(int32_t)));
     MFH_CUDA_CHECK(cudaMemcpyAsync(h->d_cache_slot, q.cache_slot.data(), q.cache_slot.size() * sizeof(int32_t),
                                    cudaMemcpyHostToDevice, st));
     if (!q.items.empty()) {
-        MFH_CUDA_CHECK(cudaMalloc(&h->d_items, q.items.size() * sizeof(ProcItem)));
+        MFH_CUDA_CHECK(guarded_malloc(h, (void**)&h->d_items, q.items.size() * sizeof(ProcItem)));
         MFH_CUDA_CHECK(cudaMemcpyAsync(h->d_items, q.items.data(), q.items.size() * sizeof(ProcItem),
                                        cudaMemcpyHostToDevice, st));
     }
@@ -111,24 +133,36 @@ static int commit_plan(mfh_handle h, const Plan& p, cudaStream_t st)
             if (b < q.row_first || b >= q.row_first + q.row_count) L[0] |= SLOT_SKIP_ROW;
             if (!q.own[(size_t)b * q.n_blk + b]) L[0] |= SLOT_NO_H0;
         }
-        MFH_CUDA_CHECK(cudaMalloc(&h->d_slot_list, lists.size() * sizeof(int32_t)));
+        MFH_CUDA_CHECK(guarded_malloc(h, (void**)&h->d_slot_list, lists.size() * sizeof(int32_t)));
         MFH_CUDA_CHECK(cudaMemcpy(h->d_slot_list, lists.data(), lists.size() * sizeof(int32_t),
                                   cudaMemcpyHostToDevice));
     }
     if (!q.pair_items.empty()) {
-        MFH_CUDA_CHECK(cudaMalloc(&h->d_pair_items, q.pair_items.size() * sizeof(ProcItem)));
+        MFH_CUDA_CHECK(guarded_malloc(h, (void**)&h->d_pair_items, q.pair_items.size() * sizeof(ProcItem)));
         MFH_CUDA_CHECK(cudaMemcpyAsync(h->d_pair_items, q.pair_items.data(), q.pair_items.size() * sizeof(ProcItem),
                                        cudaMemcpyHostToDevice, st));
     }
-    MFH_CUDA_CHECK(cudaMalloc(&h->d_counter, 2 * sizeof(int32_t)));
-    MFH_CUDA_CHECK(cudaMalloc(&h->d_io, (size_t)2 * h->D * q.k * cb));
+    MFH_CUDA_CHECK(guarded_malloc(h, (void**)&h->d_counter, (3 + (size_t)q.n_blk) * sizeof(int32_t)));
+    MFH_CUDA_CHECK(cudaMemsetAsync(h->d_counter, 0, (3 + (size_t)q.n_blk) * sizeof(int32_t), st));
+    {   // fused tail (launch-bound regime): contributions the last-arrival reduce waits for per block row
+        std::vector<int32_t> expected(q.n_blk, 0);
+        for (const ProcItem& it : q.items) {
+            ++expected[it.n];
+            if (it.col_slot >= 0) ++expected[it.m];
+        }
+        MFH_CUDA_CHECK(guarded_malloc(h, (void**)&h->d_expected, expected.size() * sizeof(int32_t)));
+        MFH_CUDA_CHECK(cudaMemcpy(h->d_expected, expected.data(), expected.size() * sizeof(int32_t), cudaMemcpyHostToDevice));
+        h->fused_tail = q.mode == MFH_MODE_PROCEDURAL && q.k == 1 && q.part_world == 1 && !q.items.empty() &&
+                        h->D <= kFusedTailMaxD;
+    }
+    MFH_CUDA_CHECK(guarded_malloc(h, (void**)&h->d_io, (size_t)2 * h->D * q.k * cb));
     MFH_CUDA_CHECK(cudaMemsetAsync(h->d_io, 0, (size_t)2 * h->D * q.k * cb, st));   // MFH_PART_ROWS leaves foreign rows untouched
     // scratch of the chained drivers, allocated here so that mfh_chebyshev* / mfh_lanczos_bounds never allocate
     // (they can be captured in a CUDA graph without a warm-up call)
-    MFH_CUDA_CHECK(cudaMalloc(&h->d_cheb, cheb_scratch_bytes(h->D, h->dtype, q.k)));
-    if (q.k == 1) MFH_CUDA_CHECK(cudaMalloc(&h->d_lanczos, lanczos_scratch_bytes(h->D, h->dtype)));
+    MFH_CUDA_CHECK(guarded_malloc(h, (void**)&h->d_cheb, cheb_scratch_bytes(h->D, h->dtype, q.k)));
+    if (q.k == 1) MFH_CUDA_CHECK(guarded_malloc(h, (void**)&h->d_lanczos, lanczos_scratch_bytes(h->D, h->dtype)));
     if (h->kind == MFH_SRC_DIAG_PLUS_GUE) {
-        MFH_CUDA_CHECK(cudaMalloc(&h->d_h0, (size_t)h->D * (h->dtype == MFH_C128 ? 8 : 4)));
+        MFH_CUDA_CHECK(guarded_malloc(h, (void**)&h->d_h0, (size_t)h->D * (h->dtype == MFH_C128 ? 8 : 4)));
         int rc = launch_h0(h, h->d_h0, st);
         if (rc) return rc;
     }
@@ -168,7 +202,12 @@ static int apply_impl(mfh_handle h, const void* psi, void* phi, const double* la
     if (overlap) {
         if ((rc = launch_partial_overlap(h, psi, st))) return rc;
     } else if (p.k == 1) {
-        if ((rc = launch_proc_single(h, psi, st))) return rc;
+        const bool fused = h->fused_tail;   // the kernel reduces as well: one launch per apply
+        if ((rc = launch_proc_single(h, psi, fused ? phi : nullptr, lambdas ? lambdas[0] : h->lambda, st))) return rc;
+        if (fused) {
+            if (ev) { cudaEventRecord(ev[2], st); cudaEventRecord(ev[3], st); }
+            return MFH_OK;
+        }
     } else if (p.slot_multi >= 0 && p.covered_blocks < p.owned_blocks) {
         if ((rc = launch_proc_multi(h, psi, st))) return rc;
     }
@@ -274,6 +313,7 @@ MFH_API int mfh_destroy(mfh_handle h)
 {
     if (!h) return MFH_OK;
     free_plan_resources(h);
+    for (cudaEvent_t e : h->timing_events) cudaEventDestroy(e);
     if (h->d_gen_tab) cudaFree(h->d_gen_tab);
     delete h;
     return MFH_OK;
@@ -321,7 +361,7 @@ MFH_API int mfh_set_block(mfh_handle h, int32_t n, int32_t m, const void* block,
         rc = launch_store_block(h, slot, block, st);
     } else if (h->dtype == MFH_C64 && p.k > 1) {
         // tiled cache: stage on the device (one reusable block, freed with the plan), then re-lay
-        if (!h->d_stage) MFH_CUDA_CHECK(cudaMalloc(&h->d_stage, bytes));
+        if (!h->d_stage) MFH_CUDA_CHECK(guarded_malloc(h, (void**)&h->d_stage, bytes));
         MFH_CUDA_CHECK(cudaMemcpyAsync(h->d_stage, block, bytes, cudaMemcpyHostToDevice, st));
         rc = launch_store_block(h, slot, h->d_stage, st);
         MFH_CUDA_CHECK(cudaStreamSynchronize(st));   // the host block and the staging block may be reused
@@ -531,8 +571,8 @@ MFH_API int mfh_get_plan(mfh_handle h, char* json_out, size_t json_cap)
              p.n_blk, p.k, (long long)p.n_cached, p.cached_per_row,
              (double)p.covered_blocks / (double)std::max<int64_t>(p.owned_blocks, 1), p.cache_bytes, p.work_bytes, p.n_slots,
              p.items.size(), p.pair_items.size(), p.R, p.Q,
-             1 + (p.n_cached > 0) + ((p.k == 1 && !p.items.empty()) ||
-                                      (p.k > 1 && p.covered_blocks < p.owned_blocks)));
+             h->fused_tail ? 1 : 1 + (p.n_cached > 0) + ((p.k == 1 && !p.items.empty()) ||
+                                                          (p.k > 1 && p.covered_blocks < p.owned_blocks)));
     copy_json(buf, json_out, json_cap);
     return MFH_OK;
 }
@@ -549,7 +589,51 @@ MFH_API int mfh_apply(mfh_handle h, const void* psi_dev, void* phi_dev, int32_t 
         set_error("mfh_apply: k=%d differs from the planned k=%d", k, h->plan.k);
         return MFH_ERR_INVALID_ARG;
     }
-    return apply_impl(h, psi_dev, phi_dev, lambdas_host, (cudaStream_t)stream);
+    cudaEvent_t* ev = nullptr;   // armed by mfh_timing_begin: events around the launches of this apply, no synchronisation
+    if (h->timing_pos < h->timing_n) ev = h->timing_events.data() + 4 * (size_t)h->timing_pos++;
+    return apply_impl(h, psi_dev, phi_dev, lambdas_host, (cudaStream_t)stream, ev);
+}
+
+static void timing_clear(mfh_handle h)
+{
+    for (cudaEvent_t e : h->timing_events) cudaEventDestroy(e);
+    h->timing_events.clear();
+    h->timing_n = h->timing_pos = 0;
+}
+
+MFH_API int mfh_timing_begin(mfh_handle h, int32_t n_applies)
+{
+    if (!h || n_applies < 1 || n_applies > 65536) { set_error("mfh_timing_begin: need a handle and 1 <= n_applies <= 65536"); return MFH_ERR_INVALID_ARG; }
+    if (!h->planned) { set_error("mfh_timing_begin: call mfh_plan first"); return MFH_ERR_BAD_STATE; }
+    timing_clear(h);
+    h->timing_events.reserve(4 * (size_t)n_applies);
+    for (int i = 0; i < 4 * n_applies; ++i) {
+        cudaEvent_t e;
+        if (cudaEventCreate(&e) != cudaSuccess) {
+            timing_clear(h);
+            set_error("mfh_timing_begin: cudaEventCreate failed");
+            return MFH_ERR_CUDA;
+        }
+        h->timing_events.push_back(e);
+    }
+    h->timing_n = n_applies;
+    return MFH_OK;
+}
+
+MFH_API int mfh_timing_end(mfh_handle h, float* ms_out, int32_t* n_recorded, void* stream)
+{
+    if (!h || !ms_out || !n_recorded) { set_error("mfh_timing_end: NULL pointer"); return MFH_ERR_INVALID_ARG; }
+    const int n = h->timing_pos;
+    cudaError_t e = cudaStreamSynchronize((cudaStream_t)stream);
+    for (int a = 0; a < n && e == cudaSuccess; ++a) {
+        cudaEvent_t* ev = h->timing_events.data() + 4 * (size_t)a;
+        for (int i = 0; i < 3 && e == cudaSuccess; ++i) e = cudaEventElapsedTime(&ms_out[4 * a + i], ev[i], ev[i + 1]);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms_out[4 * a + 3], ev[0], ev[3]);
+    }
+    *n_recorded = n;
+    timing_clear(h);
+    MFH_CUDA_CHECK(e);
+    return MFH_OK;
 }
 
 MFH_API int mfh_apply_timed(mfh_handle h, const void* psi_dev, void* phi_dev, int32_t k,
@@ -857,6 +941,47 @@ MFH_API int mfh_materialize_block(mfh_handle h, int32_t n, int32_t m, void* bloc
         return MFH_ERR_INVALID_ARG;
     }
     return launch_fill_block(h, B, n, m, block_dev, (cudaStream_t)stream);
+}
+
+MFH_API int mfh_debug_poison(mfh_handle h, void* stream)
+{
+    if (!h || !h->planned) { set_error("mfh_debug_poison: handle not planned"); return MFH_ERR_BAD_STATE; }
+    cudaStream_t st = (cudaStream_t)stream;
+    const Plan& p = h->plan;
+    MFH_CUDA_CHECK(cudaMemsetAsync(h->d_work, 0xFF, p.work_bytes, st));                                 // NaN in float and double
+    MFH_CUDA_CHECK(cudaMemsetAsync(h->d_cheb, 0xFF, (size_t)5 * h->D * p.k * complex_bytes(h->dtype), st));
+    return MFH_OK;
+}
+
+MFH_API int mfh_debug_corrupt_guard(mfh_handle h, int32_t buffer_index, int32_t after)
+{
+    if (!h || !h->planned) { set_error("mfh_debug_corrupt_guard: handle not planned"); return MFH_ERR_BAD_STATE; }
+    if (buffer_index < 0 || buffer_index >= (int32_t)h->guarded.size()) {
+        set_error("mfh_debug_corrupt_guard: buffer %d of %zu", buffer_index, h->guarded.size());
+        return MFH_ERR_INVALID_ARG;
+    }
+    const auto& g = h->guarded[buffer_index];
+    char* at = (char*)g.first + (after ? GUARD_BYTES + g.second : GUARD_BYTES - 1);   // first byte after / last byte before
+    MFH_CUDA_CHECK(cudaMemset(at, 0, 1));
+    return MFH_OK;
+}
+
+MFH_API int mfh_debug_selfcheck(mfh_handle h, int64_t* bad_guard_bytes, void* stream)
+{
+    if (!h || !bad_guard_bytes) { set_error("mfh_debug_selfcheck: NULL pointer"); return MFH_ERR_INVALID_ARG; }
+    if (!h->planned) { set_error("mfh_debug_selfcheck: handle not planned"); return MFH_ERR_BAD_STATE; }
+    cudaStream_t st = (cudaStream_t)stream;
+    MFH_CUDA_CHECK(cudaStreamSynchronize(st));
+    std::vector<unsigned char> buf(GUARD_BYTES);
+    int64_t bad = 0;
+    for (const auto& g : h->guarded)
+        for (int side = 0; side < 2; ++side) {
+            const char* src = (const char*)g.first + (side ? GUARD_BYTES + g.second : 0);
+            MFH_CUDA_CHECK(cudaMemcpy(buf.data(), src, GUARD_BYTES, cudaMemcpyDeviceToHost));
+            for (unsigned char c : buf) bad += (c != GUARD_BYTE);
+        }
+    *bad_guard_bytes = bad;
+    return MFH_OK;
 }
 
 MFH_API int mfh_debug_bessel_j(double x, int32_t l_max, double* out_host)

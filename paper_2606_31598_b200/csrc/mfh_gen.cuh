@@ -101,20 +101,26 @@ __device__ __forceinline__ void pair_words(const PhiloxKeys& K, uint32_t lo, uin
 // a 256-entry table of (1/c, -K2 ln c), a 33-entry table of K2 (32-e) ln 2 and a degree-4
 // polynomial for log1p (remainder r^5/5 <= 6e-15).  sqrt(L) = L y (1 + e + 3/2 e^2), y = rsqrt.approx(L)
 // (2^-21), e = 1/2 - 1/2 L y^2: third-order correct (1e-19 relative).  The angle 2 pi u2 is split into a
-// 1024-entry table of (cos A, sin A) at the bin centres and a residual |b| <= pi/1024:
+// 1024-entry table of (cos A, sin A) at the bin centres and a residual |b| <= pi/1024 (b = (x1 mod 2^22) ang - 2^21 ang:
 // sin b = b - b^3/6 (2e-15), cos b = 1 - b^2/2 + b^4/24 (1e-18), combined by angle addition.
 constexpr int GEN_LOG_BITS = 8;
 constexpr int GEN_SC_BITS = 10;
 
+// Layout: the shared-memory copy is aligned to 16 KB, tsc (16 KB) first, tlog (4 KB) second, so that a table index
+// placed in bits 4..13 (tsc, elog) or 4..11 (tlog) is OR-ed into the table's shared address by the same LOP3 that masks
+// it ((x & mask) | base): no integer add per look-up.
 struct GenTabD {                         // built on the host by make_gen_table(), copied to shared memory
-    double2 tlog[1 << GEN_LOG_BITS];     // (1/c, -K2 ln c)
     double2 tsc[1 << GEN_SC_BITS];       // (cos A, sin A),  A = 2 pi (idx 2^22 + 2^21 + 1/2) 2^-32
+    double2 tlog[1 << GEN_LOG_BITS];     // (1/c, -K2 ln c)
     double elog[34];                     // K2 (32 - e) ln 2 for e = -1..31  (index e + 1)
 };
+constexpr uint32_t GEN_TAB_ALIGN = 16384;
+static_assert(sizeof(double2) * (1 << GEN_SC_BITS) == GEN_TAB_ALIGN, "tsc must fill the alignment unit");
 
 struct GenConstD {                       // kernel-parameter constants (constant bank operands)
     double c1, c2, c3, c4;               // -K2 log1p(r) = r (c1 + r (c2 + r (c3 + r c4)))
     double ang;                          // 2 pi 2^-32
+    double ang_off;                      // -2^21 ang: centres the residual angle, folded into one FMA
 };
 
 struct GenHostD {
@@ -136,10 +142,19 @@ template <> struct Gen<double> {
     {
         // radius: d = x0 + 1/2 exactly (2^52 + x0 by bit pattern, minus 2^52 - 1/2)
         const double d = __hiloint2double(0x43300000, (int)x0) - 0x1.fffffffffffffp51;
-        const int hi = __double2hiint(d);
-        const double m = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, __double2loint(d));
-        const double2 tl = tab->tlog[(hi >> (20 - GEN_LOG_BITS)) & ((1 << GEN_LOG_BITS) - 1)];
-        const double el = tab->elog[(hi >> 20) - 1022];
+        const uint32_t hi = (uint32_t)__double2hiint(d);
+        uint32_t mh;                                                     // mantissa with exponent 0: one LOP3
+        asm("lop3.b32 %0, %1, 0x000fffff, 0x3ff00000, 0xEA;" : "=r"(mh) : "r"(hi));
+        const double m = __hiloint2double((int)mh, __double2loint(d));
+        // shared-memory addresses of the look-ups: (index field & mask) | table base in ONE LOP3 each (see GenTabD)
+        const uint32_t ts = (uint32_t)__cvta_generic_to_shared(tab);    // 16 KB aligned; loop invariant
+        uint32_t a_log, a_exp;
+        asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(a_log) : "r"(hi >> (20 - GEN_LOG_BITS - 4)), "n"(((1 << GEN_LOG_BITS) - 1) << 4), "r"(ts + GEN_TAB_ALIGN));
+        asm("lop3.b32 %0, %1, 0x3ff8, %2, 0xEA;" : "=r"(a_exp) : "r"(hi >> 17), "r"(ts));
+        double2 tl;
+        double el;
+        asm("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(tl.x), "=d"(tl.y) : "r"(a_log));
+        asm("ld.shared.f64 %0, [%1 + %2];" : "=d"(el) : "r"(a_exp), "n"((int)(GEN_TAB_ALIGN + sizeof(double2) * (1 << GEN_LOG_BITS)) - 1022 * 8));
         const double r = fma(m, tl.x, -1.0);
         double p = fma(r, gc.c4, gc.c3);
         p = fma(r, p, gc.c2);
@@ -147,17 +162,19 @@ template <> struct Gen<double> {
         const double L = fma(r, p, tl.y + el);
         double y;
         asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(L));
-        // sqrt(L) = sq (1 + e + 3/2 e^2 + O(e^3)) with sq = L y, e = 1/2 - 1/2 L y^2 (|e| <= 2^-21):
-        // the second-order term removes the -3/2 delta^2 bias a single Newton step would leave in
-        // every entry (1.9e-13, which a Chebyshev propagation over 151 applies would add up)
+        // sqrt(L) = sq (1 + e/2 + 3/8 e^2 + O(e^3)) with sq = L y, e = 1 - L y^2 (|e| <= 2^-20): the second-order
+        // term removes the -3/2 delta^2 bias a single Newton step would leave in every entry (1.9e-13, which a
+        // Chebyshev propagation over 151 applies would add up)
         const double sq = L * y;
-        const double hy = __hiloint2double(__double2hiint(y) - 0x00100000, __double2loint(y));   // y / 2
-        const double e = fma(-sq, hy, 0.5);
-        const double rad = fma(sq, e * fma(e, 1.5, 1.0), sq);
-        // angle
-        const double2 cs = tab->tsc[x1 >> (32 - GEN_SC_BITS)];
-        const int resid = (int)(x1 & ((1u << (32 - GEN_SC_BITS)) - 1u)) - (1 << (31 - GEN_SC_BITS));
-        const double bb = (double)resid * gc.ang;
+        const double e = fma(-sq, y, 1.0);
+        const double rad = fma(sq, e * fma(e, 0.375, 0.5), sq);
+        // angle: residual of x1 inside its bin, centred by the constant term of one FMA (exact: 2^21 ang is ang scaled
+        // by a power of two)
+        uint32_t a_sc;
+        asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(a_sc) : "r"(x1 >> (32 - GEN_SC_BITS - 4)), "n"(((1 << GEN_SC_BITS) - 1) << 4), "r"(ts));
+        double2 cs;
+        asm("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(cs.x), "=d"(cs.y) : "r"(a_sc));
+        const double bb = fma((double)(int)(x1 & ((1u << (32 - GEN_SC_BITS)) - 1u)), gc.ang, gc.ang_off);
         const double b2 = bb * bb;
         const double sb = fma(b2 * (-1.0 / 6.0), bb, bb);
         const double q = fma(b2, 1.0 / 24.0, -0.5) * b2;
@@ -228,16 +245,19 @@ __device__ __forceinline__ void analytic_entry(const AnalyticArgs& A, uint32_t i
     hi = (T)(i < j ? a * A.sphi : -(a * A.sphi));
 }
 
-// Copy the generator table to shared memory (all threads of the CTA; caller synchronises).
+// Copy the generator table to shared memory (all threads of the CTA; caller synchronises).  The table is STATIC shared
+// memory, so its address is a link-time constant that folds into the immediate offset of every table look-up (with a
+// dynamic allocation each look-up paid an extra integer add for the base).
 template <typename T>
-__device__ __forceinline__ const typename Gen<T>::Tab* stage_gen_table(const GenArgs<T>& G, void* smem)
+__device__ __forceinline__ const typename Gen<T>::Tab* stage_gen_table(const GenArgs<T>& G)
 {
+    __shared__ __align__(Gen<T>::TAB_BYTES > 0 ? GEN_TAB_ALIGN : 16) typename Gen<T>::Tab s_gen_tab;
     if constexpr (Gen<T>::TAB_BYTES > 0) {
         const uint4* src = reinterpret_cast<const uint4*>(G.tab_global);
-        uint4* dst = reinterpret_cast<uint4*>(smem);
+        uint4* dst = reinterpret_cast<uint4*>(&s_gen_tab);
         for (int t = threadIdx.x; t < Gen<T>::TAB_BYTES / 16; t += blockDim.x) dst[t] = src[t];
     }
-    return reinterpret_cast<const typename Gen<T>::Tab*>(smem);
+    return &s_gen_tab;
 }
 
 // General entry H_ij for any (i,j): conjugate below the diagonal, real and scaled by 1/sqrt(D)

@@ -94,7 +94,10 @@ struct mfh_handle_s {
     mfh::ProcItem* d_pair_items = nullptr;
     int32_t* d_slot_list = nullptr;   // [n_blk][n_slots+1]: count | flags, then the valid slots in ascending order
     double* d_lambdas = nullptr;    // MFH_MAX_K doubles, refreshed by every apply
-    int32_t* d_counter = nullptr;   // dynamic work counters: [0] procedural kernel, [1] pair kernel
+    int32_t* d_counter = nullptr;   // dynamic work counters: [0] procedural kernel, [1] pair kernel, [2] CTAs finished,
+                                    // [3 .. 3 + n_blk) finished contributions per block row (fused tail)
+    int32_t* d_expected = nullptr;  // [n_blk] contributions the fused tail waits for per block row
+    bool fused_tail = false;        // small procedural k = 1 plans: the fused kernel also reduces (one launch per apply)
     void* d_cheb = nullptr;         // 3 vectors of Chebyshev scratch
     void* d_io = nullptr;           // psi/phi staging of mfh_apply_host
     void* d_lanczos = nullptr;      // 3 Lanczos vectors + alpha/beta/norm scalars + reduction partials
@@ -107,6 +110,9 @@ struct mfh_handle_s {
     // attribute is per device, so it is remembered per handle, not per process
     std::vector<std::pair<const void*, int>> smem_attr;
     void* d_stage = nullptr;        // mfh_set_block: one reusable B x B staging block (tiled caches)
+    std::vector<std::pair<void*, size_t>> guarded;   // (allocation base, user bytes) of every guarded plan buffer
+    std::vector<cudaEvent_t> timing_events;   // mfh_timing_begin: 4 events per armed apply
+    int32_t timing_n = 0, timing_pos = 0;
 };
 
 namespace mfh {
@@ -149,7 +155,7 @@ int launch_fill_block(mfh_handle h, int32_t B, int32_t n, int32_t m, void* out, 
 int launch_fill_cache(mfh_handle h, cudaStream_t st);
 int launch_store_block(mfh_handle h, int32_t slot, const void* src_dev, cudaStream_t st);   // external block -> cache slot
 int launch_h0(mfh_handle h, void* out, cudaStream_t st);
-int launch_proc_single(mfh_handle h, const void* psi, cudaStream_t st);
+int launch_proc_single(mfh_handle h, const void* psi, void* phi, double lambda, cudaStream_t st);
 bool partial_overlap_supported(mfh_handle h);
 int launch_partial_overlap(mfh_handle h, const void* psi, cudaStream_t st);   // cached + generated in one kernel
 int launch_proc_multi(mfh_handle h, const void* psi, cudaStream_t st);

@@ -110,6 +110,7 @@ void make_gen_table(int64_t D, GenHostD& out)
     out.gc.c3 = (double)(-K2 / 3.0L);
     out.gc.c4 = (double)(K2 / 4.0L);
     out.gc.ang = (double)(2.0L * PI / 4294967296.0L);
+    out.gc.ang_off = -2097152.0 * out.gc.ang;   // exact: a power-of-two multiple of the rounded constant
 }
 
 // Offsets covered by a Hermitian pair cache with c band offsets: circular block distance < c.

@@ -64,7 +64,6 @@ __global__ void __launch_bounds__(256) fill_kernel(const GenArgs<T> G, int32_t B
                                                    typename Cplx<T>::type* __restrict__ out)
 {
     using CT = typename Cplx<T>::type;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
     int32_t n, m;
     size_t base;
     if (cache_slot) {
@@ -78,7 +77,7 @@ __global__ void __launch_bounds__(256) fill_kernel(const GenArgs<T> G, int32_t B
         m = single_m;
         base = 0;
     }
-    const typename Gen<T>::Tab* tab = stage_gen_table<T>(G, smem_raw);
+    const typename Gen<T>::Tab* tab = stage_gen_table<T>(G);
     __syncthreads();
     for (int32_t a = blockIdx.y; a < B; a += gridDim.y) {
         const uint32_t i = (uint32_t)n * B + a;
@@ -101,10 +100,10 @@ static int launch_fill_t(mfh_handle h, dim3 grid, int32_t B, int32_t n_blk, cons
 {
     using CT = typename Cplx<T>::type;
     if (h->kind == MFH_SRC_ANALYTIC)
-        fill_kernel<T, SRC_ANALYTIC><<<grid, 256, Gen<T>::TAB_BYTES, st>>>(make_gen_args<T>(h), B, n_blk, cache_slot, n, m,
+        fill_kernel<T, SRC_ANALYTIC><<<grid, 256, 0, st>>>(make_gen_args<T>(h), B, n_blk, cache_slot, n, m,
                                                                             tiled, (CT*)out);
     else
-        fill_kernel<T, SRC_SEEDED><<<grid, 256, Gen<T>::TAB_BYTES, st>>>(make_gen_args<T>(h), B, n_blk, cache_slot, n, m,
+        fill_kernel<T, SRC_SEEDED><<<grid, 256, 0, st>>>(make_gen_args<T>(h), B, n_blk, cache_slot, n, m,
                                                                           tiled, (CT*)out);
     MFH_CUDA_CHECK(cudaGetLastError());
     return MFH_OK;
@@ -212,7 +211,47 @@ template <typename T> struct ProcParams {
     const typename Cplx<T>::type* psi;
     typename Cplx<T>::type* work;   // [n_slots][D]
     int32_t* counter;
+    // fused tail (small procedural plans: one launch per apply).  done[b] counts the finished contributions to block
+    // row b; the CTA that delivers the last one adds the block row's partial slots in list order and writes phi.
+    int32_t* done;                  // nullptr: the reduce kernel runs after this one
+    int32_t* fin;                   // CTAs that have left the item loop (the last one resets the item counter)
+    const int32_t* expected;        // [n_blk] contributions per block row
+    const int32_t* slot_list;       // [n_blk][n_slots + 1]
+    int32_t n_slots;
+    const T* h0;                    // H0 diagonal or nullptr
+    typename Cplx<T>::type* phi;
+    double lambda;
 };
+
+// phi^[b] = h0 (.) psi^[b] + lambda * sum over the valid slots of block row b, in ascending slot order (the order of
+// reduce_kernel's plain path): partial sums written by other CTAs are read through L2 (ld.global.cg).
+template <typename T>
+__device__ __forceinline__ void reduce_block_row(const ProcParams<T>& P, int b)
+{
+    using CT = typename Cplx<T>::type;
+    const int32_t* list = P.slot_list + (size_t)b * (P.n_slots + 1);
+    const int cnt = list[0] & SLOT_COUNT_MASK;
+    for (int a = threadIdx.x; a < P.B; a += PROC_THREADS) {
+        const size_t i = (size_t)b * P.B + a;
+        double sr = 0.0, si = 0.0;
+        for (int t = 0; t < cnt; ++t) {
+            const CT x = __ldcg(P.work + (size_t)list[1 + t] * P.D + i);
+            sr += (double)x.x;
+            si += (double)x.y;
+        }
+        double outr = P.lambda * sr, outi = P.lambda * si;
+        if (P.h0) {
+            const CT p = P.psi[i];
+            const double d = (double)P.h0[i];
+            outr = fma(d, (double)p.x, outr);
+            outi = fma(d, (double)p.y, outi);
+        }
+        CT o;
+        o.x = (T)outr;
+        o.y = (T)outi;
+        P.phi[i] = o;
+    }
+}
 
 // The item loop of one CTA: runs until the device counter is exhausted.
 template <typename T, int R, int SRC = SRC_SEEDED>
@@ -222,11 +261,11 @@ __device__ __forceinline__ void proc_items(const ProcParams<T>& P, unsigned char
     constexpr int W = PROC_WARPS, TR = 32 * R;
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const int B = P.B;
-    const typename Gen<T>::Tab* tab = stage_gen_table<T>(P.G, smem_raw);
-    CT* colsum = reinterpret_cast<CT*>(smem_raw + Gen<T>::TAB_BYTES);   // [B]     column-side sums of the item
+    const typename Gen<T>::Tab* tab = stage_gen_table<T>(P.G);
+    CT* colsum = reinterpret_cast<CT*>(smem_raw);                      // [B]     column-side sums of the item
     CT* rowred = colsum + B;                                           // [W][TR] row sums of the tile per warp
     CT* psiw = rowred + W * TR + w * 32;                               // [32]    psi of the warp's sub-tile
-    __shared__ int s_item;
+    __shared__ int s_item, s_red[2];
     const int n_ct = B / 32;
 
     for (;;) {
@@ -318,6 +357,27 @@ __device__ __forceinline__ void proc_items(const ProcParams<T>& P, unsigned char
             CT* dst = P.work + (size_t)I.col_slot * P.D + (size_t)I.m * B;
             for (int c = tid; c < B; c += PROC_THREADS) dst[c] = colsum[c];
         }
+        if (P.done) {
+            __threadfence();                 // this thread's partial sums are visible device-wide ...
+            __syncthreads();                 // ... before thread 0 announces the item
+            if (tid == 0) {
+                int r0 = -1, r1 = -1;
+                if (atomicAdd(&P.done[I.n], 1) == P.expected[I.n] - 1) r0 = I.n;
+                if (I.col_slot >= 0 && atomicAdd(&P.done[I.m], 1) == P.expected[I.m] - 1) r1 = I.m;
+                if (r0 >= 0) P.done[r0] = 0;   // last contribution of this launch: leave the counter clean for the next
+                if (r1 >= 0) P.done[r1] = 0;
+                s_red[0] = r0;
+                s_red[1] = r1;
+                __threadfence();
+            }
+            __syncthreads();
+            for (int q = 0; q < 2; ++q)
+                if (s_red[q] >= 0) reduce_block_row<T>(P, s_red[q]);
+        }
+    }
+    if (P.done && tid == 0 && atomicAdd(P.fin, 1) == (int)gridDim.x - 1) {
+        *P.counter = 0;                      // every CTA has left the item loop: self-cleaning, no memset launch
+        *P.fin = 0;
     }
 }
 
@@ -433,11 +493,20 @@ partial_overlap_kernel(const ProcParams<double> P, const StripParams<double> S, 
 }
 
 template <typename T, int R>
-static int launch_proc_single_t(mfh_handle h, const void* psi, cudaStream_t st)
+static int launch_proc_single_t(mfh_handle h, const void* psi, void* phi, double lambda, cudaStream_t st)
 {
     using CT = typename Cplx<T>::type;
     const Plan& p = h->plan;
     ProcParams<T> P;
+    const bool fused = h->fused_tail && phi != nullptr;
+    P.done = fused ? h->d_counter + 3 : nullptr;
+    P.fin = h->d_counter + 2;
+    P.expected = h->d_expected;
+    P.slot_list = h->d_slot_list;
+    P.n_slots = std::max(p.n_slots, 1);
+    P.h0 = (const T*)h->d_h0;
+    P.phi = (CT*)phi;
+    P.lambda = lambda;
     P.G = make_gen_args<T>(h);
     P.B = p.B;
     P.n_blk = p.n_blk;
@@ -449,7 +518,7 @@ static int launch_proc_single_t(mfh_handle h, const void* psi, cudaStream_t st)
     P.work = (CT*)h->d_work;
     P.counter = h->d_counter;
     auto smem_for = [](int B) {
-        return (size_t)Gen<T>::TAB_BYTES + (size_t)(B + PROC_WARPS * 32 * R + PROC_WARPS * 32) * sizeof(CT);
+        return (size_t)(B + PROC_WARPS * 32 * R + PROC_WARPS * 32) * sizeof(CT);   // + the static generator table
     };
     const size_t smem = smem_for(p.B);
     const bool analytic = (h->kind == MFH_SRC_ANALYTIC);
@@ -459,20 +528,22 @@ static int launch_proc_single_t(mfh_handle h, const void* psi, cudaStream_t st)
     MFH_CUDA_CHECK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, PROC_THREADS, smem));
     if (per_sm < 1) per_sm = 1;
     const int grid = std::min<int>(P.n_items, h->sm_count * per_sm);
-    MFH_CUDA_CHECK(cudaMemsetAsync(h->d_counter, 0, sizeof(int32_t), st));
+    if (!fused) MFH_CUDA_CHECK(cudaMemsetAsync(h->d_counter, 0, sizeof(int32_t), st));   // the fused tail resets it itself
     kern<<<grid, PROC_THREADS, smem, st>>>(P);
     MFH_CUDA_CHECK(cudaGetLastError());
     return MFH_OK;
 }
 
-int launch_proc_single(mfh_handle h, const void* psi, cudaStream_t st)
+// phi != nullptr on a handle with fused_tail: the kernel also reduces (one launch per apply) and the caller skips
+// launch_reduce.
+int launch_proc_single(mfh_handle h, const void* psi, void* phi, double lambda, cudaStream_t st)
 {
     if (h->plan.items.empty()) return MFH_OK;
     const bool f64 = (h->dtype == MFH_C128);
     switch (h->plan.R) {
-    case 4: return f64 ? launch_proc_single_t<double, 4>(h, psi, st) : launch_proc_single_t<float, 4>(h, psi, st);
-    case 2: return f64 ? launch_proc_single_t<double, 2>(h, psi, st) : launch_proc_single_t<float, 2>(h, psi, st);
-    case 1: return f64 ? launch_proc_single_t<double, 1>(h, psi, st) : launch_proc_single_t<float, 1>(h, psi, st);
+    case 4: return f64 ? launch_proc_single_t<double, 4>(h, psi, phi, lambda, st) : launch_proc_single_t<float, 4>(h, psi, phi, lambda, st);
+    case 2: return f64 ? launch_proc_single_t<double, 2>(h, psi, phi, lambda, st) : launch_proc_single_t<float, 2>(h, psi, phi, lambda, st);
+    case 1: return f64 ? launch_proc_single_t<double, 1>(h, psi, phi, lambda, st) : launch_proc_single_t<float, 1>(h, psi, phi, lambda, st);
     }
     set_error("unsupported rows per lane %d", h->plan.R);
     return MFH_ERR_INVALID_ARG;
@@ -499,6 +570,8 @@ template <int R> static int launch_partial_overlap_t(mfh_handle h, const void* p
     P.psi = (const double2*)psi;
     P.work = (double2*)h->d_work;
     P.counter = h->d_counter;
+    P.done = nullptr;
+    P.fin = nullptr;
     StripParams<double> S;
     S.B = p.B;
     S.n_blk = p.n_blk;
@@ -511,7 +584,7 @@ template <int R> static int launch_partial_overlap_t(mfh_handle h, const void* p
     S.work = (double2*)h->d_work;
     S.counter = h->d_counter + 1;
     auto smem_for = [](int B) {
-        return (size_t)Gen<double>::TAB_BYTES + (size_t)(B + PROC_WARPS * 32 * R + PROC_WARPS * 32) * sizeof(double2);
+        return (size_t)(B + PROC_WARPS * 32 * R + PROC_WARPS * 32) * sizeof(double2);   // + the static generator table
     };
     const size_t smem = smem_for(p.B);
     auto kern = partial_overlap_kernel<R>;
@@ -560,8 +633,8 @@ __global__ void __launch_bounds__(32 * W) proc_multi_kernel(const MultiParams<T>
     using CT = typename Cplx<T>::type;
     constexpr int CH = 32;                         // columns per staged chunk
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const typename Gen<T>::Tab* tab = stage_gen_table<T>(P.G, smem_raw);
-    CT(*psis)[KT] = reinterpret_cast<CT(*)[KT]>(smem_raw + Gen<T>::TAB_BYTES);   // [CH][KT]
+    const typename Gen<T>::Tab* tab = stage_gen_table<T>(P.G);
+    CT(*psis)[KT] = reinterpret_cast<CT(*)[KT]>(smem_raw);                       // [CH][KT]
     const int tid = threadIdx.x;
     const uint32_t i = blockIdx.x * (32 * W) + tid;
     const int n = (int)(i / (uint32_t)P.B);
@@ -617,7 +690,7 @@ static int launch_proc_multi_t(mfh_handle h, const void* psi, cudaStream_t st)
     P.cache_slot = h->d_cache_slot;
     P.psi = (const CT*)psi;
     P.work = (CT*)h->d_work;
-    const size_t smem = (size_t)Gen<T>::TAB_BYTES + 32 * KT * sizeof(CT);
+    const size_t smem = 32 * KT * sizeof(CT);
     // 32W rows per CTA must divide B; prefer 128-row CTAs, fall back to one warp.
     const bool analytic = (h->kind == MFH_SRC_ANALYTIC);
     if (p.B % 128 == 0) {

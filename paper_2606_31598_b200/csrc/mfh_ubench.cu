@@ -102,6 +102,136 @@ static int run_mix(int sm_count, cudaStream_t st, double* units_per_s)
     return MFH_OK;
 }
 
+// ---- component ceilings: the library's OWN device functions, one component at a time ----------
+// The synthetic mixes above issue instruction counts typed in from the SASS; these kernels call the generator code
+// of mfh_gen.cuh itself, in the fused kernel's shape (8 warps, 2 CTAs per SM, 4 rows per lane, one column per step),
+// so they follow every change of the generator:
+//   COMP_PHILOX      pair_words() for 4 rows x 1 column per step, words xor-reduced          -> pairs/s
+//   COMP_PHILOX_BM   + Gen<T>::normals() (tables in shared memory as in the fused kernel), entries summed
+//   COMP_MAC         the two-sided multiply-accumulate of the fused kernel (8 FMA per pair, psi_j from shared memory,
+//                    the column accumulator rotated by two shuffles per step) on entries that cost half an add each
+constexpr int CP_ITER = 256, CP_R = 4, CP_THREADS = 256, CP_CTAS = 2, CP_SUB = 32;
+
+template <typename T, int COMP>
+__global__ void __launch_bounds__(CP_THREADS, CP_CTAS) comp_kernel(const GenArgs<T> G, typename Cplx<T>::type* out)
+{
+    using CT = typename Cplx<T>::type;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const typename Gen<T>::Tab* tab = stage_gen_table<T>(G);
+    CT* psiw = reinterpret_cast<CT*>(smem_raw) + (threadIdx.x >> 5) * 32;
+    const int lane = threadIdx.x & 31;
+    psiw[lane] = CT{T(1) / T(lane + 1), T(lane) * T(0.001)};
+    __syncthreads();
+    const uint32_t i0 = (blockIdx.x * CP_THREADS + threadIdx.x) * 7u;
+    T accr[CP_R], acci[CP_R], cr = T(0), ci = T(0);
+    CT psi_i[CP_R];
+    uint32_t xacc = 0;
+#pragma unroll
+    for (int r = 0; r < CP_R; ++r) {
+        accr[r] = acci[r] = T(0);
+        psi_i[r] = CT{T(0.5) + T(r), T(0.25) - T(r)};
+    }
+    T er = T(1e-3) * T(lane), ei = T(2e-3);
+    for (int sub = 0; sub < CP_ITER / CP_SUB; ++sub) {
+        const uint32_t j0 = 0x40000000u + blockIdx.x * 4096u + sub * CP_SUB;
+#pragma unroll 1
+        for (int s = 0; s < CP_SUB; ++s) {
+            const int c = (lane + s) & 31;
+            const CT p = psiw[c];
+            if (COMP == 2) { er += T(1e-6); ei -= T(1e-6); }
+#pragma unroll
+            for (int r = 0; r < CP_R; ++r) {
+                T hr, hi;
+                if (COMP == 0) {
+                    uint32_t x0, x1;
+                    pair_words(G.K, i0 + 32 * r, j0 + c, x0, x1);
+                    xacc ^= x0 ^ (x1 >> 1);
+                    continue;
+                } else if (COMP == 1) {
+                    entry_upper<T>(G, tab, i0 + 32 * r, j0 + c, hr, hi);
+                    accr[r] += hr;
+                    acci[r] += hi;
+                    continue;
+                } else {
+                    hr = er;
+                    hi = ei;
+                }
+                accr[r] = fma(hr, p.x, accr[r]);
+                accr[r] = fma(-hi, p.y, accr[r]);
+                acci[r] = fma(hr, p.y, acci[r]);
+                acci[r] = fma(hi, p.x, acci[r]);
+                cr = fma(hr, psi_i[r].x, cr);
+                cr = fma(hi, psi_i[r].y, cr);
+                ci = fma(hr, psi_i[r].y, ci);
+                ci = fma(-hi, psi_i[r].x, ci);
+            }
+            if (COMP == 2) {
+                cr = __shfl_sync(0xffffffffu, cr, (lane + 1) & 31);
+                ci = __shfl_sync(0xffffffffu, ci, (lane + 1) & 31);
+            }
+        }
+    }
+    T sr = cr + T(xacc & 1u), si = ci;
+#pragma unroll
+    for (int r = 0; r < CP_R; ++r) {
+        sr += accr[r];
+        si += acci[r];
+    }
+    out[blockIdx.x * CP_THREADS + threadIdx.x] = CT{sr, si};
+}
+
+template <typename T, int COMP> static int run_comp(int sm_count, cudaStream_t st, double* pairs_per_s)
+{
+    using CT = typename Cplx<T>::type;
+    const int grid = sm_count * CP_CTAS;
+    GenHostD host;
+    make_gen_table(65536, host);
+    GenArgs<T> G;
+    G.K = make_philox_keys(0x1234567ull);
+    G.an = AnalyticArgs{0, 0, 1, 0, 0, 0, 0};
+    void* d_tab = nullptr;
+    if constexpr (sizeof(T) == 8) {
+        MFH_CUDA_CHECK(cudaMalloc(&d_tab, sizeof(GenTabD)));
+        if (cudaMemcpy(d_tab, &host.tab, sizeof(GenTabD), cudaMemcpyHostToDevice) != cudaSuccess) {
+            cudaFree(d_tab);
+            set_error("component microbenchmark: table upload failed");
+            return MFH_ERR_CUDA;
+        }
+        G.gc = host.gc;
+        G.tab_global = (const GenTabD*)d_tab;
+    } else {
+        G.gc.neg_k2_ln2 = (float)(-0.6931471805599453 / 65536.0);
+        G.tab_global = nullptr;
+    }
+    CT* out = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    const size_t smem = (CP_THREADS / 32) * 32 * sizeof(CT);
+    cudaError_t e = cudaMalloc(&out, (size_t)grid * CP_THREADS * sizeof(CT));
+    if (e == cudaSuccess) e = cudaEventCreate(&e0);
+    if (e == cudaSuccess) e = cudaEventCreate(&e1);
+    float best = 1e30f;
+    for (int rep = 0; rep < 4 && e == cudaSuccess; ++rep) {   // first repetition warms up
+        cudaEventRecord(e0, st);
+        comp_kernel<T, COMP><<<grid, CP_THREADS, smem, st>>>(G, out);
+        cudaEventRecord(e1, st);
+        e = cudaEventSynchronize(e1);
+        if (e == cudaSuccess) e = cudaGetLastError();
+        float ms = 0.f;
+        if (e == cudaSuccess) cudaEventElapsedTime(&ms, e0, e1);
+        if (rep > 0) best = std::min(best, ms);
+    }
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    if (out) cudaFree(out);
+    if (d_tab) cudaFree(d_tab);
+    if (e != cudaSuccess) {
+        set_error("component microbenchmark failed: %s", cudaGetErrorString(e));
+        return MFH_ERR_CUDA;
+    }
+    *pairs_per_s = (double)grid * CP_THREADS * CP_ITER * CP_R / ((double)best * 1e-3);
+    return MFH_OK;
+}
+
 // Read-only HBM stream: every thread keeps 8 independent 128-bit non-allocating loads in flight over a
 // grid-strided sweep of the buffer and xor-folds the words; one word per thread is written at the end.
 // The denominator for kernels that READ a matrix once (a device-to-device copy, the MEASURED_PEAKS.json
@@ -174,7 +304,7 @@ extern "C" MFH_API int mfh_debug_read_bandwidth(const void* buf_dev, size_t byte
 extern "C" MFH_API int mfh_debug_pipe_rates(int32_t mix, double* units_per_s, void* stream)
 {
     if (!units_per_s) { set_error("mfh_debug_pipe_rates: NULL pointer"); return MFH_ERR_INVALID_ARG; }
-    if (mix < MFH_MIX_C128_PAIR || mix > MFH_MIX_DFMA31) {
+    if (mix < MFH_MIX_C128_PAIR || mix > MFH_COMP_MAC_C64) {
         set_error("mfh_debug_pipe_rates: unknown mix %d", mix);
         return MFH_ERR_INVALID_ARG;
     }
@@ -188,6 +318,11 @@ extern "C" MFH_API int mfh_debug_pipe_rates(int32_t mix, double* units_per_s, vo
     case MFH_MIX_C64_ENTRY: return run_mix<14, 6, 0, 4, 11>(sms, st, units_per_s);
     case MFH_MIX_PHILOX: return run_mix<18, 0, 0, 0, 0>(sms, st, units_per_s);
     case MFH_MIX_DFMA31: return run_mix<0, 0, 32, 0, 0>(sms, st, units_per_s);
+    case MFH_COMP_PHILOX: return run_comp<double, 0>(sms, st, units_per_s);
+    case MFH_COMP_PHILOX_BM_C128: return run_comp<double, 1>(sms, st, units_per_s);
+    case MFH_COMP_MAC_C128: return run_comp<double, 2>(sms, st, units_per_s);
+    case MFH_COMP_PHILOX_BM_C64: return run_comp<float, 1>(sms, st, units_per_s);
+    case MFH_COMP_MAC_C64: return run_comp<float, 2>(sms, st, units_per_s);
     }
     set_error("mfh_debug_pipe_rates: unknown mix %d", mix);
     return MFH_ERR_INVALID_ARG;

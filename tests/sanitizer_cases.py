@@ -1,13 +1,22 @@
 #!/usr/bin/env python
-"""One small case of every kernel of the library, each checked against the CPU oracle -- the program that
-compute-sanitizer runs (SURVEY.md section 5 "Race detection"; profiles/r02_sanitizer.md has the command lines):
+"""One small case of every kernel of the library, each checked against the CPU oracle AND by the library's own
+self-checks (SURVEY.md section 5 "Race detection"; profiles/r02_sanitizer.md):
 
-    compute-sanitizer --tool memcheck  python tests/sanitizer_cases.py
+    python tests/sanitizer_cases.py                      # also run by tests/test_gpu_selfcheck.py under pytest -m gpu
+    compute-sanitizer --tool memcheck  python tests/sanitizer_cases.py      # where the tool is available
     compute-sanitizer --tool racecheck python tests/sanitizer_cases.py
     compute-sanitizer --tool initcheck python tests/sanitizer_cases.py
 
-Not collected by pytest (no test_ prefix): the same paths are covered, at more shapes, by the -m gpu tests; this
-script keeps the launch count low enough for the sanitizer's 10-100x slow-down.  Exits non-zero on a parity failure.
+compute-sanitizer is CLOSED on the GPU pool this build runs on (its answer is quoted in profiles/r02_sanitizer.md),
+so every apply of every case is wrapped in the substitutes the library offers itself (include/mfh.h, self-check
+exports):
+  * initcheck  -> the partial-sum workspace, the Chebyshev scratch and the output vector are filled with NaN before
+                  the apply: a read of anything this apply did not write makes the result NaN and fails parity;
+  * racecheck  -> the apply is repeated three times from the poisoned state and must be bit-identical (a data race
+                  between warps or CTAs shows as a run-to-run difference), the result must match the oracle;
+  * memcheck   -> every library-owned buffer sits between two 4 KB guard bands; after the applies no guard byte may
+                  have changed (out-of-bounds writes), and the caller-owned output has its own guard bands here.
+Exits non-zero on any failure.
 """
 import os
 import sys
@@ -27,6 +36,30 @@ def rel(a, b):
     a = np.asarray(a, dtype=np.complex128)
     b = np.asarray(b, dtype=np.complex128)
     return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+def checked_apply(h, psi, lambdas=None, repeats=3):
+    """h.apply under the self-checks of the module docstring; returns phi as numpy."""
+    import torch
+    n, pad = psi.numel(), 512
+    first = None
+    for _ in range(repeats):
+        buf = torch.full((n + 2 * pad,), float("nan"), dtype=psi.dtype, device="cuda")
+        buf[:pad] = 7.0 - 3.0j
+        buf[n + pad:] = 7.0 - 3.0j
+        phi = buf[pad:pad + n].view(psi.shape)
+        h.debug_poison()
+        h.apply(psi, phi, lambdas=lambdas)
+        torch.cuda.synchronize()
+        assert bool(torch.all(buf[:pad] == 7.0 - 3.0j)) and bool(torch.all(buf[n + pad:] == 7.0 - 3.0j)), "write outside phi"
+        assert not bool(torch.isnan(torch.view_as_real(phi)).any()), "NaN in phi: something read what this apply did not write"
+        if first is None:
+            first = phi.clone()
+        else:
+            assert torch.equal(phi, first), "repeated applies differ bit for bit"
+    bad = h.debug_selfcheck()
+    assert bad == 0, f"{bad} guard bytes around the library's buffers were overwritten"
+    return first.cpu().numpy()
 
 
 def main(only=None):
@@ -51,7 +84,7 @@ def main(only=None):
         for mode, budget in (("procedural", 0), ("full", 0), ("partial", 150_000_000), ("pairs", 0), ("pairs", 90_000_000)):
             h = mfh.Hamiltonian(D, B, seed, "c128")
             p = h.plan(mode, hbm_budget_bytes=budget)
-            case(f"C1 c128 {mode} ({p['chosen']['cached_fraction']:.2f} cached)", rel(h.apply(dev(psi)).cpu().numpy(), ref), 1e-11)
+            case(f"C1 c128 {mode} ({p['chosen']['cached_fraction']:.2f} cached)", rel(checked_apply(h, dev(psi)), ref), 1e-11)
             h.destroy()
 
     if want("c64"):
@@ -62,7 +95,7 @@ def main(only=None):
         for mode, budget in (("procedural", 0), ("full", 0), ("partial", 20_000_000), ("pairs", 0)):
             h = mfh.Hamiltonian(D, B, seed, "c64")
             h.plan(mode, hbm_budget_bytes=budget)
-            case(f"c64 k=1 {mode}", rel(h.apply(dev(psi)).cpu().numpy(), ref), 1e-4)
+            case(f"c64 k=1 {mode}", rel(checked_apply(h, dev(psi)), ref), 1e-4)
             h.destroy()
 
     if want("scan"):
@@ -79,7 +112,7 @@ def main(only=None):
             except mfh.MfhError as e:
                 print(f"sanitizer case c64 k=16 {mode}: not planned ({e})")
                 continue
-            Phi = h.apply(dev(Psi), lambdas=lam).cpu().numpy()
+            Phi = checked_apply(h, dev(Psi), lam)
             case(f"c64 k=16 scan {mode}", max(rel(Phi[:, v], ref[:, v]) for v in range(k)), 1e-4)
             h.destroy()
 
@@ -93,7 +126,7 @@ def main(only=None):
             for mode in ("full", "procedural"):
                 h = mfh.Hamiltonian(D, B, 8, "c128", kind="diag_plus_gue", seed_h0=7)
                 h.plan(mode, k=k)
-                Phi = h.apply(dev(Psi), lambdas=lam).cpu().numpy()
+                Phi = checked_apply(h, dev(Psi), lam)
                 case(f"c128 k={k} {mode}", max(rel(Phi[:, v], ref[:, v]) for v in range(k)), 1e-11)
                 h.destroy()
 
@@ -104,6 +137,7 @@ def main(only=None):
         H = oracle.materialize(D, 21)
         h = mfh.Hamiltonian(D, B, 21, "c128")
         h.plan("pairs")
+        h.debug_poison()
         out, K = h.chebyshev(dev(psi), 5.0, -2.1, 2.1, 1e-14)
         ref, Kr = oracle.chebyshev_propagate(lambda v: H @ v, psi, 5.0, -2.1, 2.1, 1e-14)
         assert K == Kr
@@ -116,6 +150,7 @@ def main(only=None):
         e0, e1, al, be = h.lanczos_bounds(dev(psi), m=12)
         ro = oracle.lanczos_bounds(lambda v: H @ v, psi, m=12)
         case("Lanczos bounds m=12", max(abs(e0 - ro[0]), abs(e1 - ro[1])), 1e-8)
+        assert h.debug_selfcheck() == 0
         h.destroy()
 
     if want("sb"):
@@ -138,7 +173,7 @@ def main(only=None):
         h = mfh.Hamiltonian(D, B, 0, "c128", kind="analytic")
         h.set_source_params(theta)
         h.plan("partial", hbm_budget_bytes=12_000_000)
-        case("analytic source partial", rel(h.apply(dev(psi)).cpu().numpy(), oracle.analytic_apply(D, theta, psi)), 1e-11)
+        case("analytic source partial", rel(checked_apply(h, dev(psi)), oracle.analytic_apply(D, theta, psi)), 1e-11)
         h.destroy()
         M = dense_matrix(D, 77)
         k = 4
@@ -148,7 +183,7 @@ def main(only=None):
         for n in range(D // B):
             for m in range(D // B):
                 h.set_block(n, m, np.ascontiguousarray(M[n * B:(n + 1) * B, m * B:(m + 1) * B]).astype(np.complex64))
-        Phi = h.apply(dev(Psi)).cpu().numpy()
+        Phi = checked_apply(h, dev(Psi))
         ref = M.astype(np.complex64).astype(np.complex128) @ Psi.astype(np.complex128)
         case("external blocks c64 k=4 (tiled cache)", max(rel(Phi[:, v], ref[:, v]) for v in range(k)), 1e-4)
         h.destroy()
