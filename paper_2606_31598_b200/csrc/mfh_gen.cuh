@@ -10,6 +10,7 @@
 // sincospi cost ~210 instructions per entry; the table-driven forms below cost ~50 and keep the
 // absolute error of an entry below 1e-13 of its scale (tolerance of phi: 1e-11 relative L2).
 #pragma once
+#include <cstddef>
 #include <cstdint>
 #include <cuda_runtime.h>
 
@@ -106,16 +107,14 @@ __device__ __forceinline__ void pair_words(const PhiloxKeys& K, uint32_t lo, uin
 constexpr int GEN_LOG_BITS = 8;
 constexpr int GEN_SC_BITS = 10;
 
-// Layout: the shared-memory copy is aligned to 16 KB, tsc (16 KB) first, tlog (4 KB) second, so that a table index
-// placed in bits 4..13 (tsc, elog) or 4..11 (tlog) is OR-ed into the table's shared address by the same LOP3 that masks
-// it ((x & mask) | base): no integer add per look-up.
 struct GenTabD {                         // built on the host by make_gen_table(), copied to shared memory
     double2 tsc[1 << GEN_SC_BITS];       // (cos A, sin A),  A = 2 pi (idx 2^22 + 2^21 + 1/2) 2^-32
     double2 tlog[1 << GEN_LOG_BITS];     // (1/c, -K2 ln c)
     double elog[34];                     // K2 (32 - e) ln 2 for e = -1..31  (index e + 1)
 };
-constexpr uint32_t GEN_TAB_ALIGN = 16384;
-static_assert(sizeof(double2) * (1 << GEN_SC_BITS) == GEN_TAB_ALIGN, "tsc must fill the alignment unit");
+// The shared-memory copy every generating kernel stages (stage_gen_table): a FILE-SCOPE __shared__ object, so that
+// its address is a compile-time constant inside each kernel.
+__shared__ __align__(16) GenTabD g_gen_tab_d;
 
 struct GenConstD {                       // kernel-parameter constants (constant bank operands)
     double c1, c2, c3, c4;               // -K2 log1p(r) = r (c1 + r (c2 + r (c3 + r c4)))
@@ -137,7 +136,7 @@ template <> struct Gen<double> {
     using Const = GenConstD;
     static constexpr int TAB_BYTES = (int)sizeof(GenTabD);
 
-    __device__ __forceinline__ static void normals(const GenTabD* __restrict__ tab, const GenConstD& gc,
+    __device__ __forceinline__ static void normals(const GenTabD*, const GenConstD& gc,
                                                    uint32_t x0, uint32_t x1, double& a, double& b)
     {
         // radius: d = x0 + 1/2 exactly (2^52 + x0 by bit pattern, minus 2^52 - 1/2)
@@ -146,15 +145,11 @@ template <> struct Gen<double> {
         uint32_t mh;                                                     // mantissa with exponent 0: one LOP3
         asm("lop3.b32 %0, %1, 0x000fffff, 0x3ff00000, 0xEA;" : "=r"(mh) : "r"(hi));
         const double m = __hiloint2double((int)mh, __double2loint(d));
-        // shared-memory addresses of the look-ups: (index field & mask) | table base in ONE LOP3 each (see GenTabD)
-        const uint32_t ts = (uint32_t)__cvta_generic_to_shared(tab);    // 16 KB aligned; loop invariant
-        uint32_t a_log, a_exp;
-        asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(a_log) : "r"(hi >> (20 - GEN_LOG_BITS - 4)), "n"(((1 << GEN_LOG_BITS) - 1) << 4), "r"(ts + GEN_TAB_ALIGN));
-        asm("lop3.b32 %0, %1, 0x3ff8, %2, 0xEA;" : "=r"(a_exp) : "r"(hi >> 17), "r"(ts));
-        double2 tl;
-        double el;
-        asm("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(tl.x), "=d"(tl.y) : "r"(a_log));
-        asm("ld.shared.f64 %0, [%1 + %2];" : "=d"(el) : "r"(a_exp), "n"((int)(GEN_TAB_ALIGN + sizeof(double2) * (1 << GEN_LOG_BITS)) - 1022 * 8));
+        // byte offsets of the look-ups; the table is a file-scope __shared__ object, so its address is a compile-time
+        // constant that folds into the immediate of each LDS (no integer add for the base)
+        const char* tb = reinterpret_cast<const char*>(&g_gen_tab_d);
+        const double2 tl = *reinterpret_cast<const double2*>(tb + offsetof(GenTabD, tlog) + ((hi >> (20 - GEN_LOG_BITS - 4)) & (((1u << GEN_LOG_BITS) - 1u) << 4)));
+        const double el = *reinterpret_cast<const double*>(tb + ((int)offsetof(GenTabD, elog) - 1022 * 8) + ((hi >> 17) & 0x3ff8u));
         const double r = fma(m, tl.x, -1.0);
         double p = fma(r, gc.c4, gc.c3);
         p = fma(r, p, gc.c2);
@@ -170,10 +165,7 @@ template <> struct Gen<double> {
         const double rad = fma(sq, e * fma(e, 0.375, 0.5), sq);
         // angle: residual of x1 inside its bin, centred by the constant term of one FMA (exact: 2^21 ang is ang scaled
         // by a power of two)
-        uint32_t a_sc;
-        asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(a_sc) : "r"(x1 >> (32 - GEN_SC_BITS - 4)), "n"(((1 << GEN_SC_BITS) - 1) << 4), "r"(ts));
-        double2 cs;
-        asm("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(cs.x), "=d"(cs.y) : "r"(a_sc));
+        const double2 cs = *reinterpret_cast<const double2*>(tb + offsetof(GenTabD, tsc) + ((x1 >> (32 - GEN_SC_BITS - 4)) & (((1u << GEN_SC_BITS) - 1u) << 4)));
         const double bb = fma((double)(int)(x1 & ((1u << (32 - GEN_SC_BITS)) - 1u)), gc.ang, gc.ang_off);
         const double b2 = bb * bb;
         const double sb = fma(b2 * (-1.0 / 6.0), bb, bb);
@@ -245,19 +237,18 @@ __device__ __forceinline__ void analytic_entry(const AnalyticArgs& A, uint32_t i
     hi = (T)(i < j ? a * A.sphi : -(a * A.sphi));
 }
 
-// Copy the generator table to shared memory (all threads of the CTA; caller synchronises).  The table is STATIC shared
-// memory, so its address is a link-time constant that folds into the immediate offset of every table look-up (with a
-// dynamic allocation each look-up paid an extra integer add for the base).
+// Copy the generator table to shared memory (all threads of the CTA; caller synchronises).
 template <typename T>
 __device__ __forceinline__ const typename Gen<T>::Tab* stage_gen_table(const GenArgs<T>& G)
 {
-    __shared__ __align__(Gen<T>::TAB_BYTES > 0 ? GEN_TAB_ALIGN : 16) typename Gen<T>::Tab s_gen_tab;
     if constexpr (Gen<T>::TAB_BYTES > 0) {
         const uint4* src = reinterpret_cast<const uint4*>(G.tab_global);
-        uint4* dst = reinterpret_cast<uint4*>(&s_gen_tab);
+        uint4* dst = reinterpret_cast<uint4*>(&g_gen_tab_d);
         for (int t = threadIdx.x; t < Gen<T>::TAB_BYTES / 16; t += blockDim.x) dst[t] = src[t];
+        return &g_gen_tab_d;
+    } else {
+        return nullptr;
     }
-    return &s_gen_tab;
 }
 
 // General entry H_ij for any (i,j): conjugate below the diagonal, real and scaled by 1/sqrt(D)
