@@ -211,7 +211,8 @@ def measure_config(torch, mfh, name: str, steps: int, warmup: int, with_e2e: boo
     psi_np = make_psi(D, cfg["psi_seed"], k=k, dtype=cfg["dtype"])
     lam = lambda_grid(k) if k > 1 else None
     t0 = time.perf_counter()
-    h, plan = make_handle(mfh, cfg, max(steps, 1))
+    # configs[4] (C5) is one Chebyshev propagation of 151 applies: that is the job its plan is made for
+    h, plan = make_handle(mfh, cfg, 151 if "t" in cfg else max(steps, 1))
     torch.cuda.synchronize()
     plan_s = time.perf_counter() - t0
     info = h.get_plan()
@@ -390,6 +391,29 @@ def measure_auto_planner(torch, mfh) -> dict:
     return out
 
 
+def measure_pipe_model(mfh) -> dict:
+    """Which instruction classes of the generator overlap on this GPU: units/s of the library's
+    synthetic kernels and the clocks one warp instruction of the class costs a scheduler at 1.965 GHz nominal.  A pair
+    of classes that takes the sum of its parts does not overlap."""
+    n = {"pipe_wide16": 32, "pipe_lop32": 32, "pipe_dfma32": 33, "pipe_dfma32_reg3": 33, "pipe_wide16_dfma32": 65,
+         "pipe_lop32_dfma32": 65, "pipe_wide16_lop32": 64}
+    out = {}
+    for name, instr in n.items():
+        r = mfh.pipe_rate(name)
+        clk = 148 * 4 * 1.965e9 / (r / 32.0)      # scheduler clocks per warp-unit
+        out[name] = {"units_per_s": r, "clk_per_warp_unit": clk, "instructions_per_unit": instr}
+    c = {k: v["clk_per_warp_unit"] for k, v in out.items()}
+    out["summary"] = {
+        "dfma_clk_immediate_operands": c["pipe_dfma32"] / 33, "dfma_clk_three_register_operands": c["pipe_dfma32_reg3"] / 33,
+        "wide_plus_dfma_over_sum": c["pipe_wide16_dfma32"] / (c["pipe_wide16"] + c["pipe_dfma32"]),
+        "lop_plus_dfma_over_max": c["pipe_lop32_dfma32"] / max(c["pipe_lop32"], c["pipe_dfma32"]),
+        "wide_plus_lop_over_sum": c["pipe_wide16_lop32"] / (c["pipe_wide16"] + c["pipe_lop32"]),
+        "fp64_peak_fraction_with_three_register_dfma": (c["pipe_dfma32"] / 33) / (c["pipe_dfma32_reg3"] / 33) * (2.0 / (c["pipe_dfma32"] / 33)),
+        "note": "ratios near 1.0 over the SUM mean the two classes serialise (32x32->64 multiply against DFMA and "
+                "against logic ops); near 1.0 over the MAX mean they overlap (logic ops under DFMA)"}
+    return out
+
+
 def roofline_for(res: dict, hbm_gbs: float, peak_src: str) -> dict:
     """Roofline of the dominant kernel of one apply."""
     cfg = res["cfg"]
@@ -411,8 +435,12 @@ def roofline_for(res: dict, hbm_gbs: float, peak_src: str) -> dict:
         flops = 8.0 * D * D * k * res["plan"]["cached_fraction"]
         tf = flops / (kern["cached"] * 1e-3) / 1e12
         peak = 148 * 64 * 2 * 1.965e9 / 1e12
+        # second number: the rate at which DFMAs with three register operands issue on this GPU (measured now); the
+        # kernel's multiply-accumulates read the entry, the psi value and the accumulator from registers
+        reg3 = res["pipe_rate"]("pipe_dfma32_reg3") * 33 * 2 / 1e12
         return {"kernel": "cached_multi_kernel_c128", "bound": "alu", "achieved": tf, "peak": peak, "unit": "TFLOP/s",
                 "frac": tf / peak, "traffic": None, "traffic_source": None,
+                "three_register_dfma_ceiling": reg3, "frac_of_three_register_dfma_ceiling": tf / reg3,
                 "peak_source": "nominal FP64: 148 SMs x 64 DFMA lanes/clk x 2 flop x 1.965 GHz (B200_PROFILING.md unit counts; "
                                "the SM clock under FP64 load is power-capped below that)",
                 "kernel_ms": kern["cached"], "share_of_step": kern["cached"] / max(kern["total"], 1e-9)}
@@ -668,6 +696,10 @@ def main():
             extras["C1-graph"] = measure_graph_replay(torch, mfh)
         except Exception as e:
             extras["C1-graph"] = {"error": str(e)}
+        try:
+            extras["pipe-model"] = measure_pipe_model(mfh)
+        except Exception as e:
+            extras["pipe-model"] = {"error": str(e)}
         try:
             extras["C4-partitioned"] = measure_partition_projection(torch, mfh)
         except Exception as e:

@@ -354,9 +354,17 @@ MFH_API int mfh_debug_h0(mfh_handle h, void* h0_dev, void* stream);
  *   MFH_COMP_MAC_C128        the two-sided multiply-accumulate alone (8 DFMA per pair, psi_j from shared memory, the
  *                            column accumulator rotated by shuffles) on entries that cost half an add each
  *   MFH_COMP_PHILOX_BM_C64 / MFH_COMP_MAC_C64   the same for the complex64 CUDA-core kernel (SFU Box-Muller, FFMA)
+ * Pipe model (which instruction classes of the generator overlap on this GPU; units per second of the synthetic
+ * kernel, one unit = the named instructions per lane):
+ *   MFH_PIPE_WIDE16 (16 32x32->64 multiplies + 16 xors), MFH_PIPE_LOP32 (32 logic ops), MFH_PIPE_DFMA32 (32 DFMA with
+ *   immediate operands), MFH_PIPE_DFMA32_REG3 (32 DFMA with three register operands), and the pairs
+ *   MFH_PIPE_WIDE16_DFMA32, MFH_PIPE_LOP32_DFMA32, MFH_PIPE_WIDE16_LOP32: a pair that takes as long as the sum of
+ *   its parts does not overlap.
  * Synchronises `stream`.  Errors: INVALID_ARG, CUDA. */
 enum { MFH_MIX_C128_PAIR = 0, MFH_MIX_C64_ENTRY = 1, MFH_MIX_PHILOX = 2, MFH_MIX_DFMA31 = 3, MFH_COMP_PHILOX = 4,
-       MFH_COMP_PHILOX_BM_C128 = 5, MFH_COMP_MAC_C128 = 6, MFH_COMP_PHILOX_BM_C64 = 7, MFH_COMP_MAC_C64 = 8 };
+       MFH_COMP_PHILOX_BM_C128 = 5, MFH_COMP_MAC_C128 = 6, MFH_COMP_PHILOX_BM_C64 = 7, MFH_COMP_MAC_C64 = 8,
+       MFH_PIPE_WIDE16 = 9, MFH_PIPE_LOP32 = 10, MFH_PIPE_DFMA32 = 11, MFH_PIPE_DFMA32_REG3 = 12,
+       MFH_PIPE_WIDE16_DFMA32 = 13, MFH_PIPE_LOP32_DFMA32 = 14, MFH_PIPE_WIDE16_LOP32 = 15 };
 MFH_API int mfh_debug_pipe_rates(int32_t mix, double* units_per_s, void* stream);
 
 /* Read-only HBM stream probe: times a kernel that reads `bytes` of buf_dev once (8 independent 128-bit

@@ -96,6 +96,7 @@ static int commit_plan(mfh_handle h, const Plan& p, cudaStream_t st)
 {
     free_plan_resources(h);
     h->plan = p;
+    h->plan.strip_tiled = partial_overlap_supported(h);   // the streaming role reads 16 KB tiles (mfh_proc.cu)
     const Plan& q = h->plan;
     const size_t cb = complex_bytes(h->dtype);
     cudaError_t e;
@@ -508,6 +509,7 @@ MFH_API int mfh_plan(mfh_handle h, int32_t mode, int32_t k, int64_t n_applies_hi
         p.k = k;
         p.cached_per_row = c.cached_per_row;
         p.pairs = c.pairs;
+        p.stream_sms = c.stream_sms;
         p.part_rank = part.rank;
         p.part_world = part.world;
         p.part_scheme = part.scheme;
@@ -564,13 +566,13 @@ MFH_API int mfh_get_plan(mfh_handle h, char* json_out, size_t json_cap)
              "{\"partition\":{\"scheme\":\"%s\",\"rank\":%d,\"world\":%d,\"owned_blocks\":%lld,\"first_block_row\":%d,\"block_rows\":%d},"
              "\"mode\":\"%s\",\"B\":%d,\"n_blk\":%d,\"k\":%d,\"cached_blocks\":%lld,\"cached_per_row\":%d,"
              "\"cached_fraction\":%.6g,\"cache_bytes\":%zu,\"work_bytes\":%zu,\"partial_slots\":%d,\"proc_items\":%zu,\"pair_items\":%zu,"
-             "\"proc_rows_per_lane\":%d,\"proc_row_strips\":%d,\"launches_per_apply\":%d}",
+             "\"proc_rows_per_lane\":%d,\"proc_row_strips\":%d,\"stream_sms\":%d,\"launches_per_apply\":%d}",
              p.part_scheme == MFH_PART_ROWS ? "rows" : (p.part_scheme == MFH_PART_PAIRS ? "pairs" : "none"), p.part_rank, p.part_world,
              (long long)p.owned_blocks, p.row_first, p.row_count,
              p.mode == MFH_MODE_FULL ? "full" : (p.mode == MFH_MODE_PARTIAL ? "partial" : (p.mode == MFH_MODE_PAIRS ? "pairs" : "procedural")), p.B,
              p.n_blk, p.k, (long long)p.n_cached, p.cached_per_row,
              (double)p.covered_blocks / (double)std::max<int64_t>(p.owned_blocks, 1), p.cache_bytes, p.work_bytes, p.n_slots,
-             p.items.size(), p.pair_items.size(), p.R, p.Q,
+             p.items.size(), p.pair_items.size(), p.R, p.Q, p.stream_sms,
              h->fused_tail ? 1 : 1 + (p.n_cached > 0) + ((p.k == 1 && !p.items.empty()) ||
                                                           (p.k > 1 && p.covered_blocks < p.owned_blocks)));
     copy_json(buf, json_out, json_cap);

@@ -44,12 +44,25 @@ __host__ __device__ inline size_t tiled_cache_offset(int B, int a, int b)
     return ((size_t)rt * (B >> 4) + kt) * 4096 + (size_t)r * 32 + (size_t)((c ^ (r & 7)) << 2) + (size_t)((b & 1) << 1);
 }
 
+// Strip-tiled cache layout of one-vector PARTIAL plans (the streaming role of partial_overlap_kernel, mfh_proc.cu):
+// element (a, b) of a B x B block, in complex elements from the block start.  A tile is 8 rows x `cols` columns
+// (cols = STRIP_PIECE_BYTES of complex: 64 complex128 / 128 complex64), 8 KB contiguous, tiles ordered column chunk
+// fastest inside an 8-row strip -- so a strip's pass over a block is one contiguous run and every stage of a
+// streaming warp's ring is ONE bulk copy.
+constexpr int STRIP_PIECE_BYTES = 1024;
+__host__ __device__ inline size_t strip_tile_offset(int B, int cols, int a, int b)
+{
+    return ((size_t)(a >> 3) * (B / cols) + (size_t)(b / cols)) * (size_t)(8 * cols) + (size_t)(a & 7) * cols + (size_t)(b % cols);
+}
+
 struct Plan {
     int32_t mode = 0;          // MFH_MODE_* actually committed
     int32_t B = 0, n_blk = 0, k = 0;
     int32_t Q = 1;             // row strips per block in the procedural kernel
     int32_t R = 4;             // rows per lane in the procedural kernel (row tile = 32*R rows)
+    int32_t stream_sms = 0;    // partial plans: SMs whose CTAs stream cached blocks while the others generate (Eq. 33)
     bool pairs = false;        // Hermitian pair cache: store block (n,m), n <= m, use it for both sides
+    bool strip_tiled = false;  // cached blocks stored in the strip-tiled layout (partial plans run by partial_overlap_kernel)
     int64_t n_cached = 0;      // stored blocks
     int64_t covered_blocks = 0;   // block positions (n,m) served from the cache
     int32_t cached_per_row = 0;

@@ -29,6 +29,33 @@ static double gen_entries_per_s(int dtype, int k)
     return 1.0 / (1.0 / gen + (double)k / mac);
 }
 
+// Read bandwidth of n SMs streaming alone (2 CTAs x 8 warps per SM, 16 x 128-bit loads in flight per lane), measured
+// on one B200 with the other SMs idle: one SM pulls up to ~140 GB/s, 48 SMs already 6.0 TB/s, 64 SMs 7.0 TB/s
+// (DESIGN.md 6.6).  Derated by 7 % for the strip loop's arithmetic and psi staging.
+static double stream_bw_of_sms(int n, int sm_count)
+{
+    static const double pts[] = {0, 16, 32, 40, 48, 56, 64, 80, 96, 148};
+    static const double gbs[] = {0, 2331, 4377, 5262, 6017, 6549, 6964, 7319, 7449, 7430};
+    const double x = 148.0 * n / std::max(sm_count, 1);
+    for (int i = 1; i < 10; ++i)
+        if (x <= pts[i]) return 0.93e9 * (gbs[i - 1] + (gbs[i] - gbs[i - 1]) * (x - pts[i - 1]) / (pts[i] - pts[i - 1]));
+    return 0.93e9 * gbs[9];
+}
+
+// Eq. 33 with the SMs partitioned between the two parts: n SMs stream the cached bytes, S - n generate;
+// T(n) = max(bytes / BW(n), t_gen S / (S - n)).  Returns the n that minimises it and the time.
+int choose_stream_sms(double cache_bytes, double t_gen_all_sms, int sm_count, double* t_out)
+{
+    int best = 1;
+    double tb = 1e300;
+    for (int n = 1; n < sm_count; ++n) {
+        const double t = std::max(cache_bytes / stream_bw_of_sms(n, sm_count), t_gen_all_sms * sm_count / (double)(sm_count - n));
+        if (t < tb) { tb = t; best = n; }
+    }
+    if (t_out) *t_out = tb;
+    return best;
+}
+
 static void appendf(std::string& s, const char* fmt, ...)
 {
     char buf[512];
@@ -328,6 +355,12 @@ Candidate evaluate_candidate(int64_t D, int dtype, int k, int B, int cached_per_
     int launches = 1 + (p.n_cached > 0) + (p.covered_blocks < p.owned_blocks);
     c.t_reduce = (double)p.n_slots * 0.6 * D * k * cb / kBwRead;
     c.t_apply = c.t_cached + c.t_proc + c.t_reduce + launches * kLaunch;   // Eq. 32 (not overlapped)
+    if (k == 1 && !pairs && p.n_cached > 0 && !p.items.empty()) {
+        // one kernel, SMs partitioned between streaming and generating (Eq. 33: the max, not the sum)
+        double t_max = 0.0;
+        c.stream_sms = choose_stream_sms(c.cache_bytes, c.t_proc, sm_count, &t_max);
+        c.t_apply = t_max + c.t_reduce + 2 * kLaunch;
+    }
     const double stored = c.cache_bytes / cb;
     c.t_fill = stored / gen_entries_per_s(dtype, 0) + c.cache_bytes / kBwWrite;
     c.t_job = (double)std::max<int64_t>(n_applies, 1) * c.t_apply + c.t_fill;

@@ -88,7 +88,8 @@ __global__ void __launch_bounds__(256) fill_kernel(const GenArgs<T> G, int32_t B
             CT v;
             v.x = hr;
             v.y = hi;
-            if (tiled) reinterpret_cast<CT*>(reinterpret_cast<T*>(out + base) + tiled_cache_offset(B, a, b))[0] = v;
+            if (tiled == 1) reinterpret_cast<CT*>(reinterpret_cast<T*>(out + base) + tiled_cache_offset(B, a, b))[0] = v;
+            else if (tiled == 2) out[base + strip_tile_offset(B, STRIP_PIECE_BYTES / (int)sizeof(CT), a, b)] = v;
             else row[b] = v;
         }
     }
@@ -125,9 +126,11 @@ int launch_fill_cache(mfh_handle h, cudaStream_t st)
     int rc = ensure_gen_table(h, st);
     if (rc) return rc;
     dim3 grid(p.n_blk * p.n_blk, std::min(p.B, 64));
+    // layouts: 0 row-major blocks, 1 the 16 KB tiles of complex64 k-vector plans, 2 the strip tiles of partial plans
+    const int strip = p.strip_tiled ? 2 : 0;
     return h->dtype == MFH_C128
-               ? launch_fill_t<double>(h, grid, p.B, p.n_blk, h->d_cache_slot, 0, 0, 0, h->d_cache, st)
-               : launch_fill_t<float>(h, grid, p.B, p.n_blk, h->d_cache_slot, 0, 0, p.k > 1 ? 1 : 0, h->d_cache, st);
+               ? launch_fill_t<double>(h, grid, p.B, p.n_blk, h->d_cache_slot, 0, 0, strip, h->d_cache, st)
+               : launch_fill_t<float>(h, grid, p.B, p.n_blk, h->d_cache_slot, 0, 0, p.k > 1 ? 1 : strip, h->d_cache, st);
 }
 
 // External block (Eq. 10) -> cache slot: a plain copy for row-major caches, a re-layout for the tiled cache
@@ -234,7 +237,18 @@ __device__ __forceinline__ void reduce_block_row(const ProcParams<T>& P, int b)
     for (int a = threadIdx.x; a < P.B; a += PROC_THREADS) {
         const size_t i = (size_t)b * P.B + a;
         double sr = 0.0, si = 0.0;
-        for (int t = 0; t < cnt; ++t) {
+        int t = 0;
+        for (; t + 8 <= cnt; t += 8) {   // eight independent loads in flight, added in list order
+            CT x[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) x[u] = __ldcg(P.work + (size_t)list[1 + t + u] * P.D + i);
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                sr += (double)x[u].x;
+                si += (double)x[u].y;
+            }
+        }
+        for (; t < cnt; ++t) {
             const CT x = __ldcg(P.work + (size_t)list[1 + t] * P.D + i);
             sr += (double)x.x;
             si += (double)x.y;
@@ -409,86 +423,183 @@ template <typename T> struct StripParams {
     int32_t* counter;
 };
 
-constexpr int STRIP_RPW = 4, STRIP_ROWS = PROC_WARPS * STRIP_RPW, STRIP_U = 4;
+// Streaming role.  A strip is STRIP_ROWS = 8 whole operator rows over all cached blocks of the block row.  The bytes
+// are moved by the TMA engine, not by load instructions: STRIP_WS warps per CTA each run their OWN two-stage ring --
+// a stage is one 8 KB tile of the strip-tiled cache layout (8 row pieces of 1 KB, contiguous: ONE bulk copy) plus the
+// matching 1 KB of psi^[m] -- and multiply what they loaded themselves: no CTA-wide barrier, no hand-over between
+// warps.  Measured on B200: bulk copies issued by one thread are serviced one after the other
+// (~0.27 us each whatever their size up to 32 KB), copies of different warps overlap; a register-staged loop tops
+// out near 56 GB/s per SM, a CTA-wide ring with one issuing thread near 30 GB/s per CTA, per-warp rings reach the
+// ~125 GB/s an SM's 64 B/clk port allows -- which is what lets FEW SMs pull most of the HBM bandwidth while the
+// others generate.  Lane = 16-byte unit of a row piece; 8 complex row accumulators per lane, summed over the lanes by
+// shuffles at the end of the strip, one warp per strip: no atomics, fixed summation order.
+constexpr int STRIP_ROWS = 8;                   // rows per strip (and per tile)
+constexpr int STRIP_PIECE = STRIP_PIECE_BYTES;   // bytes of one row piece (and of the psi piece)
+constexpr int STRIP_TILE = STRIP_ROWS * STRIP_PIECE;
+constexpr int STRIP_STAGE = STRIP_TILE + STRIP_PIECE;
+constexpr int STRIP_WS = 4;                     // streaming warps per CTA (one per scheduler)
+constexpr int STRIP_SMEM = STRIP_WS * 2 * STRIP_STAGE;
 
-__device__ __forceinline__ double2 ldg_stream_d2(const double2* p)
+__device__ __forceinline__ uint32_t sm_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void sm_mbar_wait(uint64_t* bar, uint32_t parity)
 {
-    double2 v;
-    asm volatile("ld.global.nc.L1::no_allocate.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
-    return v;
+    uint32_t done;
+    do {
+        asm volatile(
+            "{\n\t"
+            ".reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t"
+            "}\n"
+            : "=r"(done)
+            : "r"(sm_u32(bar)), "r"(parity)
+            : "memory");
+    } while (!done);
+}
+__device__ __forceinline__ void bulk_load(void* dst_smem, const void* src, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(sm_u32(dst_smem)),
+                 "l"(src), "r"(bytes), "r"(sm_u32(bar))
+                 : "memory");
 }
 
-__device__ __forceinline__ void cached_strips(const StripParams<double>& S, unsigned char* smem_raw)
+// acc += h * p for the 16-byte unit: one complex128 entry, or two complex64 entries
+__device__ __forceinline__ void unit_fma(const double2& h, const double2& p, double& ar, double& ai)
 {
-    double2* psis = reinterpret_cast<double2*>(smem_raw);   // [B]
-    __shared__ int s_strip;
+    ar = fma(h.x, p.x, ar);
+    ar = fma(-h.y, p.y, ar);
+    ai = fma(h.x, p.y, ai);
+    ai = fma(h.y, p.x, ai);
+}
+__device__ __forceinline__ void unit_fma(const float4& h, const float4& p, float& ar, float& ai)
+{
+    ar = fmaf(h.x, p.x, ar);
+    ar = fmaf(-h.y, p.y, ar);
+    ai = fmaf(h.x, p.y, ai);
+    ai = fmaf(h.y, p.x, ai);
+    ar = fmaf(h.z, p.z, ar);
+    ar = fmaf(-h.w, p.w, ar);
+    ai = fmaf(h.z, p.w, ai);
+    ai = fmaf(h.w, p.z, ai);
+}
+template <typename T> struct Unit16;
+template <> struct Unit16<double> { using type = double2; };
+template <> struct Unit16<float> { using type = float4; };
+
+template <typename T>
+__device__ __forceinline__ void cached_strips(const StripParams<T>& S, unsigned char* smem_raw)
+{
+    using CT = typename Cplx<T>::type;
+    using U16 = typename Unit16<T>::type;
+    constexpr int COLS = STRIP_PIECE / (int)sizeof(CT);     // columns per piece
+    constexpr int UPL = STRIP_PIECE / 16 / 32;              // 16-byte units per lane and row piece
+    __shared__ __align__(8) uint64_t full[STRIP_WS][2];
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
-    const int B = S.B;
-    for (;;) {
-        __syncthreads();
-        if (tid == 0) s_strip = atomicAdd(S.counter, 1);
-        __syncthreads();
-        const int it = s_strip;
-        if (it >= S.n_strips) break;
-        const int64_t row0 = (int64_t)it * STRIP_ROWS;
-        const int n = (int)(row0 / B);
-        const int a0 = (int)(row0 % B) + w * STRIP_RPW;
-        double accr[STRIP_RPW], acci[STRIP_RPW];
-#pragma unroll
-        for (int r = 0; r < STRIP_RPW; ++r) accr[r] = acci[r] = 0.0;
-        for (int m = 0; m < S.n_blk; ++m) {
-            const int32_t slot = S.cache_slot[n * S.n_blk + m];
-            if (slot < 0) continue;
-            __syncthreads();
-            for (int c = tid; c < B; c += PROC_THREADS) psis[c] = S.psi[(size_t)m * B + c];
-            __syncthreads();
-            const double2* rowp = S.cache + (size_t)slot * B * B + (size_t)a0 * B;
-            for (int c = lane; c < B; c += 32 * STRIP_U) {
-                double2 hv[STRIP_RPW][STRIP_U];
-#pragma unroll
-                for (int r = 0; r < STRIP_RPW; ++r)
-#pragma unroll
-                    for (int u = 0; u < STRIP_U; ++u)
-                        if (c + 32 * u < B) hv[r][u] = ldg_stream_d2(rowp + (size_t)r * B + c + 32 * u);
-#pragma unroll
-                for (int u = 0; u < STRIP_U; ++u) {
-                    if (c + 32 * u < B) {
-                        const double2 p = psis[c + 32 * u];
-#pragma unroll
-                        for (int r = 0; r < STRIP_RPW; ++r) {
-                            accr[r] = fma(hv[r][u].x, p.x, accr[r]);
-                            accr[r] = fma(-hv[r][u].y, p.y, accr[r]);
-                            acci[r] = fma(hv[r][u].x, p.y, acci[r]);
-                            acci[r] = fma(hv[r][u].y, p.x, acci[r]);
-                        }
-                    }
-                }
-            }
+    if (w < STRIP_WS) {
+        const int B = S.B, chunks = B / COLS;
+        unsigned char* ring = smem_raw + (size_t)w * 2 * STRIP_STAGE;
+        if (lane == 0) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(sm_u32(&full[w][0])), "r"(1) : "memory");
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(sm_u32(&full[w][1])), "r"(1) : "memory");
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         }
+        __syncwarp();
+        uint32_t g = 0;                       // tiles this warp has consumed so far (stage = g & 1, parity = (g >> 1) & 1)
+        for (;;) {
+            int it = 0;
+            if (lane == 0) it = atomicAdd(S.counter, 1);
+            it = __shfl_sync(0xffffffffu, it, 0);
+            if (it >= S.n_strips) break;
+            const int64_t row0 = (int64_t)it * STRIP_ROWS;
+            const int n = (int)(row0 / B), a0 = (int)(row0 % B);
+            const int32_t* slots = S.cache_slot + (size_t)n * S.n_blk;
+            // tile sequence of the strip: cached blocks in ascending m (fixed summation order), column chunks inside
+            int m_next = 0, ch_next = 0;      // next tile to ISSUE
+            int32_t slot_next = -1;
+            auto advance_block = [&]() {      // move (m_next, slot_next) to the next cached block, or past the end
+                while (m_next < S.n_blk && (slot_next = slots[m_next]) < 0) ++m_next;
+            };
+            advance_block();
+            auto issue = [&](uint32_t gi) {   // issue the next tile of the sequence into stage gi & 1; false at the end
+                if (m_next >= S.n_blk) return false;
+                if (lane == 0) {
+                    unsigned char* dst = ring + (size_t)(gi & 1u) * STRIP_STAGE;
+                    uint64_t* bar = &full[w][gi & 1u];
+                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the stage was read by generic loads
+                    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(sm_u32(bar)), "r"(STRIP_STAGE) : "memory");
+                    bulk_load(dst, S.cache + (size_t)slot_next * B * B + strip_tile_offset(B, COLS, a0, ch_next * COLS), STRIP_TILE, bar);
+                    bulk_load(dst + STRIP_TILE, S.psi + (size_t)m_next * B + (size_t)ch_next * COLS, STRIP_PIECE, bar);
+                }
+                if (++ch_next == chunks) {
+                    ch_next = 0;
+                    ++m_next;
+                    advance_block();
+                }
+                return true;
+            };
+            T ar[STRIP_ROWS], ai[STRIP_ROWS];
 #pragma unroll
-        for (int r = 0; r < STRIP_RPW; ++r) {
+            for (int r = 0; r < STRIP_ROWS; ++r) ar[r] = ai[r] = T(0);
+            int in_flight = 0;
+            if (issue(g)) ++in_flight;
+            if (issue(g + 1)) ++in_flight;
+            while (in_flight > 0) {
+                const uint32_t st = g & 1u;
+                sm_mbar_wait(&full[w][st], (g >> 1) & 1u);
+                const U16* tile = reinterpret_cast<const U16*>(ring + (size_t)st * STRIP_STAGE);
+                const U16* psip = tile + STRIP_TILE / 16;
+                U16 pv[UPL];
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                accr[r] += __shfl_xor_sync(0xffffffffu, accr[r], o);
-                acci[r] += __shfl_xor_sync(0xffffffffu, acci[r], o);
+                for (int q = 0; q < UPL; ++q) pv[q] = psip[lane + 32 * q];
+#pragma unroll
+                for (int r = 0; r < STRIP_ROWS; ++r) {
+                    U16 hv[UPL];
+#pragma unroll
+                    for (int q = 0; q < UPL; ++q) hv[q] = tile[r * (STRIP_PIECE / 16) + lane + 32 * q];
+#pragma unroll
+                    for (int q = 0; q < UPL; ++q) unit_fma(hv[q], pv[q], ar[r], ai[r]);
+                }
+                __syncwarp();                 // every lane has read the stage: it may be refilled
+                --in_flight;
+                if (issue(g + 2)) ++in_flight;
+                ++g;
             }
-            if (lane == 0)
-                S.work[(size_t)S.slot_cache * S.D + row0 + w * STRIP_RPW + r] = double2{accr[r], acci[r]};
+#pragma unroll
+            for (int r = 0; r < STRIP_ROWS; ++r) {
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+                    ar[r] += __shfl_xor_sync(0xffffffffu, ar[r], o);
+                    ai[r] += __shfl_xor_sync(0xffffffffu, ai[r], o);
+                }
+                if (lane == r) S.work[(size_t)S.slot_cache * S.D + row0 + r] = CT{ar[r], ai[r]};
+            }
         }
     }
+    __syncthreads();                          // the idle warps wait here; the shared memory is free for the next role
 }
 
-template <int R>
-__global__ void __launch_bounds__(PROC_THREADS, 2)
-partial_overlap_kernel(const ProcParams<double> P, const StripParams<double> S, int first_wave)
+// SM-partitioned roles (Eq. 33): the CTAs of `stream_sms` SMs -- spread evenly over the SM ids -- stream cached strips,
+// the CTAs of the other SMs generate; whoever exhausts its own queue takes work from the other.  Both CTAs of an SM
+// have the same role, so a streaming warp never shares an SM with generator warps except in the tail.
+__device__ __forceinline__ bool sm_streams(int stream_sms, int n_sm)
 {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    if ((int)blockIdx.x < first_wave) {
-        proc_items<double, R>(P, smem_raw);
-        cached_strips(S, smem_raw);
+    uint32_t smid;
+    asm("mov.u32 %0, %%smid;" : "=r"(smid));
+    smid %= (uint32_t)n_sm;
+    return ((smid + 1) * (uint32_t)stream_sms) / (uint32_t)n_sm != (smid * (uint32_t)stream_sms) / (uint32_t)n_sm;
+}
+
+template <typename T, int R>
+__global__ void __launch_bounds__(PROC_THREADS, 2)
+partial_overlap_kernel(const ProcParams<T> P, const StripParams<T> S, int stream_sms, int n_sm)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    if (!sm_streams(stream_sms, n_sm)) {
+        proc_items<T, R>(P, smem_raw);
+        cached_strips<T>(S, smem_raw);
     } else {
-        cached_strips(S, smem_raw);
-        proc_items<double, R>(P, smem_raw);
+        cached_strips<T>(S, smem_raw);
+        proc_items<T, R>(P, smem_raw);
     }
 }
 
@@ -552,60 +663,64 @@ int launch_proc_single(mfh_handle h, const void* psi, void* phi, double lambda, 
 bool partial_overlap_supported(mfh_handle h)
 {
     const Plan& p = h->plan;
-    return h->kind != MFH_SRC_ANALYTIC && h->dtype == MFH_C128 && p.k == 1 && !p.pairs && p.n_cached > 0 && !p.items.empty() &&
-           h->D % STRIP_ROWS == 0 && p.B % STRIP_ROWS == 0;
+    const int cols = STRIP_PIECE / (int)complex_bytes(h->dtype);   // a row piece must not cross a block
+    return h->kind != MFH_SRC_ANALYTIC && p.k == 1 && !p.pairs && p.n_cached > 0 && !p.items.empty() && p.B % cols == 0;
 }
 
-template <int R> static int launch_partial_overlap_t(mfh_handle h, const void* psi, cudaStream_t st)
+template <typename T, int R> static int launch_partial_overlap_t(mfh_handle h, const void* psi, cudaStream_t st)
 {
+    using CT = typename Cplx<T>::type;
     const Plan& p = h->plan;
-    ProcParams<double> P;
-    P.G = make_gen_args<double>(h);
+    ProcParams<T> P;
+    P.G = make_gen_args<T>(h);
     P.B = p.B;
     P.n_blk = p.n_blk;
     P.n_items = (int32_t)p.items.size();
     P.slot_row0 = p.slot_row0;
     P.D = h->D;
     P.items = h->d_items;
-    P.psi = (const double2*)psi;
-    P.work = (double2*)h->d_work;
+    P.psi = (const CT*)psi;
+    P.work = (CT*)h->d_work;
     P.counter = h->d_counter;
     P.done = nullptr;
     P.fin = nullptr;
-    StripParams<double> S;
+    StripParams<T> S;
     S.B = p.B;
     S.n_blk = p.n_blk;
     S.slot_cache = p.slot_cache;
     S.n_strips = (int32_t)(h->D / STRIP_ROWS);
     S.D = h->D;
     S.cache_slot = h->d_cache_slot;
-    S.cache = (const double2*)h->d_cache;
-    S.psi = (const double2*)psi;
-    S.work = (double2*)h->d_work;
+    S.cache = (const CT*)h->d_cache;
+    S.psi = (const CT*)psi;
+    S.work = (CT*)h->d_work;
     S.counter = h->d_counter + 1;
-    auto smem_for = [](int B) {
-        return (size_t)(B + PROC_WARPS * 32 * R + PROC_WARPS * 32) * sizeof(double2);   // + the static generator table
-    };
-    const size_t smem = smem_for(p.B);
-    auto kern = partial_overlap_kernel<R>;
-    if (int rc = ensure_dyn_smem(h, kern, (int)smem_for(MFH_MAX_B))) return rc;
-    int per_sm = 1;
+    // dynamic shared memory: the generator's arrays or the streaming ring, whichever is larger, with two CTAs per SM
+    const size_t gen_smem = (size_t)(p.B + PROC_WARPS * 32 * R + PROC_WARPS * 32) * sizeof(CT);   // + the static generator table
+    auto kern = partial_overlap_kernel<T, R>;
+    if (int rc = ensure_dyn_smem(h, kern, 96 * 1024)) return rc;
+    const size_t smem = std::max(gen_smem, (size_t)STRIP_SMEM);
+    int per_sm = 0;
     MFH_CUDA_CHECK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, PROC_THREADS, smem));
-    if (per_sm < 1) per_sm = 1;
+    if (per_sm < 1) {
+        set_error("partial plan: the fused kernel does not fit an SM (B = %d)", p.B);
+        return MFH_ERR_UNSUPPORTED;
+    }
     const int grid = h->sm_count * per_sm;
-    const int first_wave = per_sm > 1 ? h->sm_count * (per_sm / 2) : grid / 2;   // CTAs that prefer generated items
     MFH_CUDA_CHECK(cudaMemsetAsync(h->d_counter, 0, 2 * sizeof(int32_t), st));
-    kern<<<grid, PROC_THREADS, smem, st>>>(P, S, first_wave);
+    const int stream_sms = p.stream_sms > 0 ? std::min(p.stream_sms, h->sm_count - 1) : h->sm_count / 3;
+    kern<<<grid, PROC_THREADS, smem, st>>>(P, S, stream_sms, h->sm_count);
     MFH_CUDA_CHECK(cudaGetLastError());
     return MFH_OK;
 }
 
 int launch_partial_overlap(mfh_handle h, const void* psi, cudaStream_t st)
 {
+    const bool f64 = (h->dtype == MFH_C128);
     switch (h->plan.R) {
-    case 4: return launch_partial_overlap_t<4>(h, psi, st);
-    case 2: return launch_partial_overlap_t<2>(h, psi, st);
-    case 1: return launch_partial_overlap_t<1>(h, psi, st);
+    case 4: return f64 ? launch_partial_overlap_t<double, 4>(h, psi, st) : launch_partial_overlap_t<float, 4>(h, psi, st);
+    case 2: return f64 ? launch_partial_overlap_t<double, 2>(h, psi, st) : launch_partial_overlap_t<float, 2>(h, psi, st);
+    case 1: return f64 ? launch_partial_overlap_t<double, 1>(h, psi, st) : launch_partial_overlap_t<float, 1>(h, psi, st);
     }
     set_error("unsupported rows per lane %d", h->plan.R);
     return MFH_ERR_INVALID_ARG;

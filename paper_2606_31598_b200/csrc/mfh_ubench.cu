@@ -18,17 +18,19 @@ constexpr int UB_ITER = 1024, UB_CH = 4, UB_THREADS = 256, UB_CTAS_PER_SM = 4;
 
 // One unit per chain and iteration: NW wide multiplies (+ NW xors), NL further ALU ops, ND dfma,
 // NM mufu, NF ffma.
-template <int NW, int NL, int ND, int NM, int NF>
+// REG3: the DFMA chain takes three register operands (x = fma(x, y, z)) instead of two immediates.
+template <int NW, int NL, int ND, int NM, int NF, bool REG3 = false>
 __global__ void __launch_bounds__(UB_THREADS) ubench_kernel(uint32_t* out, uint32_t seed)
 {
     uint32_t a[UB_CH], c[UB_CH];
-    double d[UB_CH];
+    double d[UB_CH], d2[UB_CH];
     float f[UB_CH];
 #pragma unroll
     for (int q = 0; q < UB_CH; ++q) {
         a[q] = threadIdx.x * (2 * q + 3) + seed;
         c[q] = a[q] ^ (0x9e3779b9u * (q + 1));
         d[q] = 1.0 + 1e-9 * a[q];
+        d2[q] = 0.5 + 1e-9 * c[q];
         f[q] = 1.0f + 1e-6f * q;
     }
     for (int it = 0; it < UB_ITER; ++it) {
@@ -47,7 +49,7 @@ __global__ void __launch_bounds__(UB_THREADS) ubench_kernel(uint32_t* out, uint3
             if (ND > 0) {
                 double x = d[q] + __hiloint2double(0x3e000000, (int)a[q]);
 #pragma unroll
-                for (int r = 0; r < ND - 1; ++r) x = fma(x, 0.99999999, 1e-9);
+                for (int r = 0; r < ND - 1; ++r) x = REG3 ? fma(x, d2[q], d[q]) : fma(x, 0.99999999, 1e-9);
                 d[q] = x;
             }
             if (NM + NF > 0) {
@@ -62,11 +64,11 @@ __global__ void __launch_bounds__(UB_THREADS) ubench_kernel(uint32_t* out, uint3
     }
     uint32_t r = 0;
 #pragma unroll
-    for (int q = 0; q < UB_CH; ++q) r ^= a[q] ^ c[q] ^ (uint32_t)d[q] ^ __float_as_uint(f[q]);
+    for (int q = 0; q < UB_CH; ++q) r ^= a[q] ^ c[q] ^ (uint32_t)d[q] ^ (uint32_t)d2[q] ^ __float_as_uint(f[q]);
     out[blockIdx.x * blockDim.x + threadIdx.x] = r;
 }
 
-template <int NW, int NL, int ND, int NM, int NF>
+template <int NW, int NL, int ND, int NM, int NF, bool REG3 = false>
 static int run_mix(int sm_count, cudaStream_t st, double* units_per_s)
 {
     const int grid = sm_count * UB_CTAS_PER_SM;
@@ -81,7 +83,7 @@ static int run_mix(int sm_count, cudaStream_t st, double* units_per_s)
     float best = 1e30f;
     for (int rep = 0; rep < 4; ++rep) {   // first repetition warms up
         cudaEventRecord(e0, st);
-        ubench_kernel<NW, NL, ND, NM, NF><<<grid, UB_THREADS, 0, st>>>(out, (uint32_t)rep);
+        ubench_kernel<NW, NL, ND, NM, NF, REG3><<<grid, UB_THREADS, 0, st>>>(out, (uint32_t)rep);
         cudaEventRecord(e1, st);
         cudaError_t e = cudaEventSynchronize(e1);
         float ms = 0.f;
@@ -304,7 +306,7 @@ extern "C" MFH_API int mfh_debug_read_bandwidth(const void* buf_dev, size_t byte
 extern "C" MFH_API int mfh_debug_pipe_rates(int32_t mix, double* units_per_s, void* stream)
 {
     if (!units_per_s) { set_error("mfh_debug_pipe_rates: NULL pointer"); return MFH_ERR_INVALID_ARG; }
-    if (mix < MFH_MIX_C128_PAIR || mix > MFH_COMP_MAC_C64) {
+    if (mix < MFH_MIX_C128_PAIR || mix > MFH_PIPE_WIDE16_LOP32) {
         set_error("mfh_debug_pipe_rates: unknown mix %d", mix);
         return MFH_ERR_INVALID_ARG;
     }
@@ -323,6 +325,14 @@ extern "C" MFH_API int mfh_debug_pipe_rates(int32_t mix, double* units_per_s, vo
     case MFH_COMP_MAC_C128: return run_comp<double, 2>(sms, st, units_per_s);
     case MFH_COMP_PHILOX_BM_C64: return run_comp<float, 1>(sms, st, units_per_s);
     case MFH_COMP_MAC_C64: return run_comp<float, 2>(sms, st, units_per_s);
+    // pipe model: which instruction classes overlap on sm_100
+    case MFH_PIPE_WIDE16: return run_mix<16, 0, 0, 0, 0>(sms, st, units_per_s);
+    case MFH_PIPE_LOP32: return run_mix<0, 32, 0, 0, 0>(sms, st, units_per_s);
+    case MFH_PIPE_DFMA32: return run_mix<0, 0, 33, 0, 0>(sms, st, units_per_s);
+    case MFH_PIPE_DFMA32_REG3: return run_mix<0, 0, 33, 0, 0, true>(sms, st, units_per_s);
+    case MFH_PIPE_WIDE16_DFMA32: return run_mix<16, 0, 33, 0, 0>(sms, st, units_per_s);
+    case MFH_PIPE_LOP32_DFMA32: return run_mix<0, 32, 33, 0, 0>(sms, st, units_per_s);
+    case MFH_PIPE_WIDE16_LOP32: return run_mix<16, 32, 0, 0, 0>(sms, st, units_per_s);
     }
     set_error("mfh_debug_pipe_rates: unknown mix %d", mix);
     return MFH_ERR_INVALID_ARG;
