@@ -87,9 +87,12 @@ static size_t lanczos_scratch_bytes(int64_t D, int dtype)
     return (size_t)3 * D * complex_bytes(dtype) + (2 * 4096 + 8 + (size_t)lz_partial_doubles()) * sizeof(double);
 }
 
-// Largest D whose procedural k = 1 plans fold the reduce into the fused kernel: below it an apply is launch-bound
-// (C1: 58 us, three launches); above it the separate reduce kernel costs < 1 % and keeps its wider parallelism.
-static const int64_t kFusedTailMaxD = 32768;
+// Largest D whose procedural k = 1 plans fold the reduce into the fused kernel (one launch per apply).  The reduce of
+// a block row is done by the ONE CTA that delivers its last contribution, so it pays off only while a block row's
+// partial sums are small: measured at C1 (D = 4096, 72 partial slots, 590 KB per block row) the single launch is
+// 2-3 us SLOWER than kernel + reduce kernel (59.0 against 55.4 us per apply replayed from a graph: the apply is bound
+// by the one-item-per-CTA generator wave, not by launches), so the tail is kept for D <= 2048 only.
+static const int64_t kFusedTailMaxD = 2048;
 
 // Allocate and upload everything plan `p` needs, then fill the cache.
 static int commit_plan(mfh_handle h, const Plan& p, cudaStream_t st)

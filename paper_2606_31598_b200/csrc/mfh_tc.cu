@@ -419,21 +419,26 @@ __global__ void __launch_bounds__(CT_THREADS, 2) cached_multi_tc_kernel(const Ct
                                  (size_t)((i_base - (uint32_t)n * P.B) / TC_TP) * (P.B / (CT_KF / 2)) * CT_RAW;
 
     if (w == TC_GEN_WARPS + 1) {
-        // ---- TMA producer: one lane ----
-        if (lane == 0) {
-            for (int t = 0; t < n_tiles; ++t) {
-                const int s = t % CT_STAGES, u = t / CT_STAGES;
-                if (u > 0) mbar_wait(&raw_empty[s], (u - 1) & 1);
-                const uint32_t psi_bytes = (uint32_t)((CT_KF / 2) * P.k * sizeof(float2));
+        // ---- TMA producer: lane 0 copies the tiles, lane 1 the psi rows.  Bulk copies issued by ONE thread are serviced
+        // one after the other (~0.27 us each on B200); copies of different lanes overlap, so the two
+        // copies of a stage come from two lanes. ----
+        const uint32_t psi_bytes = (uint32_t)((CT_KF / 2) * P.k * sizeof(float2));
+        for (int t = 0; t < n_tiles; ++t) {
+            const int s = t % CT_STAGES, u = t / CT_STAGES;
+            if (u > 0) mbar_wait(&raw_empty[s], (u - 1) & 1);
+            if (lane == 0)
                 asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&raw_full[s])),
                              "r"(CT_RAW + psi_bytes)
                              : "memory");
+            __syncwarp();
+            if (lane == 1) {
                 // the 16 psi rows of the tile are contiguous in [D][k]: one 1-D bulk copy
                 asm volatile(
                     "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
                         smem_u32(psis + s * CT_PSI)),
                     "l"(P.psi + ((size_t)m * P.B + (size_t)t * (CT_KF / 2)) * P.k), "r"(psi_bytes), "r"(smem_u32(&raw_full[s]))
                     : "memory");
+            } else if (lane == 0) {
                 // tile t of the strip: 16 KB contiguous in the tiled cache layout (mfh_internal.cuh tiled_cache_offset)
                 asm volatile(
                     "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(

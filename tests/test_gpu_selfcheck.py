@@ -43,7 +43,7 @@ def test_fused_tail_single_launch_is_deterministic_and_self_cleaning():
     bit-identical (the device counters clean themselves) and match the oracle."""
     import oracle
     import torch
-    D, B = 4096, 512
+    D, B = 2048, 256
     psi_np = make_psi(D, 99)
     psi = torch.from_numpy(psi_np).cuda()
     for dtype, tol in (("c128", 1e-11), ("c64", 1e-4)):
