@@ -439,7 +439,7 @@ def roofline_for(res: dict, hbm_gbs: float, peak_src: str) -> dict:
         # kernel's multiply-accumulates read the entry, the psi value and the accumulator from registers
         reg3 = res["pipe_rate"]("pipe_dfma32_reg3") * 33 * 2 / 1e12
         return {"kernel": "cached_multi_kernel_c128", "bound": "alu", "achieved": tf, "peak": peak, "unit": "TFLOP/s",
-                "frac": tf / peak, "traffic": None, "traffic_source": None,
+                "frac": tf / peak, **ncu_traffic("cached_multi_kernel_c128", D),
                 "three_register_dfma_ceiling": reg3, "frac_of_three_register_dfma_ceiling": tf / reg3,
                 "peak_source": "nominal FP64: 148 SMs x 64 DFMA lanes/clk x 2 flop x 1.965 GHz (B200_PROFILING.md unit counts; "
                                "the SM clock under FP64 load is power-capped below that)",
@@ -465,7 +465,7 @@ def roofline_for(res: dict, hbm_gbs: float, peak_src: str) -> dict:
     cnt = SASS_COUNTS[key]
     issue_peak = ISSUE_LANES_PER_S / cnt["instr_per_entry"]
     kname = "proc_single_kernel" if k == 1 else ("proc_multi_tc_kernel" if cfg["dtype"] == "c64" else "proc_multi_kernel")
-    out = {"kernel": kname, "bound": "alu", "achieved": rate / 1e9, "unit": "Gentries/s", "traffic": None, "traffic_source": None,
+    out = {"kernel": kname, "bound": "alu", "achieved": rate / 1e9, "unit": "Gentries/s", **ncu_traffic(kname, D),
            "issue_slot_peak": issue_peak / 1e9, "frac_of_issue_slots": rate / issue_peak,
            "instr_per_entry": cnt["instr_per_entry"], "sass_counts_source": cnt["source"],
            "kernel_ms": kern["procedural"], "share_of_step": kern["procedural"] / max(kern["total"], 1e-9)}
@@ -506,10 +506,10 @@ def roofline_for(res: dict, hbm_gbs: float, peak_src: str) -> dict:
 # lanes (B200_PROFILING.md unit counts, 1.965 GHz).
 ISSUE_LANES_PER_S = 148 * 4 * 32 * 1.965e9
 FP64_LANES_PER_S = 148 * 64 * 1.965e9
-SASS_COUNTS = {("c128", "k1"): {"instr_per_entry": 45.25, "fp64_per_entry": 16.0, "source": "profiles/r02_proc_single_sass.md"},
+SASS_COUNTS = {("c128", "k1"): {"instr_per_entry": 43.875, "fp64_per_entry": 16.0, "source": "profiles/r02_proc_single_sass.md"},
                ("c128", "kN"): {"instr_per_entry": 150.0, "fp64_per_entry": 0, "source": "DESIGN.md 6.3"},
                ("c64", "k1"): {"instr_per_entry": 40.0, "fp64_per_entry": 0, "source": "DESIGN.md 6.2"},
-               ("c64", "kN"): {"instr_per_entry": 60.0, "fp64_per_entry": 0, "source": "DESIGN.md 6.3"}}
+               ("c64", "kN"): {"instr_per_entry": 64.0, "fp64_per_entry": 0, "source": "profiles/r02_proc_multi_tc_c3_ncu_full.md (2.14e9 warp instructions / 1.07e9 entries x 32 lanes)"}}
 MIX_OF = {("c128", "k1"): ("c128_pair", 2), ("c64", "kN"): ("c64_entry", 1)}
 COMPONENTS_OF = {("c128", "k1"): {"kernels": ("comp_philox", "comp_philox_bm_c128", "comp_mac_c128"), "entries_per_pair": 2},
                  ("c64", "k1"): {"kernels": ("comp_philox", "comp_philox_bm_c64", "comp_mac_c64"), "entries_per_pair": 2}}
@@ -517,10 +517,13 @@ COMPONENTS_OF = {("c128", "k1"): {"kernels": ("comp_philox", "comp_philox_bm_c12
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full captures, keyed by
 # (kernel, D): (bytes per launch, the capture it was read from).  A kernel without a capture reports "traffic": null.
-NCU_TRAFFIC = {("cached_kernel", 65536): (68.724718e9 + 4.461824e6, "profiles/r01_cached_c2_ncu_full.md"),
-               ("partial_overlap_kernel", 131072): (146.039268e9 + 247.162624e6, "profiles/r01_partial_overlap_c5_ncu_full.md"),
+NCU_TRAFFIC = {("cached_kernel", 65536): (68.725132e9 + 5.106432e6, "profiles/r02_cached_c2_ncu_full.md"),
+               ("partial_overlap_kernel", 131072): (146.236774e9 + 252.962816e6, "profiles/r02_partial_overlap_c5_ncu_full.md"),
                ("cached_pairs_kernel", 65536): (35.438780e9 + 249.902592e6, "profiles/r01_pairs_c2_ncu_full.md"),
-               ("cached_multi_tc_kernel", 32768): (8.596603e9 + 134.462720e6, "profiles/r01_cached_multi_tc_c3_ncu_full.md")}
+               ("cached_multi_tc_kernel", 32768): (8.595413e9 + 135.389184e6, "profiles/r02_cached_multi_tc_c3_ncu_full.md"),
+               ("cached_multi_kernel_c128", 32768): (17.203616e9 + 268.850432e6, "profiles/r02_cached_multi_c128_c3_ncu_full.md"),
+               ("proc_single_kernel", 262144): (22.890752e6 + 631.663104e6, "profiles/r02_proc_single_c4_ncu_full.md"),
+               ("proc_multi_tc_kernel", 32768): (4.513792e6 + 81.728768e6, "profiles/r02_proc_multi_tc_c3_ncu_full.md")}
 
 
 def ncu_traffic(kernel: str, D: int) -> dict:

@@ -141,6 +141,15 @@ MFH_API int mfh_plan_node_analytic(int64_t D, int32_t dtype, int32_t k, int32_t 
  * mfh_surrogate_fit: mu, sigma from the data (sigma = 1 for constant features), seeded initial weights, `epochs`
  * full-batch Adam steps of size lr; *final_loss = Eq. 26 at the end.  mfh_surrogate_loss_grad: Eq. 26 and its
  * gradient with respect to [W1 | b1 | W2 | b2] (test export; grad_out may be NULL).  Errors: INVALID_ARG. */
+/* The feature vector x(p) of a candidate plan, MFH_SURROGATE_FEATURES doubles written to x_out:
+ *   (log D, log R, log N_blk, log b, log N_task, p_row, W(p), 1_full, 1_partial, 1_procedural, 1_pairs [this build's
+ *    fourth storage mode], log F_mv, M_op/M_free, M_work/M_free, M_tot/M_free, 1_complex64, log GPU memory, log SMs)
+ * from the plan's own numbers (the fields of a candidate record of mfh_plan / mfh_plan_analytic).  mode is the
+ * candidate's committed mode (not AUTO).  Errors: INVALID_ARG. */
+#define MFH_SURROGATE_FEATURES 18
+MFH_API int mfh_surrogate_features(int64_t D, int32_t dtype, int32_t k, int32_t mode, int32_t B, double flops_per_apply,
+                                   double cache_bytes, double work_bytes, double free_bytes, int64_t n_task, int32_t p_row,
+                                   int64_t waves, double gpu_bytes, int32_t sms, double* x_out);
 MFH_API int64_t mfh_surrogate_theta_size(int32_t n_features, int32_t hidden);
 MFH_API int mfh_surrogate_fit(const double* X, const double* t_seconds, int64_t n, int32_t n_features, int32_t hidden,
                               int32_t epochs, double lr, uint64_t seed, double* theta_out, double* final_loss);
@@ -161,6 +170,15 @@ MFH_API int mfh_surrogate_loss_grad(const double* theta, int32_t n_features, int
 MFH_API int mfh_plan(mfh_handle h, int32_t mode, int32_t k, int64_t n_applies_hint,
                      int64_t hbm_budget_bytes, int32_t measure, void* stream, char* json_out,
                      size_t json_cap);
+
+/* Algorithm 3, hybrid mode ("ranks the memory-feasible candidates by t_NN(p) W(p) ... a local measurement
+ * remains the final decision rule"): as mfh_plan(MFH_MODE_AUTO, measure = 1), but the feasible candidates are ordered by
+ * the surrogate's prediction t_NN = exp(f_theta(x(p))) (theta from mfh_surrogate_fit on MFH_SURROGATE_FEATURES
+ * features) and only the k_nn best are committed and timed; the best measured one (Eq. 23) stays committed.  Each
+ * candidate's memory is released before the next is tried.  The JSON record carries "planner":"hybrid" and every
+ * candidate's "surrogate_apply_s".  Errors as mfh_plan; INVALID_ARG for theta == NULL, hidden < 1, k_nn < 1. */
+MFH_API int mfh_plan_hybrid(mfh_handle h, const double* theta, int32_t hidden, int32_t k, int64_t n_applies_hint,
+                            int64_t hbm_budget_bytes, int32_t k_nn, void* stream, char* json_out, size_t json_cap);
 
 /* phi = H psi for k vectors (Eq. 7; Eq. 12 for k > 1), asynchronous on `stream`, no host
  * synchronisation, no allocation.  k must equal the k given to mfh_plan.

@@ -34,7 +34,7 @@ SYMBOLS = ["mfh_create", "mfh_plan_analytic", "mfh_plan_node_analytic", "mfh_pla
            "mfh_chebyshev", "mfh_chebyshev_imag", "mfh_chebyshev_scan", "mfh_chebyshev_steps", "mfh_lanczos_bounds", "mfh_destroy", "mfh_last_error", "mfh_get_plan", "mfh_debug_philox",
            "mfh_materialize_block", "mfh_debug_h0", "mfh_debug_bessel_j", "mfh_debug_poison", "mfh_debug_selfcheck", "mfh_debug_corrupt_guard", "mfh_debug_pipe_rates", "mfh_sb_create", "mfh_sb_plan", "mfh_sb_apply",
            "mfh_sb_destroy", "mfh_set_partition", "mfh_get_partition_rows", "mfh_set_exchange", "mfh_debug_read_bandwidth", "mfh_set_source_params", "mfh_set_block", "mfh_surrogate_theta_size", "mfh_surrogate_fit",
-           "mfh_surrogate_predict", "mfh_surrogate_loss_grad"]
+           "mfh_surrogate_predict", "mfh_surrogate_loss_grad", "mfh_surrogate_features", "mfh_plan_hybrid"]
 
 _lib = None
 

@@ -450,9 +450,11 @@ MFH_API int mfh_plan_node_analytic(int64_t D, int32_t dtype, int32_t k, int32_t 
     return rc;
 }
 
-MFH_API int mfh_plan(mfh_handle h, int32_t mode, int32_t k, int64_t n_applies_hint,
-                     int64_t hbm_budget_bytes, int32_t measure, void* stream, char* json_out,
-                     size_t json_cap)
+// Shared body of mfh_plan and mfh_plan_hybrid.  theta != nullptr: Algorithm 3, hybrid mode -- the memory-feasible
+// candidates are ranked by the surrogate's t_NN(p) (Eq. 25), only the k_nn best are committed and timed (Algorithm 2),
+// the best measured one is kept (Eq. 23).
+static int plan_core(mfh_handle h, int32_t mode, int32_t k, int64_t n_applies_hint, int64_t hbm_budget_bytes, int32_t measure,
+                     void* stream, char* json_out, size_t json_cap, const double* theta, int32_t hidden, int32_t k_nn)
 {
     if (!h) { set_error("mfh_plan: NULL handle"); return MFH_ERR_INVALID_ARG; }
     if (k < 1 || k > MFH_MAX_K || mode < MFH_MODE_AUTO || mode > MFH_MODE_PAIRS || hbm_budget_bytes < 0) {
@@ -519,8 +521,22 @@ MFH_API int mfh_plan(mfh_handle h, int32_t mode, int32_t k, int64_t n_applies_hi
         build_tables(p, h->D, h->dtype, h->sm_count);
         return p;
     };
+    if (theta) {   // Algorithm 3: rank the feasible candidates by the surrogate's predicted apply time
+        std::vector<double> x(MFH_SURROGATE_FEATURES);
+        for (auto& c : cands) {
+            if (!c.feasible) continue;
+            rc = mfh_surrogate_features(h->D, h->dtype, k, c.mode, c.B, c.flops, c.cache_bytes, c.work_bytes, budget, 1, 1, 1,
+                                        (double)total_b, h->sm_count, x.data());
+            if (!rc) rc = mfh_surrogate_predict(theta, MFH_SURROGATE_FEATURES, hidden, x.data(), 1, &c.t_nn);
+            if (rc) return rc;
+        }
+        std::stable_sort(cands.begin(), cands.end(), [](const Candidate& a, const Candidate& b) {
+            if (a.feasible != b.feasible) return a.feasible;
+            return a.feasible && a.t_nn < b.t_nn;
+        });
+    }
     if (measure) {   // Algorithm 2: K_bench best feasible candidates, argmin of the measured time
-        const int K_bench = 8;
+        const int K_bench = theta ? std::max(k_nn, 1) : 8;
         int tried = 0;
         for (auto& c : cands) {
             if (!c.feasible || tried >= K_bench) continue;
@@ -555,9 +571,23 @@ MFH_API int mfh_plan(mfh_handle h, int32_t mode, int32_t k, int64_t n_applies_hi
     }
     rc = commit_plan(h, make_plan(cands[0]), st);
     if (rc) return rc;
-    h->plan.json = plan_json(h->D, h->dtype, k, n_applies_hint, budget, measure, cands);
+    h->plan.json = plan_json(h->D, h->dtype, k, n_applies_hint, budget, theta ? 2 : measure, cands);
     copy_json(h->plan.json, json_out, json_cap);
     return MFH_OK;
+}
+
+MFH_API int mfh_plan(mfh_handle h, int32_t mode, int32_t k, int64_t n_applies_hint,
+                     int64_t hbm_budget_bytes, int32_t measure, void* stream, char* json_out,
+                     size_t json_cap)
+{
+    return plan_core(h, mode, k, n_applies_hint, hbm_budget_bytes, measure, stream, json_out, json_cap, nullptr, 0, 0);
+}
+
+MFH_API int mfh_plan_hybrid(mfh_handle h, const double* theta, int32_t hidden, int32_t k, int64_t n_applies_hint,
+                            int64_t hbm_budget_bytes, int32_t k_nn, void* stream, char* json_out, size_t json_cap)
+{
+    if (!theta || hidden < 1 || k_nn < 1) { set_error("mfh_plan_hybrid: need theta, hidden >= 1, k_nn >= 1"); return MFH_ERR_INVALID_ARG; }
+    return plan_core(h, MFH_MODE_AUTO, k, n_applies_hint, hbm_budget_bytes, 1, stream, json_out, json_cap, theta, hidden, k_nn);
 }
 
 MFH_API int mfh_get_plan(mfh_handle h, char* json_out, size_t json_cap)

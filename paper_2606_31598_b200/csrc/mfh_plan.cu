@@ -376,8 +376,8 @@ static void candidate_json(std::string& s, const Candidate& c)
     appendf(s, "\"cache_bytes\":%.0f,\"work_bytes\":%.0f,\"total_bytes\":%.0f,\"feasible\":%s,",
             c.cache_bytes, c.work_bytes, c.cache_bytes + c.work_bytes, c.feasible ? "true" : "false");
     appendf(s, "\"model_apply_s\":%.6g,\"model_cached_s\":%.6g,\"model_proc_s\":%.6g,\"model_fill_s\":%.6g,"
-               "\"model_job_s\":%.6g,\"flops_per_apply\":%.6g,\"measured_apply_s\":%.6g}",
-            c.t_apply, c.t_cached, c.t_proc, c.t_fill, c.t_job, c.flops, c.t_measured);
+               "\"model_job_s\":%.6g,\"flops_per_apply\":%.6g,\"measured_apply_s\":%.6g,\"surrogate_apply_s\":%.6g}",
+            c.t_apply, c.t_cached, c.t_proc, c.t_fill, c.t_job, c.flops, c.t_measured, c.t_nn);
 }
 
 // Largest c in [0, c_max] with ok(c) (ok is monotone: more cached blocks need more memory); bisection,
@@ -461,7 +461,7 @@ std::string plan_json(int64_t D, int dtype, int k, int64_t n_applies, double bud
     appendf(s, "{\"D\":%lld,\"dtype\":\"%s\",\"k\":%d,\"n_applies_hint\":%lld,\"budget_bytes\":%.0f,"
                "\"alpha\":%.2f,\"planner\":\"%s\",\"dense_bytes\":%.0f,\"chosen\":",
             (long long)D, dtype == MFH_C128 ? "c128" : "c64", k, (long long)n_applies, budget, kAlpha,
-            measured ? "measured" : "analytic", (double)D * D * complex_bytes(dtype));
+            measured == 2 ? "hybrid" : (measured ? "measured" : "analytic"), (double)D * D * complex_bytes(dtype));
     if (!cands.empty()) candidate_json(s, cands[0]);
     else s += "null";
     s += ",\"candidates\":[";

@@ -26,6 +26,7 @@ struct Candidate {
     double t_cached = 0, t_proc = 0, t_reduce = 0;       // seconds per apply, by part
     double t_apply = 0, t_fill = 0, t_job = 0, flops = 0;
     double t_measured = -1.0;                            // Algorithm 2 (Eq. 21), -1 = not measured
+    double t_nn = -1.0;                                  // Algorithm 3 (Eq. 25): the surrogate's prediction, -1 = none
     bool feasible = false;                               // Eq. 18
 };
 

@@ -75,6 +75,39 @@ using namespace mfh;
 
 extern "C" {
 
+MFH_API int mfh_surrogate_features(int64_t D, int32_t dtype, int32_t k, int32_t mode, int32_t B, double flops_per_apply,
+                                   double cache_bytes, double work_bytes, double free_bytes, int64_t n_task, int32_t p_row,
+                                   int64_t waves, double gpu_bytes, int32_t sms, double* x_out)
+{
+    if (!x_out || D < 1 || B < 1 || k < 1 || n_task < 1 || p_row < 1 || waves < 1 || !(flops_per_apply > 0.0) ||
+        !(free_bytes > 0.0) || !(gpu_bytes > 0.0) || sms < 1 || mode < MFH_MODE_PROCEDURAL || mode > MFH_MODE_PAIRS ||
+        (dtype != MFH_C128 && dtype != MFH_C64)) {
+        set_error("mfh_surrogate_features: invalid argument");
+        return MFH_ERR_INVALID_ARG;
+    }
+    // x(p) of P:370, in the order of paper_2606_31598_b200/surrogate.py FEATURES
+    double* x = x_out;
+    x[0] = std::log((double)D);
+    x[1] = std::log((double)k);
+    x[2] = std::log((double)(D / B));
+    x[3] = std::log((double)B);
+    x[4] = std::log((double)n_task);
+    x[5] = (double)p_row;
+    x[6] = (double)waves;
+    x[7] = mode == MFH_MODE_FULL;
+    x[8] = mode == MFH_MODE_PARTIAL;
+    x[9] = mode == MFH_MODE_PROCEDURAL;
+    x[10] = mode == MFH_MODE_PAIRS;
+    x[11] = std::log(flops_per_apply);
+    x[12] = cache_bytes / free_bytes;
+    x[13] = work_bytes / free_bytes;
+    x[14] = (cache_bytes + work_bytes) / free_bytes;
+    x[15] = dtype == MFH_C64;
+    x[16] = std::log(gpu_bytes);
+    x[17] = std::log((double)sms);
+    return MFH_OK;
+}
+
 MFH_API int64_t mfh_surrogate_theta_size(int32_t n_features, int32_t hidden)
 {
     if (n_features < 1 || hidden < 1) return 0;

@@ -24,13 +24,21 @@ F = len(FEATURES)
 
 def features(D: int, dtype: str, k: int, cand: dict, free_bytes: float, n_task: int = 1, p_row: int = 1, waves: int = 1,
              gpu_bytes: float = 180e9, sms: int = 148) -> np.ndarray:
-    """Feature row of one candidate record (the dicts in plan["candidates"])."""
-    mode = cand["mode"]
-    return np.array([math.log(D), math.log(k), math.log(cand["n_blk"]), math.log(cand["B"]), math.log(n_task),
-                     float(p_row), float(waves), float(mode == "full"), float(mode == "partial"),
-                     float(mode == "procedural"), float(mode == "pairs"), math.log(cand["flops_per_apply"]),
-                     cand["cache_bytes"] / free_bytes, cand["work_bytes"] / free_bytes, cand["total_bytes"] / free_bytes,
-                     float(dtype == "c64"), math.log(gpu_bytes), math.log(sms)], dtype=np.float64)
+    """Feature row x(p) of one candidate record (the dicts in plan["candidates"]): marshalling around
+    mfh_surrogate_features, which holds the feature map."""
+    from .binding import DTYPES, MODES
+    out = np.empty(F, dtype=np.float64)
+    L = lib()
+    L.mfh_surrogate_features.argtypes = [ctypes.c_int64, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32,
+                                         ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_int64,
+                                         ctypes.c_int32, ctypes.c_int64, ctypes.c_double, ctypes.c_int32,
+                                         ctypes.POINTER(ctypes.c_double)]
+    rc = L.mfh_surrogate_features(D, DTYPES[dtype], k, MODES[cand["mode"]], int(cand["B"]), float(cand["flops_per_apply"]),
+                                  float(cand["cache_bytes"]), float(cand["work_bytes"]), float(free_bytes), int(n_task), int(p_row),
+                                  int(waves), float(gpu_bytes), int(sms), _p(out))
+    if rc != MFH_OK:
+        raise MfhError(rc, lib().mfh_last_error().decode())
+    return out
 
 
 def _p(a):
@@ -123,28 +131,30 @@ def load_log(path: str):
 
 
 def hybrid_plan(theta, D: int, dtype: str, k: int = 1, seed: int = 0, kind: str = "gue", seed_h0: int = 0,
-                n_applies_hint: int = 1, hbm_budget_bytes: int = 0, k_nn: int = 3, hidden: int = 16):
-    """Algorithm 3, hybrid mode: enumerate the memory-feasible candidates with the analytic planner, rank
-    them by t_NN(p), commit and time only the top `k_nn` on the device and keep the best measured one (Eq. 23).
-    Returns (handle with the chosen plan committed, report).  Needs CUDA."""
-    import torch
-    from .binding import Hamiltonian, plan_analytic
-    free = torch.cuda.mem_get_info()[0]
-    budget = hbm_budget_bytes if hbm_budget_bytes > 0 else 0.9 * free
-    rec = plan_analytic(D, dtype, k=k, n_applies_hint=n_applies_hint, hbm_free_bytes=int(budget / 0.9))
-    ranked = rank(theta, D, dtype, k, rec, rec["budget_bytes"], hidden)[:k_nn]
+                n_applies_hint: int = 1, hbm_budget_bytes: int = 0, k_nn: int = 3, hidden: int = 16, B: int = 0):
+    """Algorithm 3, hybrid mode through mfh_plan_hybrid: the library enumerates the memory-feasible candidates,
+    ranks them by t_NN(p), commits and times only the top `k_nn` on the device (releasing each before the next) and keeps
+    the best measured one (Eq. 23).  Returns (handle with the chosen plan committed, report).  Needs CUDA."""
+    from .binding import Hamiltonian, _check, _stream
+    h = Hamiltonian(D, B, seed, dtype, kind=kind, seed_h0=seed_h0)
+    try:
+        th = np.ascontiguousarray(theta, dtype=np.float64)
+        assert th.size == theta_size(F, hidden), (th.size, theta_size(F, hidden))
+        buf = ctypes.create_string_buffer(1 << 16)
+        L = lib()
+        L.mfh_plan_hybrid.argtypes = [ctypes.c_void_p, ctypes.POINTER(ctypes.c_double), ctypes.c_int32, ctypes.c_int32, ctypes.c_int64,
+                                      ctypes.c_int64, ctypes.c_int32, ctypes.c_void_p, ctypes.c_char_p, ctypes.c_size_t]
+        _check(L.mfh_plan_hybrid(h._h, _p(th), hidden, k, n_applies_hint, int(hbm_budget_bytes), k_nn, _stream(), buf, len(buf)))
+        h.k = k
+        rec = json.loads(buf.value.decode())
+    except Exception:
+        h.destroy()
+        raise
     n = max(n_applies_hint, 1)
-    tried, best = [], None
-    for cand, t_nn in ranked:
-        h = Hamiltonian(D, cand["B"], seed, dtype, kind=kind, seed_h0=seed_h0)
-        r = h.plan(cand["mode"], k=k, n_applies_hint=n_applies_hint, hbm_budget_bytes=int(budget), measure=True)
-        c = r["chosen"]
-        job = n * c["measured_apply_s"] + c["model_fill_s"]
-        tried.append({"mode": c["mode"], "B": c["B"], "t_nn_s": t_nn, "measured_apply_s": c["measured_apply_s"], "job_s": job})
-        if best is None or job < best[1]:
-            if best is not None:
-                best[0].destroy()
-            best = (h, job, tried[-1])
-        else:
-            h.destroy()
-    return best[0], {"feasible_candidates": sum(c["feasible"] for c in rec["candidates"]), "timed": tried, "chosen": best[2]}
+    timed = [{"mode": c["mode"], "B": c["B"], "t_nn_s": c["surrogate_apply_s"], "measured_apply_s": c["measured_apply_s"],
+              "job_s": n * c["measured_apply_s"] + c["model_fill_s"]} for c in rec["candidates"] if c["measured_apply_s"] > 0]
+    c = rec["chosen"]
+    chosen = {"mode": c["mode"], "B": c["B"], "t_nn_s": c["surrogate_apply_s"], "measured_apply_s": c["measured_apply_s"],
+              "job_s": n * c["measured_apply_s"] + c["model_fill_s"]}
+    return h, {"planner": rec["planner"], "feasible_candidates": sum(x["feasible"] for x in rec["candidates"]), "timed": timed,
+               "chosen": chosen}

@@ -60,3 +60,30 @@ def test_fused_tail_single_launch_is_deterministic_and_self_cleaning():
         err = np.linalg.norm(first.cpu().numpy().astype(np.complex128) - ref) / np.linalg.norm(ref)
         assert err <= tol, (dtype, err)
         h.destroy()
+
+
+def test_handle_belongs_to_its_device_and_a_second_device_works():
+    """include/mfh.h "Devices": a handle lives on the device current in mfh_plan (kernel attributes are kept per handle,
+    not per process).  With two GPUs the same process plans and applies on both; with one GPU only the refusal of a
+    foreign current device can be checked -- skipped there."""
+    import oracle
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two CUDA devices in one process")
+    D, B = 4096, 4096                     # B = 4096: the fused kernel needs > 48 KB of dynamic shared memory
+    psi = make_psi(D, 5)
+    ref = oracle.apply(D, B, 77, psi)
+    outs = []
+    for dev in (0, 1):
+        with torch.cuda.device(dev):
+            h = mfh.Hamiltonian(D, B, 77, "c128")
+            h.plan("procedural")
+            phi = h.apply(torch.from_numpy(psi).cuda()).cpu().numpy()
+            assert np.linalg.norm(phi - ref) / np.linalg.norm(ref) <= 1e-11, dev
+            outs.append((h, phi))
+    with torch.cuda.device(1):            # handle of device 0 used while device 1 is current: refused, not launched
+        with pytest.raises(mfh.MfhError) as e:
+            outs[0][0].apply(torch.from_numpy(psi).cuda())
+        assert e.value.code == mfh.MFH_ERR_BAD_STATE
+    for h, _ in outs:
+        h.destroy()

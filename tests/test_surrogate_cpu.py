@@ -135,3 +135,24 @@ def test_library_surrogate_matches_the_hand_worked_case():
     assert p[0] == pytest.approx(vals["t_nn_1"], rel=1e-14) and p[1] == pytest.approx(vals["t_nn_2"], rel=1e-14)
     loss, _ = sur.loss_grad(theta, X, t, hidden=1)
     assert loss == pytest.approx(vals["loss"], rel=1e-14)
+
+
+def test_feature_map_behind_the_c_abi_matches_its_definition():
+    """x(p) of P:370 is computed by mfh_surrogate_features; here the definition written out, for every candidate of an
+    analytic plan record, and the stored rows of the shipped log stay reproducible."""
+    import math
+    rec = mfh.plan_analytic(32768, "c64", k=16, n_applies_hint=10, hbm_free_bytes=180 * 10**9)
+    free = rec["budget_bytes"]
+    for c in rec["candidates"]:
+        x = sur.features(32768, "c64", 16, c, free, n_task=20, p_row=2, waves=5, gpu_bytes=47.6e9, sms=142)
+        m = c["mode"]
+        want = [math.log(32768), math.log(16), math.log(c["n_blk"]), math.log(c["B"]), math.log(20), 2.0, 5.0,
+                float(m == "full"), float(m == "partial"), float(m == "procedural"), float(m == "pairs"),
+                math.log(c["flops_per_apply"]), c["cache_bytes"] / free, c["work_bytes"] / free, c["total_bytes"] / free, 1.0,
+                math.log(47.6e9), math.log(142)]
+        assert np.allclose(x, want, rtol=1e-15, atol=0), m
+    import ctypes
+    L = mfh.lib()
+    out = (ctypes.c_double * 18)()
+    assert L.mfh_surrogate_features(4096, 0, 1, 0, 512, 1e9, 0.0, 1e6, 1e9, 1, 1, 1, 1e11, 148, out) == mfh.MFH_ERR_INVALID_ARG   # mode AUTO
+    assert L.mfh_plan_hybrid(None, None, 16, 1, 1, 0, 3, None, None, 0) == mfh.MFH_ERR_INVALID_ARG
