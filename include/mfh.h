@@ -62,7 +62,10 @@ enum { MFH_SRC_GUE = 0,           /* H = lambda * V(seed)                       
 enum { MFH_MODE_AUTO = 0, MFH_MODE_PROCEDURAL = 1, MFH_MODE_PARTIAL = 2, MFH_MODE_FULL = 3,
        /* Hermitian (canonical-pair) cache, Eq. 27: block (n,m), n <= m, is stored once
         * and used for phi^[n] += C psi^[m] and phi^[m] += C^dagger psi^[n]; as many pairs as the budget
-        * allows (nearest block diagonals first), the rest is generated.  Half the bytes of FULL. */
+        * allows (nearest block diagonals first), the rest is generated.  Half the memory of FULL.  One vector: every
+        * loaded entry is used for both positions (half the bytes per apply as well).  k vectors (complex64, B % 128
+        * == 0): the tensor-core kernel reads the stored block a second time, transposed, for the mirrored position
+        * (same bytes per apply as FULL; complex128 k-vector plans do not support the pair cache). */
        MFH_MODE_PAIRS = 4 };
 
 #define MFH_MAX_K 16       /* largest number of simultaneous vectors */

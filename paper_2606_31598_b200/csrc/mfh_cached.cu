@@ -510,9 +510,12 @@ static int launch_pairs_t(mfh_handle h, const void* psi, cudaStream_t st)
 int launch_cached_pairs(mfh_handle h, const void* psi, cudaStream_t st)
 {
     const Plan& p = h->plan;
-    if (p.pair_items.empty()) return MFH_OK;
+    if (p.n_cached == 0) return MFH_OK;
     if (p.k != 1) {
-        set_error("the pair cache with k > 1 is not supported yet");
+        // k vectors (complex64, B % 128 == 0): the tensor-core kernel serves the stored block directly and the mirrored
+        // position by a second, transposed read of the same block (mfh_tc.cu)
+        if (tc_cached_multi_supported(h->dtype, p.k, p.B)) return launch_cached_multi_tc(h, psi, st);
+        set_error("the pair cache with k > 1 needs complex64 and B %% 128 == 0");
         return MFH_ERR_UNSUPPORTED;
     }
     // U 128-bit loads per row per lane x 4 rows in flight; U = 4 at 2 CTAs/SM measured best on C2

@@ -289,7 +289,8 @@ void build_tables(Plan& p, int64_t D, int dtype, int sm_count)
                     push_items(p.items, n, m, kd);
                 }
     }
-    if (p.pairs)   // stored blocks: off-diagonal pairs feed both sides, diagonal blocks the row side only
+    if (p.pairs && p.k == 1)   // stored blocks: off-diagonal pairs feed both sides, diagonal blocks the row side only
+                               // (k-vector pair plans are served block by block by the tensor-core kernel)
         for (int n = 0; n < N; ++n)
             for (int m = n; m < N; ++m)
                 if (p.cache_slot[(size_t)n * N + m] >= 0)
@@ -335,6 +336,8 @@ Candidate evaluate_candidate(int64_t D, int dtype, int k, int B, int cached_per_
     const double entries = (double)p.owned_blocks * B * B;                     // entries this rank applies
     c.cached_fraction = f;
     c.t_cached = c.cache_bytes / kBwRead;
+    if (pairs && k > 1)   // the mirrored positions are served by a second read of the stored blocks (mfh_tc.cu)
+        c.t_cached = (c.cache_bytes + (double)(p.covered_blocks - p.n_cached) * B * B * cb) / kBwRead;
     if (k == 1) {
         // generations: one per mirrored pair, one per one-sided entry, ~half of a diagonal block
         double gens = 0.0;
@@ -418,7 +421,8 @@ int enumerate_candidates(int64_t D, int dtype, int k, int mode, int B_req, int64
         std::vector<std::pair<int, bool>> cs;   // (cached_per_row or band offsets, pairs)
         if (mode == MFH_MODE_AUTO || mode == MFH_MODE_PROCEDURAL) cs.push_back({0, false});
         if (mode == MFH_MODE_AUTO || mode == MFH_MODE_FULL) cs.push_back({N, false});
-        if ((mode == MFH_MODE_AUTO || mode == MFH_MODE_PAIRS) && k == 1 && B % (dtype == MFH_C128 ? 32 : 64) == 0) {
+        const bool pairs_ok = k == 1 ? B % (dtype == MFH_C128 ? 32 : 64) == 0 : tc_cached_multi_supported(dtype, k, B);
+        if ((mode == MFH_MODE_AUTO || mode == MFH_MODE_PAIRS) && pairs_ok) {
             // Hermitian pair cache: the largest number of block diagonals that fits (Eq. 27 over
             // canonical pairs)
             int c = largest_fitting(pair_full_offsets(N), [&](int cc) { return fits(cc, true); });
@@ -442,7 +446,8 @@ int enumerate_candidates(int64_t D, int dtype, int k, int mode, int B_req, int64
             Candidate cand = evaluate_candidate(D, dtype, k, B, c, pairs, n_applies, sm_count, part);
             cand.feasible = (cand.cache_bytes + cand.work_bytes <= budget_bytes);   // Eq. 18
             // cached k-vector blocks: B % 128 == 0 (tensor-core kernel for complex64, FP64 CUDA-core kernel for complex128)
-            if (k > 1 && c > 0 && (pairs || !(tc_cached_multi_supported(dtype, k, B) || cached_multi_c128_supported(dtype, k, B))))
+            if (k > 1 && c > 0 && !(pairs ? tc_cached_multi_supported(dtype, k, B)
+                                          : (tc_cached_multi_supported(dtype, k, B) || cached_multi_c128_supported(dtype, k, B))))
                 cand.feasible = false;
             out.push_back(cand);
         }

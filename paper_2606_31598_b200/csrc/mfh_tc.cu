@@ -384,7 +384,13 @@ __global__ void __launch_bounds__(CT_THREADS, 2) cached_multi_tc_kernel(const Ct
     const int m = blockIdx.y;
     const uint32_t i_base = blockIdx.x * TC_TP;
     const int n = (int)(i_base / (uint32_t)P.B);
-    const int32_t slot = P.cache_slot[n * P.n_blk + m];
+    int32_t slot = P.cache_slot[n * P.n_blk + m];
+    // Hermitian pair cache (MFH_MODE_PAIRS with k > 1): position (n,m) marked -2 is served by the stored canonical block
+    // C = H^[m,n]: phi^[n] += C^dagger psi^[m].  The CTA's 128 output rows are 128 COLUMNS of C; it reads C a second
+    // time, transposed (TR): a stage is 16 rows of C x those 128 columns = eight 2 KB pieces of eight neighbouring
+    // tiles.  (This halves the MEMORY of a k-vector operator, not the bytes per apply: DESIGN.md 6.5.)
+    const bool TR = (slot == -2);
+    if (TR) slot = P.cache_slot[m * P.n_blk + n];
     if (slot < 0) return;   // generated block: the fused kernel's
     // 1024-byte aligned stage base (128B swizzle pattern repeats every 8 rows x 128 B)
     unsigned char* smem = smem_raw_ + ((1024u - (smem_u32(smem_raw_) & 1023u)) & 1023u);
@@ -415,8 +421,9 @@ __global__ void __launch_bounds__(CT_THREADS, 2) cached_multi_tc_kernel(const Ct
     const uint32_t d_tmem = s_tmem;
     const int n_tiles = P.B / (CT_KF / 2);
     // the strip's tiles: block slot, row tile (i_base - n B) / 128, then B/16 tiles of 16 KB
-    const unsigned char* strip = reinterpret_cast<const unsigned char*>(P.cache) + (size_t)slot * P.B * P.B * 8 +
-                                 (size_t)((i_base - (uint32_t)n * P.B) / TC_TP) * (P.B / (CT_KF / 2)) * CT_RAW;
+    const unsigned char* block = reinterpret_cast<const unsigned char*>(P.cache) + (size_t)slot * P.B * P.B * 8;
+    const uint32_t rt_own = (i_base - (uint32_t)n * P.B) / TC_TP;   // the CTA's 128-row (TR: 128-column) tile index in its block
+    const unsigned char* strip = block + (size_t)rt_own * (P.B / (CT_KF / 2)) * CT_RAW;
 
     if (w == TC_GEN_WARPS + 1) {
         // ---- TMA producer: lane 0 copies the tiles, lane 1 the psi rows.  Bulk copies issued by ONE thread are serviced
@@ -431,6 +438,19 @@ __global__ void __launch_bounds__(CT_THREADS, 2) cached_multi_tc_kernel(const Ct
                              "r"(CT_RAW + psi_bytes)
                              : "memory");
             __syncwarp();
+            if (TR) {
+                // 16 rows of C (row tile t / 8, rows 16 (t % 8) ..) x the CTA's 128 columns: column tiles 8 rt_own .. + 7,
+                // one 2 KB piece of each, issued by eight lanes
+                if (lane >= 2 && lane < 10) {
+                    const int j = lane - 2;
+                    asm volatile(
+                        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                            smem_u32(smem + s * CT_RAW + j * 2048)),
+                        "l"(block + ((size_t)(t >> 3) * (P.B / (CT_KF / 2)) + 8 * rt_own + j) * CT_RAW + (size_t)(t & 7) * 2048), "r"(2048),
+                        "r"(smem_u32(&raw_full[s]))
+                        : "memory");
+                }
+            }
             if (lane == 1) {
                 // the 16 psi rows of the tile are contiguous in [D][k]: one 1-D bulk copy
                 asm volatile(
@@ -438,7 +458,7 @@ __global__ void __launch_bounds__(CT_THREADS, 2) cached_multi_tc_kernel(const Ct
                         smem_u32(psis + s * CT_PSI)),
                     "l"(P.psi + ((size_t)m * P.B + (size_t)t * (CT_KF / 2)) * P.k), "r"(psi_bytes), "r"(smem_u32(&raw_full[s]))
                     : "memory");
-            } else if (lane == 0) {
+            } else if (lane == 0 && !TR) {
                 // tile t of the strip: 16 KB contiguous in the tiled cache layout (mfh_internal.cuh tiled_cache_offset)
                 asm volatile(
                     "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
@@ -481,11 +501,25 @@ __global__ void __launch_bounds__(CT_THREADS, 2) cached_multi_tc_kernel(const Ct
             mbar_wait(&raw_full[s], u & 1);
             const float2 x = (v < k) ? reinterpret_cast<const float2*>(psis + s * CT_PSI)[qb * k + v] : float2{0.f, 0.f};
             float4 raw[4];
-            const unsigned char* rp = smem + s * CT_RAW + p * 128;
+            if (!TR) {
+                const unsigned char* rp = smem + s * CT_RAW + p * 128;
 #pragma unroll
-            for (int gg = 0; gg < 4; ++gg) {
-                const int g = gsel + 2 * gg;   // logical 16-byte chunk of the row; 128B swizzle: chunk ^ (row % 8)
-                raw[gg] = *reinterpret_cast<const float4*>(rp + ((g ^ (p & 7)) << 4));
+                for (int gg = 0; gg < 4; ++gg) {
+                    const int g = gsel + 2 * gg;   // logical 16-byte chunk of the row; 128B swizzle: chunk ^ (row % 8)
+                    raw[gg] = *reinterpret_cast<const float4*>(rp + ((g ^ (p & 7)) << 4));
+                }
+            } else {
+                // lane p = column b of C: piece p / 16, column p % 16; K index 2 a + c over the 16 rows a of the stage,
+                // chunk g <-> rows 2 g, 2 g + 1 (so the TMEM columns are the same as in the direct use)
+                const unsigned char* cp = smem + s * CT_RAW + (p >> 4) * 2048 + (p & 1) * 8;
+                const int cc = (p & 15) >> 1;
+#pragma unroll
+                for (int gg = 0; gg < 4; ++gg) {
+                    const int a0 = 2 * (gsel + 2 * gg), a1 = a0 + 1;
+                    const float2 e0 = *reinterpret_cast<const float2*>(cp + a0 * 128 + ((cc ^ (a0 & 7)) << 4));
+                    const float2 e1 = *reinterpret_cast<const float2*>(cp + a1 * 128 + ((cc ^ (a1 & 7)) << 4));
+                    raw[gg] = make_float4(e0.x, e0.y, e1.x, e1.y);
+                }
             }
             float prh, prl, pih, pil;
             split_tf32(x.x, prh, prl);
@@ -513,10 +547,13 @@ __global__ void __launch_bounds__(CT_THREADS, 2) cached_multi_tc_kernel(const Ct
             {
                 float* b = reinterpret_cast<float*>(bimg + ts * CT_BSTAGE);
                 constexpr int BT = CT_B_TILE / 4;
-                *reinterpret_cast<float2*>(b + o_re) = make_float2(prh, -pih);        // n = v:      Re Psi, -Im Psi
-                *reinterpret_cast<float2*>(b + o_im) = make_float2(pih, prh);         // n = 16 + v: Im Psi,  Re Psi
-                *reinterpret_cast<float2*>(b + BT + o_re) = make_float2(prl, -pil);
-                *reinterpret_cast<float2*>(b + BT + o_im) = make_float2(pil, prl);
+                // direct use: [Re Phi | Im Phi] += Re C [Re Psi | Im Psi] + Im C [-Im Psi | Re Psi];
+                // transposed use (conjugate): ...   + Im C [ Im Psi | -Re Psi]
+                const float sg = TR ? -1.f : 1.f;
+                *reinterpret_cast<float2*>(b + o_re) = make_float2(prh, -sg * pih);       // n = v:      Re Psi, -+Im Psi
+                *reinterpret_cast<float2*>(b + o_im) = make_float2(pih, sg * prh);        // n = 16 + v: Im Psi,  +-Re Psi
+                *reinterpret_cast<float2*>(b + BT + o_re) = make_float2(prl, -sg * pil);
+                *reinterpret_cast<float2*>(b + BT + o_im) = make_float2(pil, sg * prl);
             }
             asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");

@@ -32,6 +32,8 @@ VARIANTS = {
     "C5-pairs": dict(CONFIGS["C5"], mode="pairs"),
     # C3's coupling scan with V cached (8.6 GB): each stored block is read once for the 16 vectors
     "C3-cached": dict(CONFIGS["C3"], mode="full"),
+    # ... and from the Hermitian pair cache (4.4 GB): the mirrored positions by a second, transposed read
+    "C3-pairs": dict(CONFIGS["C3"], mode="pairs"),
     # the same scan in double precision from cached complex128 blocks (17.2 GB): FP64 CUDA-core kernel
     "C3-c128-cached": dict(CONFIGS["C3"], mode="full", dtype="c128"),
 }

@@ -44,8 +44,8 @@ def test_materialized_block_matches_the_formula(dtype, n, m):
 @pytest.mark.parametrize("mode", ["procedural", "partial", "full", "pairs"])
 @pytest.mark.parametrize("k", [1, 4])
 def test_apply_in_every_mode_vs_oracle(dtype, mode, k):
-    if mode == "pairs" and k > 1:
-        pytest.skip("the pair cache serves one vector")
+    if mode == "pairs" and k > 1 and dtype == "c128":
+        pytest.skip("the k-vector pair cache is the complex64 tensor-core kernel's (transposed second read)")
     D, B = 2048, 256
     Psi = make_psi(D, 41, k=k, dtype=dtype)
     h = handle(D, B, dtype, lam=0.8)

@@ -29,8 +29,8 @@ def upload(h, H, B, store, dtype, device_blocks=False):
 @pytest.mark.parametrize("store,herm", [("full", True), ("full", False), ("pairs", True)])
 @pytest.mark.parametrize("k", [1, 4])
 def test_external_operator_vs_oracle(dtype, store, herm, k):
-    if store == "pairs" and k > 1:
-        pytest.skip("the pair cache serves one vector")
+    if store == "pairs" and k > 1 and dtype == "c128":
+        pytest.skip("the k-vector pair cache is the complex64 tensor-core kernel's (transposed second read)")
     D, B = 1024, 128
     H = dense_matrix(D, 11, hermitian=herm)
     if dtype == "c64":

@@ -27,10 +27,10 @@ def _cases():
         for dtype in ("c128", "c64"):
             for mode in ("procedural", "partial", "full", "pairs"):
                 k = int(rng.choice([1, 1, 1, 2, 3, 5, 8, 13, 16]))
-                if mode == "pairs" and (k > 1 or (dtype == "c64" and B % 64)):
-                    k = 1
-                    if dtype == "c64" and B % 64:
-                        continue
+                if mode == "pairs" and k > 1 and not (dtype == "c64" and B % 128 == 0):
+                    k = 1                                      # k-vector pair caches: complex64, B % 128 == 0 only
+                if mode == "pairs" and k == 1 and dtype == "c64" and B % 64:
+                    continue
                 if k > 1 and mode in ("partial", "full") and B % 128:
                     continue                                   # cached k-vector kernels need B % 128 == 0
                 frac = float(rng.choice([0.2, 0.45, 0.7]))
