@@ -400,10 +400,10 @@ __global__ void __launch_bounds__(CT_THREADS, 2) cached_multi_tc_kernel(const Ct
     if (tid == 0) {
         for (int s = 0; s < CT_STAGES; ++s) {
             mbar_init(&raw_full[s], 1);
-            mbar_init(&raw_empty[s], TC_GEN_WARPS);
+            mbar_init(&raw_empty[s], TC_GEN_WARPS / 2);
         }
         for (int s = 0; s < CT_TSTAGES; ++s) {
-            mbar_init(&a_full[s], TC_GEN_WARPS);
+            mbar_init(&a_full[s], TC_GEN_WARPS / 2);
             mbar_init(&a_empty[s], 1);
         }
         mbar_init(&done, 1);
@@ -488,72 +488,66 @@ __global__ void __launch_bounds__(CT_THREADS, 2) cached_multi_tc_kernel(const Ct
             __syncwarp();
         }
     } else {
-        // ---- converter warps: thread = (row p, 4 of the 8 four-float groups of the row) ----
-        const int p = tid & (TC_TP - 1), gsel = tid >> 7, k = P.k;
+        // ---- converter warps: two groups of four warps take the tiles alternately (group g: tiles g, g + 2, ...), so
+        // that the per-tile chain of a warp (wait, load, split, tcgen05.st, wait::st, fences, arrive) of one tile
+        // overlaps with the other group's; thread = row p, all eight four-float groups of the row ----
+        const int p = tid & (TC_TP - 1), grp = tid >> 7, k = P.k;
         const uint32_t a_lane = d_tmem + ((uint32_t)(p & ~31) << 16);
-        const int v = tid & 15, qb = tid >> 4;   // psi element (column qb of the tile, vector v)
-        // psi image element (n, k'): rows n = v and 16 + v, K positions k' = 2 qb and 2 qb + 1 (adjacent floats)
-        const int o_re = ((v & 7) * 16 + (v >> 3) * CT_SBO + (qb >> 1) * 128 + (qb & 1) * 8) / 4;
-        const int o_im = o_re + 2 * CT_SBO / 4;
-        for (int t = 0; t < n_tiles; ++t) {
+        const int v = p & 15, qb0 = p >> 4;      // psi elements (columns qb0 and qb0 + 8 of the tile, vector v)
+        for (int t = grp; t < n_tiles; t += 2) {
             const int s = t % CT_STAGES, u = t / CT_STAGES;
             const int ts = t % CT_TSTAGES, tu = t / CT_TSTAGES;
             mbar_wait(&raw_full[s], u & 1);
-            const float2 x = (v < k) ? reinterpret_cast<const float2*>(psis + s * CT_PSI)[qb * k + v] : float2{0.f, 0.f};
-            float4 raw[4];
+            float2 x[2];
+#pragma unroll
+            for (int h2 = 0; h2 < 2; ++h2)
+                x[h2] = (v < k) ? reinterpret_cast<const float2*>(psis + s * CT_PSI)[(qb0 + 8 * h2) * k + v] : float2{0.f, 0.f};
+            float4 raw[8];
             if (!TR) {
                 const unsigned char* rp = smem + s * CT_RAW + p * 128;
 #pragma unroll
-                for (int gg = 0; gg < 4; ++gg) {
-                    const int g = gsel + 2 * gg;   // logical 16-byte chunk of the row; 128B swizzle: chunk ^ (row % 8)
-                    raw[gg] = *reinterpret_cast<const float4*>(rp + ((g ^ (p & 7)) << 4));
-                }
+                for (int g = 0; g < 8; ++g) raw[g] = *reinterpret_cast<const float4*>(rp + ((g ^ (p & 7)) << 4));
             } else {
-                // lane p = column b of C: piece p / 16, column p % 16; K index 2 a + c over the 16 rows a of the stage,
-                // chunk g <-> rows 2 g, 2 g + 1 (so the TMEM columns are the same as in the direct use)
                 const unsigned char* cp = smem + s * CT_RAW + (p >> 4) * 2048 + (p & 1) * 8;
                 const int cc = (p & 15) >> 1;
 #pragma unroll
-                for (int gg = 0; gg < 4; ++gg) {
-                    const int a0 = 2 * (gsel + 2 * gg), a1 = a0 + 1;
+                for (int g = 0; g < 8; ++g) {
+                    const int a0 = 2 * g, a1 = a0 + 1;
                     const float2 e0 = *reinterpret_cast<const float2*>(cp + a0 * 128 + ((cc ^ (a0 & 7)) << 4));
                     const float2 e1 = *reinterpret_cast<const float2*>(cp + a1 * 128 + ((cc ^ (a1 & 7)) << 4));
-                    raw[gg] = make_float4(e0.x, e0.y, e1.x, e1.y);
+                    raw[g] = make_float4(e0.x, e0.y, e1.x, e1.y);
                 }
             }
-            float prh, prl, pih, pil;
-            split_tf32(x.x, prh, prl);
-            split_tf32(x.y, pih, pil);
             if (tu > 0) mbar_wait(&a_empty[ts], (tu - 1) & 1);
 #pragma unroll
-            for (int gg = 0; gg < 4; ++gg) {
-                const int g = gsel + 2 * gg;
-                // A_hi = the raw words (the tensor core reads only the TF32 part, i.e. truncates), A_lo = x - trunc(x),
-                // exact: one instruction per value less than rounding hi to nearest.  The truncation of hi is undone
-                // by lo; what remains one-sided is the tensor core's truncation of lo itself (2^-21 of x) and the
-                // dropped lo x lo term, far below the fp32 accumulation error that dominates (1e-5).
-                const float l0 = raw[gg].x - __uint_as_float(__float_as_uint(raw[gg].x) & 0xffffe000u);
-                const float l1 = raw[gg].y - __uint_as_float(__float_as_uint(raw[gg].y) & 0xffffe000u);
-                const float l2 = raw[gg].z - __uint_as_float(__float_as_uint(raw[gg].z) & 0xffffe000u);
-                const float l3 = raw[gg].w - __uint_as_float(__float_as_uint(raw[gg].w) & 0xffffe000u);
+            for (int g = 0; g < 8; ++g) {
+                const float l0 = raw[g].x - __uint_as_float(__float_as_uint(raw[g].x) & 0xffffe000u);
+                const float l1 = raw[g].y - __uint_as_float(__float_as_uint(raw[g].y) & 0xffffe000u);
+                const float l2 = raw[g].z - __uint_as_float(__float_as_uint(raw[g].z) & 0xffffe000u);
+                const float l3 = raw[g].w - __uint_as_float(__float_as_uint(raw[g].w) & 0xffffe000u);
                 const uint32_t ta = a_lane + (uint32_t)(TC_ACC_COLS + ts * CT_A_STAGE_COLS + 4 * g);
-                tmem_st4(ta, raw[gg].x, raw[gg].y, raw[gg].z, raw[gg].w);
+                tmem_st4(ta, raw[g].x, raw[g].y, raw[g].z, raw[g].w);
                 tmem_st4(ta + CT_KF, l0, l1, l2, l3);
             }
-            // every lane has consumed its shared-memory words (the splits depend on them): only now may
-            // the TMA producer overwrite the raw stage
             __syncwarp();
             if (lane == 0) mbar_arrive(&raw_empty[s]);
             {
                 float* b = reinterpret_cast<float*>(bimg + ts * CT_BSTAGE);
                 constexpr int BT = CT_B_TILE / 4;
-                // direct use: [Re Phi | Im Phi] += Re C [Re Psi | Im Psi] + Im C [-Im Psi | Re Psi];
-                // transposed use (conjugate): ...   + Im C [ Im Psi | -Re Psi]
                 const float sg = TR ? -1.f : 1.f;
-                *reinterpret_cast<float2*>(b + o_re) = make_float2(prh, -sg * pih);       // n = v:      Re Psi, -+Im Psi
-                *reinterpret_cast<float2*>(b + o_im) = make_float2(pih, sg * prh);        // n = 16 + v: Im Psi,  +-Re Psi
-                *reinterpret_cast<float2*>(b + BT + o_re) = make_float2(prl, -sg * pil);
-                *reinterpret_cast<float2*>(b + BT + o_im) = make_float2(pil, sg * prl);
+#pragma unroll
+                for (int h2 = 0; h2 < 2; ++h2) {
+                    const int qb = qb0 + 8 * h2;
+                    const int o_re = ((v & 7) * 16 + (v >> 3) * CT_SBO + (qb >> 1) * 128 + (qb & 1) * 8) / 4;
+                    const int o_im = o_re + 2 * CT_SBO / 4;
+                    float prh, prl, pih, pil;
+                    split_tf32(x[h2].x, prh, prl);
+                    split_tf32(x[h2].y, pih, pil);
+                    *reinterpret_cast<float2*>(b + o_re) = make_float2(prh, -sg * pih);
+                    *reinterpret_cast<float2*>(b + o_im) = make_float2(pih, sg * prh);
+                    *reinterpret_cast<float2*>(b + BT + o_re) = make_float2(prl, -sg * pil);
+                    *reinterpret_cast<float2*>(b + BT + o_im) = make_float2(pil, sg * prl);
+                }
             }
             asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
