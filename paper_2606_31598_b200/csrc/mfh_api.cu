@@ -606,8 +606,9 @@ MFH_API int mfh_get_plan(mfh_handle h, char* json_out, size_t json_cap)
              p.n_blk, p.k, (long long)p.n_cached, p.cached_per_row,
              (double)p.covered_blocks / (double)std::max<int64_t>(p.owned_blocks, 1), p.cache_bytes, p.work_bytes, p.n_slots,
              p.items.size(), p.pair_items.size(), p.R, p.Q, p.stream_sms,
-             h->fused_tail ? 1 : 1 + (p.n_cached > 0) + ((p.k == 1 && !p.items.empty()) ||
-                                                          (p.k > 1 && p.covered_blocks < p.owned_blocks)));
+             h->fused_tail ? 1 : (partial_overlap_supported(h) ? 2 /* one kernel for both parts + reduce */
+                                  : 1 + (p.n_cached > 0) + ((p.k == 1 && !p.items.empty()) ||
+                                                            (p.k > 1 && p.covered_blocks < p.owned_blocks))));
     copy_json(buf, json_out, json_cap);
     return MFH_OK;
 }

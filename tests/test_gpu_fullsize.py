@@ -299,6 +299,27 @@ def test_c5_partial_pair_cache_every_row_vs_procedural():
     check(phi, phi_p, 1e-13, "C5 partial pairs vs procedural, all rows")
 
 
+def test_complex64_partial_cache_mid_size_every_row():
+    """The partial-cache kernel in complex64 (streaming role: 16-byte unit = two entries) beyond the small shapes of
+    the sweep: D = 32768, B = 1024, half the blocks cached, against a full oracle apply and the generated operator."""
+    D, B, seed = 32768, 1024, 77
+    psi = make_psi(D, 5, dtype="c64")
+    ref = oracle.apply(D, B, seed, psi)
+    h = mfh.Hamiltonian(D, B, seed, "c64")
+    plan = h.plan("partial", n_applies_hint=100, hbm_budget_bytes=int(0.5 * D * D * 8))
+    assert plan["chosen"]["mode"] == "partial" and 0.3 < plan["chosen"]["cached_fraction"] < 0.6
+    assert h.get_plan()["launches_per_apply"] == 2 and h.get_plan()["stream_sms"] > 0
+    d_psi = to_dev(psi)
+    phi = h.apply(d_psi).cpu().numpy()
+    h.destroy()
+    check(phi, ref, 1e-4, "c64 partial cache, all rows")
+    hp = mfh.Hamiltonian(D, B, seed, "c64")
+    hp.plan("procedural")
+    phi_p = hp.apply(d_psi).cpu().numpy()
+    hp.destroy()
+    check(phi, phi_p, 2e-6, "c64 partial vs generated, all rows")
+
+
 def test_system_bath_paper_size_stratified_rows_and_c64_vs_c128():
     """The paper's 18-qubit shape: d_S = 4, d_B = 65536, complex64, two cached operators of 32 GiB."""
     import torch
