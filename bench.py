@@ -530,7 +530,7 @@ COMPONENTS_OF = {("c128", "k1"): {"kernels": ("comp_philox", "comp_philox_bm_c12
 NCU_TRAFFIC = {("cached_kernel", 65536): (68.725132e9 + 5.106432e6, "profiles/r02_cached_c2_ncu_full.md"),
                ("partial_overlap_kernel", 131072): (146.236774e9 + 252.962816e6, "profiles/r02_partial_overlap_c5_ncu_full.md"),
                ("cached_pairs_kernel", 65536): (35.438780e9 + 249.902592e6, "profiles/r01_pairs_c2_ncu_full.md"),
-               ("cached_multi_tc_kernel", 32768): (8.595413e9 + 135.389184e6, "profiles/r02_cached_multi_tc_c3_ncu_full.md"),
+               ("cached_multi_tc_kernel", 32768): (8.595266e9 + 135.4e6, "profiles/r02_cached_multi_tc_c3_ncu_full.md"),
                ("cached_multi_kernel_c128", 32768): (17.203616e9 + 268.850432e6, "profiles/r02_cached_multi_c128_c3_ncu_full.md"),
                ("proc_single_kernel", 262144): (22.890752e6 + 631.663104e6, "profiles/r02_proc_single_c4_ncu_full.md"),
                ("proc_multi_tc_kernel", 32768): (4.513792e6 + 81.728768e6, "profiles/r02_proc_multi_tc_c3_ncu_full.md")}
