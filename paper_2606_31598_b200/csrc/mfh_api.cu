@@ -57,7 +57,7 @@ static cudaError_t guarded_malloc(mfh_handle h, void** user, size_t bytes)
 static int free_plan_resources(mfh_handle h)
 {
     void** ptrs[] = {&h->d_cache, &h->d_work, &h->d_h0, (void**)&h->d_cache_slot, (void**)&h->d_items,
-                     (void**)&h->d_pair_items,
+                     (void**)&h->d_pair_items, (void**)&h->d_tc_pairs, (void**)&h->d_tc_skip,
                      (void**)&h->d_slot_list, (void**)&h->d_counter, (void**)&h->d_expected, &h->d_cheb, &h->d_io, &h->d_lanczos, &h->d_stage};
     for (void** p : ptrs) *p = nullptr;
     for (auto& g : h->guarded) cudaFree(g.first);
@@ -145,6 +145,12 @@ static int commit_plan(mfh_handle h, const Plan& p, cudaStream_t st)
         MFH_CUDA_CHECK(guarded_malloc(h, (void**)&h->d_pair_items, q.pair_items.size() * sizeof(ProcItem)));
         MFH_CUDA_CHECK(cudaMemcpyAsync(h->d_pair_items, q.pair_items.data(), q.pair_items.size() * sizeof(ProcItem),
                                        cudaMemcpyHostToDevice, st));
+    }
+    if (!q.tc_pairs.empty()) {   // two-sided tensor-core generator (k-vector complex64 plans)
+        MFH_CUDA_CHECK(guarded_malloc(h, (void**)&h->d_tc_pairs, q.tc_pairs.size() * sizeof(int32_t)));
+        MFH_CUDA_CHECK(cudaMemcpyAsync(h->d_tc_pairs, q.tc_pairs.data(), q.tc_pairs.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+        MFH_CUDA_CHECK(guarded_malloc(h, (void**)&h->d_tc_skip, q.tc_skip.size()));
+        MFH_CUDA_CHECK(cudaMemcpyAsync(h->d_tc_skip, q.tc_skip.data(), q.tc_skip.size(), cudaMemcpyHostToDevice, st));
     }
     MFH_CUDA_CHECK(guarded_malloc(h, (void**)&h->d_counter, (3 + (size_t)q.n_blk) * sizeof(int32_t)));
     MFH_CUDA_CHECK(cudaMemsetAsync(h->d_counter, 0, (3 + (size_t)q.n_blk) * sizeof(int32_t), st));
@@ -518,6 +524,7 @@ static int plan_core(mfh_handle h, int32_t mode, int32_t k, int64_t n_applies_hi
         p.part_rank = part.rank;
         p.part_world = part.world;
         p.part_scheme = part.scheme;
+        p.allow_tc_pairs = c.tc_pairs && (h->kind != MFH_SRC_ANALYTIC);
         build_tables(p, h->D, h->dtype, h->sm_count);
         return p;
     };

@@ -68,6 +68,8 @@ struct Plan {
     int32_t cached_per_row = 0;
     int32_t n_slots = 0;       // partial vectors in the workspace
     int32_t slot_cache = -1, slot_row0 = -1, slot_col0 = -1, slot_multi = -1;
+    int32_t slot_mcol0 = -1;   // k-vector two-sided generator (mfh_tc.cu): column-side slots, one per (row block, 128-row strip)
+    bool allow_tc_pairs = true;   // caller: the source is seeded (the two-sided tensor-core generator is the Philox path)
     size_t cache_bytes = 0, work_bytes = 0;
     int32_t part_rank = 0, part_world = 1, part_scheme = 0;   // mfh_set_partition
     int64_t owned_blocks = 0;     // block positions this rank is responsible for (n_blk^2 on one GPU)
@@ -77,6 +79,8 @@ struct Plan {
     std::vector<uint8_t> pair_kind;    // [n_blk*n_blk]
     std::vector<ProcItem> items;       // fused generate-and-apply kernel
     std::vector<ProcItem> pair_items;  // cached pair kernel (pairs mode)
+    std::vector<int32_t> tc_pairs;     // k-vector two-sided generator: (row block, column block) of every pair it serves
+    std::vector<uint8_t> tc_skip;      // [n_blk*n_blk] 1 = position served by the two-sided generator (one-sided kernel skips it)
     std::vector<uint8_t> slot_valid;   // [n_blk][n_slots]
     std::string json;
 };
@@ -105,6 +109,8 @@ struct mfh_handle_s {
     int32_t* d_cache_slot = nullptr;
     mfh::ProcItem* d_items = nullptr;
     mfh::ProcItem* d_pair_items = nullptr;
+    int32_t* d_tc_pairs = nullptr;    // plan.tc_pairs
+    uint8_t* d_tc_skip = nullptr;     // plan.tc_skip
     int32_t* d_slot_list = nullptr;   // [n_blk][n_slots+1]: count | flags, then the valid slots in ascending order
     double* d_lambdas = nullptr;    // MFH_MAX_K doubles, refreshed by every apply
     int32_t* d_counter = nullptr;   // dynamic work counters: [0] procedural kernel, [1] pair kernel, [2] CTAs finished,
@@ -174,6 +180,7 @@ int launch_partial_overlap(mfh_handle h, const void* psi, cudaStream_t st);   //
 int launch_proc_multi(mfh_handle h, const void* psi, cudaStream_t st);
 bool tc_multi_supported(mfh_handle h);                                   // mfh_tc.cu
 int launch_proc_multi_tc(mfh_handle h, const void* psi, cudaStream_t st);
+bool tc_pairs_supported(int dtype, int k, int B, int part_world);        // two-sided tensor-core generator
 bool tc_cached_multi_supported(int dtype, int k, int B);
 bool cached_multi_c128_supported(int dtype, int k, int B);               // mfh_cached.cu
 int launch_cached_multi_tc(mfh_handle h, const void* psi, cudaStream_t st);

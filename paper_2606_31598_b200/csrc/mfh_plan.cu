@@ -255,6 +255,25 @@ void build_tables(Plan& p, int64_t D, int dtype, int sm_count)
         p.slot_multi = s;
         s += N;
     }
+    // k-vector two-sided generator (complex64, mfh_tc.cu): a block pair whose two positions are both generated is
+    // generated ONCE; its column side gets one slot per (row block, 128-row strip), like the one-vector kernel's
+    p.tc_pairs.clear();
+    p.tc_skip.clear();
+    p.slot_mcol0 = -1;
+    const int tcS = p.B / 128;
+    if (p.allow_tc_pairs && tc_pairs_supported(dtype, p.k, p.B, part.world)) {
+        for (int n = 0; n < N; ++n)
+            for (int m = n + 1; m < N; ++m)
+                if (uncached(n, m) && uncached(m, n)) {
+                    p.tc_pairs.push_back(n);
+                    p.tc_pairs.push_back(m);
+                }
+        if (!p.tc_pairs.empty()) {
+            p.tc_skip.assign((size_t)N * N, 0);
+            p.slot_mcol0 = s;
+            s += N * tcS;
+        }
+    }
     p.n_slots = s;
     p.slot_valid.assign((size_t)N * std::max(s, 1), 0);
     auto valid = [&](int b, int slot) -> uint8_t& { return p.slot_valid[(size_t)b * p.n_slots + slot]; };
@@ -262,6 +281,11 @@ void build_tables(Plan& p, int64_t D, int dtype, int sm_count)
         if (p.slot_cache >= 0) valid(b, p.slot_cache) = 1;
         if (p.slot_multi >= 0)
             for (int m = 0; m < N; ++m) valid(b, p.slot_multi + m) = own(b, m);   // nobody writes a block that is not ours
+    }
+    for (size_t q = 0; q + 1 < p.tc_pairs.size(); q += 2) {
+        const int n = p.tc_pairs[q], m = p.tc_pairs[q + 1];
+        p.tc_skip[(size_t)n * N + m] = p.tc_skip[(size_t)m * N + n] = 1;
+        for (int t = 0; t < tcS; ++t) valid(m, p.slot_mcol0 + n * tcS + t) = 1;
     }
     const int strip = p.B / p.Q;
     auto push_items = [&](std::vector<ProcItem>& dst, int n, int m, uint8_t kd) {
@@ -311,7 +335,7 @@ static size_t fixed_work_bytes(int64_t D, int dtype, int k)
 }
 
 Candidate evaluate_candidate(int64_t D, int dtype, int k, int B, int cached_per_row, bool pairs,
-                             int64_t n_applies, int sm_count, const Partition& part)
+                             int64_t n_applies, int sm_count, const Partition& part, double budget_bytes)
 {
     Candidate c;
     Plan p;
@@ -324,6 +348,13 @@ Candidate evaluate_candidate(int64_t D, int dtype, int k, int B, int cached_per_
     p.part_scheme = part.scheme;
     c.pairs = pairs;
     build_tables(p, D, dtype, sm_count);
+    if (budget_bytes >= 0 && !p.tc_pairs.empty() &&
+        (double)p.cache_bytes + (double)p.work_bytes + (double)fixed_work_bytes(D, dtype, k) > budget_bytes) {
+        // the column-side slots of the two-sided k-vector generator do not fit: one-sided generation instead
+        p.allow_tc_pairs = false;
+        build_tables(p, D, dtype, sm_count);
+    }
+    c.tc_pairs = p.allow_tc_pairs;
     c.B = B;
     c.mode = p.mode;
     c.cached_per_row = cached_per_row;
@@ -353,7 +384,9 @@ Candidate evaluate_candidate(int64_t D, int dtype, int k, int B, int cached_per_
         }
         c.t_proc = t;
     } else {
-        c.t_proc = (1.0 - f) * entries / gen_entries_per_s(dtype, k);
+        // the two-sided generator produces both positions of a pair from one generation
+        const double gens = (1.0 - f) * entries - 0.5 * (double)p.tc_pairs.size() * B * B;
+        c.t_proc = gens / gen_entries_per_s(dtype, k);
     }
     int launches = 1 + (p.n_cached > 0) + (p.covered_blocks < p.owned_blocks);
     c.t_reduce = (double)p.n_slots * 0.6 * D * k * cb / kBwRead;
@@ -415,7 +448,7 @@ int enumerate_candidates(int64_t D, int dtype, int k, int mode, int B_req, int64
         const int N = (int)(D / B);
         // cache budget -> cached blocks per row (Eq. 27 with full blocks; rows kept balanced)
         auto fits = [&](int c, bool pairs) {
-            Candidate t = evaluate_candidate(D, dtype, k, B, c, pairs, n_applies, sm_count, part);
+            Candidate t = evaluate_candidate(D, dtype, k, B, c, pairs, n_applies, sm_count, part, budget_bytes);
             return t.cache_bytes + t.work_bytes <= budget_bytes;
         };
         std::vector<std::pair<int, bool>> cs;   // (cached_per_row or band offsets, pairs)
@@ -443,7 +476,7 @@ int enumerate_candidates(int64_t D, int dtype, int k, int mode, int B_req, int64
                     if (cc > 0 && cc < c) cs.push_back({cc, false});
         }
         for (auto [c, pairs] : cs) {
-            Candidate cand = evaluate_candidate(D, dtype, k, B, c, pairs, n_applies, sm_count, part);
+            Candidate cand = evaluate_candidate(D, dtype, k, B, c, pairs, n_applies, sm_count, part, budget_bytes);
             cand.feasible = (cand.cache_bytes + cand.work_bytes <= budget_bytes);   // Eq. 18
             // cached k-vector blocks: B % 128 == 0 (tensor-core kernel for complex64, FP64 CUDA-core kernel for complex128)
             if (k > 1 && c > 0 && !(pairs ? tc_cached_multi_supported(dtype, k, B)

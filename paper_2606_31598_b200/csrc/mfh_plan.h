@@ -20,6 +20,8 @@ struct Candidate {
     int B = 0, n_blk = 0, mode = 0, cached_per_row = 0;
     int64_t n_cached = 0;
     bool pairs = false;                                  // Hermitian pair cache
+    bool tc_pairs = true;                                // k-vector complex64 plans: may use the two-sided generator (needs
+                                                         // N_blk B/128 extra partial slots; dropped when they do not fit)
     int stream_sms = 0;                                  // partial plans: SMs that stream while the others generate
     double cached_fraction = 0;                          // share of the D^2 entries served from the cache
     double cache_bytes = 0, work_bytes = 0;              // M_op, M_work (Eq. 14-17)
@@ -33,7 +35,7 @@ struct Candidate {
 void choose_tiling(int B, int n_blk, int n_pairs, int sm_count, int& R, int& Q);
 void build_tables(Plan& p, int64_t D, int dtype, int sm_count);
 Candidate evaluate_candidate(int64_t D, int dtype, int k, int B, int cached_per_row, bool pairs,
-                             int64_t n_applies, int sm_count, const Partition& part = Partition());
+                             int64_t n_applies, int sm_count, const Partition& part = Partition(), double budget_bytes = -1.0);
 int pair_full_offsets(int n_blk);
 int choose_stream_sms(double cache_bytes, double t_gen_all_sms, int sm_count, double* t_out);
 int enumerate_candidates(int64_t D, int dtype, int k, int mode, int B_req, int64_t n_applies,

@@ -82,6 +82,21 @@ __device__ __forceinline__ void tmem_st4(uint32_t taddr, float a, float b, float
                  : "memory");
 }
 
+// One elected lane of a converged warp (elect.sync): unlike `lane == 0` the compiler knows that exactly one thread is
+// active, so the warp-uniform tcgen05 instructions inside need no per-instruction election loop.
+__device__ __forceinline__ bool elect_one()
+{
+    uint32_t pred;
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "elect.sync _|p, 0xffffffff;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t"
+        "}\n"
+        : "=r"(pred));
+    return pred != 0;
+}
+
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
 {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
@@ -154,6 +169,7 @@ struct TcParams {
     int32_t B, n_blk, k, slot_multi;
     int64_t D;
     const int32_t* cache_slot;
+    const uint8_t* skip;   // [n_blk*n_blk] positions served by the two-sided generator (nullptr: none)
     const float2* psi;   // [D][k]
     float2* work;        // [n_slots][D][k]
 };
@@ -235,7 +251,7 @@ __device__ __forceinline__ void tc_mma_warp(const TcParams& P, unsigned char* sm
         const int s = t % TC_STAGES, u = t / TC_STAGES;
         mbar_wait(&full[s], u & 1);
         asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-        if (lane == 0) {
+        if (elect_one()) {
             const uint32_t b0 = smem_u32(smem + s * TC_STAGE);
             const uint32_t a0 = d_tmem + (uint32_t)(TC_A_COL0 + s * TC_A_STAGE_COLS);
 #pragma unroll
@@ -267,6 +283,7 @@ __global__ void __launch_bounds__(TC_THREADS, 2) proc_multi_tc_kernel(const TcPa
     const uint32_t i_base = blockIdx.x * TC_TP;
     const int n = (int)(i_base / (uint32_t)P.B);
     if (P.cache_slot[n * P.n_blk + m] != -1) return;   // cached block: not this kernel's
+    if (P.skip && P.skip[n * P.n_blk + m]) return;     // generated once for both sides by proc_pairs_tc_kernel
 
     if (tid == 0) {
         for (int s = 0; s < TC_STAGES; ++s) {
@@ -302,6 +319,378 @@ __global__ void __launch_bounds__(TC_THREADS, 2) proc_multi_tc_kernel(const TcPa
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(d_tmem), "n"(TC_TMEM_COLS) : "memory");
 }
 
+// --------------------------------------------------------------------------------------------
+// Two-sided k-vector generator (complex64): "generates ... each V block once" AND uses the Hermitian structure
+// (Eq. 11): for a block pair n < m whose two positions are both generated, every entry
+// V_ij (i in block n, j in block m) is generated ONCE and used for  Phi_i += V_ij Psi_j  (row side, exactly the
+// one-sided kernel's TMEM A operand) and for  Phi_j += conj(V_ij) Psi_i  (column side).
+//
+// The column side contracts over the tile's ROWS, which are the lanes of the row side's A operand, so it cannot
+// reuse that operand.  It swaps the operand roles instead: the generated tile is the B operand in shared memory,
+//     B[n = column c][k' = (row r, part)] = (Re V_rc, Im V_rc),      K-major, 128-byte swizzle,
+// written by the generator threads straight from their registers (raw value = TF32 hi part as the tensor core reads
+// it, and a second image x - trunc(x)), and the strip's psi rows are the A operand, resident in TMEM for the whole
+// item (a strip of 128 rows x all columns of the block):
+//     A[(op, v)][k' = (r, part)]:  op = Re:  (Re Psi_rv,  Im Psi_rv);   op = Im:  (Im Psi_rv, -Re Psi_rv).
+// 128 rows x 2 parts = 256 k' would need 256 TMEM columns; the strip's two 64-row halves are stacked in the LANES
+// instead (lanes 0-63: rows 0-63, lanes 64-127: rows 64-127; inside a half: 32 lanes hi image, 32 lanes lo image)
+// and the B operand lists the tile's columns twice (N = 64: columns for the first half of the rows, then for the
+// second half), so one MMA does two K-steps' worth of useful work in the two diagonal quadrants of its [128 x 64]
+// result and the other two quadrants are never read.  A unit = two tiles (32 columns): 16 K-steps x (raw, lo)
+// = 32 MMAs of N = 64; its [128 x 64] accumulator is read out by four epilogue warps, the four quadrant pieces
+// (hi/lo x row halves) are added through shared memory and written to the column-side partial slot of
+// (row block, strip) -- a fixed order, no atomics.
+//
+// One persistent CTA per SM (all 512 TMEM columns): 16 generator warps in two groups that take the tiles
+// alternately (thread = half a row of a tile, as in the one-sided kernel), 4 epilogue warps (they also build the
+// psi operand of every item), one warp issuing the row-side MMAs, one the column-side MMAs.
+// --------------------------------------------------------------------------------------------
+constexpr int T2_GEN_WARPS = 16;
+constexpr int T2_W_EPI = T2_GEN_WARPS;            // warps 16..19: TMEM lane quadrants 0..3
+constexpr int T2_W_DMMA = T2_GEN_WARPS + 4;       // row-side MMA issuer (allocates TMEM)
+constexpr int T2_W_MMMA = T2_GEN_WARPS + 5;       // column-side MMA issuer
+constexpr int T2_THREADS = 32 * (T2_GEN_WARPS + 6);
+constexpr int T2_COL_DACC = 0;                    // row-side accumulator [128 x 64] (TC_ACC_COLS)
+constexpr int T2_COL_MACC = 64;                   // column-side accumulator [128 x 64]
+constexpr int T2_COL_PSI = 128;                   // psi operand of the column side: 128 columns = (row % 64, part)
+constexpr int T2_COL_ASTAGE = 256;                // row-side A stages: [group][2] x 64 columns
+constexpr int T2_UNIT_COLS = 32;                  // columns per unit (two tiles)
+constexpr int T2_IMG = 128 * T2_UNIT_COLS * 8;    // one image (raw or lo) of a unit: 32 KB
+constexpr int T2_UNIT = 2 * T2_IMG;
+constexpr int T2_XCH = 4 * 32 * 32 * 4;           // epilogue exchange: [quadrant][column][lane] floats
+constexpr int T2_SMEM = 1024 + 2 * T2_UNIT + 4 * TC_STAGE + 2 * T2_XCH;
+
+struct T2Params {
+    GenArgs<float> G;
+    int32_t B, n_blk, k, slot_multi, slot_mcol0, S, n_items;
+    int64_t D;
+    const int32_t* pairs;   // (row block, column block) per pair
+    const float2* psi;
+    float2* work;
+};
+
+struct T2Bars {
+    uint64_t dfull[2][2], dempty[2][2];   // row-side stage of group g
+    uint64_t mfull[2], mempty[2];         // unit buffers
+    uint64_t macc_full, macc_empty;       // column-side accumulator
+    uint64_t psi_full;                    // psi operand of the item in TMEM
+    uint64_t ddone, dacc_empty;           // row-side accumulator
+};
+
+// K-major, SWIZZLE_128B: rows of 128 bytes (32 TF32), 8-row groups 1 KB apart.
+__device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t addr)
+{
+    return (uint64_t)((addr >> 4) & 0x3fffu) | (1ull << 16) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
+}
+
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32])
+{
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+          "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]),
+          "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]),
+          "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+        : "r"(taddr)
+        : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+
+// Generator group g (256 threads): tiles 2u + g of every unit u.  Row side exactly as tc_generate<+1>; column side:
+// the thread's 8 entries of row p go to the unit buffer as (Re, Im) pairs at
+//   [(p % 64) / 16] 8 KB  +  [p / 64] 4 KB  +  [column / 8] 1 KB  +  [column % 8] 128 B  +  16-byte chunk ((p % 16) / 2) ^ (column % 8)  +  (p % 2) 8 B
+// -- 16 lanes cover one 128-byte row, so the stores are conflict-free.
+__device__ __forceinline__ void t2_generate(const T2Params& P, unsigned char* ubuf, unsigned char* bimg, T2Bars& bar, uint32_t d_tmem)
+{
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int g = tid >> 8, lt = tid & 255;
+    const int p = lt & (TC_TP - 1), gsel = lt >> 7;
+    const uint32_t a_lane = d_tmem + ((uint32_t)(p & ~31) << 16);
+    const int v = lt & 15, qb = lt >> 4, k = P.k;
+    const int o_re = ((v & 7) * 16 + (v >> 3) * TC_SBO + (qb >> 2) * 128 + (qb & 3) * 4) / 4;
+    const int o_im = o_re + 2 * TC_SBO / 4;
+    const int n_units = P.B / T2_UNIT_COLS;
+    const uint32_t chunk = (uint32_t)(p & 15) >> 1;
+    const uint32_t m_row = (uint32_t)((p & 63) >> 4) * 8192u + (uint32_t)(p >> 6) * 4096u + (uint32_t)(p & 1) * 8u;
+    uint32_t gt = 0;   // tiles of this group so far = units so far
+    for (int item = blockIdx.x; item < P.n_items; item += gridDim.x) {
+        const int pr = item / P.S, strip = item - pr * P.S;
+        const int rb = P.pairs[2 * pr], cb = P.pairs[2 * pr + 1];
+        const uint32_t i = (uint32_t)rb * P.B + strip * TC_TP + p;
+        for (int u = 0; u < n_units; ++u, ++gt) {
+            const int s2 = gt & 1;
+            const uint32_t use = gt >> 1;
+            const uint32_t j0 = (uint32_t)cb * P.B + (2 * u + g) * TC_TQ;
+            const float2 x = (v < k && qb < TC_TQ) ? P.psi[(size_t)(j0 + qb) * k + v] : float2{0.f, 0.f};
+            float rh[TC_NG][4], rl[TC_NG][4], ih[TC_NG][4], il[TC_NG][4];
+#pragma unroll
+            for (int gg = 0; gg < TC_NG; ++gg)
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const uint32_t j = j0 + 4 * (gsel + 2 * gg) + e;
+                    float hr, hi;
+                    entry_upper<float>(P.G, nullptr, i, j, hr, hi);
+                    rh[gg][e] = hr;
+                    rl[gg][e] = hr - __uint_as_float(__float_as_uint(hr) & 0xffffe000u);
+                    ih[gg][e] = hi;
+                    il[gg][e] = hi - __uint_as_float(__float_as_uint(hi) & 0xffffe000u);
+                }
+            float prh, prl, pih, pil;
+            split_tf32(x.x, prh, prl);
+            split_tf32(x.y, pih, pil);
+            if (use > 0) mbar_wait(&bar.dempty[g][s2], (use - 1) & 1);   // row-side MMAs that read this stage are done
+            const int stg = 2 * g + s2;
+#pragma unroll
+            for (int gg = 0; gg < TC_NG; ++gg) {
+                const uint32_t ta = a_lane + (uint32_t)(T2_COL_ASTAGE + stg * TC_A_STAGE_COLS + 4 * (gsel + 2 * gg));
+                tmem_st4(ta + 0 * TC_TQ, rh[gg][0], rh[gg][1], rh[gg][2], rh[gg][3]);
+                tmem_st4(ta + 1 * TC_TQ, rl[gg][0], rl[gg][1], rl[gg][2], rl[gg][3]);
+                tmem_st4(ta + 2 * TC_TQ, ih[gg][0], ih[gg][1], ih[gg][2], ih[gg][3]);
+                tmem_st4(ta + 3 * TC_TQ, il[gg][0], il[gg][1], il[gg][2], il[gg][3]);
+            }
+            if (qb < TC_TQ) {
+                float* b = reinterpret_cast<float*>(bimg + stg * TC_STAGE);
+                constexpr int BT = TC_B_TILE / 4;
+                b[0 * BT + o_re] = prh;  b[0 * BT + o_im] = pih;
+                b[1 * BT + o_re] = prl;  b[1 * BT + o_im] = pil;
+                b[2 * BT + o_re] = -pih; b[2 * BT + o_im] = prh;
+                b[3 * BT + o_re] = -pil; b[3 * BT + o_im] = prl;
+            }
+            if (use > 0) mbar_wait(&bar.mempty[s2], (use - 1) & 1);      // column-side MMAs of the unit two back are done
+            unsigned char* ub = ubuf + s2 * T2_UNIT;
+#pragma unroll
+            for (int gg = 0; gg < TC_NG; ++gg)
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const uint32_t c8 = 4u * gsel + e;
+                    const uint32_t off = m_row + (uint32_t)(2 * g + gg) * 1024u + c8 * 128u + ((chunk ^ c8) << 4);
+                    *reinterpret_cast<float2*>(ub + off) = make_float2(rh[gg][e], ih[gg][e]);
+                    *reinterpret_cast<float2*>(ub + T2_IMG + off) = make_float2(rl[gg][e], il[gg][e]);
+                }
+            asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            __syncwarp();
+            if (lane == 0) {
+                mbar_arrive(&bar.dfull[g][s2]);
+                mbar_arrive(&bar.mfull[s2]);
+            }
+        }
+    }
+}
+
+// Row-side MMA warp: the one-sided kernel's 8 MMAs per tile, tiles in column order (group = tile parity).
+__device__ __forceinline__ void t2_row_mma(const T2Params& P, unsigned char* bimg, T2Bars& bar, uint32_t d_tmem)
+{
+    const int lane = threadIdx.x & 31;
+    const int n_tiles = P.B / TC_TQ, n_units = P.B / T2_UNIT_COLS;
+    uint32_t items_done = 0;
+    for (int item = blockIdx.x; item < P.n_items; item += gridDim.x, ++items_done) {
+        for (int t = 0; t < n_tiles; ++t) {
+            const int g = t & 1;
+            const uint32_t gt = items_done * n_units + (t >> 1);
+            const int s2 = gt & 1, stg = 2 * g + s2;
+            mbar_wait(&bar.dfull[g][s2], (gt >> 1) & 1);
+            if (t == 0 && items_done > 0) mbar_wait(&bar.dacc_empty, (items_done - 1) & 1);   // the epilogue has read the accumulator
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            if (elect_one()) {
+                const uint32_t b0 = smem_u32(bimg + stg * TC_STAGE);
+                const uint32_t a0 = d_tmem + (uint32_t)(T2_COL_ASTAGE + stg * TC_A_STAGE_COLS);
+#pragma unroll
+                for (int ks = 0; ks < TC_TQ / 8; ++ks) {
+                    const uint32_t ko = ks * 2 * TC_LBO;
+                    const uint32_t er_h = a0 + 0 * TC_TQ + 8 * ks, er_l = a0 + 1 * TC_TQ + 8 * ks;
+                    const uint32_t ei_h = a0 + 2 * TC_TQ + 8 * ks, ei_l = a0 + 3 * TC_TQ + 8 * ks;
+                    const uint64_t b1 = umma_desc(b0 + 0 * TC_B_TILE + ko);
+                    const uint64_t b2 = umma_desc(b0 + 2 * TC_B_TILE + ko);
+                    umma_tf32_ts<64>(d_tmem + T2_COL_DACC, er_h, b1, (t | ks) != 0);
+                    umma_tf32_ts<32>(d_tmem + T2_COL_DACC, er_l, b1, 1);
+                    umma_tf32_ts<64>(d_tmem + T2_COL_DACC, ei_h, b2, 1);
+                    umma_tf32_ts<32>(d_tmem + T2_COL_DACC, ei_l, b2, 1);
+                }
+                umma_commit(&bar.dempty[g][s2]);
+                if (t == n_tiles - 1) umma_commit(&bar.ddone);
+            }
+            __syncwarp();
+        }
+    }
+}
+
+// Column-side MMA warp: per unit 16 K-steps x (raw image, lo image), A = the item's psi operand in TMEM.
+__device__ __forceinline__ void t2_col_mma(const T2Params& P, unsigned char* ubuf, T2Bars& bar, uint32_t d_tmem)
+{
+    const int lane = threadIdx.x & 31;
+    const int n_units = P.B / T2_UNIT_COLS;
+    uint32_t gu = 0, items_done = 0;
+    for (int item = blockIdx.x; item < P.n_items; item += gridDim.x, ++items_done) {
+        mbar_wait(&bar.psi_full, items_done & 1);
+        for (int u = 0; u < n_units; ++u, ++gu) {
+            const int ub = gu & 1;
+            mbar_wait(&bar.mfull[ub], (gu >> 1) & 1);
+            if (gu > 0) mbar_wait(&bar.macc_empty, (gu - 1) & 1);
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            if (elect_one()) {
+                const uint32_t base = smem_u32(ubuf + ub * T2_UNIT);
+#pragma unroll
+                for (int img = 0; img < 2; ++img)
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) {
+                        const uint64_t b = umma_desc_sw128(base + img * T2_IMG + (j >> 2) * 8192 + (j & 3) * 32);
+                        umma_tf32_ts<64>(d_tmem + T2_COL_MACC, d_tmem + T2_COL_PSI + 8 * j, b, (img | j) != 0);
+                    }
+                umma_commit(&bar.mempty[ub]);
+                umma_commit(&bar.macc_full);
+            }
+            __syncwarp();
+        }
+    }
+}
+
+// Epilogue warps q = 0..3 (TMEM lanes 32q..): q = 2 (row half) + (0: hi image, 1: lo image); lane = op * 16 + v.
+__device__ __forceinline__ void t2_epilogue(const T2Params& P, float* xch, T2Bars& bar, uint32_t d_tmem)
+{
+    const int tid = threadIdx.x, lane = tid & 31, q = (tid >> 5) - T2_W_EPI;
+    const int h = q >> 1, lohi = q & 1, op = lane >> 4, v = lane & 15, k = P.k;
+    const int et = tid - 32 * T2_W_EPI;   // 0..127
+    const int n_units = P.B / T2_UNIT_COLS;
+    const uint32_t lane_base = d_tmem + ((uint32_t)(32 * q) << 16);
+    uint32_t gu = 0, items_done = 0;
+    for (int item = blockIdx.x; item < P.n_items; item += gridDim.x, ++items_done) {
+        const int pr = item / P.S, strip = item - pr * P.S;
+        const int rb = P.pairs[2 * pr], cb = P.pairs[2 * pr + 1];
+        const size_t row0 = (size_t)rb * P.B + (size_t)strip * TC_TP;
+        // psi operand of the item (every column-side MMA of the previous item has completed: its last macc_full was waited for)
+        const float2* src = P.psi + (row0 + 64 * h) * k + v;
+#pragma unroll 4
+        for (int r2 = 0; r2 < 32; ++r2) {
+            float2 x0 = float2{0.f, 0.f}, x1 = float2{0.f, 0.f};
+            if (v < k) {
+                x0 = src[(size_t)(2 * r2) * k];
+                x1 = src[(size_t)(2 * r2 + 1) * k];
+            }
+            float a0 = op ? x0.y : x0.x, a1 = op ? -x0.x : x0.y, a2 = op ? x1.y : x1.x, a3 = op ? -x1.x : x1.y;
+            if (lohi) {
+                a0 -= __uint_as_float(__float_as_uint(a0) & 0xffffe000u);
+                a1 -= __uint_as_float(__float_as_uint(a1) & 0xffffe000u);
+                a2 -= __uint_as_float(__float_as_uint(a2) & 0xffffe000u);
+                a3 -= __uint_as_float(__float_as_uint(a3) & 0xffffe000u);
+            }
+            tmem_st4(lane_base + (uint32_t)(T2_COL_PSI + 4 * r2), a0, a1, a2, a3);
+        }
+        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&bar.psi_full);
+        float2* out_col = P.work + ((size_t)(P.slot_mcol0 + rb * P.S + strip) * P.D + (size_t)cb * P.B) * k;
+        for (int u = 0; u < n_units; ++u, ++gu) {
+            mbar_wait(&bar.macc_full, gu & 1);
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            uint32_t r[32];
+            tmem_ld32(lane_base + (uint32_t)(T2_COL_MACC + 32 * h), r);
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&bar.macc_empty);
+            float* X = xch + (gu & 1) * (T2_XCH / 4);
+#pragma unroll
+            for (int c = 0; c < 32; ++c) X[(q * 32 + c) * 32 + lane] = __uint_as_float(r[c]);
+            asm volatile("bar.sync 1, 128;" ::: "memory");
+            const int vv = et & 15, cc = et >> 4;
+#pragma unroll
+            for (int i4 = 0; i4 < 4; ++i4) {
+                const int c = cc + 8 * i4;
+                float re = 0.f, im = 0.f;
+#pragma unroll
+                for (int qq = 0; qq < 4; ++qq) {
+                    re += X[(qq * 32 + c) * 32 + vv];
+                    im += X[(qq * 32 + c) * 32 + 16 + vv];
+                }
+                if (vv < k) out_col[(size_t)(u * T2_UNIT_COLS + c) * k + vv] = make_float2(re, im);
+            }
+        }
+        mbar_wait(&bar.ddone, items_done & 1);
+        tc_epilogue(d_tmem + T2_COL_DACC, q, P.work + ((size_t)(P.slot_multi + cb) * P.D + row0 + 32 * q + lane) * k, k);
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&bar.dacc_empty);
+    }
+}
+
+__global__ void __launch_bounds__(T2_THREADS, 1) proc_pairs_tc_kernel(const T2Params P)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw2_[];
+    __shared__ __align__(8) T2Bars bar;
+    __shared__ uint32_t s_tmem;
+    const int tid = threadIdx.x, w = tid >> 5;
+    unsigned char* ubuf = smem_raw2_ + ((1024u - (smem_u32(smem_raw2_) & 1023u)) & 1023u);   // 1 KB aligned (128-byte swizzle atoms)
+    unsigned char* bimg = ubuf + 2 * T2_UNIT;
+    float* xch = reinterpret_cast<float*>(bimg + 4 * TC_STAGE);
+    if (tid == 0) {
+        for (int g = 0; g < 2; ++g)
+            for (int s = 0; s < 2; ++s) {
+                mbar_init(&bar.dfull[g][s], T2_GEN_WARPS / 2);
+                mbar_init(&bar.dempty[g][s], 1);
+            }
+        for (int s = 0; s < 2; ++s) {
+            mbar_init(&bar.mfull[s], T2_GEN_WARPS);
+            mbar_init(&bar.mempty[s], 1);
+        }
+        mbar_init(&bar.macc_full, 1);
+        mbar_init(&bar.macc_empty, 4);
+        mbar_init(&bar.psi_full, 4);
+        mbar_init(&bar.ddone, 1);
+        mbar_init(&bar.dacc_empty, 4);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (w == T2_W_DMMA) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&s_tmem)), "n"(512) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    const uint32_t d_tmem = s_tmem;
+
+    if (w < T2_GEN_WARPS) t2_generate(P, ubuf, bimg, bar, d_tmem);
+    else if (w < T2_W_DMMA) t2_epilogue(P, xch, bar, d_tmem);
+    else if (w == T2_W_DMMA) t2_row_mma(P, bimg, bar, d_tmem);
+    else t2_col_mma(P, ubuf, bar, d_tmem);
+
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (w == T2_W_DMMA) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(d_tmem), "n"(512) : "memory");
+}
+
+bool tc_pairs_supported(int dtype, int k, int B, int part_world)
+{
+    return dtype == MFH_C64 && k > 1 && k <= 16 && B % TC_TP == 0 && part_world <= 1;
+}
+
+static int launch_proc_pairs_tc(mfh_handle h, const void* psi, cudaStream_t st)
+{
+    const Plan& p = h->plan;
+    T2Params P;
+    P.G.K = make_philox_keys(h->seed);
+    P.G.gc.neg_k2_ln2 = (float)(-0.6931471805599453 / (double)h->D);
+    P.G.tab_global = nullptr;
+    P.B = p.B;
+    P.n_blk = p.n_blk;
+    P.k = p.k;
+    P.slot_multi = p.slot_multi;
+    P.slot_mcol0 = p.slot_mcol0;
+    P.S = p.B / TC_TP;
+    P.n_items = (int32_t)(p.tc_pairs.size() / 2) * P.S;
+    P.D = h->D;
+    P.pairs = h->d_tc_pairs;
+    P.psi = (const float2*)psi;
+    P.work = (float2*)h->d_work;
+    if (int rc = ensure_dyn_smem(h, proc_pairs_tc_kernel, T2_SMEM)) return rc;
+    proc_pairs_tc_kernel<<<std::min(P.n_items, h->sm_count), T2_THREADS, T2_SMEM, st>>>(P);
+    MFH_CUDA_CHECK(cudaGetLastError());
+    return MFH_OK;
+}
+
 bool tc_multi_supported(mfh_handle h)
 {
     // seeded source only: the generator warps of this kernel are the Philox / SFU Box-Muller path
@@ -321,8 +710,13 @@ int launch_proc_multi_tc(mfh_handle h, const void* psi, cudaStream_t st)
     P.slot_multi = p.slot_multi;
     P.D = h->D;
     P.cache_slot = h->d_cache_slot;
+    P.skip = p.tc_pairs.empty() ? nullptr : h->d_tc_skip;
     P.psi = (const float2*)psi;
     P.work = (float2*)h->d_work;
+    if (!p.tc_pairs.empty())   // block pairs generated once for both sides
+        if (int rc = launch_proc_pairs_tc(h, psi, st)) return rc;
+    // what is left for the one-sided kernel: diagonal blocks and positions whose mirror image is cached
+    if (p.owned_blocks - p.covered_blocks - (int64_t)p.tc_pairs.size() <= 0) return MFH_OK;
     const size_t smem = (size_t)TC_STAGES * TC_STAGE;
     if (int rc = ensure_dyn_smem(h, proc_multi_tc_kernel, (int)smem)) return rc;
     proc_multi_tc_kernel<<<dim3((unsigned)(h->D / TC_TP), p.n_blk), TC_THREADS, smem, st>>>(P);
@@ -473,7 +867,7 @@ __global__ void __launch_bounds__(CT_THREADS, 2) cached_multi_tc_kernel(const Ct
             const int s = t % CT_TSTAGES, u = t / CT_TSTAGES;
             mbar_wait(&a_full[s], u & 1);
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-            if (lane == 0) {
+            if (elect_one()) {
                 const uint32_t b0 = smem_u32(bimg + s * CT_BSTAGE);
                 const uint32_t a0 = d_tmem + (uint32_t)(TC_ACC_COLS + s * CT_A_STAGE_COLS);
 #pragma unroll
