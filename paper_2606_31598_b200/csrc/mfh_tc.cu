@@ -137,10 +137,9 @@ __device__ __forceinline__ void split_tf32(float x, float& hi, float& lo)
 
 // Epilogue of warp w < 4: TMEM lanes 32w..32w+31 hold rows 32w + lane of the [128 x 32] accumulator
 // (columns 0..15 real parts, 16..31 imaginary parts of the k vectors); dst = this row's k outputs.
-__device__ __forceinline__ void tc_epilogue(uint32_t d_tmem, int w, float2* dst, int k)
+__device__ __forceinline__ void tc_epilogue_load(uint32_t d_tmem, int w, float (&acc)[32])
 {
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
-    float acc[32];
 #pragma unroll
     for (int half = 0; half < 2; ++half) {   // columns [0,32): A_hi B_hi + A_lo B_hi;  [32,64): A_hi B_lo
         uint32_t r[32];
@@ -159,9 +158,18 @@ __device__ __forceinline__ void tc_epilogue(uint32_t d_tmem, int w, float2* dst,
 #pragma unroll
         for (int c = 0; c < 32; ++c) acc[c] = half ? acc[c] + __uint_as_float(r[c]) : __uint_as_float(r[c]);
     }
+}
+__device__ __forceinline__ void tc_epilogue_store(const float (&acc)[32], float2* dst, int k)
+{
 #pragma unroll
     for (int vv = 0; vv < 16; ++vv)
         if (vv < k) dst[vv] = make_float2(acc[vv], acc[16 + vv]);
+}
+__device__ __forceinline__ void tc_epilogue(uint32_t d_tmem, int w, float2* dst, int k)
+{
+    float acc[32];
+    tc_epilogue_load(d_tmem, w, acc);
+    tc_epilogue_store(acc, dst, k);
 }
 
 struct TcParams {
@@ -347,18 +355,24 @@ __global__ void __launch_bounds__(TC_THREADS, 2) proc_multi_tc_kernel(const TcPa
 // --------------------------------------------------------------------------------------------
 constexpr int T2_GEN_WARPS = 16;
 constexpr int T2_W_EPI = T2_GEN_WARPS;            // warps 16..19: TMEM lane quadrants 0..3
-constexpr int T2_W_DMMA = T2_GEN_WARPS + 4;       // row-side MMA issuer (allocates TMEM)
-constexpr int T2_W_MMMA = T2_GEN_WARPS + 5;       // column-side MMA issuer
-constexpr int T2_THREADS = 32 * (T2_GEN_WARPS + 6);
+// Warp w runs on scheduler w % 4.  The MMA issuers sit on schedulers 2 and 3; two more warps on schedulers 0 and 1, fed
+// through shared memory, do the cross-quadrant sums and the stores of the column side.  That keeps the epilogue warps'
+// loop short (the column-side MMA warp waits for them before every unit: measured 17 % of its time when they also
+// summed and stored) and spreads the helper instructions over the four schedulers (a generator warp on a busier
+// scheduler makes the other 15 wait at every unit).
+constexpr int T2_W_SUM = T2_GEN_WARPS + 4;        // warps 20, 21: cross-quadrant sums and stores of the column side
+constexpr int T2_W_DMMA = T2_GEN_WARPS + 6;       // row-side MMA issuer (allocates TMEM)
+constexpr int T2_W_MMMA = T2_GEN_WARPS + 7;       // column-side MMA issuer
+constexpr int T2_THREADS = 32 * (T2_GEN_WARPS + 8);
 constexpr int T2_COL_DACC = 0;                    // row-side accumulator [128 x 64] (TC_ACC_COLS)
 constexpr int T2_COL_MACC = 64;                   // column-side accumulator [128 x 64]
-constexpr int T2_COL_PSI = 128;                   // psi operand of the column side: 128 columns = (row % 64, part)
-constexpr int T2_COL_ASTAGE = 256;                // row-side A stages: [group][2] x 64 columns
+constexpr int T2_COL_PSI = 128;                   // psi operand of the column side, two buffers (item parity) of 128 columns = (row % 64, part)
+constexpr int T2_COL_ASTAGE = 384;                // row-side A stage of each group: 64 columns
 constexpr int T2_UNIT_COLS = 32;                  // columns per unit (two tiles)
 constexpr int T2_IMG = 128 * T2_UNIT_COLS * 8;    // one image (raw or lo) of a unit: 32 KB
 constexpr int T2_UNIT = 2 * T2_IMG;
 constexpr int T2_XCH = 4 * 32 * 32 * 4;           // epilogue exchange: [quadrant][column][lane] floats
-constexpr int T2_SMEM = 1024 + 2 * T2_UNIT + 4 * TC_STAGE + 2 * T2_XCH;
+constexpr int T2_SMEM = 1024 + 2 * T2_UNIT + 2 * TC_STAGE + 2 * T2_XCH;
 
 struct T2Params {
     GenArgs<float> G;
@@ -370,7 +384,7 @@ struct T2Params {
 };
 
 struct T2Bars {
-    uint64_t dfull[2][2], dempty[2][2];   // row-side stage of group g
+    uint64_t dfull[2], dempty[2];         // row-side stage of group g
     uint64_t mfull[2], mempty[2];         // unit buffers
     uint64_t macc_full, macc_empty;       // column-side accumulator
     uint64_t psi_full;                    // psi operand of the item in TMEM
@@ -440,8 +454,20 @@ __device__ __forceinline__ void t2_generate(const T2Params& P, unsigned char* ub
             float prh, prl, pih, pil;
             split_tf32(x.x, prh, prl);
             split_tf32(x.y, pih, pil);
-            if (use > 0) mbar_wait(&bar.dempty[g][s2], (use - 1) & 1);   // row-side MMAs that read this stage are done
-            const int stg = 2 * g + s2;
+            if (use > 0) mbar_wait(&bar.mempty[s2], (use - 1) & 1);      // column-side MMAs of the unit two back are done
+            unsigned char* ub = ubuf + s2 * T2_UNIT;
+#pragma unroll
+            for (int gg = 0; gg < TC_NG; ++gg)
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const uint32_t c8 = 4u * gsel + e;
+                    const uint32_t off = m_row + (uint32_t)(2 * g + gg) * 1024u + c8 * 128u + ((chunk ^ c8) << 4);
+                    *reinterpret_cast<float2*>(ub + off) = make_float2(rh[gg][e], ih[gg][e]);
+                    *reinterpret_cast<float2*>(ub + T2_IMG + off) = make_float2(rl[gg][e], il[gg][e]);
+                }
+            // (the row side second: the MMAs of this group's previous tile finish during the stores above)
+            if (gt > 0) mbar_wait(&bar.dempty[g], (gt - 1) & 1);   // the row-side MMAs of this group's previous tile are done
+            const int stg = g;
 #pragma unroll
             for (int gg = 0; gg < TC_NG; ++gg) {
                 const uint32_t ta = a_lane + (uint32_t)(T2_COL_ASTAGE + stg * TC_A_STAGE_COLS + 4 * (gsel + 2 * gg));
@@ -458,23 +484,12 @@ __device__ __forceinline__ void t2_generate(const T2Params& P, unsigned char* ub
                 b[2 * BT + o_re] = -pih; b[2 * BT + o_im] = prh;
                 b[3 * BT + o_re] = -pil; b[3 * BT + o_im] = prl;
             }
-            if (use > 0) mbar_wait(&bar.mempty[s2], (use - 1) & 1);      // column-side MMAs of the unit two back are done
-            unsigned char* ub = ubuf + s2 * T2_UNIT;
-#pragma unroll
-            for (int gg = 0; gg < TC_NG; ++gg)
-#pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                    const uint32_t c8 = 4u * gsel + e;
-                    const uint32_t off = m_row + (uint32_t)(2 * g + gg) * 1024u + c8 * 128u + ((chunk ^ c8) << 4);
-                    *reinterpret_cast<float2*>(ub + off) = make_float2(rh[gg][e], ih[gg][e]);
-                    *reinterpret_cast<float2*>(ub + T2_IMG + off) = make_float2(rl[gg][e], il[gg][e]);
-                }
             asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
             __syncwarp();
             if (lane == 0) {
-                mbar_arrive(&bar.dfull[g][s2]);
+                mbar_arrive(&bar.dfull[g]);
                 mbar_arrive(&bar.mfull[s2]);
             }
         }
@@ -491,26 +506,26 @@ __device__ __forceinline__ void t2_row_mma(const T2Params& P, unsigned char* bim
         for (int t = 0; t < n_tiles; ++t) {
             const int g = t & 1;
             const uint32_t gt = items_done * n_units + (t >> 1);
-            const int s2 = gt & 1, stg = 2 * g + s2;
-            mbar_wait(&bar.dfull[g][s2], (gt >> 1) & 1);
+            const int stg = g;
+            mbar_wait(&bar.dfull[g], gt & 1);
             if (t == 0 && items_done > 0) mbar_wait(&bar.dacc_empty, (items_done - 1) & 1);   // the epilogue has read the accumulator
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             if (elect_one()) {
-                const uint32_t b0 = smem_u32(bimg + stg * TC_STAGE);
+                const uint64_t bd = umma_desc(smem_u32(bimg + stg * TC_STAGE));   // the start-address field takes plain additions
                 const uint32_t a0 = d_tmem + (uint32_t)(T2_COL_ASTAGE + stg * TC_A_STAGE_COLS);
 #pragma unroll
                 for (int ks = 0; ks < TC_TQ / 8; ++ks) {
                     const uint32_t ko = ks * 2 * TC_LBO;
                     const uint32_t er_h = a0 + 0 * TC_TQ + 8 * ks, er_l = a0 + 1 * TC_TQ + 8 * ks;
                     const uint32_t ei_h = a0 + 2 * TC_TQ + 8 * ks, ei_l = a0 + 3 * TC_TQ + 8 * ks;
-                    const uint64_t b1 = umma_desc(b0 + 0 * TC_B_TILE + ko);
-                    const uint64_t b2 = umma_desc(b0 + 2 * TC_B_TILE + ko);
+                    const uint64_t b1 = bd + (uint64_t)((0 * TC_B_TILE + ko) >> 4);
+                    const uint64_t b2 = bd + (uint64_t)((2 * TC_B_TILE + ko) >> 4);
                     umma_tf32_ts<64>(d_tmem + T2_COL_DACC, er_h, b1, (t | ks) != 0);
                     umma_tf32_ts<32>(d_tmem + T2_COL_DACC, er_l, b1, 1);
                     umma_tf32_ts<64>(d_tmem + T2_COL_DACC, ei_h, b2, 1);
                     umma_tf32_ts<32>(d_tmem + T2_COL_DACC, ei_l, b2, 1);
                 }
-                umma_commit(&bar.dempty[g][s2]);
+                umma_commit(&bar.dempty[g]);
                 if (t == n_tiles - 1) umma_commit(&bar.ddone);
             }
             __syncwarp();
@@ -532,13 +547,14 @@ __device__ __forceinline__ void t2_col_mma(const T2Params& P, unsigned char* ubu
             if (gu > 0) mbar_wait(&bar.macc_empty, (gu - 1) & 1);
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             if (elect_one()) {
-                const uint32_t base = smem_u32(ubuf + ub * T2_UNIT);
+                const uint64_t bd = umma_desc_sw128(smem_u32(ubuf + ub * T2_UNIT));
+                const uint32_t a0 = d_tmem + (uint32_t)(T2_COL_PSI + 128 * (items_done & 1));
 #pragma unroll
                 for (int img = 0; img < 2; ++img)
 #pragma unroll
                     for (int j = 0; j < 16; ++j) {
-                        const uint64_t b = umma_desc_sw128(base + img * T2_IMG + (j >> 2) * 8192 + (j & 3) * 32);
-                        umma_tf32_ts<64>(d_tmem + T2_COL_MACC, d_tmem + T2_COL_PSI + 8 * j, b, (img | j) != 0);
+                        const uint64_t b = bd + (uint64_t)((img * T2_IMG + (j >> 2) * 8192 + (j & 3) * 32) >> 4);
+                        umma_tf32_ts<64>(d_tmem + T2_COL_MACC, a0 + 8 * j, b, (img | j) != 0);
                     }
                 umma_commit(&bar.mempty[ub]);
                 umma_commit(&bar.macc_full);
@@ -549,22 +565,21 @@ __device__ __forceinline__ void t2_col_mma(const T2Params& P, unsigned char* ubu
 }
 
 // Epilogue warps q = 0..3 (TMEM lanes 32q..): q = 2 (row half) + (0: hi image, 1: lo image); lane = op * 16 + v.
+// They also build the psi operand of the NEXT item into the other TMEM buffer, a few rows per unit, so that neither
+// MMA warp waits at an item boundary, and they free the row-side accumulator before they store what they read.
 __device__ __forceinline__ void t2_epilogue(const T2Params& P, float* xch, T2Bars& bar, uint32_t d_tmem)
 {
     const int tid = threadIdx.x, lane = tid & 31, q = (tid >> 5) - T2_W_EPI;
     const int h = q >> 1, lohi = q & 1, op = lane >> 4, v = lane & 15, k = P.k;
-    const int et = tid - 32 * T2_W_EPI;   // 0..127
     const int n_units = P.B / T2_UNIT_COLS;
+    const int per = (32 + n_units - 2) / (n_units - 1);   // row pairs of the next psi operand built per unit (n_units >= 4)
     const uint32_t lane_base = d_tmem + ((uint32_t)(32 * q) << 16);
-    uint32_t gu = 0, items_done = 0;
-    for (int item = blockIdx.x; item < P.n_items; item += gridDim.x, ++items_done) {
+    // row pairs [r2a, r2b) of the psi operand of `item` into buffer `buf`
+    auto psi_rows = [&](int item, int buf, int r2a, int r2b) {
         const int pr = item / P.S, strip = item - pr * P.S;
-        const int rb = P.pairs[2 * pr], cb = P.pairs[2 * pr + 1];
-        const size_t row0 = (size_t)rb * P.B + (size_t)strip * TC_TP;
-        // psi operand of the item (every column-side MMA of the previous item has completed: its last macc_full was waited for)
-        const float2* src = P.psi + (row0 + 64 * h) * k + v;
+        const float2* src = P.psi + ((size_t)P.pairs[2 * pr] * P.B + (size_t)strip * TC_TP + 64 * h) * k + v;
 #pragma unroll 4
-        for (int r2 = 0; r2 < 32; ++r2) {
+        for (int r2 = r2a; r2 < r2b; ++r2) {
             float2 x0 = float2{0.f, 0.f}, x1 = float2{0.f, 0.f};
             if (v < k) {
                 x0 = src[(size_t)(2 * r2) * k];
@@ -577,13 +592,25 @@ __device__ __forceinline__ void t2_epilogue(const T2Params& P, float* xch, T2Bar
                 a2 -= __uint_as_float(__float_as_uint(a2) & 0xffffe000u);
                 a3 -= __uint_as_float(__float_as_uint(a3) & 0xffffe000u);
             }
-            tmem_st4(lane_base + (uint32_t)(T2_COL_PSI + 4 * r2), a0, a1, a2, a3);
+            tmem_st4(lane_base + (uint32_t)(T2_COL_PSI + 128 * buf + 4 * r2), a0, a1, a2, a3);
         }
+    };
+    auto psi_publish = [&]() {
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         __syncwarp();
         if (lane == 0) mbar_arrive(&bar.psi_full);
-        float2* out_col = P.work + ((size_t)(P.slot_mcol0 + rb * P.S + strip) * P.D + (size_t)cb * P.B) * k;
+    };
+    if ((int)blockIdx.x < P.n_items) {
+        psi_rows(blockIdx.x, 0, 0, 32);
+        psi_publish();
+    }
+    uint32_t gu = 0, items_done = 0;
+    for (int item = blockIdx.x; item < P.n_items; item += gridDim.x, ++items_done) {
+        const int pr = item / P.S, strip = item - pr * P.S;
+        const int rb = P.pairs[2 * pr], cb = P.pairs[2 * pr + 1];
+        const size_t row0 = (size_t)rb * P.B + (size_t)strip * TC_TP;
+        const int next = item + gridDim.x;
         for (int u = 0; u < n_units; ++u, ++gu) {
             mbar_wait(&bar.macc_full, gu & 1);
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
@@ -592,28 +619,60 @@ __device__ __forceinline__ void t2_epilogue(const T2Params& P, float* xch, T2Bar
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
             __syncwarp();
             if (lane == 0) mbar_arrive(&bar.macc_empty);
-            float* X = xch + (gu & 1) * (T2_XCH / 4);
+            // hand the quadrant piece to the sum warps: named barriers 1 + b (buffer b full) and 3 + b (buffer b read)
+            const int xb = gu & 1;
+            float* X = xch + xb * (T2_XCH / 4);
+            if (gu >= 2) asm volatile("bar.sync %0, 192;" ::"r"(3 + xb) : "memory");
 #pragma unroll
             for (int c = 0; c < 32; ++c) X[(q * 32 + c) * 32 + lane] = __uint_as_float(r[c]);
-            asm volatile("bar.sync 1, 128;" ::: "memory");
-            const int vv = et & 15, cc = et >> 4;
-#pragma unroll
-            for (int i4 = 0; i4 < 4; ++i4) {
-                const int c = cc + 8 * i4;
-                float re = 0.f, im = 0.f;
-#pragma unroll
-                for (int qq = 0; qq < 4; ++qq) {
-                    re += X[(qq * 32 + c) * 32 + vv];
-                    im += X[(qq * 32 + c) * 32 + 16 + vv];
-                }
-                if (vv < k) out_col[(size_t)(u * T2_UNIT_COLS + c) * k + vv] = make_float2(re, im);
+            asm volatile("bar.arrive %0, 192;" ::"r"(1 + xb) : "memory");
+            // the column-side MMA warp has passed its wait for THIS item's operand (its unit 0 is complete), so the
+            // next arrival on psi_full cannot overtake it; the other buffer's readers (previous item) are done
+            if (next < P.n_items && u * per < 32) {
+                psi_rows(next, (items_done + 1) & 1, u * per, min(32, (u + 1) * per));
+                if ((u + 1) * per >= 32) psi_publish();
             }
         }
         mbar_wait(&bar.ddone, items_done & 1);
-        tc_epilogue(d_tmem + T2_COL_DACC, q, P.work + ((size_t)(P.slot_multi + cb) * P.D + row0 + 32 * q + lane) * k, k);
+        float acc[32];
+        tc_epilogue_load(d_tmem + T2_COL_DACC, q, acc);
         asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
         __syncwarp();
-        if (lane == 0) mbar_arrive(&bar.dacc_empty);
+        if (lane == 0) mbar_arrive(&bar.dacc_empty);   // the next item's row-side MMAs may start
+        tc_epilogue_store(acc, P.work + ((size_t)(P.slot_multi + cb) * P.D + row0 + 32 * q + lane) * k, k);
+    }
+}
+
+// Sum warps (64 threads): out[c][v] = sum over the four quadrant pieces (row halves x hi/lo images), thread = (v, c % 4).
+__device__ __forceinline__ void t2_col_sums(const T2Params& P, const float* xch)
+{
+    const int et = threadIdx.x - 32 * T2_W_SUM, vv = et & 15, cc = et >> 4, k = P.k;
+    const int n_units = P.B / T2_UNIT_COLS;
+    uint32_t gu = 0;
+    for (int item = blockIdx.x; item < P.n_items; item += gridDim.x) {
+        const int pr = item / P.S, strip = item - pr * P.S;
+        const int rb = P.pairs[2 * pr], cb = P.pairs[2 * pr + 1];
+        float2* out_col = P.work + ((size_t)(P.slot_mcol0 + rb * P.S + strip) * P.D + (size_t)cb * P.B) * k;
+        for (int u = 0; u < n_units; ++u, ++gu) {
+            const int xb = gu & 1;
+            const float* X = xch + xb * (T2_XCH / 4);
+            asm volatile("bar.sync %0, 192;" ::"r"(1 + xb) : "memory");
+            float re[8], im[8];
+#pragma unroll
+            for (int i8 = 0; i8 < 8; ++i8) {
+                const int c = cc + 4 * i8;
+                re[i8] = im[i8] = 0.f;
+#pragma unroll
+                for (int qq = 0; qq < 4; ++qq) {
+                    re[i8] += X[(qq * 32 + c) * 32 + vv];
+                    im[i8] += X[(qq * 32 + c) * 32 + 16 + vv];
+                }
+            }
+            asm volatile("bar.arrive %0, 192;" ::"r"(3 + xb) : "memory");   // the buffer may be overwritten
+#pragma unroll
+            for (int i8 = 0; i8 < 8; ++i8)
+                if (vv < k) out_col[(size_t)(u * T2_UNIT_COLS + cc + 4 * i8) * k + vv] = make_float2(re[i8], im[i8]);
+        }
     }
 }
 
@@ -625,13 +684,12 @@ __global__ void __launch_bounds__(T2_THREADS, 1) proc_pairs_tc_kernel(const T2Pa
     const int tid = threadIdx.x, w = tid >> 5;
     unsigned char* ubuf = smem_raw2_ + ((1024u - (smem_u32(smem_raw2_) & 1023u)) & 1023u);   // 1 KB aligned (128-byte swizzle atoms)
     unsigned char* bimg = ubuf + 2 * T2_UNIT;
-    float* xch = reinterpret_cast<float*>(bimg + 4 * TC_STAGE);
+    float* xch = reinterpret_cast<float*>(bimg + 2 * TC_STAGE);
     if (tid == 0) {
-        for (int g = 0; g < 2; ++g)
-            for (int s = 0; s < 2; ++s) {
-                mbar_init(&bar.dfull[g][s], T2_GEN_WARPS / 2);
-                mbar_init(&bar.dempty[g][s], 1);
-            }
+        for (int g = 0; g < 2; ++g) {
+            mbar_init(&bar.dfull[g], T2_GEN_WARPS / 2);
+            mbar_init(&bar.dempty[g], 1);
+        }
         for (int s = 0; s < 2; ++s) {
             mbar_init(&bar.mfull[s], T2_GEN_WARPS);
             mbar_init(&bar.mempty[s], 1);
@@ -653,9 +711,10 @@ __global__ void __launch_bounds__(T2_THREADS, 1) proc_pairs_tc_kernel(const T2Pa
     const uint32_t d_tmem = s_tmem;
 
     if (w < T2_GEN_WARPS) t2_generate(P, ubuf, bimg, bar, d_tmem);
-    else if (w < T2_W_DMMA) t2_epilogue(P, xch, bar, d_tmem);
+    else if (w < T2_W_EPI + 4) t2_epilogue(P, xch, bar, d_tmem);
+    else if (w < T2_W_SUM + 2) t2_col_sums(P, xch);
     else if (w == T2_W_DMMA) t2_row_mma(P, bimg, bar, d_tmem);
-    else t2_col_mma(P, ubuf, bar, d_tmem);
+    else if (w == T2_W_MMMA) t2_col_mma(P, ubuf, bar, d_tmem);
 
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
