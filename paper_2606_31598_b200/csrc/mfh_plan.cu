@@ -285,6 +285,7 @@ void build_tables(Plan& p, int64_t D, int dtype, int sm_count)
     for (size_t q = 0; q + 1 < p.tc_pairs.size(); q += 2) {
         const int n = p.tc_pairs[q], m = p.tc_pairs[q + 1];
         p.tc_skip[(size_t)n * N + m] = p.tc_skip[(size_t)m * N + n] = 1;
+        valid(m, p.slot_multi + n) = 0;   // position (m, n) arrives through the column-side slots instead
         for (int t = 0; t < tcS; ++t) valid(m, p.slot_mcol0 + n * tcS + t) = 1;
     }
     const int strip = p.B / p.Q;
