@@ -44,6 +44,19 @@ __host__ __device__ inline size_t tiled_cache_offset(int B, int a, int b)
     return ((size_t)rt * (B >> 4) + kt) * 4096 + (size_t)r * 32 + (size_t)((c ^ (r & 7)) << 2) + (size_t)((b & 1) << 1);
 }
 
+// Unit-image layout of the off-diagonal blocks of a complex64 k-vector PAIR cache (two-sided cached kernel,
+// mfh_tc.cu): element (a, b) of a B x B block, in BYTES from the block start.  A unit = 128 rows x 32 columns = 32 KB
+// contiguous (one bulk copy), units ordered column range fastest inside a 128-row strip.  Inside a unit the image is
+// the K-major, 128-byte-swizzled shared-memory B operand of the column side (row = block column, K = (block row,
+// re/im)): [(r % 64) / 16] 8 KB, [r / 64] 4 KB, [c / 8] 1 KB, [c % 8] 128 B, 16-byte chunk ((r % 16) / 2) ^ (c % 8),
+// [r % 2] 8 B -- exactly what the generator threads of pairs_tc_kernel write for a generated unit.
+__host__ __device__ inline size_t unit_image_offset(int B, int a, int b)
+{
+    const int strip = a >> 7, r = a & 127, u = b >> 5, c = b & 31;
+    return ((size_t)strip * (B >> 5) + u) * 32768 + (size_t)((r & 63) >> 4) * 8192 + (size_t)(r >> 6) * 4096 + (size_t)(c >> 3) * 1024 +
+           (size_t)(c & 7) * 128 + (size_t)((((r & 15) >> 1) ^ (c & 7)) << 4) + (size_t)(r & 1) * 8;
+}
+
 // Strip-tiled cache layout of one-vector PARTIAL plans (the streaming role of partial_overlap_kernel, mfh_proc.cu):
 // element (a, b) of a B x B block, in complex elements from the block start.  A tile is 8 rows x `cols` columns
 // (cols = STRIP_PIECE_BYTES of complex: 64 complex128 / 128 complex64), 8 KB contiguous, tiles ordered column chunk
@@ -63,13 +76,16 @@ struct Plan {
     int32_t stream_sms = 0;    // partial plans: SMs whose CTAs stream cached blocks while the others generate (Eq. 33)
     bool pairs = false;        // Hermitian pair cache: store block (n,m), n <= m, use it for both sides
     bool strip_tiled = false;  // cached blocks stored in the strip-tiled layout (partial plans run by partial_overlap_kernel)
+    bool pair_units = false;   // complex64 k-vector pair cache: off-diagonal stored blocks in the unit-image layout, served
+                               // for both sides from ONE read by cached_pairs_tc_kernel
     int64_t n_cached = 0;      // stored blocks
     int64_t covered_blocks = 0;   // block positions (n,m) served from the cache
     int32_t cached_per_row = 0;
     int32_t n_slots = 0;       // partial vectors in the workspace
     int32_t slot_cache = -1, slot_row0 = -1, slot_col0 = -1, slot_multi = -1;
     int32_t slot_mcol0 = -1;   // k-vector two-sided generator (mfh_tc.cu): column-side slots, one per (row block, 128-row strip)
-    bool allow_tc_pairs = true;   // caller: the source is seeded (the two-sided tensor-core generator is the Philox path)
+    bool allow_tc_pairs = true;   // caller: the column-side slots of the two-sided k-vector kernels fit the budget
+    bool gen_two_sided = true;    // caller: the source is seeded (the two-sided tensor-core GENERATOR is the Philox path)
     size_t cache_bytes = 0, work_bytes = 0;
     int32_t part_rank = 0, part_world = 1, part_scheme = 0;   // mfh_set_partition
     int64_t owned_blocks = 0;     // block positions this rank is responsible for (n_blk^2 on one GPU)
@@ -80,7 +96,8 @@ struct Plan {
     std::vector<ProcItem> items;       // fused generate-and-apply kernel
     std::vector<ProcItem> pair_items;  // cached pair kernel (pairs mode)
     std::vector<int32_t> tc_pairs;     // k-vector two-sided generator: (row block, column block) of every pair it serves
-    std::vector<uint8_t> tc_skip;      // [n_blk*n_blk] 1 = position served by the two-sided generator (one-sided kernel skips it)
+    std::vector<uint8_t> tc_skip;      // [n_blk*n_blk] 1 = position served by a two-sided kernel (the one-sided kernels skip it)
+    std::vector<int32_t> tc_cpairs;    // two-sided cached kernel: (row block, column block, cache slot) of every stored pair
     std::vector<uint8_t> slot_valid;   // [n_blk][n_slots]
     std::string json;
 };
@@ -111,6 +128,7 @@ struct mfh_handle_s {
     mfh::ProcItem* d_pair_items = nullptr;
     int32_t* d_tc_pairs = nullptr;    // plan.tc_pairs
     uint8_t* d_tc_skip = nullptr;     // plan.tc_skip
+    int32_t* d_tc_cpairs = nullptr;   // plan.tc_cpairs
     int32_t* d_slot_list = nullptr;   // [n_blk][n_slots+1]: count | flags, then the valid slots in ascending order
     double* d_lambdas = nullptr;    // MFH_MAX_K doubles, refreshed by every apply
     int32_t* d_counter = nullptr;   // dynamic work counters: [0] procedural kernel, [1] pair kernel, [2] CTAs finished,
@@ -172,7 +190,6 @@ int launch_philox_debug(uint64_t seed, uint32_t stream_id, const uint32_t* i, co
                         int64_t n, uint32_t* words, cudaStream_t st);
 int launch_fill_block(mfh_handle h, int32_t B, int32_t n, int32_t m, void* out, cudaStream_t st);
 int launch_fill_cache(mfh_handle h, cudaStream_t st);
-int launch_store_block(mfh_handle h, int32_t slot, const void* src_dev, cudaStream_t st);   // external block -> cache slot
 int launch_h0(mfh_handle h, void* out, cudaStream_t st);
 int launch_proc_single(mfh_handle h, const void* psi, void* phi, double lambda, cudaStream_t st);
 bool partial_overlap_supported(mfh_handle h);
@@ -184,6 +201,8 @@ bool tc_pairs_supported(int dtype, int k, int B, int part_world);        // two-
 bool tc_cached_multi_supported(int dtype, int k, int B);
 bool cached_multi_c128_supported(int dtype, int k, int B);               // mfh_cached.cu
 int launch_cached_multi_tc(mfh_handle h, const void* psi, cudaStream_t st);
+int launch_cached_pairs_tc(mfh_handle h, const void* psi, cudaStream_t st);
+int launch_store_block_at(mfh_handle h, int32_t slot, int32_t n, int32_t m, const void* src_dev, cudaStream_t st);
 int launch_cached(mfh_handle h, const void* psi, cudaStream_t st);
 int launch_cached_pairs(mfh_handle h, const void* psi, cudaStream_t st);
 int launch_reduce(mfh_handle h, const void* psi, void* phi, const double* lambdas_host, cudaStream_t st);

@@ -258,17 +258,26 @@ void build_tables(Plan& p, int64_t D, int dtype, int sm_count)
     // k-vector two-sided generator (complex64, mfh_tc.cu): a block pair whose two positions are both generated is
     // generated ONCE; its column side gets one slot per (row block, 128-row strip), like the one-vector kernel's
     p.tc_pairs.clear();
+    p.tc_cpairs.clear();
     p.tc_skip.clear();
     p.slot_mcol0 = -1;
+    p.pair_units = false;
     const int tcS = p.B / 128;
     if (p.allow_tc_pairs && tc_pairs_supported(dtype, p.k, p.B, part.world)) {
         for (int n = 0; n < N; ++n)
-            for (int m = n + 1; m < N; ++m)
-                if (uncached(n, m) && uncached(m, n)) {
+            for (int m = n + 1; m < N; ++m) {
+                if (p.gen_two_sided && uncached(n, m) && uncached(m, n)) {
                     p.tc_pairs.push_back(n);
                     p.tc_pairs.push_back(m);
+                } else if (p.pairs && p.cache_slot[(size_t)n * N + m] >= 0 && p.cache_slot[(size_t)m * N + n] == -2) {
+                    // stored pair: unit-image layout, both positions from one read (pairs_tc_kernel<true>)
+                    p.tc_cpairs.push_back(n);
+                    p.tc_cpairs.push_back(m);
+                    p.tc_cpairs.push_back(p.cache_slot[(size_t)n * N + m]);
                 }
-        if (!p.tc_pairs.empty()) {
+            }
+        p.pair_units = !p.tc_cpairs.empty();
+        if (!p.tc_pairs.empty() || !p.tc_cpairs.empty()) {
             p.tc_skip.assign((size_t)N * N, 0);
             p.slot_mcol0 = s;
             s += N * tcS;
@@ -282,12 +291,13 @@ void build_tables(Plan& p, int64_t D, int dtype, int sm_count)
         if (p.slot_multi >= 0)
             for (int m = 0; m < N; ++m) valid(b, p.slot_multi + m) = own(b, m);   // nobody writes a block that is not ours
     }
-    for (size_t q = 0; q + 1 < p.tc_pairs.size(); q += 2) {
-        const int n = p.tc_pairs[q], m = p.tc_pairs[q + 1];
+    auto two_sided = [&](int n, int m) {
         p.tc_skip[(size_t)n * N + m] = p.tc_skip[(size_t)m * N + n] = 1;
         valid(m, p.slot_multi + n) = 0;   // position (m, n) arrives through the column-side slots instead
         for (int t = 0; t < tcS; ++t) valid(m, p.slot_mcol0 + n * tcS + t) = 1;
-    }
+    };
+    for (size_t q = 0; q + 1 < p.tc_pairs.size(); q += 2) two_sided(p.tc_pairs[q], p.tc_pairs[q + 1]);
+    for (size_t q = 0; q + 2 < p.tc_cpairs.size(); q += 3) two_sided(p.tc_cpairs[q], p.tc_cpairs[q + 1]);
     const int strip = p.B / p.Q;
     auto push_items = [&](std::vector<ProcItem>& dst, int n, int m, uint8_t kd) {
         valid(n, p.slot_row0 + m) = 1;
@@ -349,7 +359,7 @@ Candidate evaluate_candidate(int64_t D, int dtype, int k, int B, int cached_per_
     p.part_scheme = part.scheme;
     c.pairs = pairs;
     build_tables(p, D, dtype, sm_count);
-    if (budget_bytes >= 0 && !p.tc_pairs.empty() &&
+    if (budget_bytes >= 0 && (!p.tc_pairs.empty() || !p.tc_cpairs.empty()) &&
         (double)p.cache_bytes + (double)p.work_bytes + (double)fixed_work_bytes(D, dtype, k) > budget_bytes) {
         // the column-side slots of the two-sided k-vector generator do not fit: one-sided generation instead
         p.allow_tc_pairs = false;
@@ -368,7 +378,7 @@ Candidate evaluate_candidate(int64_t D, int dtype, int k, int B, int cached_per_
     const double entries = (double)p.owned_blocks * B * B;                     // entries this rank applies
     c.cached_fraction = f;
     c.t_cached = c.cache_bytes / kBwRead;
-    if (pairs && k > 1)   // the mirrored positions are served by a second read of the stored blocks (mfh_tc.cu)
+    if (pairs && k > 1 && !p.pair_units)   // the mirrored positions are served by a second read of the stored blocks (mfh_tc.cu)
         c.t_cached = (c.cache_bytes + (double)(p.covered_blocks - p.n_cached) * B * B * cb) / kBwRead;
     if (k == 1) {
         // generations: one per mirrored pair, one per one-sided entry, ~half of a diagonal block

@@ -88,7 +88,8 @@ __global__ void __launch_bounds__(256) fill_kernel(const GenArgs<T> G, int32_t B
             CT v;
             v.x = hr;
             v.y = hi;
-            if (tiled == 1) reinterpret_cast<CT*>(reinterpret_cast<T*>(out + base) + tiled_cache_offset(B, a, b))[0] = v;
+            if (tiled == 3 && n != m) *reinterpret_cast<CT*>(reinterpret_cast<char*>(out + base) + unit_image_offset(B, a, b)) = v;
+            else if (tiled == 1 || tiled == 3) reinterpret_cast<CT*>(reinterpret_cast<T*>(out + base) + tiled_cache_offset(B, a, b))[0] = v;
             else if (tiled == 2) out[base + strip_tile_offset(B, STRIP_PIECE_BYTES / (int)sizeof(CT), a, b)] = v;
             else row[b] = v;
         }
@@ -126,30 +127,33 @@ int launch_fill_cache(mfh_handle h, cudaStream_t st)
     int rc = ensure_gen_table(h, st);
     if (rc) return rc;
     dim3 grid(p.n_blk * p.n_blk, std::min(p.B, 64));
-    // layouts: 0 row-major blocks, 1 the 16 KB tiles of complex64 k-vector plans, 2 the strip tiles of partial plans
+    // layouts: 0 row-major blocks, 1 the 16 KB tiles of complex64 k-vector plans, 2 the strip tiles of partial plans,
+    // 3 a k-vector pair cache: unit images for the off-diagonal blocks, 16 KB tiles for the diagonal ones
     const int strip = p.strip_tiled ? 2 : 0;
     return h->dtype == MFH_C128
                ? launch_fill_t<double>(h, grid, p.B, p.n_blk, h->d_cache_slot, 0, 0, strip, h->d_cache, st)
-               : launch_fill_t<float>(h, grid, p.B, p.n_blk, h->d_cache_slot, 0, 0, p.k > 1 ? 1 : strip, h->d_cache, st);
+               : launch_fill_t<float>(h, grid, p.B, p.n_blk, h->d_cache_slot, 0, 0, p.k > 1 ? (p.pair_units ? 3 : 1) : strip, h->d_cache, st);
 }
 
 // External block (Eq. 10) -> cache slot: a plain copy for row-major caches, a re-layout for the tiled cache
 // of complex64 k-vector plans (mfh_internal.cuh tiled_cache_offset).
-__global__ void __launch_bounds__(256) retile_kernel(int32_t B, const float2* __restrict__ src, float2* __restrict__ dst)
+__global__ void __launch_bounds__(256) retile_kernel(int32_t B, int32_t units, const float2* __restrict__ src, float2* __restrict__ dst)
 {
     for (int64_t e = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; e < (int64_t)B * B; e += (int64_t)gridDim.x * blockDim.x) {
         const int a = (int)(e / B), b = (int)(e % B);
-        reinterpret_cast<float2*>(reinterpret_cast<float*>(dst) + tiled_cache_offset(B, a, b))[0] = src[e];
+        if (units) *reinterpret_cast<float2*>(reinterpret_cast<char*>(dst) + unit_image_offset(B, a, b)) = src[e];
+        else reinterpret_cast<float2*>(reinterpret_cast<float*>(dst) + tiled_cache_offset(B, a, b))[0] = src[e];
     }
 }
 
-int launch_store_block(mfh_handle h, int32_t slot, const void* src_dev, cudaStream_t st)
+// (n, m): the block's position -- an off-diagonal block of a k-vector pair cache is stored as unit images
+int launch_store_block_at(mfh_handle h, int32_t slot, int32_t n, int32_t m, const void* src_dev, cudaStream_t st)
 {
     const Plan& p = h->plan;
     const size_t cb = complex_bytes(h->dtype), bytes = (size_t)p.B * p.B * cb;
     char* dst = (char*)h->d_cache + (size_t)slot * bytes;
     if (h->dtype == MFH_C64 && p.k > 1) {
-        retile_kernel<<<std::min(p.B * p.B / 256, 148 * 8), 256, 0, st>>>(p.B, (const float2*)src_dev, (float2*)dst);
+        retile_kernel<<<std::min(p.B * p.B / 256, 148 * 8), 256, 0, st>>>(p.B, (p.pair_units && n != m) ? 1 : 0, (const float2*)src_dev, (float2*)dst);
         MFH_CUDA_CHECK(cudaGetLastError());
     } else {
         MFH_CUDA_CHECK(cudaMemcpyAsync(dst, src_dev, bytes, cudaMemcpyDeviceToDevice, st));

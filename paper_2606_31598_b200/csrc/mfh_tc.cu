@@ -291,7 +291,7 @@ __global__ void __launch_bounds__(TC_THREADS, 2) proc_multi_tc_kernel(const TcPa
     const uint32_t i_base = blockIdx.x * TC_TP;
     const int n = (int)(i_base / (uint32_t)P.B);
     if (P.cache_slot[n * P.n_blk + m] != -1) return;   // cached block: not this kernel's
-    if (P.skip && P.skip[n * P.n_blk + m]) return;     // generated once for both sides by proc_pairs_tc_kernel
+    if (P.skip && P.skip[n * P.n_blk + m]) return;     // served for both sides by pairs_tc_kernel
 
     if (tid == 0) {
         for (int s = 0; s < TC_STAGES; ++s) {
@@ -373,12 +373,18 @@ constexpr int T2_IMG = 128 * T2_UNIT_COLS * 8;    // one image (raw or lo) of a 
 constexpr int T2_UNIT = 2 * T2_IMG;
 constexpr int T2_XCH = 4 * 32 * 32 * 4;           // epilogue exchange: [quadrant][column][lane] floats
 constexpr int T2_SMEM = 1024 + 2 * T2_UNIT + 2 * TC_STAGE + 2 * T2_XCH;
+// cached variant (stored pair blocks instead of generated ones): a producer warp, TMA stages of raw unit images
+constexpr int T2C_W_TMA = T2_GEN_WARPS + 8;
+constexpr int T2C_THREADS = 32 * (T2_GEN_WARPS + 9);
+constexpr int T2C_STAGES = 3;
+constexpr int T2C_SMEM = 1024 + T2C_STAGES * T2_IMG + 2 * T2_IMG + 2 * TC_STAGE + 2 * T2_XCH;
 
 struct T2Params {
     GenArgs<float> G;
-    int32_t B, n_blk, k, slot_multi, slot_mcol0, S, n_items;
+    int32_t B, n_blk, k, slot_multi, slot_mcol0, S, n_items, pstride;
     int64_t D;
-    const int32_t* pairs;   // (row block, column block) per pair
+    const int32_t* pairs;   // (row block, column block[, cache slot]) per pair, pstride ints each
+    const float2* cache;    // cached variant: stored blocks in the unit-image layout (mfh_internal.cuh unit_image_offset)
     const float2* psi;
     float2* work;
 };
@@ -389,6 +395,7 @@ struct T2Bars {
     uint64_t macc_full, macc_empty;       // column-side accumulator
     uint64_t psi_full;                    // psi operand of the item in TMEM
     uint64_t ddone, dacc_empty;           // row-side accumulator
+    uint64_t raw_full[T2C_STAGES], raw_empty[T2C_STAGES];   // cached variant: TMA stages of raw unit images
 };
 
 // K-major, SWIZZLE_128B: rows of 128 bytes (32 TF32), 8-row groups 1 KB apart.
@@ -431,7 +438,7 @@ __device__ __forceinline__ void t2_generate(const T2Params& P, unsigned char* ub
     uint32_t gt = 0;   // tiles of this group so far = units so far
     for (int item = blockIdx.x; item < P.n_items; item += gridDim.x) {
         const int pr = item / P.S, strip = item - pr * P.S;
-        const int rb = P.pairs[2 * pr], cb = P.pairs[2 * pr + 1];
+        const int rb = P.pairs[P.pstride * pr], cb = P.pairs[P.pstride * pr + 1];
         const uint32_t i = (uint32_t)rb * P.B + strip * TC_TP + p;
         for (int u = 0; u < n_units; ++u, ++gt) {
             const int s2 = gt & 1;
@@ -496,6 +503,112 @@ __device__ __forceinline__ void t2_generate(const T2Params& P, unsigned char* ub
     }
 }
 
+// Converter group g of the cached variant (256 threads): the unit's raw image has been landed by a bulk copy in the
+// layout the generator threads write; a thread reads the same 8 entries it would have generated (tile 2u + g, row p,
+// column groups gsel, gsel + 2), writes their low parts x - trunc(x) to the lo image and the four row-side images to
+// TMEM.  The raw stage is freed by the column-side MMAs' commit, not by the converters.
+__device__ __forceinline__ void t2_convert(const T2Params& P, unsigned char* rawbuf, unsigned char* lobuf, unsigned char* bimg, T2Bars& bar,
+                                           uint32_t d_tmem)
+{
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int g = tid >> 8, lt = tid & 255;
+    const int p = lt & (TC_TP - 1), gsel = lt >> 7;
+    const uint32_t a_lane = d_tmem + ((uint32_t)(p & ~31) << 16);
+    const int v = lt & 15, qb = lt >> 4, k = P.k;
+    const int o_re = ((v & 7) * 16 + (v >> 3) * TC_SBO + (qb >> 2) * 128 + (qb & 3) * 4) / 4;
+    const int o_im = o_re + 2 * TC_SBO / 4;
+    const int n_units = P.B / T2_UNIT_COLS;
+    const uint32_t chunk = (uint32_t)(p & 15) >> 1;
+    const uint32_t m_row = (uint32_t)((p & 63) >> 4) * 8192u + (uint32_t)(p >> 6) * 4096u + (uint32_t)(p & 1) * 8u;
+    uint32_t gt = 0;   // units so far
+    for (int item = blockIdx.x; item < P.n_items; item += gridDim.x) {
+        const int pr = item / P.S;
+        const int cb = P.pairs[P.pstride * pr + 1];
+        for (int u = 0; u < n_units; ++u, ++gt) {
+            const int s2 = gt & 1, st = gt % T2C_STAGES;
+            const uint32_t use = gt >> 1;
+            const uint32_t j0 = (uint32_t)cb * P.B + (2 * u + g) * TC_TQ;
+            const float2 x = (v < k && qb < TC_TQ) ? P.psi[(size_t)(j0 + qb) * k + v] : float2{0.f, 0.f};   // in flight during the wait
+            mbar_wait(&bar.raw_full[st], (gt / T2C_STAGES) & 1);
+            const unsigned char* raw = rawbuf + st * T2_IMG;
+            float rh[TC_NG][4], rl[TC_NG][4], ih[TC_NG][4], il[TC_NG][4];
+            uint32_t off[TC_NG][4];
+#pragma unroll
+            for (int gg = 0; gg < TC_NG; ++gg)
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const uint32_t c8 = 4u * gsel + e;
+                    off[gg][e] = m_row + (uint32_t)(2 * g + gg) * 1024u + c8 * 128u + ((chunk ^ c8) << 4);
+                    const float2 w = *reinterpret_cast<const float2*>(raw + off[gg][e]);
+                    rh[gg][e] = w.x;
+                    ih[gg][e] = w.y;
+                }
+#pragma unroll
+            for (int gg = 0; gg < TC_NG; ++gg)
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    rl[gg][e] = rh[gg][e] - __uint_as_float(__float_as_uint(rh[gg][e]) & 0xffffe000u);
+                    il[gg][e] = ih[gg][e] - __uint_as_float(__float_as_uint(ih[gg][e]) & 0xffffe000u);
+                }
+            float prh, prl, pih, pil;
+            split_tf32(x.x, prh, prl);
+            split_tf32(x.y, pih, pil);
+            if (use > 0) mbar_wait(&bar.mempty[s2], (use - 1) & 1);   // the column-side MMAs of the unit two back are done
+            unsigned char* lo = lobuf + s2 * T2_IMG;
+#pragma unroll
+            for (int gg = 0; gg < TC_NG; ++gg)
+#pragma unroll
+                for (int e = 0; e < 4; ++e) *reinterpret_cast<float2*>(lo + off[gg][e]) = make_float2(rl[gg][e], il[gg][e]);
+            if (gt > 0) mbar_wait(&bar.dempty[g], (gt - 1) & 1);      // the row-side MMAs of this group's previous tile are done
+#pragma unroll
+            for (int gg = 0; gg < TC_NG; ++gg) {
+                const uint32_t ta = a_lane + (uint32_t)(T2_COL_ASTAGE + g * TC_A_STAGE_COLS + 4 * (gsel + 2 * gg));
+                tmem_st4(ta + 0 * TC_TQ, rh[gg][0], rh[gg][1], rh[gg][2], rh[gg][3]);
+                tmem_st4(ta + 1 * TC_TQ, rl[gg][0], rl[gg][1], rl[gg][2], rl[gg][3]);
+                tmem_st4(ta + 2 * TC_TQ, ih[gg][0], ih[gg][1], ih[gg][2], ih[gg][3]);
+                tmem_st4(ta + 3 * TC_TQ, il[gg][0], il[gg][1], il[gg][2], il[gg][3]);
+            }
+            if (qb < TC_TQ) {
+                float* b = reinterpret_cast<float*>(bimg + g * TC_STAGE);
+                constexpr int BT = TC_B_TILE / 4;
+                b[0 * BT + o_re] = prh;  b[0 * BT + o_im] = pih;
+                b[1 * BT + o_re] = prl;  b[1 * BT + o_im] = pil;
+                b[2 * BT + o_re] = -pih; b[2 * BT + o_im] = prh;
+                b[3 * BT + o_re] = -pil; b[3 * BT + o_im] = prl;
+            }
+            asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            __syncwarp();
+            if (lane == 0) {
+                mbar_arrive(&bar.dfull[g]);
+                mbar_arrive(&bar.mfull[s2]);
+            }
+        }
+    }
+}
+
+// Producer warp of the cached variant: one 32 KB bulk copy per unit into a ring of T2C_STAGES raw stages.
+__device__ __forceinline__ void t2_produce(const T2Params& P, unsigned char* rawbuf, T2Bars& bar)
+{
+    const int n_units = P.B / T2_UNIT_COLS;
+    uint32_t gt = 0;
+    if (!elect_one()) return;
+    for (int item = blockIdx.x; item < P.n_items; item += gridDim.x) {
+        const int pr = item / P.S, strip = item - pr * P.S;
+        const unsigned char* blk = reinterpret_cast<const unsigned char*>(P.cache) + (size_t)P.pairs[P.pstride * pr + 2] * P.B * P.B * 8 +
+                                   (size_t)strip * n_units * T2_IMG;
+        for (int u = 0; u < n_units; ++u, ++gt) {
+            const int st = gt % T2C_STAGES;
+            if (gt >= T2C_STAGES) mbar_wait(&bar.raw_empty[st], (gt / T2C_STAGES - 1) & 1);
+            asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(&bar.raw_full[st])), "r"(T2_IMG) : "memory");
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(rawbuf + st * T2_IMG)),
+                         "l"(blk + (size_t)u * T2_IMG), "r"(T2_IMG), "r"(smem_u32(&bar.raw_full[st]))
+                         : "memory");
+        }
+    }
+}
+
 // Row-side MMA warp: the one-sided kernel's 8 MMAs per tile, tiles in column order (group = tile parity).
 __device__ __forceinline__ void t2_row_mma(const T2Params& P, unsigned char* bimg, T2Bars& bar, uint32_t d_tmem)
 {
@@ -534,7 +647,9 @@ __device__ __forceinline__ void t2_row_mma(const T2Params& P, unsigned char* bim
 }
 
 // Column-side MMA warp: per unit 16 K-steps x (raw image, lo image), A = the item's psi operand in TMEM.
-__device__ __forceinline__ void t2_col_mma(const T2Params& P, unsigned char* ubuf, T2Bars& bar, uint32_t d_tmem)
+// CACHED: the raw image is the TMA stage of the unit (freed by this warp's commit), the lo image one of two buffers.
+template <bool CACHED>
+__device__ __forceinline__ void t2_col_mma(const T2Params& P, unsigned char* ubuf, unsigned char* lobuf, T2Bars& bar, uint32_t d_tmem)
 {
     const int lane = threadIdx.x & 31;
     const int n_units = P.B / T2_UNIT_COLS;
@@ -547,16 +662,19 @@ __device__ __forceinline__ void t2_col_mma(const T2Params& P, unsigned char* ubu
             if (gu > 0) mbar_wait(&bar.macc_empty, (gu - 1) & 1);
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             if (elect_one()) {
-                const uint64_t bd = umma_desc_sw128(smem_u32(ubuf + ub * T2_UNIT));
+                const int st = gu % T2C_STAGES;
+                const uint64_t bd_raw = umma_desc_sw128(smem_u32(CACHED ? ubuf + st * T2_IMG : ubuf + ub * T2_UNIT));
+                const uint64_t bd_lo = CACHED ? umma_desc_sw128(smem_u32(lobuf + ub * T2_IMG)) : bd_raw + (uint64_t)(T2_IMG >> 4);
                 const uint32_t a0 = d_tmem + (uint32_t)(T2_COL_PSI + 128 * (items_done & 1));
 #pragma unroll
                 for (int img = 0; img < 2; ++img)
 #pragma unroll
                     for (int j = 0; j < 16; ++j) {
-                        const uint64_t b = bd + (uint64_t)((img * T2_IMG + (j >> 2) * 8192 + (j & 3) * 32) >> 4);
+                        const uint64_t b = (img ? bd_lo : bd_raw) + (uint64_t)(((j >> 2) * 8192 + (j & 3) * 32) >> 4);
                         umma_tf32_ts<64>(d_tmem + T2_COL_MACC, a0 + 8 * j, b, (img | j) != 0);
                     }
                 umma_commit(&bar.mempty[ub]);
+                if (CACHED) umma_commit(&bar.raw_empty[st]);
                 umma_commit(&bar.macc_full);
             }
             __syncwarp();
@@ -577,7 +695,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params& P, float* xch, T2Bar
     // row pairs [r2a, r2b) of the psi operand of `item` into buffer `buf`
     auto psi_rows = [&](int item, int buf, int r2a, int r2b) {
         const int pr = item / P.S, strip = item - pr * P.S;
-        const float2* src = P.psi + ((size_t)P.pairs[2 * pr] * P.B + (size_t)strip * TC_TP + 64 * h) * k + v;
+        const float2* src = P.psi + ((size_t)P.pairs[P.pstride * pr] * P.B + (size_t)strip * TC_TP + 64 * h) * k + v;
 #pragma unroll 4
         for (int r2 = r2a; r2 < r2b; ++r2) {
             float2 x0 = float2{0.f, 0.f}, x1 = float2{0.f, 0.f};
@@ -608,10 +726,26 @@ __device__ __forceinline__ void t2_epilogue(const T2Params& P, float* xch, T2Bar
     uint32_t gu = 0, items_done = 0;
     for (int item = blockIdx.x; item < P.n_items; item += gridDim.x, ++items_done) {
         const int pr = item / P.S, strip = item - pr * P.S;
-        const int rb = P.pairs[2 * pr], cb = P.pairs[2 * pr + 1];
+        const int rb = P.pairs[P.pstride * pr], cb = P.pairs[P.pstride * pr + 1];
         const size_t row0 = (size_t)rb * P.B + (size_t)strip * TC_TP;
         const int next = item + gridDim.x;
+        const float2* nsrc = nullptr;
+        if (next < P.n_items) {
+            const int npr = next / P.S, nstrip = next - npr * P.S;
+            nsrc = P.psi + ((size_t)P.pairs[P.pstride * npr] * P.B + (size_t)nstrip * TC_TP + 64 * h) * k + v;
+        }
         for (int u = 0; u < n_units; ++u, ++gu) {
+            // rows of the next item's psi operand handled in this unit: loaded now, in flight during the wait
+            const bool pipelined = per <= 2;
+            const int r2a = u * per;
+            float2 nx[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) nx[i] = float2{0.f, 0.f};
+            if (pipelined && nsrc && r2a < 32 && v < k) {
+#pragma unroll
+                for (int i = 0; i < 4; ++i)
+                    if (2 * r2a + i < 64 && i < 2 * per) nx[i] = nsrc[(size_t)(2 * r2a + i) * k];
+            }
             mbar_wait(&bar.macc_full, gu & 1);
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             uint32_t r[32];
@@ -628,9 +762,26 @@ __device__ __forceinline__ void t2_epilogue(const T2Params& P, float* xch, T2Bar
             asm volatile("bar.arrive %0, 192;" ::"r"(1 + xb) : "memory");
             // the column-side MMA warp has passed its wait for THIS item's operand (its unit 0 is complete), so the
             // next arrival on psi_full cannot overtake it; the other buffer's readers (previous item) are done
-            if (next < P.n_items && u * per < 32) {
-                psi_rows(next, (items_done + 1) & 1, u * per, min(32, (u + 1) * per));
-                if ((u + 1) * per >= 32) psi_publish();
+            if (next < P.n_items && r2a < 32) {
+                const int buf = (items_done + 1) & 1;
+                if (pipelined) {
+#pragma unroll
+                    for (int i = 0; i < 2; ++i) {
+                        if (i >= per || r2a + i >= 32) break;
+                        const float2 x0 = nx[2 * i], x1 = nx[2 * i + 1];
+                        float a0 = op ? x0.y : x0.x, a1 = op ? -x0.x : x0.y, a2 = op ? x1.y : x1.x, a3 = op ? -x1.x : x1.y;
+                        if (lohi) {
+                            a0 -= __uint_as_float(__float_as_uint(a0) & 0xffffe000u);
+                            a1 -= __uint_as_float(__float_as_uint(a1) & 0xffffe000u);
+                            a2 -= __uint_as_float(__float_as_uint(a2) & 0xffffe000u);
+                            a3 -= __uint_as_float(__float_as_uint(a3) & 0xffffe000u);
+                        }
+                        tmem_st4(lane_base + (uint32_t)(T2_COL_PSI + 128 * buf + 4 * (r2a + i)), a0, a1, a2, a3);
+                    }
+                } else {
+                    psi_rows(next, buf, r2a, min(32, r2a + per));
+                }
+                if (r2a + per >= 32) psi_publish();
             }
         }
         mbar_wait(&bar.ddone, items_done & 1);
@@ -651,7 +802,7 @@ __device__ __forceinline__ void t2_col_sums(const T2Params& P, const float* xch)
     uint32_t gu = 0;
     for (int item = blockIdx.x; item < P.n_items; item += gridDim.x) {
         const int pr = item / P.S, strip = item - pr * P.S;
-        const int rb = P.pairs[2 * pr], cb = P.pairs[2 * pr + 1];
+        const int rb = P.pairs[P.pstride * pr], cb = P.pairs[P.pstride * pr + 1];
         float2* out_col = P.work + ((size_t)(P.slot_mcol0 + rb * P.S + strip) * P.D + (size_t)cb * P.B) * k;
         for (int u = 0; u < n_units; ++u, ++gu) {
             const int xb = gu & 1;
@@ -676,14 +827,18 @@ __device__ __forceinline__ void t2_col_sums(const T2Params& P, const float* xch)
     }
 }
 
-__global__ void __launch_bounds__(T2_THREADS, 1) proc_pairs_tc_kernel(const T2Params P)
+template <bool CACHED>
+__global__ void __launch_bounds__(CACHED ? T2C_THREADS : T2_THREADS, 1) pairs_tc_kernel(const T2Params P)
 {
     extern __shared__ __align__(128) unsigned char smem_raw2_[];
     __shared__ __align__(8) T2Bars bar;
     __shared__ uint32_t s_tmem;
     const int tid = threadIdx.x, w = tid >> 5;
-    unsigned char* ubuf = smem_raw2_ + ((1024u - (smem_u32(smem_raw2_) & 1023u)) & 1023u);   // 1 KB aligned (128-byte swizzle atoms)
-    unsigned char* bimg = ubuf + 2 * T2_UNIT;
+    // 1 KB aligned (128-byte swizzle atoms).  Generated: [unit buffers: raw + lo images][B images][exchange];
+    // cached: [raw stages][lo buffers][B images][exchange]
+    unsigned char* ubuf = smem_raw2_ + ((1024u - (smem_u32(smem_raw2_) & 1023u)) & 1023u);
+    unsigned char* lobuf = ubuf + T2C_STAGES * T2_IMG;                       // cached variant only
+    unsigned char* bimg = CACHED ? lobuf + 2 * T2_IMG : ubuf + 2 * T2_UNIT;
     float* xch = reinterpret_cast<float*>(bimg + 2 * TC_STAGE);
     if (tid == 0) {
         for (int g = 0; g < 2; ++g) {
@@ -693,6 +848,10 @@ __global__ void __launch_bounds__(T2_THREADS, 1) proc_pairs_tc_kernel(const T2Pa
         for (int s = 0; s < 2; ++s) {
             mbar_init(&bar.mfull[s], T2_GEN_WARPS);
             mbar_init(&bar.mempty[s], 1);
+        }
+        for (int s = 0; s < T2C_STAGES; ++s) {
+            mbar_init(&bar.raw_full[s], 1);
+            mbar_init(&bar.raw_empty[s], 1);
         }
         mbar_init(&bar.macc_full, 1);
         mbar_init(&bar.macc_empty, 4);
@@ -710,11 +869,14 @@ __global__ void __launch_bounds__(T2_THREADS, 1) proc_pairs_tc_kernel(const T2Pa
     asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
     const uint32_t d_tmem = s_tmem;
 
-    if (w < T2_GEN_WARPS) t2_generate(P, ubuf, bimg, bar, d_tmem);
-    else if (w < T2_W_EPI + 4) t2_epilogue(P, xch, bar, d_tmem);
+    if (w < T2_GEN_WARPS) {
+        if (CACHED) t2_convert(P, ubuf, lobuf, bimg, bar, d_tmem);
+        else t2_generate(P, ubuf, bimg, bar, d_tmem);
+    } else if (w < T2_W_EPI + 4) t2_epilogue(P, xch, bar, d_tmem);
     else if (w < T2_W_SUM + 2) t2_col_sums(P, xch);
     else if (w == T2_W_DMMA) t2_row_mma(P, bimg, bar, d_tmem);
-    else if (w == T2_W_MMMA) t2_col_mma(P, ubuf, bar, d_tmem);
+    else if (w == T2_W_MMMA) t2_col_mma<CACHED>(P, ubuf, lobuf, bar, d_tmem);
+    else if (CACHED && w == T2C_W_TMA) t2_produce(P, ubuf, bar);
 
     asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
@@ -726,10 +888,9 @@ bool tc_pairs_supported(int dtype, int k, int B, int part_world)
     return dtype == MFH_C64 && k > 1 && k <= 16 && B % TC_TP == 0 && part_world <= 1;
 }
 
-static int launch_proc_pairs_tc(mfh_handle h, const void* psi, cudaStream_t st)
+static void t2_common_params(mfh_handle h, const void* psi, T2Params& P)
 {
     const Plan& p = h->plan;
-    T2Params P;
     P.G.K = make_philox_keys(h->seed);
     P.G.gc.neg_k2_ln2 = (float)(-0.6931471805599453 / (double)h->D);
     P.G.tab_global = nullptr;
@@ -739,13 +900,37 @@ static int launch_proc_pairs_tc(mfh_handle h, const void* psi, cudaStream_t st)
     P.slot_multi = p.slot_multi;
     P.slot_mcol0 = p.slot_mcol0;
     P.S = p.B / TC_TP;
-    P.n_items = (int32_t)(p.tc_pairs.size() / 2) * P.S;
     P.D = h->D;
-    P.pairs = h->d_tc_pairs;
+    P.cache = (const float2*)h->d_cache;
     P.psi = (const float2*)psi;
     P.work = (float2*)h->d_work;
-    if (int rc = ensure_dyn_smem(h, proc_pairs_tc_kernel, T2_SMEM)) return rc;
-    proc_pairs_tc_kernel<<<std::min(P.n_items, h->sm_count), T2_THREADS, T2_SMEM, st>>>(P);
+}
+
+// Generated block pairs: both positions from one generation.
+static int launch_proc_pairs_tc(mfh_handle h, const void* psi, cudaStream_t st)
+{
+    T2Params P;
+    t2_common_params(h, psi, P);
+    P.pstride = 2;
+    P.pairs = h->d_tc_pairs;
+    P.n_items = (int32_t)(h->plan.tc_pairs.size() / 2) * P.S;
+    if (int rc = ensure_dyn_smem(h, pairs_tc_kernel<false>, T2_SMEM)) return rc;
+    pairs_tc_kernel<false><<<std::min(P.n_items, h->sm_count), T2_THREADS, T2_SMEM, st>>>(P);
+    MFH_CUDA_CHECK(cudaGetLastError());
+    return MFH_OK;
+}
+
+// Stored pair blocks (complex64 k-vector pair cache): both positions from ONE read of the stored block.
+int launch_cached_pairs_tc(mfh_handle h, const void* psi, cudaStream_t st)
+{
+    T2Params P;
+    t2_common_params(h, psi, P);
+    P.pstride = 3;
+    P.pairs = h->d_tc_cpairs;
+    P.n_items = (int32_t)(h->plan.tc_cpairs.size() / 3) * P.S;
+    if (P.n_items == 0) return MFH_OK;
+    if (int rc = ensure_dyn_smem(h, pairs_tc_kernel<true>, T2C_SMEM)) return rc;
+    pairs_tc_kernel<true><<<std::min(P.n_items, h->sm_count), T2C_THREADS, T2C_SMEM, st>>>(P);
     MFH_CUDA_CHECK(cudaGetLastError());
     return MFH_OK;
 }
@@ -823,6 +1008,7 @@ struct CtParams {
     int32_t B, n_blk, k, slot_multi;
     int64_t D;
     const int32_t* cache_slot;
+    const uint8_t* skip;   // positions served by the two-sided cached kernel (nullptr: none)
     const float2* cache;   // tiled layout
     const float2* psi;
     float2* work;
@@ -837,8 +1023,9 @@ __global__ void __launch_bounds__(CT_THREADS, 2) cached_multi_tc_kernel(const Ct
     const int m = blockIdx.y;
     const uint32_t i_base = blockIdx.x * TC_TP;
     const int n = (int)(i_base / (uint32_t)P.B);
+    if (P.skip && P.skip[n * P.n_blk + m]) return;   // both positions of a stored pair: pairs_tc_kernel<true>, from one read
     int32_t slot = P.cache_slot[n * P.n_blk + m];
-    // Hermitian pair cache (MFH_MODE_PAIRS with k > 1): position (n,m) marked -2 is served by the stored canonical block
+    // Hermitian pair cache (MFH_MODE_PAIRS with k > 1) without the unit-image layout (partitioned handles): position (n,m) marked -2 is served by the stored canonical block
     // C = H^[m,n]: phi^[n] += C^dagger psi^[m].  The CTA's 128 output rows are 128 COLUMNS of C; it reads C a second
     // time, transposed (TR): a stage is 16 rows of C x those 128 columns = eight 2 KB pieces of eight neighbouring
     // tiles.  (This halves the MEMORY of a k-vector operator, not the bytes per apply: DESIGN.md 6.5.)
@@ -1031,13 +1218,14 @@ int launch_cached_multi_tc(mfh_handle h, const void* psi, cudaStream_t st)
     P.slot_multi = p.slot_multi;
     P.D = h->D;
     P.cache_slot = h->d_cache_slot;
+    P.skip = p.tc_cpairs.empty() ? nullptr : h->d_tc_skip;
     P.cache = (const float2*)h->d_cache;
     P.psi = (const float2*)psi;
     P.work = (float2*)h->d_work;
     if (int rc = ensure_dyn_smem(h, cached_multi_tc_kernel, CT_SMEM)) return rc;
     cached_multi_tc_kernel<<<dim3((unsigned)(h->D / TC_TP), p.n_blk), CT_THREADS, CT_SMEM, st>>>(P);
     MFH_CUDA_CHECK(cudaGetLastError());
-    return MFH_OK;
+    return launch_cached_pairs_tc(h, psi, st);   // stored off-diagonal pairs in the unit-image layout: both sides from one read
 }
 
 }  // namespace mfh
