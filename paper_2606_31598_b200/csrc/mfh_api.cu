@@ -57,7 +57,7 @@ static cudaError_t guarded_malloc(mfh_handle h, void** user, size_t bytes)
 static int free_plan_resources(mfh_handle h)
 {
     void** ptrs[] = {&h->d_cache, &h->d_work, &h->d_h0, (void**)&h->d_cache_slot, (void**)&h->d_items,
-                     (void**)&h->d_pair_items, (void**)&h->d_tc_pairs, (void**)&h->d_tc_skip, (void**)&h->d_tc_cpairs,
+                     (void**)&h->d_pair_items, (void**)&h->d_tc_pairs, (void**)&h->d_tc_skip, (void**)&h->d_tc_cpairs, (void**)&h->d_tc_left, (void**)&h->d_ct_left,
                      (void**)&h->d_slot_list, (void**)&h->d_counter, (void**)&h->d_expected, &h->d_cheb, &h->d_io, &h->d_lanczos, &h->d_stage};
     for (void** p : ptrs) *p = nullptr;
     for (auto& g : h->guarded) cudaFree(g.first);
@@ -149,6 +149,14 @@ static int commit_plan(mfh_handle h, const Plan& p, cudaStream_t st)
     if (!q.tc_pairs.empty()) {   // two-sided tensor-core generator (k-vector complex64 plans)
         MFH_CUDA_CHECK(guarded_malloc(h, (void**)&h->d_tc_pairs, q.tc_pairs.size() * sizeof(int32_t)));
         MFH_CUDA_CHECK(cudaMemcpyAsync(h->d_tc_pairs, q.tc_pairs.data(), q.tc_pairs.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    }
+    if (!q.tc_left.empty()) {
+        MFH_CUDA_CHECK(guarded_malloc(h, (void**)&h->d_tc_left, q.tc_left.size() * sizeof(int32_t)));
+        MFH_CUDA_CHECK(cudaMemcpyAsync(h->d_tc_left, q.tc_left.data(), q.tc_left.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
+    }
+    if (!q.ct_left.empty()) {
+        MFH_CUDA_CHECK(guarded_malloc(h, (void**)&h->d_ct_left, q.ct_left.size() * sizeof(int32_t)));
+        MFH_CUDA_CHECK(cudaMemcpyAsync(h->d_ct_left, q.ct_left.data(), q.ct_left.size() * sizeof(int32_t), cudaMemcpyHostToDevice, st));
     }
     if (!q.tc_cpairs.empty()) {   // two-sided cached kernel (k-vector complex64 pair caches)
         MFH_CUDA_CHECK(guarded_malloc(h, (void**)&h->d_tc_cpairs, q.tc_cpairs.size() * sizeof(int32_t)));
@@ -613,19 +621,21 @@ MFH_API int mfh_get_plan(mfh_handle h, char* json_out, size_t json_cap)
              "{\"partition\":{\"scheme\":\"%s\",\"rank\":%d,\"world\":%d,\"owned_blocks\":%lld,\"first_block_row\":%d,\"block_rows\":%d},"
              "\"mode\":\"%s\",\"B\":%d,\"n_blk\":%d,\"k\":%d,\"cached_blocks\":%lld,\"cached_per_row\":%d,"
              "\"cached_fraction\":%.6g,\"cache_bytes\":%zu,\"work_bytes\":%zu,\"partial_slots\":%d,\"proc_items\":%zu,\"pair_items\":%zu,"
-             "\"proc_rows_per_lane\":%d,\"proc_row_strips\":%d,\"stream_sms\":%d,\"two_sided_pairs\":%zu,\"launches_per_apply\":%d}",
+             "\"proc_rows_per_lane\":%d,\"proc_row_strips\":%d,\"stream_sms\":%d,\"two_sided_pairs\":%zu,\"two_sided_stored_pairs\":%zu,\"launches_per_apply\":%d}",
              p.part_scheme == MFH_PART_ROWS ? "rows" : (p.part_scheme == MFH_PART_PAIRS ? "pairs" : "none"), p.part_rank, p.part_world,
              (long long)p.owned_blocks, p.row_first, p.row_count,
              p.mode == MFH_MODE_FULL ? "full" : (p.mode == MFH_MODE_PARTIAL ? "partial" : (p.mode == MFH_MODE_PAIRS ? "pairs" : "procedural")), p.B,
              p.n_blk, p.k, (long long)p.n_cached, p.cached_per_row,
              (double)p.covered_blocks / (double)std::max<int64_t>(p.owned_blocks, 1), p.cache_bytes, p.work_bytes, p.n_slots,
-             p.items.size(), p.pair_items.size(), p.R, p.Q, p.stream_sms, p.tc_pairs.size() / 2,
+             p.items.size(), p.pair_items.size(), p.R, p.Q, p.stream_sms, p.tc_pairs.size() / 2, p.tc_cpairs.size() / 3,
              h->fused_tail ? 1 : (partial_overlap_supported(h) ? 2 /* one kernel for both parts + reduce */
                                   : 1 + (p.n_cached > 0) + ((p.k == 1 && !p.items.empty()) ||
                                                             (p.k > 1 && p.covered_blocks < p.owned_blocks)) +
                                     // the two-sided k-vector generator and the one-sided kernel for what it leaves
                                     (p.k > 1 && !p.tc_pairs.empty() && tc_multi_supported(h) &&
-                                     p.owned_blocks - p.covered_blocks - (int64_t)p.tc_pairs.size() > 0)));
+                                     p.owned_blocks - p.covered_blocks - (int64_t)p.tc_pairs.size() > 0) +
+                                    // stored pairs served by the two-sided cached kernel, next to the kernel for the diagonal blocks
+                                    (p.k > 1 && !p.tc_cpairs.empty())));
     copy_json(buf, json_out, json_cap);
     return MFH_OK;
 }

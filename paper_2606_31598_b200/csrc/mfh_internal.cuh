@@ -97,6 +97,8 @@ struct Plan {
     std::vector<ProcItem> pair_items;  // cached pair kernel (pairs mode)
     std::vector<int32_t> tc_pairs;     // k-vector two-sided generator: (row block, column block) of every pair it serves
     std::vector<uint8_t> tc_skip;      // [n_blk*n_blk] 1 = position served by a two-sided kernel (the one-sided kernels skip it)
+    std::vector<int32_t> tc_left;      // generated positions the two-sided generator leaves to the one-sided kernel: (row block, column block)
+    std::vector<int32_t> ct_left;      // cached positions the two-sided cached kernel leaves to cached_multi_tc_kernel
     std::vector<int32_t> tc_cpairs;    // two-sided cached kernel: (row block, column block, cache slot) of every stored pair
     std::vector<uint8_t> slot_valid;   // [n_blk][n_slots]
     std::string json;
@@ -129,6 +131,8 @@ struct mfh_handle_s {
     int32_t* d_tc_pairs = nullptr;    // plan.tc_pairs
     uint8_t* d_tc_skip = nullptr;     // plan.tc_skip
     int32_t* d_tc_cpairs = nullptr;   // plan.tc_cpairs
+    int32_t* d_tc_left = nullptr;     // plan.tc_left
+    int32_t* d_ct_left = nullptr;     // plan.ct_left
     int32_t* d_slot_list = nullptr;   // [n_blk][n_slots+1]: count | flags, then the valid slots in ascending order
     double* d_lambdas = nullptr;    // MFH_MAX_K doubles, refreshed by every apply
     int32_t* d_counter = nullptr;   // dynamic work counters: [0] procedural kernel, [1] pair kernel, [2] CTAs finished,

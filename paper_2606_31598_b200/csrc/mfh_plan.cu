@@ -297,6 +297,24 @@ void build_tables(Plan& p, int64_t D, int dtype, int sm_count)
         for (int t = 0; t < tcS; ++t) valid(m, p.slot_mcol0 + n * tcS + t) = 1;
     };
     for (size_t q = 0; q + 1 < p.tc_pairs.size(); q += 2) two_sided(p.tc_pairs[q], p.tc_pairs[q + 1]);
+    p.ct_left.clear();
+    if (!p.tc_cpairs.empty())
+        for (int n = 0; n < N; ++n)
+            for (int m = 0; m < N; ++m) {
+                const int32_t cs = p.cache_slot[(size_t)n * N + m];
+                if ((cs >= 0 || cs == -2) && !p.tc_skip[(size_t)n * N + m]) {
+                    p.ct_left.push_back(n);
+                    p.ct_left.push_back(m);
+                }
+            }
+    p.tc_left.clear();
+    if (!p.tc_pairs.empty())
+        for (int n = 0; n < N; ++n)
+            for (int m = 0; m < N; ++m)
+                if (uncached(n, m) && !p.tc_skip[(size_t)n * N + m]) {
+                    p.tc_left.push_back(n);
+                    p.tc_left.push_back(m);
+                }
     for (size_t q = 0; q + 2 < p.tc_cpairs.size(); q += 3) two_sided(p.tc_cpairs[q], p.tc_cpairs[q + 1]);
     const int strip = p.B / p.Q;
     auto push_items = [&](std::vector<ProcItem>& dst, int n, int m, uint8_t kd) {
@@ -378,7 +396,11 @@ Candidate evaluate_candidate(int64_t D, int dtype, int k, int B, int cached_per_
     const double entries = (double)p.owned_blocks * B * B;                     // entries this rank applies
     c.cached_fraction = f;
     c.t_cached = c.cache_bytes / kBwRead;
-    if (pairs && k > 1 && !p.pair_units)   // the mirrored positions are served by a second read of the stored blocks (mfh_tc.cu)
+    if (pairs && k > 1)
+        // the mirrored positions cost a second pass: a second, transposed read of the stored blocks, or -- with the
+        // unit-image layout -- the column side of the two-sided kernel, which reads every block once but is bound by
+        // the tensor pipe and shared memory at the same time per stored byte (measured, C3: 1.25 ms for the pair cache
+        // against 1.26 ms for the full cache)
         c.t_cached = (c.cache_bytes + (double)(p.covered_blocks - p.n_cached) * B * B * cb) / kBwRead;
     if (k == 1) {
         // generations: one per mirrored pair, one per one-sided entry, ~half of a diagonal block

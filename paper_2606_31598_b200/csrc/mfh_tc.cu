@@ -178,9 +178,32 @@ struct TcParams {
     int64_t D;
     const int32_t* cache_slot;
     const uint8_t* skip;   // [n_blk*n_blk] positions served by the two-sided generator (nullptr: none)
+    const int32_t* pos;    // compact list of the (row block, column block) positions to run (blockIdx.y), or nullptr: all
     const float2* psi;   // [D][k]
     float2* work;        // [n_slots][D][k]
 };
+
+// The 8 entries of one generator thread in one tile: row i, column groups gsel and gsel + 2.
+template <int REL>
+__device__ __forceinline__ void tc_tile_entries(const GenArgs<float>& G, uint32_t i, uint32_t j0, int gsel, float (&rh)[2][4],
+                                                float (&rl)[2][4], float (&ih)[2][4], float (&il)[2][4])
+{
+#pragma unroll
+    for (int gg = 0; gg < 2; ++gg)
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const uint32_t j = j0 + 4 * (gsel + 2 * gg) + e;
+            float hr, hi;
+            if (REL > 0) entry_upper<float>(G, nullptr, i, j, hr, hi);
+            else if (REL < 0) entry_lower<float>(G, nullptr, i, j, hr, hi);
+            else entry_any<float>(G, nullptr, i, j, hr, hi);
+            // A_hi = the value itself (the tensor core reads its TF32 part), A_lo = x - trunc(x), exact
+            rh[gg][e] = hr;
+            rl[gg][e] = hr - __uint_as_float(__float_as_uint(hr) & 0xffffe000u);
+            ih[gg][e] = hi;
+            il[gg][e] = hi - __uint_as_float(__float_as_uint(hi) & 0xffffe000u);
+        }
+}
 
 // Generator warps (8 x 32 threads).  Per tile of 128 rows x 16 columns a thread produces the two
 // 4-column groups g, g + 2 of row p (8 entries, one 16-byte store per operand image and group) and
@@ -194,7 +217,8 @@ __device__ __forceinline__ void tc_generate(const TcParams& P, unsigned char* sm
     const int p = tid & (TC_TP - 1), gsel = tid >> 7;
     const uint32_t i = i_base + p;
     const uint32_t a_lane = d_tmem + ((uint32_t)(p & ~31) << 16);   // this warp's 32 TMEM lanes: rows 32 (warp % 4) ..
-    const int v = tid & 15, qb = tid >> 4, k = P.k;
+    // (vector, column) of this thread's psi element: a warp covers 8 vectors x 4 columns = 32 distinct banks of a B image
+    const int v = (tid & 7) | ((tid >> 2) & 8), qb = ((tid >> 3) & 3) | ((tid >> 6) << 2), k = P.k;
     // psi element (n, q) of a K-major B image: n = v (real part rows) and n = 16 + v (imaginary part rows)
     const int o_re = ((v & 7) * 16 + (v >> 3) * TC_SBO + (qb >> 2) * 128 + (qb & 3) * 4) / 4;
     const int o_im = o_re + 2 * TC_SBO / 4;
@@ -204,21 +228,11 @@ __device__ __forceinline__ void tc_generate(const TcParams& P, unsigned char* sm
         const uint32_t j0 = (uint32_t)m * P.B + t * TC_TQ;
         const float2 x = (v < k && qb < TC_TQ) ? P.psi[(size_t)(j0 + qb) * k + v] : float2{0.f, 0.f};   // consumed after the entries
         float rh[TC_NG][4], rl[TC_NG][4], ih[TC_NG][4], il[TC_NG][4];
-#pragma unroll
-        for (int gg = 0; gg < TC_NG; ++gg)
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                const uint32_t j = j0 + 4 * (gsel + 2 * gg) + e;
-                float hr, hi;
-                if (REL > 0) entry_upper<float>(P.G, nullptr, i, j, hr, hi);
-                else if (REL < 0) entry_lower<float>(P.G, nullptr, i, j, hr, hi);
-                else entry_any<float>(P.G, nullptr, i, j, hr, hi);
-                // A_hi = the value itself (the tensor core reads its TF32 part), A_lo = x - trunc(x), exact
-                rh[gg][e] = hr;
-                rl[gg][e] = hr - __uint_as_float(__float_as_uint(hr) & 0xffffe000u);
-                ih[gg][e] = hi;
-                il[gg][e] = hi - __uint_as_float(__float_as_uint(hi) & 0xffffe000u);
-            }
+        if (REL != 0) tc_tile_entries<REL>(P.G, i, j0, gsel, rh, rl, ih, il);
+        // diagonal block: only the tiles that cross the diagonal need the general rule (8 of B/16 per 128-row strip)
+        else if (j0 >= i_base + TC_TP) tc_tile_entries<1>(P.G, i, j0, gsel, rh, rl, ih, il);
+        else if (j0 + TC_TQ <= i_base) tc_tile_entries<-1>(P.G, i, j0, gsel, rh, rl, ih, il);
+        else tc_tile_entries<0>(P.G, i, j0, gsel, rh, rl, ih, il);
         float prh, prl, pih, pil;
         split_tf32(x.x, prh, prl);
         split_tf32(x.y, pih, pil);
@@ -287,8 +301,8 @@ __global__ void __launch_bounds__(TC_THREADS, 2) proc_multi_tc_kernel(const TcPa
     __shared__ __align__(8) uint64_t full[TC_STAGES], empty[TC_STAGES], done;
     __shared__ uint32_t s_tmem;
     const int tid = threadIdx.x, w = tid >> 5;
-    const int m = blockIdx.y;
-    const uint32_t i_base = blockIdx.x * TC_TP;
+    const int m = P.pos ? P.pos[2 * blockIdx.y + 1] : (int)blockIdx.y;
+    const uint32_t i_base = (P.pos ? (uint32_t)P.pos[2 * blockIdx.y] * P.B : 0u) + blockIdx.x * TC_TP;
     const int n = (int)(i_base / (uint32_t)P.B);
     if (P.cache_slot[n * P.n_blk + m] != -1) return;   // cached block: not this kernel's
     if (P.skip && P.skip[n * P.n_blk + m]) return;     // served for both sides by pairs_tc_kernel
@@ -429,7 +443,8 @@ __device__ __forceinline__ void t2_generate(const T2Params& P, unsigned char* ub
     const int g = tid >> 8, lt = tid & 255;
     const int p = lt & (TC_TP - 1), gsel = lt >> 7;
     const uint32_t a_lane = d_tmem + ((uint32_t)(p & ~31) << 16);
-    const int v = lt & 15, qb = lt >> 4, k = P.k;
+    // (vector, column) of this thread's psi element: a warp covers 8 vectors x 4 columns = 32 distinct banks of a B image
+    const int v = (lt & 7) | ((lt >> 2) & 8), qb = ((lt >> 3) & 3) | ((lt >> 6) << 2), k = P.k;
     const int o_re = ((v & 7) * 16 + (v >> 3) * TC_SBO + (qb >> 2) * 128 + (qb & 3) * 4) / 4;
     const int o_im = o_re + 2 * TC_SBO / 4;
     const int n_units = P.B / T2_UNIT_COLS;
@@ -514,7 +529,8 @@ __device__ __forceinline__ void t2_convert(const T2Params& P, unsigned char* raw
     const int g = tid >> 8, lt = tid & 255;
     const int p = lt & (TC_TP - 1), gsel = lt >> 7;
     const uint32_t a_lane = d_tmem + ((uint32_t)(p & ~31) << 16);
-    const int v = lt & 15, qb = lt >> 4, k = P.k;
+    // (vector, column) of this thread's psi element: a warp covers 8 vectors x 4 columns = 32 distinct banks of a B image
+    const int v = (lt & 7) | ((lt >> 2) & 8), qb = ((lt >> 3) & 3) | ((lt >> 6) << 2), k = P.k;
     const int o_re = ((v & 7) * 16 + (v >> 3) * TC_SBO + (qb >> 2) * 128 + (qb & 3) * 4) / 4;
     const int o_im = o_re + 2 * TC_SBO / 4;
     const int n_units = P.B / T2_UNIT_COLS;
@@ -758,7 +774,7 @@ __device__ __forceinline__ void t2_epilogue(const T2Params& P, float* xch, T2Bar
             float* X = xch + xb * (T2_XCH / 4);
             if (gu >= 2) asm volatile("bar.sync %0, 192;" ::"r"(3 + xb) : "memory");
 #pragma unroll
-            for (int c = 0; c < 32; ++c) X[(q * 32 + c) * 32 + lane] = __uint_as_float(r[c]);
+            for (int c = 0; c < 32; ++c) X[(q * 32 + c) * 32 + (lane ^ ((c & 1) << 4))] = __uint_as_float(r[c]);   // odd columns swapped by halves: the sum warps read without bank conflicts
             asm volatile("bar.arrive %0, 192;" ::"r"(1 + xb) : "memory");
             // the column-side MMA warp has passed its wait for THIS item's operand (its unit 0 is complete), so the
             // next arrival on psi_full cannot overtake it; the other buffer's readers (previous item) are done
@@ -815,8 +831,8 @@ __device__ __forceinline__ void t2_col_sums(const T2Params& P, const float* xch)
                 re[i8] = im[i8] = 0.f;
 #pragma unroll
                 for (int qq = 0; qq < 4; ++qq) {
-                    re[i8] += X[(qq * 32 + c) * 32 + vv];
-                    im[i8] += X[(qq * 32 + c) * 32 + 16 + vv];
+                    re[i8] += X[(qq * 32 + c) * 32 + (vv ^ ((c & 1) << 4))];
+                    im[i8] += X[(qq * 32 + c) * 32 + ((16 + vv) ^ ((c & 1) << 4))];
                 }
             }
             asm volatile("bar.arrive %0, 192;" ::"r"(3 + xb) : "memory");   // the buffer may be overwritten
@@ -955,6 +971,7 @@ int launch_proc_multi_tc(mfh_handle h, const void* psi, cudaStream_t st)
     P.D = h->D;
     P.cache_slot = h->d_cache_slot;
     P.skip = p.tc_pairs.empty() ? nullptr : h->d_tc_skip;
+    P.pos = p.tc_left.empty() ? nullptr : h->d_tc_left;
     P.psi = (const float2*)psi;
     P.work = (float2*)h->d_work;
     if (!p.tc_pairs.empty())   // block pairs generated once for both sides
@@ -963,7 +980,8 @@ int launch_proc_multi_tc(mfh_handle h, const void* psi, cudaStream_t st)
     if (p.owned_blocks - p.covered_blocks - (int64_t)p.tc_pairs.size() <= 0) return MFH_OK;
     const size_t smem = (size_t)TC_STAGES * TC_STAGE;
     if (int rc = ensure_dyn_smem(h, proc_multi_tc_kernel, (int)smem)) return rc;
-    proc_multi_tc_kernel<<<dim3((unsigned)(h->D / TC_TP), p.n_blk), TC_THREADS, smem, st>>>(P);
+    if (P.pos) proc_multi_tc_kernel<<<dim3((unsigned)(p.B / TC_TP), (unsigned)(p.tc_left.size() / 2)), TC_THREADS, smem, st>>>(P);
+    else proc_multi_tc_kernel<<<dim3((unsigned)(h->D / TC_TP), p.n_blk), TC_THREADS, smem, st>>>(P);
     MFH_CUDA_CHECK(cudaGetLastError());
     return MFH_OK;
 }
@@ -1009,6 +1027,7 @@ struct CtParams {
     int64_t D;
     const int32_t* cache_slot;
     const uint8_t* skip;   // positions served by the two-sided cached kernel (nullptr: none)
+    const int32_t* pos;    // compact list of the (row block, column block) positions to run (blockIdx.y), or nullptr: all
     const float2* cache;   // tiled layout
     const float2* psi;
     float2* work;
@@ -1020,8 +1039,8 @@ __global__ void __launch_bounds__(CT_THREADS, 2) cached_multi_tc_kernel(const Ct
     __shared__ __align__(8) uint64_t raw_full[CT_STAGES], raw_empty[CT_STAGES], a_full[CT_TSTAGES], a_empty[CT_TSTAGES], done;
     __shared__ uint32_t s_tmem;
     const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
-    const int m = blockIdx.y;
-    const uint32_t i_base = blockIdx.x * TC_TP;
+    const int m = P.pos ? P.pos[2 * blockIdx.y + 1] : (int)blockIdx.y;
+    const uint32_t i_base = (P.pos ? (uint32_t)P.pos[2 * blockIdx.y] * P.B : 0u) + blockIdx.x * TC_TP;
     const int n = (int)(i_base / (uint32_t)P.B);
     if (P.skip && P.skip[n * P.n_blk + m]) return;   // both positions of a stored pair: pairs_tc_kernel<true>, from one read
     int32_t slot = P.cache_slot[n * P.n_blk + m];
@@ -1219,11 +1238,13 @@ int launch_cached_multi_tc(mfh_handle h, const void* psi, cudaStream_t st)
     P.D = h->D;
     P.cache_slot = h->d_cache_slot;
     P.skip = p.tc_cpairs.empty() ? nullptr : h->d_tc_skip;
+    P.pos = p.ct_left.empty() ? nullptr : h->d_ct_left;
     P.cache = (const float2*)h->d_cache;
     P.psi = (const float2*)psi;
     P.work = (float2*)h->d_work;
     if (int rc = ensure_dyn_smem(h, cached_multi_tc_kernel, CT_SMEM)) return rc;
-    cached_multi_tc_kernel<<<dim3((unsigned)(h->D / TC_TP), p.n_blk), CT_THREADS, CT_SMEM, st>>>(P);
+    if (P.pos) cached_multi_tc_kernel<<<dim3((unsigned)(p.B / TC_TP), (unsigned)(p.ct_left.size() / 2)), CT_THREADS, CT_SMEM, st>>>(P);
+    else cached_multi_tc_kernel<<<dim3((unsigned)(h->D / TC_TP), p.n_blk), CT_THREADS, CT_SMEM, st>>>(P);
     MFH_CUDA_CHECK(cudaGetLastError());
     return launch_cached_pairs_tc(h, psi, st);   // stored off-diagonal pairs in the unit-image layout: both sides from one read
 }
