@@ -453,17 +453,26 @@ def roofline_for(res: dict, hbm_gbs: float, peak_src: str) -> dict:
     if kern["cached"] >= kern["procedural"]:
         # HBM-bound cached streaming: algorithmic bytes = stored entries * bytes per entry
         nbytes = res["plan"]["cache_bytes"]
-        if res["plan"]["mode"] == "pairs" and k > 1:
-            # k-vector pair cache: every stored off-diagonal block is read twice (direct and transposed use)
+        one_read = res["plan"].get("two_sided_stored_pairs", 0) > 0   # unit-image layout: both positions from one read
+        if res["plan"]["mode"] == "pairs" and k > 1 and not one_read:
+            # k-vector pair cache without the unit-image layout: every stored off-diagonal block is read twice
             nb = D // cfg["B"]
             nbytes = 2 * nbytes - nb * cfg["B"] ** 2 * (8 if cfg["dtype"] == "c64" else 16)
         gbs = nbytes / (kern["cached"] * 1e-3) / 1e9
         name = "cached_pairs_kernel" if (res["plan"]["mode"] == "pairs" and k == 1) else (
-            "cached_kernel" if k == 1 else ("cached_multi_tc_kernel" if cfg["dtype"] == "c64" else "cached_multi_kernel_c128"))
-        return {"kernel": name, "bound": "hbm", "achieved": gbs, "peak": hbm_gbs, "unit": "GB/s",
-                "frac": gbs / hbm_gbs, **ncu_traffic(name, cfg["D"]), "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": nbytes, "kernel_ms": kern["cached"],
-                "share_of_step": kern["cached"] / max(kern["total"], 1e-9)}
+            "cached_kernel" if k == 1 else (("pairs_tc_kernel<true>" if one_read else "cached_multi_tc_kernel") if cfg["dtype"] == "c64" else "cached_multi_kernel_c128"))
+        out = {"kernel": name, "bound": "hbm", "achieved": gbs, "peak": hbm_gbs, "unit": "GB/s",
+               "frac": gbs / hbm_gbs, **ncu_traffic(name, cfg["D"]), "peak_source": peak_src,
+               "algorithmic_bytes_per_launch": nbytes, "kernel_ms": kern["cached"],
+               "share_of_step": kern["cached"] / max(kern["total"], 1e-9)}
+        if one_read:
+            # half the bytes of the full cache for the same entries: the HBM fraction halves by construction; what
+            # bounds this kernel is on-chip (ncu: tensor pipe 72 %, shared memory 74 %, SM clock power-capped to 1.5 GHz)
+            nb = D // cfg["B"]
+            out["applied_bytes_equivalent_gbs"] = (2 * nbytes - nb * cfg["B"] ** 2 * 8) / (kern["cached"] * 1e-3) / 1e9
+            out["note"] = ("every stored block is read once and serves both positions; bound by the tensor pipe and shared "
+                           "memory (profiles/r02_pairs_tc_cached_c3_ncu_full.md), not by HBM")
+        return out
     # ALU-bound fused generate-and-apply: unit = matrix entries applied per second by that kernel.
     # Headline denominator = an implementation-independent pipe peak from the guide's unit counts and clocks: the FP64
     # pipe for the complex128 kernel (64 DFMA lanes/clk/SM), the issue slots for the complex64 tensor-core generator;
@@ -472,9 +481,12 @@ def roofline_for(res: dict, hbm_gbs: float, peak_src: str) -> dict:
     entries = D * D * (1.0 - res["plan"]["cached_fraction"])
     rate = entries / (kern["procedural"] * 1e-3)
     key = (cfg["dtype"], "k1" if k == 1 else "kN")
+    two_sided = k > 1 and res["plan"].get("two_sided_pairs", 0) > 0   # block pairs generated once for both positions
+    if two_sided:
+        key = (cfg["dtype"], "kN2")
     cnt = SASS_COUNTS[key]
     issue_peak = ISSUE_LANES_PER_S / cnt["instr_per_entry"]
-    kname = "proc_single_kernel" if k == 1 else ("proc_multi_tc_kernel" if cfg["dtype"] == "c64" else "proc_multi_kernel")
+    kname = "proc_single_kernel" if k == 1 else (("pairs_tc_kernel<false>" if two_sided else "proc_multi_tc_kernel") if cfg["dtype"] == "c64" else "proc_multi_kernel")
     out = {"kernel": kname, "bound": "alu", "achieved": rate / 1e9, "unit": "Gentries/s", **ncu_traffic(kname, D),
            "issue_slot_peak": issue_peak / 1e9, "frac_of_issue_slots": rate / issue_peak,
            "instr_per_entry": cnt["instr_per_entry"], "sass_counts_source": cnt["source"],
@@ -493,6 +505,9 @@ def roofline_for(res: dict, hbm_gbs: float, peak_src: str) -> dict:
     if mix is not None:
         # second number: ceiling measured live on this GPU by a synthetic kernel with the inner loop's instruction counts
         name, entries_per_unit = mix
+        if two_sided:   # applied entries per generated entry: both positions of a pair from one generation
+            nb = D // cfg["B"]
+            entries_per_unit = nb * nb / (nb * nb - res["plan"]["two_sided_pairs"])
         mix_peak = res["pipe_rate"](name) * entries_per_unit
         out.update({"mix_ceiling": mix_peak / 1e9, "frac_of_mix_ceiling": rate / mix_peak,
                     "mix_ceiling_source": f"measured now: mfh_debug_pipe_rates({name}) x {entries_per_unit} entries per unit "
@@ -519,8 +534,13 @@ FP64_LANES_PER_S = 148 * 64 * 1.965e9
 SASS_COUNTS = {("c128", "k1"): {"instr_per_entry": 43.875, "fp64_per_entry": 16.0, "source": "profiles/r02_proc_single_sass.md"},
                ("c128", "kN"): {"instr_per_entry": 150.0, "fp64_per_entry": 0, "source": "DESIGN.md 6.3"},
                ("c64", "k1"): {"instr_per_entry": 40.0, "fp64_per_entry": 0, "source": "DESIGN.md 6.2"},
-               ("c64", "kN"): {"instr_per_entry": 64.0, "fp64_per_entry": 0, "source": "profiles/r02_proc_multi_tc_c3_ncu_full.md (2.14e9 warp instructions / 1.07e9 entries x 32 lanes)"}}
-MIX_OF = {("c128", "k1"): ("c128_pair", 2), ("c64", "kN"): ("c64_entry", 1)}
+               ("c64", "kN"): {"instr_per_entry": 64.0, "fp64_per_entry": 0, "source": "profiles/r02_proc_multi_tc_c3_ncu_full.md (2.14e9 warp instructions / 1.07e9 entries x 32 lanes)"},
+               # two-sided generator: everything the step executes, per APPLIED entry (generator 67.75 per generated entry
+               # in its SASS; epilogue, sum, MMA warps and barrier waits on top; the one-sided kernel for the diagonal blocks)
+               ("c64", "kN2"): {"instr_per_entry": 41.3, "fp64_per_entry": 0,
+                                "source": "profiles/r02_pairs_tc_generated_c3_ncu_full.md + r02_proc_multi_tc_diag_c3_ncu_full.md "
+                                          "((1.316e9 + 0.069e9) warp instructions / 1.07e9 applied entries x 32 lanes)"}}
+MIX_OF = {("c128", "k1"): ("c128_pair", 2), ("c64", "kN"): ("c64_entry", 1), ("c64", "kN2"): ("c64_entry", 1)}
 COMPONENTS_OF = {("c128", "k1"): {"kernels": ("comp_philox", "comp_philox_bm_c128", "comp_mac_c128"), "entries_per_pair": 2},
                  ("c64", "k1"): {"kernels": ("comp_philox", "comp_philox_bm_c64", "comp_mac_c64"), "entries_per_pair": 2}}
 
@@ -533,7 +553,9 @@ NCU_TRAFFIC = {("cached_kernel", 65536): (68.725132e9 + 5.106432e6, "profiles/r0
                ("cached_multi_tc_kernel", 32768): (8.595266e9 + 135.4e6, "profiles/r02_cached_multi_tc_c3_ncu_full.md"),
                ("cached_multi_kernel_c128", 32768): (17.203616e9 + 268.850432e6, "profiles/r02_cached_multi_c128_c3_ncu_full.md"),
                ("proc_single_kernel", 262144): (22.890752e6 + 631.663104e6, "profiles/r02_proc_single_c4_ncu_full.md"),
-               ("proc_multi_tc_kernel", 32768): (4.513792e6 + 81.728768e6, "profiles/r02_proc_multi_tc_c3_ncu_full.md")}
+               ("proc_multi_tc_kernel", 32768): (4.513792e6 + 81.728768e6, "profiles/r02_proc_multi_tc_c3_ncu_full.md"),
+               ("pairs_tc_kernel<false>", 32768): (7.638784e6 + 526.364672e6, "profiles/r02_pairs_tc_generated_c3_ncu_full.md"),
+               ("pairs_tc_kernel<true>", 32768): (4.221867e9 + 584.702208e6, "profiles/r02_pairs_tc_cached_c3_ncu_full.md")}
 
 
 def ncu_traffic(kernel: str, D: int) -> dict:

@@ -133,8 +133,10 @@ def test_c2_pair_cache_every_row():
 
 
 def test_c3_scan_every_row_generated_and_cached():
-    """C3 against a FULL oracle scan (all 32768 rows x 16 columns): the tcgen05 generator kernel (configs[2] as
-    written) and the same operator from cached complex64 blocks (bulk TMA -> TMEM -> tcgen05)."""
+    """C3 against a FULL oracle scan (all 32768 rows x 16 columns): the tcgen05 generator kernels (configs[2] as
+    written: the 496 off-diagonal block pairs generated once for both positions by the two-sided kernel, the 32
+    diagonal blocks by the one-sided one) and the same operator from cached complex64 blocks (bulk TMA -> TMEM ->
+    tcgen05)."""
     c = CONFIGS["C3"]
     D, B, k = c["D"], c["B"], c["k"]
     Psi = make_psi(D, c["psi_seed"], k=k, dtype="c64")
@@ -147,6 +149,8 @@ def test_c3_scan_every_row_generated_and_cached():
         assert plan["chosen"]["mode"] == mode
         if mode == "full":
             assert plan["chosen"]["cache_bytes"] == D * D * 8
+        else:
+            assert h.get_plan()["two_sided_pairs"] == (D // B) * (D // B - 1) // 2
         Phi = h.apply(to_dev(Psi), lambdas=lam).cpu().numpy()
         h.destroy()
         for v in range(k):
@@ -159,8 +163,9 @@ def test_c3_scan_every_row_generated_and_cached():
 
 
 def test_c3_scan_from_the_pair_cache_every_row():
-    """C3's operator from the Hermitian pair cache (4.4 GB instead of 8.6 GB): stored blocks used directly and, for
-    the mirrored positions, read a second time transposed by the same tensor-core kernel."""
+    """C3's operator from the Hermitian pair cache (4.4 GB instead of 8.6 GB): every stored off-diagonal block is read
+    ONCE per apply and serves both positions (two-sided cached kernel, unit-image layout); the diagonal blocks go
+    through the one-sided cached kernel."""
     c = CONFIGS["C3"]
     D, B, k = c["D"], c["B"], c["k"]
     Psi = make_psi(D, c["psi_seed"], k=k, dtype="c64")
@@ -170,6 +175,7 @@ def test_c3_scan_from_the_pair_cache_every_row():
     plan = h.plan("pairs", k=k)
     N = D // B
     assert plan["chosen"]["mode"] == "pairs" and plan["chosen"]["cache_bytes"] == N * (N + 1) // 2 * B * B * 8
+    assert h.get_plan()["two_sided_stored_pairs"] == N * (N - 1) // 2
     Phi = h.apply(to_dev(Psi), lambdas=lam).cpu().numpy()
     h.destroy()
     for v in range(k):

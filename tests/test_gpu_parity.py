@@ -219,6 +219,36 @@ def test_scan_c64_tensor_core_and_cuda_core_shapes(D, B, k):
         assert rel_l2(Phi[:, v], ref[:, v]) <= TOL["c64"], v
 
 
+def test_scan_c64_two_sided_tensor_core_kernels_and_their_fallbacks():
+    """complex64 k-vector plans use the Hermitian structure on the tensor cores (Eq. 11): a block
+    pair whose two positions are generated is generated ONCE (pairs_tc_kernel<false>), a stored pair of a pair cache is
+    read ONCE (pairs_tc_kernel<true>, unit-image layout); both need B/128 extra partial slots per block row and fall
+    back to the one-sided kernels when those do not fit the budget.  Same oracle, same tolerance, every path."""
+    D, B, k = 2048, 256, 16
+    nb = D // B
+    Psi = make_psi(D, 17, k=k, dtype="c64")
+    lam = 0.25 + lambda_grid(k)
+    ref = oracle.apply_scan(D, B, 8, 7, lam, Psi)
+    # mode, budget, generated pairs served two-sided, stored pairs served two-sided
+    cases = [("procedural", 0, nb * (nb - 1) // 2, 0),          # every off-diagonal pair generated once
+             ("procedural", 6_000_000, 0, 0),                   # the column-side slots do not fit: one-sided generation
+             ("pairs", 0, 0, nb * (nb - 1) // 2),               # every stored off-diagonal pair read once
+             ("pairs", 14_000_000, 0, 0)]                       # tight budget: as many stored pairs as fit WITHOUT the extra
+                                                                # slots (transposed second read), the rest generated one-sided
+    for mode, budget, n_gen, n_stored in cases:
+        h = mfh.Hamiltonian(D, B, 8, "c64", kind="diag_plus_gue", seed_h0=7)
+        h.plan(mode, k=k, hbm_budget_bytes=budget)
+        gp = h.get_plan()
+        assert (gp["two_sided_pairs"], gp["two_sided_stored_pairs"]) == (n_gen, n_stored), (mode, budget, gp)
+        if mode == "pairs" and budget:
+            assert 0 < gp["cached_blocks"] < nb * (nb + 1) // 2, gp
+        h.debug_poison()                                          # a slot that is read but not written turns the result into NaN
+        Phi = h.apply(to_dev(Psi), lambdas=lam).cpu().numpy()
+        for v in range(k):
+            assert rel_l2(Phi[:, v], ref[:, v]) <= TOL["c64"], (mode, budget, v)
+        h.destroy()
+
+
 @pytest.mark.parametrize("mode,budget", [("full", 0), ("partial", 12e6), ("partial", 24e6)])
 @pytest.mark.parametrize("dtype,k", [("c64", 16), ("c64", 5), ("c128", 16), ("c128", 8), ("c128", 3), ("c128", 2)])
 def test_scan_cached_blocks_k_vectors(mode, budget, dtype, k):
