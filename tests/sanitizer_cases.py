@@ -99,7 +99,8 @@ def main(only=None):
             h.destroy()
 
     if want("scan"):
-        # k = 16 complex64 scan: proc_multi_tc_kernel (tcgen05, A generated into TMEM), cached_multi_tc_kernel (bulk TMA),
+        # k = 16 complex64 scan: pairs_tc_kernel<false> (block pairs generated once for both positions) + proc_multi_tc_kernel
+        # (diagonal blocks; tcgen05, A generated into TMEM), cached_multi_tc_kernel (bulk TMA), pairs_tc_kernel<true> (pair cache),
         # and a partial k-vector plan (both in one apply)
         D, B, k = 2048, 256, 16
         Psi = make_psi(D, 9, k=k, dtype="c64")
