@@ -304,7 +304,9 @@ MFH_API int mfh_destroy(mfh_handle h);
 /* Thread-local message of the last failing call ("" if none). */
 MFH_API const char* mfh_last_error(void);
 
-/* JSON description of the committed plan (mode, B, cached blocks, bytes, launches per apply). */
+/* JSON description of the committed plan (mode, B, cached blocks, bytes, launches per apply; "two_sided_pairs" /
+ * "two_sided_stored_pairs": block pairs of a complex64 k-vector plan that are generated / read from the pair cache
+ * ONCE for both positions by the two-sided tensor-core kernels). */
 MFH_API int mfh_get_plan(mfh_handle h, char* json_out, size_t json_cap);
 
 /* ---- system-bath Hamiltonian (the paper's own workload shape, R19) -------

@@ -87,7 +87,7 @@ def test_lanczos_argument_errors_and_c64():
     assert abs(e0 - r0) < 1e-4 and abs(e1 - r1) < 1e-4
 
 
-@pytest.mark.parametrize("dtype,mode", [("c128", "procedural"), ("c128", "full"), ("c64", "procedural"), ("c64", "full")])
+@pytest.mark.parametrize("dtype,mode", [("c128", "procedural"), ("c128", "full"), ("c64", "procedural"), ("c64", "full"), ("c64", "pairs")])
 def test_coupling_scan_propagation_k_columns(dtype, mode):
     """mfh_chebyshev_scan: k states propagated under k Hamiltonians H_v = diag(h0) + lambda_v V at once (one k-vector
     plan, every block generated or read once per term), against the exact eigh propagator of each H_v and the
