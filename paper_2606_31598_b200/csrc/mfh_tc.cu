@@ -49,6 +49,12 @@ __device__ __forceinline__ uint64_t umma_desc(uint32_t addr)
            (1ull << 46);
 }
 
+__device__ __forceinline__ uint64_t umma_desc_sbo(uint32_t addr, int sbo)
+{
+    return (uint64_t)((addr >> 4) & 0x3fffu) | ((uint64_t)(TC_LBO >> 4) << 16) | ((uint64_t)(sbo >> 4) << 32) |
+           (1ull << 46);
+}
+
 // Instruction descriptor: D = F32, A = B = TF32, both K-major, M = 128, N = 32 or 64.
 constexpr uint32_t tc_idesc(int n)
 {
@@ -433,6 +439,26 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32])
     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 }
 
+// Row side of the two-sided kernels: INTERLEAVED operand layout (the cached kernel's, 6.5): K index k' = 2 c + part, so
+// a thread's (re, im) pairs go to TMEM and to the column side's shared-memory image from the same register pairs.
+// A stage: [A_hi: 32 columns][A_lo: 32 columns]; psi images B_hi | B_lo adjacent (N = 64 for A_hi, N = 32 for A_lo):
+//   row v:      (Re Psi_cv, -Im Psi_cv) at k' = (2c, 2c+1)   -> Re Phi;   row 16 + v: (Im Psi_cv, Re Psi_cv) -> Im Phi.
+constexpr int T2_BT = TC_N * 32 * 4;          // one psi image: 32 rows x 32 k' floats = 4 KB (T2_BT x 2 = TC_STAGE)
+constexpr int T2_BSBO = (32 / 4) * 128;       // 1 KB between 8-row groups of a psi image
+__device__ __forceinline__ void t2_psi_image(unsigned char* stage, int v, int qb, float2 x)
+{
+    float* b = reinterpret_cast<float*>(stage);
+    const int o_re = ((v & 7) * 16 + (v >> 3) * T2_BSBO + (qb >> 1) * 128 + (qb & 1) * 8) / 4;
+    const int o_im = o_re + 2 * T2_BSBO / 4;
+    float prh, prl, pih, pil;
+    split_tf32(x.x, prh, prl);
+    split_tf32(x.y, pih, pil);
+    *reinterpret_cast<float2*>(b + o_re) = make_float2(prh, -pih);
+    *reinterpret_cast<float2*>(b + o_im) = make_float2(pih, prh);
+    *reinterpret_cast<float2*>(b + T2_BT / 4 + o_re) = make_float2(prl, -pil);
+    *reinterpret_cast<float2*>(b + T2_BT / 4 + o_im) = make_float2(pil, prl);
+}
+
 // Generator group g (256 threads): tiles 2u + g of every unit u.  Row side exactly as tc_generate<+1>; column side:
 // the thread's 8 entries of row p go to the unit buffer as (Re, Im) pairs at
 //   [(p % 64) / 16] 8 KB  +  [p / 64] 4 KB  +  [column / 8] 1 KB  +  [column % 8] 128 B  +  16-byte chunk ((p % 16) / 2) ^ (column % 8)  +  (p % 2) 8 B
@@ -445,8 +471,6 @@ __device__ __forceinline__ void t2_generate(const T2Params& P, unsigned char* ub
     const uint32_t a_lane = d_tmem + ((uint32_t)(p & ~31) << 16);
     // (vector, column) of this thread's psi element: a warp covers 8 vectors x 4 columns = 32 distinct banks of a B image
     const int v = (lt & 7) | ((lt >> 2) & 8), qb = ((lt >> 3) & 3) | ((lt >> 6) << 2), k = P.k;
-    const int o_re = ((v & 7) * 16 + (v >> 3) * TC_SBO + (qb >> 2) * 128 + (qb & 3) * 4) / 4;
-    const int o_im = o_re + 2 * TC_SBO / 4;
     const int n_units = P.B / T2_UNIT_COLS;
     const uint32_t chunk = (uint32_t)(p & 15) >> 1;
     const uint32_t m_row = (uint32_t)((p & 63) >> 4) * 8192u + (uint32_t)(p >> 6) * 4096u + (uint32_t)(p & 1) * 8u;
@@ -460,7 +484,7 @@ __device__ __forceinline__ void t2_generate(const T2Params& P, unsigned char* ub
             const uint32_t use = gt >> 1;
             const uint32_t j0 = (uint32_t)cb * P.B + (2 * u + g) * TC_TQ;
             const float2 x = (v < k && qb < TC_TQ) ? P.psi[(size_t)(j0 + qb) * k + v] : float2{0.f, 0.f};
-            float rh[TC_NG][4], rl[TC_NG][4], ih[TC_NG][4], il[TC_NG][4];
+            float2 ent[TC_NG][4], elo[TC_NG][4];   // (re, im) of the 8 entries and their low parts x - trunc(x)
 #pragma unroll
             for (int gg = 0; gg < TC_NG; ++gg)
 #pragma unroll
@@ -468,14 +492,10 @@ __device__ __forceinline__ void t2_generate(const T2Params& P, unsigned char* ub
                     const uint32_t j = j0 + 4 * (gsel + 2 * gg) + e;
                     float hr, hi;
                     entry_upper<float>(P.G, nullptr, i, j, hr, hi);
-                    rh[gg][e] = hr;
-                    rl[gg][e] = hr - __uint_as_float(__float_as_uint(hr) & 0xffffe000u);
-                    ih[gg][e] = hi;
-                    il[gg][e] = hi - __uint_as_float(__float_as_uint(hi) & 0xffffe000u);
+                    ent[gg][e] = make_float2(hr, hi);
+                    elo[gg][e] = make_float2(hr - __uint_as_float(__float_as_uint(hr) & 0xffffe000u),
+                                             hi - __uint_as_float(__float_as_uint(hi) & 0xffffe000u));
                 }
-            float prh, prl, pih, pil;
-            split_tf32(x.x, prh, prl);
-            split_tf32(x.y, pih, pil);
             if (use > 0) mbar_wait(&bar.mempty[s2], (use - 1) & 1);      // column-side MMAs of the unit two back are done
             unsigned char* ub = ubuf + s2 * T2_UNIT;
 #pragma unroll
@@ -484,28 +504,20 @@ __device__ __forceinline__ void t2_generate(const T2Params& P, unsigned char* ub
                 for (int e = 0; e < 4; ++e) {
                     const uint32_t c8 = 4u * gsel + e;
                     const uint32_t off = m_row + (uint32_t)(2 * g + gg) * 1024u + c8 * 128u + ((chunk ^ c8) << 4);
-                    *reinterpret_cast<float2*>(ub + off) = make_float2(rh[gg][e], ih[gg][e]);
-                    *reinterpret_cast<float2*>(ub + T2_IMG + off) = make_float2(rl[gg][e], il[gg][e]);
+                    *reinterpret_cast<float2*>(ub + off) = ent[gg][e];
+                    *reinterpret_cast<float2*>(ub + T2_IMG + off) = elo[gg][e];
                 }
             // (the row side second: the MMAs of this group's previous tile finish during the stores above)
             if (gt > 0) mbar_wait(&bar.dempty[g], (gt - 1) & 1);   // the row-side MMAs of this group's previous tile are done
-            const int stg = g;
 #pragma unroll
             for (int gg = 0; gg < TC_NG; ++gg) {
-                const uint32_t ta = a_lane + (uint32_t)(T2_COL_ASTAGE + stg * TC_A_STAGE_COLS + 4 * (gsel + 2 * gg));
-                tmem_st4(ta + 0 * TC_TQ, rh[gg][0], rh[gg][1], rh[gg][2], rh[gg][3]);
-                tmem_st4(ta + 1 * TC_TQ, rl[gg][0], rl[gg][1], rl[gg][2], rl[gg][3]);
-                tmem_st4(ta + 2 * TC_TQ, ih[gg][0], ih[gg][1], ih[gg][2], ih[gg][3]);
-                tmem_st4(ta + 3 * TC_TQ, il[gg][0], il[gg][1], il[gg][2], il[gg][3]);
+                const uint32_t ta = a_lane + (uint32_t)(T2_COL_ASTAGE + g * TC_A_STAGE_COLS + 8 * (gsel + 2 * gg));
+                tmem_st4(ta, ent[gg][0].x, ent[gg][0].y, ent[gg][1].x, ent[gg][1].y);
+                tmem_st4(ta + 4, ent[gg][2].x, ent[gg][2].y, ent[gg][3].x, ent[gg][3].y);
+                tmem_st4(ta + 32, elo[gg][0].x, elo[gg][0].y, elo[gg][1].x, elo[gg][1].y);
+                tmem_st4(ta + 36, elo[gg][2].x, elo[gg][2].y, elo[gg][3].x, elo[gg][3].y);
             }
-            if (qb < TC_TQ) {
-                float* b = reinterpret_cast<float*>(bimg + stg * TC_STAGE);
-                constexpr int BT = TC_B_TILE / 4;
-                b[0 * BT + o_re] = prh;  b[0 * BT + o_im] = pih;
-                b[1 * BT + o_re] = prl;  b[1 * BT + o_im] = pil;
-                b[2 * BT + o_re] = -pih; b[2 * BT + o_im] = prh;
-                b[3 * BT + o_re] = -pil; b[3 * BT + o_im] = prl;
-            }
+            t2_psi_image(bimg + g * TC_STAGE, v, qb, x);
             asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -531,8 +543,6 @@ __device__ __forceinline__ void t2_convert(const T2Params& P, unsigned char* raw
     const uint32_t a_lane = d_tmem + ((uint32_t)(p & ~31) << 16);
     // (vector, column) of this thread's psi element: a warp covers 8 vectors x 4 columns = 32 distinct banks of a B image
     const int v = (lt & 7) | ((lt >> 2) & 8), qb = ((lt >> 3) & 3) | ((lt >> 6) << 2), k = P.k;
-    const int o_re = ((v & 7) * 16 + (v >> 3) * TC_SBO + (qb >> 2) * 128 + (qb & 3) * 4) / 4;
-    const int o_im = o_re + 2 * TC_SBO / 4;
     const int n_units = P.B / T2_UNIT_COLS;
     const uint32_t chunk = (uint32_t)(p & 15) >> 1;
     const uint32_t m_row = (uint32_t)((p & 63) >> 4) * 8192u + (uint32_t)(p >> 6) * 4096u + (uint32_t)(p & 1) * 8u;
@@ -547,7 +557,7 @@ __device__ __forceinline__ void t2_convert(const T2Params& P, unsigned char* raw
             const float2 x = (v < k && qb < TC_TQ) ? P.psi[(size_t)(j0 + qb) * k + v] : float2{0.f, 0.f};   // in flight during the wait
             mbar_wait(&bar.raw_full[st], (gt / T2C_STAGES) & 1);
             const unsigned char* raw = rawbuf + st * T2_IMG;
-            float rh[TC_NG][4], rl[TC_NG][4], ih[TC_NG][4], il[TC_NG][4];
+            float2 ent[TC_NG][4], elo[TC_NG][4];
             uint32_t off[TC_NG][4];
 #pragma unroll
             for (int gg = 0; gg < TC_NG; ++gg)
@@ -555,43 +565,30 @@ __device__ __forceinline__ void t2_convert(const T2Params& P, unsigned char* raw
                 for (int e = 0; e < 4; ++e) {
                     const uint32_t c8 = 4u * gsel + e;
                     off[gg][e] = m_row + (uint32_t)(2 * g + gg) * 1024u + c8 * 128u + ((chunk ^ c8) << 4);
-                    const float2 w = *reinterpret_cast<const float2*>(raw + off[gg][e]);
-                    rh[gg][e] = w.x;
-                    ih[gg][e] = w.y;
+                    ent[gg][e] = *reinterpret_cast<const float2*>(raw + off[gg][e]);
                 }
 #pragma unroll
             for (int gg = 0; gg < TC_NG; ++gg)
 #pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                    rl[gg][e] = rh[gg][e] - __uint_as_float(__float_as_uint(rh[gg][e]) & 0xffffe000u);
-                    il[gg][e] = ih[gg][e] - __uint_as_float(__float_as_uint(ih[gg][e]) & 0xffffe000u);
-                }
-            float prh, prl, pih, pil;
-            split_tf32(x.x, prh, prl);
-            split_tf32(x.y, pih, pil);
+                for (int e = 0; e < 4; ++e)
+                    elo[gg][e] = make_float2(ent[gg][e].x - __uint_as_float(__float_as_uint(ent[gg][e].x) & 0xffffe000u),
+                                             ent[gg][e].y - __uint_as_float(__float_as_uint(ent[gg][e].y) & 0xffffe000u));
             if (use > 0) mbar_wait(&bar.mempty[s2], (use - 1) & 1);   // the column-side MMAs of the unit two back are done
             unsigned char* lo = lobuf + s2 * T2_IMG;
 #pragma unroll
             for (int gg = 0; gg < TC_NG; ++gg)
 #pragma unroll
-                for (int e = 0; e < 4; ++e) *reinterpret_cast<float2*>(lo + off[gg][e]) = make_float2(rl[gg][e], il[gg][e]);
+                for (int e = 0; e < 4; ++e) *reinterpret_cast<float2*>(lo + off[gg][e]) = elo[gg][e];
             if (gt > 0) mbar_wait(&bar.dempty[g], (gt - 1) & 1);      // the row-side MMAs of this group's previous tile are done
 #pragma unroll
             for (int gg = 0; gg < TC_NG; ++gg) {
-                const uint32_t ta = a_lane + (uint32_t)(T2_COL_ASTAGE + g * TC_A_STAGE_COLS + 4 * (gsel + 2 * gg));
-                tmem_st4(ta + 0 * TC_TQ, rh[gg][0], rh[gg][1], rh[gg][2], rh[gg][3]);
-                tmem_st4(ta + 1 * TC_TQ, rl[gg][0], rl[gg][1], rl[gg][2], rl[gg][3]);
-                tmem_st4(ta + 2 * TC_TQ, ih[gg][0], ih[gg][1], ih[gg][2], ih[gg][3]);
-                tmem_st4(ta + 3 * TC_TQ, il[gg][0], il[gg][1], il[gg][2], il[gg][3]);
+                const uint32_t ta = a_lane + (uint32_t)(T2_COL_ASTAGE + g * TC_A_STAGE_COLS + 8 * (gsel + 2 * gg));
+                tmem_st4(ta, ent[gg][0].x, ent[gg][0].y, ent[gg][1].x, ent[gg][1].y);
+                tmem_st4(ta + 4, ent[gg][2].x, ent[gg][2].y, ent[gg][3].x, ent[gg][3].y);
+                tmem_st4(ta + 32, elo[gg][0].x, elo[gg][0].y, elo[gg][1].x, elo[gg][1].y);
+                tmem_st4(ta + 36, elo[gg][2].x, elo[gg][2].y, elo[gg][3].x, elo[gg][3].y);
             }
-            if (qb < TC_TQ) {
-                float* b = reinterpret_cast<float*>(bimg + g * TC_STAGE);
-                constexpr int BT = TC_B_TILE / 4;
-                b[0 * BT + o_re] = prh;  b[0 * BT + o_im] = pih;
-                b[1 * BT + o_re] = prl;  b[1 * BT + o_im] = pil;
-                b[2 * BT + o_re] = -pih; b[2 * BT + o_im] = prh;
-                b[3 * BT + o_re] = -pil; b[3 * BT + o_im] = prl;
-            }
+            t2_psi_image(bimg + g * TC_STAGE, v, qb, x);
             asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
@@ -640,19 +637,14 @@ __device__ __forceinline__ void t2_row_mma(const T2Params& P, unsigned char* bim
             if (t == 0 && items_done > 0) mbar_wait(&bar.dacc_empty, (items_done - 1) & 1);   // the epilogue has read the accumulator
             asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
             if (elect_one()) {
-                const uint64_t bd = umma_desc(smem_u32(bimg + stg * TC_STAGE));   // the start-address field takes plain additions
+                // interleaved layout: 4 K-steps of 8 k' = 4 columns x (re, im); A_hi x [B_hi | B_lo] (N = 64), A_lo x B_hi (N = 32)
+                const uint64_t bd = umma_desc_sbo(smem_u32(bimg + stg * TC_STAGE), T2_BSBO);   // the start-address field takes plain additions
                 const uint32_t a0 = d_tmem + (uint32_t)(T2_COL_ASTAGE + stg * TC_A_STAGE_COLS);
 #pragma unroll
-                for (int ks = 0; ks < TC_TQ / 8; ++ks) {
-                    const uint32_t ko = ks * 2 * TC_LBO;
-                    const uint32_t er_h = a0 + 0 * TC_TQ + 8 * ks, er_l = a0 + 1 * TC_TQ + 8 * ks;
-                    const uint32_t ei_h = a0 + 2 * TC_TQ + 8 * ks, ei_l = a0 + 3 * TC_TQ + 8 * ks;
-                    const uint64_t b1 = bd + (uint64_t)((0 * TC_B_TILE + ko) >> 4);
-                    const uint64_t b2 = bd + (uint64_t)((2 * TC_B_TILE + ko) >> 4);
-                    umma_tf32_ts<64>(d_tmem + T2_COL_DACC, er_h, b1, (t | ks) != 0);
-                    umma_tf32_ts<32>(d_tmem + T2_COL_DACC, er_l, b1, 1);
-                    umma_tf32_ts<64>(d_tmem + T2_COL_DACC, ei_h, b2, 1);
-                    umma_tf32_ts<32>(d_tmem + T2_COL_DACC, ei_l, b2, 1);
+                for (int ks = 0; ks < 4; ++ks) {
+                    const uint64_t b = bd + (uint64_t)((ks * 2 * TC_LBO) >> 4);
+                    umma_tf32_ts<64>(d_tmem + T2_COL_DACC, a0 + 8 * ks, b, (t | ks) != 0);
+                    umma_tf32_ts<32>(d_tmem + T2_COL_DACC, a0 + 32 + 8 * ks, b, 1);
                 }
                 umma_commit(&bar.dempty[g]);
                 if (t == n_tiles - 1) umma_commit(&bar.ddone);
@@ -1015,12 +1007,6 @@ constexpr int CT_A_STAGE_COLS = 2 * CT_KF;    // A_hi, A_lo: 32 TMEM columns eac
 constexpr int CT_THREADS = 32 * (TC_GEN_WARPS + 2);   // 8 converter warps, MMA warp, TMA warp
 constexpr int CT_PSI = (CT_KF / 2) * 16 * 8;  // psi rows of one tile: 16 columns x <= 16 vectors x 8 B
 constexpr int CT_SMEM = CT_STAGES * (CT_RAW + CT_PSI) + CT_TSTAGES * CT_BSTAGE + 1024;   // + alignment slack
-
-__device__ __forceinline__ uint64_t umma_desc_sbo(uint32_t addr, int sbo)
-{
-    return (uint64_t)((addr >> 4) & 0x3fffu) | ((uint64_t)(TC_LBO >> 4) << 16) | ((uint64_t)(sbo >> 4) << 32) |
-           (1ull << 46);
-}
 
 struct CtParams {
     int32_t B, n_blk, k, slot_multi;
