@@ -65,9 +65,9 @@ enum { MFH_MODE_AUTO = 0, MFH_MODE_PROCEDURAL = 1, MFH_MODE_PARTIAL = 2, MFH_MOD
         * allows (nearest block diagonals first), the rest is generated.  Half the memory of FULL.  One vector: every
         * loaded entry is used for both positions (half the bytes per apply as well).  k vectors (complex64, B % 128
         * == 0): a stored off-diagonal block is read ONCE per apply and serves both positions on the tensor cores (row
-        * side from TMEM, column side with the block as shared-memory operand; half the bytes of FULL) -- on a
-        * partitioned handle, or when the extra partial slots do not fit the budget, the mirrored position is served by
-        * a second, transposed read instead (same bytes as FULL).  complex128 k-vector plans do not support the pair
+        * side from TMEM, column side with the block as shared-memory operand; half the bytes of FULL) -- when the
+        * extra partial slots do not fit the budget, the mirrored position is served by a second, transposed read
+        * instead (same bytes as FULL).  complex128 k-vector plans do not support the pair
         * cache. */
        MFH_MODE_PAIRS = 4 };
 

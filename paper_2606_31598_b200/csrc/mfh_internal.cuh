@@ -201,7 +201,7 @@ int launch_partial_overlap(mfh_handle h, const void* psi, cudaStream_t st);   //
 int launch_proc_multi(mfh_handle h, const void* psi, cudaStream_t st);
 bool tc_multi_supported(mfh_handle h);                                   // mfh_tc.cu
 int launch_proc_multi_tc(mfh_handle h, const void* psi, cudaStream_t st);
-bool tc_pairs_supported(int dtype, int k, int B, int part_world);        // two-sided tensor-core generator
+bool tc_pairs_supported(int dtype, int k, int B);        // two-sided tensor-core generator
 bool tc_cached_multi_supported(int dtype, int k, int B);
 bool cached_multi_c128_supported(int dtype, int k, int B);               // mfh_cached.cu
 int launch_cached_multi_tc(mfh_handle h, const void* psi, cudaStream_t st);

@@ -263,7 +263,9 @@ void build_tables(Plan& p, int64_t D, int dtype, int sm_count)
     p.slot_mcol0 = -1;
     p.pair_units = false;
     const int tcS = p.B / 128;
-    if (p.allow_tc_pairs && tc_pairs_supported(dtype, p.k, p.B, part.world)) {
+    if (p.allow_tc_pairs && tc_pairs_supported(dtype, p.k, p.B)) {
+        // (partitioned handles: only pairs whose two positions this rank owns -- all of its pairs under MFH_PART_PAIRS,
+        // the pairs inside its slab of block rows under MFH_PART_ROWS; uncached() is false for positions not owned)
         for (int n = 0; n < N; ++n)
             for (int m = n + 1; m < N; ++m) {
                 if (p.gen_two_sided && uncached(n, m) && uncached(m, n)) {

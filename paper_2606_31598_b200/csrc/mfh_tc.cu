@@ -891,9 +891,9 @@ __global__ void __launch_bounds__(CACHED ? T2C_THREADS : T2_THREADS, 1) pairs_tc
     if (w == T2_W_DMMA) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(d_tmem), "n"(512) : "memory");
 }
 
-bool tc_pairs_supported(int dtype, int k, int B, int part_world)
+bool tc_pairs_supported(int dtype, int k, int B)
 {
-    return dtype == MFH_C64 && k > 1 && k <= 16 && B % TC_TP == 0 && part_world <= 1;
+    return dtype == MFH_C64 && k > 1 && k <= 16 && B % TC_TP == 0;
 }
 
 static void t2_common_params(mfh_handle h, const void* psi, T2Params& P)
@@ -1030,7 +1030,7 @@ __global__ void __launch_bounds__(CT_THREADS, 2) cached_multi_tc_kernel(const Ct
     const int n = (int)(i_base / (uint32_t)P.B);
     if (P.skip && P.skip[n * P.n_blk + m]) return;   // both positions of a stored pair: pairs_tc_kernel<true>, from one read
     int32_t slot = P.cache_slot[n * P.n_blk + m];
-    // Hermitian pair cache (MFH_MODE_PAIRS with k > 1) without the unit-image layout (partitioned handles): position (n,m) marked -2 is served by the stored canonical block
+    // Hermitian pair cache (MFH_MODE_PAIRS with k > 1) without the unit-image layout (no room for the column-side slots): position (n,m) marked -2 is served by the stored canonical block
     // C = H^[m,n]: phi^[n] += C^dagger psi^[m].  The CTA's 128 output rows are 128 COLUMNS of C; it reads C a second
     // time, transposed (TR): a stage is 16 rows of C x those 128 columns = eight 2 KB pieces of eight neighbouring
     // tiles.  (This halves the MEMORY of a k-vector operator, not the bytes per apply: DESIGN.md 6.5.)
