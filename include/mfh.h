@@ -211,6 +211,31 @@ MFH_API int mfh_apply_timed(mfh_handle h, const void* psi_dev, void* phi_dev, in
 MFH_API int mfh_timing_begin(mfh_handle h, int32_t n_applies);
 MFH_API int mfh_timing_end(mfh_handle h, float* ms_out, int32_t* n_recorded, void* stream);
 
+/* Allocation-free entry point: phi = lambda * V(seed) psi for ONE complex128 vector, V the seeded GUE operator of
+ * mfh_create(kind = MFH_SRC_GUE) (Eq. 4-5; entries as BASELINE.json configs[0]), generated on the fly.  For
+ * callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it):
+ * no handle and no plan; this call and everything below it calls no cudaMalloc, no cudaFree and no allocating library
+ * routine.  Its scratch (generator table + 16 partial sums per row, added in a fixed order: deterministic, no atomics)
+ * is ONE file-scope device array of 32 KB + 16 * MFH_STATIC_MAX_D * 16 B = 4.03 MB that every GPU which loads the
+ * library holds until the process exits.
+ *   D         matrix dimension: a multiple of 128, 128 <= D <= MFH_STATIC_MAX_D; a larger D is refused with
+ *             MFH_ERR_INVALID_ARG and a message that names the limit (use mfh_create / mfh_plan / mfh_apply there)
+ *   psi_dev   D complex128 (interleaved re, im), DEVICE pointer, 16-byte aligned, caller-owned, read only
+ *   phi_dev   D complex128, DEVICE pointer, 16-byte aligned, caller-owned, overwritten; must not alias psi_dev
+ *   stream    cudaStream_t of the CURRENT device (NULL = default stream); the call is asynchronous
+ * The result equals mfh_apply on a procedural complex128 plan of the same (D, seed, lambda) up to the summation order
+ * (<= 1e-11 relative L2, tests/test_zz_no_alloc.py).
+ * SHARED STATE: all calls on one device use the same scratch array, which keeps the last call's contents (nothing in
+ * it has to start at zero: every value a call reads it has written itself).  Calls that overlap on the GPU -- two
+ * streams, or two host threads on different streams -- race on it: issue them on one stream or order them with events.
+ * Host-side set-up is guarded by a mutex.  The first call on a device resolves the array's device address
+ * (cudaGetSymbolAddress); a call whose D differs from the previous call's on that device re-uploads the 20 KB generator
+ * table with a stream-ordered cudaMemcpyAsync from host memory.
+ * Errors: MFH_ERR_INVALID_ARG (NULL / aliased pointers, D out of range or not a multiple of 128), MFH_ERR_UNSUPPORTED
+ * (device ordinal >= 64), MFH_ERR_CUDA. */
+#define MFH_STATIC_MAX_D 16384
+MFH_API int mfh_apply_static(int64_t D, uint64_t seed, double lambda, const void* psi_dev, void* phi_dev, void* stream);
+
 /* Same as mfh_apply but with HOST buffers: copies psi to the device, applies, copies phi back and
  * synchronises `stream` (the end-to-end call bench.py times).  Host buffers should be pinned. */
 MFH_API int mfh_apply_host(mfh_handle h, const void* psi_host, void* phi_host, int32_t k,

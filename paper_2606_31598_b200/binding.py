@@ -34,7 +34,7 @@ SYMBOLS = ["mfh_create", "mfh_plan_analytic", "mfh_plan_node_analytic", "mfh_pla
            "mfh_chebyshev", "mfh_chebyshev_imag", "mfh_chebyshev_scan", "mfh_chebyshev_steps", "mfh_lanczos_bounds", "mfh_destroy", "mfh_last_error", "mfh_get_plan", "mfh_debug_philox",
            "mfh_materialize_block", "mfh_debug_h0", "mfh_debug_bessel_j", "mfh_debug_poison", "mfh_debug_selfcheck", "mfh_debug_corrupt_guard", "mfh_debug_pipe_rates", "mfh_sb_create", "mfh_sb_plan", "mfh_sb_apply",
            "mfh_sb_destroy", "mfh_set_partition", "mfh_get_partition_rows", "mfh_set_exchange", "mfh_debug_read_bandwidth", "mfh_set_source_params", "mfh_set_block", "mfh_surrogate_theta_size", "mfh_surrogate_fit",
-           "mfh_surrogate_predict", "mfh_surrogate_loss_grad", "mfh_surrogate_features", "mfh_plan_hybrid"]
+           "mfh_surrogate_predict", "mfh_surrogate_loss_grad", "mfh_surrogate_features", "mfh_plan_hybrid", "mfh_apply_static"]
 
 _lib = None
 
@@ -63,6 +63,7 @@ def lib():
     L.mfh_plan.argtypes = [vp, i32, i32, i64, i64, i32, vp, cp, sz]
     L.mfh_apply.argtypes = [vp, vp, vp, i32, ctypes.POINTER(dbl), vp]
     L.mfh_apply_host.argtypes = [vp, vp, vp, i32, ctypes.POINTER(dbl), vp]
+    L.mfh_apply_static.argtypes = [i64, u64, dbl, vp, vp, vp]
     L.mfh_apply_timed.argtypes = [vp, vp, vp, i32, ctypes.POINTER(dbl), vp, ctypes.POINTER(ctypes.c_float)]
     L.mfh_timing_begin.argtypes = [vp, i32]
     L.mfh_timing_end.argtypes = [vp, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(i32), vp]
@@ -370,6 +371,21 @@ class SystemBath:
             self.destroy()
         except Exception:
             pass
+
+
+STATIC_MAX_D = 16384   # include/mfh.h MFH_STATIC_MAX_D
+
+
+def apply_static(D: int, seed: int, lam: float, psi, phi=None):
+    """phi = lam * V(seed) psi through mfh_apply_static: no handle, no plan, no allocation inside the library (the
+    output tensor is the caller's; one is made here only when none is passed).  complex128, one vector, D <= STATIC_MAX_D."""
+    import torch
+    assert psi.is_cuda and psi.dtype == torch.complex128 and psi.is_contiguous() and psi.numel() == D
+    if phi is None:
+        phi = torch.empty_like(psi)
+    assert phi.is_cuda and phi.dtype == torch.complex128 and phi.is_contiguous() and phi.numel() == D
+    _check(lib().mfh_apply_static(int(D), int(seed), float(lam), psi.data_ptr(), phi.data_ptr(), _stream()))
+    return phi
 
 
 def debug_philox(seed: int, stream_id: int, i, j):
