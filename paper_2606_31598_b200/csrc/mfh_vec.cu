@@ -2,6 +2,7 @@
 // H0 + lambda V epilogue (BASELINE.json configs[2]) and the Chebyshev recurrence updates
 // (Eq. 41-44).  All are HBM-trivial next to the O(D^2) apply.
 #include <algorithm>
+#include <cstdint>
 #include "mfh_internal.cuh"
 
 namespace mfh {
@@ -86,6 +87,60 @@ __global__ void __launch_bounds__(256) reduce_kernel(int64_t D, int32_t B, int32
     }
 }
 
+// complex64 with many slots (the k-vector plans with column-side slots, C3: 32 .. 280 per block row): the same fixed
+// summation order, two neighbouring elements per thread (one 16-byte load per slot, eight in flight).  One CTA per 64
+// element pairs, the LAST block rows first: the slot count grows with the block row, and the hardware scheduler
+// balances a heaviest-first list of CTAs.
+__global__ void __launch_bounds__(256) reduce2_kernel_c64(int64_t D, int32_t B, int32_t k, int32_t n_slots,
+                                                          const int32_t* __restrict__ slot_list, const float2* __restrict__ work,
+                                                          const float* __restrict__ h0, const float2* __restrict__ psi,
+                                                          float2* __restrict__ phi, LamArr lam)
+{
+    constexpr int G = RED_G, EPB = 256 / G;              // element PAIRS per CTA
+    __shared__ double part[G][EPB][4];
+    const int64_t total = D * k;                         // k even: a pair never crosses a row
+    const int ex = threadIdx.x % EPB, g = threadIdx.x / EPB;
+    const int64_t e = 2 * (((int64_t)gridDim.x - 1 - blockIdx.x) * EPB + ex);
+    const bool live = e < total;
+    const int64_t i = live ? e / k : 0;
+    const int32_t* list = slot_list + (size_t)(i / B) * (n_slots + 1);
+    const int head = list[0];
+    const int cnt = head & SLOT_COUNT_MASK;
+    const int chunk = (cnt + G - 1) / G;
+    int t = g * chunk;
+    const int t_end = live ? min(cnt, t + chunk) : 0;
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+    for (; t + 8 <= t_end; t += 8) {
+        float4 x[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) x[u] = *reinterpret_cast<const float4*>(work + (size_t)list[1 + t + u] * total + e);
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            s0 += (double)x[u].x; s1 += (double)x[u].y; s2 += (double)x[u].z; s3 += (double)x[u].w;
+        }
+    }
+    for (; t < t_end; ++t) {
+        const float4 x = *reinterpret_cast<const float4*>(work + (size_t)list[1 + t] * total + e);
+        s0 += (double)x.x; s1 += (double)x.y; s2 += (double)x.z; s3 += (double)x.w;
+    }
+    part[g][ex][0] = s0; part[g][ex][1] = s1; part[g][ex][2] = s2; part[g][ex][3] = s3;
+    __syncthreads();
+    if (g != 0 || !live || (head & SLOT_SKIP_ROW)) return;
+#pragma unroll
+    for (int gg = 1; gg < G; ++gg) {
+        s0 += part[gg][ex][0]; s1 += part[gg][ex][1]; s2 += part[gg][ex][2]; s3 += part[gg][ex][3];
+    }
+    const int v = (int)(e - i * k);
+    double o0 = lam.v[v] * s0, o1 = lam.v[v] * s1, o2 = lam.v[v + 1] * s2, o3 = lam.v[v + 1] * s3;
+    if (h0 && !(head & SLOT_NO_H0)) {
+        const float4 p = *reinterpret_cast<const float4*>(psi + e);
+        const double d = (double)h0[i];
+        o0 = fma(d, (double)p.x, o0); o1 = fma(d, (double)p.y, o1);
+        o2 = fma(d, (double)p.z, o2); o3 = fma(d, (double)p.w, o3);
+    }
+    *reinterpret_cast<float4*>(phi + e) = make_float4((float)o0, (float)o1, (float)o2, (float)o3);
+}
+
 template <typename T, int G>
 static int launch_reduce_t(mfh_handle h, const void* psi, void* phi, const LamArr& lam, cudaStream_t st)
 {
@@ -106,6 +161,15 @@ int launch_reduce(mfh_handle h, const void* psi, void* phi, const double* lambda
     LamArr lam;
     for (int v = 0; v < MFH_MAX_K; ++v) lam.v[v] = (v < p.k) ? (lambdas ? lambdas[v] : h->lambda) : 0.0;
     const bool split = ((int64_t)p.B * p.k) % RED_E == 0 && p.n_slots >= 16;
+    if (h->dtype == MFH_C64 && split && p.k % 2 == 0 && p.n_slots >= 64 && ((uintptr_t)psi % 16 == 0) && ((uintptr_t)phi % 16 == 0)) {
+        const int64_t pairs = h->D * p.k / 2;
+        const int epb = 256 / RED_G;
+        reduce2_kernel_c64<<<(unsigned)((pairs + epb - 1) / epb), 256, 0, st>>>(h->D, p.B, p.k, std::max(p.n_slots, 1), h->d_slot_list,
+                                                                                (const float2*)h->d_work, (const float*)h->d_h0,
+                                                                                (const float2*)psi, (float2*)phi, lam);
+        MFH_CUDA_CHECK(cudaGetLastError());
+        return MFH_OK;
+    }
     if (h->dtype == MFH_C128)
         return split ? launch_reduce_t<double, RED_G>(h, psi, phi, lam, st) : launch_reduce_t<double, 1>(h, psi, phi, lam, st);
     return split ? launch_reduce_t<float, RED_G>(h, psi, phi, lam, st) : launch_reduce_t<float, 1>(h, psi, phi, lam, st);
