@@ -535,11 +535,11 @@ SASS_COUNTS = {("c128", "k1"): {"instr_per_entry": 43.875, "fp64_per_entry": 16.
                ("c128", "kN"): {"instr_per_entry": 150.0, "fp64_per_entry": 0, "source": "DESIGN.md 6.3"},
                ("c64", "k1"): {"instr_per_entry": 40.0, "fp64_per_entry": 0, "source": "DESIGN.md 6.2"},
                ("c64", "kN"): {"instr_per_entry": 64.0, "fp64_per_entry": 0, "source": "profiles/r02_proc_multi_tc_c3_ncu_full.md (2.14e9 warp instructions / 1.07e9 entries x 32 lanes)"},
-               # two-sided generator: everything the step executes, per APPLIED entry (generator 67.75 per generated entry
+               # two-sided generator: everything the step executes, per APPLIED entry (generator 63.5 per generated entry
                # in its SASS; epilogue, sum, MMA warps and barrier waits on top; the one-sided kernel for the diagonal blocks)
-               ("c64", "kN2"): {"instr_per_entry": 41.3, "fp64_per_entry": 0,
+               ("c64", "kN2"): {"instr_per_entry": 38.3, "fp64_per_entry": 0,
                                 "source": "profiles/r02_pairs_tc_generated_c3_ncu_full.md + r02_proc_multi_tc_diag_c3_ncu_full.md "
-                                          "((1.316e9 + 0.069e9) warp instructions / 1.07e9 applied entries x 32 lanes)"}}
+                                          "((1.217e9 + 0.069e9) warp instructions / 1.07e9 applied entries x 32 lanes)"}}
 MIX_OF = {("c128", "k1"): ("c128_pair", 2), ("c64", "kN"): ("c64_entry", 1), ("c64", "kN2"): ("c64_entry", 1)}
 COMPONENTS_OF = {("c128", "k1"): {"kernels": ("comp_philox", "comp_philox_bm_c128", "comp_mac_c128"), "entries_per_pair": 2},
                  ("c64", "k1"): {"kernels": ("comp_philox", "comp_philox_bm_c64", "comp_mac_c64"), "entries_per_pair": 2}}
@@ -554,8 +554,8 @@ NCU_TRAFFIC = {("cached_kernel", 65536): (68.725132e9 + 5.106432e6, "profiles/r0
                ("cached_multi_kernel_c128", 32768): (17.203616e9 + 268.850432e6, "profiles/r02_cached_multi_c128_c3_ncu_full.md"),
                ("proc_single_kernel", 262144): (22.890752e6 + 631.663104e6, "profiles/r02_proc_single_c4_ncu_full.md"),
                ("proc_multi_tc_kernel", 32768): (4.513792e6 + 81.728768e6, "profiles/r02_proc_multi_tc_c3_ncu_full.md"),
-               ("pairs_tc_kernel<false>", 32768): (7.638784e6 + 526.364672e6, "profiles/r02_pairs_tc_generated_c3_ncu_full.md"),
-               ("pairs_tc_kernel<true>", 32768): (4.221867e9 + 584.702208e6, "profiles/r02_pairs_tc_cached_c3_ncu_full.md")}
+               ("pairs_tc_kernel<false>", 32768): (6.530304e6 + 527.058688e6, "profiles/r02_pairs_tc_generated_c3_ncu_full.md"),
+               ("pairs_tc_kernel<true>", 32768): (4.219875e9 + 583.816448e6, "profiles/r02_pairs_tc_cached_c3_ncu_full.md")}
 
 
 def ncu_traffic(kernel: str, D: int) -> dict:
