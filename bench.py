@@ -402,7 +402,7 @@ def measure_pipe_model(mfh) -> dict:
     synthetic kernels and the clocks one warp instruction of the class costs a scheduler at 1.965 GHz nominal.  A pair
     of classes that takes the sum of its parts does not overlap."""
     n = {"pipe_wide16": 32, "pipe_lop32": 32, "pipe_dfma32": 33, "pipe_dfma32_reg3": 33, "pipe_wide16_dfma32": 65,
-         "pipe_lop32_dfma32": 65, "pipe_wide16_lop32": 64}
+         "pipe_lop32_dfma32": 65, "pipe_wide16_lop32": 64, "pipe_cmac_regs": 1, "pipe_cmac_lds": 1}
     out = {}
     for name, instr in n.items():
         r = mfh.pipe_rate(name)
@@ -414,6 +414,7 @@ def measure_pipe_model(mfh) -> dict:
         "wide_plus_dfma_over_sum": c["pipe_wide16_dfma32"] / (c["pipe_wide16"] + c["pipe_dfma32"]),
         "lop_plus_dfma_over_max": c["pipe_lop32_dfma32"] / max(c["pipe_lop32"], c["pipe_dfma32"]),
         "wide_plus_lop_over_sum": c["pipe_wide16_lop32"] / (c["pipe_wide16"] + c["pipe_lop32"]),
+        "dfma_clk_mac_stream_one_operand_reused": c["pipe_cmac_regs"], "dfma_clk_k_vector_inner_loop": c["pipe_cmac_lds"],
         "fp64_peak_fraction_with_three_register_dfma": (c["pipe_dfma32"] / 33) / (c["pipe_dfma32_reg3"] / 33) * (2.0 / (c["pipe_dfma32"] / 33)),
         "note": "ratios near 1.0 over the SUM mean the two classes serialise (32x32->64 multiply against DFMA and "
                 "against logic ops); near 1.0 over the MAX mean they overlap (logic ops under DFMA)"}
@@ -444,9 +445,16 @@ def roofline_for(res: dict, hbm_gbs: float, peak_src: str) -> dict:
         # second number: the rate at which DFMAs with three register operands issue on this GPU (measured now); the
         # kernel's multiply-accumulates read the entry, the psi value and the accumulator from registers
         reg3 = res["pipe_rate"]("pipe_dfma32_reg3") * 33 * 2 / 1e12
+        # third and fourth number: the complex multiply-accumulate stream alone (psi in registers: all but the first DFMA
+        # of a run take the entry from the operand reuse cache, 2 clocks each) and this kernel's inner loop as written
+        # (entry and psi values from shared memory every column), both measured now by the library's microbenchmarks
+        cmac_regs = res["pipe_rate"]("pipe_cmac_regs") * 2 / 1e12
+        cmac_lds = res["pipe_rate"]("pipe_cmac_lds") * 2 / 1e12
         return {"kernel": "cached_multi_kernel_c128", "bound": "alu", "achieved": tf, "peak": peak, "unit": "TFLOP/s",
                 "frac": tf / peak, **ncu_traffic("cached_multi_kernel_c128", D),
                 "three_register_dfma_ceiling": reg3, "frac_of_three_register_dfma_ceiling": tf / reg3,
+                "mac_stream_in_registers_ceiling": cmac_regs, "inner_loop_from_shared_memory_ceiling": cmac_lds,
+                "frac_of_inner_loop_ceiling": tf / cmac_lds,
                 "peak_source": "nominal FP64: 148 SMs x 64 DFMA lanes/clk x 2 flop x 1.965 GHz (B200_PROFILING.md unit counts; "
                                "the SM clock under FP64 load is power-capped below that)",
                 "kernel_ms": kern["cached"], "share_of_step": kern["cached"] / max(kern["total"], 1e-9)}

@@ -411,11 +411,17 @@ MFH_API int mfh_debug_h0(mfh_handle h, void* h0_dev, void* stream);
  *   immediate operands), MFH_PIPE_DFMA32_REG3 (32 DFMA with three register operands), and the pairs
  *   MFH_PIPE_WIDE16_DFMA32, MFH_PIPE_LOP32_DFMA32, MFH_PIPE_WIDE16_LOP32: a pair that takes as long as the sum of
  *   its parts does not overlap.
+ * FP64 multiply-accumulate streams of the cached complex128 k-vector kernel (units = DFMA thread instructions per
+ * second): MFH_PIPE_CMAC_REGS -- the complex multiply-accumulate alone, psi values in registers, 16 DFMA in a row per
+ * entry component (the ceiling of the pattern: every DFMA but the first of a run takes the entry from the operand
+ * reuse cache); MFH_PIPE_CMAC_LDS -- that kernel's inner loop as written, entry and psi values from shared memory every
+ * column (the ceiling of the loop).
  * Synchronises `stream`.  Errors: INVALID_ARG, CUDA. */
 enum { MFH_MIX_C128_PAIR = 0, MFH_MIX_C64_ENTRY = 1, MFH_MIX_PHILOX = 2, MFH_MIX_DFMA31 = 3, MFH_COMP_PHILOX = 4,
        MFH_COMP_PHILOX_BM_C128 = 5, MFH_COMP_MAC_C128 = 6, MFH_COMP_PHILOX_BM_C64 = 7, MFH_COMP_MAC_C64 = 8,
        MFH_PIPE_WIDE16 = 9, MFH_PIPE_LOP32 = 10, MFH_PIPE_DFMA32 = 11, MFH_PIPE_DFMA32_REG3 = 12,
-       MFH_PIPE_WIDE16_DFMA32 = 13, MFH_PIPE_LOP32_DFMA32 = 14, MFH_PIPE_WIDE16_LOP32 = 15 };
+       MFH_PIPE_WIDE16_DFMA32 = 13, MFH_PIPE_LOP32_DFMA32 = 14, MFH_PIPE_WIDE16_LOP32 = 15,
+       MFH_PIPE_CMAC_REGS = 16, MFH_PIPE_CMAC_LDS = 17 };
 MFH_API int mfh_debug_pipe_rates(int32_t mix, double* units_per_s, void* stream);
 
 /* Read-only HBM stream probe: times a kernel that reads `bytes` of buf_dev once (8 independent 128-bit

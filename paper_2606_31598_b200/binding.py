@@ -409,7 +409,7 @@ def bessel_j_table(x: float, l_max: int):
 MIXES = {"c128_pair": 0, "c64_entry": 1, "philox": 2, "dfma31": 3, "comp_philox": 4, "comp_philox_bm_c128": 5,
          "comp_mac_c128": 6, "comp_philox_bm_c64": 7, "comp_mac_c64": 8, "pipe_wide16": 9, "pipe_lop32": 10,
          "pipe_dfma32": 11, "pipe_dfma32_reg3": 12, "pipe_wide16_dfma32": 13, "pipe_lop32_dfma32": 14,
-         "pipe_wide16_lop32": 15}
+         "pipe_wide16_lop32": 15, "pipe_cmac_regs": 16, "pipe_cmac_lds": 17}
 
 
 def pipe_rate(mix: str) -> float:
