@@ -249,6 +249,26 @@ def test_scan_c64_two_sided_tensor_core_kernels_and_their_fallbacks():
         h.destroy()
 
 
+@pytest.mark.parametrize("D,B,k", [(4096, 2048, 16), (8192, 4096, 7), (768, 384, 16), (3072, 1536, 2)])
+@pytest.mark.parametrize("mode", ["procedural", "pairs"])
+def test_scan_c64_two_sided_kernels_block_sizes(D, B, k, mode):
+    """The two-sided tensor-core kernels build the next item's psi operand a few rows per unit (B / 32 units per item):
+    one row pair per unit from B = 2048 (the block size the measured planner picks for C3's operator), two up to
+    B = 1024, more below; B = 384 and 1536 are multiples of 128 that are not powers of two."""
+    Psi = make_psi(D, 23, k=k, dtype="c64")
+    lam = 0.5 + lambda_grid(k)
+    h = mfh.Hamiltonian(D, B, 8, "c64", kind="diag_plus_gue", seed_h0=7)
+    h.plan(mode, k=k)
+    gp = h.get_plan()
+    assert gp["two_sided_pairs" if mode == "procedural" else "two_sided_stored_pairs"] == (D // B) * (D // B - 1) // 2
+    h.debug_poison()
+    Phi = h.apply(to_dev(Psi), lambdas=lam).cpu().numpy()
+    ref = oracle.apply_scan(D, B, 8, 7, lam, Psi)
+    for v in range(k):
+        assert rel_l2(Phi[:, v], ref[:, v]) <= TOL["c64"], v
+    h.destroy()
+
+
 @pytest.mark.parametrize("mode,budget", [("full", 0), ("partial", 12e6), ("partial", 24e6)])
 @pytest.mark.parametrize("dtype,k", [("c64", 16), ("c64", 5), ("c128", 16), ("c128", 8), ("c128", 3), ("c128", 2)])
 def test_scan_cached_blocks_k_vectors(mode, budget, dtype, k):
