@@ -350,8 +350,10 @@ __global__ void __launch_bounds__(TC_THREADS, 2) proc_multi_tc_kernel(const TcPa
 // --------------------------------------------------------------------------------------------
 // Two-sided k-vector generator (complex64): "generates ... each V block once" AND uses the Hermitian structure
 // (Eq. 11): for a block pair n < m whose two positions are both generated, every entry
-// V_ij (i in block n, j in block m) is generated ONCE and used for  Phi_i += V_ij Psi_j  (row side, exactly the
-// one-sided kernel's TMEM A operand) and for  Phi_j += conj(V_ij) Psi_i  (column side).
+// V_ij (i in block n, j in block m) is generated ONCE and used for  Phi_i += V_ij Psi_j  (row side: the tile is the
+// TMEM A operand as in the one-sided kernel, here in the cached kernel's interleaved (re, im) layout, see
+// t2_psi_image) and for  Phi_j += conj(V_ij) Psi_i  (column side).  pairs_tc_kernel<true> is the same kernel for
+// STORED pairs of a pair cache: the generator warps become converters of unit images landed by bulk copies.
 //
 // The column side contracts over the tile's ROWS, which are the lanes of the row side's A operand, so it cannot
 // reuse that operand.  It swaps the operand roles instead: the generated tile is the B operand in shared memory,
@@ -371,7 +373,8 @@ __global__ void __launch_bounds__(TC_THREADS, 2) proc_multi_tc_kernel(const TcPa
 //
 // One persistent CTA per SM (all 512 TMEM columns): 16 generator warps in two groups that take the tiles
 // alternately (thread = half a row of a tile, as in the one-sided kernel), 4 epilogue warps (they also build the
-// psi operand of every item), one warp issuing the row-side MMAs, one the column-side MMAs.
+// psi operand of the NEXT item into the other of two TMEM buffers), 2 sum warps, one warp issuing the row-side MMAs,
+// one the column-side MMAs (+ a bulk-copy producer warp in the cached variant).
 // --------------------------------------------------------------------------------------------
 constexpr int T2_GEN_WARPS = 16;
 constexpr int T2_W_EPI = T2_GEN_WARPS;            // warps 16..19: TMEM lane quadrants 0..3
