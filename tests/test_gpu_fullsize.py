@@ -162,6 +162,30 @@ def test_c3_scan_every_row_generated_and_cached():
         assert rel_l2(out["procedural"][:, v], out["full"][:, v]) <= 5e-5, v
 
 
+@pytest.mark.parametrize("mode", ["procedural", "pairs"])
+def test_c3_two_sided_kernels_repeat_bit_identically(mode):
+    """Race check of the two-sided tensor-core kernels at full size (compute-sanitizer is closed on this pool, DESIGN.md
+    section 10): 100 applies from a periodically poisoned workspace must be bit-identical (the kernels hand tiles, unit
+    images, TMEM stages and accumulators between 24 warps through 15 mbarriers and 4 named barriers; the race of round 1
+    showed as sporadic wrong rows at full size only) and no guard byte around the library's buffers may change."""
+    import torch
+    c = CONFIGS["C3"]
+    D, B, k = c["D"], c["B"], c["k"]
+    Psi = to_dev(make_psi(D, c["psi_seed"], k=k, dtype="c64"))
+    lam = lambda_grid(k)
+    h = mfh.Hamiltonian(D, B, c["seed"], "c64", kind="diag_plus_gue", seed_h0=c["seed_h0"])
+    h.plan(mode, k=k)
+    first = h.apply(Psi, lambdas=lam).clone()
+    out = torch.empty_like(first)
+    for r in range(100):
+        if r % 10 == 0:
+            h.debug_poison()
+        h.apply(Psi, out, lambdas=lam)
+        assert torch.equal(out, first), r
+    assert h.debug_selfcheck() == 0
+    h.destroy()
+
+
 def test_c3_scan_from_the_pair_cache_every_row():
     """C3's operator from the Hermitian pair cache (4.4 GB instead of 8.6 GB): every stored off-diagonal block is read
     ONCE per apply and serves both positions (two-sided cached kernel, unit-image layout); the diagonal blocks go
