@@ -299,6 +299,7 @@ void build_tables(Plan& p, int64_t D, int dtype, int sm_count)
         for (int t = 0; t < tcS; ++t) valid(m, p.slot_mcol0 + n * tcS + t) = 1;
     };
     for (size_t q = 0; q + 1 < p.tc_pairs.size(); q += 2) two_sided(p.tc_pairs[q], p.tc_pairs[q + 1]);
+    for (size_t q = 0; q + 2 < p.tc_cpairs.size(); q += 3) two_sided(p.tc_cpairs[q], p.tc_cpairs[q + 1]);
     p.ct_left.clear();
     if (!p.tc_cpairs.empty())
         for (int n = 0; n < N; ++n)
@@ -317,7 +318,6 @@ void build_tables(Plan& p, int64_t D, int dtype, int sm_count)
                     p.tc_left.push_back(n);
                     p.tc_left.push_back(m);
                 }
-    for (size_t q = 0; q + 2 < p.tc_cpairs.size(); q += 3) two_sided(p.tc_cpairs[q], p.tc_cpairs[q + 1]);
     const int strip = p.B / p.Q;
     auto push_items = [&](std::vector<ProcItem>& dst, int n, int m, uint8_t kd) {
         valid(n, p.slot_row0 + m) = 1;
