@@ -92,3 +92,29 @@ def test_static_entry_point_at_its_maximum_size():
     rows = np.arange(0, D, 257, dtype=np.int64)
     ref = oracle.apply(D, 2048, seed, psi, rows=rows)
     assert rel_l2(got[rows], ref) <= TOL
+
+
+def test_static_entry_point_under_cuda_graph_capture():
+    """The reason the entry point exists: after one warm-up call for this D (address look-up, generator table in place)
+    it issues kernel launches only, so it can be recorded into a CUDA graph -- where cudaMalloc is not allowed -- and
+    replayed."""
+    import torch
+    D, seed, lam = 2048, 77, 1.25
+    x = to_dev(make_psi(D, 5))
+    y = torch.empty_like(x)
+    mfh.apply_static(D, seed, lam, x, y)                      # warm-up outside the capture
+    torch.cuda.synchronize()
+    ref = y.clone()
+    g = torch.cuda.CUDAGraph()
+    y.zero_()
+    with torch.cuda.graph(g):
+        mfh.apply_static(D, seed, lam, x, y)
+    y.zero_()
+    for _ in range(3):
+        g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(y, ref)
+    x.copy_(to_dev(make_psi(D, 6)))                           # new input in the captured buffer, replay again
+    g.replay()
+    torch.cuda.synchronize()
+    assert rel_l2(y.cpu().numpy(), existing_path(D, 256, seed, lam, x)) <= TOL
